@@ -1,0 +1,323 @@
+"""Pins for the oracle (CPU only). The oracle is checked against things other than itself:
+values the paper prints (tests/golden/paper_worked_example.txt), a dense brute-force
+restatement of Eq. 3-5 + closure on tiny inputs, closed forms, invariants, library routines
+(numpy stable argsort) and generated truth. A plausible mistake (dropped term, wrong sign or
+index, strict vs inclusive threshold, transposed operand) fails at least one of these."""
+import os
+
+import numpy as np
+import pytest
+
+import gen
+import oracle
+from oracle import bruteforce as bf
+
+W, P = 320, 640000
+
+
+def load_golden(path):
+    vec, rows = {}, {}
+    for line in open(path):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        head, vals = line.split(":")
+        head = head.split()
+        vals = [int(v) for v in vals.split()]
+        if len(head) == 1:
+            vec[head[0]] = vals
+        else:
+            rows.setdefault(head[0], {})[int(head[1])] = vals
+    return vec, rows
+
+
+# ------------------------------------------------------------------ paper's worked example
+def test_paper_worked_example(golden_dir):
+    vec, rows = load_golden(os.path.join(golden_dir, "paper_worked_example.txt"))
+    X, TOT, w = vec["X"], vec["TOT"], vec["W"][0]
+    D = bf.distance_matrix(X)
+    for r, vals in rows["DX"].items():  # Eq. 3
+        assert D[r - 1].tolist() == vals
+    A = bf.adjacency_1d(X, w)
+    for r, vals in rows["AX"].items():  # Eq. 4
+        assert A[r - 1].tolist() == vals
+    M = bf.masked_tot(TOT, A)
+    for r, vals in rows["M"].items():  # Eq. 6
+        assert M[r - 1].tolist() == vals
+    anti = M - M.T
+    for r, vals in rows["ANTI"].items():  # Eq. 7
+        assert anti[r - 1].tolist() == vals
+    for lift in ("paper", "lex", "none"):
+        lm = bf.local_maxima(TOT, A, lift=lift)
+        assert (lm + 1).tolist() == vec["LOCAL_MAXIMA"]
+        assert len(lm) == vec["HIT_COUNT"][0]
+
+
+def test_worked_example_components_and_centroids():
+    # Derived from Eq. 9 on the paper's example (not printed): components at w=5 are {1,2,5},{3,4};
+    # here component == box of the local maximum, so both definitions agree.
+    X = np.array([20, 21, 90, 92, 18]); TOT = np.array([50, 200, 300, 25, 100])
+    z = np.zeros(5, dtype=np.int64)
+    A = bf.adjacency(X, z, z, 5, 0, 0)
+    assert bf.components(A).tolist() == [0, 0, 2, 2, 0]
+    cent = bf.box_centroid(X, TOT, A)
+    lm = bf.local_maxima(TOT, A)
+    assert cent[lm[0]] == 7000 / 350 == 20.0
+    assert cent[lm[1]] == pytest.approx(29300 / 325)
+    # At the north_star's w = 1 the same data gives {1,2},{3},{4},{5}; run the C++ oracle.
+    o = oracle.run(X, z, z, TOT, W, 0)
+    assert o["perm"].tolist() == [0, 1, 2, 3, 4]  # all ToA equal: stable order = input order
+    assert o["label"].tolist() == [0, 0, 2, 3, 4]
+    assert o["n_clusters"] == 4
+    assert o["c_sum_tot"].tolist() == [250, 300, 25, 100]
+    assert o["c_sum_tot_x"].tolist() == [50 * 20 + 200 * 21, 300 * 90, 25 * 92, 100 * 18]
+    assert o["c_cx"][0] == np.float32(5200) / np.float32(250)
+    assert o["c_cx"][1:].tolist() == [90.0, 92.0, 18.0]
+
+
+def test_tie_break_later_pixel_wins():
+    # equal ToT -> the pixel later in the stream wins.
+    x = np.array([10, 11, 12]); y = np.array([5, 5, 5]); toa = np.array([100, 100, 100]); tot = np.array([7, 9, 9])
+    A = bf.adjacency(x, y, toa, 1, 1, W)
+    assert bf.local_maxima(tot, A, "paper").tolist() == [2]
+    assert bf.local_maxima(tot, A, "lex").tolist() == [2]
+    assert sorted(bf.local_maxima(tot, A, "none").tolist()) == [1, 2]  # over-counting without the lift
+    toa2 = np.array([100, 105, 103])  # sorted order: idx 0 (100), idx 2 (103), idx 1 (105)
+    o = oracle.run(x, y, toa2, tot, W, P)
+    assert o["perm"].tolist() == [0, 2, 1]
+    assert o["n_clusters"] == 1 and o["c_toa_peak"].tolist() == [105]  # tot 9 at sorted pos 1 and 2 -> pos 2
+
+
+# ------------------------------------------------------------------ brute force on tiny inputs
+def assert_same(o, b):
+    assert o["n_clusters"] == b["n_clusters"]
+    for k in ("perm", "label", "c_label", "c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_toa_peak"):
+        assert np.array_equal(o[k], b[k]), k
+    assert np.array_equal(o["c_cx"].view(np.uint32), b["c_cx"].view(np.uint32))
+    assert np.array_equal(o["c_cy"].view(np.uint32), b["c_cy"].view(np.uint32))
+
+
+def tiny_random(rng, n, span_xy=6, span_t=900, shots=2):
+    x = rng.integers(0, span_xy, n) + rng.integers(0, 2) * (256 - span_xy)
+    y = rng.integers(0, span_xy, n) + rng.integers(0, 2) * (256 - span_xy)
+    toa = rng.integers(0, shots, n) * P + rng.integers(0, span_t, n)
+    tot = rng.integers(1, 6, n)
+    return x, y, toa.astype(np.uint64), tot
+
+
+@pytest.mark.parametrize("seed", range(40))
+def test_bruteforce_random(seed):
+    rng = np.random.default_rng(seed)
+    n = int(rng.integers(2, 65))
+    x, y, toa, tot = tiny_random(rng, n, span_xy=int(rng.integers(2, 9)), span_t=int(rng.integers(1, 1500)),
+                                 shots=int(rng.integers(1, 4)))
+    assert_same(oracle.run(x, y, toa, tot, W, P), bf.cluster_bruteforce(x, y, toa, tot, W, P))
+
+
+def test_bruteforce_adversarial():
+    cases = []
+    # chain A-B-C with |tA - tC| > W: still one component (transitive closure)
+    cases.append(([10, 11, 12], [10, 10, 10], [1000, 1000 + W, 1000 + 2 * W], [5, 6, 7]))
+    # dt == W links, dt == W + 1 does not (inclusive threshold)
+    cases.append(([10, 11, 20, 21], [10, 10, 10, 10], [0, W, 0, W + 1], [5, 6, 7, 8]))
+    # repeated address inside the window is adjacent (dx = dy = 0 satisfies Eq. 5), outside is not
+    cases.append(([7, 7, 7], [9, 9, 9], [0, 100, 100 + W + 1], [3, 3, 3]))
+    # sensor corners, no wrap-around
+    cases.append(([0, 255, 0, 255, 1, 254], [0, 255, 255, 0, 1, 254], [5, 5, 5, 5, 5, 5], [1, 2, 3, 4, 5, 6]))
+    # hits straddling a shot boundary: tick sP-1 and sP are different shots (never linked)
+    cases.append(([50, 50, 51], [60, 60, 60], [P - 1, P, P + 1], [9, 9, 9]))
+    # all hits identical
+    cases.append(([3] * 8, [4] * 8, [777] * 8, [2] * 8))
+    # dx = 2 is not adjacent; diagonal is
+    cases.append(([10, 12, 13, 14], [10, 10, 11, 12], [0, 0, 0, 0], [1, 1, 1, 1]))
+    # unsorted input with equal ToA in different input order (stable sort)
+    cases.append(([1, 2, 3, 4, 5], [1, 1, 1, 1, 1], [50, 40, 50, 40, 45], [1, 2, 3, 4, 5]))
+    for x, y, toa, tot in cases:
+        x, y, tot = np.array(x), np.array(y), np.array(tot)
+        toa = np.array(toa, dtype=np.uint64)
+        o = oracle.run(x, y, toa, tot, W, P)
+        assert_same(o, bf.cluster_bruteforce(x, y, toa, tot, W, P))
+    o = oracle.run(*[np.array(c) for c in cases[0][:2]], np.array(cases[0][2], dtype=np.uint64), np.array(cases[0][3]), W, P)
+    assert o["n_clusters"] == 1
+    o = oracle.run(np.array(cases[1][0]), np.array(cases[1][1]), np.array(cases[1][2], dtype=np.uint64), np.array(cases[1][3]), W, P)
+    assert o["n_clusters"] == 3
+    o = oracle.run(np.array(cases[4][0]), np.array(cases[4][1]), np.array(cases[4][2], dtype=np.uint64), np.array(cases[4][3]), W, P)
+    assert o["label"].tolist() == [0, 1, 1] and o["c_shot"].tolist() == [0, 1]
+
+
+def test_empty_and_single():
+    e16, e64 = np.zeros(0, np.uint16), np.zeros(0, np.uint64)
+    o = oracle.run(e16, e16, e64, e16, W, P)
+    assert o["n_clusters"] == 0 and o["perm"].shape == (0,) and o["c_cx"].shape == (0,)
+    o = oracle.run([17], [200], [3 * P + 12345], [321], W, P)
+    assert o["n_clusters"] == 1 and o["label"].tolist() == [0]
+    assert o["c_size"].tolist() == [1] and o["c_cx"].tolist() == [17.0] and o["c_cy"].tolist() == [200.0]
+    assert o["c_toa_peak"].tolist() == [3 * P + 12345] and o["c_shot"].tolist() == [3]
+
+
+def test_shot_period_zero_is_one_shot():
+    x = np.array([5, 6]); y = np.array([5, 5]); toa = np.array([P - 1, P], dtype=np.uint64); tot = np.array([1, 1])
+    assert oracle.run(x, y, toa, tot, W, P)["n_clusters"] == 2
+    assert oracle.run(x, y, toa, tot, W, 0)["n_clusters"] == 1
+    assert_same(oracle.run(x, y, toa, tot, W, 0), bf.cluster_bruteforce(x, y, toa, tot, W, 0))
+
+
+# ------------------------------------------------------------------ closed forms
+def test_two_pixel_closed_form():
+    for (x1, y1, t1), (x2, y2, t2) in [((100, 50, 3), (101, 51, 9)), ((255, 0, 1023), (254, 0, 1)), ((0, 7, 13), (0, 8, 29))]:
+        o = oracle.run([x1, x2], [y1, y2], [10, 20], [t1, t2], W, P)
+        assert o["n_clusters"] == 1 and o["c_size"].tolist() == [2]
+        assert o["c_sum_tot"].tolist() == [t1 + t2]
+        assert o["c_cx"][0] == np.float32(t1 * x1 + t2 * x2) / np.float32(t1 + t2)
+        assert o["c_cy"][0] == np.float32(t1 * y1 + t2 * y2) / np.float32(t1 + t2)
+        assert abs(float(o["c_cx"][0]) - (t1 * x1 + t2 * x2) / (t1 + t2)) < 2e-5  # exact value within fp32 rounding
+        assert o["c_toa_peak"].tolist() == [10 if t1 > t2 else 20]
+
+
+# ------------------------------------------------------------------ invariants on the configs
+WORKLOADS = [(0, 1000), (1, 300), (2, 150), (3, 40), (4, 150)]
+
+
+@pytest.fixture(scope="module", params=WORKLOADS, ids=lambda p: "cfg%d" % p[0])
+def wl(request):
+    cfg, shots = request.param
+    w = gen.generate(cfg, shots=shots)
+    return w, oracle.run(w.x, w.y, w.toa, w.tot, W, P)
+
+
+def test_invariants(wl):
+    w, o = wl
+    n = w.n
+    perm, label = o["perm"].astype(np.int64), o["label"].astype(np.int64)
+    k = np.arange(n)
+    # perm: the unique stable sort (library pin: numpy's stable argsort; (shot, toa) order == toa order)
+    assert np.array_equal(perm, np.argsort(w.toa, kind="stable"))
+    assert np.all(label <= k)
+    assert np.array_equal(label[label], label)
+    assert o["n_clusters"] == int(np.sum(label == k))
+    assert np.array_equal(o["c_label"], k[label == k])
+    assert int(o["c_size"].sum()) == n
+    assert int(o["c_sum_tot"].sum()) == int(w.tot.astype(np.int64).sum())
+    assert int(o["c_sum_tot_x"].sum()) == int((w.tot.astype(np.int64) * w.x).sum())
+    assert int(o["c_sum_tot_y"].sum()) == int((w.tot.astype(np.int64) * w.y).sum())
+    # independent numpy recomputation of the per-cluster sums from the labels
+    xs, ys, ts, toas = w.x[perm].astype(np.int64), w.y[perm].astype(np.int64), w.tot[perm].astype(np.int64), w.toa[perm]
+    slot = np.cumsum(label == k) - 1
+    c = slot[label]
+    nc = o["n_clusters"]
+    assert np.array_equal(np.bincount(c, minlength=nc), o["c_size"])
+    assert np.array_equal(np.bincount(c, weights=ts, minlength=nc).astype(np.int64), o["c_sum_tot"])
+    assert np.array_equal(np.bincount(c, weights=ts * xs, minlength=nc).astype(np.int64), o["c_sum_tot_x"])
+    assert np.array_equal(np.bincount(c, weights=ts * ys, minlength=nc).astype(np.int64), o["c_sum_tot_y"])
+    # centroid inside the bounding box of the members; all members in the root's shot
+    xmin = np.full(nc, 1 << 30); xmax = np.full(nc, -1)
+    np.minimum.at(xmin, c, xs); np.maximum.at(xmax, c, xs)
+    assert np.all(o["c_cx"] >= xmin) and np.all(o["c_cx"] <= xmax)
+    shot = (toas // np.uint64(P)).astype(np.int64)
+    assert np.array_equal(shot[label], shot)
+    assert np.array_equal(o["c_shot"], shot[label == k])
+    # peak: member with max (tot, k)
+    key = ts * (n + 1) + k
+    best = np.zeros(nc, dtype=np.int64)
+    np.maximum.at(best, c, key)
+    assert np.array_equal(o["c_toa_peak"], toas[best % (n + 1)])
+    # singles: centroid is the pixel itself
+    single = o["c_size"] == 1
+    roots = k[label == k]
+    assert np.array_equal(o["c_cx"][single], xs[roots[single]].astype(np.float32))
+    assert np.array_equal(o["c_toa_peak"][single], toas[roots[single]])
+
+
+def test_every_link_is_valid_and_closed(wl):
+    """Labels are a valid closure: every adjacent pair (brute force inside each shot) has equal
+    labels, and every non-root hit has an adjacent hit with the same label (so no component is
+    the union of two unrelated pieces, checked per component by BFS-free counting)."""
+    w, o = wl
+    perm, label = o["perm"].astype(np.int64), o["label"].astype(np.int64)
+    xs, ys, toas = w.x[perm].astype(np.int64), w.y[perm].astype(np.int64), w.toa[perm].astype(np.int64)
+    shot = toas // P
+    bounds = np.flatnonzero(np.diff(shot)) + 1
+    starts = np.concatenate([[0], bounds]); ends = np.concatenate([bounds, [len(shot)]])
+    checked = 0
+    for a, b in list(zip(starts, ends))[:25]:
+        X, Y, T, L = xs[a:b], ys[a:b], toas[a:b], label[a:b]
+        A = (np.abs(X[:, None] - X[None, :]) <= 1) & (np.abs(Y[:, None] - Y[None, :]) <= 1) & (np.abs(T[:, None] - T[None, :]) <= W)
+        np.fill_diagonal(A, False)
+        i, j = np.nonzero(A)
+        assert np.array_equal(L[i], L[j])
+        assert np.array_equal(bf.components(A.astype(np.int64)) + a, L)
+        checked += 1
+    assert checked > 0
+
+
+def test_transform_invariants():
+    w = gen.generate(2, shots=60)
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P)
+    # translation in x by a adds a * sum_tot to sum_tot_x
+    a = 3
+    o2 = oracle.run(w.x + a, w.y, w.toa, w.tot, W, P)
+    assert np.array_equal(o2["label"], o["label"])
+    assert np.array_equal(o2["c_sum_tot_x"], o["c_sum_tot_x"] + a * o["c_sum_tot"])
+    # adding m*P to every ToA changes only shot and toa_peak
+    m = 7
+    o3 = oracle.run(w.x, w.y, w.toa + np.uint64(m * P), w.tot, W, P)
+    for k in ("perm", "label", "c_size", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_cx", "c_cy"):
+        assert np.array_equal(o3[k], o[k]), k
+    assert np.array_equal(o3["c_shot"], o["c_shot"] + m)
+    assert np.array_equal(o3["c_toa_peak"], o["c_toa_peak"] + np.uint64(m * P))
+    # swapping x and y swaps the sums (catches a transposed operand)
+    o4 = oracle.run(w.y, w.x, w.toa, w.tot, W, P)
+    assert np.array_equal(o4["c_sum_tot_x"], o["c_sum_tot_y"]) and np.array_equal(o4["c_cy"], o["c_cx"])
+    # growing W never increases the cluster count; W = 0 still links equal-ToA neighbours
+    counts = [oracle.run(w.x, w.y, w.toa, w.tot, ww, P)["n_clusters"] for ww in (0, 5, 30, 320, 5000)]
+    assert all(c1 >= c2 for c1, c2 in zip(counts, counts[1:]))
+    assert counts[0] > counts[3]
+
+
+def test_permutation_invariance_distinct_toa():
+    # With distinct ToA the cluster SET does not depend on the input order.
+    rng = np.random.default_rng(5)
+    w = gen.generate(0, shots=30)
+    toa = w.toa * np.uint64(4000) + np.arange(w.n, dtype=np.uint64) % np.uint64(4000)  # make ToA distinct, keep order
+    Pd, Wd = P * 4000, W * 4000
+    assert len(np.unique(toa)) == w.n
+    o = oracle.run(w.x, w.y, toa, w.tot, Wd, Pd)
+    p = rng.permutation(w.n)
+    o2 = oracle.run(w.x[p], w.y[p], toa[p], w.tot[p], Wd, Pd)
+    assert np.array_equal(p[o2["perm"]], o["perm"])
+    for k in ("label", "c_size", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_toa_peak", "c_cx", "c_cy"):
+        assert np.array_equal(o2[k], o[k]), k
+
+
+def test_local_maxima_vs_components():
+    # #local maxima at w = 1 >= n_clusters with at least one per component (links the paper's
+    # definition of a hit, Eq. 6-7, with the north_star's connected component).
+    w = gen.generate(2, shots=3)
+    for s in range(3):
+        ws = w.slice_shots(s, s + 1)
+        o = oracle.run(ws.x, ws.y, ws.toa, ws.tot, W, P)
+        perm = o["perm"].astype(np.int64)
+        A = bf.adjacency(ws.x[perm], ws.y[perm], ws.toa[perm].astype(np.int64), 1, 1, W)
+        lm = bf.local_maxima(ws.tot[perm], A, "lex")
+        assert len(lm) >= o["n_clusters"]
+        assert set(o["label"][lm].tolist()) == set(o["c_label"].tolist())
+
+
+# ------------------------------------------------------------------ generated truth
+def test_well_separated_truth():
+    w = gen.generate(5, shots=400, truth=True)
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P)
+    assert o["n_clusters"] == len(w.truth["cx"]) == 4000  # exact particle count
+    assert np.array_equal(np.sort(o["c_size"]), np.sort(w.truth["k"]))
+    # match clusters to particles per shot by nearest centre
+    err = []
+    cs = o["c_shot"].astype(np.int64)
+    for s in range(0, 400, 7):
+        m = cs == s
+        t = w.truth["shot"] == s
+        cx, cy = o["c_cx"][m].astype(np.float64), o["c_cy"][m].astype(np.float64)
+        d = np.hypot(cx[:, None] - w.truth["cx"][t][None, :], cy[:, None] - w.truth["cy"][t][None, :])
+        assert sorted(d.argmin(axis=1).tolist()) == list(range(10))  # one-to-one
+        err.extend(d.min(axis=1).tolist())
+    err = np.array(err)
+    assert err.mean() < 0.3 and err.max() < 1.0  # truncated, noisy footprint: tolerance, not equality
