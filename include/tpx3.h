@@ -1,0 +1,144 @@
+/* tpx3.h — C ABI of the B200-native TimePix3 cluster + centroid hot path.
+ *
+ * What the library computes (arxiv/paper_2603_04942, cited as PAPER.md:<line>):
+ *   input   a stream of pixel events (X, Y, ToA, ToT) from a TimePix3 sensor
+ *   S0/S1   shot = ToA div P (most recent laser trigger); stable sort of the
+ *           events by (shot, ToA) (the stream is "essentially unsorted")
+ *   S2      neighbourhood relation A = A^X (.) A^Y (.) A^ToF, |D| <= w inclusive    PAPER.md:117-126, Eq. 4-5
+ *           with w_x = w_y = 1 (8-connectivity), w_t = W ticks, same shot only; a particle hit
+ *           is a connected component of that relation (BASELINE.json north_star)
+ *   S3      label[k] = smallest sorted index in k's component; hit count
+ *   S4      per hit: size, sum ToT, sum ToT*X, sum ToT*Y (exact integers); the brightest pixel
+ *           (max ToT, ties: the later pixel in the sorted stream wins)
+ *   S5      centroid = sum(ToT*X) / sum(ToT), same for Y                             PAPER.md:156-165, Eq. 8-9
+ *           computed as fp32(int64) / fp32(int64), IEEE round-to-nearest divide.
+ *
+ * Conventions
+ *   - Every pointer marked [dev] is device memory on the plan's CUDA device, owned by the
+ *     caller (the Python binding passes PyTorch tensors); [host] is host memory. The library
+ *     never frees or reallocates caller memory and never writes its inputs.
+ *   - `workspace` is a [dev] scratch buffer of at least the `workspace_bytes` reported by
+ *     tpx3_plan, 256-byte aligned. Its contents are undefined between calls.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *     Device-pointer calls only ENQUEUE work on that stream and return; there is no hidden
+ *     synchronisation. Outputs are valid once the stream has reached the end of the call.
+ *   - `perm[k]`  = original (input) index of the event at sorted position k.
+ *     `label[k]` = sorted position of the first event of k's hit; indexed by SORTED position.
+ *     Clusters are listed in ascending `label` order (exactly one valid output exists).
+ *   - Preconditions on the data: x < sensor_w, y < sensor_h, tot >= 1. They are only checked
+ *     under TPX3_FLAG_VALIDATE_INPUT (result in tpx3_status).
+ *   - Errors: every call returns 0 (TPX3_OK) or a negative tpx3_error_t. Errors that can only
+ *     be detected on the device (capacity, validation) are recorded in a device status word
+ *     read by tpx3_status. No exceptions, no exit(), no output on stdout, no CPU fallback.
+ */
+#ifndef TPX3_H_
+#define TPX3_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  TPX3_OK = 0,
+  TPX3_ERR_INVALID_ARG = -1,   /* null pointer, bad struct_size, n > max_hits, bad config      */
+  TPX3_ERR_CAPACITY = -2,      /* max_clusters too small (device-detected; see tpx3_status)     */
+  TPX3_ERR_OUT_OF_RANGE = -3,  /* x/y outside the sensor or tot == 0 (under VALIDATE_INPUT)     */
+  TPX3_ERR_CUDA = -4,          /* a CUDA runtime call failed                                    */
+  TPX3_ERR_UNIMPLEMENTED = -5
+} tpx3_error_t;
+
+enum {
+  TPX3_FLAG_VALIDATE_INPUT = 1u << 0, /* check the data preconditions on the device            */
+  TPX3_FLAG_FORCE_GENERAL = 1u << 1   /* never take the shot-contiguous fused path              */
+};
+
+typedef struct tpx3_plan_s* tpx3_plan_t;
+
+typedef struct {
+  uint32_t struct_size;        /* = sizeof(tpx3_config_t); ABI guard                           */
+  uint16_t sensor_w, sensor_h; /* pixels; 1..256 each (TimePix3: 256 x 256)       */
+  uint32_t toa_window_ticks;   /* W: |dToA| <= W links, inclusive; < 2^31       */
+  uint64_t shot_period_ticks;  /* P: shot = ToA div P; 0 = the whole input is one shot         */
+  uint64_t max_hits;           /* largest n of any later call; 1 .. 2^28                       */
+  int32_t device;              /* CUDA device ordinal                                          */
+  uint32_t flags;              /* TPX3_FLAG_*                                                  */
+} tpx3_config_t;
+
+/* Per-hit (cluster) outputs, structure of arrays, each of capacity max_clusters. [dev] */
+typedef struct {
+  uint32_t* label;      /* sorted position of the hit's first pixel (ascending)                */
+  uint32_t* size;       /* number of pixels                                                    */
+  uint32_t* shot;       /* ToA div P of the hit, low 32 bits                                   */
+  int64_t* sum_tot;     /* sum ToT                                                             */
+  int64_t* sum_tot_x;   /* sum ToT * X                                                         */
+  int64_t* sum_tot_y;   /* sum ToT * Y                                                         */
+  uint64_t* toa_peak;   /* ToA of the brightest pixel (max (ToT, sorted position))             */
+  float* cx;            /* fp32(sum_tot_x) / fp32(sum_tot), Eq. 9                              */
+  float* cy;
+} tpx3_clusters_t;
+
+/* Device status of the most recent call on a workspace (tpx3_status). */
+typedef struct {
+  uint32_t error;       /* 0 or -(tpx3_error_t) of the first device-detected error             */
+  uint32_t path;        /* 1 = fused shot-tile path, 2 = general path (global sort + hash link) */
+  uint32_t n_clusters;  /* hits found by the last cluster / centroid call                      */
+  uint32_t sort_passes; /* radix passes the general path ran (0 on the fused path)             */
+  uint64_t n;           /* events of the last call                                             */
+} tpx3_status_t;
+
+/* Validate `cfg`, create a plan (host metadata only) and report the device workspace size the
+ * other calls need for up to cfg->max_hits events. Host only; no device memory is allocated. */
+int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace_bytes);
+
+/* S0-S3. x, y, tot: uint16[n]; toa: uint64[n] (all [dev], SoA, 14 B/event).
+ * Outputs [dev]: perm uint32[n], label uint32[n], n_clusters uint32[1]. n may be 0. */
+int tpx3_cluster(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64_t n,
+                 const uint16_t* x, const uint16_t* y, const uint64_t* toa, const uint16_t* tot,
+                 uint32_t* perm, uint32_t* label, uint32_t* n_clusters);
+
+/* S4-S5 for ANY (perm, label) satisfying the post-conditions of tpx3_cluster (perm a
+ * permutation; label[k] <= k; label[label[k]] == label[k]). Writes min(n_clusters,
+ * max_clusters) entries of `out` and the true count to n_clusters [dev]; if the count exceeds
+ * max_clusters the status word records TPX3_ERR_CAPACITY. */
+int tpx3_centroid(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64_t n,
+                  const uint16_t* x, const uint16_t* y, const uint64_t* toa, const uint16_t* tot,
+                  const uint32_t* perm, const uint32_t* label, uint64_t max_clusters,
+                  const tpx3_clusters_t* out, uint32_t* n_clusters);
+
+/* S0-S5 in one call (same results as tpx3_cluster followed by tpx3_centroid). When the input
+ * is shot-contiguous (shot = ToA div P never decreases along the stream, as in a TimePix3
+ * readout where disorder is confined to one readout window) and every shot fits one
+ * shared-memory tile, the whole path runs as ONE fused kernel; otherwise the general kernels
+ * run. The decision is taken on the device; tpx3_status reports which path ran. */
+int tpx3_cluster_centroid(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64_t n,
+                          const uint16_t* x, const uint16_t* y, const uint64_t* toa,
+                          const uint16_t* tot, uint32_t* perm, uint32_t* label,
+                          uint64_t max_clusters, const tpx3_clusters_t* out, uint32_t* n_clusters);
+
+/* End-to-end variant with HOST buffers: copies x, y, toa, tot [host] to the device, runs
+ * tpx3_cluster_centroid and copies perm, label (either may be NULL to skip), the first
+ * min(n_clusters, max_clusters) entries of every non-NULL array of `out_host` and the count
+ * back, then synchronises the stream. `device_io` is a [dev] staging buffer of at least
+ * tpx3_host_io_bytes(n, max_clusters) bytes. Returns the device status error, if any. */
+size_t tpx3_host_io_bytes(uint64_t n, uint64_t max_clusters);
+int tpx3_process_host(tpx3_plan_t plan, void* workspace, void* device_io, void* cuda_stream,
+                      uint64_t n, const uint16_t* x, const uint16_t* y, const uint64_t* toa,
+                      const uint16_t* tot, uint32_t* perm, uint32_t* label, uint64_t max_clusters,
+                      const tpx3_clusters_t* out_host, uint32_t* n_clusters_host);
+
+/* Synchronise `cuda_stream` and copy the workspace's status word to *out [host]. */
+int tpx3_status(tpx3_plan_t plan, const void* workspace, void* cuda_stream, tpx3_status_t* out);
+
+/* Number of kernels the library has launched through this plan (for launch accounting). */
+uint64_t tpx3_launch_count(tpx3_plan_t plan);
+
+int tpx3_free(tpx3_plan_t plan);
+const char* tpx3_strerror(int err);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPX3_H_ */

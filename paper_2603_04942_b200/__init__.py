@@ -1,0 +1,296 @@
+"""paper_2603_04942_b200 — thin Python binding of libtpx3 (include/tpx3.h).
+
+The binding only marshals arguments: PyTorch supplies device memory and the CUDA stream; every
+step of the hot path (sort, link, label compression, reduction, centroid) runs in the CUDA
+kernels of csrc/. There is no CPU fallback: if the library cannot be built or loaded, or the
+tensors are not CUDA tensors, the calls raise.
+
+Function names follow the C ABI: plan / cluster / centroid / cluster_centroid / process_host /
+status / free (tpx3_* in the header).
+"""
+from __future__ import annotations
+
+import ctypes
+from dataclasses import dataclass
+
+from . import _build
+
+__all__ = [
+    "Tpx3Error", "Config", "Clusters", "Plan", "plan", "load_library", "exported_symbols",
+    "FLAG_VALIDATE_INPUT", "FLAG_FORCE_GENERAL", "strerror", "shard_shots",
+]
+
+FLAG_VALIDATE_INPUT = 1 << 0
+FLAG_FORCE_GENERAL = 1 << 1
+
+OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_OUT_OF_RANGE, ERR_CUDA, ERR_UNIMPLEMENTED = 0, -1, -2, -3, -4, -5
+
+# Every symbol include/tpx3.h declares (tests check the built library exports all of them).
+exported_symbols = (
+    "tpx3_plan", "tpx3_cluster", "tpx3_centroid", "tpx3_cluster_centroid", "tpx3_host_io_bytes",
+    "tpx3_process_host", "tpx3_status", "tpx3_launch_count", "tpx3_free", "tpx3_strerror",
+)
+
+
+class Tpx3Error(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__("%s failed: %s (%d)" % (where, strerror(code), code))
+
+
+class _CConfig(ctypes.Structure):
+    _fields_ = [
+        ("struct_size", ctypes.c_uint32), ("sensor_w", ctypes.c_uint16), ("sensor_h", ctypes.c_uint16),
+        ("toa_window_ticks", ctypes.c_uint32), ("shot_period_ticks", ctypes.c_uint64),
+        ("max_hits", ctypes.c_uint64), ("device", ctypes.c_int32), ("flags", ctypes.c_uint32),
+    ]
+
+
+class _CClusters(ctypes.Structure):
+    _fields_ = [(k, ctypes.c_void_p) for k in
+                ("label", "size", "shot", "sum_tot", "sum_tot_x", "sum_tot_y", "toa_peak", "cx", "cy")]
+
+
+class _CStatus(ctypes.Structure):
+    _fields_ = [("error", ctypes.c_uint32), ("path", ctypes.c_uint32), ("n_clusters", ctypes.c_uint32),
+                ("sort_passes", ctypes.c_uint32), ("n", ctypes.c_uint64)]
+
+
+_lib = None
+
+
+def load_library(build: bool = True) -> ctypes.CDLL:
+    """Load (building first if stale) libtpx3.so and declare the prototypes. Raises on failure."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build() if build else _build.LIB
+    lib = ctypes.CDLL(path)
+    vp, u64, u32p = ctypes.c_void_p, ctypes.c_uint64, ctypes.c_void_p
+    lib.tpx3_plan.restype = ctypes.c_int
+    lib.tpx3_plan.argtypes = [ctypes.POINTER(_CConfig), ctypes.POINTER(vp), ctypes.POINTER(ctypes.c_size_t)]
+    lib.tpx3_cluster.restype = ctypes.c_int
+    lib.tpx3_cluster.argtypes = [vp, vp, vp, u64, vp, vp, vp, vp, vp, vp, u32p]
+    lib.tpx3_centroid.restype = ctypes.c_int
+    lib.tpx3_centroid.argtypes = [vp, vp, vp, u64, vp, vp, vp, vp, vp, vp, u64, ctypes.POINTER(_CClusters), u32p]
+    lib.tpx3_cluster_centroid.restype = ctypes.c_int
+    lib.tpx3_cluster_centroid.argtypes = [vp, vp, vp, u64, vp, vp, vp, vp, vp, vp, u64,
+                                          ctypes.POINTER(_CClusters), u32p]
+    lib.tpx3_host_io_bytes.restype = ctypes.c_size_t
+    lib.tpx3_host_io_bytes.argtypes = [u64, u64]
+    lib.tpx3_process_host.restype = ctypes.c_int
+    lib.tpx3_process_host.argtypes = [vp, vp, vp, vp, u64, vp, vp, vp, vp, vp, vp, u64,
+                                      ctypes.POINTER(_CClusters), vp]
+    lib.tpx3_status.restype = ctypes.c_int
+    lib.tpx3_status.argtypes = [vp, vp, vp, ctypes.POINTER(_CStatus)]
+    lib.tpx3_launch_count.restype = ctypes.c_uint64
+    lib.tpx3_launch_count.argtypes = [vp]
+    lib.tpx3_free.restype = ctypes.c_int
+    lib.tpx3_free.argtypes = [vp]
+    lib.tpx3_strerror.restype = ctypes.c_char_p
+    lib.tpx3_strerror.argtypes = [ctypes.c_int]
+    _lib = lib
+    return lib
+
+
+def strerror(code: int) -> str:
+    return load_library().tpx3_strerror(int(code)).decode()
+
+
+@dataclass
+class Config:
+    sensor_w: int = 256
+    sensor_h: int = 256
+    toa_window_ticks: int = 320
+    shot_period_ticks: int = 640000
+    max_hits: int = 1 << 20
+    device: int = 0
+    flags: int = 0
+
+
+_CLUSTER_FIELDS = (
+    ("label", "uint32"), ("size", "uint32"), ("shot", "uint32"), ("sum_tot", "int64"), ("sum_tot_x", "int64"),
+    ("sum_tot_y", "int64"), ("toa_peak", "uint64"), ("cx", "float32"), ("cy", "float32"),
+)
+
+
+class Clusters:
+    """Per-hit output arrays (structure of arrays) of capacity ``max_clusters``.
+    device tensors (torch) or pinned host tensors, depending on who allocated them."""
+
+    def __init__(self, max_clusters: int, device, pin: bool = False):
+        import torch
+
+        self.max_clusters = int(max_clusters)
+        cap = max(self.max_clusters, 1)
+        for name, dt in _CLUSTER_FIELDS:
+            t = torch.empty(cap, dtype=getattr(torch, dt), device=device, pin_memory=pin)
+            setattr(self, name, t)
+
+    def _c(self) -> _CClusters:
+        c = _CClusters()
+        for name, _ in _CLUSTER_FIELDS:
+            setattr(c, name, getattr(self, name).data_ptr())
+        return c
+
+    def numpy(self, n: int) -> dict:
+        """First n entries of every array as numpy (keys prefixed c_, like the oracle's)."""
+        return {"c_" + name: getattr(self, name)[:n].cpu().numpy() for name, _ in _CLUSTER_FIELDS}
+
+
+def _stream_ptr(stream) -> int:
+    import torch
+
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def _check_dev(t, dtype, n, name):
+    import torch
+
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError("%s must be a CUDA tensor (there is no CPU path)" % name)
+    if t.dtype != dtype or not t.is_contiguous() or t.numel() < n:
+        raise TypeError("%s must be a contiguous %s tensor with at least %d elements" % (name, dtype, n))
+
+
+class Plan:
+    """tpx3_plan + a torch-allocated workspace on the plan's device."""
+
+    def __init__(self, cfg: Config):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2603_04942_b200 needs a CUDA device; there is no CPU fallback")
+        self.lib = load_library()
+        self.cfg = cfg
+        c = _CConfig(ctypes.sizeof(_CConfig), cfg.sensor_w, cfg.sensor_h, cfg.toa_window_ticks,
+                     cfg.shot_period_ticks, cfg.max_hits, cfg.device, cfg.flags)
+        h = ctypes.c_void_p()
+        ws = ctypes.c_size_t()
+        rc = self.lib.tpx3_plan(ctypes.byref(c), ctypes.byref(h), ctypes.byref(ws))
+        if rc != OK:
+            raise Tpx3Error(rc, "tpx3_plan")
+        self.handle = h
+        self.workspace_bytes = int(ws.value)
+        self.device = torch.device("cuda", cfg.device)
+        self.workspace = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=self.device)
+        self._io = None
+
+    # -- S0-S3 ---------------------------------------------------------------------------------
+    def cluster(self, x, y, toa, tot, perm=None, label=None, n_clusters=None, stream=None):
+        import torch
+
+        n = int(x.numel())
+        self._check_inputs(x, y, toa, tot, n)
+        perm = torch.empty(max(n, 1), dtype=torch.uint32, device=self.device) if perm is None else perm
+        label = torch.empty(max(n, 1), dtype=torch.uint32, device=self.device) if label is None else label
+        n_clusters = torch.empty(1, dtype=torch.uint32, device=self.device) if n_clusters is None else n_clusters
+        rc = self.lib.tpx3_cluster(self.handle, self.workspace.data_ptr(), _stream_ptr(stream), n, x.data_ptr(),
+                                   y.data_ptr(), toa.data_ptr(), tot.data_ptr(), perm.data_ptr(), label.data_ptr(),
+                                   n_clusters.data_ptr())
+        if rc != OK:
+            raise Tpx3Error(rc, "tpx3_cluster")
+        return perm, label, n_clusters
+
+    # -- S4-S5 ---------------------------------------------------------------------------------
+    def centroid(self, x, y, toa, tot, perm, label, clusters: Clusters, n_clusters=None, stream=None):
+        import torch
+
+        n = int(x.numel())
+        self._check_inputs(x, y, toa, tot, n)
+        _check_dev(perm, torch.uint32, n, "perm")
+        _check_dev(label, torch.uint32, n, "label")
+        n_clusters = torch.empty(1, dtype=torch.uint32, device=self.device) if n_clusters is None else n_clusters
+        c = clusters._c()
+        rc = self.lib.tpx3_centroid(self.handle, self.workspace.data_ptr(), _stream_ptr(stream), n, x.data_ptr(),
+                                    y.data_ptr(), toa.data_ptr(), tot.data_ptr(), perm.data_ptr(), label.data_ptr(),
+                                    clusters.max_clusters, ctypes.byref(c), n_clusters.data_ptr())
+        if rc != OK:
+            raise Tpx3Error(rc, "tpx3_centroid")
+        return n_clusters
+
+    # -- S0-S5 fused ---------------------------------------------------------------------------
+    def cluster_centroid(self, x, y, toa, tot, clusters: Clusters, perm=None, label=None, n_clusters=None,
+                         stream=None):
+        import torch
+
+        n = int(x.numel())
+        self._check_inputs(x, y, toa, tot, n)
+        perm = torch.empty(max(n, 1), dtype=torch.uint32, device=self.device) if perm is None else perm
+        label = torch.empty(max(n, 1), dtype=torch.uint32, device=self.device) if label is None else label
+        n_clusters = torch.empty(1, dtype=torch.uint32, device=self.device) if n_clusters is None else n_clusters
+        c = clusters._c()
+        rc = self.lib.tpx3_cluster_centroid(self.handle, self.workspace.data_ptr(), _stream_ptr(stream), n,
+                                            x.data_ptr(), y.data_ptr(), toa.data_ptr(), tot.data_ptr(),
+                                            perm.data_ptr(), label.data_ptr(), clusters.max_clusters,
+                                            ctypes.byref(c), n_clusters.data_ptr())
+        if rc != OK:
+            raise Tpx3Error(rc, "tpx3_cluster_centroid")
+        return perm, label, n_clusters
+
+    # -- end to end with host buffers ------------------------------------------------------------
+    def process_host(self, x, y, toa, tot, clusters_host: Clusters, perm=None, label=None, stream=None) -> int:
+        """x, y, toa, tot: host tensors (pinned for full copy speed). perm / label: host uint32
+        tensors or None. Copies in, runs the fused call, copies out, synchronises. Returns the hit count."""
+        import torch
+
+        n = int(x.numel())
+        need = int(self.lib.tpx3_host_io_bytes(n, clusters_host.max_clusters))
+        if self._io is None or self._io.numel() < need:
+            self._io = torch.empty(need, dtype=torch.uint8, device=self.device)
+        nc = ctypes.c_uint32(0)
+        c = clusters_host._c()
+        rc = self.lib.tpx3_process_host(
+            self.handle, self.workspace.data_ptr(), self._io.data_ptr(), _stream_ptr(stream), n, x.data_ptr(),
+            y.data_ptr(), toa.data_ptr(), tot.data_ptr(), perm.data_ptr() if perm is not None else None,
+            label.data_ptr() if label is not None else None, clusters_host.max_clusters, ctypes.byref(c),
+            ctypes.addressof(nc))
+        if rc != OK:
+            raise Tpx3Error(rc, "tpx3_process_host")
+        return int(nc.value)
+
+    def status(self, stream=None) -> dict:
+        s = _CStatus()
+        rc = self.lib.tpx3_status(self.handle, self.workspace.data_ptr(), _stream_ptr(stream), ctypes.byref(s))
+        if rc != OK:
+            raise Tpx3Error(rc, "tpx3_status")
+        return {"error": -int(s.error), "path": int(s.path), "n_clusters": int(s.n_clusters),
+                "sort_passes": int(s.sort_passes), "n": int(s.n)}
+
+    def launch_count(self) -> int:
+        return int(self.lib.tpx3_launch_count(self.handle))
+
+    def free(self):
+        if self.handle:
+            self.lib.tpx3_free(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+    def _check_inputs(self, x, y, toa, tot, n):
+        import torch
+
+        _check_dev(x, torch.uint16, n, "x")
+        _check_dev(y, torch.uint16, n, "y")
+        _check_dev(toa, torch.uint64, n, "toa")
+        _check_dev(tot, torch.uint16, n, "tot")
+        if n > self.cfg.max_hits:
+            raise Tpx3Error(ERR_INVALID_ARG, "n > max_hits")
+
+
+def plan(cfg: Config) -> Plan:
+    return Plan(cfg)
+
+
+def shard_shots(n_shots: int, world_size: int, rank: int) -> tuple[int, int]:
+    """Contiguous shot range [s0, s1) of `rank`: shots are independent units (no link crosses a
+    shot boundary), so multi-GPU runs shard whole shots with no data-path collective."""
+    base, rem = divmod(int(n_shots), int(world_size))
+    s0 = rank * base + min(rank, rem)
+    return s0, s0 + base + (1 if rank < rem else 0)

@@ -1,0 +1,58 @@
+// Internal definitions shared by the kernels of libtpx3 (sm_100a). Not part of the ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tpx3.h"
+
+namespace tpx3 {
+
+constexpr int kNumSMs = 148;               // B200
+constexpr uint32_t kEmpty = 0xFFFFFFFFu;   // empty hash slot / "no hit"
+constexpr uint64_t kMaxHits = 1ull << 28;  // sorted index fits 28 bits
+
+// Device-resident control block at the start of the workspace.
+struct Ctrl {
+  tpx3_status_t status;          // error, path, n_clusters, sort_passes, n
+  unsigned long long toa_min;    // general path: min / max ToA of the call
+  unsigned long long toa_max;
+  uint32_t npass;                // general path: radix passes to run (>= 1)
+  uint32_t fused_state;          // 0 = not attempted, 1 = succeeded, 2 = failed (general path must run)
+  uint32_t tile_ticket;          // fused path: dynamic tile counter
+  uint32_t n_roots;              // scratch root counter
+  uint32_t pad[4];
+};
+static_assert(sizeof(Ctrl) <= 256, "Ctrl must fit the 256-byte workspace header");
+
+// Parameters every kernel needs (passed by value).
+struct Params {
+  uint64_t n;
+  uint64_t P;        // shot period (0 = one shot)
+  uint32_t W;        // ToA window, inclusive
+  uint32_t sensor_w, sensor_h;
+  uint32_t flags;
+  uint64_t slabs_per_shot_p1;  // ceil(P / (W+1)) + 1 (general path slab numbering), 0 if P == 0
+};
+
+__device__ __forceinline__ void set_error(Ctrl* c, int err) {
+  atomicCAS(&c->status.error, 0u, (uint32_t)(-err));
+}
+
+__device__ __forceinline__ uint32_t lanemask_lt() {
+  uint32_t m;
+  asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+  return m;
+}
+
+// 64-bit unsigned atomic min / max on global memory.
+__device__ __forceinline__ void atomic_min_u64(unsigned long long* p, unsigned long long v) { atomicMin(p, v); }
+__device__ __forceinline__ void atomic_max_u64(unsigned long long* p, unsigned long long v) { atomicMax(p, v); }
+
+// Fill `n` 32-bit words (general_only: skipped when the fused path already succeeded).
+__global__ void __launch_bounds__(256) k_fill_u32(Ctrl* c, int general_only, uint32_t* p, uint64_t n, uint32_t v) {
+  if (general_only && c->fused_state == 1) return;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x)
+    p[i] = v;
+}
+
+}  // namespace tpx3

@@ -1,0 +1,361 @@
+// libtpx3 — host side of the C ABI declared in include/tpx3.h: plan, workspace layout, kernel
+// launches. All device work is enqueued on the caller's stream; nothing here synchronises
+// except tpx3_status and tpx3_process_host (which say so in the header).
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "tpx3_centroid.cuh"
+#include "tpx3_common.cuh"
+#include "tpx3_fused.cuh"
+#include "tpx3_link.cuh"
+#include "tpx3_sort.cuh"
+
+using namespace tpx3;
+
+struct tpx3_plan_s {
+  tpx3_config_t cfg;
+  Params prm;               // n filled per call
+  size_t workspace_bytes;
+  uint64_t launches;
+  int num_sms;
+  // workspace offsets (bytes from the workspace base), sized for cfg.max_hits
+  size_t off_keyA, off_keyB, off_idxA, off_idxB, off_xy, off_tot, off_slab, off_table, off_counts;
+  size_t off_slot, off_peak, off_blkcnt, off_tiles;
+  uint32_t table_mask_max;
+};
+
+namespace {
+
+inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+inline uint32_t table_size_for(uint64_t n) {  // power of two >= 2n, >= 1024
+  uint64_t s = 1024;
+  while (s < 2 * n) s <<= 1;
+  return (uint32_t)s;
+}
+
+#define TPX3_LAUNCH(plan, kernel, grid, block, smem, stream, ...)          \
+  do {                                                                     \
+    kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);            \
+    ++(plan)->launches;                                                    \
+  } while (0)
+
+inline int cuda_ok(cudaError_t e) { return e == cudaSuccess ? TPX3_OK : TPX3_ERR_CUDA; }
+
+inline uint32_t grid_for(uint64_t n, int threads, int num_sms, int per_sm = 8) {
+  uint64_t b = (n + threads - 1) / threads;
+  uint64_t cap = (uint64_t)num_sms * per_sm;
+  if (b > cap) b = cap;
+  return (uint32_t)(b ? b : 1);
+}
+
+struct Ws {
+  Ctrl* ctrl;
+  uint64_t *keyA, *keyB, *slab;
+  uint32_t *idxA, *idxB, *xy, *table, *counts, *slot, *blkcnt;
+  uint16_t* tot;
+  unsigned long long* peak;
+  unsigned long long* tiles;
+};
+
+inline Ws carve(const tpx3_plan_s* p, void* workspace) {
+  char* b = (char*)workspace;
+  Ws w;
+  w.ctrl = (Ctrl*)b;
+  w.keyA = (uint64_t*)(b + p->off_keyA);
+  w.keyB = (uint64_t*)(b + p->off_keyB);
+  w.idxA = (uint32_t*)(b + p->off_idxA);
+  w.idxB = (uint32_t*)(b + p->off_idxB);
+  w.xy = (uint32_t*)(b + p->off_xy);
+  w.tot = (uint16_t*)(b + p->off_tot);
+  w.slab = (uint64_t*)(b + p->off_slab);
+  w.table = (uint32_t*)(b + p->off_table);
+  w.counts = (uint32_t*)(b + p->off_counts);
+  w.slot = (uint32_t*)(b + p->off_slot);
+  w.peak = (unsigned long long*)(b + p->off_peak);
+  w.blkcnt = (uint32_t*)(b + p->off_blkcnt);
+  w.tiles = (unsigned long long*)(b + p->off_tiles);
+  return w;
+}
+
+// ---- general path: S0-S3 ------------------------------------------------------------------
+int enqueue_general_cluster(tpx3_plan_s* p, const Ws& w, cudaStream_t st, uint64_t n, const uint16_t* x,
+                            const uint16_t* y, const uint64_t* toa, const uint16_t* tot, uint32_t* perm,
+                            uint32_t* label, uint32_t* n_clusters) {
+  Params prm = p->prm;
+  prm.n = n;
+  const int sms = p->num_sms;
+  TPX3_LAUNCH(p, k_minmax, grid_for(n, 256 * 8, sms), 256, 0, st, w.ctrl, toa, n);
+  TPX3_LAUNCH(p, k_sort_setup, 1, 1, 0, st, w.ctrl);
+  SortGeom g = sort_geom(n);
+  SortBufs b;
+  b.key[0] = w.keyA; b.key[1] = w.keyB; b.idx[0] = w.idxA; b.idx[1] = w.idxB; b.counts = w.counts;
+  // Passes needed for the largest span a ToA can have; the ones past the device-computed
+  // `npass` return at once. 64-bit ToA => at most 8 passes.
+  for (int pass = 0; pass < kMaxPasses; ++pass) {
+    TPX3_LAUNCH(p, k_radix_hist, g.nblk, kSortThreads, 0, st, w.ctrl, pass, toa, b, n, g);
+    TPX3_LAUNCH(p, k_radix_scan, 1, 1024, 0, st, w.ctrl, pass, w.counts, (uint32_t)(kRadix * g.nblk));
+    TPX3_LAUNCH(p, k_radix_scatter, g.nblk, kSortThreads, 0, st, w.ctrl, pass, toa, b, perm, n, g);
+  }
+  TPX3_LAUNCH(p, k_gather, grid_for(n, 256, sms), 256, 0, st, w.ctrl, prm, w.keyA, w.keyB, perm, x, y, tot, w.xy,
+              w.tot, w.slab, label);
+  uint32_t tsize = table_size_for(n);
+  TPX3_LAUNCH(p, k_fill_u32, grid_for(tsize, 256, sms), 256, 0, st, w.ctrl, 1, w.table, (uint64_t)tsize, kEmpty);
+  TPX3_LAUNCH(p, k_hash_insert, grid_for(n, 256, sms), 256, 0, st, w.ctrl, n, w.xy, w.slab, w.table, tsize - 1);
+  TPX3_LAUNCH(p, k_link, grid_for(n, 256, sms), 256, 0, st, w.ctrl, prm, w.keyA, w.keyB, w.xy, w.slab, w.table,
+              tsize - 1, label);
+  TPX3_LAUNCH(p, k_compress, grid_for(n, 256, sms), 256, 0, st, w.ctrl, n, label, n_clusters);
+  return cuda_ok(cudaGetLastError());
+}
+
+// ---- S4-S5 from (perm, label) -------------------------------------------------------------
+int enqueue_centroid(tpx3_plan_s* p, const Ws& w, cudaStream_t st, int general_only, uint64_t n, const uint16_t* x,
+                     const uint16_t* y, const uint64_t* toa, const uint16_t* tot, const uint32_t* perm,
+                     const uint32_t* label, uint64_t max_clusters, const tpx3_clusters_t& out, uint32_t* n_clusters) {
+  Params prm = p->prm;
+  prm.n = n;
+  const int sms = p->num_sms;
+  uint32_t nblk = (uint32_t)((n + kCentTile - 1) / kCentTile);
+  if (nblk == 0) nblk = 1;
+  TPX3_LAUNCH(p, k_root_count, nblk, kCentThreads, 0, st, w.ctrl, general_only, n, label, w.blkcnt);
+  TPX3_LAUNCH(p, k_root_scan, 1, 1024, 0, st, w.ctrl, general_only, w.blkcnt, nblk, max_clusters, n_clusters);
+  TPX3_LAUNCH(p, k_root_slots, nblk, kCentThreads, 0, st, w.ctrl, general_only, n, label, w.blkcnt, w.slot,
+              max_clusters, out, w.peak);
+  TPX3_LAUNCH(p, k_accumulate, grid_for(n, 256, sms), 256, 0, st, w.ctrl, general_only, n, x, y, tot, perm, label,
+              w.slot, max_clusters, out, w.peak);
+  TPX3_LAUNCH(p, k_finalize, grid_for(max_clusters < n ? max_clusters : n, 256, sms), 256, 0, st, w.ctrl,
+              general_only, prm, toa, perm, n_clusters, max_clusters, out, w.peak);
+  return cuda_ok(cudaGetLastError());
+}
+
+bool clusters_ok(const tpx3_clusters_t* o) {
+  return o && o->label && o->size && o->shot && o->sum_tot && o->sum_tot_x && o->sum_tot_y && o->toa_peak && o->cx &&
+         o->cy;
+}
+
+}  // namespace
+
+extern "C" {
+
+int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace_bytes) {
+  if (!cfg || !out_plan || !workspace_bytes) return TPX3_ERR_INVALID_ARG;
+  if (cfg->struct_size != sizeof(tpx3_config_t)) return TPX3_ERR_INVALID_ARG;
+  if (cfg->sensor_w == 0 || cfg->sensor_h == 0 || cfg->sensor_w > 256 || cfg->sensor_h > 256)
+    return TPX3_ERR_INVALID_ARG;
+  if (cfg->max_hits == 0 || cfg->max_hits > kMaxHits) return TPX3_ERR_INVALID_ARG;
+  if (cfg->toa_window_ticks >= (1u << 31)) return TPX3_ERR_INVALID_ARG;
+  if (cfg->device < 0) return TPX3_ERR_INVALID_ARG;
+  tpx3_plan_s* p = new (std::nothrow) tpx3_plan_s();
+  if (!p) return TPX3_ERR_CUDA;
+  p->cfg = *cfg;
+  p->launches = 0;
+  p->num_sms = kNumSMs;
+  Params& prm = p->prm;
+  prm.n = 0;
+  prm.P = cfg->shot_period_ticks;
+  prm.W = cfg->toa_window_ticks;
+  prm.sensor_w = cfg->sensor_w;
+  prm.sensor_h = cfg->sensor_h;
+  prm.flags = cfg->flags;
+  prm.slabs_per_shot_p1 = prm.P ? (prm.P + prm.W) / (prm.W + 1ull) + 1ull : 0ull;
+  const uint64_t N = cfg->max_hits;
+  size_t o = 256;  // Ctrl
+  // general-path cluster buffers
+  p->off_keyA = o; o = align_up(o + 8 * N);
+  p->off_keyB = o; o = align_up(o + 8 * N);
+  p->off_idxA = o; o = align_up(o + 4 * N);
+  p->off_idxB = o; o = align_up(o + 4 * N);
+  p->off_xy = o; o = align_up(o + 4 * N);
+  p->off_tot = o; o = align_up(o + 2 * N);
+  p->off_slab = o; o = align_up(o + 8 * N);
+  p->off_table = o; o = align_up(o + 4 * (size_t)table_size_for(N));
+  p->off_counts = o; o = align_up(o + 4 * (size_t)kRadix * kSortMaxBlocks);
+  // centroid buffers alias the sort buffers (the two steps never run concurrently and the
+  // centroid step takes perm/label from the caller, not from the workspace)
+  p->off_slot = p->off_keyA;                    // 4N <= 8N
+  p->off_peak = p->off_keyB;                    // 8N
+  p->off_blkcnt = p->off_idxA;                  // 4 * ceil(N/4096) <= 4N
+  p->off_tiles = o; o = align_up(o + 8 * (size_t)(N / 256 + 1024));  // fused path tile status words
+  p->workspace_bytes = o;
+  *workspace_bytes = o;
+  *out_plan = p;
+  return TPX3_OK;
+}
+
+int tpx3_cluster(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x, const uint16_t* y,
+                 const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label, uint32_t* n_clusters) {
+  if (!p || !workspace || !n_clusters) return TPX3_ERR_INVALID_ARG;
+  if (n > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
+  if (n && (!x || !y || !toa || !tot || !perm || !label)) return TPX3_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  Ws w = carve(p, workspace);
+  TPX3_LAUNCH(p, k_ctrl_init, 1, 1, 0, st, w.ctrl, n);
+  TPX3_LAUNCH(p, k_fill_u32, 1, 32, 0, st, w.ctrl, 0, n_clusters, (uint64_t)1, 0u);
+  if (n == 0) return cuda_ok(cudaGetLastError());
+  return enqueue_general_cluster(p, w, st, n, x, y, toa, tot, perm, label, n_clusters);
+}
+
+int tpx3_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x, const uint16_t* y,
+                  const uint64_t* toa, const uint16_t* tot, const uint32_t* perm, const uint32_t* label,
+                  uint64_t max_clusters, const tpx3_clusters_t* out, uint32_t* n_clusters) {
+  if (!p || !workspace || !n_clusters) return TPX3_ERR_INVALID_ARG;
+  if (n > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
+  if (n && (!x || !y || !toa || !tot || !perm || !label)) return TPX3_ERR_INVALID_ARG;
+  if (max_clusters && !clusters_ok(out)) return TPX3_ERR_INVALID_ARG;
+  if (n && !out) return TPX3_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  Ws w = carve(p, workspace);
+  TPX3_LAUNCH(p, k_ctrl_init, 1, 1, 0, st, w.ctrl, n);
+  if (n == 0) {
+    TPX3_LAUNCH(p, k_fill_u32, 1, 32, 0, st, w.ctrl, 0, n_clusters, (uint64_t)1, 0u);
+    return cuda_ok(cudaGetLastError());
+  }
+  return enqueue_centroid(p, w, st, 0, n, x, y, toa, tot, perm, label, max_clusters, *out, n_clusters);
+}
+
+int tpx3_cluster_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x,
+                          const uint16_t* y, const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label,
+                          uint64_t max_clusters, const tpx3_clusters_t* out, uint32_t* n_clusters) {
+  if (!p || !workspace || !n_clusters) return TPX3_ERR_INVALID_ARG;
+  if (n > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
+  if (n && (!x || !y || !toa || !tot || !perm || !label || !out)) return TPX3_ERR_INVALID_ARG;
+  if (max_clusters && !clusters_ok(out)) return TPX3_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  Ws w = carve(p, workspace);
+  TPX3_LAUNCH(p, k_ctrl_init, 1, 1, 0, st, w.ctrl, n);
+  TPX3_LAUNCH(p, k_fill_u32, 1, 32, 0, st, w.ctrl, 0, n_clusters, (uint64_t)1, 0u);
+  if (n == 0) return cuda_ok(cudaGetLastError());
+  Params prm = p->prm;
+  prm.n = n;
+  int rc = TPX3_OK;
+  if (!(p->cfg.flags & TPX3_FLAG_FORCE_GENERAL)) {
+    rc = enqueue_fused(p->num_sms, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, label, max_clusters,
+                       *out, n_clusters);
+    if (rc != TPX3_OK) return rc;
+  }
+  // General path: every kernel below returns at once if the fused kernel succeeded.
+  rc = enqueue_general_cluster(p, w, st, n, x, y, toa, tot, perm, label, n_clusters);
+  if (rc != TPX3_OK) return rc;
+  return enqueue_centroid(p, w, st, 1, n, x, y, toa, tot, perm, label, max_clusters, *out, n_clusters);
+}
+
+size_t tpx3_host_io_bytes(uint64_t n, uint64_t max_clusters) {
+  size_t o = 0;
+  o = align_up(o + 2 * n);        // x
+  o = align_up(o + 2 * n);        // y
+  o = align_up(o + 8 * n);        // toa
+  o = align_up(o + 2 * n);        // tot
+  o = align_up(o + 4 * n);        // perm
+  o = align_up(o + 4 * n);        // label
+  o = align_up(o + 4 * max_clusters) * 1;  // label
+  o = align_up(o + 4 * max_clusters);      // size
+  o = align_up(o + 4 * max_clusters);      // shot
+  o = align_up(o + 8 * max_clusters);      // sum_tot
+  o = align_up(o + 8 * max_clusters);      // sum_tot_x
+  o = align_up(o + 8 * max_clusters);      // sum_tot_y
+  o = align_up(o + 8 * max_clusters);      // toa_peak
+  o = align_up(o + 4 * max_clusters);      // cx
+  o = align_up(o + 4 * max_clusters);      // cy
+  o = align_up(o + 256);                   // n_clusters
+  return o;
+}
+
+int tpx3_process_host(tpx3_plan_t p, void* workspace, void* device_io, void* cuda_stream, uint64_t n, const uint16_t* x,
+                      const uint16_t* y, const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label,
+                      uint64_t max_clusters, const tpx3_clusters_t* out_host, uint32_t* n_clusters_host) {
+  if (!p || !workspace || !device_io || !n_clusters_host) return TPX3_ERR_INVALID_ARG;
+  if (n > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
+  if (n && (!x || !y || !toa || !tot)) return TPX3_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  char* b = (char*)device_io;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { char* r = b + o; o = align_up(o + bytes); return r; };
+  uint16_t* dx = (uint16_t*)take(2 * n);
+  uint16_t* dy = (uint16_t*)take(2 * n);
+  uint64_t* dtoa = (uint64_t*)take(8 * n);
+  uint16_t* dtot = (uint16_t*)take(2 * n);
+  uint32_t* dperm = (uint32_t*)take(4 * n);
+  uint32_t* dlabel = (uint32_t*)take(4 * n);
+  tpx3_clusters_t d;
+  d.label = (uint32_t*)take(4 * max_clusters);
+  d.size = (uint32_t*)take(4 * max_clusters);
+  d.shot = (uint32_t*)take(4 * max_clusters);
+  d.sum_tot = (int64_t*)take(8 * max_clusters);
+  d.sum_tot_x = (int64_t*)take(8 * max_clusters);
+  d.sum_tot_y = (int64_t*)take(8 * max_clusters);
+  d.toa_peak = (uint64_t*)take(8 * max_clusters);
+  d.cx = (float*)take(4 * max_clusters);
+  d.cy = (float*)take(4 * max_clusters);
+  uint32_t* dn = (uint32_t*)take(256);
+  cudaError_t e = cudaSuccess;
+  if (n) {
+    e = cudaMemcpyAsync(dx, x, 2 * n, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dy, y, 2 * n, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dtoa, toa, 8 * n, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dtot, tot, 2 * n, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return TPX3_ERR_CUDA;
+  }
+  int rc = tpx3_cluster_centroid(p, workspace, cuda_stream, n, dx, dy, dtoa, dtot, dperm, dlabel, max_clusters, &d, dn);
+  if (rc != TPX3_OK) return rc;
+  e = cudaMemcpyAsync(n_clusters_host, dn, 4, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && perm && n) e = cudaMemcpyAsync(perm, dperm, 4 * n, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && label && n) e = cudaMemcpyAsync(label, dlabel, 4 * n, cudaMemcpyDeviceToHost, st);
+  if (e != cudaSuccess) return TPX3_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return TPX3_ERR_CUDA;  // the count decides the copy sizes
+  uint64_t nc = *n_clusters_host;
+  if (nc > max_clusters) nc = max_clusters;
+  if (out_host && nc) {
+    const tpx3_clusters_t& h = *out_host;
+    if (h.label) e = cudaMemcpyAsync(h.label, d.label, 4 * nc, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && h.size) e = cudaMemcpyAsync(h.size, d.size, 4 * nc, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && h.shot) e = cudaMemcpyAsync(h.shot, d.shot, 4 * nc, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && h.sum_tot) e = cudaMemcpyAsync(h.sum_tot, d.sum_tot, 8 * nc, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && h.sum_tot_x) e = cudaMemcpyAsync(h.sum_tot_x, d.sum_tot_x, 8 * nc, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && h.sum_tot_y) e = cudaMemcpyAsync(h.sum_tot_y, d.sum_tot_y, 8 * nc, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && h.toa_peak) e = cudaMemcpyAsync(h.toa_peak, d.toa_peak, 8 * nc, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && h.cx) e = cudaMemcpyAsync(h.cx, d.cx, 4 * nc, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && h.cy) e = cudaMemcpyAsync(h.cy, d.cy, 4 * nc, cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return TPX3_ERR_CUDA;
+  }
+  tpx3_status_t s;
+  rc = tpx3_status(p, workspace, cuda_stream, &s);
+  if (rc != TPX3_OK) return rc;
+  return s.error ? -(int)s.error : TPX3_OK;
+}
+
+int tpx3_status(tpx3_plan_t p, const void* workspace, void* cuda_stream, tpx3_status_t* out) {
+  if (!p || !workspace || !out) return TPX3_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  if (cudaMemcpyAsync(out, workspace, sizeof(tpx3_status_t), cudaMemcpyDeviceToHost, st) != cudaSuccess)
+    return TPX3_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return TPX3_ERR_CUDA;
+  return TPX3_OK;
+}
+
+uint64_t tpx3_launch_count(tpx3_plan_t p) { return p ? p->launches : 0; }
+
+int tpx3_free(tpx3_plan_t p) {
+  if (!p) return TPX3_ERR_INVALID_ARG;
+  delete p;
+  return TPX3_OK;
+}
+
+const char* tpx3_strerror(int err) {
+  switch (err) {
+    case TPX3_OK: return "ok";
+    case TPX3_ERR_INVALID_ARG: return "invalid argument";
+    case TPX3_ERR_CAPACITY: return "max_clusters too small";
+    case TPX3_ERR_OUT_OF_RANGE: return "event outside the sensor or ToT == 0";
+    case TPX3_ERR_CUDA: return "CUDA runtime error";
+    case TPX3_ERR_UNIMPLEMENTED: return "not implemented";
+    default: return "unknown error";
+  }
+}
+
+}  // extern "C"

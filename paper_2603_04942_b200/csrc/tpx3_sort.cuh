@@ -1,0 +1,198 @@
+// General path, S0/S1: stable LSD radix sort of the events by ToA (key = ToA - min ToA; the
+// (shot, ToA) order of the contract is the ToA order because shot = ToA div P is monotone in
+// ToA — SURVEY.md §8a S0). 8-bit digits; the number of passes is decided on the
+// device from the key span, so no host synchronisation is needed: every pass is enqueued and
+// the ones past `npass` return immediately.
+//
+// Per pass: digit histogram per block -> exclusive scan (digit-major) -> stable scatter.
+// Stability inside a tile comes from warp-ordered ranking with __match_any_sync (each warp owns
+// a contiguous slice of the tile; items are visited in ascending position).
+#pragma once
+#include "tpx3_common.cuh"
+
+namespace tpx3 {
+
+constexpr int kSortThreads = 256;
+constexpr int kSortWarps = kSortThreads / 32;
+constexpr int kSortItems = 8;                               // per thread per tile
+constexpr int kSortTile = kSortThreads * kSortItems;        // 2048
+constexpr int kSortMaxBlocks = kNumSMs * 8;                 // 1184
+constexpr int kRadixBits = 8;
+constexpr int kRadix = 1 << kRadixBits;
+constexpr int kMaxPasses = 8;
+
+struct SortGeom {
+  uint32_t nblk;            // blocks
+  uint32_t tiles_per_blk;   // tiles each block walks sequentially
+};
+
+inline SortGeom sort_geom(uint64_t n) {
+  uint64_t tiles = (n + kSortTile - 1) / kSortTile;
+  SortGeom g;
+  g.nblk = (uint32_t)(tiles < (uint64_t)kSortMaxBlocks ? (tiles ? tiles : 1) : kSortMaxBlocks);
+  g.tiles_per_blk = (uint32_t)((tiles + g.nblk - 1) / g.nblk);
+  if (g.tiles_per_blk == 0) g.tiles_per_blk = 1;
+  return g;
+}
+
+// ---- min / max ToA ------------------------------------------------------------------------
+__global__ void k_ctrl_init(Ctrl* c, uint64_t n) {
+  c->status.error = 0; c->status.path = 0; c->status.n_clusters = 0; c->status.sort_passes = 0;
+  c->status.n = n;
+  c->toa_min = ~0ull; c->toa_max = 0ull; c->npass = 1; c->fused_state = 0; c->tile_ticket = 0; c->n_roots = 0;
+}
+
+__global__ void __launch_bounds__(256) k_minmax(Ctrl* c, const uint64_t* __restrict__ toa, uint64_t n) {
+  if (c->fused_state == 1) return;
+  unsigned long long lo = ~0ull, hi = 0ull;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+    unsigned long long t = toa[i];
+    lo = t < lo ? t : lo;
+    hi = t > hi ? t : hi;
+  }
+  for (int o = 16; o; o >>= 1) {
+    unsigned long long a = __shfl_xor_sync(0xffffffffu, lo, o), b = __shfl_xor_sync(0xffffffffu, hi, o);
+    lo = a < lo ? a : lo;
+    hi = b > hi ? b : hi;
+  }
+  if ((threadIdx.x & 31) == 0) { atomic_min_u64(&c->toa_min, lo); atomic_max_u64(&c->toa_max, hi); }
+}
+
+__global__ void k_sort_setup(Ctrl* c) {
+  if (c->fused_state == 1) return;
+  unsigned long long span = c->toa_max >= c->toa_min ? c->toa_max - c->toa_min : 0ull;
+  int bits = span ? 64 - __clzll((long long)span) : 1;
+  uint32_t np = (uint32_t)((bits + kRadixBits - 1) / kRadixBits);
+  c->npass = np ? np : 1;
+  c->status.sort_passes = c->npass;
+  c->status.path = 2;
+}
+
+// ---- one radix pass -----------------------------------------------------------------------
+// Source of pass p: p == 0 reads ToA (key = toa - min, idx = position); p >= 1 reads key/idx
+// buffer (p-1)&1. Destination: key buffer p&1; idx buffer p&1, or `perm` on the last pass.
+struct SortBufs {
+  uint64_t* key[2];
+  uint32_t* idx[2];
+  uint32_t* counts;   // [kRadix][nblk]
+};
+
+__device__ __forceinline__ uint64_t sort_load_key(int pass, const Ctrl* c, const uint64_t* toa, const SortBufs& b, uint64_t i) {
+  return pass == 0 ? toa[i] - c->toa_min : b.key[(pass - 1) & 1][i];
+}
+
+__global__ void __launch_bounds__(kSortThreads) k_radix_hist(Ctrl* c, int pass, const uint64_t* __restrict__ toa,
+                                                           SortBufs b, uint64_t n, SortGeom g) {
+  if (c->fused_state == 1 || (uint32_t)pass >= c->npass) return;
+  __shared__ uint32_t hist[kRadix];
+  hist[threadIdx.x] = 0;
+  __syncthreads();
+  const int shift = pass * kRadixBits;
+  uint64_t t0 = (uint64_t)blockIdx.x * g.tiles_per_blk * kSortTile;
+  uint64_t t1 = t0 + (uint64_t)g.tiles_per_blk * kSortTile;
+  if (t1 > n) t1 = n;
+  for (uint64_t i = t0 + threadIdx.x; i < t1; i += kSortThreads) {
+    uint64_t k = sort_load_key(pass, c, toa, b, i);
+    atomicAdd(&hist[(uint32_t)(k >> shift) & (kRadix - 1)], 1u);
+  }
+  __syncthreads();
+  b.counts[(size_t)threadIdx.x * g.nblk + blockIdx.x] = hist[threadIdx.x];
+}
+
+// Exclusive scan of counts[kRadix * nblk] in place (single block of 1024 threads).
+__global__ void __launch_bounds__(1024) k_radix_scan(Ctrl* c, int pass, uint32_t* counts, uint32_t total) {
+  if (c->fused_state == 1 || (uint32_t)pass >= c->npass) return;
+  __shared__ uint32_t warp_sums[32];
+  const uint32_t per = (total + 1023) / 1024;
+  uint32_t beg = threadIdx.x * per, end = beg + per;
+  if (beg > total) beg = total;
+  if (end > total) end = total;
+  uint32_t s = 0;
+  for (uint32_t i = beg; i < end; ++i) s += counts[i];
+  // block exclusive scan of s
+  uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5, v = s;
+  for (int o = 1; o < 32; o <<= 1) {
+    uint32_t t = __shfl_up_sync(0xffffffffu, v, o);
+    if (lane >= (uint32_t)o) v += t;
+  }
+  if (lane == 31) warp_sums[w] = v;
+  __syncthreads();
+  if (w == 0) {
+    uint32_t ws = warp_sums[lane], x = ws;
+    for (int o = 1; o < 32; o <<= 1) {
+      uint32_t t = __shfl_up_sync(0xffffffffu, x, o);
+      if (lane >= (uint32_t)o) x += t;
+    }
+    warp_sums[lane] = x - ws;
+  }
+  __syncthreads();
+  uint32_t run = warp_sums[w] + v - s;
+  for (uint32_t i = beg; i < end; ++i) {
+    uint32_t t = counts[i];
+    counts[i] = run;
+    run += t;
+  }
+}
+
+__global__ void __launch_bounds__(kSortThreads) k_radix_scatter(Ctrl* c, int pass, const uint64_t* __restrict__ toa,
+                                                              SortBufs b, uint32_t* __restrict__ perm, uint64_t n,
+                                                              SortGeom g) {
+  if (c->fused_state == 1 || (uint32_t)pass >= c->npass) return;
+  __shared__ uint32_t running[kRadix];
+  __shared__ uint32_t warp_cnt[kSortWarps][kRadix];
+  const int shift = pass * kRadixBits;
+  const bool last = (uint32_t)pass + 1 == c->npass;
+  uint64_t* __restrict__ dkey = b.key[pass & 1];
+  uint32_t* __restrict__ didx = last ? perm : b.idx[pass & 1];
+  const uint32_t* __restrict__ sidx = pass == 0 ? nullptr : b.idx[(pass - 1) & 1];
+  const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5, lt = lanemask_lt();
+  running[threadIdx.x] = b.counts[(size_t)threadIdx.x * g.nblk + blockIdx.x];
+  uint64_t t0 = (uint64_t)blockIdx.x * g.tiles_per_blk * kSortTile;
+  for (uint32_t t = 0; t < g.tiles_per_blk; ++t, t0 += kSortTile) {
+    if (t0 >= n) break;
+    for (int i = threadIdx.x; i < kSortWarps * kRadix; i += kSortThreads) (&warp_cnt[0][0])[i] = 0;
+    __syncthreads();
+    uint64_t key[kSortItems];
+    uint32_t rank[kSortItems];
+    const uint64_t wbase = t0 + (uint64_t)w * (32 * kSortItems) + lane;
+#pragma unroll
+    for (int i = 0; i < kSortItems; ++i) {
+      uint64_t pos = wbase + (uint64_t)i * 32;
+      bool valid = pos < n;
+      key[i] = valid ? sort_load_key(pass, c, toa, b, pos) : 0;
+      uint32_t d = valid ? ((uint32_t)(key[i] >> shift) & (kRadix - 1)) : (uint32_t)kRadix;
+      uint32_t peers = __match_any_sync(0xffffffffu, d);
+      uint32_t lr = __popc(peers & lt);
+      uint32_t base = valid ? warp_cnt[w][d] : 0;
+      __syncwarp();
+      if (valid && lr == 0) warp_cnt[w][d] = base + __popc(peers);
+      __syncwarp();
+      rank[i] = base + lr;
+    }
+    __syncthreads();
+    {  // thread d: exclusive prefix over warps, seeded with the block's running global offset
+      uint32_t d = threadIdx.x, run = running[d];
+#pragma unroll
+      for (int ww = 0; ww < kSortWarps; ++ww) {
+        uint32_t cnt = warp_cnt[ww][d];
+        warp_cnt[ww][d] = run;
+        run += cnt;
+      }
+      running[d] = run;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < kSortItems; ++i) {
+      uint64_t pos = wbase + (uint64_t)i * 32;
+      if (pos < n) {
+        uint32_t d = (uint32_t)(key[i] >> shift) & (kRadix - 1);
+        uint32_t dst = warp_cnt[w][d] + rank[i];
+        dkey[dst] = key[i];
+        didx[dst] = pass == 0 ? (uint32_t)pos : sidx[pos];
+      }
+    }
+    __syncthreads();
+  }
+}
+
+}  // namespace tpx3

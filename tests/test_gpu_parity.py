@@ -1,0 +1,262 @@
+"""GPU parity tests: the CUDA path (through the C ABI, include/tpx3.h) against the CPU oracle,
+element by element, on the same seeded inputs.
+
+Bar (BASELINE.json north_star): perm, label, hit count and the integer sums bit-exact; toa_peak,
+shot, size bit-exact; centroids within 1e-6 px absolute — asserted here as exact fp32 equality
+as well, because both sides compute fp32(int64)/fp32(int64) with an IEEE RN divide (R12).
+"""
+import numpy as np
+import pytest
+
+import gen
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+W, P = 320, 640000
+CENTROID_TOL = 1e-6  # px, north_star
+
+
+@pytest.fixture(scope="module")
+def tpx3():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    import paper_2603_04942_b200 as m
+
+    m.load_library()
+    return m
+
+
+def to_dev(a):
+    import torch
+
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run_gpu(m, x, y, toa, tot, W=W, P=P, mode="fused", flags=0, max_clusters=None, sensor=(256, 256)):
+    """mode: 'fused' = tpx3_cluster_centroid; 'split' = tpx3_cluster then tpx3_centroid."""
+    import torch
+
+    n = len(x)
+    pl = m.plan(m.Config(sensor_w=sensor[0], sensor_h=sensor[1], toa_window_ticks=W, shot_period_ticks=P,
+                         max_hits=max(n, 1), flags=flags))
+    dx, dy, dtoa, dtot = (to_dev(np.asarray(x, dtype=np.uint16)), to_dev(np.asarray(y, dtype=np.uint16)),
+                          to_dev(np.asarray(toa, dtype=np.uint64)), to_dev(np.asarray(tot, dtype=np.uint16)))
+    cap = n if max_clusters is None else max_clusters
+    cl = m.Clusters(cap, pl.device)
+    if mode == "fused":
+        perm, label, nc = pl.cluster_centroid(dx, dy, dtoa, dtot, cl)
+    else:
+        perm, label, nc = pl.cluster(dx, dy, dtoa, dtot)
+        nc_a = int(nc.cpu().numpy()[0])
+        nc = pl.centroid(dx, dy, dtoa, dtot, perm, label, cl)
+        assert int(nc.cpu().numpy()[0]) == nc_a
+    torch.cuda.synchronize()
+    st = pl.status()
+    ncl = int(nc.cpu().numpy()[0])
+    out = {"perm": perm[:n].cpu().numpy(), "label": label[:n].cpu().numpy(), "n_clusters": ncl, "status": st}
+    out.update(cl.numpy(min(ncl, cap)))
+    pl.free()
+    return out
+
+
+def assert_parity(g, o, what=""):
+    assert g["n_clusters"] == o["n_clusters"], what
+    np.testing.assert_array_equal(g["perm"], o["perm"], err_msg=what + " perm")
+    np.testing.assert_array_equal(g["label"], o["label"], err_msg=what + " label")
+    for k in ("c_label", "c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_toa_peak"):
+        np.testing.assert_array_equal(g[k], o[k], err_msg=what + " " + k)
+    for k in ("c_cx", "c_cy"):
+        assert np.all(np.abs(g[k].astype(np.float64) - o[k].astype(np.float64)) <= CENTROID_TOL), what + " " + k
+        np.testing.assert_array_equal(g[k], o[k], err_msg=what + " " + k + " (bitwise fp32)")
+
+
+def check(m, x, y, toa, tot, W=W, P=P, modes=("fused", "split"), flags=0, what=""):
+    o = oracle.run(x, y, toa, tot, W, P, threads=0)
+    res = None
+    for mode in modes:
+        res = run_gpu(m, x, y, toa, tot, W, P, mode=mode, flags=flags)
+        assert res["status"]["error"] == 0
+        assert_parity(res, o, "%s [%s]" % (what, mode))
+    return res, o
+
+
+# ------------------------------------------------------------------ the five configs
+def test_cfg0_full(tpx3):
+    w = gen.generate(0)  # ~75k hits, 1000 shots: several tiles and a ragged tail
+    res, o = check(tpx3, w.x, w.y, w.toa, w.tot, what="cfg0")
+    assert o["n_clusters"] > 9000
+
+
+@pytest.mark.parametrize("cfg,shots", [(1, 3000), (2, 1500), (3, 600), (4, 1500)])
+def test_cfg_subsets(tpx3, cfg, shots):
+    w = gen.generate(cfg, shots=shots)
+    check(tpx3, w.x, w.y, w.toa, w.tot, what="cfg%d" % cfg)
+
+
+def test_cfg4_requires_sort(tpx3):
+    w = gen.generate(4, shots=300)
+    assert np.any(np.diff(w.toa.astype(np.int64)) < 0)  # delivered out of order
+    res, o = check(tpx3, w.x, w.y, w.toa, w.tot, what="cfg4")
+    assert np.any(res["perm"] != np.arange(w.n))
+
+
+def test_force_general_path(tpx3):
+    w = gen.generate(2, shots=800)
+    res, _ = check(tpx3, w.x, w.y, w.toa, w.tot, flags=tpx3.FLAG_FORCE_GENERAL, modes=("fused",), what="general")
+    assert res["status"]["path"] == 2
+
+
+def test_globally_shuffled_input(tpx3):
+    # shots interleaved in the stream: not shot-contiguous, the general path (global sort) must run
+    w = gen.generate(2, shots=500)
+    rng = np.random.default_rng(7)
+    p = rng.permutation(w.n)
+    res, _ = check(tpx3, w.x[p], w.y[p], w.toa[p], w.tot[p], what="shuffled")
+    assert res["status"]["path"] == 2
+
+
+def test_single_shot_P0(tpx3):
+    # P = 0: the whole input is one shot (links may cross the 640000-tick boundaries)
+    w = gen.generate(1, shots=400)
+    check(tpx3, w.x, w.y, w.toa, w.tot, P=0, what="P=0")
+
+
+def test_dense_single_shot_chain(tpx3):
+    # one shot far larger than any tile, dense in time: long chains across slabs
+    rng = np.random.default_rng(11)
+    n = 300000
+    x = rng.integers(0, 256, n); y = rng.integers(0, 256, n)
+    toa = np.sort(rng.integers(0, 600000, n)).astype(np.uint64) + 5 * P
+    tot = rng.integers(1, 1024, n)
+    check(tpx3, x, y, toa, tot, what="dense shot")
+    check(tpx3, x, y, toa, tot, W=3, what="dense shot W=3")
+
+
+# ------------------------------------------------------------------ edge cases
+def test_empty_and_single(tpx3):
+    z16 = np.zeros(0, dtype=np.uint16); z64 = np.zeros(0, dtype=np.uint64)
+    for mode in ("fused", "split"):
+        r = run_gpu(tpx3, z16, z16, z64, z16, mode=mode)
+        assert r["n_clusters"] == 0 and r["status"]["error"] == 0
+    check(tpx3, [7], [9], [123456789], [55], what="single")
+
+
+def test_all_identical(tpx3):
+    n = 5000
+    check(tpx3, np.full(n, 100), np.full(n, 17), np.full(n, 10**9), np.full(n, 3), what="identical")
+
+
+def test_window_inclusive_and_shot_boundary(tpx3):
+    # dt == W links, dt == W+1 does not ("<="); sP-1 | sP never link (R6)
+    x = [10, 11, 50, 51, 90, 91]; y = [10, 10, 50, 50, 90, 90]
+    toa = [1000, 1000 + W, 5000, 5000 + W + 1, 3 * P - 1, 3 * P]
+    res, o = check(tpx3, x, y, toa, [5, 6, 7, 8, 9, 10], what="window")
+    assert res["n_clusters"] == 5
+
+
+def test_chain_longer_than_window(tpx3):
+    # A-B-C with |tA - tC| > W: one component by transitivity
+    n = 4000
+    x = (np.arange(n) % 200) + 20; y = np.full(n, 100) + (np.arange(n) // 200 % 2)
+    toa = 7 * P + np.arange(n) * 100
+    res, o = check(tpx3, x, y, toa, np.full(n, 9), what="chain")
+
+
+def test_corners_and_repeated_addresses(tpx3):
+    x = [0, 0, 255, 255, 0, 255, 128, 128, 128]; y = [0, 0, 255, 255, 255, 0, 128, 128, 128]
+    toa = [10, 20, 30, 40, 50, 60, 70, 70 + W, 70 + 2 * W]
+    check(tpx3, x, y, toa, [1, 2, 3, 4, 5, 6, 7, 8, 9], what="corners")
+
+
+def test_tie_break_later_pixel_wins(tpx3):
+    res, o = check(tpx3, [10, 11, 12], [5, 5, 5], [100, 100, 100], [7, 9, 9], what="tie")
+    assert res["c_toa_peak"].tolist() == [100]
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_random_small(tpx3, seed):
+    rng = np.random.default_rng(100 + seed)
+    n = int(rng.integers(2, 3000))
+    side = int(rng.integers(4, 40))
+    x = rng.integers(0, side, n); y = rng.integers(0, side, n)
+    toa = rng.integers(0, 4 * P, n).astype(np.uint64)
+    tot = rng.integers(1, 1024, n)
+    Wr = int(rng.choice([0, 1, 320, 5000, 700000]))
+    Pr = int(rng.choice([0, P, 1000]))
+    check(tpx3, x, y, toa, tot, W=Wr, P=Pr, what="random %d" % seed)
+
+
+def test_large_values(tpx3):
+    # ToT up to 65535, ToA near 2^63: integer sums stay exact
+    rng = np.random.default_rng(5)
+    n = 20000
+    x = rng.integers(250, 256, n); y = rng.integers(250, 256, n)
+    toa = (np.uint64(1) << np.uint64(62)) + rng.integers(0, 10 * P, n).astype(np.uint64)
+    tot = rng.integers(60000, 65536, n)
+    check(tpx3, x, y, toa, tot, what="large values")
+
+
+def test_centroid_accepts_oracle_labels(tpx3):
+    # tpx3_centroid is defined on ANY valid (perm, label): feed it the oracle's
+    import torch
+
+    w = gen.generate(2, shots=300)
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P)
+    pl = tpx3.plan(tpx3.Config(max_hits=w.n))
+    cl = tpx3.Clusters(w.n, pl.device)
+    nc = pl.centroid(to_dev(w.x), to_dev(w.y), to_dev(w.toa), to_dev(w.tot), to_dev(o["perm"]), to_dev(o["label"]), cl)
+    torch.cuda.synchronize()
+    ncl = int(nc.cpu().numpy()[0])
+    g = {"perm": o["perm"], "label": o["label"], "n_clusters": ncl}
+    g.update(cl.numpy(ncl))
+    assert_parity(g, o, "oracle labels")
+
+
+# ------------------------------------------------------------------ error behaviour
+def test_capacity_error(tpx3):
+    w = gen.generate(0, shots=50)
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P)
+    for mode in ("fused", "split"):
+        r = run_gpu(tpx3, w.x, w.y, w.toa, w.tot, mode=mode, max_clusters=10)
+        assert r["status"]["error"] == tpx3.ERR_CAPACITY
+        assert r["n_clusters"] == o["n_clusters"]  # the true count is still reported
+        np.testing.assert_array_equal(r["c_sum_tot"], o["c_sum_tot"][:10])
+
+
+def test_validate_input(tpx3):
+    r = run_gpu(tpx3, [1, 2, 300], [1, 2, 3], [10, 20, 30], [5, 5, 5], flags=tpx3.FLAG_VALIDATE_INPUT)
+    assert r["status"]["error"] == tpx3.ERR_OUT_OF_RANGE
+    r = run_gpu(tpx3, [1, 2, 3], [1, 2, 3], [10, 20, 30], [5, 0, 5], flags=tpx3.FLAG_VALIDATE_INPUT)
+    assert r["status"]["error"] == tpx3.ERR_OUT_OF_RANGE
+    r = run_gpu(tpx3, [1, 2, 3], [1, 2, 3], [10, 20, 30], [5, 5, 5], flags=tpx3.FLAG_VALIDATE_INPUT)
+    assert r["status"]["error"] == 0
+
+
+def test_invalid_args(tpx3):
+    with pytest.raises(tpx3.Tpx3Error):
+        tpx3.plan(tpx3.Config(sensor_w=0))
+    with pytest.raises(tpx3.Tpx3Error):
+        tpx3.plan(tpx3.Config(max_hits=(1 << 28) + 1))
+    pl = tpx3.plan(tpx3.Config(max_hits=16))
+    with pytest.raises(tpx3.Tpx3Error):
+        w = gen.generate(0, shots=5)
+        pl.cluster(to_dev(w.x), to_dev(w.y), to_dev(w.toa), to_dev(w.tot))
+
+
+def test_process_host_end_to_end(tpx3):
+    import torch
+
+    w = gen.generate(1, shots=500)
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P)
+    pl = tpx3.plan(tpx3.Config(max_hits=w.n))
+    hx, hy, htoa, htot = (torch.from_numpy(a).pin_memory() for a in (w.x, w.y, w.toa, w.tot))
+    cl = tpx3.Clusters(w.n, "cpu", pin=True)
+    perm = torch.empty(w.n, dtype=torch.uint32).pin_memory()
+    label = torch.empty(w.n, dtype=torch.uint32).pin_memory()
+    ncl = pl.process_host(hx, hy, htoa, htot, cl, perm, label)
+    g = {"perm": perm.numpy(), "label": label.numpy(), "n_clusters": ncl}
+    g.update(cl.numpy(ncl))
+    assert_parity(g, o, "process_host")
