@@ -114,7 +114,8 @@ def test_globally_shuffled_input(tpx3):
     w = gen.generate(2, shots=500)
     rng = np.random.default_rng(7)
     p = rng.permutation(w.n)
-    res, _ = check(tpx3, w.x[p], w.y[p], w.toa[p], w.tot[p], what="shuffled")
+    check(tpx3, w.x[p], w.y[p], w.toa[p], w.tot[p], modes=("split",), what="shuffled")
+    res, _ = check(tpx3, w.x[p], w.y[p], w.toa[p], w.tot[p], modes=("fused",), what="shuffled")
     assert res["status"]["path"] == 2
 
 
