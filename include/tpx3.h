@@ -135,6 +135,25 @@ int tpx3_status(tpx3_plan_t plan, const void* workspace, void* cuda_stream, tpx3
 /* Number of kernels the library has launched through this plan (for launch accounting). */
 uint64_t tpx3_launch_count(tpx3_plan_t plan);
 
+/* Optional per-stage device timing. While enabled, every call brackets each stage it enqueues
+ * with a pair of CUDA events recorded on the call's stream (no synchronisation at call time).
+ * tpx3_profile_read waits for the recorded events, writes the summed durations since the last
+ * read to *out [host] and recycles the events. Stages: */
+enum {
+  TPX3_STAGE_FUSED = 0,    /* the fused shot-tile kernel (S0-S5)                                */
+  TPX3_STAGE_SORT = 1,     /* general path: min/max, radix passes                               */
+  TPX3_STAGE_LINK = 2,     /* general path: gather, hash insert, link, compress                 */
+  TPX3_STAGE_CENTROID = 3, /* general path / tpx3_centroid: root ordinals, sums, divide         */
+  TPX3_STAGE_COUNT = 4
+};
+typedef struct {
+  double ms[TPX3_STAGE_COUNT];         /* summed device time of the stage, milliseconds        */
+  uint64_t launches[TPX3_STAGE_COUNT]; /* kernels launched inside the stage                     */
+  uint64_t calls;                      /* API calls profiled                                    */
+} tpx3_profile_t;
+int tpx3_profile_enable(tpx3_plan_t plan, int enable);
+int tpx3_profile_read(tpx3_plan_t plan, tpx3_profile_t* out);
+
 int tpx3_free(tpx3_plan_t plan);
 const char* tpx3_strerror(int err);
 

@@ -28,8 +28,10 @@ OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_OUT_OF_RANGE, ERR_CUDA, ERR_UNIMPLEMENTED
 # Every symbol include/tpx3.h declares (tests check the built library exports all of them).
 exported_symbols = (
     "tpx3_plan", "tpx3_cluster", "tpx3_centroid", "tpx3_cluster_centroid", "tpx3_host_io_bytes",
-    "tpx3_process_host", "tpx3_status", "tpx3_launch_count", "tpx3_free", "tpx3_strerror",
+    "tpx3_process_host", "tpx3_status", "tpx3_launch_count", "tpx3_profile_enable", "tpx3_profile_read",
+    "tpx3_free", "tpx3_strerror",
 )
+STAGES = ("fused", "sort", "link", "centroid")
 
 
 class Tpx3Error(RuntimeError):
@@ -54,6 +56,10 @@ class _CClusters(ctypes.Structure):
 class _CStatus(ctypes.Structure):
     _fields_ = [("error", ctypes.c_uint32), ("path", ctypes.c_uint32), ("n_clusters", ctypes.c_uint32),
                 ("sort_passes", ctypes.c_uint32), ("n", ctypes.c_uint64)]
+
+
+class _CProfile(ctypes.Structure):
+    _fields_ = [("ms", ctypes.c_double * 4), ("launches", ctypes.c_uint64 * 4), ("calls", ctypes.c_uint64)]
 
 
 _lib = None
@@ -85,6 +91,10 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.tpx3_status.argtypes = [vp, vp, vp, ctypes.POINTER(_CStatus)]
     lib.tpx3_launch_count.restype = ctypes.c_uint64
     lib.tpx3_launch_count.argtypes = [vp]
+    lib.tpx3_profile_enable.restype = ctypes.c_int
+    lib.tpx3_profile_enable.argtypes = [vp, ctypes.c_int]
+    lib.tpx3_profile_read.restype = ctypes.c_int
+    lib.tpx3_profile_read.argtypes = [vp, ctypes.POINTER(_CProfile)]
     lib.tpx3_free.restype = ctypes.c_int
     lib.tpx3_free.argtypes = [vp]
     lib.tpx3_strerror.restype = ctypes.c_char_p
@@ -261,6 +271,20 @@ class Plan:
 
     def launch_count(self) -> int:
         return int(self.lib.tpx3_launch_count(self.handle))
+
+    def profile_enable(self, enable: bool = True):
+        rc = self.lib.tpx3_profile_enable(self.handle, int(bool(enable)))
+        if rc != OK:
+            raise Tpx3Error(rc, "tpx3_profile_enable")
+
+    def profile_read(self) -> dict:
+        """Summed per-stage device time (ms) and kernel launches since the last read."""
+        pr = _CProfile()
+        rc = self.lib.tpx3_profile_read(self.handle, ctypes.byref(pr))
+        if rc != OK:
+            raise Tpx3Error(rc, "tpx3_profile_read")
+        return {"calls": int(pr.calls), "ms": {k: float(pr.ms[i]) for i, k in enumerate(STAGES)},
+                "launches": {k: int(pr.launches[i]) for i, k in enumerate(STAGES)}}
 
     def free(self):
         if self.handle:

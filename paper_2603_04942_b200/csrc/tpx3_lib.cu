@@ -4,6 +4,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "tpx3_centroid.cuh"
 #include "tpx3_common.cuh"
@@ -23,6 +24,12 @@ struct tpx3_plan_s {
   size_t off_keyA, off_keyB, off_idxA, off_idxB, off_xy, off_tot, off_slab, off_table, off_counts;
   size_t off_slot, off_peak, off_blkcnt, off_tiles;
   uint32_t table_mask_max;
+  // optional per-stage timing (tpx3_profile_*)
+  bool profiling;
+  struct Span { int stage; cudaEvent_t a, b; uint64_t launches0, launches1; };
+  std::vector<Span> spans;
+  std::vector<cudaEvent_t> free_events;
+  uint64_t profiled_calls;
 };
 
 namespace {
@@ -49,6 +56,33 @@ inline uint32_t grid_for(uint64_t n, int threads, int num_sms, int per_sm = 8) {
   if (b > cap) b = cap;
   return (uint32_t)(b ? b : 1);
 }
+
+// RAII bracket of one stage: records an event pair on the stream when profiling is enabled.
+struct StageTimer {
+  tpx3_plan_s* p;
+  cudaStream_t st;
+  size_t slot;
+  bool on;
+  static cudaEvent_t take(tpx3_plan_s* p) {
+    cudaEvent_t e = nullptr;
+    if (!p->free_events.empty()) { e = p->free_events.back(); p->free_events.pop_back(); return e; }
+    cudaEventCreate(&e);
+    return e;
+  }
+  StageTimer(tpx3_plan_s* plan, cudaStream_t stream, int stage) : p(plan), st(stream), slot(0), on(plan->profiling) {
+    if (!on) return;
+    tpx3_plan_s::Span s;
+    s.stage = stage; s.a = take(p); s.b = take(p); s.launches0 = p->launches; s.launches1 = p->launches;
+    cudaEventRecord(s.a, st);
+    slot = p->spans.size();
+    p->spans.push_back(s);
+  }
+  ~StageTimer() {
+    if (!on) return;
+    cudaEventRecord(p->spans[slot].b, st);
+    p->spans[slot].launches1 = p->launches;
+  }
+};
 
 struct Ws {
   Ctrl* ctrl;
@@ -86,10 +120,12 @@ int enqueue_general_cluster(tpx3_plan_s* p, const Ws& w, cudaStream_t st, uint64
   Params prm = p->prm;
   prm.n = n;
   const int sms = p->num_sms;
+  SortBufs b;
+  SortGeom g = sort_geom(n);
+  {
+  StageTimer timer(p, st, TPX3_STAGE_SORT);
   TPX3_LAUNCH(p, k_minmax, grid_for(n, 256 * 8, sms), 256, 0, st, w.ctrl, toa, n);
   TPX3_LAUNCH(p, k_sort_setup, 1, 1, 0, st, w.ctrl);
-  SortGeom g = sort_geom(n);
-  SortBufs b;
   b.key[0] = w.keyA; b.key[1] = w.keyB; b.idx[0] = w.idxA; b.idx[1] = w.idxB; b.counts = w.counts;
   // Passes needed for the largest span a ToA can have; the ones past the device-computed
   // `npass` return at once. 64-bit ToA => at most 8 passes.
@@ -98,6 +134,8 @@ int enqueue_general_cluster(tpx3_plan_s* p, const Ws& w, cudaStream_t st, uint64
     TPX3_LAUNCH(p, k_radix_scan, 1, 1024, 0, st, w.ctrl, pass, w.counts, (uint32_t)(kRadix * g.nblk));
     TPX3_LAUNCH(p, k_radix_scatter, g.nblk, kSortThreads, 0, st, w.ctrl, pass, toa, b, perm, n, g);
   }
+  }
+  StageTimer timer(p, st, TPX3_STAGE_LINK);
   TPX3_LAUNCH(p, k_gather, grid_for(n, 256, sms), 256, 0, st, w.ctrl, prm, w.keyA, w.keyB, perm, x, y, tot, w.xy,
               w.tot, w.slab, label);
   uint32_t tsize = table_size_for(n);
@@ -118,6 +156,7 @@ int enqueue_centroid(tpx3_plan_s* p, const Ws& w, cudaStream_t st, int general_o
   const int sms = p->num_sms;
   uint32_t nblk = (uint32_t)((n + kCentTile - 1) / kCentTile);
   if (nblk == 0) nblk = 1;
+  StageTimer timer(p, st, TPX3_STAGE_CENTROID);
   TPX3_LAUNCH(p, k_root_count, nblk, kCentThreads, 0, st, w.ctrl, general_only, n, label, w.blkcnt);
   TPX3_LAUNCH(p, k_root_scan, 1, 1024, 0, st, w.ctrl, general_only, w.blkcnt, nblk, max_clusters, n_clusters);
   TPX3_LAUNCH(p, k_root_slots, nblk, kCentThreads, 0, st, w.ctrl, general_only, n, label, w.blkcnt, w.slot,
@@ -150,6 +189,8 @@ int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace
   if (!p) return TPX3_ERR_CUDA;
   p->cfg = *cfg;
   p->launches = 0;
+  p->profiling = false;
+  p->profiled_calls = 0;
   p->num_sms = kNumSMs;
   Params& prm = p->prm;
   prm.n = 0;
@@ -191,6 +232,7 @@ int tpx3_cluster(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, 
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
   Ws w = carve(p, workspace);
+  if (p->profiling) ++p->profiled_calls;
   TPX3_LAUNCH(p, k_ctrl_init, 1, 1, 0, st, w.ctrl, n);
   TPX3_LAUNCH(p, k_fill_u32, 1, 32, 0, st, w.ctrl, 0, n_clusters, (uint64_t)1, 0u);
   if (n == 0) return cuda_ok(cudaGetLastError());
@@ -208,6 +250,7 @@ int tpx3_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n,
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
   Ws w = carve(p, workspace);
+  if (p->profiling) ++p->profiled_calls;
   TPX3_LAUNCH(p, k_ctrl_init, 1, 1, 0, st, w.ctrl, n);
   if (n == 0) {
     TPX3_LAUNCH(p, k_fill_u32, 1, 32, 0, st, w.ctrl, 0, n_clusters, (uint64_t)1, 0u);
@@ -226,6 +269,7 @@ int tpx3_cluster_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uin
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
   Ws w = carve(p, workspace);
+  if (p->profiling) ++p->profiled_calls;
   TPX3_LAUNCH(p, k_ctrl_init, 1, 1, 0, st, w.ctrl, n);
   TPX3_LAUNCH(p, k_fill_u32, 1, 32, 0, st, w.ctrl, 0, n_clusters, (uint64_t)1, 0u);
   if (n == 0) return cuda_ok(cudaGetLastError());
@@ -340,8 +384,36 @@ int tpx3_status(tpx3_plan_t p, const void* workspace, void* cuda_stream, tpx3_st
 
 uint64_t tpx3_launch_count(tpx3_plan_t p) { return p ? p->launches : 0; }
 
+int tpx3_profile_enable(tpx3_plan_t p, int enable) {
+  if (!p) return TPX3_ERR_INVALID_ARG;
+  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  p->profiling = enable != 0;
+  return TPX3_OK;
+}
+
+int tpx3_profile_read(tpx3_plan_t p, tpx3_profile_t* out) {
+  if (!p || !out) return TPX3_ERR_INVALID_ARG;
+  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  memset(out, 0, sizeof(*out));
+  int rc = TPX3_OK;
+  for (auto& s : p->spans) {
+    float ms = 0.f;
+    if (cudaEventSynchronize(s.b) != cudaSuccess || cudaEventElapsedTime(&ms, s.a, s.b) != cudaSuccess) rc = TPX3_ERR_CUDA;
+    out->ms[s.stage] += ms;
+    out->launches[s.stage] += s.launches1 - s.launches0;
+    p->free_events.push_back(s.a);
+    p->free_events.push_back(s.b);
+  }
+  p->spans.clear();
+  out->calls = p->profiled_calls;
+  p->profiled_calls = 0;
+  return rc;
+}
+
 int tpx3_free(tpx3_plan_t p) {
   if (!p) return TPX3_ERR_INVALID_ARG;
+  for (auto& s : p->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
+  for (auto e : p->free_events) cudaEventDestroy(e);
   delete p;
   return TPX3_OK;
 }
