@@ -1,0 +1,404 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the TimePix3 cluster + centroid hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg1]
+
+One "step" = one pass of the whole hot path (S0-S5: shot/key, stable sort, neighbour link, label
+compression, segmented reduction, centroid — tpx3_cluster_centroid) over the whole synthetic
+workload. Default workload: BASELINE.json configs[1] (electron VMI at 1 kHz, 100 000 shots x 30
+electrons, about 3.6e7 pixel hits, 0.5 GB of input: larger than the 126 MB L2, so no explicit L2
+flush is needed between steps). Metric: pixel hits/s clustered + centroided, device-timed.
+
+Multi-GPU (torchrun, one rank per GPU): shots are independent units, so every rank processes its
+own contiguous range of `shots` shots (rank r: shots [r*S, (r+1)*S)) with no data-path
+collective; "scaling": "weak". torch.distributed is used for the barrier and the max-over-ranks
+timing only.
+
+Rank 0 prints ONE JSON line. `--impl reference` times the CPU oracle (oracle/) on a bounded
+sample of the same workload on the host cores; it is a deliberately plain program,
+a reported baseline and not the optimisation target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "pixel hits/sec clustered+centroided (device-timed, 1 B200); % of HBM peak"
+UNIT = "pixel hits/s"
+WORKLOADS = {  # name -> (generator config id, default shots)   [BASELINE.json configs]
+    "cfg0": (0, 1000), "cfg1": (1, 100000), "cfg2": (2, 200000), "cfg3": (3, 50000),
+    "cfg4_1M": (4, None), "cfg4_16M": (4, None), "cfg4_64M": (4, None), "cfg4_256M": (4, None),
+}
+CFG4_CHUNK = {"cfg4_1M": 1 << 20, "cfg4_16M": 1 << 24, "cfg4_64M": 1 << 26, "cfg4_256M": 1 << 28}
+FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def make_workload(name: str, shots: int | None, rank: int):
+    """Seeded synthetic input of the named BASELINE.json config (recipe: DESIGN.md 'Input recipe')."""
+    import gen
+
+    cfg_id, dflt = WORKLOADS[name]
+    if cfg_id == 4:
+        chunk = CFG4_CHUNK[name]
+        # one shot-aligned chunk of config 4 (about 900 hits/shot): generate a little more than
+        # needed and trim to the largest whole-shot prefix <= chunk hits
+        s = shots if shots is not None else int(chunk / 850) + 64
+        return gen.generate(4, shots=s, shot_begin=rank * s, max_hits=chunk)
+    s = shots if shots is not None else dflt
+    return gen.generate(cfg_id, shots=s, shot_begin=rank * s)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self, t0: float, t1: float) -> dict:
+        sm, smax, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        rows = [r for t, r in self.rows if t0 - 0.05 <= t <= t1 + 0.15] or [r for _, r in self.rows[-3:]]
+        for r in rows:
+            f = [c.strip() for c in r.split(",")]
+            try:
+                sm.append(float(f[0]))
+                smax.append(float(f[1]))
+            except Exception:
+                continue
+            for nme, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def host_threads() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def time_oracle(w, shots: int, threads: int = 0):
+    """Oracle (sort + per-shot BFS + sums + centroid) on the first `shots` shots; returns (seconds, hits, clusters)."""
+    import oracle
+
+    s = w.slice_shots(0, min(shots, w.shots))
+    t0 = time.perf_counter()
+    o = oracle.run(s.x, s.y, s.toa, s.tot, w.toa_window_ticks, w.shot_period_ticks, threads=threads)
+    return time.perf_counter() - t0, s.n, o["n_clusters"]
+
+
+def sized_oracle_sample(w, target_s: float):
+    """Pick a whole-shot prefix of the workload that takes about target_s seconds of oracle time."""
+    probe = max(1, min(w.shots, 2000))
+    dt, hits, _ = time_oracle(w, probe)
+    rate = hits / max(dt, 1e-6)
+    per_shot = max(w.n / max(w.shots, 1), 1.0)
+    shots = int(max(1, min(w.shots, rate * target_s / per_shot)))
+    return shots
+
+
+def cpu_baseline(w, target_s: float = 12.0) -> dict:
+    shots = sized_oracle_sample(w, target_s)
+    dt, hits, ncl = time_oracle(w, shots)
+    return {"value": hits / dt, "unit": UNIT, "cores": host_threads(), "kind": "oracle",
+            "sample": "first %d shots of %s (%d pixel hits, %d particle hits), %.2f s, OpenMP over shots; "
+                      "sort is single-threaded" % (shots, w.name, hits, ncl, dt),
+            "particle_hits_per_s": ncl / dt}
+
+
+def run_reference(args):
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return 0
+    cfg_id, dflt = WORKLOADS[args.workload]
+    # the oracle only ever sees a bounded sample: do not generate more shots than it can use
+    cap = args.shots if args.shots is not None else (min(dflt, 20000) if dflt else 20000)
+    w = make_workload(args.workload, cap, 0)
+    per_step = max(0.5, min(5.0, 120.0 / max(args.steps + args.warmup, 1)))
+    shots = sized_oracle_sample(w, per_step)
+    for _ in range(args.warmup):
+        time_oracle(w, shots)
+    t_total, hits, ncl = 0.0, 0, 0
+    for _ in range(args.steps):
+        dt, hits, ncl = time_oracle(w, shots)
+        t_total += dt
+    ms = 1e3 * t_total / max(args.steps, 1)
+    val = hits / (ms * 1e-3)
+    sample = "first %d shots of %s per step (%d pixel hits, %d particle hits)" % (shots, w.name, hits, ncl)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+        "config": {"workload": w.name, "shots": w.shots, "pixel_hits": w.n, "sample": sample,
+                   "what": "CPU oracle (oracle/tpx3_oracle.cpp) on host cores; no GPU work"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": host_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# Algorithmic bytes: what the method must move once, per pixel hit and
+# per particle hit. Inputs 14 B/hit (x, y, tot u16 + toa u64), outputs perm + label 8 B/hit,
+# cluster row 52 B (label, size, shot u32; three i64 sums; toa_peak u64; cx, cy f32).
+BYTES_PER_HIT_IN = 14
+BYTES_PER_HIT_OUT = 8
+BYTES_PER_CLUSTER = 52
+STAGE_BYTES = {  # per stage of the general path: single-touch floor of that stage
+    "fused": lambda n, c: (BYTES_PER_HIT_IN + BYTES_PER_HIT_OUT) * n + BYTES_PER_CLUSTER * c,
+    "sort": lambda n, c: (8 + 4) * n,                      # read toa, write perm
+    "link": lambda n, c: (4 + 6 + 8 + 4) * n,              # perm, x/y/tot gather, toa, label
+    "centroid": lambda n, c: (4 + 4 + 6) * n + BYTES_PER_CLUSTER * c,
+}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2603_04942_b200 as m
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    m.load_library()  # fails loudly if libtpx3.so cannot be built / loaded
+
+    w = make_workload(args.workload, args.shots, rank)
+    n = w.n
+    cfg = m.Config(max_hits=max(n, 1), toa_window_ticks=w.toa_window_ticks, shot_period_ticks=w.shot_period_ticks,
+                   device=local, flags=(m.FLAG_FORCE_GENERAL if args.force_general else 0))
+    pl = m.plan(cfg)
+    stream = torch.cuda.Stream(device=local)
+    max_clusters = max(n // 2, 1024)  # hits have >= 3 pixels in every config; capacity errors are reported
+    host = [torch.from_numpy(a).pin_memory() for a in (w.x, w.y, w.toa, w.tot)]
+    dev = [t.to("cuda", non_blocking=True) for t in host]
+    cl = m.Clusters(max_clusters, pl.device)
+    perm = torch.empty(max(n, 1), dtype=torch.uint32, device=pl.device)
+    label = torch.empty(max(n, 1), dtype=torch.uint32, device=pl.device)
+    nc = torch.zeros(1, dtype=torch.uint32, device=pl.device)
+    torch.cuda.synchronize()
+
+    def step():
+        pl.cluster_centroid(*dev, cl, perm=perm, label=label, n_clusters=nc, stream=stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    barrier()
+    st = pl.status(stream)
+    if st["error"]:
+        raise RuntimeError("device status error %d (%s)" % (st["error"], m.strerror(st["error"])))
+    ncl = st["n_clusters"]
+
+    # ---- timed region: K steps, device-timed with CUDA events on the launching stream ----------
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    pl.profile_enable(True)
+    pl.profile_read()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = pl.launch_count()
+    barrier()
+    t_wall0 = time.time()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    barrier()
+    t_wall1 = time.time()
+    launches = pl.launch_count() - l0
+    ms_total = ev0.elapsed_time(ev1)
+    prof = pl.profile_read()
+    pl.profile_enable(False)
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+        tot = torch.tensor([n, ncl], dtype=torch.int64, device="cuda")
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+        n_all, ncl_all = int(tot[0].item()), int(tot[1].item())
+    else:
+        n_all, ncl_all = n, ncl
+    ms_step = ms_total / max(args.steps, 1)
+    value = n_all / (ms_step * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers (tpx3_process_host) --------------------
+    clh = m.Clusters(max_clusters, "cpu", pin=True)
+    for _ in range(2):
+        pl.process_host(*host, clh, stream=stream)
+    barrier()
+    e2e_steps = max(1, min(args.steps, 5))
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        ncl_e2e = pl.process_host(*host, clh, stream=stream)  # synchronises the stream itself
+    torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    assert ncl_e2e == ncl, (ncl_e2e, ncl)
+    if rank == 0:
+        sampler.stop()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant stage (CUDA-event time per stage, recorded on `stream`) ------
+    peak, peak_src = measured_peak()
+    stage_ms = {k: v / max(prof["calls"], 1) for k, v in prof["ms"].items()}
+    dom = max(stage_ms, key=lambda k: stage_ms[k])
+    dom_bytes = STAGE_BYTES[dom](n, ncl)
+    dom_gbs = dom_bytes / (stage_ms[dom] * 1e-3) / 1e9 if stage_ms[dom] > 0 else 0.0
+    whole_bytes = STAGE_BYTES["fused"](n, ncl)
+    roofline = {
+        "bound": "hbm", "kernel": {"fused": "k_fused_shot_tiles", "sort": "general path: radix sort stage",
+                                   "link": "general path: gather + hash link + compress stage",
+                                   "centroid": "centroid stage"}[dom],
+        "achieved": dom_gbs, "peak": peak, "unit": "GB/s", "frac": dom_gbs / peak, "traffic": None,
+        "peak_source": peak_src, "algorithmic_bytes_per_launch": dom_bytes,
+        "stage_ms": stage_ms, "stage_launches": {k: v / max(prof["calls"], 1) for k, v in prof["launches"].items()},
+        "whole_path": {"algorithmic_bytes_per_step": whole_bytes,
+                       "achieved": whole_bytes / (ms_step * 1e-3) / 1e9 * (n_all / max(n, 1)) / max(world, 1),
+                       "frac": whole_bytes / (ms_step * 1e-3) / 1e9 / peak},
+    }
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")  # ncu --set full dram bytes, per launch
+    try:
+        with open(traffic_file) as f:
+            tr = json.load(f)
+        key = "%s:%s" % (w.name, dom)
+        if key in tr:
+            roofline["traffic"] = tr[key]["dram_bytes_per_launch"]
+            roofline["traffic_source"] = tr[key].get("source")
+    except Exception:
+        pass
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(w, args.cpu_seconds)
+
+    h2d = BYTES_PER_HIT_IN * n
+    d2h = 4 + BYTES_PER_CLUSTER * ncl
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int64", "data": "synthetic",
+        "config": {
+            "workload": w.name, "shots_per_gpu": w.shots, "pixel_hits_per_gpu": n, "particle_hits_per_gpu": ncl,
+            "pixel_hits_total": n_all, "particle_hits_total": ncl_all, "toa_window_ticks": w.toa_window_ticks,
+            "shot_period_ticks": w.shot_period_ticks, "path": {1: "fused", 2: "general"}.get(st["path"], st["path"]),
+            "sort_passes": st["sort_passes"], "parallelism": "shots sharded over %d gpu(s), no collective" % world,
+            "l2": "inputs (%.0f MB) larger than the 126 MB L2; no flush between steps" % (14 * n / 1e6)
+                  if 14 * n > 2 * 126e6 else "inputs fit L2 (%.0f MB): DRAM traffic is not exercised" % (14 * n / 1e6),
+            "input_hash": {"toa": __import__("gen").array_hash(w.toa), "x": __import__("gen").array_hash(w.x)},
+        },
+        "particle_hits_per_s": ncl_all / (ms_step * 1e-3),
+        "e2e": {"value": n_all / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": e2e_s * 1e3, "api": "tpx3_process_host (pinned host buffers; cluster table copied "
+                "back, perm/label left on the device)"},
+        "gpu_launches": launches,
+        "roofline": roofline,
+        "clocks": sampler.summary(t_wall0, time.time()),
+        "context": "paper: ~25x faster than acquisition at 1 kHz, ~10 particles/shot, PyTorch on a Titan RTX "
+                   "(PAPER.md:179) ~ 2.5e5 particle hits/s; other hardware, context only",
+    }
+    if cpu is not None:
+        line["cpu_baseline"] = cpu
+    print(json.dumps(line), flush=True)
+    pl.free()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
+    ap.add_argument("--workload", choices=sorted(WORKLOADS), default="cfg1")
+    ap.add_argument("--shots", type=int, default=None, help="override the number of shots (testing only)")
+    ap.add_argument("--force-general", action="store_true", help="never take the fused shot-tile path")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        print("note: timing rules ask for >= 3 warm-up steps", file=sys.stderr)
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
