@@ -231,7 +231,9 @@ def run_ours(args):
     w = make_workload(args.workload, args.shots, rank)
     n = w.n
     cfg = m.Config(max_hits=max(n, 1), toa_window_ticks=w.toa_window_ticks, shot_period_ticks=w.shot_period_ticks,
-                   device=local, flags=(m.FLAG_FORCE_GENERAL if args.force_general else 0))
+                   device=local, flags=(m.FLAG_FORCE_GENERAL if args.force_general else 0),
+                   max_shot_hits=(args.max_shot_hits if args.max_shot_hits is not None
+                                  else __import__("gen").max_shot_hits(w.cfg_id)))
     pl = m.plan(cfg)
     stream = torch.cuda.Stream(device=local)
     max_clusters = max(n // 2, 1024)  # hits have >= 3 pixels in every config; capacity errors are reported
@@ -359,7 +361,7 @@ def run_ours(args):
             "workload": w.name, "shots_per_gpu": w.shots, "pixel_hits_per_gpu": n, "particle_hits_per_gpu": ncl,
             "pixel_hits_total": n_all, "particle_hits_total": ncl_all, "toa_window_ticks": w.toa_window_ticks,
             "shot_period_ticks": w.shot_period_ticks, "path": {1: "fused", 2: "general"}.get(st["path"], st["path"]),
-            "sort_passes": st["sort_passes"], "parallelism": "shots sharded over %d gpu(s), no collective" % world,
+            "sort_passes": st["sort_passes"], "max_shot_hits": cfg.max_shot_hits, "parallelism": "shots sharded over %d gpu(s), no collective" % world,
             "l2": "inputs (%.0f MB) larger than the 126 MB L2; no flush between steps" % (14 * n / 1e6)
                   if 14 * n > 2 * 126e6 else "inputs fit L2 (%.0f MB): DRAM traffic is not exercised" % (14 * n / 1e6),
             "input_hash": {"toa": __import__("gen").array_hash(w.toa), "x": __import__("gen").array_hash(w.x)},
@@ -392,6 +394,8 @@ def main():
     ap.add_argument("--workload", choices=sorted(WORKLOADS), default="cfg1")
     ap.add_argument("--shots", type=int, default=None, help="override the number of shots (testing only)")
     ap.add_argument("--force-general", action="store_true", help="never take the fused shot-tile path")
+    ap.add_argument("--max-shot-hits", type=int, default=None,
+                    help="tile-size hint for the plan (default: the workload recipe's bound on hits per shot)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     args = ap.parse_args()

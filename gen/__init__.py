@@ -132,6 +132,16 @@ def particles_per_shot(cfg_id: int) -> int:
     return int(_load().tpx3gen_particles_per_shot(cfg_id))
 
 
+_KMAX = {0: 12, 1: 20, 2: 30, 3: 16, 4: 30, 5: 12}
+
+
+def max_shot_hits(cfg_id: int) -> int:
+    """Upper bound on the pixel hits one shot of a config can hold (particles x largest footprint,
+    + 5 % noise hits in config 3): a fact of the recipe, used as the library's tile-size hint."""
+    h = particles_per_shot(cfg_id) * _KMAX[cfg_id]
+    return h + h // 20 if cfg_id == 3 else h
+
+
 def generate(cfg_id: int, shots: int | None = None, seed: int | None = None, shot_begin: int = 0,
              truth: bool = False, threads: int = 0, max_hits: int | None = None) -> Workload:
     """Generate ``shots`` shots of config ``cfg_id`` starting at shot ``shot_begin``.

@@ -65,6 +65,11 @@ typedef struct {
   uint64_t max_hits;           /* largest n of any later call; 1 .. 2^28                       */
   int32_t device;              /* CUDA device ordinal                                          */
   uint32_t flags;              /* TPX3_FLAG_*                                                  */
+  uint32_t max_shot_hits;      /* hint: most events one shot can hold; sizes the fused path's
+                                  tiles (0 = 4096). <= 1024: 4096-event tiles, 2 CTAs per SM;
+                                  <= 4096: 8192-event tiles; larger, or a shot that exceeds the
+                                  hint: the general path runs (same results, slower).          */
+  uint32_t reserved;           /* must be 0                                                    */
 } tpx3_config_t;
 
 /* Per-hit (cluster) outputs, structure of arrays, each of capacity max_clusters. [dev] */

@@ -45,6 +45,7 @@ class _CConfig(ctypes.Structure):
         ("struct_size", ctypes.c_uint32), ("sensor_w", ctypes.c_uint16), ("sensor_h", ctypes.c_uint16),
         ("toa_window_ticks", ctypes.c_uint32), ("shot_period_ticks", ctypes.c_uint64),
         ("max_hits", ctypes.c_uint64), ("device", ctypes.c_int32), ("flags", ctypes.c_uint32),
+        ("max_shot_hits", ctypes.c_uint32), ("reserved", ctypes.c_uint32),
     ]
 
 
@@ -116,6 +117,7 @@ class Config:
     max_hits: int = 1 << 20
     device: int = 0
     flags: int = 0
+    max_shot_hits: int = 0  # hint: most events in one shot (0 = 4096); sizes the fused path's tiles
 
 
 _CLUSTER_FIELDS = (
@@ -176,7 +178,7 @@ class Plan:
         self.lib = load_library()
         self.cfg = cfg
         c = _CConfig(ctypes.sizeof(_CConfig), cfg.sensor_w, cfg.sensor_h, cfg.toa_window_ticks,
-                     cfg.shot_period_ticks, cfg.max_hits, cfg.device, cfg.flags)
+                     cfg.shot_period_ticks, cfg.max_hits, cfg.device, cfg.flags, cfg.max_shot_hits, 0)
         h = ctypes.c_void_p()
         ws = ctypes.c_size_t()
         rc = self.lib.tpx3_plan(ctypes.byref(c), ctypes.byref(h), ctypes.byref(ws))

@@ -20,7 +20,9 @@ struct Ctrl {
   uint32_t fused_state;          // 0 = not attempted, 1 = succeeded, 2 = failed (general path must run)
   uint32_t tile_ticket;          // fused path: dynamic tile counter
   uint32_t n_roots;              // scratch root counter
-  uint32_t pad[4];
+  uint32_t tiles_done;           // fused path: tiles finished
+  uint32_t fused_fail;           // fused path: some tile could not be handled
+  uint32_t pad[2];
 };
 static_assert(sizeof(Ctrl) <= 256, "Ctrl must fit the 256-byte workspace header");
 

@@ -24,6 +24,7 @@ struct tpx3_plan_s {
   size_t off_keyA, off_keyB, off_idxA, off_idxB, off_xy, off_tot, off_slab, off_table, off_counts;
   size_t off_slot, off_peak, off_blkcnt, off_tiles;
   uint32_t table_mask_max;
+  FusedGeom fused;          // which fused variant serves this plan (variant 0: none)
   // optional per-stage timing (tpx3_profile_*)
   bool profiling;
   struct Span { int stage; cudaEvent_t a, b; uint64_t launches0, launches1; };
@@ -184,7 +185,7 @@ int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace
     return TPX3_ERR_INVALID_ARG;
   if (cfg->max_hits == 0 || cfg->max_hits > kMaxHits) return TPX3_ERR_INVALID_ARG;
   if (cfg->toa_window_ticks >= (1u << 31)) return TPX3_ERR_INVALID_ARG;
-  if (cfg->device < 0) return TPX3_ERR_INVALID_ARG;
+  if (cfg->device < 0 || cfg->reserved != 0) return TPX3_ERR_INVALID_ARG;
   tpx3_plan_s* p = new (std::nothrow) tpx3_plan_s();
   if (!p) return TPX3_ERR_CUDA;
   p->cfg = *cfg;
@@ -200,6 +201,7 @@ int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace
   prm.sensor_h = cfg->sensor_h;
   prm.flags = cfg->flags;
   prm.slabs_per_shot_p1 = prm.P ? (prm.P + prm.W) / (prm.W + 1ull) + 1ull : 0ull;
+  p->fused = fused_geom(prm.P, prm.W, cfg->max_shot_hits);
   const uint64_t N = cfg->max_hits;
   size_t o = 256;  // Ctrl
   // general-path cluster buffers
@@ -217,7 +219,7 @@ int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace
   p->off_slot = p->off_keyA;                    // 4N <= 8N
   p->off_peak = p->off_keyB;                    // 8N
   p->off_blkcnt = p->off_idxA;                  // 4 * ceil(N/4096) <= 4N
-  p->off_tiles = o; o = align_up(o + 8 * (size_t)(N / 256 + 1024));  // fused path tile status words
+  p->off_tiles = o; o = align_up(o + 8 * (size_t)(N / 1024 + 1024));  // fused path tile status words (S >= 3072)
   p->workspace_bytes = o;
   *workspace_bytes = o;
   *out_plan = p;
@@ -233,8 +235,7 @@ int tpx3_cluster(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, 
   if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
   Ws w = carve(p, workspace);
   if (p->profiling) ++p->profiled_calls;
-  TPX3_LAUNCH(p, k_ctrl_init, 1, 1, 0, st, w.ctrl, n);
-  TPX3_LAUNCH(p, k_fill_u32, 1, 32, 0, st, w.ctrl, 0, n_clusters, (uint64_t)1, 0u);
+  TPX3_LAUNCH(p, k_ctrl_init, 1, 256, 0, st, w.ctrl, n, w.tiles, 0u, n_clusters);
   if (n == 0) return cuda_ok(cudaGetLastError());
   return enqueue_general_cluster(p, w, st, n, x, y, toa, tot, perm, label, n_clusters);
 }
@@ -251,11 +252,8 @@ int tpx3_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n,
   if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
   Ws w = carve(p, workspace);
   if (p->profiling) ++p->profiled_calls;
-  TPX3_LAUNCH(p, k_ctrl_init, 1, 1, 0, st, w.ctrl, n);
-  if (n == 0) {
-    TPX3_LAUNCH(p, k_fill_u32, 1, 32, 0, st, w.ctrl, 0, n_clusters, (uint64_t)1, 0u);
-    return cuda_ok(cudaGetLastError());
-  }
+  TPX3_LAUNCH(p, k_ctrl_init, 1, 256, 0, st, w.ctrl, n, w.tiles, 0u, n_clusters);
+  if (n == 0) return cuda_ok(cudaGetLastError());
   return enqueue_centroid(p, w, st, 0, n, x, y, toa, tot, perm, label, max_clusters, *out, n_clusters);
 }
 
@@ -270,15 +268,19 @@ int tpx3_cluster_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uin
   if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
   Ws w = carve(p, workspace);
   if (p->profiling) ++p->profiled_calls;
-  TPX3_LAUNCH(p, k_ctrl_init, 1, 1, 0, st, w.ctrl, n);
-  TPX3_LAUNCH(p, k_fill_u32, 1, 32, 0, st, w.ctrl, 0, n_clusters, (uint64_t)1, 0u);
+  const bool try_fused = !(p->cfg.flags & TPX3_FLAG_FORCE_GENERAL) && p->fused.variant != 0 && n != 0;
+  const uint32_t num_tiles = try_fused ? (uint32_t)((n + p->fused.S - 1) / p->fused.S) : 0u;
+  TPX3_LAUNCH(p, k_ctrl_init, num_tiles > 256 * 64 ? 64 : (num_tiles + 255) / 256 + 1, 256, 0, st, w.ctrl, n, w.tiles,
+              num_tiles, n_clusters);
   if (n == 0) return cuda_ok(cudaGetLastError());
   Params prm = p->prm;
   prm.n = n;
   int rc = TPX3_OK;
-  if (!(p->cfg.flags & TPX3_FLAG_FORCE_GENERAL)) {
-    rc = enqueue_fused(p->num_sms, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, label, max_clusters,
-                       *out, n_clusters);
+  if (try_fused) {
+    bool launched = false;
+    StageTimer timer(p, st, TPX3_STAGE_FUSED);
+    rc = enqueue_fused(p->fused, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, label, max_clusters,
+                       *out, n_clusters, &launched);
     if (rc != TPX3_OK) return rc;
   }
   // General path: every kernel below returns at once if the fused kernel succeeded.

@@ -36,10 +36,18 @@ inline SortGeom sort_geom(uint64_t n) {
 }
 
 // ---- min / max ToA ------------------------------------------------------------------------
-__global__ void k_ctrl_init(Ctrl* c, uint64_t n) {
-  c->status.error = 0; c->status.path = 0; c->status.n_clusters = 0; c->status.sort_passes = 0;
-  c->status.n = n;
-  c->toa_min = ~0ull; c->toa_max = 0ull; c->npass = 1; c->fused_state = 0; c->tile_ticket = 0; c->n_roots = 0;
+// Also clears the fused path's tile status words and the caller's hit counter.
+__global__ void __launch_bounds__(256) k_ctrl_init(Ctrl* c, uint64_t n, unsigned long long* tiles, uint32_t num_tiles,
+                                                 uint32_t* n_clusters) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) {
+    c->status.error = 0; c->status.path = 0; c->status.n_clusters = 0; c->status.sort_passes = 0;
+    c->status.n = n;
+    c->toa_min = ~0ull; c->toa_max = 0ull; c->npass = 1; c->fused_state = 0; c->tile_ticket = 0; c->n_roots = 0;
+    c->tiles_done = 0; c->fused_fail = 0;
+    if (n_clusters) *n_clusters = 0;
+  }
+  for (uint32_t t = i; t < num_tiles; t += gridDim.x * blockDim.x) tiles[t] = 0ull;
 }
 
 __global__ void __launch_bounds__(256) k_minmax(Ctrl* c, const uint64_t* __restrict__ toa, uint64_t n) {

@@ -44,13 +44,13 @@ def test_plan_validation_host_only():
 
     def mk(**kw):
         d = dict(struct_size=ctypes.sizeof(m._CConfig), sensor_w=256, sensor_h=256, toa_window_ticks=320,
-                 shot_period_ticks=640000, max_hits=1 << 20, device=0, flags=0)
+                 shot_period_ticks=640000, max_hits=1 << 20, device=0, flags=0, max_shot_hits=0, reserved=0)
         d.update(kw)
         return m._CConfig(**d)
 
     assert lib.tpx3_plan(None, ctypes.byref(h), ctypes.byref(ws)) == m.ERR_INVALID_ARG
     for bad in (dict(struct_size=4), dict(sensor_w=0), dict(sensor_h=257), dict(max_hits=0),
-                dict(max_hits=(1 << 28) + 1), dict(toa_window_ticks=1 << 31), dict(device=-1)):
+                dict(max_hits=(1 << 28) + 1), dict(toa_window_ticks=1 << 31), dict(device=-1), dict(reserved=1)):
         c = mk(**bad)
         assert lib.tpx3_plan(ctypes.byref(c), ctypes.byref(h), ctypes.byref(ws)) == m.ERR_INVALID_ARG, bad
     c = mk()

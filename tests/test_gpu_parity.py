@@ -35,13 +35,14 @@ def to_dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
-def run_gpu(m, x, y, toa, tot, W=W, P=P, mode="fused", flags=0, max_clusters=None, sensor=(256, 256)):
+def run_gpu(m, x, y, toa, tot, W=W, P=P, mode="fused", flags=0, max_clusters=None, sensor=(256, 256),
+            max_shot_hits=0):
     """mode: 'fused' = tpx3_cluster_centroid; 'split' = tpx3_cluster then tpx3_centroid."""
     import torch
 
     n = len(x)
     pl = m.plan(m.Config(sensor_w=sensor[0], sensor_h=sensor[1], toa_window_ticks=W, shot_period_ticks=P,
-                         max_hits=max(n, 1), flags=flags))
+                         max_hits=max(n, 1), flags=flags, max_shot_hits=max_shot_hits))
     dx, dy, dtoa, dtot = (to_dev(np.asarray(x, dtype=np.uint16)), to_dev(np.asarray(y, dtype=np.uint16)),
                           to_dev(np.asarray(toa, dtype=np.uint64)), to_dev(np.asarray(tot, dtype=np.uint16)))
     cap = n if max_clusters is None else max_clusters
@@ -73,11 +74,11 @@ def assert_parity(g, o, what=""):
         np.testing.assert_array_equal(g[k], o[k], err_msg=what + " " + k + " (bitwise fp32)")
 
 
-def check(m, x, y, toa, tot, W=W, P=P, modes=("fused", "split"), flags=0, what=""):
+def check(m, x, y, toa, tot, W=W, P=P, modes=("fused", "split"), flags=0, what="", max_shot_hits=0):
     o = oracle.run(x, y, toa, tot, W, P, threads=0)
     res = None
     for mode in modes:
-        res = run_gpu(m, x, y, toa, tot, W, P, mode=mode, flags=flags)
+        res = run_gpu(m, x, y, toa, tot, W, P, mode=mode, flags=flags, max_shot_hits=max_shot_hits)
         assert res["status"]["error"] == 0
         assert_parity(res, o, "%s [%s]" % (what, mode))
     return res, o
@@ -86,14 +87,61 @@ def check(m, x, y, toa, tot, W=W, P=P, modes=("fused", "split"), flags=0, what="
 # ------------------------------------------------------------------ the five configs
 def test_cfg0_full(tpx3):
     w = gen.generate(0)  # ~75k hits, 1000 shots: several tiles and a ragged tail
-    res, o = check(tpx3, w.x, w.y, w.toa, w.tot, what="cfg0")
+    res, o = check(tpx3, w.x, w.y, w.toa, w.tot, modes=("split", "fused"), what="cfg0")
     assert o["n_clusters"] > 9000
+    assert res["status"]["path"] == 1  # the fused shot-tile kernel served the call
 
 
 @pytest.mark.parametrize("cfg,shots", [(1, 3000), (2, 1500), (3, 600), (4, 1500)])
 def test_cfg_subsets(tpx3, cfg, shots):
     w = gen.generate(cfg, shots=shots)
-    check(tpx3, w.x, w.y, w.toa, w.tot, what="cfg%d" % cfg)
+    res, _ = check(tpx3, w.x, w.y, w.toa, w.tot, modes=("split", "fused"), what="cfg%d" % cfg)
+    assert res["status"]["path"] == 1
+
+
+@pytest.mark.parametrize("cfg,shots,hint", [(0, 1000, 256), (1, 3000, 640), (1, 3000, 1024), (2, 1200, 1536),
+                                            (4, 1200, 1536), (4, 1200, 4096)])
+def test_fused_tile_variants(tpx3, cfg, shots, hint):
+    # max_shot_hits picks the tile variant (4096-event tiles for <= 1024, 8192 otherwise) and the slice length
+    w = gen.generate(cfg, shots=shots)
+    res, _ = check(tpx3, w.x, w.y, w.toa, w.tot, modes=("fused",), max_shot_hits=hint, what="cfg%d hint %d" % (cfg, hint))
+    assert res["status"]["path"] == 1
+
+
+def test_fused_falls_back_when_a_shot_exceeds_the_hint(tpx3):
+    w = gen.generate(3, shots=100)  # ~2100 events per shot
+    res, _ = check(tpx3, w.x, w.y, w.toa, w.tot, modes=("fused",), max_shot_hits=512, what="cfg3 hint 512")
+    assert res["status"]["path"] == 2
+
+
+def test_fused_shots_aligned_with_slices(tpx3):
+    # shots of exactly S = 4096 and 2048 events: shot starts fall exactly on slice boundaries
+    rng = np.random.default_rng(3)
+    for per in (4096, 2048, 1):
+        shots = 40 if per > 1 else 9000
+        n = per * shots
+        x = rng.integers(0, 256, n); y = rng.integers(0, 256, n)
+        toa = (np.repeat(np.arange(shots), per) * P + rng.integers(0, 60000, n)).astype(np.uint64)
+        tot = rng.integers(1, 1024, n)
+        res, _ = check(tpx3, x, y, toa, tot, modes=("fused",), what="aligned %d" % per)
+        assert res["status"]["path"] == 1
+
+
+def test_fused_sparse_shot_numbers(tpx3):
+    # empty shots in between and a shot number jump too wide for the 32-bit tile key
+    rng = np.random.default_rng(4)
+    n = 30000
+    shot = np.sort(rng.integers(0, 200, n)) * 37
+    x = rng.integers(0, 64, n); y = rng.integers(0, 64, n)
+    toa = (shot * P + rng.integers(0, 20000, n)).astype(np.uint64)
+    tot = rng.integers(1, 1024, n)
+    res, _ = check(tpx3, x, y, toa, tot, modes=("fused",), what="sparse shots")
+    assert res["status"]["path"] == 1
+    shot2 = shot.astype(np.uint64).copy()
+    shot2[n // 2:] += np.uint64(1 << 40)
+    toa2 = shot2 * np.uint64(P) + (toa % np.uint64(P))
+    res, _ = check(tpx3, x, y, toa2, tot, modes=("fused",), what="shot jump")
+    assert res["status"]["path"] in (1, 2)
 
 
 def test_cfg4_requires_sort(tpx3):
