@@ -463,72 +463,90 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
   const uint16_t* totS = unsorted ? totA : totB + lo;
   unsigned char* freeR = smem + (unsorted ? L::kRegB : L::kRegA);   // 8T bytes no longer needed
 
-  // ---- S2: hash multimap cell -> events, probe own + 4 forward cells, union-find ---------------
-  uint32_t* tab = reinterpret_cast<uint32_t*>(freeR);                 // [HS] (cell << 16 | k), kNone = empty
+  // ---- S2: chained hash cell -> events, probe own + 4 forward cells, union-find -----------------
+  // bucket head and chain links both carry (cell << 16 | event), so a chain is walked without
+  // touching the records; only a cell match reads the candidate's key (same shot, |dToA| <= W).
+  uint32_t* bhead = reinterpret_cast<uint32_t*>(freeR);               // [HS] kNone = empty bucket
+  uint32_t* nextc = reinterpret_cast<uint32_t*>(smem + L::kRegC);     // [T]  next node of the bucket chain
   uint32_t* parent = reinterpret_cast<uint32_t*>(smem + L::kRegD);    // [T]
-  uint32_t* head = reinterpret_cast<uint32_t*>(smem + L::kRegC);      // [T] chain head per root
   {
     uint4 e = make_uint4(kNone, kNone, kNone, kNone);
-    uint4* t4 = reinterpret_cast<uint4*>(tab);
+    uint4* t4 = reinterpret_cast<uint4*>(bhead);
 #pragma unroll
     for (int q = 0; q < (int)(HS / 4 / THREADS); ++q) t4[q * THREADS + tid] = e;
-    for (uint32_t k = tid; k < mm; k += THREADS) { parent[k] = k; head[k] = kNone; }
+    for (uint32_t k = tid; k < mm; k += THREADS) parent[k] = k;
   }
   __syncthreads();
   constexpr uint32_t kHashShift = 32u - (T == 8192 ? 14u : (T == 4096 ? 13u : (T == 2048 ? 12u : 11u)));
   static_assert(T == 8192 || T == 4096 || T == 2048 || T == 1024, "hash shift table");
   for (uint32_t k = tid; k < mm; k += THREADS) {
     const uint32_t cell = xyS[k], loc = keyS[k] >> tof_bits;
-    uint32_t h = ((cell | (loc << 16)) * 0x9E3779B1u) >> kHashShift;
-    const uint32_t word = (cell << 16) | k;
-    for (;;) {
-      if (tab[h] == kNone && atomicCAS(&tab[h], kNone, word) == kNone) break;
-      h = (h + 1u) & (HS - 1u);
-    }
+    const uint32_t h = ((cell | (loc << 16)) * 0x9E3779B1u) >> kHashShift;
+    nextc[k] = atomicExch(&bhead[h], (cell << 16) | k);
   }
   __syncthreads();
-  for (uint32_t k = tid; k < mm; k += THREADS) {
-    const uint32_t cell = xyS[k], key = keyS[k], loc = key >> tof_bits;
+  for (uint32_t k0 = 0; k0 < mm; k0 += THREADS) {   // block-uniform trip count; lanes past mm idle
+    const uint32_t k = k0 + tid;
+    const bool act = k < mm;
+    const uint32_t cell = act ? xyS[k] : 0u, key = act ? keyS[k] : 0u, loc = key >> tof_bits;
     const uint32_t x = cell & 0xFFu, y = cell >> 8;
-    // own cell (earlier events only: each unordered pair once), then E, SW, S, SE (all events)
-#pragma unroll
-    for (int q = 0; q < 5; ++q) {
-      const int dx = (q == 1 || q == 4) ? 1 : (q == 2 ? -1 : 0), dy = (q >= 2) ? 1 : 0;
-      if (dx > 0 && x + 1u >= a.sensor_w) continue;
-      if (dx < 0 && x == 0u) continue;
-      if (dy > 0 && y + 1u >= a.sensor_h) continue;
-      const uint32_t c = (uint32_t)((int)cell + dx + dy * 256);
-      uint32_t h = ((c | (loc << 16)) * 0x9E3779B1u) >> kHashShift;
+    // neighbour cells still to visit: bit q of {own, E, SW, S, SE}; sensor edges removed
+    uint32_t todo = 0;
+    if (act) {
+      const bool xe = x + 1u < a.sensor_w, xw = x > 0u, ys = y + 1u < a.sensor_h;
+      todo = 1u | (xe ? 2u : 0u) | ((xw && ys) ? 4u : 0u) | (ys ? 8u : 0u) | ((xe && ys) ? 16u : 0u);
+    }
+    // one flattened loop over all five chains keeps the lanes of a warp in step; matching
+    // candidates are only recorded here (up to 8, packed 2 per register) and united afterwards
+    uint32_t cand[4] = {0u, 0u, 0u, 0u};
+    uint32_t ncand = 0, cur = kNone, c = 0, q = 0;
+    uint32_t rk = k;   // current guess of k's root
+    auto unite = [&](uint32_t j) {
+      uint32_t ra = rk, rb = j;
       for (;;) {
-        const uint32_t wv = tab[h];
-        if (wv == kNone) break;
-        if ((wv >> 16) == c) {
-          const uint32_t j = wv & 0xFFFFu;
-          if (q != 0 || j < k) {
-            const uint32_t kj = keyS[j];
-            const uint32_t dt = key > kj ? key - kj : kj - key;
-            if ((kj >> tof_bits) == loc && dt <= a.W) {
-              // lock-free union: hook the larger root under the smaller
-              uint32_t ra = k, rb = j;
-              for (;;) {
-                uint32_t p;
-                while ((p = parent[ra]) != ra) { uint32_t g = parent[p]; if (g != p) parent[ra] = g; ra = p; }
-                while ((p = parent[rb]) != rb) { uint32_t g = parent[p]; if (g != p) parent[rb] = g; rb = p; }
-                if (ra == rb) break;
-                if (ra < rb) { uint32_t t = ra; ra = rb; rb = t; }
-                const uint32_t old = atomicMin(&parent[ra], rb);
-                if (old == ra) break;
-                ra = old;
-              }
+        uint32_t p;
+        while ((p = parent[ra]) != ra) { uint32_t g = parent[p]; if (g != p) parent[ra] = g; ra = p; }
+        while ((p = parent[rb]) != rb) { uint32_t g = parent[p]; if (g != p) parent[rb] = g; rb = p; }
+        if (ra == rb) break;
+        if (ra < rb) { uint32_t t = ra; ra = rb; rb = t; }
+        const uint32_t old = atomicMin(&parent[ra], rb);   // hook the larger root under the smaller
+        if (old == ra) { ra = rb; break; }
+        ra = old;
+      }
+      rk = ra;
+    };
+    while (todo != 0u || cur != kNone) {
+      if (cur == kNone) {
+        q = (uint32_t)__ffs(todo) - 1u;
+        todo &= todo - 1u;
+        const uint32_t off = (q == 0u) ? 0u : (q == 1u ? 1u : 253u + q);   // 0, +1, +255, +256, +257
+        c = cell + off;
+        cur = bhead[((c | (loc << 16)) * 0x9E3779B1u) >> kHashShift];
+      } else {
+        const uint32_t j = cur & 0xFFFFu, tag = cur >> 16;
+        cur = nextc[j];
+        if (tag == c && (q != 0u || j < k)) {
+          const uint32_t kj = keyS[j];
+          const uint32_t dt = key > kj ? key - kj : kj - key;
+          if ((kj >> tof_bits) == loc && dt <= a.W) {
+            if (ncand < 8u) {
+              cand[ncand >> 1] |= j << ((ncand & 1u) * 16u);
+              ++ncand;
+            } else {
+              unite(j);   // more than 8 neighbours (heavy overlap): unite on the spot
             }
           }
         }
-        h = (h + 1u) & (HS - 1u);
       }
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      if ((uint32_t)i < ncand) unite((cand[i >> 1] >> ((i & 1) * 16)) & 0xFFFFu);
     }
   }
   __syncthreads();
 
+  uint32_t* head = reinterpret_cast<uint32_t*>(smem + L::kRegC);   // [T] member chain head per root (nextc is dead)
   // ---- S3: label = root (smallest sorted index of the component); ordinals of the roots ---------
   {
     uint32_t root_r[IPT];
@@ -548,6 +566,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
       const uint32_t k = (uint32_t)j * THREADS + tid;
       if (k < mm) {
         parent[k] = root_r[j];
+        head[k] = kNone;
         a.label[out_base + k] = out_base + root_r[j];
       }
     }
@@ -608,7 +627,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
       const int idx = jb - (int)lane;
       unsigned long long v = kTilePrefix;   // before tile 0: an empty prefix
       if (idx >= 0) {
-        do { v = ld_volatile_u64(a.tiles + idx); } while ((v >> 62) == 0ull);
+        while (((v = ld_volatile_u64(a.tiles + idx)) >> 62) == 0ull) __nanosleep(64);
       }
       const uint32_t pm = __ballot_sync(0xffffffffu, (v >> 62) == 2ull);
       const uint32_t first = pm ? (uint32_t)__ffs(pm) - 1u : 31u;   // nearest predecessor holding a prefix
