@@ -13,22 +13,30 @@
 //   needs a prefix over tiles: a decoupled look-back over per-tile status words (tiles are
 //   handed out by an atomic ticket, so every predecessor of a running tile has started).
 //
-// Per tile (all in shared memory, one CTA):
-//   load     128-bit coalesced loads of toa / x / y / tot; shot = toa div P by multiply-high with
-//            a precomputed magic number; composite key = (shot - first shot) << tof_bits | ToF
-//   sort     skipped when the keys are already ascending; otherwise stable LSD radix sort of
-//            16-bit local indices, digits ranked per warp with match.any (S1)
-//   link     multimap hash table (cell -> event) in shared memory; every event probes its own
-//            cell and the 4 "forward" neighbour cells (E, SW, S, SE), tests same shot and
-//            |dToA| <= W (Eq. 5) and unites in a lock-free union-find that
-//            always hooks the larger root under the smaller (S2)
-//   compress label = root = smallest sorted index of the component; ordinals by block scan (S3)
-//   reduce   members chained to their root (one atomicExch each); one thread per hit walks
-//            the chain: exact 64-bit sums, brightest pixel by (ToT, sorted index) (S4, :150)
+// Per tile (all in shared memory, one CTA; k = sorted position inside the tile):
+//   load     128-bit coalesced loads of toa / x / y / tot. rel = toa - (first shot of the tile)*P
+//            fits 32 bits; shot offset sl = rel div P by a 32-bit multiply-high; tof = rel - sl*P.
+//            key = sl << tb | tof with 2^tb > max tof + W, so |key_i - key_j| <= W already implies
+//            "same shot" and ONE compare is the whole time test of Eq. 5.
+//   sort     skipped when the keys are already ascending; otherwise stable LSD radix sort of 16-bit
+//            local indices, digits ranked per warp with ballots (S1)
+//   hash     open table of 4-slot buckets (one 128-bit load reads a bucket), key (shot, cell),
+//            entry = cell << 16 | k+1; a bucket that overflows spills to the next one and marks
+//            itself, so the common probe is straight-line code
+//   link     every event probes S, E, SE, SW and its own cell ("forward" cells), applies the time
+//            test and keeps only links that are not implied by other neighbour pairs (two
+//            candidates that are themselves adjacent in space and time are linked by one of them).
+//            The first kept link is a plain store parent[k] = j (forward order => no cycles); the
+//            few others go to a list that is united afterwards with compare-and-swap hooks (S2)
+//   label    root per event by pointer chasing, label = smallest k of the component (shared-memory
+//            atomicMin per event), ordinals of the labels by block scan (S3)
+//   reduce   members chained to their label (one atomicExch each); one thread per hit walks the
+//            chain: exact 64-bit sums, brightest pixel by (ToT, sorted index) (S4)
 //   centroid fp32(sum tot*x) / fp32(sum tot), IEEE RN (S5, Eq. 9)
 //
-// A tile that cannot be handled (a shot longer than L, a decreasing shot number, key wider than
-// 32 bits) marks the call as failed; the general kernels, enqueued behind this one, then run.
+// A tile that cannot be handled (a shot longer than L, a decreasing shot number, shot offset and
+// time of flight too wide for one 32-bit key) marks the call as failed; the general kernels, enqueued behind this one,
+// then redo the call.
 #pragma once
 #include "tpx3_common.cuh"
 
@@ -74,6 +82,28 @@ __device__ __forceinline__ uint64_t div64(uint64_t n, const Div64& d) {
   return q >> d.shift;
 }
 
+// ---- exact 32-bit division by an invariant divisor -------------------------------------------
+// Granlund & Montgomery 1994, Fig. 4.1 (N = 32): l = ceil(log2 d), m' = floor(2^32 (2^l - d) / d) + 1,
+// q = (t + ((n - t) >> sh1)) >> sh2 with t = mulhi(m', n), sh1 = min(l, 1), sh2 = max(l - 1, 0).
+struct Div32 {
+  uint32_t m, sh1, sh2;
+};
+
+inline Div32 make_div32(uint32_t d) {
+  uint32_t l = 0;
+  while (((uint64_t)1 << l) < d) ++l;
+  Div32 r;
+  r.m = (uint32_t)((((uint64_t)1 << 32) * (((uint64_t)1 << l) - d)) / d + 1);
+  r.sh1 = l < 1 ? l : 1;
+  r.sh2 = l ? l - 1 : 0;
+  return r;
+}
+
+__device__ __forceinline__ uint32_t div32(uint32_t n, const Div32& d) {
+  const uint32_t t = __umulhi(d.m, n);
+  return (t + ((n - t) >> d.sh1)) >> d.sh2;
+}
+
 // ---- tile status words for the decoupled look-back -------------------------------------------
 constexpr unsigned long long kTileAggregate = 1ull << 62;  // value = hits of this tile
 constexpr unsigned long long kTilePrefix = 2ull << 62;     // value = hits of tiles 0..this
@@ -102,6 +132,7 @@ struct FusedArgs {
   uint64_t n;
   uint64_t P;
   Div64 divP;
+  Div32 divP32;
   uint32_t W;
   uint32_t S;          // slice length (events); tile b owns shots starting in [b*S, (b+1)*S)
   uint32_t num_tiles;
@@ -119,40 +150,80 @@ struct FusedArgs {
 };
 
 constexpr uint32_t kNone = 0xFFFFFFFFu;
+constexpr uint32_t kGold = 0x9E3779B1u;
 
+// Shared-memory map (bytes). Records are uint2 {key, xy | tot << 16}.
+//   A [0, 8T)    sorted records (unsorted input only)            } the hash table takes the 16T bytes
+//   X [8T, 16T)  sort index buffers + warp digit counters        } next to the live records: A+X when
+//   B [16T, 24T) records as loaded (input order)                 } the input was sorted, X+B otherwise
+//   P [24T, 26T) bucket fill counters (u16) -> parent (u16)
+//   L [26T, 27.5T) deferred links
+// After the link step the hash region is reused: minidx u32[T] | head u32[T] | lab u16[T] |
+// rootpos u16[T] | nxt u16[T]  (14T <= 16T).
 template <int T>
 struct FusedSmem {
-  // byte offsets inside the dynamic shared memory block
-  static constexpr int kRegA = 0;            // 8T  unsorted->sorted records OR hash / lists
-  static constexpr int kRegB = 8 * T;        // 8T  records as loaded (input order)
-  static constexpr int kRegC = 16 * T;       // 4T  sort index double buffer -> chain heads
-  static constexpr int kRegD = 20 * T;       // 4T  warp digit counters (sort) -> parent
-  static constexpr int kMisc = 24 * T;       // small block-wide scalars
+  static constexpr int kRegA = 0;
+  static constexpr int kRegX = 8 * T;
+  static constexpr int kRegB = 16 * T;
+  static constexpr int kPar = 24 * T;
+  static constexpr int kList = 26 * T;
+  static constexpr int kListCap = 3 * T / 8;           // deferred links the list holds
+  static constexpr int kMisc = kList + 4 * kListCap;   // 27.5 T
   static constexpr int kMiscBytes = 512;
   static constexpr int kBytes = kMisc + kMiscBytes;
 };
 
 struct FusedMisc {
-  unsigned long long s_lo;     // shot number of the first owned event
   unsigned int lo, hi;         // owned range, relative to the tile base
   unsigned int fail;
-  unsigned int unsorted;
-  unsigned int max_tof, max_local;
+  unsigned int max_tof, max_sl;
   unsigned int ticket;
   unsigned int n_roots;
   unsigned int ord_base;
+  unsigned int n_list;         // deferred links pushed (may exceed the capacity: overflow)
   unsigned int warp_sums[33];
-  unsigned int is_last;
 };
 static_assert(sizeof(FusedMisc) <= 512, "FusedMisc must fit kMiscBytes");
+
+__device__ __forceinline__ uint32_t absdiff_u32(uint32_t a, uint32_t b) { return a > b ? a - b : b - a; }
+
+// ---- union-find on 16-bit parents (two per 32-bit word) ----------------------------------------
+__device__ __forceinline__ uint32_t uf_find(const uint16_t* par, uint32_t x) {
+  uint32_t p;
+  while ((p = par[x]) != x) x = p;
+  return x;
+}
+
+// Hooks the larger root under the smaller with a compare-and-swap on the word that holds it; only a
+// node that still is a root (parent == self) is ever changed, so no cycle can form.
+__device__ __forceinline__ void uf_unite(uint16_t* par, uint32_t a, uint32_t b) {
+  for (;;) {
+    a = uf_find(par, a);
+    b = uf_find(par, b);
+    if (a == b) return;
+    if (a < b) { const uint32_t t = a; a = b; b = t; }
+    uint32_t* w = reinterpret_cast<uint32_t*>(par + (a & ~1u));
+    const uint32_t sh = (a & 1u) * 16u;
+    uint32_t old = *reinterpret_cast<volatile uint32_t*>(w);
+    for (;;) {
+      if (((old >> sh) & 0xFFFFu) != a) break;   // a was hooked meanwhile: find again
+      const uint32_t nw = (old & ~(0xFFFFu << sh)) | (b << sh);
+      const uint32_t prev = atomicCAS(w, old, nw);
+      if (prev == old) return;
+      old = prev;
+    }
+  }
+}
 
 // One tile per CTA. T = tile capacity (events), THREADS = T / 8.
 template <int T, int THREADS>
 __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_tiles(FusedArgs a) {
-  constexpr int IPT = T / THREADS;  // 8 consecutive events per thread in the load phase
+  constexpr int IPT = T / THREADS;  // 8 events per thread
   static_assert(IPT == 8, "the 128-bit load phase assumes 8 events per thread");
   constexpr int WARPS = THREADS / 32;
-  constexpr uint32_t HS = 2u * T;   // hash slots
+  constexpr uint32_t NB = T;        // hash buckets of 4 slots (16 bytes each)
+  constexpr uint32_t kHashShift = 32u - (T == 8192 ? 13u : 12u);
+  static_assert(T == 8192 || T == 4096, "hash shift table");
   using L = FusedSmem<T>;
   extern __shared__ __align__(16) unsigned char smem[];
   FusedMisc* misc = reinterpret_cast<FusedMisc*>(smem + L::kMisc);
@@ -164,12 +235,11 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
     misc->lo = kNone;
     misc->hi = kNone;
     misc->fail = 0;
-    misc->unsorted = 0;
     misc->max_tof = 0;
-    misc->max_local = 0;
+    misc->max_sl = 0;
     misc->n_roots = 0;
     misc->ord_base = 0;
-    misc->is_last = 0;
+    misc->n_list = 0;
   }
   __syncthreads();
   const uint32_t b = misc->ticket;
@@ -177,8 +247,9 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
   const uint64_t avail = a.n - base;                   // > 0 by construction
   const uint32_t cnt = avail < (uint64_t)T ? (uint32_t)avail : (uint32_t)T;  // events readable
   const uint32_t p0 = tid * IPT;                       // this thread's 8 tile-relative positions
+  const uint32_t P32 = (uint32_t)a.P;
 
-  // ---- load ToA (2 events per 128-bit load), shot numbers, boundaries --------------------------
+  // ---- load ToA (2 events per 128-bit load) ----------------------------------------------------
   uint64_t toa_r[IPT];
   if (p0 + IPT <= cnt) {
     const uint4* src = reinterpret_cast<const uint4*>(a.toa + base + p0);
@@ -192,123 +263,126 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
 #pragma unroll
     for (int j = 0; j < IPT; ++j) toa_r[j] = (p0 + j < cnt) ? a.toa[base + p0 + j] : 0ull;
   }
-  // shot of the event just before this thread's first one (previous lane, or a global load)
-  uint64_t s_first = div64(toa_r[0], a.divP);
-  uint64_t s_last = div64(toa_r[IPT - 1], a.divP);
-  uint64_t s_prev;
-  {
-    uint32_t lo32 = __shfl_up_sync(0xffffffffu, (uint32_t)s_last, 1);
-    uint32_t hi32 = __shfl_up_sync(0xffffffffu, (uint32_t)(s_last >> 32), 1);
-    s_prev = ((uint64_t)hi32 << 32) | lo32;
-    if (lane == 0) {
-      if (base + p0 > 0 && p0 < cnt) s_prev = div64(a.toa[base + p0 - 1], a.divP);
-      else s_prev = ~0ull;  // position 0 of the stream: always a shot start
+  // the event just before this warp's first one (lanes > 0 get it from the previous lane)
+  uint64_t t_prev = 0;
+  const bool has_prev = lane == 0 && p0 < cnt && base + p0 > 0;
+  if (has_prev) t_prev = a.toa[base + p0 - 1];
+  // reference time of the tile: start of the shot its first event belongs to
+  const uint64_t s_base = div64(a.toa[base], a.divP);
+  const uint64_t ref = s_base * a.P;
+
+  // ---- shot offsets and times of flight; shot boundaries ----------------------------------------
+  uint32_t sl[IPT], tof[IPT];
+  bool bad = false;
+#pragma unroll
+  for (int j = 0; j < IPT; ++j) {
+    const uint64_t r64 = toa_r[j] - ref;
+    const bool in = p0 + j < cnt;
+    const uint32_t rel = in ? (uint32_t)r64 : 0u;
+    sl[j] = div32(rel, a.divP32);
+    tof[j] = rel - sl[j] * P32;
+    if (in && (r64 >> 32) != 0ull) {   // rare: more than 2^32 ticks after the tile's first shot (or before it)
+      const uint64_t q = div64(r64, a.divP);
+      if (q >> 32) bad = true;
+      sl[j] = (uint32_t)q;
+      tof[j] = (uint32_t)(r64 - q * a.P);
+    }
+  }
+  uint32_t slp = __shfl_up_sync(0xffffffffu, sl[IPT - 1], 1);
+  uint32_t tofp = __shfl_up_sync(0xffffffffu, tof[IPT - 1], 1);
+  bool start0 = sl[0] != slp, viol0 = sl[0] < slp;
+  if (lane == 0) {
+    if (!has_prev) { start0 = p0 < cnt; viol0 = false; slp = 0; tofp = 0; }          // position 0 of the stream
+    else if (t_prev < ref) { start0 = true; viol0 = false; slp = 0; tofp = 0; }        // previous shot
+    else {
+      const uint64_t r64 = t_prev - ref;
+      const uint64_t q = div64(r64, a.divP);
+      slp = (q >> 32) ? kNone : (uint32_t)q;
+      tofp = (uint32_t)(r64 - q * a.P);
+      start0 = sl[0] != slp;
+      viol0 = sl[0] < slp;
     }
   }
   uint32_t bnd = 0;  // bit j: event p0+j starts a shot
   bool viol = false;
   {
-    uint64_t sp = s_prev;
+    if (p0 < cnt) {
+      if (start0) bnd |= 1u;
+      if (viol0 && p0 < a.S) viol = true;            // each position is checked by exactly one tile
+    }
 #pragma unroll
-    for (int j = 0; j < IPT; ++j) {
+    for (int j = 1; j < IPT; ++j) {
       if (p0 + j < cnt) {
-        uint64_t s = (j == 0) ? s_first : ((j == IPT - 1) ? s_last : div64(toa_r[j], a.divP));
-        bool start = (base + p0 + j == 0) || (s != sp);
-        if (start) bnd |= 1u << j;
-        if (base + p0 + j != 0 && s < sp && p0 + j < a.S) viol = true;  // each position checked once
-        sp = s;
+        if (sl[j] != sl[j - 1]) bnd |= 1u << j;
+        if (sl[j] < sl[j - 1] && p0 + j < a.S) viol = true;
       }
     }
   }
   // lo = first shot start in [0, S); hi = first shot start in [S, cnt) (or cnt == end of stream)
   {
-    uint32_t my_lo = kNone, my_hi = kNone;
+    uint32_t my_lo = kNone, my_hi = kNone, mt = 0, ml = 0;
 #pragma unroll
     for (int j = IPT - 1; j >= 0; --j) {
       if (bnd & (1u << j)) {
         if (p0 + j < a.S) my_lo = p0 + j;
         else my_hi = p0 + j;
       }
+      mt = max(mt, tof[j]);
+      ml = max(ml, sl[j]);
     }
-    // my_hi must be the FIRST start at or after S: the loop runs downwards, so it is
-#pragma unroll
-    for (int o = 16; o; o >>= 1) {
-      my_lo = min(my_lo, __shfl_xor_sync(0xffffffffu, my_lo, o));
-      my_hi = min(my_hi, __shfl_xor_sync(0xffffffffu, my_hi, o));
-    }
-    uint32_t any_viol = __any_sync(0xffffffffu, viol);
+    my_lo = __reduce_min_sync(0xffffffffu, my_lo);
+    my_hi = __reduce_min_sync(0xffffffffu, my_hi);
+    mt = __reduce_max_sync(0xffffffffu, mt);
+    ml = __reduce_max_sync(0xffffffffu, ml);
+    const uint32_t any_bad = __any_sync(0xffffffffu, bad || viol);
     if (lane == 0) {
       if (my_lo != kNone) atomicMin(&misc->lo, my_lo);
       if (my_hi != kNone) atomicMin(&misc->hi, my_hi);
-      if (any_viol) misc->fail = 1;
-    }
-  }
-  __syncthreads();
-  uint32_t lo = misc->lo, hi = misc->hi;
-  if (hi == kNone) {
-    if (base + cnt >= a.n) hi = cnt;          // the stream ends inside this tile's window
-    else if (lo != kNone) { hi = lo; if (tid == 0) misc->fail = 1; }  // last shot longer than the window
-  }
-  if (lo == kNone) { lo = 0; hi = 0; }        // no shot starts in this slice: nothing owned
-  const uint32_t m = hi - lo;                 // owned events; sorted position k <-> p = lo + k
-  // shot number of the first owned event
-  if (m && lo >= p0 && lo < p0 + IPT) {
-    uint64_t s = 0;
-#pragma unroll
-    for (int j = 0; j < IPT; ++j)
-      if (p0 + j == lo) s = div64(toa_r[j], a.divP);
-    misc->s_lo = s;
-  }
-  __syncthreads();
-  const uint64_t s_lo = misc->s_lo;
-
-  // ---- ToF and shot offset of every owned event; widths of the composite key ------------------
-  uint32_t tof_r[IPT], loc_r[IPT];
-  {
-    uint32_t mt = 0, ml = 0;
-    bool bad = false;
-#pragma unroll
-    for (int j = 0; j < IPT; ++j) {
-      const uint32_t p = p0 + j;
-      tof_r[j] = 0;
-      loc_r[j] = 0;
-      if (p >= lo && p < hi) {
-        uint64_t s = div64(toa_r[j], a.divP);
-        uint64_t d = s - s_lo;
-        if (d > 0xFFFFFFFFull) bad = true;
-        tof_r[j] = (uint32_t)(toa_r[j] - s * a.P);
-        loc_r[j] = (uint32_t)d;
-        mt = max(mt, tof_r[j]);
-        ml = max(ml, loc_r[j]);
-      }
-    }
-#pragma unroll
-    for (int o = 16; o; o >>= 1) {
-      mt = max(mt, __shfl_xor_sync(0xffffffffu, mt, o));
-      ml = max(ml, __shfl_xor_sync(0xffffffffu, ml, o));
-    }
-    uint32_t any_bad = __any_sync(0xffffffffu, bad);
-    if (lane == 0) {
       if (mt) atomicMax(&misc->max_tof, mt);
-      if (ml) atomicMax(&misc->max_local, ml);
+      if (ml) atomicMax(&misc->max_sl, ml);
       if (any_bad) misc->fail = 1;
     }
   }
-  __syncthreads();
-  const uint32_t tof_bits = misc->max_tof ? 32u - (uint32_t)__clz(misc->max_tof) : 1u;
-  const uint32_t shot_bits = misc->max_local ? 32u - (uint32_t)__clz(misc->max_local) : 0u;
-  const uint32_t key_bits = tof_bits + shot_bits;
-  const bool failed = misc->fail || key_bits > 32u;
-  const uint32_t mm = failed ? 0u : m;   // a failed tile owns nothing (the general path redoes the call)
-
-  // ---- records as loaded -> region B (key, xy, tot), 128-bit loads of x / y / tot ---------------
-  uint32_t* keyB = reinterpret_cast<uint32_t*>(smem + L::kRegB);
-  uint16_t* xyB = reinterpret_cast<uint16_t*>(smem + L::kRegB + 4 * T);
-  uint16_t* totB = reinterpret_cast<uint16_t*>(smem + L::kRegB + 6 * T);
-  uint32_t key_r[IPT];
+  // meanwhile: clear the hash region for sorted input (A + X) and the bucket counters
+  {
+    uint4* z = reinterpret_cast<uint4*>(smem + L::kRegA);
+    const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
-  for (int j = 0; j < IPT; ++j) key_r[j] = (loc_r[j] << tof_bits) | tof_r[j];
+    for (int q = 0; q < 16 * T / 16 / THREADS; ++q) z[q * THREADS + tid] = zero;
+    uint4* zc = reinterpret_cast<uint4*>(smem + L::kPar);
+    if (tid < 2 * T / 16) zc[tid] = zero;
+    static_assert(2 * T / 16 <= THREADS, "counter clear");
+  }
+  __syncthreads();
+  uint32_t lo = misc->lo, hi = misc->hi;
+  bool failed = misc->fail != 0;
+  if (hi == kNone) {
+    if (base + cnt >= a.n) hi = cnt;                      // the stream ends inside this tile's window
+    else if (lo != kNone) { hi = lo; failed = true; }     // last shot longer than the window
+  }
+  if (lo == kNone) { lo = 0; hi = 0; }                    // no shot starts in this slice: nothing owned
+  // key layout: 2^tb > max tof + W, so keys of different shots differ by more than W
+  const uint32_t tspan = misc->max_tof + a.W;
+  const uint32_t tb = tspan ? 32u - (uint32_t)__clz(tspan) : 0u;
+  const uint32_t sbits = misc->max_sl ? 32u - (uint32_t)__clz(misc->max_sl) : 0u;
+  if (tb + sbits > 32u) failed = true;
+  const uint32_t mm = failed ? 0u : hi - lo;   // owned events; a failed tile owns nothing
+  const uint32_t tmask = tb >= 32u ? 0xFFFFFFFFu : ((1u << tb) - 1u);
+  const uint32_t out_base = (uint32_t)(base + lo);  // global sorted position of local rank 0 (n <= 2^28)
+
+  // ---- records as loaded -> region B, 128-bit loads of x / y / tot ------------------------------
+  uint2* recB = reinterpret_cast<uint2*>(smem + L::kRegB);
+  bool uns = false;
   if (mm && p0 < hi && p0 + IPT > lo) {
+    uint32_t key_r[IPT];
+#pragma unroll
+    for (int j = 0; j < IPT; ++j) key_r[j] = (tb >= 32u ? 0u : (sl[j] << tb)) | tof[j];
+    const uint32_t keyp = (tb >= 32u ? 0u : (slp << tb)) | tofp;
+    // already in (shot, ToA) order? (configs 0-3 arrive sorted; config 4 does not)
+    if (p0 > lo && key_r[0] < keyp) uns = true;
+#pragma unroll
+    for (int j = 1; j < IPT; ++j)
+      if (p0 + j > lo && p0 + j < hi && key_r[j] < key_r[j - 1]) uns = true;
     uint4 vx, vy, vt;
     if (p0 + IPT <= cnt) {
       vx = ldg_nc_v4(a.x + base + p0);
@@ -330,9 +404,9 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
       vt = make_uint4(tt[0] | ((uint32_t)tt[1] << 16), tt[2] | ((uint32_t)tt[3] << 16),
                       tt[4] | ((uint32_t)tt[5] << 16), tt[6] | ((uint32_t)tt[7] << 16));
     }
+    const uint32_t xs[4] = {vx.x, vx.y, vx.z, vx.w}, ys[4] = {vy.x, vy.y, vy.z, vy.w},
+                   ts[4] = {vt.x, vt.y, vt.z, vt.w};
     if (a.flags & TPX3_FLAG_VALIDATE_INPUT) {
-      const uint32_t xs[4] = {vx.x, vx.y, vx.z, vx.w}, ys[4] = {vy.x, vy.y, vy.z, vy.w},
-                     ts[4] = {vt.x, vt.y, vt.z, vt.w};
       bool oob = false;
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
@@ -348,43 +422,29 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
       }
       if (oob) set_error(a.ctrl, TPX3_ERR_OUT_OF_RANGE);
     }
-    // xy = x | y << 8, two events per 32-bit word
-    uint4 vxy;
-    vxy.x = (vx.x & 0x00FF00FFu) | ((vy.x & 0x00FF00FFu) << 8);
-    vxy.y = (vx.y & 0x00FF00FFu) | ((vy.y & 0x00FF00FFu) << 8);
-    vxy.z = (vx.z & 0x00FF00FFu) | ((vy.z & 0x00FF00FFu) << 8);
-    vxy.w = (vx.w & 0x00FF00FFu) | ((vy.w & 0x00FF00FFu) << 8);
-    *reinterpret_cast<uint4*>(xyB + p0) = vxy;
-    *reinterpret_cast<uint4*>(totB + p0) = vt;
-    *reinterpret_cast<uint4*>(keyB + p0) = make_uint4(key_r[0], key_r[1], key_r[2], key_r[3]);
-    *reinterpret_cast<uint4*>(keyB + p0 + 4) = make_uint4(key_r[4], key_r[5], key_r[6], key_r[7]);
-  }
-  __syncthreads();
-  // already in (shot, ToA) order? (configs 0-3 arrive sorted; config 4 does not)
-  {
-    bool uns = false;
+    // record word 1: x | y << 8 | tot << 16
+    uint32_t w1[IPT];
 #pragma unroll
-    for (int j = 0; j < IPT; ++j) {
-      const uint32_t p = p0 + j;
-      if (p > lo && p < lo + mm) {
-        uint32_t prev = (j == 0) ? keyB[p - 1] : key_r[j - 1];
-        if (key_r[j] < prev) uns = true;
-      }
+    for (int q = 0; q < 4; ++q) {
+      w1[2 * q] = (xs[q] & 0xFFu) | ((ys[q] & 0xFFu) << 8) | (ts[q] << 16);
+      w1[2 * q + 1] = ((xs[q] >> 16) & 0xFFu) | (((ys[q] >> 16) & 0xFFu) << 8) | (ts[q] & 0xFFFF0000u);
     }
-    if (__any_sync(0xffffffffu, uns) && lane == 0) misc->unsorted = 1;
+    uint4* dst = reinterpret_cast<uint4*>(recB + p0);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) dst[q] = make_uint4(key_r[2 * q], w1[2 * q], key_r[2 * q + 1], w1[2 * q + 1]);
   }
-  __syncthreads();
-  const bool unsorted = misc->unsorted != 0;
+  const bool unsorted = __syncthreads_or(uns ? 1 : 0) != 0;
 
-  // ---- S1: stable LSD radix sort of local indices by composite key (only if needed) ------------
-  uint32_t* keyA = reinterpret_cast<uint32_t*>(smem + L::kRegA);
-  uint16_t* xyA = reinterpret_cast<uint16_t*>(smem + L::kRegA + 4 * T);
-  uint16_t* totA = reinterpret_cast<uint16_t*>(smem + L::kRegA + 6 * T);
-  const uint32_t out_base = (uint32_t)(base + lo);  // global sorted position of local rank 0 (n <= 2^28)
+  // ---- S1: stable LSD radix sort of local indices by (shot offset, tof) (only if needed) --------
+  uint2* recA = reinterpret_cast<uint2*>(smem + L::kRegA);
   if (unsorted) {
-    uint16_t* buf0 = reinterpret_cast<uint16_t*>(smem + L::kRegC);
+    uint16_t* buf0 = reinterpret_cast<uint16_t*>(smem + L::kRegX);
     uint16_t* buf1 = buf0 + T;
-    uint32_t* wcnt = reinterpret_cast<uint32_t*>(smem + L::kRegD);  // [WARPS][256]
+    uint32_t* wcnt = reinterpret_cast<uint32_t*>(smem + L::kRegX + 4 * T);  // [WARPS][256]
+    static_assert(WARPS * 256 * 4 <= 4 * T, "warp digit counters");
+    // sort key without the gap between the tof bits and the shot bits
+    const uint32_t tofb = misc->max_tof ? 32u - (uint32_t)__clz(misc->max_tof) : 1u;
+    const uint32_t key_bits = tofb + sbits;
     const uint32_t npass = (key_bits + 7u) / 8u;
     const uint32_t dbits = (key_bits + npass - 1u) / npass;         // <= 8
     const uint32_t radix = 1u << dbits, dmask = radix - 1u;
@@ -400,16 +460,24 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
       for (int j = 0; j < IPT; ++j) {
         const uint32_t k = warp * (32u * IPT) + (uint32_t)j * 32u + lane;   // warps own ascending slices
         const bool valid = k < mm;
-        uint32_t s = valid ? (pass == 0 ? k : (uint32_t)src[k]) : 0u;
-        uint32_t d = valid ? ((keyB[lo + s] >> shift) & dmask) : 256u;      // 256: "no event"
-        uint32_t peers = __match_any_sync(0xffffffffu, d);
-        uint32_t lr = __popc(peers & lt);
-        uint32_t c0 = valid ? wcnt[warp * 256u + d] : 0u;
+        const uint32_t s = valid ? (pass == 0 ? k : (uint32_t)src[k]) : 0u;
+        const uint32_t key = valid ? recB[lo + s].x : 0u;
+        const uint32_t sk = ((key >> tb) << tofb) | (key & tmask);
+        const uint32_t d = (sk >> shift) & dmask;
+        // lanes holding the same digit (ballot per digit bit; match.any is 20x dearer on sm_100)
+        uint32_t peers = __ballot_sync(0xffffffffu, valid);
+        for (uint32_t bit = 0; bit < dbits; ++bit) {
+          const bool one = (d >> bit) & 1u;
+          const uint32_t bal = __ballot_sync(0xffffffffu, one);
+          peers &= one ? bal : ~bal;
+        }
+        const uint32_t lr = __popc(peers & lt);
+        const uint32_t c0 = valid ? wcnt[warp * 256u + d] : 0u;
         __syncwarp();
         if (valid && lr == 0) wcnt[warp * 256u + d] = c0 + __popc(peers);
         __syncwarp();
         e_src[j] = s;
-        e_dig[j] = d;
+        e_dig[j] = valid ? d : 256u;                                        // 256: "no event"
         e_rank[j] = c0 + lr;
       }
       __syncthreads();
@@ -449,141 +517,207 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
     // gather the records into sorted order (region A) and emit perm
     for (uint32_t k = tid; k < mm; k += THREADS) {
       const uint32_t s = fin[k];
-      keyA[k] = keyB[lo + s];
-      xyA[k] = xyB[lo + s];
-      totA[k] = totB[lo + s];
+      recA[k] = recB[lo + s];
       a.perm[out_base + k] = out_base + s;
     }
+    __syncthreads();
+    // the hash table now takes X + B: clear it
+    uint4* z = reinterpret_cast<uint4*>(smem + L::kRegX);
+    const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+    for (int q = 0; q < 16 * T / 16 / THREADS; ++q) z[q * THREADS + tid] = zero;
+    __syncthreads();
   } else {
     for (uint32_t k = tid; k < mm; k += THREADS) a.perm[out_base + k] = out_base + k;
   }
-  __syncthreads();
-  const uint32_t* keyS = unsorted ? keyA : keyB + lo;
-  const uint16_t* xyS = unsorted ? xyA : xyB + lo;
-  const uint16_t* totS = unsorted ? totA : totB + lo;
-  unsigned char* freeR = smem + (unsorted ? L::kRegB : L::kRegA);   // 8T bytes no longer needed
+  const uint2* recS = unsorted ? recA : recB + lo;
+  unsigned char* hreg = smem + (unsorted ? L::kRegX : L::kRegA);   // 16T bytes: hash table, later the label / chain arrays
+  uint32_t* tab = reinterpret_cast<uint32_t*>(hreg);               // [NB][4]
+  uint32_t* cnt32 = reinterpret_cast<uint32_t*>(smem + L::kPar);   // bucket fill counters, u16 pairs
+  uint16_t* par = reinterpret_cast<uint16_t*>(smem + L::kPar);     // parent (after the insert step)
+  uint32_t* list = reinterpret_cast<uint32_t*>(smem + L::kList);   // deferred links k << 16 | j
 
-  // ---- S2: chained hash cell -> events, probe own + 4 forward cells, union-find -----------------
-  // bucket head and chain links both carry (cell << 16 | event), so a chain is walked without
-  // touching the records; only a cell match reads the candidate's key (same shot, |dToA| <= W).
-  uint32_t* bhead = reinterpret_cast<uint32_t*>(freeR);               // [HS] kNone = empty bucket
-  uint32_t* nextc = reinterpret_cast<uint32_t*>(smem + L::kRegC);     // [T]  next node of the bucket chain
-  uint32_t* parent = reinterpret_cast<uint32_t*>(smem + L::kRegD);    // [T]
-  {
-    uint4 e = make_uint4(kNone, kNone, kNone, kNone);
-    uint4* t4 = reinterpret_cast<uint4*>(bhead);
-#pragma unroll
-    for (int q = 0; q < (int)(HS / 4 / THREADS); ++q) t4[q * THREADS + tid] = e;
-    for (uint32_t k = tid; k < mm; k += THREADS) parent[k] = k;
-  }
-  __syncthreads();
-  constexpr uint32_t kHashShift = 32u - (T == 8192 ? 14u : (T == 4096 ? 13u : (T == 2048 ? 12u : 11u)));
-  static_assert(T == 8192 || T == 4096 || T == 2048 || T == 1024, "hash shift table");
+  // ---- hash insert: entry = cell << 16 | k+1 into bucket hash(shot offset, cell) ------------------
+  // Slot c of a bucket is taken by the c-th arrival (counter); arrivals past the 4th mark the bucket
+  // (bit 15 of slot 3) and spill to the next bucket.
   for (uint32_t k = tid; k < mm; k += THREADS) {
-    const uint32_t cell = xyS[k], loc = keyS[k] >> tof_bits;
-    const uint32_t h = ((cell | (loc << 16)) * 0x9E3779B1u) >> kHashShift;
-    nextc[k] = atomicExch(&bhead[h], (cell << 16) | k);
+    const uint2 r = recS[k];
+    const uint32_t cell = r.y & 0xFFFFu, slk = r.x >> tb;
+    uint32_t h = ((cell | (slk << 16)) * kGold) >> kHashShift;
+    const uint32_t entry = (cell << 16) | (k + 1u);
+    for (;;) {
+      const uint32_t sh = (h & 1u) * 16u;
+      const uint32_t c = (atomicAdd(&cnt32[h >> 1], 1u << sh) >> sh) & 0xFFFFu;
+      if (c < 4u) { atomicOr(&tab[4u * h + c], entry); break; }
+      atomicOr(&tab[4u * h + 3u], 0x8000u);
+      h = (h + 1u) & (NB - 1u);
+    }
   }
   __syncthreads();
-  for (uint32_t k0 = 0; k0 < mm; k0 += THREADS) {   // block-uniform trip count; lanes past mm idle
-    const uint32_t k = k0 + tid;
-    const bool act = k < mm;
-    const uint32_t cell = act ? xyS[k] : 0u, key = act ? keyS[k] : 0u, loc = key >> tof_bits;
-    const uint32_t x = cell & 0xFFu, y = cell >> 8;
-    // neighbour cells still to visit: bit q of {own, E, SW, S, SE}; sensor edges removed
-    uint32_t todo = 0;
-    if (act) {
-      const bool xe = x + 1u < a.sensor_w, xw = x > 0u, ys = y + 1u < a.sensor_h;
-      todo = 1u | (xe ? 2u : 0u) | ((xw && ys) ? 4u : 0u) | (ys ? 8u : 0u) | ((xe && ys) ? 16u : 0u);
-    }
-    // one flattened loop over all five chains keeps the lanes of a warp in step; matching
-    // candidates are only recorded here (up to 8, packed 2 per register) and united afterwards
-    uint32_t cand[4] = {0u, 0u, 0u, 0u};
-    uint32_t ncand = 0, cur = kNone, c = 0, q = 0;
-    uint32_t rk = k;   // current guess of k's root
-    auto unite = [&](uint32_t j) {
-      uint32_t ra = rk, rb = j;
-      for (;;) {
-        uint32_t p;
-        while ((p = parent[ra]) != ra) { uint32_t g = parent[p]; if (g != p) parent[ra] = g; ra = p; }
-        while ((p = parent[rb]) != rb) { uint32_t g = parent[p]; if (g != p) parent[rb] = g; rb = p; }
-        if (ra == rb) break;
-        if (ra < rb) { uint32_t t = ra; ra = rb; rb = t; }
-        const uint32_t old = atomicMin(&parent[ra], rb);   // hook the larger root under the smaller
-        if (old == ra) { ra = rb; break; }
-        ra = old;
-      }
-      rk = ra;
-    };
-    while (todo != 0u || cur != kNone) {
-      if (cur == kNone) {
-        q = (uint32_t)__ffs(todo) - 1u;
-        todo &= todo - 1u;
-        const uint32_t off = (q == 0u) ? 0u : (q == 1u ? 1u : 253u + q);   // 0, +1, +255, +256, +257
-        c = cell + off;
-        cur = bhead[((c | (loc << 16)) * 0x9E3779B1u) >> kHashShift];
-      } else {
-        const uint32_t j = cur & 0xFFFFu, tag = cur >> 16;
-        cur = nextc[j];
-        if (tag == c && (q != 0u || j < k)) {
-          const uint32_t kj = keyS[j];
-          const uint32_t dt = key > kj ? key - kj : kj - key;
-          if ((kj >> tof_bits) == loc && dt <= a.W) {
-            if (ncand < 8u) {
-              cand[ncand >> 1] |= j << ((ncand & 1u) * 16u);
-              ++ncand;
-            } else {
-              unite(j);   // more than 8 neighbours (heavy overlap): unite on the spot
-            }
-          }
+
+  // ---- S2: probe the forward cells, prune implied links, first link = parent, others deferred ---
+  // Scans one neighbour cell completely (home bucket and, while marked, the following ones) and
+  // hands every event that passes the time test to `sink`. Used for the rare cases only.
+  auto scan_cell = [&](uint32_t c, uint32_t slk, uint32_t key, uint32_t lim, auto&& sink) {
+    uint32_t h = ((c | (slk << 16)) * kGold) >> kHashShift;
+    const uint32_t want = c << 16;
+    for (;;) {
+      const uint4 e = *reinterpret_cast<const uint4*>(tab + 4u * h);
+      const uint32_t es[4] = {e.x, e.y, e.z, e.w & ~0x8000u};
+#pragma unroll
+      for (int s = 0; s < 4; ++s) {
+        const uint32_t d = (es[s] ^ want) - 1u;
+        if (d < lim) {
+          const uint32_t kj = recS[d].x;
+          if (absdiff_u32(kj, key) <= a.W) sink(d);
         }
       }
+      if (!(e.w & 0x8000u)) break;
+      h = (h + 1u) & (NB - 1u);
     }
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      if ((uint32_t)i < ncand) unite((cand[i >> 1] >> ((i & 1) * 16)) & 0xFFFFu);
+  };
+  auto push_link = [&](uint32_t k, uint32_t j) {
+    const uint32_t pos = atomicAdd(&misc->n_list, 1u);
+    if (pos < (uint32_t)L::kListCap) list[pos] = (k << 16) | j;
+  };
+  for (uint32_t k0 = 0; k0 < mm; k0 += THREADS) {
+    const uint32_t k = k0 + tid;
+    if (k < mm) {
+      const uint2 r = recS[k];
+      const uint32_t key = r.x, cell = r.y & 0xFFFFu, slk = key >> tb, hs = slk << 16;
+      const uint32_t x = cell & 0xFFu, y = cell >> 8;
+      const bool xe = x + 1u < a.sensor_w, xw = x > 0u, ys = y + 1u < a.sensor_h;
+      uint32_t slow = 0;
+      // one forward cell: candidate index (or k), its key, and whether it passed the time test
+      auto probe = [&](uint32_t off, bool valid, uint32_t lim, uint32_t bit, uint32_t& jc, uint32_t& kc) -> bool {
+        const uint32_t c = cell + off;
+        const uint32_t h = ((c | hs) * kGold) >> kHashShift;
+        const uint4 e = *reinterpret_cast<const uint4*>(tab + 4u * h);
+        const uint32_t want = c << 16;
+        const uint32_t d0 = (e.x ^ want) - 1u, d1 = (e.y ^ want) - 1u, d2 = (e.z ^ want) - 1u,
+                       d3 = ((e.w & ~0x8000u) ^ want) - 1u;
+        const bool m0 = d0 < lim, m1 = d1 < lim, m2 = d2 < lim, m3 = d3 < lim;
+        const uint32_t nm = (uint32_t)m0 + (uint32_t)m1 + (uint32_t)m2 + (uint32_t)m3;
+        const uint32_t j = m0 ? d0 : (m1 ? d1 : (m2 ? d2 : d3));
+        const bool any = valid && nm != 0u;
+        jc = any ? j : k;
+        kc = recS[jc].x;
+        if (valid && (nm > 1u || (e.w & 0x8000u))) slow |= bit;
+        return any && absdiff_u32(kc, key) <= a.W;
+      };
+      uint32_t jS, kS, jE, kE, jSE, kSE, jSW, kSW, jO, kO;
+      const bool pS = probe(256u, ys, (uint32_t)T, 1u, jS, kS);
+      const bool pE = probe(1u, xe, (uint32_t)T, 2u, jE, kE);
+      const bool pSE = probe(257u, xe && ys, (uint32_t)T, 4u, jSE, kSE);
+      const bool pSW = probe(255u, xw && ys, (uint32_t)T, 8u, jSW, kSW);
+      const bool pO = probe(0u, true, k, 16u, jO, kO);   // own cell: only earlier events (d < k)
+      // A candidate c is dropped when another candidate a of this event is adjacent to c in space
+      // (fixed by the cell geometry) and in time: the pair (a, c) is linked by a or c itself.
+      const uint32_t W = a.W;
+      const bool keepS = pS;
+      const bool keepE = pE && !(pS && absdiff_u32(kE, kS) <= W);
+      const bool keepSE = pSE && !(pS && absdiff_u32(kSE, kS) <= W) && !(pE && absdiff_u32(kSE, kE) <= W);
+      const bool keepSW = pSW && !(pS && absdiff_u32(kSW, kS) <= W);
+      const bool keepO = pO && !(pS && absdiff_u32(kO, kS) <= W) && !(pE && absdiff_u32(kO, kE) <= W) &&
+                         !(pSE && absdiff_u32(kO, kSE) <= W) && !(pSW && absdiff_u32(kO, kSW) <= W);
+      uint32_t parent = k;
+      bool have = false;
+      auto take = [&](bool keep, uint32_t j) {
+        if (keep) {
+          if (!have) { parent = j; have = true; }
+          else push_link(k, j);
+        }
+      };
+      take(keepS, jS);
+      take(keepE, jE);
+      take(keepSE, jSE);
+      take(keepSW, jSW);
+      take(keepO, jO);
+      par[k] = (uint16_t)parent;
+      // rare: a neighbour cell holds several events, or its bucket overflowed: link them all
+      while (slow) {
+        const uint32_t q = (uint32_t)__ffs(slow) - 1u;
+        slow &= slow - 1u;
+        const uint32_t off = q == 0u ? 256u : (q == 1u ? 1u : (q == 2u ? 257u : (q == 3u ? 255u : 0u)));
+        scan_cell(cell + off, slk, key, q == 4u ? k : (uint32_t)T, [&](uint32_t j) { push_link(k, j); });
+      }
     }
   }
   __syncthreads();
-
-  uint32_t* head = reinterpret_cast<uint32_t*>(smem + L::kRegC);   // [T] member chain head per root (nextc is dead)
-  // ---- S3: label = root (smallest sorted index of the component); ordinals of the roots ---------
+  // ---- deferred links: union by compare-and-swap hooks ---------------------------------------------
   {
-    uint32_t root_r[IPT];
-#pragma unroll
-    for (int j = 0; j < IPT; ++j) {
-      const uint32_t k = (uint32_t)j * THREADS + tid;
-      uint32_t r = k;
-      if (k < mm) {
-        uint32_t p;
-        while ((p = parent[r]) != r) r = p;
+    const uint32_t nl = misc->n_list;
+    if (nl > (uint32_t)L::kListCap) {
+      // the list overflowed (very dense tile): redo the probes, uniting on the spot
+      for (uint32_t k = tid; k < mm; k += THREADS) {
+        const uint2 r = recS[k];
+        const uint32_t key = r.x, cell = r.y & 0xFFFFu, slk = key >> tb;
+        const uint32_t x = cell & 0xFFu, y = cell >> 8;
+        const bool xe = x + 1u < a.sensor_w, xw = x > 0u, ys = y + 1u < a.sensor_h;
+        auto un = [&](uint32_t j) { uf_unite(par, k, j); };
+        if (ys) scan_cell(cell + 256u, slk, key, (uint32_t)T, un);
+        if (xe) scan_cell(cell + 1u, slk, key, (uint32_t)T, un);
+        if (xe && ys) scan_cell(cell + 257u, slk, key, (uint32_t)T, un);
+        if (xw && ys) scan_cell(cell + 255u, slk, key, (uint32_t)T, un);
+        scan_cell(cell, slk, key, k, un);
       }
-      root_r[j] = r;
-    }
-    __syncthreads();
-#pragma unroll
-    for (int j = 0; j < IPT; ++j) {
-      const uint32_t k = (uint32_t)j * THREADS + tid;
-      if (k < mm) {
-        parent[k] = root_r[j];
-        head[k] = kNone;
-        a.label[out_base + k] = out_base + root_r[j];
+      __syncthreads();
+    } else {
+      for (uint32_t i = tid; i < nl; i += THREADS) {
+        const uint32_t e = list[i];
+        uf_unite(par, e >> 16, e & 0xFFFFu);
       }
     }
   }
+  __syncthreads();   // the hash table is dead from here on
+
+  // ---- S3: label = smallest sorted index of the component ------------------------------------------
+  uint32_t* minidx = reinterpret_cast<uint32_t*>(hreg);                 // [T] by root
+  uint32_t* head = reinterpret_cast<uint32_t*>(hreg + 4 * T);           // [T] member chain head per label
+  uint16_t* lab = reinterpret_cast<uint16_t*>(hreg + 8 * T);            // [T] label per event
+  uint16_t* rootpos = reinterpret_cast<uint16_t*>(hreg + 10 * T);       // [T] ordinal -> label
+  uint16_t* nxt = reinterpret_cast<uint16_t*>(hreg + 12 * T);           // [T] next member of the same hit
+  {
+    uint4* f = reinterpret_cast<uint4*>(hreg);
+    const uint4 ones = make_uint4(kNone, kNone, kNone, kNone);
+#pragma unroll
+    for (int q = 0; q < 8 * T / 16 / THREADS; ++q) f[q * THREADS + tid] = ones;   // minidx and head
+  }
+  uint32_t root_r[IPT];
+#pragma unroll
+  for (int j = 0; j < IPT; ++j) {
+    const uint32_t k = (uint32_t)j * THREADS + tid;
+    root_r[j] = k < mm ? uf_find(par, k) : 0u;
+  }
   __syncthreads();
-  uint16_t* nxt = reinterpret_cast<uint16_t*>(freeR);            // [T] next member of the same hit
-  uint16_t* rootpos = reinterpret_cast<uint16_t*>(freeR + 2 * T);  // [T] ordinal -> sorted index of the root
+#pragma unroll
+  for (int j = 0; j < IPT; ++j) {
+    const uint32_t k = (uint32_t)j * THREADS + tid;
+    if (k < mm) atomicMin(&minidx[root_r[j]], k);
+  }
+  __syncthreads();
+#pragma unroll
+  for (int j = 0; j < IPT; ++j) {
+    const uint32_t k = (uint32_t)j * THREADS + tid;
+    if (k < mm) {
+      const uint32_t l = minidx[root_r[j]];
+      lab[k] = (uint16_t)l;
+      a.label[out_base + k] = out_base + l;
+      if (l != k) nxt[k] = (uint16_t)atomicExch(&head[l], k);   // kNone truncates to 0xFFFF = end
+    }
+  }
+  __syncthreads();
   uint32_t n_roots;
   {
     // blocked arrangement: thread owns sorted positions [8 tid, 8 tid + 8)
-    const uint4 q0 = *reinterpret_cast<const uint4*>(parent + p0);
-    const uint4 q1 = *reinterpret_cast<const uint4*>(parent + p0 + 4);
-    const uint32_t pr[IPT] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w};
+    const uint4 q0 = *reinterpret_cast<const uint4*>(lab + p0);
+    const uint32_t lw[4] = {q0.x, q0.y, q0.z, q0.w};
     uint32_t flags = 0, cntr = 0;
 #pragma unroll
-    for (int j = 0; j < IPT; ++j)
-      if (p0 + j < mm && pr[j] == p0 + j) { flags |= 1u << j; ++cntr; }
+    for (int j = 0; j < IPT; ++j) {
+      const uint32_t l = (lw[j >> 1] >> ((j & 1) * 16)) & 0xFFFFu;
+      if (p0 + j < mm && l == p0 + j) { flags |= 1u << j; ++cntr; }
+    }
     uint32_t inc = cntr;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -613,13 +747,10 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
   if (tid == 0) {
     st_volatile_u64(a.tiles + b, (b == 0 ? kTilePrefix : kTileAggregate) | (unsigned long long)n_roots);
   }
+  __syncthreads();   // rootpos complete
 
-  // ---- S4: chain every member to its root --------------------------------------------------------
-  for (uint32_t k = tid; k < mm; k += THREADS) {
-    const uint32_t r = parent[k];
-    if (r != k) nxt[k] = (uint16_t)atomicExch(&head[r], k);   // kNone truncates to 0xFFFF = end
-  }
-  // ---- ordinal of this tile's first hit: decoupled look-back over the predecessors (warp 0) ----
+  // ---- ordinal of this tile's first hit: decoupled look-back over the predecessors (warp 0);
+  //      the other warps already walk their chains ----------------------------------------------------
   if (warp == 0 && b > 0) {
     uint32_t prefix = 0;
     int jb = (int)b - 1;
@@ -627,7 +758,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
       const int idx = jb - (int)lane;
       unsigned long long v = kTilePrefix;   // before tile 0: an empty prefix
       if (idx >= 0) {
-        while (((v = ld_volatile_u64(a.tiles + idx)) >> 62) == 0ull) __nanosleep(64);
+        while (((v = ld_volatile_u64(a.tiles + idx)) >> 62) == 0ull) __nanosleep(40);
       }
       const uint32_t pm = __ballot_sync(0xffffffffu, (v >> 62) == 2ull);
       const uint32_t first = pm ? (uint32_t)__ffs(pm) - 1u : 31u;   // nearest predecessor holding a prefix
@@ -643,42 +774,51 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
       st_volatile_u64(a.tiles + b, kTilePrefix | (unsigned long long)(prefix + n_roots));
     }
   }
-  __syncthreads();
 
   // ---- S4/S5: one thread per hit walks its chain: exact sums, brightest pixel, centroid ---------
   {
-    const uint32_t ord_base = misc->ord_base;
-    const uint32_t tof_mask = (tof_bits >= 32u) ? 0xFFFFFFFFu : ((1u << tof_bits) - 1u);
     bool over = false;
-    for (uint32_t c = tid; c < n_roots; c += THREADS) {
-      const uint32_t r = rootpos[c];
+    uint32_t ord_base = 0;
+    for (uint32_t c0 = 0; c0 < n_roots || c0 == 0; c0 += THREADS) {   // block-uniform trip count, >= 1
+      const uint32_t c = c0 + tid;
       unsigned long long st = 0, sx = 0, sy = 0;
-      uint32_t size = 0, best = 0, k = r;
-      do {
-        const uint32_t cell = xyS[k], t = totS[k];
-        st += t;
-        sx += (unsigned long long)(t * (cell & 0xFFu));
-        sy += (unsigned long long)(t * (cell >> 8));
-        ++size;
-        best = max(best, (t << 16) | k);   // (ToT, sorted index): the later pixel wins ties
-        if (k == r) k = head[r];
-        else { const uint32_t nk = nxt[k]; k = (nk == 0xFFFFu) ? kNone : nk; }
-      } while (k != kNone);
-      const uint64_t o = (uint64_t)ord_base + c;
-      if (o < a.max_clusters) {
-        const uint32_t kp = best & 0xFFFFu, keyp = keyS[kp];
-        a.out.label[o] = out_base + r;
-        a.out.size[o] = size;
-        a.out.shot[o] = (uint32_t)(s_lo + (uint64_t)(keyS[r] >> tof_bits));
-        a.out.sum_tot[o] = (long long)st;
-        a.out.sum_tot_x[o] = (long long)sx;
-        a.out.sum_tot_y[o] = (long long)sy;
-        a.out.toa_peak[o] = (s_lo + (uint64_t)(keyp >> tof_bits)) * a.P + (uint64_t)(keyp & tof_mask);
-        const float fst = __ll2float_rn((long long)st);
-        a.out.cx[o] = __fdiv_rn(__ll2float_rn((long long)sx), fst);
-        a.out.cy[o] = __fdiv_rn(__ll2float_rn((long long)sy), fst);
-      } else {
-        over = true;
+      uint32_t size = 0, best = 0, r = 0;
+      if (c < n_roots) {
+        r = rootpos[c];
+        uint32_t k = r;
+        do {
+          const uint32_t w1 = recS[k].y;
+          const uint32_t t = w1 >> 16;
+          st += t;
+          sx += (unsigned long long)(t * (w1 & 0xFFu));
+          sy += (unsigned long long)(t * ((w1 >> 8) & 0xFFu));
+          ++size;
+          best = max(best, (t << 16) | k);   // (ToT, sorted index): the later pixel wins ties
+          if (k == r) k = head[r];
+          else { const uint32_t nk = nxt[k]; k = (nk == 0xFFFFu) ? kNone : nk; }
+        } while (k != kNone);
+      }
+      if (c0 == 0) {
+        __syncthreads();   // the look-back result
+        ord_base = misc->ord_base;
+      }
+      if (c < n_roots) {
+        const uint64_t o = (uint64_t)ord_base + c;
+        if (o < a.max_clusters) {
+          const uint32_t keyp = recS[best & 0xFFFFu].x, keyr = recS[r].x;
+          a.out.label[o] = out_base + r;
+          a.out.size[o] = size;
+          a.out.shot[o] = (uint32_t)(s_base + (uint64_t)(keyr >> tb));
+          a.out.sum_tot[o] = (long long)st;
+          a.out.sum_tot_x[o] = (long long)sx;
+          a.out.sum_tot_y[o] = (long long)sy;
+          a.out.toa_peak[o] = ref + (uint64_t)(keyp >> tb) * a.P + (uint64_t)(keyp & tmask);
+          const float fst = __ll2float_rn((long long)st);
+          a.out.cx[o] = __fdiv_rn(__ll2float_rn((long long)sx), fst);
+          a.out.cy[o] = __fdiv_rn(__ll2float_rn((long long)sy), fst);
+        } else {
+          over = true;
+        }
       }
     }
     if (over) set_error(a.ctrl, TPX3_ERR_CAPACITY);
@@ -715,7 +855,7 @@ struct FusedGeom {
 
 inline FusedGeom fused_geom(uint64_t P, uint32_t W, uint32_t max_shot_hits) {
   FusedGeom g{0, 0, 0};
-  if (P == 0 || P > (1ull << 24) || W >= (1u << 24)) return g;   // ToF must fit the 32-bit composite key
+  if (P == 0 || P > (1ull << 24) || W >= (1u << 24)) return g;   // tof + W must fit the 32-bit tile key
   const uint32_t Lh = max_shot_hits ? max_shot_hits : 4096u;
   if (Lh <= 1024u) { g.variant = 1; g.T = 4096; }
   else if (Lh <= 4096u) { g.variant = 2; g.T = 8192; }
@@ -752,6 +892,7 @@ inline int enqueue_fused(const FusedGeom& g, uint64_t* launches, Ctrl* ctrl, uns
   a.n = prm.n;
   a.P = prm.P;
   a.divP = make_div64(prm.P);
+  a.divP32 = make_div32((uint32_t)prm.P);
   a.W = prm.W;
   a.S = g.S;
   a.num_tiles = (uint32_t)((prm.n + g.S - 1) / g.S);
