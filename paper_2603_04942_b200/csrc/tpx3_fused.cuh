@@ -10,8 +10,9 @@
 //   events (L = the largest shot the variant supports) to reach the end of its last shot. The
 //   global sorted position of an event is tile start + local rank: perm and label need no
 //   inter-tile communication. Only the ordinal of a hit in the ascending-label cluster table
-//   needs a prefix over tiles: a decoupled look-back over per-tile status words (tiles are
-//   handed out by an atomic ticket, so every predecessor of a running tile has started).
+//   needs a prefix over tiles: tiles write their hits to a staging table at their own position
+//   and a small second kernel (k_fused_compact) moves them to their ordinals, so that no tile
+//   ever waits for another one (a look-back inside the kernel cost 24-59 % of the warp time).
 //
 // Per tile (all in shared memory, one CTA; k = sorted position inside the tile):
 //   load     128-bit coalesced loads of toa / x / y / tot. rel = toa - (first shot of the tile)*P
@@ -32,7 +33,7 @@
 //            atomicMin per event), ordinals of the labels by block scan (S3)
 //   reduce   members chained to their label (one atomicExch each); one thread per hit walks the
 //            chain: exact 64-bit sums, brightest pixel by (ToT, sorted index) (S4)
-//   centroid fp32(sum tot*x) / fp32(sum tot), IEEE RN (S5, Eq. 9)
+//   centroid fp32(sum tot*x) / fp32(sum tot), IEEE RN (S5, Eq. 9), in k_fused_compact
 //
 // A tile that cannot be handled (a shot longer than L, a decreasing shot number, shot offset and
 // time of flight too wide for one 32-bit key) marks the call as failed; the general kernels, enqueued behind this one,
@@ -104,20 +105,6 @@ __device__ __forceinline__ uint32_t div32(uint32_t n, const Div32& d) {
   return (t + ((n - t) >> d.sh1)) >> d.sh2;
 }
 
-// ---- tile status words for the decoupled look-back -------------------------------------------
-constexpr unsigned long long kTileAggregate = 1ull << 62;  // value = hits of this tile
-constexpr unsigned long long kTilePrefix = 2ull << 62;     // value = hits of tiles 0..this
-constexpr unsigned long long kTileValueMask = 0xFFFFFFFFull;
-
-__device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned long long* p) {
-  unsigned long long v;
-  asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p));
-  return v;
-}
-__device__ __forceinline__ void st_volatile_u64(unsigned long long* p, unsigned long long v) {
-  asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
-
 __device__ __forceinline__ uint4 ldg_nc_v4(const void* p) {
   uint4 r;
   asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
@@ -147,6 +134,9 @@ struct FusedArgs {
   uint64_t max_clusters;
   tpx3_clusters_t out;
   uint32_t* n_clusters;
+  uint4* stage_a;      // staging table, indexed by sorted position: {label, size, sum tot, -}
+  uint4* stage_b;      //                                            {sum tot*x (lo, hi), sum tot*y (lo, hi)}
+  uint64_t* stage_c;   //                                            ToA of the brightest pixel
 };
 
 constexpr uint32_t kNone = 0xFFFFFFFFu;
@@ -177,9 +167,7 @@ struct FusedMisc {
   unsigned int lo, hi;         // owned range, relative to the tile base
   unsigned int fail;
   unsigned int max_tof, max_sl;
-  unsigned int ticket;
   unsigned int n_roots;
-  unsigned int ord_base;
   unsigned int n_list;         // deferred links pushed (may exceed the capacity: overflow)
   unsigned int warp_sums[33];
 };
@@ -229,20 +217,17 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
   FusedMisc* misc = reinterpret_cast<FusedMisc*>(smem + L::kMisc);
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
 
-  // ---- ticket: tiles are processed in start order (look-back needs started predecessors) ----
   if (tid == 0) {
-    misc->ticket = atomicAdd(&a.ctrl->tile_ticket, 1u);
     misc->lo = kNone;
     misc->hi = kNone;
     misc->fail = 0;
     misc->max_tof = 0;
     misc->max_sl = 0;
     misc->n_roots = 0;
-    misc->ord_base = 0;
     misc->n_list = 0;
   }
   __syncthreads();
-  const uint32_t b = misc->ticket;
+  const uint32_t b = blockIdx.x;
   const uint64_t base = (uint64_t)b * a.S;             // first event this tile looks at
   const uint64_t avail = a.n - base;                   // > 0 by construction
   const uint32_t cnt = avail < (uint64_t)T ? (uint32_t)avail : (uint32_t)T;  // events readable
@@ -743,107 +728,110 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
       if (flags & (1u << j)) rootpos[ord++] = (uint16_t)(p0 + j);
     n_roots = misc->n_roots;
   }
-  // publish this tile's hit count as early as possible
-  if (tid == 0) {
-    st_volatile_u64(a.tiles + b, (b == 0 ? kTilePrefix : kTileAggregate) | (unsigned long long)n_roots);
-  }
   __syncthreads();   // rootpos complete
 
-  // ---- ordinal of this tile's first hit: decoupled look-back over the predecessors (warp 0);
-  //      the other warps already walk their chains ----------------------------------------------------
-  if (warp == 0 && b > 0) {
-    uint32_t prefix = 0;
-    int jb = (int)b - 1;
-    for (;;) {
-      const int idx = jb - (int)lane;
-      unsigned long long v = kTilePrefix;   // before tile 0: an empty prefix
-      if (idx >= 0) {
-        while (((v = ld_volatile_u64(a.tiles + idx)) >> 62) == 0ull) __nanosleep(40);
-      }
-      const uint32_t pm = __ballot_sync(0xffffffffu, (v >> 62) == 2ull);
-      const uint32_t first = pm ? (uint32_t)__ffs(pm) - 1u : 31u;   // nearest predecessor holding a prefix
-      uint32_t val = lane <= first ? (uint32_t)(v & kTileValueMask) : 0u;
-#pragma unroll
-      for (int o = 16; o; o >>= 1) val += __shfl_xor_sync(0xffffffffu, val, o);
-      prefix += val;
-      if (pm) break;
-      jb -= 32;
-    }
-    if (lane == 0) {
-      misc->ord_base = prefix;
-      st_volatile_u64(a.tiles + b, kTilePrefix | (unsigned long long)(prefix + n_roots));
-    }
-  }
-
-  // ---- S4/S5: one thread per hit walks its chain: exact sums, brightest pixel, centroid ---------
-  {
-    bool over = false;
-    uint32_t ord_base = 0;
-    for (uint32_t c0 = 0; c0 < n_roots || c0 == 0; c0 += THREADS) {   // block-uniform trip count, >= 1
-      const uint32_t c = c0 + tid;
-      unsigned long long st = 0, sx = 0, sy = 0;
-      uint32_t size = 0, best = 0, r = 0;
-      if (c < n_roots) {
-        r = rootpos[c];
-        uint32_t k = r;
-        do {
-          const uint32_t w1 = recS[k].y;
-          const uint32_t t = w1 >> 16;
-          st += t;
-          sx += (unsigned long long)(t * (w1 & 0xFFu));
-          sy += (unsigned long long)(t * ((w1 >> 8) & 0xFFu));
-          ++size;
-          best = max(best, (t << 16) | k);   // (ToT, sorted index): the later pixel wins ties
-          if (k == r) k = head[r];
-          else { const uint32_t nk = nxt[k]; k = (nk == 0xFFFFu) ? kNone : nk; }
-        } while (k != kNone);
-      }
-      if (c0 == 0) {
-        __syncthreads();   // the look-back result
-        ord_base = misc->ord_base;
-      }
-      if (c < n_roots) {
-        const uint64_t o = (uint64_t)ord_base + c;
-        if (o < a.max_clusters) {
-          const uint32_t keyp = recS[best & 0xFFFFu].x, keyr = recS[r].x;
-          a.out.label[o] = out_base + r;
-          a.out.size[o] = size;
-          a.out.shot[o] = (uint32_t)(s_base + (uint64_t)(keyr >> tb));
-          a.out.sum_tot[o] = (long long)st;
-          a.out.sum_tot_x[o] = (long long)sx;
-          a.out.sum_tot_y[o] = (long long)sy;
-          a.out.toa_peak[o] = ref + (uint64_t)(keyp >> tb) * a.P + (uint64_t)(keyp & tmask);
-          const float fst = __ll2float_rn((long long)st);
-          a.out.cx[o] = __fdiv_rn(__ll2float_rn((long long)sx), fst);
-          a.out.cy[o] = __fdiv_rn(__ll2float_rn((long long)sy), fst);
-        } else {
-          over = true;
-        }
-      }
-    }
-    if (over) set_error(a.ctrl, TPX3_ERR_CAPACITY);
+  // ---- S4: one thread per hit walks its chain: exact sums, brightest pixel. The hit goes to the
+  //      staging table at the tile's own position out_base + c (a tile has no more hits than events);
+  //      k_fused_compact moves it to its ordinal once every tile's count is known -------------------
+  for (uint32_t c = tid; c < n_roots; c += THREADS) {
+    const uint32_t r = rootpos[c];
+    unsigned long long sx = 0, sy = 0;
+    uint32_t st = 0, size = 0, best = 0, k = r;
+    do {
+      const uint32_t w1 = recS[k].y;
+      const uint32_t t = w1 >> 16;
+      st += t;                                             // <= 65535 * 8192 < 2^32
+      sx += (unsigned long long)(t * (w1 & 0xFFu));
+      sy += (unsigned long long)(t * ((w1 >> 8) & 0xFFu));
+      ++size;
+      best = max(best, (t << 16) | k);   // (ToT, sorted index): the later pixel wins ties
+      if (k == r) k = head[r];
+      else { const uint32_t nk = nxt[k]; k = (nk == 0xFFFFu) ? kNone : nk; }
+    } while (k != kNone);
+    const uint32_t keyp = recS[best & 0xFFFFu].x;
+    const uint64_t o = (uint64_t)out_base + c;
+    a.stage_a[o] = make_uint4(out_base + r, size, st, 0u);
+    a.stage_b[o] = make_uint4((uint32_t)sx, (uint32_t)(sx >> 32), (uint32_t)sy, (uint32_t)(sy >> 32));
+    a.stage_c[o] = ref + (uint64_t)(keyp >> tb) * a.P + (uint64_t)(keyp & tmask);
   }
 
   // ---- completion: the last tile to finish publishes the outcome of the call --------------------
   if (tid == 0) {
+    a.tiles[b] = ((unsigned long long)out_base << 32) | (unsigned long long)n_roots;
     if (failed) atomicExch(&a.ctrl->fused_fail, 1u);
     __threadfence();
     const uint32_t done = atomicAdd(&a.ctrl->tiles_done, 1u);
     if (done + 1u == a.num_tiles) {
       __threadfence();
       const uint32_t any_fail = atomicAdd(&a.ctrl->fused_fail, 0u);
-      if (any_fail) {
-        a.ctrl->fused_state = 2;   // the general kernels behind this one redo the call
-        if (a.ctrl->status.error == (uint32_t)(-TPX3_ERR_CAPACITY)) a.ctrl->status.error = 0;
-      } else {
-        const uint32_t total = (uint32_t)(ld_volatile_u64(a.tiles + (a.num_tiles - 1u)) & kTileValueMask);
-        *a.n_clusters = total;
-        a.ctrl->status.n_clusters = total;
-        a.ctrl->status.path = 1;
-        a.ctrl->status.sort_passes = 0;
-        a.ctrl->fused_state = 1;
-      }
+      // 2: the general kernels behind this one redo the call; 1: k_fused_compact finishes it
+      a.ctrl->fused_state = any_fail ? 2u : 1u;
     }
+  }
+}
+
+// ---- S5 + ordering: staging table -> cluster table -----------------------------------------------
+// Runs behind k_fused_shot_tiles (same stream), so every tile's hit count is final: no tile waits
+// for another one. CTA i takes a contiguous range of tiles, sums the counts of all tiles before
+// its range (the tile words are a few hundred KB and L2-resident) and copies its tiles' hits to
+// their ordinals, ascending label order. Also computes what needs no tile state: shot = ToA of
+// the brightest pixel div P (the pixel belongs to the hit's shot, R6) and the centroid
+// fp32(sum tot*x) / fp32(sum tot), IEEE RN (Eq. 9).
+constexpr int kCompactThreads = 256;
+
+__global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, uint32_t tiles_per_cta) {
+  if (a.ctrl->fused_state != 1u) return;   // the fused kernel gave up: the general path redoes the call
+  __shared__ unsigned long long s_part[kCompactThreads / 32];
+  __shared__ unsigned long long s_prefix;
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  const uint32_t t0 = blockIdx.x * tiles_per_cta;
+  const uint32_t t1 = min(t0 + tiles_per_cta, a.num_tiles);
+  if (t0 >= a.num_tiles) return;
+  unsigned long long sum = 0;
+  for (uint32_t t = tid; t < t0; t += kCompactThreads) sum += a.tiles[t] & 0xFFFFFFFFull;
+#pragma unroll
+  for (int o = 16; o; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+  if (lane == 0) s_part[warp] = sum;
+  __syncthreads();
+  if (tid == 0) {
+    unsigned long long p = 0;
+    for (int w = 0; w < kCompactThreads / 32; ++w) p += s_part[w];
+    s_prefix = p;
+  }
+  __syncthreads();
+  unsigned long long prefix = s_prefix;
+  bool over = false;
+  for (uint32_t t = t0; t < t1; ++t) {
+    const unsigned long long w = a.tiles[t];
+    const uint32_t cnt = (uint32_t)(w & 0xFFFFFFFFull);
+    const uint64_t src = w >> 32;
+    for (uint32_t c = tid; c < cnt; c += kCompactThreads) {
+      const uint64_t o = prefix + c;
+      if (o >= a.max_clusters) { over = true; continue; }
+      const uint4 va = a.stage_a[src + c], vb = a.stage_b[src + c];
+      const uint64_t toa_peak = a.stage_c[src + c];
+      const long long st = (long long)va.z;
+      const long long sx = (long long)(((unsigned long long)vb.y << 32) | vb.x);
+      const long long sy = (long long)(((unsigned long long)vb.w << 32) | vb.z);
+      a.out.label[o] = va.x;
+      a.out.size[o] = va.y;
+      a.out.shot[o] = (uint32_t)div64(toa_peak, a.divP);
+      a.out.sum_tot[o] = st;
+      a.out.sum_tot_x[o] = sx;
+      a.out.sum_tot_y[o] = sy;
+      a.out.toa_peak[o] = toa_peak;
+      const float fst = __ll2float_rn(st);
+      a.out.cx[o] = __fdiv_rn(__ll2float_rn(sx), fst);
+      a.out.cy[o] = __fdiv_rn(__ll2float_rn(sy), fst);
+    }
+    prefix += cnt;
+  }
+  if (over) set_error(a.ctrl, TPX3_ERR_CAPACITY);
+  if (t1 == a.num_tiles && tid == 0) {
+    *a.n_clusters = (uint32_t)prefix;
+    a.ctrl->status.n_clusters = (uint32_t)prefix;
+    a.ctrl->status.path = 1;
+    a.ctrl->status.sort_passes = 0;
   }
 }
 
@@ -881,7 +869,8 @@ inline int launch_fused(const FusedArgs& a, cudaStream_t st) {
 inline int enqueue_fused(const FusedGeom& g, uint64_t* launches, Ctrl* ctrl, unsigned long long* tiles,
                          cudaStream_t st, const Params& prm, const uint16_t* x, const uint16_t* y,
                          const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label,
-                         uint64_t max_clusters, const tpx3_clusters_t& out, uint32_t* n_clusters, bool* launched) {
+                         uint64_t max_clusters, const tpx3_clusters_t& out, uint32_t* n_clusters, void* stage,
+                         bool* launched) {
   *launched = false;
   if (g.variant == 0 || prm.n == 0) return TPX3_OK;
   // the 128-bit load phase needs 16-byte aligned inputs (PyTorch allocations are 256-byte aligned)
@@ -904,9 +893,21 @@ inline int enqueue_fused(const FusedGeom& g, uint64_t* launches, Ctrl* ctrl, uns
   a.max_clusters = max_clusters;
   a.out = out;
   a.n_clusters = n_clusters;
+  // staging table: 40 bytes per event position (aliases the general path's sort buffers)
+  a.stage_a = reinterpret_cast<uint4*>(stage);
+  a.stage_b = a.stage_a + prm.n;
+  a.stage_c = reinterpret_cast<uint64_t*>(a.stage_b + prm.n);
   int rc = g.variant == 1 ? launch_fused<4096, 512>(a, st) : launch_fused<8192, 1024>(a, st);
-  if (rc == TPX3_OK) { ++*launches; *launched = true; }
-  return rc;
+  if (rc != TPX3_OK) return rc;
+  ++*launches;
+  uint32_t ctas = a.num_tiles < (uint32_t)(kNumSMs * 8) ? a.num_tiles : (uint32_t)(kNumSMs * 8);
+  const uint32_t tiles_per_cta = (a.num_tiles + ctas - 1) / ctas;
+  ctas = (a.num_tiles + tiles_per_cta - 1) / tiles_per_cta;
+  k_fused_compact<<<ctas, kCompactThreads, 0, st>>>(a, tiles_per_cta);
+  if (cudaGetLastError() != cudaSuccess) return TPX3_ERR_CUDA;
+  ++*launches;
+  *launched = true;
+  return TPX3_OK;
 }
 
 }  // namespace tpx3

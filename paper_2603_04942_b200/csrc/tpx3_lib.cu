@@ -214,6 +214,8 @@ int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace
   p->off_slab = o; o = align_up(o + 8 * N);
   p->off_table = o; o = align_up(o + 4 * (size_t)table_size_for(N));
   p->off_counts = o; o = align_up(o + 4 * (size_t)kRadix * kSortMaxBlocks);
+  // the fused path's staging table (40 bytes per event) aliases keyA .. table
+  if (p->off_counts - p->off_keyA < 40 * (size_t)N) { delete p; return TPX3_ERR_INVALID_ARG; }
   // centroid buffers alias the sort buffers (the two steps never run concurrently and the
   // centroid step takes perm/label from the caller, not from the workspace)
   p->off_slot = p->off_keyA;                    // 4N <= 8N
@@ -280,7 +282,7 @@ int tpx3_cluster_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uin
     bool launched = false;
     StageTimer timer(p, st, TPX3_STAGE_FUSED);
     rc = enqueue_fused(p->fused, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, label, max_clusters,
-                       *out, n_clusters, &launched);
+                       *out, n_clusters, (char*)workspace + p->off_keyA, &launched);
     if (rc != TPX3_OK) return rc;
   }
   // General path: every kernel below returns at once if the fused kernel succeeded.
