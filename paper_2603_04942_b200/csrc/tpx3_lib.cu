@@ -51,13 +51,6 @@ inline uint32_t table_size_for(uint64_t n) {  // power of two >= 2n, >= 1024
 
 inline int cuda_ok(cudaError_t e) { return e == cudaSuccess ? TPX3_OK : TPX3_ERR_CUDA; }
 
-inline uint32_t grid_for(uint64_t n, int threads, int num_sms, int per_sm = 8) {
-  uint64_t b = (n + threads - 1) / threads;
-  uint64_t cap = (uint64_t)num_sms * per_sm;
-  if (b > cap) b = cap;
-  return (uint32_t)(b ? b : 1);
-}
-
 // RAII bracket of one stage: records an event pair on the stream when profiling is enabled.
 struct StageTimer {
   tpx3_plan_s* p;
@@ -114,58 +107,152 @@ inline Ws carve(const tpx3_plan_s* p, void* workspace) {
   return w;
 }
 
-// ---- general path: S0-S3 ------------------------------------------------------------------
-int enqueue_general_cluster(tpx3_plan_s* p, const Ws& w, cudaStream_t st, uint64_t n, const uint16_t* x,
-                            const uint16_t* y, const uint64_t* toa, const uint16_t* tot, uint32_t* perm,
-                            uint32_t* label, uint32_t* n_clusters) {
-  Params prm = p->prm;
-  prm.n = n;
-  const int sms = p->num_sms;
-  SortBufs b;
-  SortGeom g = sort_geom(n);
-  {
-  StageTimer timer(p, st, TPX3_STAGE_SORT);
-  TPX3_LAUNCH(p, k_minmax, grid_for(n, 256 * 8, sms), 256, 0, st, w.ctrl, toa, n);
-  TPX3_LAUNCH(p, k_sort_setup, 1, 1, 0, st, w.ctrl);
-  b.key[0] = w.keyA; b.key[1] = w.keyB; b.idx[0] = w.idxA; b.idx[1] = w.idxB; b.counts = w.counts;
-  // Passes needed for the largest span a ToA can have; the ones past the device-computed
-  // `npass` return at once. 64-bit ToA => at most 8 passes.
-  for (int pass = 0; pass < kMaxPasses; ++pass) {
-    TPX3_LAUNCH(p, k_radix_hist, g.nblk, kSortThreads, 0, st, w.ctrl, pass, toa, b, n, g);
-    TPX3_LAUNCH(p, k_radix_scan, 1, 1024, 0, st, w.ctrl, pass, w.counts, (uint32_t)(kRadix * g.nblk));
-    TPX3_LAUNCH(p, k_radix_scatter, g.nblk, kSortThreads, 0, st, w.ctrl, pass, toa, b, perm, n, g);
+// ---- general path: S0-S3 (cluster) and S4-S5 (centroid) ------------------------------------------
+// Everything the general kernels need, by value: the same launch sequence is enqueued by the host
+// (tpx3_cluster, tpx3_centroid, plans without a fused variant) or, when the fused kernel gave up,
+// by k_fallback_dispatch on the device.
+struct GenArgs {
+  Ws w;
+  Params prm;            // n filled in
+  SortGeom g;
+  uint32_t tsize;        // hash table slots
+  uint32_t cent_nblk;
+  int sms;
+  int general_only;      // centroid kernels: skip when the fused path succeeded
+  const uint16_t *x, *y, *tot;
+  const uint64_t* toa;
+  uint32_t *perm, *label, *n_clusters;
+  uint64_t max_clusters;
+  tpx3_clusters_t out;
+};
+
+__host__ __device__ inline uint32_t grid_for_hd(uint64_t n, int threads, int num_sms, int per_sm = 8) {
+  uint64_t b = (n + threads - 1) / threads;
+  uint64_t cap = (uint64_t)num_sms * per_sm;
+  if (b > cap) b = cap;
+  return (uint32_t)(b ? b : 1);
+}
+
+// GP(stage, kernel, grid, block, args...) is defined by the includer (host launch or device tail launch).
+#define TPX3_GENERAL_CLUSTER_SEQUENCE(A)                                                                              \
+  do {                                                                                                                \
+    const uint64_t n_ = (A).prm.n;                                                                                    \
+    SortBufs b_;                                                                                                      \
+    b_.key[0] = (A).w.keyA; b_.key[1] = (A).w.keyB; b_.idx[0] = (A).w.idxA; b_.idx[1] = (A).w.idxB;                   \
+    b_.counts = (A).w.counts;                                                                                         \
+    GP(TPX3_STAGE_SORT, k_minmax, grid_for_hd(n_, 256 * 8, (A).sms), 256, (A).w.ctrl, (A).toa, n_);                   \
+    GP(TPX3_STAGE_SORT, k_sort_setup, 1, 1, (A).w.ctrl);                                                              \
+    /* passes needed for the largest span a ToA can have; the ones past the device-computed npass return at once */  \
+    for (int pass_ = 0; pass_ < kMaxPasses; ++pass_) {                                                                \
+      GP(TPX3_STAGE_SORT, k_radix_hist, (A).g.nblk, kSortThreads, (A).w.ctrl, pass_, (A).toa, b_, n_, (A).g);         \
+      GP(TPX3_STAGE_SORT, k_radix_scan, 1, 1024, (A).w.ctrl, pass_, (A).w.counts, (uint32_t)(kRadix * (A).g.nblk));   \
+      GP(TPX3_STAGE_SORT, k_radix_scatter, (A).g.nblk, kSortThreads, (A).w.ctrl, pass_, (A).toa, b_, (A).perm, n_,    \
+         (A).g);                                                                                                      \
+    }                                                                                                                 \
+    GP(TPX3_STAGE_LINK, k_gather, grid_for_hd(n_, 256, (A).sms), 256, (A).w.ctrl, (A).prm, (A).w.keyA, (A).w.keyB,    \
+       (A).perm, (A).x, (A).y, (A).tot, (A).w.xy, (A).w.tot, (A).w.slab, (A).label);                                  \
+    GP(TPX3_STAGE_LINK, k_fill_u32, grid_for_hd((A).tsize, 256, (A).sms), 256, (A).w.ctrl, 1, (A).w.table,            \
+       (uint64_t)(A).tsize, kEmpty);                                                                                  \
+    GP(TPX3_STAGE_LINK, k_hash_insert, grid_for_hd(n_, 256, (A).sms), 256, (A).w.ctrl, n_, (A).w.xy, (A).w.slab,      \
+       (A).w.table, (A).tsize - 1);                                                                                   \
+    GP(TPX3_STAGE_LINK, k_link, grid_for_hd(n_, 256, (A).sms), 256, (A).w.ctrl, (A).prm, (A).w.keyA, (A).w.keyB,      \
+       (A).w.xy, (A).w.slab, (A).w.table, (A).tsize - 1, (A).label);                                                  \
+    GP(TPX3_STAGE_LINK, k_compress, grid_for_hd(n_, 256, (A).sms), 256, (A).w.ctrl, n_, (A).label, (A).n_clusters);   \
+  } while (0)
+
+#define TPX3_GENERAL_CENTROID_SEQUENCE(A)                                                                             \
+  do {                                                                                                                \
+    const uint64_t n_ = (A).prm.n;                                                                                    \
+    GP(TPX3_STAGE_CENTROID, k_root_count, (A).cent_nblk, kCentThreads, (A).w.ctrl, (A).general_only, n_, (A).label,   \
+       (A).w.blkcnt);                                                                                                 \
+    GP(TPX3_STAGE_CENTROID, k_root_scan, 1, 1024, (A).w.ctrl, (A).general_only, (A).w.blkcnt, (A).cent_nblk,          \
+       (A).max_clusters, (A).n_clusters);                                                                             \
+    GP(TPX3_STAGE_CENTROID, k_root_slots, (A).cent_nblk, kCentThreads, (A).w.ctrl, (A).general_only, n_, (A).label,   \
+       (A).w.blkcnt, (A).w.slot, (A).max_clusters, (A).out, (A).w.peak);                                              \
+    GP(TPX3_STAGE_CENTROID, k_accumulate, grid_for_hd(n_, 256, (A).sms), 256, (A).w.ctrl, (A).general_only, n_,       \
+       (A).x, (A).y, (A).tot, (A).perm, (A).label, (A).w.slot, (A).max_clusters, (A).out, (A).w.peak);                \
+    GP(TPX3_STAGE_CENTROID, k_finalize,                                                                               \
+       grid_for_hd((A).max_clusters < n_ ? (A).max_clusters : n_, 256, (A).sms), 256, (A).w.ctrl, (A).general_only,   \
+       (A).prm, (A).toa, (A).perm, (A).n_clusters, (A).max_clusters, (A).out, (A).w.peak);                            \
+  } while (0)
+
+// Device-side fallback: one tiny kernel behind the fused path. If the fused kernel could not serve
+// the call it enqueues the whole general path as tail launches (they run, in order, after this grid
+// and before anything the host enqueued later on the stream). A successful fused call thus pays for
+// one empty launch instead of the 36 early-exit launches of the general path.
+__global__ void k_fallback_dispatch(GenArgs a) {
+  if (a.w.ctrl->fused_state == 1u) return;
+#define GP(stage, kernel, grid, block, ...) kernel<<<(grid), (block), 0, cudaStreamTailLaunch>>>(__VA_ARGS__)
+  TPX3_GENERAL_CLUSTER_SEQUENCE(a);
+  TPX3_GENERAL_CENTROID_SEQUENCE(a);
+#undef GP
+}
+
+GenArgs make_gen_args(tpx3_plan_s* p, const Ws& w, int general_only, uint64_t n, const uint16_t* x, const uint16_t* y,
+                      const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label, uint64_t max_clusters,
+                      const tpx3_clusters_t* out, uint32_t* n_clusters) {
+  GenArgs a;
+  memset(&a, 0, sizeof(a));
+  a.w = w;
+  a.prm = p->prm;
+  a.prm.n = n;
+  a.g = sort_geom(n);
+  a.tsize = table_size_for(n);
+  a.cent_nblk = (uint32_t)((n + kCentTile - 1) / kCentTile);
+  if (a.cent_nblk == 0) a.cent_nblk = 1;
+  a.sms = p->num_sms;
+  a.general_only = general_only;
+  a.x = x; a.y = y; a.tot = tot; a.toa = toa;
+  a.perm = perm; a.label = label; a.n_clusters = n_clusters;
+  a.max_clusters = max_clusters;
+  if (out) a.out = *out;
+  return a;
+}
+
+// Host-side enqueue with per-stage timing brackets.
+struct HostLauncher {
+  tpx3_plan_s* p;
+  cudaStream_t st;
+  int cur;
+  bool open;
+  size_t slot;
+  void enter(int stage) {
+    if (!p->profiling || (open && cur == stage)) return;
+    leave();
+    tpx3_plan_s::Span s;
+    s.stage = stage; s.a = StageTimer::take(p); s.b = StageTimer::take(p); s.launches0 = p->launches; s.launches1 = p->launches;
+    cudaEventRecord(s.a, st);
+    slot = p->spans.size();
+    p->spans.push_back(s);
+    cur = stage;
+    open = true;
   }
+  void leave() {
+    if (!open) return;
+    cudaEventRecord(p->spans[slot].b, st);
+    p->spans[slot].launches1 = p->launches;
+    open = false;
   }
-  StageTimer timer(p, st, TPX3_STAGE_LINK);
-  TPX3_LAUNCH(p, k_gather, grid_for(n, 256, sms), 256, 0, st, w.ctrl, prm, w.keyA, w.keyB, perm, x, y, tot, w.xy,
-              w.tot, w.slab, label);
-  uint32_t tsize = table_size_for(n);
-  TPX3_LAUNCH(p, k_fill_u32, grid_for(tsize, 256, sms), 256, 0, st, w.ctrl, 1, w.table, (uint64_t)tsize, kEmpty);
-  TPX3_LAUNCH(p, k_hash_insert, grid_for(n, 256, sms), 256, 0, st, w.ctrl, n, w.xy, w.slab, w.table, tsize - 1);
-  TPX3_LAUNCH(p, k_link, grid_for(n, 256, sms), 256, 0, st, w.ctrl, prm, w.keyA, w.keyB, w.xy, w.slab, w.table,
-              tsize - 1, label);
-  TPX3_LAUNCH(p, k_compress, grid_for(n, 256, sms), 256, 0, st, w.ctrl, n, label, n_clusters);
+};
+
+int enqueue_general_cluster(tpx3_plan_s* p, const GenArgs& a, cudaStream_t st) {
+  HostLauncher hl{p, st, -1, false, 0};
+#define GP(stage, kernel, grid, block, ...)                        \
+  do {                                                             \
+    hl.enter(stage);                                               \
+    kernel<<<(grid), (block), 0, st>>>(__VA_ARGS__);               \
+    ++p->launches;                                                 \
+  } while (0)
+  TPX3_GENERAL_CLUSTER_SEQUENCE(a);
+  hl.leave();
   return cuda_ok(cudaGetLastError());
 }
 
-// ---- S4-S5 from (perm, label) -------------------------------------------------------------
-int enqueue_centroid(tpx3_plan_s* p, const Ws& w, cudaStream_t st, int general_only, uint64_t n, const uint16_t* x,
-                     const uint16_t* y, const uint64_t* toa, const uint16_t* tot, const uint32_t* perm,
-                     const uint32_t* label, uint64_t max_clusters, const tpx3_clusters_t& out, uint32_t* n_clusters) {
-  Params prm = p->prm;
-  prm.n = n;
-  const int sms = p->num_sms;
-  uint32_t nblk = (uint32_t)((n + kCentTile - 1) / kCentTile);
-  if (nblk == 0) nblk = 1;
-  StageTimer timer(p, st, TPX3_STAGE_CENTROID);
-  TPX3_LAUNCH(p, k_root_count, nblk, kCentThreads, 0, st, w.ctrl, general_only, n, label, w.blkcnt);
-  TPX3_LAUNCH(p, k_root_scan, 1, 1024, 0, st, w.ctrl, general_only, w.blkcnt, nblk, max_clusters, n_clusters);
-  TPX3_LAUNCH(p, k_root_slots, nblk, kCentThreads, 0, st, w.ctrl, general_only, n, label, w.blkcnt, w.slot,
-              max_clusters, out, w.peak);
-  TPX3_LAUNCH(p, k_accumulate, grid_for(n, 256, sms), 256, 0, st, w.ctrl, general_only, n, x, y, tot, perm, label,
-              w.slot, max_clusters, out, w.peak);
-  TPX3_LAUNCH(p, k_finalize, grid_for(max_clusters < n ? max_clusters : n, 256, sms), 256, 0, st, w.ctrl,
-              general_only, prm, toa, perm, n_clusters, max_clusters, out, w.peak);
+int enqueue_centroid(tpx3_plan_s* p, const GenArgs& a, cudaStream_t st) {
+  HostLauncher hl{p, st, -1, false, 0};
+  TPX3_GENERAL_CENTROID_SEQUENCE(a);
+  hl.leave();
+#undef GP
   return cuda_ok(cudaGetLastError());
 }
 
@@ -239,7 +326,8 @@ int tpx3_cluster(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, 
   if (p->profiling) ++p->profiled_calls;
   TPX3_LAUNCH(p, k_ctrl_init, 1, 256, 0, st, w.ctrl, n, w.tiles, 0u, n_clusters);
   if (n == 0) return cuda_ok(cudaGetLastError());
-  return enqueue_general_cluster(p, w, st, n, x, y, toa, tot, perm, label, n_clusters);
+  GenArgs ga = make_gen_args(p, w, 0, n, x, y, toa, tot, perm, label, 0, nullptr, n_clusters);
+  return enqueue_general_cluster(p, ga, st);
 }
 
 int tpx3_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x, const uint16_t* y,
@@ -256,7 +344,9 @@ int tpx3_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n,
   if (p->profiling) ++p->profiled_calls;
   TPX3_LAUNCH(p, k_ctrl_init, 1, 256, 0, st, w.ctrl, n, w.tiles, 0u, n_clusters);
   if (n == 0) return cuda_ok(cudaGetLastError());
-  return enqueue_centroid(p, w, st, 0, n, x, y, toa, tot, perm, label, max_clusters, *out, n_clusters);
+  GenArgs ga = make_gen_args(p, w, 0, n, x, y, toa, tot, const_cast<uint32_t*>(perm), const_cast<uint32_t*>(label),
+                             max_clusters, out, n_clusters);
+  return enqueue_centroid(p, ga, st);
 }
 
 int tpx3_cluster_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x,
@@ -278,17 +368,23 @@ int tpx3_cluster_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uin
   Params prm = p->prm;
   prm.n = n;
   int rc = TPX3_OK;
+  GenArgs ga = make_gen_args(p, w, 1, n, x, y, toa, tot, perm, label, max_clusters, out, n_clusters);
   if (try_fused) {
     bool launched = false;
     StageTimer timer(p, st, TPX3_STAGE_FUSED);
     rc = enqueue_fused(p->fused, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, label, max_clusters,
                        *out, n_clusters, (char*)workspace + p->off_keyA, &launched);
     if (rc != TPX3_OK) return rc;
+    if (launched) {
+      // the general path, only if the fused kernel gave up: decided and enqueued on the device
+      k_fallback_dispatch<<<1, 1, 0, st>>>(ga);
+      ++p->launches;
+      return cuda_ok(cudaGetLastError());
+    }
   }
-  // General path: every kernel below returns at once if the fused kernel succeeded.
-  rc = enqueue_general_cluster(p, w, st, n, x, y, toa, tot, perm, label, n_clusters);
+  rc = enqueue_general_cluster(p, ga, st);
   if (rc != TPX3_OK) return rc;
-  return enqueue_centroid(p, w, st, 1, n, x, y, toa, tot, perm, label, max_clusters, *out, n_clusters);
+  return enqueue_centroid(p, ga, st);
 }
 
 size_t tpx3_host_io_bytes(uint64_t n, uint64_t max_clusters) {
