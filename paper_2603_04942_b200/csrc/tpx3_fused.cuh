@@ -141,6 +141,7 @@ struct FusedArgs {
 
 constexpr uint32_t kNone = 0xFFFFFFFFu;
 constexpr uint32_t kGold = 0x9E3779B1u;
+constexpr uint32_t kTaskBase = 0xFFF8u;   // deferred-list entries k << 16 | (kTaskBase + direction) are scan tasks
 
 // Shared-memory map (bytes). Records are uint2 {key, xy | tot << 16}.
 //   A [0, 8T)    sorted records (unsorted input only)            } the hash table takes the 16T bytes
@@ -619,12 +620,12 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
       take(keepSW, jSW);
       take(keepO, jO);
       par[k] = (uint16_t)parent;
-      // rare: a neighbour cell holds several events, or its bucket overflowed: link them all
+      // rare: a neighbour cell holds several events, or its bucket overflowed: all of them must be
+      // linked. Queued as a task (k, direction) so that the scans run densely packed afterwards.
       while (slow) {
         const uint32_t q = (uint32_t)__ffs(slow) - 1u;
         slow &= slow - 1u;
-        const uint32_t off = q == 0u ? 256u : (q == 1u ? 1u : (q == 2u ? 257u : (q == 3u ? 255u : 0u)));
-        scan_cell(cell + off, slk, key, q == 4u ? k : (uint32_t)T, [&](uint32_t j) { push_link(k, j); });
+        push_link(k, kTaskBase + q);
       }
     }
   }
@@ -650,7 +651,16 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
     } else {
       for (uint32_t i = tid; i < nl; i += THREADS) {
         const uint32_t e = list[i];
-        uf_unite(par, e >> 16, e & 0xFFFFu);
+        const uint32_t k = e >> 16, j = e & 0xFFFFu;
+        if (j < kTaskBase) {
+          uf_unite(par, k, j);
+        } else {                                   // task: scan one forward cell of k completely
+          const uint32_t q = j - kTaskBase;
+          const uint2 r = recS[k];
+          const uint32_t off = q == 0u ? 256u : (q == 1u ? 1u : (q == 2u ? 257u : (q == 3u ? 255u : 0u)));
+          scan_cell((r.y & 0xFFFFu) + off, r.x >> tb, r.x, q == 4u ? k : (uint32_t)T,
+                    [&](uint32_t jj) { uf_unite(par, k, jj); });
+        }
       }
     }
   }
@@ -667,6 +677,19 @@ __global__ void __launch_bounds__(THREADS, (T <= 4096 ? 2 : 1)) k_fused_shot_til
     const uint4 ones = make_uint4(kNone, kNone, kNone, kNone);
 #pragma unroll
     for (int q = 0; q < 8 * T / 16 / THREADS; ++q) f[q * THREADS + tid] = ones;   // minidx and head
+  }
+  // two rounds of pointer halving (any ancestor is a valid parent, so the plain stores may race),
+  // then the roots
+#pragma unroll
+  for (int round = 0; round < 2; ++round) {
+#pragma unroll
+    for (int j = 0; j < IPT; ++j) {
+      const uint32_t k = (uint32_t)j * THREADS + tid;
+      if (k < mm) {
+        const uint32_t p1 = par[k], g = par[p1];
+        if (g != p1) par[k] = (uint16_t)g;
+      }
+    }
   }
   uint32_t root_r[IPT];
 #pragma unroll
