@@ -309,3 +309,76 @@ def test_process_host_end_to_end(tpx3):
     g = {"perm": perm.numpy(), "label": label.numpy(), "n_clusters": ncl}
     g.update(cl.numpy(ncl))
     assert_parity(g, o, "process_host")
+
+
+# ------------------------------------------------------------------ full bench sizes
+def _full_size_check(m, w, windows, hint):
+    """The bench launch configuration (bench.py: max_hits = n, max_shot_hits = the recipe's bound) at a
+    BASELINE.json full size: sampled shot windows element by element against the oracle, plus the
+    size-independent invariants on the whole output."""
+    import torch
+
+    n = w.n
+    pl = m.plan(m.Config(max_hits=n, toa_window_ticks=W, shot_period_ticks=P, max_shot_hits=hint))
+    dev = [to_dev(a) for a in (w.x, w.y, w.toa, w.tot)]
+    cl = m.Clusters(max(n // 2, 1024), pl.device)
+    perm, label, nc = pl.cluster_centroid(*dev, cl)
+    torch.cuda.synchronize()
+    st = pl.status()
+    assert st["error"] == 0 and st["path"] == 1, st
+    ncl = int(nc.cpu().numpy()[0])
+    perm, label = perm[:n].cpu().numpy(), label[:n].cpu().numpy()
+    c = cl.numpy(ncl)
+    pl.free()
+    # invariants that hold at any size (SURVEY.md §8c)
+    k = np.arange(n, dtype=np.uint32)
+    assert np.all(label <= k) and np.array_equal(label[label], label)
+    assert int(np.count_nonzero(label == k)) == ncl
+    assert np.array_equal(c["c_label"], np.flatnonzero(label == k).astype(np.uint32))
+    assert int(c["c_size"].sum()) == n
+    assert int(c["c_sum_tot"].sum()) == int(w.tot.astype(np.int64).sum())
+    assert int(c["c_sum_tot_x"].sum()) == int((w.tot.astype(np.int64) * w.x.astype(np.int64)).sum())
+    assert int(c["c_sum_tot_y"].sum()) == int((w.tot.astype(np.int64) * w.y.astype(np.int64)).sum())
+    assert np.array_equal(np.sort(perm.astype(np.int64)), np.arange(n, dtype=np.int64))  # a permutation
+    assert np.all(np.diff(w.toa[perm].astype(np.int64)) >= 0)                             # in ToA order
+    # sampled shot windows, element by element (shots are contiguous in the stream: a window of shots
+    # is a window of input positions and of sorted positions)
+    off = w.shot_offsets
+    for s0, s1 in windows:
+        a, b = int(off[s0]), int(off[s1])
+        s = w.slice_shots(s0, s1)
+        o = oracle.run(s.x, s.y, s.toa, s.tot, W, P, threads=0)
+        what = "shots [%d, %d)" % (s0, s1)
+        np.testing.assert_array_equal(perm[a:b], o["perm"] + np.uint32(a), err_msg=what + " perm")
+        np.testing.assert_array_equal(label[a:b], o["label"] + np.uint32(a), err_msg=what + " label")
+        i0, i1 = np.searchsorted(c["c_label"], [a, b])
+        assert i1 - i0 == o["n_clusters"], what
+        np.testing.assert_array_equal(c["c_label"][i0:i1], o["c_label"] + np.uint32(a), err_msg=what)
+        for key in ("c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_toa_peak", "c_cx", "c_cy"):
+            np.testing.assert_array_equal(c[key][i0:i1], o[key], err_msg=what + " " + key)
+    return ncl
+
+
+def _windows(shots, width, count):
+    starts = np.linspace(0, shots - width, count).astype(np.int64)
+    return [(int(s), int(s) + width) for s in starts]
+
+
+def test_full_size_cfg1(tpx3):
+    """BASELINE.json configs[1] in full (100 000 shots, 3.6e7 hits): the workload bench.py times."""
+    w = gen.generate(1)
+    ncl = _full_size_check(tpx3, w, _windows(w.shots, 400, 7), gen.max_shot_hits(1))
+    assert ncl > 2_800_000
+
+
+def test_full_size_cfg4_chunk_16M(tpx3):
+    """One 2^24-hit chunk of config 4 (locally shuffled: the in-tile sort runs), bench configuration."""
+    chunk = 1 << 24
+    w = gen.generate(4, shots=chunk // 850 + 64, max_hits=chunk)
+    _full_size_check(tpx3, w, _windows(w.shots, 150, 6), gen.max_shot_hits(4))
+
+
+def test_full_size_cfg3_quarter(tpx3):
+    """A quarter of config 3 (12 500 shots, 2.6e7 hits, about 2 100 hits per shot: the 8192-event tiles)."""
+    w = gen.generate(3, shots=12500)
+    _full_size_check(tpx3, w, _windows(w.shots, 60, 5), gen.max_shot_hits(3))
