@@ -326,7 +326,7 @@ def run_ours(args):
     dom_gbs = dom_bytes / (stage_ms[dom] * 1e-3) / 1e9 if stage_ms[dom] > 0 else 0.0
     whole_bytes = STAGE_BYTES["fused"](n, ncl)
     roofline = {
-        "bound": "hbm", "kernel": {"fused": "k_fused_shot_tiles", "sort": "general path: radix sort stage",
+        "bound": "hbm", "kernel": {"fused": "fused stage: k_fused_shot_tiles (95 %) + k_fused_compact", "sort": "general path: radix sort stage",
                                    "link": "general path: gather + hash link + compress stage",
                                    "centroid": "centroid stage"}[dom],
         "achieved": dom_gbs, "peak": peak, "unit": "GB/s", "frac": dom_gbs / peak, "traffic": None,
