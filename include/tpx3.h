@@ -66,9 +66,10 @@ typedef struct {
   int32_t device;              /* CUDA device ordinal                                          */
   uint32_t flags;              /* TPX3_FLAG_*                                                  */
   uint32_t max_shot_hits;      /* hint: most events one shot can hold; sizes the fused path's
-                                  tiles (0 = 4096). <= 1024: 4096-event tiles, 2 CTAs per SM;
-                                  <= 4096: 8192-event tiles; larger, or a shot that exceeds the
-                                  hint: the general path runs (same results, slower).          */
+                                  tiles (0 = 4096). <= 512: 2048-event tiles, 4 CTAs per SM;
+                                  <= 1024: 4096-event tiles, 2 CTAs per SM; <= 4096: 8192-event
+                                  tiles; larger, or a shot that exceeds the hint: the general
+                                  path runs (same results, slower).                            */
   uint32_t reserved;           /* must be 0                                                    */
 } tpx3_config_t;
 

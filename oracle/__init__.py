@@ -41,7 +41,7 @@ def _load():
         lib = ctypes.CDLL(build())
         lib.tpx3_oracle_run.restype = ctypes.c_int
         lib.tpx3_oracle_run.argtypes = [ctypes.c_uint64] + [ctypes.c_void_p] * 4 + [
-            ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int] + [ctypes.c_void_p] * 12
+            ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int] + [ctypes.c_void_p] * 14
         _lib = lib
     return _lib
 
@@ -67,10 +67,11 @@ def run(x, y, toa, tot, W: int, P: int, threads: int = 1, clusters: bool = True)
             "c_sum_tot_x": np.empty(n, dtype=np.int64), "c_sum_tot_y": np.empty(n, dtype=np.int64),
             "c_toa_peak": np.empty(n, dtype=np.uint64), "c_cx": np.empty(n, dtype=np.float32),
             "c_cy": np.empty(n, dtype=np.float32),
+            "c_sum_tot_tof": np.empty(n, dtype=np.int64), "c_ctof": np.empty(n, dtype=np.float32),
         }
         cptr = [a.ctypes.data for a in carr.values()]
     else:
-        carr, cptr = {}, [None] * 9
+        carr, cptr = {}, [None] * 11
     rc = lib.tpx3_oracle_run(n, x.ctypes.data, y.ctypes.data, toa.ctypes.data, tot.ctypes.data,
                              int(W), int(P), int(threads), perm.ctypes.data, label.ctypes.data,
                              ctypes.addressof(nc), *cptr)

@@ -111,7 +111,7 @@ def cluster_bruteforce(x, y, toa, tot, W: int, P: int) -> dict:
     out = {
         "perm": np.array(perm, dtype=np.uint32), "label": lab.astype(np.uint32), "n_clusters": len(roots),
         "c_label": [], "c_size": [], "c_shot": [], "c_sum_tot": [], "c_sum_tot_x": [], "c_sum_tot_y": [],
-        "c_toa_peak": [], "c_cx": [], "c_cy": [],
+        "c_toa_peak": [], "c_cx": [], "c_cy": [], "c_sum_tot_tof": [], "c_ctof": [],
     }
     for r in roots:
         mem = [k for k in range(n) if lab[k] == r]
@@ -119,6 +119,7 @@ def cluster_bruteforce(x, y, toa, tot, W: int, P: int) -> dict:
         sx = sum(int(ts[k]) * int(xs[k]) for k in mem)
         sy = sum(int(ts[k]) * int(ys[k]) for k in mem)
         peak = max(mem, key=lambda k: (int(ts[k]), k))
+        sf = sum(int(ts[k]) * (tl[k] - sl[k] * P) for k in mem)  # ToF = ToA - shot*P
         out["c_label"].append(r)
         out["c_size"].append(len(mem))
         out["c_shot"].append(sl[r])
@@ -128,11 +129,14 @@ def cluster_bruteforce(x, y, toa, tot, W: int, P: int) -> dict:
         out["c_toa_peak"].append(tl[peak])
         out["c_cx"].append(np.float32(sx) / np.float32(st))
         out["c_cy"].append(np.float32(sy) / np.float32(st))
+        out["c_sum_tot_tof"].append(sf)
+        out["c_ctof"].append(np.float32(sf) / np.float32(st))
     for k in ("c_label", "c_size", "c_shot"):
         out[k] = np.array(out[k], dtype=np.uint32)
-    for k in ("c_sum_tot", "c_sum_tot_x", "c_sum_tot_y"):
+    for k in ("c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_sum_tot_tof"):
         out[k] = np.array(out[k], dtype=np.int64)
     out["c_toa_peak"] = np.array(out["c_toa_peak"], dtype=np.uint64)
     out["c_cx"] = np.array(out["c_cx"], dtype=np.float32)
     out["c_cy"] = np.array(out["c_cy"], dtype=np.float32)
+    out["c_ctof"] = np.array(out["c_ctof"], dtype=np.float32)
     return out

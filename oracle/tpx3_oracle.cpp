@@ -22,6 +22,10 @@
 //      :162 (Eq. 9) with A_ij restricted to the component; fp32 IEEE divide of the two
 //      int64 sums each rounded to fp32 (reading R12). Clusters are listed in
 //      ascending label order.
+//   6. time-of-flight centroid: "this procedure is identical for X, Y and
+//      ToF", ToF = ToA - laser trigger = toa - shot*P (R6; P = 0:
+//      ToF = ToA): sum_tot_tof = sum(tot*tof) in int64, ctof = (float)sum_tot_tof / (float)sum(tot)
+//      in ticks (R20).
 //
 // Pins (tests/test_oracle_pins.py): the paper's worked example (Eq. 2-7, :106-148), brute
 // force O(n^2) adjacency + closure on tiny inputs (oracle/bruteforce.py, written directly
@@ -86,12 +90,14 @@ extern "C" {
 // Returns 0 on success. All arrays are caller-owned host memory.
 //   perm[n], label[n] (indexed by sorted position), *n_clusters
 //   cluster arrays have capacity n: c_label, c_size, c_shot (uint32; shot truncated to 32 bits),
-//   c_sum_tot, c_sum_tot_x, c_sum_tot_y (int64), c_toa_peak (uint64), c_cx, c_cy (float)
+//   c_sum_tot, c_sum_tot_x, c_sum_tot_y (int64), c_toa_peak (uint64), c_cx, c_cy (float),
+//   c_sum_tot_tof (int64), c_ctof (float)
 //   any cluster array pointer may be null (skipped).
 int tpx3_oracle_run(uint64_t n, const uint16_t* x, const uint16_t* y, const uint64_t* toa, const uint16_t* tot,
                     uint64_t W, uint64_t P, int threads, uint32_t* perm, uint32_t* label, uint64_t* n_clusters,
                     uint32_t* c_label, uint32_t* c_size, uint32_t* c_shot, int64_t* c_sum_tot, int64_t* c_sum_tot_x,
-                    int64_t* c_sum_tot_y, uint64_t* c_toa_peak, float* c_cx, float* c_cy) {
+                    int64_t* c_sum_tot_y, uint64_t* c_toa_peak, float* c_cx, float* c_cy, int64_t* c_sum_tot_tof,
+                    float* c_ctof) {
   if (n >= 0xFFFFFFFFull) return -1;
 #ifdef _OPENMP
   if (threads > 0) omp_set_num_threads(threads);
@@ -122,7 +128,7 @@ int tpx3_oracle_run(uint64_t n, const uint16_t* x, const uint16_t* y, const uint
   for (uint64_t k = 0; k < n; ++k)
     if (label[k] == k) slot[k] = (uint32_t)nc++;
   *n_clusters = nc;
-  std::vector<int64_t> st(nc, 0), sx(nc, 0), sy(nc, 0);
+  std::vector<int64_t> st(nc, 0), sx(nc, 0), sy(nc, 0), sf(nc, 0);
   std::vector<uint32_t> sz(nc, 0), peak(nc, 0), ptot(nc, 0);
   for (uint64_t k = 0; k < n; ++k) {
     uint32_t c = slot[label[k]];
@@ -132,6 +138,7 @@ int tpx3_oracle_run(uint64_t n, const uint16_t* x, const uint16_t* y, const uint
     st[c] += t;
     sx[c] += t * (int64_t)x[i];
     sy[c] += t * (int64_t)y[i];
+    sf[c] += t * (int64_t)(P ? toa[i] % P : toa[i]);  // ToF = ToA - shot*P
     if (sz[c] == 1 || tot[i] >= ptot[c]) {  // k ascending: '>=' makes the later pixel win ties
       ptot[c] = tot[i];
       peak[c] = (uint32_t)k;
@@ -149,6 +156,8 @@ int tpx3_oracle_run(uint64_t n, const uint16_t* x, const uint16_t* y, const uint
     if (c_toa_peak) c_toa_peak[c] = toa[perm[peak[c]]];
     if (c_cx) c_cx[c] = (float)sx[c] / (float)st[c];
     if (c_cy) c_cy[c] = (float)sy[c] / (float)st[c];
+    if (c_sum_tot_tof) c_sum_tot_tof[c] = sf[c];
+    if (c_ctof) c_ctof[c] = (float)sf[c] / (float)st[c];
     ++c;
   }
   return 0;

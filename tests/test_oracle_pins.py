@@ -91,10 +91,12 @@ def test_tie_break_later_pixel_wins():
 # ------------------------------------------------------------------ brute force on tiny inputs
 def assert_same(o, b):
     assert o["n_clusters"] == b["n_clusters"]
-    for k in ("perm", "label", "c_label", "c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_toa_peak"):
+    for k in ("perm", "label", "c_label", "c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_toa_peak",
+              "c_sum_tot_tof"):
         assert np.array_equal(o[k], b[k]), k
     assert np.array_equal(o["c_cx"].view(np.uint32), b["c_cx"].view(np.uint32))
     assert np.array_equal(o["c_cy"].view(np.uint32), b["c_cy"].view(np.uint32))
+    assert np.array_equal(o["c_ctof"].view(np.uint32), b["c_ctof"].view(np.uint32))
 
 
 def tiny_random(rng, n, span_xy=6, span_t=900, shots=2):
@@ -172,6 +174,50 @@ def test_two_pixel_closed_form():
         assert o["c_cy"][0] == np.float32(t1 * y1 + t2 * y2) / np.float32(t1 + t2)
         assert abs(float(o["c_cx"][0]) - (t1 * x1 + t2 * x2) / (t1 + t2)) < 2e-5  # exact value within fp32 rounding
         assert o["c_toa_peak"].tolist() == [10 if t1 > t2 else 20]
+
+
+def test_tof_centroid_closed_forms():
+    """ToT-weighted time-of-flight centroid: "identical for X, Y and ToF", ToF = ToA - trigger
+    (PAPER.md:44, 68) = ToA - shot*P (R6)."""
+    # Eq. 9 on a hand-computed example: one hit of three pixels in shot 7, ToF 100, 104, 110, ToT 10, 30, 20
+    toa = 7 * P + np.array([100, 104, 110]); tot = np.array([10, 30, 20])
+    o = oracle.run([50, 51, 50], [60, 60, 61], toa, tot, W, P)
+    assert o["n_clusters"] == 1 and o["c_shot"].tolist() == [7]
+    assert o["c_sum_tot_tof"].tolist() == [10 * 100 + 30 * 104 + 20 * 110] == [6320]
+    assert o["c_ctof"][0] == np.float32(6320) / np.float32(60)
+    assert abs(float(o["c_ctof"][0]) - 6320 / 60) < 1e-5
+    # the same through the paper-literal row reduction (Eq. 9 with the ToF vector in place of X)
+    A = bf.adjacency(np.array([50, 51, 50]), np.array([60, 60, 61]), toa, 1, 1, W) | np.eye(3, dtype=np.int64)
+    assert bf.box_centroid(toa - 7 * P, tot, A)[1] == pytest.approx(6320 / 60)
+    # single pixel: the centroid is the pixel's own ToF
+    o = oracle.run([9], [9], [3 * P + 4321], [77], W, P)
+    assert o["c_sum_tot_tof"].tolist() == [77 * 4321] and o["c_ctof"].tolist() == [4321.0]
+    # two pixels: (t1 f1 + t2 f2) / (t1 + t2)
+    o = oracle.run([9, 10], [9, 9], [P + 10, P + 30], [3, 1], W, P)
+    assert o["c_ctof"].tolist() == [15.0]
+    # P = 0: one shot, the trigger is tick 0, ToF = ToA
+    o = oracle.run([9, 10], [9, 9], [P + 10, P + 30], [3, 1], W, 0)
+    assert o["c_sum_tot_tof"].tolist() == [3 * (P + 10) + (P + 30)]
+
+
+def test_tof_centroid_transforms():
+    w = gen.generate(2, shots=60)
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P)
+    # whole shots later: only shot and toa_peak change
+    o2 = oracle.run(w.x, w.y, w.toa + np.uint64(5 * P), w.tot, W, P)
+    assert np.array_equal(o["c_sum_tot_tof"], o2["c_sum_tot_tof"]) and np.array_equal(o["c_ctof"], o2["c_ctof"])
+    # every event d ticks later inside its shot: sum_tot_tof grows by d * sum_tot, nothing else moves
+    d = 1000
+    o3 = oracle.run(w.x, w.y, w.toa + np.uint64(d), w.tot, W, P)
+    assert np.array_equal(o3["label"], o["label"])
+    assert np.array_equal(o3["c_sum_tot_tof"], o["c_sum_tot_tof"] + d * o["c_sum_tot"])
+    # the centroid lies between the earliest and the latest member ToF of the hit; conservation
+    tof = (w.toa[o["perm"]] % np.uint64(P)).astype(np.int64)
+    lo = np.full(o["n_clusters"], 1 << 62); hi = np.zeros(o["n_clusters"], dtype=np.int64)
+    slot = np.searchsorted(o["c_label"], o["label"])
+    np.minimum.at(lo, slot, tof); np.maximum.at(hi, slot, tof)
+    assert np.all(o["c_ctof"] >= lo.astype(np.float32)) and np.all(o["c_ctof"] <= hi.astype(np.float32))
+    assert int(o["c_sum_tot_tof"].sum()) == int((w.tot[o["perm"]].astype(np.int64) * tof).sum())
 
 
 # ------------------------------------------------------------------ invariants on the configs
