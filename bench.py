@@ -202,10 +202,10 @@ def run_reference(args):
 
 # Algorithmic bytes: what the method must move once, per pixel hit and
 # per particle hit. Inputs 14 B/hit (x, y, tot u16 + toa u64), outputs perm + label 8 B/hit,
-# cluster row 52 B (label, size, shot u32; three i64 sums; toa_peak u64; cx, cy f32).
+# cluster row 64 B (label, size, shot u32; four i64 sums; toa_peak u64; cx, cy, ctof f32).
 BYTES_PER_HIT_IN = 14
 BYTES_PER_HIT_OUT = 8
-BYTES_PER_CLUSTER = 52
+BYTES_PER_CLUSTER = 64
 STAGE_BYTES = {  # per stage of the general path: single-touch floor of that stage
     "fused": lambda n, c: (BYTES_PER_HIT_IN + BYTES_PER_HIT_OUT) * n + BYTES_PER_CLUSTER * c,
     "sort": lambda n, c: (8 + 4) * n,                      # read toa, write perm

@@ -10,7 +10,7 @@
  *   S3      label[k] = smallest sorted index in k's component; hit count
  *   S4      per hit: size, sum ToT, sum ToT*X, sum ToT*Y (exact integers); the brightest pixel
  *           (max ToT, ties: the later pixel in the sorted stream wins)
- *   S5      centroid = sum(ToT*X) / sum(ToT), same for Y                             PAPER.md:156-165, Eq. 8-9
+ *   S5      centroid = sum(ToT*X) / sum(ToT), same for Y and for ToF = ToA - shot*P  PAPER.md:156-165, Eq. 8-9
  *           computed as fp32(int64) / fp32(int64), IEEE round-to-nearest divide.
  *
  * Conventions
@@ -84,6 +84,10 @@ typedef struct {
   uint64_t* toa_peak;   /* ToA of the brightest pixel (max (ToT, sorted position))             */
   float* cx;            /* fp32(sum_tot_x) / fp32(sum_tot), Eq. 9                              */
   float* cy;
+  int64_t* sum_tot_tof; /* sum ToT * ToF, ToF = ToA - shot * P in ticks (P = 0: ToF = ToA); exact
+                           while it stays below 2^63 (always for P <= 2^24)                    */
+  float* ctof;          /* fp32(sum_tot_tof) / fp32(sum_tot): the ToF centroid, "identical for
+                           X, Y and ToF", PAPER.md:165                                         */
 } tpx3_clusters_t;
 
 /* Device status of the most recent call on a workspace (tpx3_status). */

@@ -51,7 +51,8 @@ class _CConfig(ctypes.Structure):
 
 class _CClusters(ctypes.Structure):
     _fields_ = [(k, ctypes.c_void_p) for k in
-                ("label", "size", "shot", "sum_tot", "sum_tot_x", "sum_tot_y", "toa_peak", "cx", "cy")]
+                ("label", "size", "shot", "sum_tot", "sum_tot_x", "sum_tot_y", "toa_peak", "cx", "cy", "sum_tot_tof",
+                 "ctof")]
 
 
 class _CStatus(ctypes.Structure):
@@ -123,6 +124,7 @@ class Config:
 _CLUSTER_FIELDS = (
     ("label", "uint32"), ("size", "uint32"), ("shot", "uint32"), ("sum_tot", "int64"), ("sum_tot_x", "int64"),
     ("sum_tot_y", "int64"), ("toa_peak", "uint64"), ("cx", "float32"), ("cy", "float32"),
+    ("sum_tot_tof", "int64"), ("ctof", "float32"),
 )
 
 

@@ -128,6 +128,7 @@ __global__ void __launch_bounds__(kCentThreads) k_root_slots(Ctrl* c, int genera
         out.sum_tot[off] = 0;
         out.sum_tot_x[off] = 0;
         out.sum_tot_y[off] = 0;
+        out.sum_tot_tof[off] = 0;
         peak[off] = 0ull;
       }
       ++off;
@@ -137,7 +138,8 @@ __global__ void __launch_bounds__(kCentThreads) k_root_slots(Ctrl* c, int genera
 
 __global__ void __launch_bounds__(256) k_accumulate(Ctrl* c, int general_only, uint64_t n,
                                                   const uint16_t* __restrict__ x, const uint16_t* __restrict__ y,
-                                                  const uint16_t* __restrict__ tot, const uint32_t* __restrict__ perm,
+                                                  const uint16_t* __restrict__ tot, const uint64_t* __restrict__ toa,
+                                                  uint64_t P, const uint32_t* __restrict__ perm,
                                                   const uint32_t* __restrict__ label, const uint32_t* __restrict__ slot,
                                                   uint64_t max_clusters, tpx3_clusters_t out, unsigned long long* peak) {
   if (general_only && c->fused_state == 1) return;
@@ -149,6 +151,9 @@ __global__ void __launch_bounds__(256) k_accumulate(Ctrl* c, int general_only, u
     atomicAdd((unsigned long long*)&out.sum_tot[s], t);
     atomicAdd((unsigned long long*)&out.sum_tot_x[s], t * (unsigned long long)x[i]);
     atomicAdd((unsigned long long*)&out.sum_tot_y[s], t * (unsigned long long)y[i]);
+    // time of flight = ToA - shot * P (P = 0: one shot triggered at tick 0)
+    const unsigned long long tof = P ? toa[i] % P : toa[i];
+    atomicAdd((unsigned long long*)&out.sum_tot_tof[s], t * tof);
     // brightest pixel: max over (ToT, sorted position) — the later pixel wins ties
     atomicMax(&peak[s], (t << 32) | (unsigned long long)k);
   }
@@ -170,6 +175,7 @@ __global__ void __launch_bounds__(256) k_finalize(Ctrl* c, int general_only, Par
     float fst = __ll2float_rn(st);
     out.cx[s] = __fdiv_rn(__ll2float_rn(sx), fst);
     out.cy[s] = __fdiv_rn(__ll2float_rn(sy), fst);
+    out.ctof[s] = __fdiv_rn(__ll2float_rn(out.sum_tot_tof[s]), fst);
   }
 }
 

@@ -137,6 +137,7 @@ struct FusedArgs {
   uint4* stage_a;      // staging table, indexed by sorted position: {label, size, sum tot, -}
   uint4* stage_b;      //                                            {sum tot*x (lo, hi), sum tot*y (lo, hi)}
   uint64_t* stage_c;   //                                            ToA of the brightest pixel
+  uint64_t* stage_d;   //                                            sum tot*tof
 };
 
 constexpr uint32_t kNone = 0xFFFFFFFFu;
@@ -758,11 +759,13 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   //      k_fused_compact moves it to its ordinal once every tile's count is known -------------------
   for (uint32_t c = tid; c < n_roots; c += THREADS) {
     const uint32_t r = rootpos[c];
-    unsigned long long sx = 0, sy = 0;
+    unsigned long long sx = 0, sy = 0, sf = 0;
     uint32_t st = 0, size = 0, best = 0, k = r;
     do {
-      const uint32_t w1 = recS[k].y;
+      const uint2 rk = recS[k];
+      const uint32_t w1 = rk.y;
       const uint32_t t = w1 >> 16;
+      sf += (unsigned long long)t * (unsigned long long)(rk.x & tmask);   // ToF = ToA - shot * P
       st += t;                                             // <= 65535 * 8192 < 2^32
       sx += (unsigned long long)(t * (w1 & 0xFFu));
       sy += (unsigned long long)(t * ((w1 >> 8) & 0xFFu));
@@ -776,6 +779,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     a.stage_a[o] = make_uint4(out_base + r, size, st, 0u);
     a.stage_b[o] = make_uint4((uint32_t)sx, (uint32_t)(sx >> 32), (uint32_t)sy, (uint32_t)(sy >> 32));
     a.stage_c[o] = ref + (uint64_t)(keyp >> tb) * a.P + (uint64_t)(keyp & tmask);
+    a.stage_d[o] = sf;
   }
 
   // ---- completion: the last tile to finish publishes the outcome of the call --------------------
@@ -846,6 +850,9 @@ __global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, 
       const float fst = __ll2float_rn(st);
       a.out.cx[o] = __fdiv_rn(__ll2float_rn(sx), fst);
       a.out.cy[o] = __fdiv_rn(__ll2float_rn(sy), fst);
+      const long long sf = (long long)a.stage_d[src + c];
+      a.out.sum_tot_tof[o] = sf;
+      a.out.ctof[o] = __fdiv_rn(__ll2float_rn(sf), fst);
     }
     prefix += cnt;
   }
@@ -918,10 +925,11 @@ inline int enqueue_fused(const FusedGeom& g, uint64_t* launches, Ctrl* ctrl, uns
   a.max_clusters = max_clusters;
   a.out = out;
   a.n_clusters = n_clusters;
-  // staging table: 40 bytes per event position (aliases the general path's sort buffers)
+  // staging table: 48 bytes per event position (aliases the general path's sort buffers)
   a.stage_a = reinterpret_cast<uint4*>(stage);
   a.stage_b = a.stage_a + prm.n;
   a.stage_c = reinterpret_cast<uint64_t*>(a.stage_b + prm.n);
+  a.stage_d = a.stage_c + prm.n;
   int rc = g.variant == 3 ? launch_fused<2048, 256>(a, st) : g.variant == 1 ? launch_fused<4096, 512>(a, st) : launch_fused<8192, 1024>(a, st);
   if (rc != TPX3_OK) return rc;
   ++*launches;

@@ -170,7 +170,8 @@ __host__ __device__ inline uint32_t grid_for_hd(uint64_t n, int threads, int num
     GP(TPX3_STAGE_CENTROID, k_root_slots, (A).cent_nblk, kCentThreads, (A).w.ctrl, (A).general_only, n_, (A).label,   \
        (A).w.blkcnt, (A).w.slot, (A).max_clusters, (A).out, (A).w.peak);                                              \
     GP(TPX3_STAGE_CENTROID, k_accumulate, grid_for_hd(n_, 256, (A).sms), 256, (A).w.ctrl, (A).general_only, n_,       \
-       (A).x, (A).y, (A).tot, (A).perm, (A).label, (A).w.slot, (A).max_clusters, (A).out, (A).w.peak);                \
+       (A).x, (A).y, (A).tot, (A).toa, (A).prm.P, (A).perm, (A).label, (A).w.slot, (A).max_clusters, (A).out,        \
+       (A).w.peak);                \
     GP(TPX3_STAGE_CENTROID, k_finalize,                                                                               \
        grid_for_hd((A).max_clusters < n_ ? (A).max_clusters : n_, 256, (A).sms), 256, (A).w.ctrl, (A).general_only,   \
        (A).prm, (A).toa, (A).perm, (A).n_clusters, (A).max_clusters, (A).out, (A).w.peak);                            \
@@ -258,7 +259,7 @@ int enqueue_centroid(tpx3_plan_s* p, const GenArgs& a, cudaStream_t st) {
 
 bool clusters_ok(const tpx3_clusters_t* o) {
   return o && o->label && o->size && o->shot && o->sum_tot && o->sum_tot_x && o->sum_tot_y && o->toa_peak && o->cx &&
-         o->cy;
+         o->cy && o->sum_tot_tof && o->ctof;
 }
 
 }  // namespace
@@ -301,8 +302,8 @@ int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace
   p->off_slab = o; o = align_up(o + 8 * N);
   p->off_table = o; o = align_up(o + 4 * (size_t)table_size_for(N));
   p->off_counts = o; o = align_up(o + 4 * (size_t)kRadix * kSortMaxBlocks);
-  // the fused path's staging table (40 bytes per event) aliases keyA .. table
-  if (p->off_counts - p->off_keyA < 40 * (size_t)N) { delete p; return TPX3_ERR_INVALID_ARG; }
+  // the fused path's staging table (48 bytes per event) aliases keyA .. table
+  if (o - p->off_keyA < 48 * (size_t)N) o = align_up(p->off_keyA + 48 * (size_t)N);
   // centroid buffers alias the sort buffers (the two steps never run concurrently and the
   // centroid step takes perm/label from the caller, not from the workspace)
   p->off_slot = p->off_keyA;                    // 4N <= 8N
@@ -404,6 +405,8 @@ size_t tpx3_host_io_bytes(uint64_t n, uint64_t max_clusters) {
   o = align_up(o + 8 * max_clusters);      // toa_peak
   o = align_up(o + 4 * max_clusters);      // cx
   o = align_up(o + 4 * max_clusters);      // cy
+  o = align_up(o + 8 * max_clusters);      // sum_tot_tof
+  o = align_up(o + 4 * max_clusters);      // ctof
   o = align_up(o + 256);                   // n_clusters
   return o;
 }
@@ -435,6 +438,8 @@ int tpx3_process_host(tpx3_plan_t p, void* workspace, void* device_io, void* cud
   d.toa_peak = (uint64_t*)take(8 * max_clusters);
   d.cx = (float*)take(4 * max_clusters);
   d.cy = (float*)take(4 * max_clusters);
+  d.sum_tot_tof = (int64_t*)take(8 * max_clusters);
+  d.ctof = (float*)take(4 * max_clusters);
   uint32_t* dn = (uint32_t*)take(256);
   cudaError_t e = cudaSuccess;
   if (n) {
@@ -464,6 +469,9 @@ int tpx3_process_host(tpx3_plan_t p, void* workspace, void* device_io, void* cud
     if (e == cudaSuccess && h.toa_peak) e = cudaMemcpyAsync(h.toa_peak, d.toa_peak, 8 * nc, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess && h.cx) e = cudaMemcpyAsync(h.cx, d.cx, 4 * nc, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess && h.cy) e = cudaMemcpyAsync(h.cy, d.cy, 4 * nc, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && h.sum_tot_tof)
+      e = cudaMemcpyAsync(h.sum_tot_tof, d.sum_tot_tof, 8 * nc, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && h.ctof) e = cudaMemcpyAsync(h.ctof, d.ctof, 4 * nc, cudaMemcpyDeviceToHost, st);
     if (e != cudaSuccess) return TPX3_ERR_CUDA;
   }
   tpx3_status_t s;

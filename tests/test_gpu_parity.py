@@ -67,8 +67,9 @@ def assert_parity(g, o, what=""):
     assert g["n_clusters"] == o["n_clusters"], what
     np.testing.assert_array_equal(g["perm"], o["perm"], err_msg=what + " perm")
     np.testing.assert_array_equal(g["label"], o["label"], err_msg=what + " label")
-    for k in ("c_label", "c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_toa_peak"):
+    for k in ("c_label", "c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_toa_peak", "c_sum_tot_tof"):
         np.testing.assert_array_equal(g[k], o[k], err_msg=what + " " + k)
+    np.testing.assert_array_equal(g["c_ctof"], o["c_ctof"], err_msg=what + " c_ctof (bitwise fp32)")
     for k in ("c_cx", "c_cy"):
         assert np.all(np.abs(g[k].astype(np.float64) - o[k].astype(np.float64)) <= CENTROID_TOL), what + " " + k
         np.testing.assert_array_equal(g[k], o[k], err_msg=what + " " + k + " (bitwise fp32)")
@@ -102,7 +103,8 @@ def test_cfg_subsets(tpx3, cfg, shots):
 @pytest.mark.parametrize("cfg,shots,hint", [(0, 1000, 256), (1, 3000, 640), (1, 3000, 1024), (2, 1200, 1536),
                                             (4, 1200, 1536), (4, 1200, 4096)])
 def test_fused_tile_variants(tpx3, cfg, shots, hint):
-    # max_shot_hits picks the tile variant (4096-event tiles for <= 1024, 8192 otherwise) and the slice length
+    # max_shot_hits picks the tile variant (2048-event tiles for <= 512, 4096 for <= 1024, 8192 otherwise)
+    # and the slice length
     w = gen.generate(cfg, shots=shots)
     res, _ = check(tpx3, w.x, w.y, w.toa, w.tot, modes=("fused",), max_shot_hits=hint, what="cfg%d hint %d" % (cfg, hint))
     assert res["status"]["path"] == 1
@@ -354,7 +356,8 @@ def _full_size_check(m, w, windows, hint):
         i0, i1 = np.searchsorted(c["c_label"], [a, b])
         assert i1 - i0 == o["n_clusters"], what
         np.testing.assert_array_equal(c["c_label"][i0:i1], o["c_label"] + np.uint32(a), err_msg=what)
-        for key in ("c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_toa_peak", "c_cx", "c_cy"):
+        for key in ("c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_toa_peak", "c_cx", "c_cy",
+                    "c_sum_tot_tof", "c_ctof"):
             np.testing.assert_array_equal(c[key][i0:i1], o[key], err_msg=what + " " + key)
     return ncl
 
@@ -382,3 +385,18 @@ def test_full_size_cfg3_quarter(tpx3):
     """A quarter of config 3 (12 500 shots, 2.6e7 hits, about 2 100 hits per shot: the 8192-event tiles)."""
     w = gen.generate(3, shots=12500)
     _full_size_check(tpx3, w, _windows(w.shots, 60, 5), gen.max_shot_hits(3))
+
+
+def test_small_tile_variant_with_in_tile_sort(tpx3):
+    """Shots of <= 120 events delivered out of order inside each shot, hint 128: the 2048-event tile
+    variant has to run its in-tile sort."""
+    w = gen.generate(0, shots=600)
+    rng = np.random.default_rng(21)
+    p = np.arange(w.n)
+    off = w.shot_offsets
+    for s in range(w.shots):
+        a, b = int(off[s]), int(off[s + 1])
+        p[a:b] = a + rng.permutation(b - a)
+    res, _ = check(tpx3, w.x[p], w.y[p], w.toa[p], w.tot[p], modes=("fused",), max_shot_hits=128, what="cfg0 shuffled")
+    assert res["status"]["path"] == 1
+    assert np.any(res["perm"] != np.arange(w.n))
