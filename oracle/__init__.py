@@ -42,6 +42,9 @@ def _load():
         lib.tpx3_oracle_run.restype = ctypes.c_int
         lib.tpx3_oracle_run.argtypes = [ctypes.c_uint64] + [ctypes.c_void_p] * 4 + [
             ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int] + [ctypes.c_void_p] * 14
+        lib.tpx3_oracle_localmax.restype = ctypes.c_int
+        lib.tpx3_oracle_localmax.argtypes = [ctypes.c_uint64] + [ctypes.c_void_p] * 4 + [
+            ctypes.c_uint64] * 4 + [ctypes.c_int] + [ctypes.c_void_p] * 14
         _lib = lib
     return _lib
 
@@ -78,6 +81,38 @@ def run(x, y, toa, tot, W: int, P: int, threads: int = 1, clusters: bool = True)
     if rc != 0:
         raise RuntimeError("tpx3_oracle_run failed: %d" % rc)
     out["n_clusters"] = int(nc.value)
+    for k, a in carr.items():
+        out[k] = a[: out["n_clusters"]].copy()
+    return out
+
+
+def run_localmax(x, y, toa, tot, wx: int, wy: int, wt: int, P: int, threads: int = 0) -> dict:
+    """Paper-literal mode (Eq. 3-9): hits = local ToT maxima of the box neighbourhood
+    (wx, wy, wt, same shot), centroid over the box about each maximum. Returns perm, lmax
+    (lmax[k] = k for a hit, 0xFFFFFFFF otherwise), n_clusters and the per-hit arrays (prefix c_)."""
+    lib = _load()
+    x = np.ascontiguousarray(x, dtype=np.uint16)
+    y = np.ascontiguousarray(y, dtype=np.uint16)
+    toa = np.ascontiguousarray(toa, dtype=np.uint64)
+    tot = np.ascontiguousarray(tot, dtype=np.uint16)
+    n = x.shape[0]
+    perm = np.empty(n, dtype=np.uint32)
+    lmax = np.empty(n, dtype=np.uint32)
+    nc = ctypes.c_uint64(0)
+    carr = {
+        "c_label": np.empty(n, dtype=np.uint32), "c_size": np.empty(n, dtype=np.uint32),
+        "c_shot": np.empty(n, dtype=np.uint32), "c_sum_tot": np.empty(n, dtype=np.int64),
+        "c_sum_tot_x": np.empty(n, dtype=np.int64), "c_sum_tot_y": np.empty(n, dtype=np.int64),
+        "c_toa_peak": np.empty(n, dtype=np.uint64), "c_cx": np.empty(n, dtype=np.float32),
+        "c_cy": np.empty(n, dtype=np.float32),
+        "c_sum_tot_tof": np.empty(n, dtype=np.int64), "c_ctof": np.empty(n, dtype=np.float32),
+    }
+    rc = lib.tpx3_oracle_localmax(n, x.ctypes.data, y.ctypes.data, toa.ctypes.data, tot.ctypes.data,
+                                  int(wx), int(wy), int(wt), int(P), int(threads), perm.ctypes.data,
+                                  lmax.ctypes.data, ctypes.addressof(nc), *[a.ctypes.data for a in carr.values()])
+    if rc != 0:
+        raise RuntimeError("tpx3_oracle_localmax failed: %d" % rc)
+    out = {"perm": perm, "lmax": lmax, "n_clusters": int(nc.value)}
     for k, a in carr.items():
         out[k] = a[: out["n_clusters"]].copy()
     return out

@@ -163,4 +163,92 @@ int tpx3_oracle_run(uint64_t n, const uint16_t* x, const uint16_t* y, const uint
   return 0;
 }
 
+
+// Paper-literal mode — the paper's own definition of a hit, §V:
+//   neighbourhood  A_ij = [|X_i-X_j| <= wx] [|Y_i-Y_j| <= wy] [|ToF_i-ToF_j| <= wt], same laser shot,
+//                  A_ii = 1                                   Eq. 3-5, PAPER.md:109-126 (inclusive, :117)
+//   hit            a pixel i with no neighbour of greater ToT (Eq. 6-7, :134-148); equal ToT: the pixel
+//                  later in the (sorted) stream wins (:150) — taken as the lexicographic order on
+//                  (ToT, sorted index), reading R7
+//   centroid       sum_j V_j A_ij ToT_j / sum_j ToT_j A_ij over ROW i of A (the box about the local
+//                  maximum), V = X, Y and ToF alike          Eq. 8-9
+// Plain definition: after the stable (shot, ToA) sort every pair of a shot is tested, O(m^2) per shot.
+// Outputs as tpx3_oracle_run, one row per hit in ascending sorted index: c_label = the sorted index of
+// the local-maximum pixel, c_size = sum_j A_ij, c_toa_peak = its ToA; lmax[k] = k for a hit, 0xFFFFFFFF else.
+int tpx3_oracle_localmax(uint64_t n, const uint16_t* x, const uint16_t* y, const uint64_t* toa, const uint16_t* tot,
+                         uint64_t wx, uint64_t wy, uint64_t wt, uint64_t P, int threads, uint32_t* perm,
+                         uint32_t* lmax, uint64_t* n_hits, uint32_t* c_label, uint32_t* c_size, uint32_t* c_shot,
+                         int64_t* c_sum_tot, int64_t* c_sum_tot_x, int64_t* c_sum_tot_y, uint64_t* c_toa_peak,
+                         float* c_cx, float* c_cy, int64_t* c_sum_tot_tof, float* c_ctof) {
+  if (n >= 0xFFFFFFFFull) return -1;
+#ifdef _OPENMP
+  if (threads > 0) omp_set_num_threads(threads);
+#endif
+  std::iota(perm, perm + n, 0u);
+  auto shot_of = [&](uint32_t i) -> uint64_t { return P ? toa[i] / P : 0; };
+  std::stable_sort(perm, perm + n, [&](uint32_t i, uint32_t j) {
+    uint64_t si = shot_of(i), sj = shot_of(j);
+    if (si != sj) return si < sj;
+    return toa[i] < toa[j];
+  });
+  std::vector<ShotRange> shots;
+  for (uint64_t k = 0; k < n;) {
+    uint64_t s = shot_of(perm[k]), e = k + 1;
+    while (e < n && shot_of(perm[e]) == s) ++e;
+    shots.push_back({k, e});
+    k = e;
+  }
+  auto adjacent = [&](uint64_t i, uint64_t j) -> bool {  // i, j sorted positions of one shot
+    uint32_t a = perm[i], b = perm[j];
+    uint64_t dx = x[a] > x[b] ? x[a] - x[b] : x[b] - x[a];
+    uint64_t dy = y[a] > y[b] ? y[a] - y[b] : y[b] - y[a];
+    uint64_t dt = toa[a] > toa[b] ? toa[a] - toa[b] : toa[b] - toa[a];  // same shot: dToF = dToA
+    return dx <= wx && dy <= wy && dt <= wt;
+  };
+#pragma omp parallel for schedule(dynamic, 16)
+  for (int64_t si = 0; si < (int64_t)shots.size(); ++si) {
+    for (uint64_t i = shots[si].a; i < shots[si].b; ++i) {
+      bool is_max = true;
+      for (uint64_t j = shots[si].a; j < shots[si].b && is_max; ++j) {
+        if (j == i || !adjacent(i, j)) continue;
+        uint16_t ti = tot[perm[i]], tj = tot[perm[j]];
+        if (tj > ti || (tj == ti && j > i)) is_max = false;
+      }
+      lmax[i] = is_max ? (uint32_t)i : 0xFFFFFFFFu;
+    }
+  }
+  uint64_t c = 0;
+  for (size_t si = 0; si < shots.size(); ++si) {
+    for (uint64_t i = shots[si].a; i < shots[si].b; ++i) {
+      if (lmax[i] != i) continue;
+      int64_t st = 0, sx = 0, sy = 0, sf = 0;
+      uint32_t sz = 0;
+      for (uint64_t j = shots[si].a; j < shots[si].b; ++j) {
+        if (!adjacent(i, j)) continue;  // j == i included: A_ii = 1
+        uint32_t b = perm[j];
+        int64_t t = tot[b];
+        ++sz;
+        st += t;
+        sx += t * (int64_t)x[b];
+        sy += t * (int64_t)y[b];
+        sf += t * (int64_t)(P ? toa[b] % P : toa[b]);
+      }
+      if (c_label) c_label[c] = (uint32_t)i;
+      if (c_size) c_size[c] = sz;
+      if (c_shot) c_shot[c] = (uint32_t)shot_of(perm[i]);
+      if (c_sum_tot) c_sum_tot[c] = st;
+      if (c_sum_tot_x) c_sum_tot_x[c] = sx;
+      if (c_sum_tot_y) c_sum_tot_y[c] = sy;
+      if (c_toa_peak) c_toa_peak[c] = toa[perm[i]];
+      if (c_cx) c_cx[c] = (float)sx / (float)st;
+      if (c_cy) c_cy[c] = (float)sy / (float)st;
+      if (c_sum_tot_tof) c_sum_tot_tof[c] = sf;
+      if (c_ctof) c_ctof[c] = (float)sf / (float)st;
+      ++c;
+    }
+  }
+  *n_hits = c;
+  return 0;
+}
+
 }  // extern "C"

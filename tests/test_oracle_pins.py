@@ -367,3 +367,118 @@ def test_well_separated_truth():
         err.extend(d.min(axis=1).tolist())
     err = np.array(err)
     assert err.mean() < 0.3 and err.max() < 1.0  # truncated, noisy footprint: tolerance, not equality
+
+
+# ------------------------------------------------------------------ paper-literal mode (NEXT #2)
+LM_KEYS = ("c_label", "c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_toa_peak", "c_sum_tot_tof")
+
+
+def test_localmax_paper_worked_example(golden_dir):
+    """X, ToT of Eq. 2 / :134 at |D| <= 5 -> "local maxima are pixel 2 and pixel 3"."""
+    g = {}
+    for line in open(os.path.join(golden_dir, "paper_worked_example.txt")):
+        if line.startswith("#") or ":" not in line:
+            continue
+        k, v = line.split(":")
+        g[k.strip()] = [int(t) for t in v.split()]
+    X, TOT, w = np.array(g["X"]), np.array(g["TOT"]), g["W"][0]
+    z = np.zeros(len(X), dtype=np.int64)
+    o = oracle.run_localmax(X, z, z, TOT, w, 0, 0, 0)
+    assert (o["c_label"] + 1).tolist() == [2, 3] and o["n_clusters"] == 2        # the paper's answer (:148)
+    assert o["lmax"].tolist() == [0xFFFFFFFF, 1, 2, 0xFFFFFFFF, 0xFFFFFFFF]
+    # Eq. 9 on rows 2 and 3 of the printed A^X (Eq. 4): boxes {1,2,5} and {3,4}
+    assert o["c_size"].tolist() == [3, 2]
+    assert o["c_sum_tot"].tolist() == [350, 325] and o["c_sum_tot_x"].tolist() == [7000, 29300]
+    assert o["c_cx"][0] == 20.0 and o["c_cx"][1] == np.float32(29300) / np.float32(325)
+
+
+def _dense_localmax(x, y, toa, tot, wx, wy, wt, Pp):
+    """The same from the paper's array formulation (oracle/bruteforce.py: Eq. 3-9 written out)."""
+    toa_l = [int(t) for t in toa]
+    shot = [t // Pp if Pp else 0 for t in toa_l]
+    perm = sorted(range(len(toa_l)), key=lambda i: (shot[i], toa_l[i]))
+    xs, ys, ts = np.asarray(x)[perm], np.asarray(y)[perm], np.asarray(tot)[perm]
+    tl = np.array([toa_l[i] for i in perm], dtype=np.int64)
+    sl = np.array([shot[i] for i in perm], dtype=np.int64)
+    A = bf.adjacency(xs, ys, tl, wx, wy, wt, shot=sl)
+    lm = bf.local_maxima(ts, A, "lex")
+    tof = tl - sl * Pp
+    return perm, lm, A, bf.box_centroid(xs, ts, A), bf.box_centroid(ys, ts, A), bf.box_centroid(tof, ts, A), ts
+
+
+@pytest.mark.parametrize("seed", range(25))
+def test_localmax_vs_dense_array_formulation(seed):
+    rng = np.random.default_rng(1000 + seed)
+    n = int(rng.integers(1, 60))
+    x, y, toa, tot = tiny_random(rng, n, span_xy=9, span_t=1200, shots=2)
+    tot = rng.integers(1, 4, n)  # many ties: the tie rule decides
+    wx, wy, wt = int(rng.integers(0, 4)), int(rng.integers(0, 4)), int(rng.integers(0, 700))
+    o = oracle.run_localmax(x, y, toa, tot, wx, wy, wt, P)
+    perm, lm, A, cx, cy, ct, ts = _dense_localmax(x, y, toa, tot, wx, wy, wt, P)
+    assert o["perm"].tolist() == perm
+    assert o["c_label"].tolist() == sorted(lm.tolist())
+    for c, i in enumerate(o["c_label"]):
+        assert o["c_size"][c] == A[i].sum() and o["c_sum_tot"][c] == (A[i] * ts).sum()
+        assert float(o["c_cx"][c]) == pytest.approx(cx[i], rel=1e-6)
+        assert float(o["c_cy"][c]) == pytest.approx(cy[i], rel=1e-6)
+        assert float(o["c_ctof"][c]) == pytest.approx(ct[i], rel=1e-6, abs=1e-6)
+
+
+def test_localmax_tie_and_window_edges():
+    # equal ToT: the later pixel of the sorted stream wins (PAPER.md:150). Sorted positions: x = 10, 12, 11;
+    # x=11 (pos 2) is adjacent to both others and is the latest -> the only hit; its box holds all three.
+    o = oracle.run_localmax([10, 11, 12], [5, 5, 5], [100, 105, 103], [9, 9, 9], 1, 1, W, P)
+    assert o["perm"].tolist() == [0, 2, 1]
+    assert o["c_label"].tolist() == [2] and o["c_size"].tolist() == [3] and o["c_cx"].tolist() == [11.0]
+    assert o["c_toa_peak"].tolist() == [105] and o["c_ctof"].tolist() == [np.float32(9 * 308) / np.float32(27)]
+    # inclusive thresholds (PAPER.md:117) in all three coordinates, and no neighbourhood across a shot
+    for dx, dy, dt, linked in [(2, 0, 0, True), (3, 0, 0, False), (0, 2, 0, True), (0, 3, 0, False),
+                               (0, 0, 50, True), (0, 0, 51, False)]:
+        o = oracle.run_localmax([100, 100 + dx], [100, 100 + dy], [1000, 1000 + dt], [5, 7], 2, 2, 50, P)
+        assert o["n_clusters"] == (1 if linked else 2), (dx, dy, dt)
+    o = oracle.run_localmax([100, 100], [100, 100], [P - 1, P], [5, 7], 2, 2, 50, P)
+    assert o["n_clusters"] == 2 and o["c_shot"].tolist() == [0, 1]
+    o = oracle.run_localmax([100, 100], [100, 100], [P - 1, P], [5, 7], 2, 2, 50, 0)
+    assert o["n_clusters"] == 1
+    # empty input
+    z = np.zeros(0, dtype=np.uint16)
+    assert oracle.run_localmax(z, z, np.zeros(0, dtype=np.uint64), z, 1, 1, W, P)["n_clusters"] == 0
+
+
+def test_localmax_equals_components_when_boxes_cover_blobs():
+    """Well-separated particles (centres >= 12 px apart, footprints within 2 px of the centre): a box of
+    half-width 4 about ANY pixel of a blob holds the whole blob and nothing else, so the paper's hit
+    (local maximum + box, Eq. 6-9) and the north_star's hit (connected component) are the same sets and
+    every sum, peak and centroid must agree — the two oracles pin each other, and the generated truth
+    pins the count."""
+    w = gen.generate(5, shots=300, truth=True)
+    a = oracle.run(w.x, w.y, w.toa, w.tot, W, P)
+    b = oracle.run_localmax(w.x, w.y, w.toa, w.tot, 4, 4, W, P)
+    assert b["n_clusters"] == a["n_clusters"] == len(w.truth["cx"])
+    assert np.array_equal(a["perm"], b["perm"])
+    # a component is listed at its first pixel, a paper hit at its brightest pixel: match through the label array
+    comp_of_hit = a["label"][b["c_label"]]
+    order = np.argsort(comp_of_hit, kind="stable")
+    assert np.array_equal(comp_of_hit[order], a["c_label"])
+    for k in ("c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_sum_tot_tof", "c_toa_peak", "c_cx",
+              "c_cy", "c_ctof"):
+        assert np.array_equal(b[k][order], a[k]), k
+
+
+def test_localmax_invariants():
+    w = gen.generate(2, shots=40)
+    o = oracle.run_localmax(w.x, w.y, w.toa, w.tot, 1, 1, W, P)
+    a = oracle.run(w.x, w.y, w.toa, w.tot, W, P)
+    n = w.n
+    k = np.arange(n, dtype=np.uint32)
+    assert np.all((o["lmax"] == k) | (o["lmax"] == 0xFFFFFFFF))
+    assert np.array_equal(np.flatnonzero(o["lmax"] == k), o["c_label"])
+    # at least one local maximum per connected component, all maxima inside components (links R2's two definitions)
+    assert o["n_clusters"] >= a["n_clusters"]
+    assert set(a["label"][o["c_label"]].tolist()) == set(a["c_label"].tolist())
+    # a box at w = 1 is a subset of the pixel's component
+    slot = np.searchsorted(a["c_label"], a["label"][o["c_label"]])
+    assert np.all(o["c_size"] <= a["c_size"][slot]) and np.all(o["c_sum_tot"] <= a["c_sum_tot"][slot])
+    assert np.all(o["c_size"] >= 1)
+    # growing the box never adds hits
+    assert oracle.run_localmax(w.x, w.y, w.toa, w.tot, 2, 2, W, P)["n_clusters"] <= o["n_clusters"]
