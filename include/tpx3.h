@@ -93,7 +93,8 @@ typedef struct {
 /* Device status of the most recent call on a workspace (tpx3_status). */
 typedef struct {
   uint32_t error;       /* 0 or -(tpx3_error_t) of the first device-detected error             */
-  uint32_t path;        /* 1 = fused shot-tile path, 2 = general path (global sort + hash link) */
+  uint32_t path;        /* 1 = fused shot-tile path, 2 = general path (global sort + hash link),
+                           3 = paper-literal local-maximum mode                                 */
   uint32_t n_clusters;  /* hits found by the last cluster / centroid call                      */
   uint32_t sort_passes; /* radix passes the general path ran (0 on the fused path)             */
   uint64_t n;           /* events of the last call                                             */
@@ -127,6 +128,21 @@ int tpx3_cluster_centroid(tpx3_plan_t plan, void* workspace, void* cuda_stream, 
                           const uint16_t* x, const uint16_t* y, const uint64_t* toa,
                           const uint16_t* tot, uint32_t* perm, uint32_t* label,
                           uint64_t max_clusters, const tpx3_clusters_t* out, uint32_t* n_clusters);
+
+/* Paper-literal mode (section V, Eq. 3-9): a hit is a pixel with no
+ * neighbour of greater (ToT, sorted position) inside the box |dX| <= wx, |dY| <= wy, |dToF| <= wt
+ * of the same shot (all inclusive; tie: the later pixel wins, :150); its centroid
+ * is Eq. 9 over that box (row i of A, A_ii = 1) for X, Y and ToF alike (:165). Uses the plan's
+ * shot period and the general path's stable sort; the plan's toa_window_ticks is not used.
+ * Outputs [dev]: perm uint32[n]; lmax uint32[n], lmax[k] = k if sorted position k is a hit and
+ * 0xFFFFFFFF otherwise; one row of `out` per hit in ascending k (label = k, size = pixels in the
+ * box, toa_peak = ToA of the local maximum, sums and centroids over the box); n_hits uint32[1].
+ * Capacity and errors as tpx3_centroid. tpx3_status reports path 3. */
+int tpx3_localmax_centroid(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64_t n,
+                           const uint16_t* x, const uint16_t* y, const uint64_t* toa,
+                           const uint16_t* tot, uint32_t wx, uint32_t wy, uint32_t wt, uint32_t* perm,
+                           uint32_t* lmax, uint64_t max_clusters, const tpx3_clusters_t* out,
+                           uint32_t* n_hits);
 
 /* End-to-end variant with HOST buffers: copies x, y, toa, tot [host] to the device, runs
  * tpx3_cluster_centroid and copies perm, label (either may be NULL to skip), the first

@@ -27,7 +27,8 @@ OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_OUT_OF_RANGE, ERR_CUDA, ERR_UNIMPLEMENTED
 
 # Every symbol include/tpx3.h declares (tests check the built library exports all of them).
 exported_symbols = (
-    "tpx3_plan", "tpx3_cluster", "tpx3_centroid", "tpx3_cluster_centroid", "tpx3_host_io_bytes",
+    "tpx3_plan", "tpx3_cluster", "tpx3_centroid", "tpx3_cluster_centroid", "tpx3_localmax_centroid",
+    "tpx3_host_io_bytes",
     "tpx3_process_host", "tpx3_status", "tpx3_launch_count", "tpx3_profile_enable", "tpx3_profile_read",
     "tpx3_free", "tpx3_strerror",
 )
@@ -84,6 +85,9 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.tpx3_cluster_centroid.restype = ctypes.c_int
     lib.tpx3_cluster_centroid.argtypes = [vp, vp, vp, u64, vp, vp, vp, vp, vp, vp, u64,
                                           ctypes.POINTER(_CClusters), u32p]
+    lib.tpx3_localmax_centroid.restype = ctypes.c_int
+    lib.tpx3_localmax_centroid.argtypes = [vp, vp, vp, u64, vp, vp, vp, vp, ctypes.c_uint32, ctypes.c_uint32,
+                                           ctypes.c_uint32, vp, vp, u64, ctypes.POINTER(_CClusters), u32p]
     lib.tpx3_host_io_bytes.restype = ctypes.c_size_t
     lib.tpx3_host_io_bytes.argtypes = [u64, u64]
     lib.tpx3_process_host.restype = ctypes.c_int
@@ -207,6 +211,25 @@ class Plan:
         if rc != OK:
             raise Tpx3Error(rc, "tpx3_cluster")
         return perm, label, n_clusters
+
+    # -- paper-literal mode (local ToT maxima + box centroid, Eq. 3-9) ----------------
+    def localmax_centroid(self, x, y, toa, tot, wx: int, wy: int, wt: int, clusters: "Clusters", perm=None,
+                          lmax=None, n_hits=None, stream=None):
+        import torch
+
+        n = int(x.numel())
+        self._check_inputs(x, y, toa, tot, n)
+        perm = torch.empty(max(n, 1), dtype=torch.uint32, device=self.device) if perm is None else perm
+        lmax = torch.empty(max(n, 1), dtype=torch.uint32, device=self.device) if lmax is None else lmax
+        n_hits = torch.empty(1, dtype=torch.uint32, device=self.device) if n_hits is None else n_hits
+        c = clusters._c()
+        rc = self.lib.tpx3_localmax_centroid(self.handle, self.workspace.data_ptr(), _stream_ptr(stream), n,
+                                             x.data_ptr(), y.data_ptr(), toa.data_ptr(), tot.data_ptr(), int(wx),
+                                             int(wy), int(wt), perm.data_ptr(), lmax.data_ptr(),
+                                             clusters.max_clusters, ctypes.byref(c), n_hits.data_ptr())
+        if rc != OK:
+            raise Tpx3Error(rc, "tpx3_localmax_centroid")
+        return perm, lmax, n_hits
 
     # -- S4-S5 ---------------------------------------------------------------------------------
     def centroid(self, x, y, toa, tot, perm, label, clusters: Clusters, n_clusters=None, stream=None):

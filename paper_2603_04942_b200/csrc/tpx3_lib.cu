@@ -10,6 +10,7 @@
 #include "tpx3_common.cuh"
 #include "tpx3_fused.cuh"
 #include "tpx3_link.cuh"
+#include "tpx3_localmax.cuh"
 #include "tpx3_sort.cuh"
 
 using namespace tpx3;
@@ -136,6 +137,12 @@ __host__ __device__ inline uint32_t grid_for_hd(uint64_t n, int threads, int num
 // GP(stage, kernel, grid, block, args...) is defined by the includer (host launch or device tail launch).
 #define TPX3_GENERAL_CLUSTER_SEQUENCE(A)                                                                              \
   do {                                                                                                                \
+    TPX3_GENERAL_SORT_SEQUENCE(A);                                                                                    \
+    TPX3_GENERAL_LINK_SEQUENCE(A);                                                                                    \
+  } while (0)
+
+#define TPX3_GENERAL_SORT_SEQUENCE(A)                                                                                 \
+  do {                                                                                                                \
     const uint64_t n_ = (A).prm.n;                                                                                    \
     SortBufs b_;                                                                                                      \
     b_.key[0] = (A).w.keyA; b_.key[1] = (A).w.keyB; b_.idx[0] = (A).w.idxA; b_.idx[1] = (A).w.idxB;                   \
@@ -149,6 +156,11 @@ __host__ __device__ inline uint32_t grid_for_hd(uint64_t n, int threads, int num
       GP(TPX3_STAGE_SORT, k_radix_scatter, (A).g.nblk, kSortThreads, (A).w.ctrl, pass_, (A).toa, b_, (A).perm, n_,    \
          (A).g);                                                                                                      \
     }                                                                                                                 \
+  } while (0)
+
+#define TPX3_GENERAL_LINK_SEQUENCE(A)                                                                                 \
+  do {                                                                                                                \
+    const uint64_t n_ = (A).prm.n;                                                                                    \
     GP(TPX3_STAGE_LINK, k_gather, grid_for_hd(n_, 256, (A).sms), 256, (A).w.ctrl, (A).prm, (A).w.keyA, (A).w.keyB,    \
        (A).perm, (A).x, (A).y, (A).tot, (A).w.xy, (A).w.tot, (A).w.slab, (A).label);                                  \
     GP(TPX3_STAGE_LINK, k_fill_u32, grid_for_hd((A).tsize, 256, (A).sms), 256, (A).w.ctrl, 1, (A).w.table,            \
@@ -245,6 +257,24 @@ int enqueue_general_cluster(tpx3_plan_s* p, const GenArgs& a, cudaStream_t st) {
     ++p->launches;                                                 \
   } while (0)
   TPX3_GENERAL_CLUSTER_SEQUENCE(a);
+  hl.leave();
+  return cuda_ok(cudaGetLastError());
+}
+
+int enqueue_localmax(tpx3_plan_s* p, const GenArgs& a, cudaStream_t st, uint32_t wx, uint32_t wy, uint64_t wt) {
+  HostLauncher hl{p, st, -1, false, 0};
+  TPX3_GENERAL_SORT_SEQUENCE(a);
+  const uint64_t n = a.prm.n;
+  // the link stage's buffers hold the sorted records (slab: ToA, xy: x | y << 8 | tot << 16); the centroid
+  // stage's ordinal kernels run on lmax in place of label
+  GP(TPX3_STAGE_LINK, k_lm_gather, grid_for_hd(n, 256, a.sms), 256, n, a.perm, a.x, a.y, a.toa, a.tot, a.w.slab, a.w.xy);
+  GP(TPX3_STAGE_LINK, k_lm_flag, grid_for_hd(n, 256, a.sms, 16), 256, n, a.prm.P, wx, wy, wt, a.w.slab, a.w.xy, a.label);
+  GP(TPX3_STAGE_CENTROID, k_root_count, a.cent_nblk, kCentThreads, a.w.ctrl, 0, n, a.label, a.w.blkcnt);
+  GP(TPX3_STAGE_CENTROID, k_root_scan, 1, 1024, a.w.ctrl, 0, a.w.blkcnt, a.cent_nblk, a.max_clusters, a.n_clusters);
+  GP(TPX3_STAGE_CENTROID, k_root_slots, a.cent_nblk, kCentThreads, a.w.ctrl, 0, n, a.label, a.w.blkcnt, a.w.slot,
+     a.max_clusters, a.out, a.w.peak);
+  GP(TPX3_STAGE_CENTROID, k_lm_emit, grid_for_hd(a.max_clusters < n ? a.max_clusters : n, 128, a.sms, 16), 128, a.w.ctrl,
+     n, a.prm.P, wx, wy, wt, a.w.slab, a.w.xy, a.n_clusters, a.max_clusters, a.out);
   hl.leave();
   return cuda_ok(cudaGetLastError());
 }
@@ -386,6 +416,24 @@ int tpx3_cluster_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uin
   rc = enqueue_general_cluster(p, ga, st);
   if (rc != TPX3_OK) return rc;
   return enqueue_centroid(p, ga, st);
+}
+
+int tpx3_localmax_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x,
+                           const uint16_t* y, const uint64_t* toa, const uint16_t* tot, uint32_t wx, uint32_t wy,
+                           uint32_t wt, uint32_t* perm, uint32_t* lmax, uint64_t max_clusters,
+                           const tpx3_clusters_t* out, uint32_t* n_hits) {
+  if (!p || !workspace || !n_hits) return TPX3_ERR_INVALID_ARG;
+  if (n > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
+  if (n && (!x || !y || !toa || !tot || !perm || !lmax || !out)) return TPX3_ERR_INVALID_ARG;
+  if (max_clusters && !clusters_ok(out)) return TPX3_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  Ws w = carve(p, workspace);
+  if (p->profiling) ++p->profiled_calls;
+  TPX3_LAUNCH(p, k_ctrl_init, 1, 256, 0, st, w.ctrl, n, w.tiles, 0u, n_hits);
+  if (n == 0) return cuda_ok(cudaGetLastError());
+  GenArgs ga = make_gen_args(p, w, 0, n, x, y, toa, tot, perm, lmax, max_clusters, out, n_hits);
+  return enqueue_localmax(p, ga, st, wx, wy, wt);
 }
 
 size_t tpx3_host_io_bytes(uint64_t n, uint64_t max_clusters) {

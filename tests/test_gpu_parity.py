@@ -400,3 +400,72 @@ def test_small_tile_variant_with_in_tile_sort(tpx3):
     res, _ = check(tpx3, w.x[p], w.y[p], w.toa[p], w.tot[p], modes=("fused",), max_shot_hits=128, what="cfg0 shuffled")
     assert res["status"]["path"] == 1
     assert np.any(res["perm"] != np.arange(w.n))
+
+
+# ------------------------------------------------------------------ paper-literal mode (NEXT #2)
+LM_KEYS = ("c_label", "c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_toa_peak", "c_sum_tot_tof",
+           "c_cx", "c_cy", "c_ctof")
+
+
+def check_localmax(m, x, y, toa, tot, wx, wy, wt, P=P, what=""):
+    import torch
+
+    o = oracle.run_localmax(x, y, toa, tot, wx, wy, wt, P)
+    n = len(x)
+    pl = m.plan(m.Config(toa_window_ticks=W, shot_period_ticks=P, max_hits=max(n, 1)))
+    dev = [to_dev(np.asarray(x, dtype=np.uint16)), to_dev(np.asarray(y, dtype=np.uint16)),
+           to_dev(np.asarray(toa, dtype=np.uint64)), to_dev(np.asarray(tot, dtype=np.uint16))]
+    cl = m.Clusters(max(n, 1), pl.device)
+    perm, lmax, nh = pl.localmax_centroid(*dev, wx, wy, wt, cl)
+    torch.cuda.synchronize()
+    st = pl.status()
+    assert st["error"] == 0, what
+    nhits = int(nh.cpu().numpy()[0])
+    assert nhits == o["n_clusters"], what
+    np.testing.assert_array_equal(perm[:n].cpu().numpy(), o["perm"], err_msg=what + " perm")
+    np.testing.assert_array_equal(lmax[:n].cpu().numpy(), o["lmax"], err_msg=what + " lmax")
+    g = cl.numpy(nhits)
+    for k in LM_KEYS:   # integers bit-exact; centroids bitwise fp32 (same int64 sums, IEEE RN divide: R12)
+        np.testing.assert_array_equal(g[k], o[k], err_msg=what + " " + k)
+    if n:
+        assert st["path"] == 3
+    pl.free()
+    return o
+
+
+def test_localmax_paper_example(tpx3):
+    # X of Eq. 2, ToT of :134, |D| <= 5 -> hits = pixel 2 and pixel 3
+    X = np.array([20, 21, 90, 92, 18]); z = np.zeros(5, dtype=np.int64); T = np.array([50, 200, 300, 25, 100])
+    o = check_localmax(tpx3, X, z, z, T, 5, 0, 0, P=0, what="paper example")
+    assert (o["c_label"] + 1).tolist() == [2, 3]
+
+
+@pytest.mark.parametrize("cfg,shots,w3", [(0, 1000, (1, 1, 320)), (1, 400, (1, 1, 320)), (1, 400, (5, 5, 320)),
+                                          (2, 150, (2, 2, 40)), (3, 40, (1, 1, 320)), (4, 150, (3, 3, 320)),
+                                          (5, 300, (4, 4, 320))])
+def test_localmax_configs(tpx3, cfg, shots, w3):
+    w = gen.generate(cfg, shots=shots)
+    check_localmax(tpx3, w.x, w.y, w.toa, w.tot, *w3, what="cfg%d w=%s" % (cfg, w3))
+
+
+def test_localmax_edges(tpx3):
+    z16 = np.zeros(0, dtype=np.uint16)
+    check_localmax(tpx3, z16, z16, np.zeros(0, dtype=np.uint64), z16, 1, 1, W, what="empty")
+    check_localmax(tpx3, [7], [9], [123456789], [55], 1, 1, W, what="single")
+    check_localmax(tpx3, np.full(300, 100), np.full(300, 17), np.full(300, 10**9), np.full(300, 3), 0, 0, 0, what="identical")
+    check_localmax(tpx3, [100, 100], [100, 100], [P - 1, P], [5, 7], 2, 2, 50, what="shot boundary")
+    check_localmax(tpx3, [100, 100], [100, 100], [P - 1, P], [5, 7], 2, 2, 50, P=0, what="P=0")
+    rng = np.random.default_rng(5)
+    for seed in range(4):
+        n = 3000
+        x = rng.integers(0, 40, n); y = rng.integers(0, 40, n)
+        toa = (rng.integers(0, 3, n) * P + rng.integers(0, 3000, n)).astype(np.uint64)
+        tot = rng.integers(1, 5, n)     # many ties
+        check_localmax(tpx3, x, y, toa, tot, int(rng.integers(0, 4)), int(rng.integers(0, 4)), int(rng.integers(0, 900)),
+                       what="random %d" % seed)
+    # large values: ToA near 2^40, ToT up to 65535, window wider than the shot
+    n = 2000
+    x = rng.integers(0, 256, n); y = rng.integers(0, 256, n)
+    toa = ((1 << 40) + rng.integers(0, 2 * P, n)).astype(np.uint64)
+    tot = rng.integers(1, 65536, n)
+    check_localmax(tpx3, x, y, toa, tot, 255, 255, 10 * P, what="large")
