@@ -245,8 +245,14 @@ def run_ours(args):
     nc = torch.zeros(1, dtype=torch.uint32, device=pl.device)
     torch.cuda.synchronize()
 
+    lm = args.mode == "localmax"
+    wx, wy, wt = args.window
+
     def step():
-        pl.cluster_centroid(*dev, cl, perm=perm, label=label, n_clusters=nc, stream=stream)
+        if lm:   # paper-literal mode: local ToT maxima + box centroid
+            pl.localmax_centroid(*dev, wx, wy, wt, cl, perm=perm, lmax=label, n_hits=nc, stream=stream)
+        else:
+            pl.cluster_centroid(*dev, cl, perm=perm, label=label, n_clusters=nc, stream=stream)
 
     def barrier():
         torch.cuda.synchronize()
@@ -297,13 +303,28 @@ def run_ours(args):
 
     # ---- end to end through the C ABI with HOST buffers (tpx3_process_host) --------------------
     clh = m.Clusters(max_clusters, "cpu", pin=True)
+
+    def e2e_step():
+        if not lm:
+            return pl.process_host(*host, clh, stream=stream)  # synchronises the stream itself
+        # no host-buffer entry point for this mode: pinned H2D copies, the call, D2H of the count and the table
+        with torch.cuda.stream(stream):
+            for d, h in zip(dev, host):
+                d.copy_(h, non_blocking=True)
+            step()
+            k = int(nc.cpu().numpy()[0])
+            for name, _ in m._CLUSTER_FIELDS:
+                getattr(clh, name)[:k].copy_(getattr(cl, name)[:k], non_blocking=True)
+        stream.synchronize()
+        return k
+
     for _ in range(2):
-        pl.process_host(*host, clh, stream=stream)
+        e2e_step()
     barrier()
     e2e_steps = max(1, min(args.steps, 5))
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        ncl_e2e = pl.process_host(*host, clh, stream=stream)  # synchronises the stream itself
+        ncl_e2e = e2e_step()
     torch.cuda.synchronize()
     e2e_s = (time.perf_counter() - t0) / e2e_steps
     if world > 1:
@@ -341,14 +362,14 @@ def run_ours(args):
         with open(traffic_file) as f:
             tr = json.load(f)
         key = "%s:%s" % (w.name, dom)
-        if key in tr:
+        if key in tr and tr[key].get("pixel_hits", n) == n:   # a capture is of one workload size
             roofline["traffic"] = tr[key]["dram_bytes_per_launch"]
             roofline["traffic_source"] = tr[key].get("source")
     except Exception:
         pass
 
     cpu = None
-    if world == 1 and not args.no_cpu_baseline:
+    if world == 1 and not args.no_cpu_baseline and not lm:
         cpu = cpu_baseline(w, args.cpu_seconds)
 
     h2d = BYTES_PER_HIT_IN * n
@@ -358,9 +379,10 @@ def run_ours(args):
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "int64", "data": "synthetic",
         "config": {
-            "workload": w.name, "shots_per_gpu": w.shots, "pixel_hits_per_gpu": n, "particle_hits_per_gpu": ncl,
+            "workload": w.name, "mode": ("paper-literal local maxima, box (wx, wy, wt) = (%d, %d, %d)" % (wx, wy, wt))
+            if lm else "connected components (north_star)", "shots_per_gpu": w.shots, "pixel_hits_per_gpu": n, "particle_hits_per_gpu": ncl,
             "pixel_hits_total": n_all, "particle_hits_total": ncl_all, "toa_window_ticks": w.toa_window_ticks,
-            "shot_period_ticks": w.shot_period_ticks, "path": {1: "fused", 2: "general"}.get(st["path"], st["path"]),
+            "shot_period_ticks": w.shot_period_ticks, "path": {1: "fused", 2: "general", 3: "localmax"}.get(st["path"], st["path"]),
             "sort_passes": st["sort_passes"], "max_shot_hits": cfg.max_shot_hits, "parallelism": "shots sharded over %d gpu(s), no collective" % world,
             "l2": "inputs (%.0f MB) larger than the 126 MB L2; no flush between steps" % (14 * n / 1e6)
                   if 14 * n > 2 * 126e6 else "inputs fit L2 (%.0f MB): DRAM traffic is not exercised" % (14 * n / 1e6),
@@ -369,7 +391,8 @@ def run_ours(args):
         "particle_hits_per_s": ncl_all / (ms_step * 1e-3),
         "e2e": {"value": n_all / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_s * 1e3, "api": "tpx3_process_host (pinned host buffers; cluster table copied "
-                "back, perm/label left on the device)"},
+                "back, perm/label left on the device)" if not lm else "pinned H2D copies + tpx3_localmax_centroid + "
+                "D2H of the count and the hit table"},
         "gpu_launches": launches,
         "roofline": roofline,
         "clocks": sampler.summary(t_wall0, time.time()),
@@ -396,6 +419,10 @@ def main():
     ap.add_argument("--force-general", action="store_true", help="never take the fused shot-tile path")
     ap.add_argument("--max-shot-hits", type=int, default=None,
                     help="tile-size hint for the plan (default: the workload recipe's bound on hits per shot)")
+    ap.add_argument("--mode", choices=("components", "localmax"), default="components",
+                    help="components: the hot path (default). localmax: the paper-literal mode, SURVEY 8f NEXT #2")
+    ap.add_argument("--window", type=int, nargs=3, default=(2, 2, 320), metavar=("WX", "WY", "WT"),
+                    help="box half-widths of --mode localmax (pixels, pixels, ticks)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     args = ap.parse_args()
