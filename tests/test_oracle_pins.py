@@ -482,3 +482,56 @@ def test_localmax_invariants():
     assert np.all(o["c_size"] >= 1)
     # growing the box never adds hits
     assert oracle.run_localmax(w.x, w.y, w.toa, w.tot, 2, 2, W, P)["n_clusters"] <= o["n_clusters"]
+
+
+# ------------------------------------------------------------------ ToA unwrapping (NEXT #4)
+from oracle import preprocess as pp  # noqa: E402
+
+TICK_NS = 1.5625
+PIX_MOD = (1 << 42) // 256            # 2^42 units of 25/4096 ns in ticks of 256 units
+JUMP_20S = int(20e9 / TICK_NS)        # "more than 20 seconds"
+
+
+def test_unwrap_constants_match_the_paper():
+    # 25/4096 ns x 2^42 = about 26.8 s for pixels, x 2^44 = about 107.4 s for the TDCs
+    assert abs(PIX_MOD * TICK_NS * 1e-9 - 26.8) < 0.05
+    assert abs(((1 << 44) // 256) * TICK_NS * 1e-9 - 107.4) < 0.05
+
+
+def test_unwrap_hand_example_out_of_order_across_the_wrap():
+    # a dim pixel with a LATER ToA (after the wrap) reports before a bright one whose ToA is
+    # just before the wrap. Counter period 1024, threshold 600; true times 1000 1019 1027 1022 1031 1044.
+    raw = [1000, 1019, 3, 1022, 7, 20]
+    out, wraps = pp.unwrap_toa(raw, 1024, 600)
+    assert out.tolist() == [1000, 1019, 1027, 1022, 1031, 1044] and wraps == 1
+    # without the edge case: each large negative shift adds one period to everything after it
+    out, wraps = pp.unwrap_toa([10, 500, 1000, 5, 400, 900, 2], 1024, 600)
+    assert out.tolist() == [10, 500, 1000, 1029, 1424, 1924, 2050] and wraps == 2
+    # strict threshold: a shift of exactly `jump` is not a wrap, jump + 1 is
+    assert pp.unwrap_toa([700, 100], 1024, 600)[1] == 0 and pp.unwrap_toa([701, 100], 1024, 600)[1] == 1
+    assert pp.unwrap_toa([100, 700], 1024, 600)[1] == 0 and pp.unwrap_toa([100, 701], 1024, 600)[1] == -1
+    assert pp.unwrap_toa([], 1024, 600, wraps_in=3) [1] == 3
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_unwrap_recovers_true_times(seed):
+    """Generated truth: true arrival times over several counter periods, delivered with local disorder
+    (dim pixels report first), wrapped to 42 bits; unwrapping must give the true times back."""
+    rng = np.random.default_rng(seed)
+    n = 20000
+    span = 3 * PIX_MOD + PIX_MOD // 3                     # about 3.3 wraps
+    t = np.sort(rng.integers(0, span, n).astype(np.int64))
+    t = t + rng.integers(0, 2000, n)                      # report order != ToA order (disorder up to 3 us)
+    start = PIX_MOD - 5000                                # the first wrap comes early
+    t = t + start
+    raw = (t % PIX_MOD).astype(np.uint64)
+    out, wraps = pp.unwrap_toa(raw, PIX_MOD, JUMP_20S)
+    assert np.array_equal(out.astype(np.int64), t) and wraps == int(t[-1] // PIX_MOD)
+    # chunked with carried state == whole
+    cuts = [0, 1, 777, 778, 9000, n]
+    w, prev, parts = 0, None, []
+    for a, b in zip(cuts[:-1], cuts[1:]):
+        o, w = pp.unwrap_toa(raw[a:b], PIX_MOD, JUMP_20S, wraps_in=w, prev_raw=prev)
+        parts.append(o)
+        prev = raw[b - 1]
+    assert np.array_equal(np.concatenate(parts), out) and w == wraps
