@@ -525,11 +525,12 @@ def test_unwrap_recovers_true_times(seed):
     start = PIX_MOD - 5000                                # the first wrap comes early
     t = t + start
     raw = (t % PIX_MOD).astype(np.uint64)
-    out, wraps = pp.unwrap_toa(raw, PIX_MOD, JUMP_20S)
-    assert np.array_equal(out.astype(np.int64), t) and wraps == int(t[-1] // PIX_MOD)
+    w0 = int(t[0] // PIX_MOD)                             # wraps before the first event: the caller's state
+    out, wraps = pp.unwrap_toa(raw, PIX_MOD, JUMP_20S, wraps_in=w0)
+    assert np.array_equal(out.astype(np.int64), t) and wraps == int(t[-1] // PIX_MOD) and wraps - w0 >= 3
     # chunked with carried state == whole
     cuts = [0, 1, 777, 778, 9000, n]
-    w, prev, parts = 0, None, []
+    w, prev, parts = w0, None, []
     for a, b in zip(cuts[:-1], cuts[1:]):
         o, w = pp.unwrap_toa(raw[a:b], PIX_MOD, JUMP_20S, wraps_in=w, prev_raw=prev)
         parts.append(o)
