@@ -144,6 +144,19 @@ int tpx3_localmax_centroid(tpx3_plan_t plan, void* workspace, void* cuda_stream,
                            uint32_t* lmax, uint64_t max_clusters, const tpx3_clusters_t* out,
                            uint32_t* n_hits);
 
+/* ToA counter unwrapping (section IV.A, :58-62), for the pixel stream
+ * or the trigger (TDC) stream, each on its own. raw uint64[n] [dev]: counter values in
+ * [0, modulus) in stream order; modulus: the counter period in the caller's tick (2^42 units of
+ * 25/4096 ns for pixels, 2^44 for TDCs); jump: the "20 seconds" threshold in ticks.
+ * Event k adds +1 to the wrap counter if raw[k-1] - raw[k] > jump (:60) and -1 if
+ * raw[k] - raw[k-1] > jump (a pre-wrap event reported after the wrap, :62); toa_out[k] =
+ * raw[k] + wraps_k * modulus (uint64[n] [dev], may not alias raw). wraps_in, has_prev, prev_raw
+ * carry the counter and the last raw value of the previous call; wraps_out int64[1] [dev]
+ * receives the counter after the last event. Enqueue only. */
+int tpx3_unwrap_toa(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64_t n, const uint64_t* raw,
+                    uint64_t modulus, uint64_t jump, int64_t wraps_in, int has_prev, uint64_t prev_raw,
+                    uint64_t* toa_out, int64_t* wraps_out);
+
 /* End-to-end variant with HOST buffers: copies x, y, toa, tot [host] to the device, runs
  * tpx3_cluster_centroid and copies perm, label (either may be NULL to skip), the first
  * min(n_clusters, max_clusters) entries of every non-NULL array of `out_host` and the count

@@ -28,7 +28,7 @@ OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_OUT_OF_RANGE, ERR_CUDA, ERR_UNIMPLEMENTED
 # Every symbol include/tpx3.h declares (tests check the built library exports all of them).
 exported_symbols = (
     "tpx3_plan", "tpx3_cluster", "tpx3_centroid", "tpx3_cluster_centroid", "tpx3_localmax_centroid",
-    "tpx3_host_io_bytes",
+    "tpx3_unwrap_toa", "tpx3_host_io_bytes",
     "tpx3_process_host", "tpx3_status", "tpx3_launch_count", "tpx3_profile_enable", "tpx3_profile_read",
     "tpx3_free", "tpx3_strerror",
 )
@@ -88,6 +88,8 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.tpx3_localmax_centroid.restype = ctypes.c_int
     lib.tpx3_localmax_centroid.argtypes = [vp, vp, vp, u64, vp, vp, vp, vp, ctypes.c_uint32, ctypes.c_uint32,
                                            ctypes.c_uint32, vp, vp, u64, ctypes.POINTER(_CClusters), u32p]
+    lib.tpx3_unwrap_toa.restype = ctypes.c_int
+    lib.tpx3_unwrap_toa.argtypes = [vp, vp, vp, u64, vp, u64, u64, ctypes.c_int64, ctypes.c_int, u64, vp, vp]
     lib.tpx3_host_io_bytes.restype = ctypes.c_size_t
     lib.tpx3_host_io_bytes.argtypes = [u64, u64]
     lib.tpx3_process_host.restype = ctypes.c_int
@@ -211,6 +213,22 @@ class Plan:
         if rc != OK:
             raise Tpx3Error(rc, "tpx3_cluster")
         return perm, label, n_clusters
+
+    # -- ToA counter unwrapping (PAPER.md IV.A) ----------------------------------------------------
+    def unwrap_toa(self, raw, modulus: int, jump: int, wraps_in: int = 0, prev_raw=None, out=None, wraps_out=None,
+                   stream=None):
+        import torch
+
+        n = int(raw.numel())
+        _check_dev(raw, torch.uint64, n, "raw")
+        out = torch.empty(max(n, 1), dtype=torch.uint64, device=self.device) if out is None else out
+        wraps_out = torch.empty(1, dtype=torch.int64, device=self.device) if wraps_out is None else wraps_out
+        rc = self.lib.tpx3_unwrap_toa(self.handle, self.workspace.data_ptr(), _stream_ptr(stream), n, raw.data_ptr(),
+                                      int(modulus), int(jump), int(wraps_in), 0 if prev_raw is None else 1,
+                                      0 if prev_raw is None else int(prev_raw), out.data_ptr(), wraps_out.data_ptr())
+        if rc != OK:
+            raise Tpx3Error(rc, "tpx3_unwrap_toa")
+        return out, wraps_out
 
     # -- paper-literal mode (local ToT maxima + box centroid, Eq. 3-9) ----------------
     def localmax_centroid(self, x, y, toa, tot, wx: int, wy: int, wt: int, clusters: "Clusters", perm=None,

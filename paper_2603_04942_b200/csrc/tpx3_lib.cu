@@ -12,6 +12,7 @@
 #include "tpx3_link.cuh"
 #include "tpx3_localmax.cuh"
 #include "tpx3_sort.cuh"
+#include "tpx3_unwrap.cuh"
 
 using namespace tpx3;
 
@@ -434,6 +435,26 @@ int tpx3_localmax_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, ui
   if (n == 0) return cuda_ok(cudaGetLastError());
   GenArgs ga = make_gen_args(p, w, 0, n, x, y, toa, tot, perm, lmax, max_clusters, out, n_hits);
   return enqueue_localmax(p, ga, st, wx, wy, wt);
+}
+
+int tpx3_unwrap_toa(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint64_t* raw,
+                    uint64_t modulus, uint64_t jump, int64_t wraps_in, int has_prev, uint64_t prev_raw,
+                    uint64_t* toa_out, int64_t* wraps_out) {
+  if (!p || !workspace || !wraps_out || modulus == 0) return TPX3_ERR_INVALID_ARG;
+  if (n > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
+  if (n && (!raw || !toa_out)) return TPX3_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  Ws w = carve(p, workspace);
+  UnwrapArgs a;
+  a.n = n; a.raw = raw; a.modulus = modulus; a.jump = jump; a.wraps_in = (long long)wraps_in;
+  a.has_prev = has_prev; a.prev_raw = prev_raw; a.out = toa_out; a.wraps_out = (long long*)wraps_out;
+  a.blk = w.counts;   // the sort's digit counters: 4 * 256 * 1184 bytes >= 4 * (2^28 / 4096 + 1)
+  a.nblk = (uint32_t)((n + kUnwrapTile - 1) / kUnwrapTile);
+  if (a.nblk) TPX3_LAUNCH(p, k_unwrap_count, a.nblk, kUnwrapThreads, 0, st, a);
+  TPX3_LAUNCH(p, k_unwrap_scan, 1, 1024, 0, st, a);
+  if (a.nblk) TPX3_LAUNCH(p, k_unwrap_apply, a.nblk, kUnwrapThreads, 0, st, a);
+  return cuda_ok(cudaGetLastError());
 }
 
 size_t tpx3_host_io_bytes(uint64_t n, uint64_t max_clusters) {

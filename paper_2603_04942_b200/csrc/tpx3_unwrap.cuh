@@ -1,0 +1,136 @@
+// ToA counter unwrapping (section IV.A, :58-62).
+//
+// The TimePix3 ToA is a counter of 42 bits (pixels) or 44 bits (TDC triggers) that wraps every 26.8 s /
+// 107.4 s. The paper's rule, a sequential scan: "Each time the ToA of the next pixel or TDC
+// is more than 20 seconds less than the previous one, the global counter of time wrappings is incremented
+// by one and the appropriate integer multiple ... is added to all subsequent data" (:60); and for pixels
+// reported out of order across a wrap: "both large negative and large positive jumps are tracked ... and
+// the appropriate time unwrapping adjustment is applied in each case" (:62) — a jump UP by more than the
+// threshold takes the counter back down by one (R22).
+//
+// The counter after event i is therefore wraps_in + sum_{k <= i} d_k with d_k in {+1, 0, -1} decided by the
+// ADJACENT difference raw[k] - raw[k-1] alone: a prefix sum, not a sequential dependence.
+//   k_unwrap_count   d_k summed per block of 4096 events
+//   k_unwrap_scan    exclusive scan of the block sums (one block); total -> wraps_out
+//   k_unwrap_apply   in-block scan, toa[i] = raw[i] + wraps_i * modulus
+#pragma once
+#include "tpx3_centroid.cuh"
+#include "tpx3_common.cuh"
+
+namespace tpx3 {
+
+constexpr int kUnwrapThreads = 256;
+constexpr int kUnwrapItems = 16;
+constexpr int kUnwrapTile = kUnwrapThreads * kUnwrapItems;   // 4096 events per block
+
+struct UnwrapArgs {
+  uint64_t n;
+  const uint64_t* raw;
+  uint64_t modulus, jump;
+  long long wraps_in;
+  int has_prev;
+  uint64_t prev_raw;
+  uint64_t* out;
+  long long* wraps_out;
+  uint32_t* blk;       // block sums (two's complement)
+  uint32_t nblk;
+};
+
+// +1: the counter wrapped between p and v; -1: v is a pre-wrap value reported after the wrap (or the way back)
+__device__ __forceinline__ int unwrap_delta(uint64_t p, uint64_t v, uint64_t jump) {
+  if (p > v) return p - v > jump ? 1 : 0;
+  return v - p > jump ? -1 : 0;
+}
+
+__device__ __forceinline__ int unwrap_delta_at(const UnwrapArgs& a, uint64_t i) {
+  if (i == 0) return a.has_prev ? unwrap_delta(a.prev_raw, a.raw[0], a.jump) : 0;
+  return unwrap_delta(a.raw[i - 1], a.raw[i], a.jump);
+}
+
+__global__ void __launch_bounds__(kUnwrapThreads) k_unwrap_count(UnwrapArgs a) {
+  __shared__ uint32_t sm[33];
+  const uint64_t base = (uint64_t)blockIdx.x * kUnwrapTile;
+  int s = 0;
+#pragma unroll 4
+  for (int i = 0; i < kUnwrapItems; ++i) {
+    const uint64_t k = base + (uint64_t)i * kUnwrapThreads + threadIdx.x;
+    if (k < a.n) s += unwrap_delta_at(a, k);
+  }
+  uint32_t total;
+  block_exclusive_scan_256((uint32_t)s, sm, &total);
+  if (threadIdx.x == 0) a.blk[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(1024) k_unwrap_scan(UnwrapArgs a) {
+  __shared__ uint32_t warp_sums[32];
+  const uint32_t nblk = a.nblk;
+  const uint32_t per = (nblk + 1023) / 1024;
+  uint32_t beg = threadIdx.x * per, end = beg + per;
+  if (beg > nblk) beg = nblk;
+  if (end > nblk) end = nblk;
+  uint32_t s = 0;
+  for (uint32_t i = beg; i < end; ++i) s += a.blk[i];
+  const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  uint32_t v = s;
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t t = __shfl_up_sync(0xffffffffu, v, o);
+    if (lane >= (uint32_t)o) v += t;
+  }
+  if (lane == 31) warp_sums[w] = v;
+  __syncthreads();
+  uint32_t ws = 0, x = 0;
+  if (w == 0) {
+    ws = warp_sums[lane]; x = ws;
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, x, o);
+      if (lane >= (uint32_t)o) x += t;
+    }
+  }
+  __syncthreads();
+  if (w == 0) {
+    warp_sums[lane] = x - ws;
+    if (lane == 31) *a.wraps_out = a.wraps_in + (long long)(int)x;
+  }
+  __syncthreads();
+  uint32_t run = warp_sums[w] + v - s;
+  for (uint32_t i = beg; i < end; ++i) {
+    const uint32_t t = a.blk[i];
+    a.blk[i] = run;
+    run += t;
+  }
+}
+
+__global__ void __launch_bounds__(kUnwrapThreads) k_unwrap_apply(UnwrapArgs a) {
+  __shared__ uint32_t sm[33];
+  // blocked arrangement: a thread owns 16 consecutive events, so the in-block order is the stream order
+  const uint64_t base = (uint64_t)blockIdx.x * kUnwrapTile + (uint64_t)threadIdx.x * kUnwrapItems;
+  uint64_t v[kUnwrapItems];
+  int pre[kUnwrapItems];
+  int s = 0;
+  uint64_t p = 0;
+  bool havep = false;
+  if (base < a.n) {
+    if (base > 0) { p = a.raw[base - 1]; havep = true; }
+    else if (a.has_prev) { p = a.prev_raw; havep = true; }
+  }
+#pragma unroll
+  for (int i = 0; i < kUnwrapItems; ++i) {
+    const uint64_t k = base + i;
+    v[i] = k < a.n ? a.raw[k] : 0ull;
+    if (k < a.n && havep) s += unwrap_delta(p, v[i], a.jump);
+    pre[i] = s;
+    p = v[i];
+    havep = true;
+  }
+  const uint32_t off = block_exclusive_scan_256((uint32_t)s, sm, nullptr) + a.blk[blockIdx.x];
+#pragma unroll
+  for (int i = 0; i < kUnwrapItems; ++i) {
+    const uint64_t k = base + i;
+    if (k < a.n) {
+      const long long wraps = a.wraps_in + (long long)(int)(off + (uint32_t)pre[i]);
+      a.out[k] = v[i] + (uint64_t)wraps * a.modulus;   // two's complement: a negative count subtracts
+    }
+  }
+}
+
+}  // namespace tpx3

@@ -469,3 +469,50 @@ def test_localmax_edges(tpx3):
     toa = ((1 << 40) + rng.integers(0, 2 * P, n)).astype(np.uint64)
     tot = rng.integers(1, 65536, n)
     check_localmax(tpx3, x, y, toa, tot, 255, 255, 10 * P, what="large")
+
+
+# ------------------------------------------------------------------ ToA unwrapping (NEXT #4)
+def test_unwrap_toa(tpx3):
+    import torch
+    from oracle import preprocess as pp
+
+    m = tpx3
+    mod = (1 << 42) // 256
+    jump = int(20e9 / 1.5625)
+    rng = np.random.default_rng(17)
+
+    def run(raw, modulus, jmp, wraps_in=0, prev=None):
+        raw = np.asarray(raw, dtype=np.uint64)
+        pl = m.plan(m.Config(max_hits=max(len(raw), 1)))
+        out, w = pl.unwrap_toa(to_dev(raw) if len(raw) else torch.empty(0, dtype=torch.uint64, device="cuda"),
+                               modulus, jmp, wraps_in=wraps_in, prev_raw=prev)
+        torch.cuda.synchronize()
+        o, wo = pp.unwrap_toa(raw, modulus, jmp, wraps_in=wraps_in, prev_raw=prev)
+        np.testing.assert_array_equal(out[: len(raw)].cpu().numpy(), o)
+        assert int(w.cpu().numpy()[0]) == wo
+        pl.free()
+        return o, wo
+
+    # the paper's edge case by hand, empty and single inputs, carried state
+    o, w = run([1000, 1019, 3, 1022, 7, 20], 1024, 600)
+    assert o.tolist() == [1000, 1019, 1027, 1022, 1031, 1044] and w == 1
+    run([], 1024, 600, wraps_in=5)
+    run([17], 1024, 600, wraps_in=2, prev=900)
+    run([701, 100, 700, 99, 700], 1024, 600, wraps_in=-1)
+    # several tiles and a ragged tail: 3.3 counter periods with reporting disorder, whole and in chunks
+    n = 300000 + 1234
+    t = np.sort(rng.integers(0, 3 * mod + mod // 3, n).astype(np.int64)) + rng.integers(0, 2000, n) + mod - 5000
+    raw = (t % mod).astype(np.uint64)
+    w0 = int(t[0] // mod)
+    o, w = run(raw, mod, jump, wraps_in=w0)
+    assert np.array_equal(o.astype(np.int64), t)
+    prev, wc = None, w0
+    for a, b in [(0, 4096), (4096, 4097), (4097, 100000), (100000, n)]:
+        oc, wc = run(raw[a:b], mod, jump, wraps_in=wc, prev=prev)
+        assert np.array_equal(oc, o[a:b])
+        prev = int(raw[b - 1])
+    assert wc == w
+    # adversarial: every event jumps (alternating +/-), counter swings negative and back
+    alt = np.where(np.arange(50000) % 2 == 0, 5, 1000).astype(np.uint64)
+    run(alt, 1024, 600)
+    run(rng.integers(0, 1024, 70000), 1024, 300)
