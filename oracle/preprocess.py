@@ -34,3 +34,52 @@ def unwrap_toa(raw, modulus: int, jump: int, wraps_in: int = 0, prev_raw=None):
         out[i] = (v + wraps * modulus) % (1 << 64)
         prev = v
     return out, wraps
+
+
+def timewalk_table(a: float, b: float, c: float, d: float, length: int) -> np.ndarray:
+    """Eq. 1, PAPER.md:74: dToF(ToT; a, b, c, d) = a / (ToT + b)^d + c, evaluated in fp64 for ToT = 0 ..
+    length-1 and rounded to the nearest integer tick (half away from zero) — the calibration product that
+    is "applied to every pixel in the data stream". a, c in ticks; ToT, b in ToT units."""
+    out = np.empty(length, dtype=np.int32)
+    for tot in range(length):
+        base = float(tot) + float(b)
+        v = float(a) / (base ** float(d)) + float(c) if base > 0.0 else float(c)
+        out[tot] = int(np.floor(abs(v) + 0.5)) * (1 if v >= 0 else -1)
+    return out
+
+
+def preprocess(x, y, toa, tot, trig, cut: int, table, P_out: int, shot_base: int = 0):
+    """Section IV.B-C in the paper's order, event by event:
+      shot    s = the most recent laser trigger: the largest s with trig[s] <= toa (PAPER.md:44, 68);
+              events before the first trigger have none and are dropped
+      cut     ToF = toa - trig[s]; the event is written "only ... if its ToF does not exceed 100 us"
+              (PAPER.md:68): keep iff ToF <= cut
+      walk    ToF' = ToF - dToF(ToT) with the calibrated table (Eq. 1, :74-76; ToT beyond the table uses its
+              last entry), clamped to [0, P_out - 1] (reading R23)
+      rebase  toa' = (shot_base + s) * P_out + ToF', so that downstream `shot = toa' div P_out` is the
+              trigger index (reading R6 made exact)
+    Kept events stay in stream order. Returns x', y', toa', tot' and the kept input indices."""
+    trig_l = [int(t) for t in np.asarray(trig)]
+    table = np.asarray(table, dtype=np.int64)
+    xs, ys, ts, os_, idx = [], [], [], [], []
+    for i, t in enumerate(int(v) for v in np.asarray(toa)):
+        lo, hi = 0, len(trig_l)          # bisect_right
+        while lo < hi:
+            mid = (lo + hi) // 2
+            if trig_l[mid] <= t:
+                lo = mid + 1
+            else:
+                hi = mid
+        s = lo - 1
+        if s < 0:
+            continue
+        tof = t - trig_l[s]
+        if tof > cut:
+            continue
+        tt = int(tot[i])
+        corr = int(table[min(tt, len(table) - 1)]) if len(table) else 0
+        tofc = min(max(tof - corr, 0), P_out - 1)
+        xs.append(int(x[i])); ys.append(int(y[i])); os_.append(tt); idx.append(i)
+        ts.append((shot_base + s) * P_out + tofc)
+    return (np.array(xs, dtype=np.uint16), np.array(ys, dtype=np.uint16), np.array(ts, dtype=np.uint64),
+            np.array(os_, dtype=np.uint16), np.array(idx, dtype=np.int64))

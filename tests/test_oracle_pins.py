@@ -536,3 +536,64 @@ def test_unwrap_recovers_true_times(seed):
         parts.append(o)
         prev = raw[b - 1]
     assert np.array_equal(np.concatenate(parts), out) and w == wraps
+
+
+# ------------------------------------------------------------------ preprocessing (NEXT #3)
+def test_timewalk_table_closed_forms():
+    # Eq. 1 at d = 1 ("typically very close to 1", :76): a / (ToT + b) + c, by hand
+    t = pp.timewalk_table(a=1000.0, b=10.0, c=-2.0, d=1.0, length=6)
+    assert t.tolist() == [98, 89, 81, 75, 69, 65]      # 100-2, 90.909-2, 83.33-2, 76.92-2, 71.43-2, 66.67-2
+    # monotone decreasing in ToT for a > 0 (dim pixels walk later), tends to c
+    t = pp.timewalk_table(500.0, 3.0, 1.0, 1.2, 1024)
+    assert np.all(np.diff(t) <= 0) and t[-1] == 1 and t[0] == int(np.floor(500.0 / 3.0 ** 1.2 + 1.0 + 0.5))
+    # a = 0: the constant c, rounded half away from zero
+    assert pp.timewalk_table(0.0, 1.0, 2.5, 1.0, 3).tolist() == [3, 3, 3]
+    assert pp.timewalk_table(0.0, 1.0, -2.5, 1.0, 3).tolist() == [-3, -3, -3]
+
+
+def test_preprocess_hand_example():
+    # triggers at 1000, 2000, 3000 (ticks); cut 300; table: ToT 0..3 -> 9, 5, 2, 0; P_out = 640000
+    trig = [1000, 2000, 3000]
+    toa = [900, 1000, 1300, 1301, 2004, 2999, 3100, 2150, 3003]
+    tot = [1, 1, 2, 2, 0, 3, 9, 1, 1]
+    x = list(range(9)); y = [2 * v for v in x]
+    xs, ys, ts, os_, idx = pp.preprocess(x, y, toa, tot, trig, 300, [9, 5, 2, 0], P)
+    # 900: before the first trigger -> dropped; 1301: ToF 301 > cut -> dropped; 2999: ToF 999 -> dropped
+    assert idx.tolist() == [1, 2, 4, 6, 7, 8]
+    # 1000: ToF 0 - 5 -> clamped to 0; 1300: 300 - 2 = 298 (ToF == cut is kept, "does not exceed");
+    # 2004: 4 - 9 -> 0; 3100: ToT 9 beyond the table -> last entry 0 -> 100; 2150 (out of order in the stream):
+    # trigger 1, 150 - 5; 3003: 3 - 5 -> 0
+    assert ts.tolist() == [0 * P + 0, 0 * P + 298, 1 * P + 0, 2 * P + 100, 1 * P + 145, 2 * P + 0]
+    assert xs.tolist() == [1, 2, 4, 6, 7, 8] and ys.tolist() == [2, 4, 8, 12, 14, 16] and os_.tolist() == [1, 2, 0, 9, 1, 1]
+    # shot_base shifts every shot number
+    assert pp.preprocess(x, y, toa, tot, trig, 300, [9, 5, 2, 0], P, shot_base=7)[2].tolist() == [
+        t + 7 * P for t in ts.tolist()]
+
+
+def test_preprocess_recovers_the_generated_stream():
+    """Generated truth: take a config-2 stream (shot s starts at s*P), move its shots onto irregular trigger
+    times, add timewalk dToF(ToT) to every pixel and sprinkle dark counts later than the cut: preprocessing
+    with the same table must give the original stream back, event for event."""
+    w = gen.generate(2, shots=30)
+    rng = np.random.default_rng(9)
+    trig = np.cumsum(rng.integers(P - 2000, P + 2000, 30)).astype(np.int64) + 12345
+    table = pp.timewalk_table(800.0, 4.0, 0.0, 1.0, 1024)
+    shot = (w.toa // np.uint64(P)).astype(np.int64)
+    tof = (w.toa % np.uint64(P)).astype(np.int64)
+    raw = trig[shot] + tof + table[np.minimum(w.tot, 1023)]
+    keep_cut = int(tof.max() + table.max())
+    # dark counts: ToF beyond the cut, random pixels; merged into the stream by raw time
+    nd = 5000
+    dshot = rng.integers(0, 30, nd)
+    draw = trig[dshot] + rng.integers(keep_cut + 1, P - 3000, nd)
+    allx = np.concatenate([w.x, rng.integers(0, 256, nd).astype(np.uint16)])
+    ally = np.concatenate([w.y, rng.integers(0, 256, nd).astype(np.uint16)])
+    alltot = np.concatenate([w.tot, rng.integers(1, 30, nd).astype(np.uint16)])
+    allraw = np.concatenate([raw, draw]).astype(np.uint64)
+    is_dark = np.concatenate([np.zeros(w.n, bool), np.ones(nd, bool)])
+    order = np.argsort(allraw, kind="stable")
+    xs, ys, ts, os_, idx = pp.preprocess(allx[order], ally[order], allraw[order], alltot[order], trig, keep_cut,
+                                         table, P)
+    assert not np.any(is_dark[order][idx]) and len(idx) == w.n          # exactly the dark counts are cut
+    back = np.argsort(order[idx], kind="stable")                        # original event order
+    assert np.array_equal(ts[back], w.toa) and np.array_equal(xs[back], w.x) and np.array_equal(os_[back], w.tot)
