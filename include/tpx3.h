@@ -157,6 +157,26 @@ int tpx3_unwrap_toa(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64
                     uint64_t modulus, uint64_t jump, int64_t wraps_in, int has_prev, uint64_t prev_raw,
                     uint64_t* toa_out, int64_t* wraps_out);
 
+/* Timewalk calibration product (Eq. 1): table_host[ToT] = a / (ToT + b)^d + c for
+ * ToT = 0 .. length-1, evaluated in fp64 and rounded to the nearest integer tick (half away from
+ * zero; ToT + b <= 0 gives c). a, c in ticks. Host only; table_host int32[length] [host]. */
+int tpx3_timewalk_table(double a, double b, double c, double d, uint32_t length, int32_t* table_host);
+
+/* Preprocessing (section IV.B-C, :66-76) of a pixel stream with
+ * unwrapped ToA against the list of laser triggers trig uint64[n_trig] [dev], ascending. Per event:
+ * s = the most recent trigger (largest s with trig[s] <= ToA; none: dropped), ToF = ToA - trig[s],
+ * dropped if ToF > cut ("does not exceed 100 us", :68), ToF' = ToF - table[min(ToT, table_len-1)]
+ * (int32[table_len] [dev], ticks; table_len = 0: no correction) clamped to [0, P - 1], ToA' =
+ * (shot_base + s) * P + ToF' with P = the plan's shot_period_ticks (must be > 0), so that the
+ * clustering calls see shot = ToA' div P = shot_base + s. Kept events are written in stream order
+ * to x_out, y_out, toa_out, tot_out (capacity n each, [dev], no aliasing of the inputs) and their
+ * input positions to index_out uint32[n] (may be NULL); n_out uint32[1] [dev]. Enqueue only. */
+int tpx3_preprocess(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x,
+                    const uint16_t* y, const uint64_t* toa, const uint16_t* tot, uint64_t n_trig,
+                    const uint64_t* trig, uint64_t cut, const int32_t* table, uint32_t table_len,
+                    uint64_t shot_base, uint16_t* x_out, uint16_t* y_out, uint64_t* toa_out,
+                    uint16_t* tot_out, uint32_t* index_out, uint32_t* n_out);
+
 /* End-to-end variant with HOST buffers: copies x, y, toa, tot [host] to the device, runs
  * tpx3_cluster_centroid and copies perm, label (either may be NULL to skip), the first
  * min(n_clusters, max_clusters) entries of every non-NULL array of `out_host` and the count

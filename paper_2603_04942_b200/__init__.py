@@ -28,7 +28,7 @@ OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_OUT_OF_RANGE, ERR_CUDA, ERR_UNIMPLEMENTED
 # Every symbol include/tpx3.h declares (tests check the built library exports all of them).
 exported_symbols = (
     "tpx3_plan", "tpx3_cluster", "tpx3_centroid", "tpx3_cluster_centroid", "tpx3_localmax_centroid",
-    "tpx3_unwrap_toa", "tpx3_host_io_bytes",
+    "tpx3_unwrap_toa", "tpx3_timewalk_table", "tpx3_preprocess", "tpx3_host_io_bytes",
     "tpx3_process_host", "tpx3_status", "tpx3_launch_count", "tpx3_profile_enable", "tpx3_profile_read",
     "tpx3_free", "tpx3_strerror",
 )
@@ -90,6 +90,11 @@ def load_library(build: bool = True) -> ctypes.CDLL:
                                            ctypes.c_uint32, vp, vp, u64, ctypes.POINTER(_CClusters), u32p]
     lib.tpx3_unwrap_toa.restype = ctypes.c_int
     lib.tpx3_unwrap_toa.argtypes = [vp, vp, vp, u64, vp, u64, u64, ctypes.c_int64, ctypes.c_int, u64, vp, vp]
+    lib.tpx3_timewalk_table.restype = ctypes.c_int
+    lib.tpx3_timewalk_table.argtypes = [ctypes.c_double] * 4 + [ctypes.c_uint32, vp]
+    lib.tpx3_preprocess.restype = ctypes.c_int
+    lib.tpx3_preprocess.argtypes = [vp, vp, vp, u64, vp, vp, vp, vp, u64, vp, u64, vp, ctypes.c_uint32, u64,
+                                    vp, vp, vp, vp, vp, vp]
     lib.tpx3_host_io_bytes.restype = ctypes.c_size_t
     lib.tpx3_host_io_bytes.argtypes = [u64, u64]
     lib.tpx3_process_host.restype = ctypes.c_int
@@ -109,6 +114,17 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.tpx3_strerror.argtypes = [ctypes.c_int]
     _lib = lib
     return lib
+
+
+def timewalk_table(a: float, b: float, c: float, d: float, length: int):
+    """Eq. 1 as an int32 numpy table in ticks (tpx3_timewalk_table, host only)."""
+    import numpy as np
+
+    out = np.empty(int(length), dtype=np.int32)
+    rc = load_library().tpx3_timewalk_table(float(a), float(b), float(c), float(d), int(length), out.ctypes.data)
+    if rc != OK:
+        raise Tpx3Error(rc, "tpx3_timewalk_table")
+    return out
 
 
 def strerror(code: int) -> str:
@@ -213,6 +229,28 @@ class Plan:
         if rc != OK:
             raise Tpx3Error(rc, "tpx3_cluster")
         return perm, label, n_clusters
+
+    # -- preprocessing: trigger assignment, ToF cut, timewalk, rebase (PAPER.md IV.B-C) ------------
+    def preprocess(self, x, y, toa, tot, trig, cut: int, table=None, shot_base: int = 0, stream=None):
+        """Returns (x', y', toa', tot', index, n_out) — device tensors of capacity n and a device count."""
+        import torch
+
+        n = int(x.numel())
+        self._check_inputs(x, y, toa, tot, n)
+        _check_dev(trig, torch.uint64, 0, "trig")
+        if table is not None:
+            _check_dev(table, torch.int32, 0, "table")
+        mk = lambda dt: torch.empty(max(n, 1), dtype=dt, device=self.device)  # noqa: E731
+        xo, yo, to, oo, io = mk(torch.uint16), mk(torch.uint16), mk(torch.uint64), mk(torch.uint16), mk(torch.uint32)
+        n_out = torch.empty(1, dtype=torch.uint32, device=self.device)
+        rc = self.lib.tpx3_preprocess(self.handle, self.workspace.data_ptr(), _stream_ptr(stream), n, x.data_ptr(),
+                                      y.data_ptr(), toa.data_ptr(), tot.data_ptr(), int(trig.numel()),
+                                      trig.data_ptr(), int(cut), 0 if table is None else table.data_ptr(),
+                                      0 if table is None else int(table.numel()), int(shot_base), xo.data_ptr(),
+                                      yo.data_ptr(), to.data_ptr(), oo.data_ptr(), io.data_ptr(), n_out.data_ptr())
+        if rc != OK:
+            raise Tpx3Error(rc, "tpx3_preprocess")
+        return xo, yo, to, oo, io, n_out
 
     # -- ToA counter unwrapping (PAPER.md IV.A) ----------------------------------------------------
     def unwrap_toa(self, raw, modulus: int, jump: int, wraps_in: int = 0, prev_raw=None, out=None, wraps_out=None,

@@ -1,6 +1,7 @@
 // libtpx3 — host side of the C ABI declared in include/tpx3.h: plan, workspace layout, kernel
 // launches. All device work is enqueued on the caller's stream; nothing here synchronises
 // except tpx3_status and tpx3_process_host (which say so in the header).
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -11,6 +12,7 @@
 #include "tpx3_fused.cuh"
 #include "tpx3_link.cuh"
 #include "tpx3_localmax.cuh"
+#include "tpx3_preprocess.cuh"
 #include "tpx3_sort.cuh"
 #include "tpx3_unwrap.cuh"
 
@@ -454,6 +456,43 @@ int tpx3_unwrap_toa(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t 
   if (a.nblk) TPX3_LAUNCH(p, k_unwrap_count, a.nblk, kUnwrapThreads, 0, st, a);
   TPX3_LAUNCH(p, k_unwrap_scan, 1, 1024, 0, st, a);
   if (a.nblk) TPX3_LAUNCH(p, k_unwrap_apply, a.nblk, kUnwrapThreads, 0, st, a);
+  return cuda_ok(cudaGetLastError());
+}
+
+int tpx3_timewalk_table(double a, double b, double c, double d, uint32_t length, int32_t* table_host) {
+  if (!table_host && length) return TPX3_ERR_INVALID_ARG;
+  for (uint32_t tot = 0; tot < length; ++tot) {
+    const double base = (double)tot + b;
+    const double v = base > 0.0 ? a / std::pow(base, d) + c : c;   // Eq. 1
+    const double r = std::floor(std::fabs(v) + 0.5);                // nearest tick, half away from zero
+    table_host[tot] = (int32_t)(v >= 0.0 ? r : -r);
+  }
+  return TPX3_OK;
+}
+
+int tpx3_preprocess(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x,
+                    const uint16_t* y, const uint64_t* toa, const uint16_t* tot, uint64_t n_trig,
+                    const uint64_t* trig, uint64_t cut, const int32_t* table, uint32_t table_len, uint64_t shot_base,
+                    uint16_t* x_out, uint16_t* y_out, uint64_t* toa_out, uint16_t* tot_out, uint32_t* index_out,
+                    uint32_t* n_out) {
+  if (!p || !workspace || !n_out) return TPX3_ERR_INVALID_ARG;
+  if (n > p->cfg.max_hits || p->cfg.shot_period_ticks == 0) return TPX3_ERR_INVALID_ARG;
+  if (n && (!x || !y || !toa || !tot || !x_out || !y_out || !toa_out || !tot_out)) return TPX3_ERR_INVALID_ARG;
+  if ((n_trig && !trig) || (table_len && !table)) return TPX3_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  Ws w = carve(p, workspace);
+  PreArgs a;
+  a.n = n; a.x = x; a.y = y; a.tot = tot; a.toa = toa; a.n_trig = n_trig; a.trig = trig; a.cut = cut;
+  a.P = p->cfg.shot_period_ticks; a.shot_base = shot_base; a.table = table; a.table_len = table_len;
+  a.x_out = x_out; a.y_out = y_out; a.tot_out = tot_out; a.toa_out = toa_out; a.index_out = index_out;
+  a.n_out = n_out;
+  a.tmp = w.keyA;       // 8 bytes per event
+  a.blk = w.counts;     // the sort's digit counters: room for 2^28 / 4096 block counts
+  a.nblk = (uint32_t)((n + kPreTile - 1) / kPreTile);
+  if (a.nblk) TPX3_LAUNCH(p, k_pre_mark, a.nblk, kPreThreads, 0, st, a);
+  TPX3_LAUNCH(p, k_pre_scan, 1, 1024, 0, st, a);
+  if (a.nblk) TPX3_LAUNCH(p, k_pre_scatter, a.nblk, kPreThreads, 0, st, a);
   return cuda_ok(cudaGetLastError());
 }
 

@@ -105,3 +105,15 @@ def test_shard_shots_partition():
             assert all(r[k][1] == r[k + 1][0] for k in range(ws - 1))
             sizes = [b - a for a, b in r]
             assert max(sizes) - min(sizes) <= 1
+
+
+def test_timewalk_table_host_helper_matches_the_oracle():
+    """tpx3_timewalk_table is host-only (Eq. 1): both sides evaluate it in fp64 and round to the
+    nearest tick, so the tables must be identical."""
+    import numpy as np
+    from oracle import preprocess as pp
+
+    for a, b, c, d, n in [(1000.0, 10.0, -2.0, 1.0, 64), (800.0, 4.0, 0.0, 1.0, 1024), (500.0, 3.0, 1.0, 1.2, 1024),
+                          (0.0, 1.0, 2.5, 1.0, 8), (123.456, 0.0, -7.25, 0.9, 300), (50.0, -2.0, 0.0, 1.0, 16)]:
+        assert np.array_equal(m.timewalk_table(a, b, c, d, n), pp.timewalk_table(a, b, c, d, n)), (a, b, c, d)
+    assert m.timewalk_table(1.0, 1.0, 1.0, 1.0, 0).shape == (0,)

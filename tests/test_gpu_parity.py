@@ -516,3 +516,83 @@ def test_unwrap_toa(tpx3):
     alt = np.where(np.arange(50000) % 2 == 0, 5, 1000).astype(np.uint64)
     run(alt, 1024, 600)
     run(rng.integers(0, 1024, 70000), 1024, 300)
+
+
+# ------------------------------------------------------------------ preprocessing (NEXT #3)
+def test_preprocess(tpx3):
+    import torch
+    from oracle import preprocess as pp
+
+    m = tpx3
+
+    def run(x, y, toa, tot, trig, cut, table, shot_base=0):
+        x = np.asarray(x, dtype=np.uint16); y = np.asarray(y, dtype=np.uint16)
+        toa = np.asarray(toa, dtype=np.uint64); tot = np.asarray(tot, dtype=np.uint16)
+        trig = np.asarray(trig, dtype=np.uint64)
+        n = len(x)
+        pl = m.plan(m.Config(max_hits=max(n, 1), shot_period_ticks=P))
+        dv = lambda a, dt: to_dev(a) if len(a) else torch.empty(0, dtype=dt, device="cuda")  # noqa: E731
+        tb = None if table is None else to_dev(np.asarray(table, dtype=np.int32))
+        xo, yo, to, oo, io, no = pl.preprocess(dv(x, torch.uint16), dv(y, torch.uint16), dv(toa, torch.uint64),
+                                               dv(tot, torch.uint16), dv(trig, torch.uint64), cut, tb, shot_base)
+        torch.cuda.synchronize()
+        k = int(no.cpu().numpy()[0])
+        ex, ey, et, eo, ei = pp.preprocess(x, y, toa, tot, trig, cut, [] if table is None else table, P, shot_base)
+        assert k == len(ei)
+        np.testing.assert_array_equal(xo[:k].cpu().numpy(), ex)
+        np.testing.assert_array_equal(yo[:k].cpu().numpy(), ey)
+        np.testing.assert_array_equal(to[:k].cpu().numpy(), et)
+        np.testing.assert_array_equal(oo[:k].cpu().numpy(), eo)
+        np.testing.assert_array_equal(io[:k].cpu().numpy().astype(np.int64), ei)
+        pl.free()
+        return k, (xo[:k], yo[:k], to[:k], oo[:k])
+
+    # hand example of the oracle pins (cut edge, clamp, ToT beyond the table, out-of-order event, no trigger yet)
+    k, _ = run(list(range(9)), [2 * v for v in range(9)], [900, 1000, 1300, 1301, 2004, 2999, 3100, 2150, 3003],
+               [1, 1, 2, 2, 0, 3, 9, 1, 1], [1000, 2000, 3000], 300, [9, 5, 2, 0], shot_base=7)
+    assert k == 6
+    # degenerate inputs: nothing in, no triggers (everything dropped), no table
+    run([], [], [], [], [5], 10, [1])
+    assert run([1, 2], [3, 4], [100, 200], [5, 6], [], 10, [1])[0] == 0
+    assert run([1, 2], [3, 4], [100, 200], [5, 6], [50], 1000, None)[0] == 2
+    # a config-2 stream moved onto irregular triggers, with timewalk and dark counts: several tiles, ragged tail
+    w = gen.generate(2, shots=400)
+    rng = np.random.default_rng(9)
+    trig = np.cumsum(rng.integers(P - 2000, P + 2000, w.shots)).astype(np.int64) + 12345
+    table = pp.timewalk_table(800.0, 4.0, 0.0, 1.0, 1024)
+    assert np.array_equal(table, m.timewalk_table(800.0, 4.0, 0.0, 1.0, 1024))
+    shot = (w.toa // np.uint64(P)).astype(np.int64)
+    tof = (w.toa % np.uint64(P)).astype(np.int64)
+    raw = trig[shot] + tof + table[np.minimum(w.tot, 1023)]
+    cut = int(tof.max() + table.max())
+    nd = w.n // 10
+    draw = trig[rng.integers(0, w.shots, nd)] + rng.integers(cut + 1, P - 3000, nd)
+    allx = np.concatenate([w.x, rng.integers(0, 256, nd).astype(np.uint16)])
+    ally = np.concatenate([w.y, rng.integers(0, 256, nd).astype(np.uint16)])
+    alltot = np.concatenate([w.tot, rng.integers(1, 30, nd).astype(np.uint16)])
+    allraw = np.concatenate([raw, draw]).astype(np.uint64)
+    order = np.argsort(allraw, kind="stable")
+    k, dev = run(allx[order], ally[order], allraw[order], alltot[order], trig, cut, table)
+    assert k == w.n
+    # and the preprocessed stream, clustered on the device, gives the hits of the original stream (the corrected
+    # stream is ordered by raw time, i.e. out of ToA order inside a shot: the sort runs)
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P)
+    pl = m.plan(m.Config(max_hits=k, toa_window_ticks=W, shot_period_ticks=P, max_shot_hits=gen.max_shot_hits(2)))
+    cl = m.Clusters(k, pl.device)
+    perm, label, nc = pl.cluster_centroid(*[t.contiguous() for t in dev], cl)
+    torch.cuda.synchronize()
+    assert pl.status()["error"] == 0
+    ncl = int(nc.cpu().numpy()[0])
+    assert ncl == o["n_clusters"]
+    g = cl.numpy(ncl)
+    # events of equal ToA are delivered in a different order here than in w, so the stable sort and with it the
+    # listing order of hits inside a shot may differ: compare the hits as a set of rows
+    keys = ("c_shot", "c_toa_peak", "c_sum_tot_x", "c_sum_tot_y", "c_sum_tot", "c_size", "c_sum_tot_tof")
+
+    def rows(d):
+        r = np.stack([d[k2].astype(np.int64) for k2 in keys] + [d["c_cx"].view(np.int32).astype(np.int64),
+                     d["c_cy"].view(np.int32).astype(np.int64), d["c_ctof"].view(np.int32).astype(np.int64)], axis=1)
+        return r[np.lexsort(r.T[::-1])]
+
+    np.testing.assert_array_equal(rows(g), rows(o))
+    pl.free()
