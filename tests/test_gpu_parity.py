@@ -596,3 +596,21 @@ def test_preprocess(tpx3):
 
     np.testing.assert_array_equal(rows(g), rows(o))
     pl.free()
+
+
+@pytest.mark.parametrize("side,per_shot,hint,Wr", [(6, 900, 1024, 320), (12, 3000, 4096, 40), (3, 400, 512, 5),
+                                                   (40, 2000, 2048, 2), (16, 1000, 1024, 100000)])
+def test_fused_dense_repeated_addresses(tpx3, side, per_shot, hint, Wr):
+    """Shot-contiguous streams whose events crowd a few pixels: many events per (shot, pixel), overflowing
+    hash buckets, more deferred links than the list holds — the fused kernel's rare paths — in all three
+    tile variants, delivered out of order inside each shot."""
+    rng = np.random.default_rng(side * 1000 + per_shot)
+    shots = 60
+    n = shots * per_shot
+    shot = np.repeat(np.arange(shots), per_shot)
+    x = rng.integers(100, 100 + side, n); y = rng.integers(250 - side, 256, n) % 256
+    tof = rng.integers(0, 3000, n)
+    toa = (shot * P + tof).astype(np.uint64)
+    tot = rng.integers(1, 1024, n)
+    res, _ = check(tpx3, x, y, toa, tot, W=Wr, modes=("fused",), max_shot_hits=hint, what="dense %d" % side)
+    assert res["status"]["path"] == 1
