@@ -583,13 +583,14 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         const uint32_t want = c << 16;
         const uint32_t d0 = (e.x ^ want) - 1u, d1 = (e.y ^ want) - 1u, d2 = (e.z ^ want) - 1u,
                        d3 = ((e.w & ~0x8000u) ^ want) - 1u;
-        const bool m0 = d0 < lim, m1 = d1 < lim, m2 = d2 < lim, m3 = d3 < lim;
-        const uint32_t nm = (uint32_t)m0 + (uint32_t)m1 + (uint32_t)m2 + (uint32_t)m3;
-        const uint32_t j = m0 ? d0 : (m1 ? d1 : (m2 ? d2 : d3));
-        const bool any = valid && nm != 0u;
-        jc = any ? j : k;
+        // a slot of this cell gives d < lim, any other slot (other cell, empty) a d >= 65535: the smallest d
+        // is the candidate, and a second-smallest d below lim means the cell holds several events
+        const uint32_t mn01 = min(d0, d1), mx01 = max(d0, d1), mn23 = min(d2, d3), mx23 = max(d2, d3);
+        const uint32_t s1 = min(mn01, mn23), s2 = min(max(mn01, mn23), min(mx01, mx23));
+        const bool any = valid && s1 < lim;
+        jc = any ? s1 : k;
         kc = recS[jc].x;
-        if (valid && (nm > 1u || (e.w & 0x8000u))) slow |= bit;
+        if (valid && (s2 < lim || (e.w & 0x8000u))) slow |= bit;
         return any && absdiff_u32(kc, key) <= a.W;
       };
       uint32_t jS, kS, jE, kE, jSE, kSE, jSW, kSW, jO, kO;
