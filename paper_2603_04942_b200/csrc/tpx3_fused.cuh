@@ -40,6 +40,7 @@
 // then redo the call.
 #pragma once
 #include "tpx3_common.cuh"
+#include "tpx3_localmax.cuh"
 
 namespace tpx3 {
 
@@ -138,6 +139,9 @@ struct FusedArgs {
   uint4* stage_b;      //                                            {sum tot*x (lo, hi), sum tot*y (lo, hi)}
   uint64_t* stage_c;   //                                            ToA of the brightest pixel
   uint64_t* stage_d;   //                                            sum tot*tof
+  uint32_t mode;       // 0: hit = connected component (north_star); 1: paper-literal mode, hit = local ToT
+                       //    maximum of the box (lm_wx, lm_wy, W) and sums over that box (tpx3_localmax.cuh)
+  uint32_t lm_wx, lm_wy;
 };
 
 constexpr uint32_t kNone = 0xFFFFFFFFu;
@@ -206,7 +210,8 @@ __device__ __forceinline__ void uf_unite(uint16_t* par, uint32_t a, uint32_t b) 
 }
 
 // One tile per CTA. T = tile capacity (events), THREADS = T / 8.
-template <int T, int THREADS>
+// MODE 0: hit = connected component (north_star). MODE 1: paper-literal mode (FusedArgs::mode).
+template <int T, int THREADS, int MODE>
 __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))) k_fused_shot_tiles(FusedArgs a) {
   constexpr int IPT = T / THREADS;  // 8 events per thread
   static_assert(IPT == 8, "the 128-bit load phase assumes 8 events per thread");
@@ -523,26 +528,14 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   uint32_t* cnt32 = reinterpret_cast<uint32_t*>(smem + L::kPar);   // bucket fill counters, u16 pairs
   uint16_t* par = reinterpret_cast<uint16_t*>(smem + L::kPar);     // parent (after the insert step)
   uint32_t* list = reinterpret_cast<uint32_t*>(smem + L::kList);   // deferred links k << 16 | j
+  uint32_t* head = reinterpret_cast<uint32_t*>(hreg + 4 * T);           // [T] member chain head per label
+  // mode 1 keeps the hash table alive until the end: its marks go where mode 0 keeps the parents, and the
+  // ordinal list may overwrite them (the ordinal step has read every mark before it writes the first ordinal)
+  uint16_t* lab = MODE ? reinterpret_cast<uint16_t*>(smem + L::kPar)
+                       : reinterpret_cast<uint16_t*>(hreg + 8 * T);     // [T] label per event
+  uint16_t* rootpos = MODE ? lab : reinterpret_cast<uint16_t*>(hreg + 10 * T);   // [T] ordinal -> label
+  uint16_t* nxt = reinterpret_cast<uint16_t*>(hreg + 12 * T);           // [T] next member of the same hit
 
-  // ---- hash insert: entry = cell << 16 | k+1 into bucket hash(shot offset, cell) ------------------
-  // Slot c of a bucket is taken by the c-th arrival (counter); arrivals past the 4th mark the bucket
-  // (bit 15 of slot 3) and spill to the next bucket.
-  for (uint32_t k = tid; k < mm; k += THREADS) {
-    const uint2 r = recS[k];
-    const uint32_t cell = r.y & 0xFFFFu, slk = r.x >> tb;
-    uint32_t h = ((cell | (slk << 16)) * kGold) >> kHashShift;
-    const uint32_t entry = (cell << 16) | (k + 1u);
-    for (;;) {
-      const uint32_t sh = (h & 1u) * 16u;
-      const uint32_t c = (atomicAdd(&cnt32[h >> 1], 1u << sh) >> sh) & 0xFFFFu;
-      if (c < 4u) { atomicOr(&tab[4u * h + c], entry); break; }
-      atomicOr(&tab[4u * h + 3u], 0x8000u);
-      h = (h + 1u) & (NB - 1u);
-    }
-  }
-  __syncthreads();
-
-  // ---- S2: probe the forward cells, prune implied links, first link = parent, others deferred ---
   // Scans one neighbour cell completely (home bucket and, while marked, the following ones) and
   // hands every event that passes the time test to `sink`. Used for the rare cases only.
   auto scan_cell = [&](uint32_t c, uint32_t slk, uint32_t key, uint32_t lim, auto&& sink) {
@@ -563,6 +556,82 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       h = (h + 1u) & (NB - 1u);
     }
   };
+  // hash insert: entry = cell << 16 | k+1 into bucket hash(shot offset, cell). Slot c of a bucket is taken by
+  // the c-th arrival (counter); arrivals past the 4th mark the bucket (bit 15 of slot 3) and spill to the next.
+  auto hash_insert = [&]() {
+    for (uint32_t k = tid; k < mm; k += THREADS) {
+      const uint2 r = recS[k];
+      const uint32_t cell = r.y & 0xFFFFu, slk = r.x >> tb;
+      uint32_t h = ((cell | (slk << 16)) * kGold) >> kHashShift;
+      const uint32_t entry = (cell << 16) | (k + 1u);
+      for (;;) {
+        const uint32_t sh = (h & 1u) * 16u;
+        const uint32_t c = (atomicAdd(&cnt32[h >> 1], 1u << sh) >> sh) & 0xFFFFu;
+        if (c < 4u) { atomicOr(&tab[4u * h + c], entry); break; }
+        atomicOr(&tab[4u * h + 3u], 0x8000u);
+        h = (h + 1u) & (NB - 1u);
+      }
+    }
+  };
+  // mode 1 with a small box: the neighbours are found through the hash, (2 wx + 1)(2 wy + 1) cells per event;
+  // a large box is cheaper to serve by walking the time window of the sorted tile
+  const bool lm_grid = MODE != 0 && (2u * a.lm_wx + 1u) * (2u * a.lm_wy + 1u) <= 81u;
+  // calls sink(j) for every event j of the box of event (cell, slk, key), the event itself included
+  auto scan_box = [&](uint32_t cell, uint32_t slk, uint32_t key, auto&& sink) {
+    const uint32_t x = cell & 0xFFu, y = cell >> 8;
+    const uint32_t x0 = x > a.lm_wx ? x - a.lm_wx : 0u, x1 = min(x + a.lm_wx, a.sensor_w - 1u);
+    const uint32_t y0 = y > a.lm_wy ? y - a.lm_wy : 0u, y1 = min(y + a.lm_wy, a.sensor_h - 1u);
+    for (uint32_t yy = y0; yy <= y1; ++yy)
+      for (uint32_t xx = x0; xx <= x1; ++xx) scan_cell((yy << 8) | xx, slk, key, (uint32_t)T, sink);
+  };
+
+  if (MODE != 0 && lm_grid) {
+    // ---- paper-literal mode (Eq. 5-7, :122-150) through the hash: k is a hit if no event of its box —
+    //      same shot, |dX| <= wx, |dY| <= wy, |dToF| <= W, all inclusive — has a greater (ToT, sorted index)
+    hash_insert();
+    __syncthreads();
+    for (uint32_t k = tid; k < mm; k += THREADS) {
+      const uint2 r = recS[k];
+      const uint32_t ti = r.y >> 16;
+      bool is_max = true;
+      scan_box(r.y & 0xFFFFu, r.x >> tb, r.x, [&](uint32_t j) {
+        const uint32_t tj = recS[j].y >> 16;
+        if (tj > ti || (tj == ti && j > k)) is_max = false;      // equal ToT: the later pixel wins (:150)
+      });
+      // the marks overwrite the bucket counters (dead since the insert barrier), not the table
+      a.label[out_base + k] = is_max ? out_base + k : kNone;
+      lab[k] = is_max ? (uint16_t)k : (uint16_t)0xFFFFu;
+    }
+    __syncthreads();
+  } else if (MODE != 0) {
+    // ---- paper-literal mode (Eq. 5-7, :122-150): k is a hit if no event of its box — same shot,
+    //      |dX| <= wx, |dY| <= wy, |dToF| <= W, all inclusive — has a greater (ToT, sorted index). The keys
+    //      ascend and keys of different shots differ by more than W, so the time neighbours of k are one
+    //      contiguous run of the sorted tile around k: walk it in shared memory, stop at the first brighter one
+    for (uint32_t k = tid; k < mm; k += THREADS) {
+      const uint2 r = recS[k];
+      const uint32_t ti = r.y >> 16;
+      bool is_max = true;
+      for (uint32_t j = k; is_max && j-- > 0u;) {
+        const uint2 q = recS[j];
+        if (r.x - q.x > a.W) break;
+        if ((q.y >> 16) > ti && lm_near(r.y, q.y, a.lm_wx, a.lm_wy)) is_max = false;    // earlier: strictly brighter
+      }
+      for (uint32_t j = k + 1u; is_max && j < mm; ++j) {
+        const uint2 q = recS[j];
+        if (q.x - r.x > a.W) break;
+        if ((q.y >> 16) >= ti && lm_near(r.y, q.y, a.lm_wx, a.lm_wy)) is_max = false;   // later: wins ties (:150)
+      }
+      lab[k] = is_max ? (uint16_t)k : (uint16_t)0xFFFFu;
+      a.label[out_base + k] = is_max ? out_base + k : kNone;
+    }
+    __syncthreads();
+  } else {
+  // ---- hash insert ----------------------------------------------------------------------------------
+  hash_insert();
+  __syncthreads();
+
+  // ---- S2: probe the forward cells, prune implied links, first link = parent, others deferred ---
   auto push_link = [&](uint32_t k, uint32_t j) {
     const uint32_t pos = atomicAdd(&misc->n_list, 1u);
     if (pos < (uint32_t)L::kListCap) list[pos] = (k << 16) | j;
@@ -670,10 +739,6 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 
   // ---- S3: label = smallest sorted index of the component ------------------------------------------
   uint32_t* minidx = reinterpret_cast<uint32_t*>(hreg);                 // [T] by root
-  uint32_t* head = reinterpret_cast<uint32_t*>(hreg + 4 * T);           // [T] member chain head per label
-  uint16_t* lab = reinterpret_cast<uint16_t*>(hreg + 8 * T);            // [T] label per event
-  uint16_t* rootpos = reinterpret_cast<uint16_t*>(hreg + 10 * T);       // [T] ordinal -> label
-  uint16_t* nxt = reinterpret_cast<uint16_t*>(hreg + 12 * T);           // [T] next member of the same hit
   {
     uint4* f = reinterpret_cast<uint4*>(hreg);
     const uint4 ones = make_uint4(kNone, kNone, kNone, kNone);
@@ -717,6 +782,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     }
   }
   __syncthreads();
+  }   // mode 0
   uint32_t n_roots;
   {
     // blocked arrangement: thread owns sorted positions [8 tid, 8 tid + 8)
@@ -758,6 +824,63 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   // ---- S4: one thread per hit walks its chain: exact sums, brightest pixel. The hit goes to the
   //      staging table at the tile's own position out_base + c (a tile has no more hits than events);
   //      k_fused_compact moves it to its ordinal once every tile's count is known -------------------
+  if (MODE != 0 && lm_grid) {
+    // paper-literal mode: the row sums of Eq. 9 over the box about every local maximum
+    for (uint32_t c = tid; c < n_roots; c += THREADS) {
+      const uint32_t r = rootpos[c];
+      const uint2 rr = recS[r];
+      unsigned long long sx = 0, sy = 0, sf = 0;
+      uint32_t st = 0, size = 0;
+      scan_box(rr.y & 0xFFFFu, rr.x >> tb, rr.x, [&](uint32_t j) {   // j == r included: A_ii = 1 (Eq. 4 diagonal)
+        const uint2 q = recS[j];
+        const uint32_t t = q.y >> 16;
+        ++size;
+        st += t;
+        sx += (unsigned long long)(t * (q.y & 0xFFu));
+        sy += (unsigned long long)(t * ((q.y >> 8) & 0xFFu));
+        sf += (unsigned long long)t * (unsigned long long)(q.x & tmask);
+      });
+      const uint64_t o = (uint64_t)out_base + c;
+      a.stage_a[o] = make_uint4(out_base + r, size, st, 0u);
+      a.stage_b[o] = make_uint4((uint32_t)sx, (uint32_t)(sx >> 32), (uint32_t)sy, (uint32_t)(sy >> 32));
+      a.stage_c[o] = ref + (uint64_t)(rr.x >> tb) * a.P + (uint64_t)(rr.x & tmask);
+      a.stage_d[o] = sf;
+    }
+  } else if (MODE != 0) {
+    // the same by walking the time window of the sorted tile (large boxes)
+    for (uint32_t c = tid; c < n_roots; c += THREADS) {
+      const uint32_t r = rootpos[c];
+      const uint2 rr = recS[r];
+      unsigned long long sx = 0, sy = 0, sf = 0;
+      uint32_t st = 0, size = 0;
+      auto add = [&](const uint2 q) {
+        if (lm_near(rr.y, q.y, a.lm_wx, a.lm_wy)) {
+          const uint32_t t = q.y >> 16;
+          ++size;
+          st += t;
+          sx += (unsigned long long)(t * (q.y & 0xFFu));
+          sy += (unsigned long long)(t * ((q.y >> 8) & 0xFFu));
+          sf += (unsigned long long)t * (unsigned long long)(q.x & tmask);
+        }
+      };
+      add(rr);                                    // A_ii = 1 (Eq. 4 diagonal)
+      for (uint32_t j = r; j-- > 0u;) {
+        const uint2 q = recS[j];
+        if (rr.x - q.x > a.W) break;
+        add(q);
+      }
+      for (uint32_t j = r + 1u; j < mm; ++j) {
+        const uint2 q = recS[j];
+        if (q.x - rr.x > a.W) break;
+        add(q);
+      }
+      const uint64_t o = (uint64_t)out_base + c;
+      a.stage_a[o] = make_uint4(out_base + r, size, st, 0u);
+      a.stage_b[o] = make_uint4((uint32_t)sx, (uint32_t)(sx >> 32), (uint32_t)sy, (uint32_t)(sy >> 32));
+      a.stage_c[o] = ref + (uint64_t)(rr.x >> tb) * a.P + (uint64_t)(rr.x & tmask);
+      a.stage_d[o] = sf;
+    }
+  } else
   for (uint32_t c = tid; c < n_roots; c += THREADS) {
     const uint32_t r = rootpos[c];
     unsigned long long sx = 0, sy = 0, sf = 0;
@@ -861,7 +984,7 @@ __global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, 
   if (t1 == a.num_tiles && tid == 0) {
     *a.n_clusters = (uint32_t)prefix;
     a.ctrl->status.n_clusters = (uint32_t)prefix;
-    a.ctrl->status.path = 1;
+    a.ctrl->status.path = a.mode ? 3 : 1;
     a.ctrl->status.sort_passes = 0;
   }
 }
@@ -885,9 +1008,9 @@ inline FusedGeom fused_geom(uint64_t P, uint32_t W, uint32_t max_shot_hits) {
   return g;
 }
 
-template <int T, int THREADS>
+template <int T, int THREADS, int MODE>
 inline int launch_fused(const FusedArgs& a, cudaStream_t st) {
-  auto kern = k_fused_shot_tiles<T, THREADS>;
+  auto kern = k_fused_shot_tiles<T, THREADS, MODE>;
   static bool configured = false;   // per process; the attribute is per function and device-wide
   if (!configured) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, FusedSmem<T>::kBytes) != cudaSuccess)
@@ -903,7 +1026,7 @@ inline int enqueue_fused(const FusedGeom& g, uint64_t* launches, Ctrl* ctrl, uns
                          cudaStream_t st, const Params& prm, const uint16_t* x, const uint16_t* y,
                          const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label,
                          uint64_t max_clusters, const tpx3_clusters_t& out, uint32_t* n_clusters, void* stage,
-                         bool* launched) {
+                         bool* launched, uint32_t mode = 0, uint32_t lm_wx = 0, uint32_t lm_wy = 0) {
   *launched = false;
   if (g.variant == 0 || prm.n == 0) return TPX3_OK;
   // the 128-bit load phase needs 16-byte aligned inputs (PyTorch allocations are 256-byte aligned)
@@ -931,7 +1054,14 @@ inline int enqueue_fused(const FusedGeom& g, uint64_t* launches, Ctrl* ctrl, uns
   a.stage_b = a.stage_a + prm.n;
   a.stage_c = reinterpret_cast<uint64_t*>(a.stage_b + prm.n);
   a.stage_d = a.stage_c + prm.n;
-  int rc = g.variant == 3 ? launch_fused<2048, 256>(a, st) : g.variant == 1 ? launch_fused<4096, 512>(a, st) : launch_fused<8192, 1024>(a, st);
+  a.mode = mode; a.lm_wx = lm_wx; a.lm_wy = lm_wy;
+  int rc;
+  if (mode == 0u)
+    rc = g.variant == 3 ? launch_fused<2048, 256, 0>(a, st)
+                        : g.variant == 1 ? launch_fused<4096, 512, 0>(a, st) : launch_fused<8192, 1024, 0>(a, st);
+  else
+    rc = g.variant == 3 ? launch_fused<2048, 256, 1>(a, st)
+                        : g.variant == 1 ? launch_fused<4096, 512, 1>(a, st) : launch_fused<8192, 1024, 1>(a, st);
   if (rc != TPX3_OK) return rc;
   ++*launches;
   uint32_t ctas = a.num_tiles < (uint32_t)(kNumSMs * 8) ? a.num_tiles : (uint32_t)(kNumSMs * 8);

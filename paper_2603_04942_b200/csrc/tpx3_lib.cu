@@ -128,6 +128,8 @@ struct GenArgs {
   uint32_t *perm, *label, *n_clusters;
   uint64_t max_clusters;
   tpx3_clusters_t out;
+  uint32_t lm_wx, lm_wy;   // paper-literal mode: box half-widths
+  uint64_t lm_wt;
 };
 
 __host__ __device__ inline uint32_t grid_for_hd(uint64_t n, int threads, int num_sms, int per_sm = 8) {
@@ -192,6 +194,27 @@ __host__ __device__ inline uint32_t grid_for_hd(uint64_t n, int threads, int num
        (A).prm, (A).toa, (A).perm, (A).n_clusters, (A).max_clusters, (A).out, (A).w.peak);                            \
   } while (0)
 
+// Paper-literal mode on the general kernels: the sort stage, then the window walks of tpx3_localmax.cuh. The
+// link stage's buffers hold the sorted records (slab: ToA, xy: x | y << 8 | tot << 16); the centroid stage's
+// ordinal kernels run on lmax (passed as `label`) in place of the labels.
+#define TPX3_LOCALMAX_SEQUENCE(A)                                                                                     \
+  do {                                                                                                                \
+    TPX3_GENERAL_SORT_SEQUENCE(A);                                                                                    \
+    const uint64_t m_ = (A).prm.n;                                                                                    \
+    GP(TPX3_STAGE_LINK, k_lm_gather, grid_for_hd(m_, 256, (A).sms), 256, m_, (A).perm, (A).x, (A).y, (A).toa,         \
+       (A).tot, (A).w.slab, (A).w.xy);                                                                                \
+    GP(TPX3_STAGE_LINK, k_lm_flag, grid_for_hd(m_, 256, (A).sms, 16), 256, m_, (A).prm.P, (A).lm_wx, (A).lm_wy,       \
+       (A).lm_wt, (A).w.slab, (A).w.xy, (A).label);                                                                   \
+    GP(TPX3_STAGE_CENTROID, k_root_count, (A).cent_nblk, kCentThreads, (A).w.ctrl, 0, m_, (A).label, (A).w.blkcnt);   \
+    GP(TPX3_STAGE_CENTROID, k_root_scan, 1, 1024, (A).w.ctrl, 0, (A).w.blkcnt, (A).cent_nblk, (A).max_clusters,       \
+       (A).n_clusters);                                                                                               \
+    GP(TPX3_STAGE_CENTROID, k_root_slots, (A).cent_nblk, kCentThreads, (A).w.ctrl, 0, m_, (A).label, (A).w.blkcnt,    \
+       (A).w.slot, (A).max_clusters, (A).out, (A).w.peak);                                                            \
+    GP(TPX3_STAGE_CENTROID, k_lm_emit, grid_for_hd((A).max_clusters < m_ ? (A).max_clusters : m_, 128, (A).sms, 16),  \
+       128, (A).w.ctrl, m_, (A).prm.P, (A).lm_wx, (A).lm_wy, (A).lm_wt, (A).w.slab, (A).w.xy, (A).n_clusters,         \
+       (A).max_clusters, (A).out);                                                                                    \
+  } while (0)
+
 // Device-side fallback: one tiny kernel behind the fused path. If the fused kernel could not serve
 // the call it enqueues the whole general path as tail launches (they run, in order, after this grid
 // and before anything the host enqueued later on the stream). A successful fused call thus pays for
@@ -201,6 +224,14 @@ __global__ void k_fallback_dispatch(GenArgs a) {
 #define GP(stage, kernel, grid, block, ...) kernel<<<(grid), (block), 0, cudaStreamTailLaunch>>>(__VA_ARGS__)
   TPX3_GENERAL_CLUSTER_SEQUENCE(a);
   TPX3_GENERAL_CENTROID_SEQUENCE(a);
+#undef GP
+}
+
+// The same for the paper-literal mode.
+__global__ void k_fallback_dispatch_lm(GenArgs a) {
+  if (a.w.ctrl->fused_state == 1u) return;
+#define GP(stage, kernel, grid, block, ...) kernel<<<(grid), (block), 0, cudaStreamTailLaunch>>>(__VA_ARGS__)
+  TPX3_LOCALMAX_SEQUENCE(a);
 #undef GP
 }
 
@@ -264,20 +295,9 @@ int enqueue_general_cluster(tpx3_plan_s* p, const GenArgs& a, cudaStream_t st) {
   return cuda_ok(cudaGetLastError());
 }
 
-int enqueue_localmax(tpx3_plan_s* p, const GenArgs& a, cudaStream_t st, uint32_t wx, uint32_t wy, uint64_t wt) {
+int enqueue_localmax(tpx3_plan_s* p, const GenArgs& a, cudaStream_t st) {
   HostLauncher hl{p, st, -1, false, 0};
-  TPX3_GENERAL_SORT_SEQUENCE(a);
-  const uint64_t n = a.prm.n;
-  // the link stage's buffers hold the sorted records (slab: ToA, xy: x | y << 8 | tot << 16); the centroid
-  // stage's ordinal kernels run on lmax in place of label
-  GP(TPX3_STAGE_LINK, k_lm_gather, grid_for_hd(n, 256, a.sms), 256, n, a.perm, a.x, a.y, a.toa, a.tot, a.w.slab, a.w.xy);
-  GP(TPX3_STAGE_LINK, k_lm_flag, grid_for_hd(n, 256, a.sms, 16), 256, n, a.prm.P, wx, wy, wt, a.w.slab, a.w.xy, a.label);
-  GP(TPX3_STAGE_CENTROID, k_root_count, a.cent_nblk, kCentThreads, a.w.ctrl, 0, n, a.label, a.w.blkcnt);
-  GP(TPX3_STAGE_CENTROID, k_root_scan, 1, 1024, a.w.ctrl, 0, a.w.blkcnt, a.cent_nblk, a.max_clusters, a.n_clusters);
-  GP(TPX3_STAGE_CENTROID, k_root_slots, a.cent_nblk, kCentThreads, a.w.ctrl, 0, n, a.label, a.w.blkcnt, a.w.slot,
-     a.max_clusters, a.out, a.w.peak);
-  GP(TPX3_STAGE_CENTROID, k_lm_emit, grid_for_hd(a.max_clusters < n ? a.max_clusters : n, 128, a.sms, 16), 128, a.w.ctrl,
-     n, a.prm.P, wx, wy, wt, a.w.slab, a.w.xy, a.n_clusters, a.max_clusters, a.out);
+  TPX3_LOCALMAX_SEQUENCE(a);
   hl.leave();
   return cuda_ok(cudaGetLastError());
 }
@@ -433,10 +453,34 @@ int tpx3_localmax_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, ui
   if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
   Ws w = carve(p, workspace);
   if (p->profiling) ++p->profiled_calls;
-  TPX3_LAUNCH(p, k_ctrl_init, 1, 256, 0, st, w.ctrl, n, w.tiles, 0u, n_hits);
+  const bool lm_fused = !(p->cfg.flags & TPX3_FLAG_FORCE_GENERAL) && p->fused.variant != 0 && wt < (1u << 24) && n != 0;
+  const uint32_t num_tiles = lm_fused ? (uint32_t)((n + p->fused.S - 1) / p->fused.S) : 0u;
+  TPX3_LAUNCH(p, k_ctrl_init, num_tiles > 256 * 64 ? 64 : (num_tiles + 255) / 256 + 1, 256, 0, st, w.ctrl, n, w.tiles,
+              num_tiles, n_hits);
   if (n == 0) return cuda_ok(cudaGetLastError());
   GenArgs ga = make_gen_args(p, w, 0, n, x, y, toa, tot, perm, lmax, max_clusters, out, n_hits);
-  return enqueue_localmax(p, ga, st, wx, wy, wt);
+  ga.lm_wx = wx; ga.lm_wy = wy; ga.lm_wt = wt;
+  // shot-contiguous streams: the fused tile kernel in its paper-literal mode (the time window takes the place
+  // of the link window in the tile key); anything else: the general kernels, enqueued from the device
+  if (lm_fused) {
+    Params prm = p->prm;
+    prm.n = n;
+    prm.W = wt;
+    bool launched = false;
+    {
+      StageTimer timer(p, st, TPX3_STAGE_FUSED);
+      int rc = enqueue_fused(p->fused, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, lmax, max_clusters,
+                             *out, n_hits, (char*)workspace + p->off_keyA, &launched, 1u, wx > 255u ? 255u : wx,
+                             wy > 255u ? 255u : wy);
+      if (rc != TPX3_OK) return rc;
+    }
+    if (launched) {
+      k_fallback_dispatch_lm<<<1, 1, 0, st>>>(ga);
+      ++p->launches;
+      return cuda_ok(cudaGetLastError());
+    }
+  }
+  return enqueue_localmax(p, ga, st);
 }
 
 int tpx3_unwrap_toa(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint64_t* raw,

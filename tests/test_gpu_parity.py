@@ -407,29 +407,34 @@ LM_KEYS = ("c_label", "c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot
            "c_cx", "c_cy", "c_ctof")
 
 
-def check_localmax(m, x, y, toa, tot, wx, wy, wt, P=P, what=""):
+def check_localmax(m, x, y, toa, tot, wx, wy, wt, P=P, what="", hints=(0, 1024)):
+    """Every route of tpx3_localmax_centroid against the plain-definition oracle: the fused tile kernel in its
+    paper-literal mode (8192- and 4096-event tiles) and the general kernels (forced)."""
     import torch
 
     o = oracle.run_localmax(x, y, toa, tot, wx, wy, wt, P)
     n = len(x)
-    pl = m.plan(m.Config(toa_window_ticks=W, shot_period_ticks=P, max_hits=max(n, 1)))
     dev = [to_dev(np.asarray(x, dtype=np.uint16)), to_dev(np.asarray(y, dtype=np.uint16)),
            to_dev(np.asarray(toa, dtype=np.uint64)), to_dev(np.asarray(tot, dtype=np.uint16))]
-    cl = m.Clusters(max(n, 1), pl.device)
-    perm, lmax, nh = pl.localmax_centroid(*dev, wx, wy, wt, cl)
-    torch.cuda.synchronize()
-    st = pl.status()
-    assert st["error"] == 0, what
-    nhits = int(nh.cpu().numpy()[0])
-    assert nhits == o["n_clusters"], what
-    np.testing.assert_array_equal(perm[:n].cpu().numpy(), o["perm"], err_msg=what + " perm")
-    np.testing.assert_array_equal(lmax[:n].cpu().numpy(), o["lmax"], err_msg=what + " lmax")
-    g = cl.numpy(nhits)
-    for k in LM_KEYS:   # integers bit-exact; centroids bitwise fp32 (same int64 sums, IEEE RN divide: R12)
-        np.testing.assert_array_equal(g[k], o[k], err_msg=what + " " + k)
-    if n:
-        assert st["path"] == 3
-    pl.free()
+    for flags, hint in [(0, h) for h in hints] + [(m.FLAG_FORCE_GENERAL, 0)]:
+        tag = "%s [flags %d hint %d]" % (what, flags, hint)
+        pl = m.plan(m.Config(toa_window_ticks=W, shot_period_ticks=P, max_hits=max(n, 1), flags=flags,
+                             max_shot_hits=hint))
+        cl = m.Clusters(max(n, 1), pl.device)
+        perm, lmax, nh = pl.localmax_centroid(*dev, wx, wy, wt, cl)
+        torch.cuda.synchronize()
+        st = pl.status()
+        assert st["error"] == 0, tag
+        nhits = int(nh.cpu().numpy()[0])
+        assert nhits == o["n_clusters"], tag
+        np.testing.assert_array_equal(perm[:n].cpu().numpy(), o["perm"], err_msg=tag + " perm")
+        np.testing.assert_array_equal(lmax[:n].cpu().numpy(), o["lmax"], err_msg=tag + " lmax")
+        g = cl.numpy(nhits)
+        for k in LM_KEYS:   # integers bit-exact; centroids bitwise fp32 (same int64 sums, IEEE RN divide: R12)
+            np.testing.assert_array_equal(g[k], o[k], err_msg=tag + " " + k)
+        if n:
+            assert st["path"] == 3, tag
+        pl.free()
     return o
 
 
@@ -445,7 +450,7 @@ def test_localmax_paper_example(tpx3):
                                           (5, 300, (4, 4, 320))])
 def test_localmax_configs(tpx3, cfg, shots, w3):
     w = gen.generate(cfg, shots=shots)
-    check_localmax(tpx3, w.x, w.y, w.toa, w.tot, *w3, what="cfg%d w=%s" % (cfg, w3))
+    check_localmax(tpx3, w.x, w.y, w.toa, w.tot, *w3, what="cfg%d w=%s" % (cfg, w3), hints=(0, gen.max_shot_hits(cfg)))
 
 
 def test_localmax_edges(tpx3):
