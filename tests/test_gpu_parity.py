@@ -619,3 +619,30 @@ def test_fused_dense_repeated_addresses(tpx3, side, per_shot, hint, Wr):
     tot = rng.integers(1, 1024, n)
     res, _ = check(tpx3, x, y, toa, tot, W=Wr, modes=("fused",), max_shot_hits=hint, what="dense %d" % side)
     assert res["status"]["path"] == 1
+
+
+def test_localmax_capacity_and_args(tpx3):
+    import torch
+
+    m = tpx3
+    w = gen.generate(1, shots=200)
+    o = oracle.run_localmax(w.x, w.y, w.toa, w.tot, 1, 1, W, P)
+    dev = [to_dev(a) for a in (w.x, w.y, w.toa, w.tot)]
+    for flags in (0, m.FLAG_FORCE_GENERAL):
+        pl = m.plan(m.Config(max_hits=w.n, shot_period_ticks=P, flags=flags))
+        cap = o["n_clusters"] // 2
+        cl = m.Clusters(cap, pl.device)
+        perm, lmax, nh = pl.localmax_centroid(*dev, 1, 1, W, cl)
+        torch.cuda.synchronize()
+        st = pl.status()
+        assert st["error"] == m.ERR_CAPACITY                       # reported, not silently truncated
+        assert int(nh.cpu().numpy()[0]) == o["n_clusters"]           # the true count
+        g = cl.numpy(cap)
+        for k in LM_KEYS:
+            np.testing.assert_array_equal(g[k], o[k][:cap], err_msg=k)   # the first `cap` rows are valid
+        np.testing.assert_array_equal(lmax[: w.n].cpu().numpy(), o["lmax"])
+        pl.free()
+    pl = m.plan(m.Config(max_hits=10))
+    with pytest.raises(m.Tpx3Error):
+        pl.localmax_centroid(*dev, 1, 1, W, m.Clusters(16, pl.device))  # n > max_hits
+    pl.free()
