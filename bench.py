@@ -365,6 +365,14 @@ def run_ours(args):
         if key in tr and tr[key].get("pixel_hits", n) == n:   # a capture is of one workload size
             roofline["traffic"] = tr[key]["dram_bytes_per_launch"]
             roofline["traffic_source"] = tr[key].get("source")
+            wi = tr[key].get("warp_instructions_per_launch")
+            if wi and stage_ms[dom] > 0:
+                # what actually bounds the kernel: warp instructions issued per second against
+                # 148 SMs x 4 schedulers x the SM clock; instruction count from the same ncu capture
+                ipeak = 148 * 4 * 1965e6
+                roofline["issue"] = {"achieved": wi / (stage_ms[dom] * 1e-3), "peak": ipeak, "unit": "warp instructions/s",
+                                     "frac": wi / (stage_ms[dom] * 1e-3) / ipeak,
+                                     "note": "peak = 148 SMs x 4 issue slots x 1965 MHz (B200_PROFILING.md unit counts)"}
     except Exception:
         pass
 
