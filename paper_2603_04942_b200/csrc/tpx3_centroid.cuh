@@ -60,43 +60,11 @@ __global__ void __launch_bounds__(kCentThreads) k_root_count(Ctrl* c, int genera
 __global__ void __launch_bounds__(1024) k_root_scan(Ctrl* c, int general_only, uint32_t* blk_cnt, uint32_t nblk,
                                                   uint64_t max_clusters, uint32_t* n_clusters) {
   if (general_only && c->fused_state == 1) return;
-  __shared__ uint32_t warp_sums[32];
-  const uint32_t per = (nblk + 1023) / 1024;
-  uint32_t beg = threadIdx.x * per, end = beg + per;
-  if (beg > nblk) beg = nblk;
-  if (end > nblk) end = nblk;
-  uint32_t s = 0;
-  for (uint32_t i = beg; i < end; ++i) s += blk_cnt[i];
-  uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5, v = s;
-  for (int o = 1; o < 32; o <<= 1) {
-    uint32_t t = __shfl_up_sync(0xffffffffu, v, o);
-    if (lane >= (uint32_t)o) v += t;
-  }
-  if (lane == 31) warp_sums[w] = v;
-  __syncthreads();
-  uint32_t ws = 0, x = 0;
-  if (w == 0) {
-    ws = warp_sums[lane]; x = ws;
-    for (int o = 1; o < 32; o <<= 1) {
-      uint32_t t = __shfl_up_sync(0xffffffffu, x, o);
-      if (lane >= (uint32_t)o) x += t;
-    }
-  }
-  __syncthreads();
-  if (w == 0) {
-    warp_sums[lane] = x - ws;
-    if (lane == 31) {
-      *n_clusters = x;
-      c->status.n_clusters = x;
-      if ((uint64_t)x > max_clusters) set_error(c, TPX3_ERR_CAPACITY);
-    }
-  }
-  __syncthreads();
-  uint32_t run = warp_sums[w] + v - s;
-  for (uint32_t i = beg; i < end; ++i) {
-    uint32_t t = blk_cnt[i];
-    blk_cnt[i] = run;
-    run += t;
+  const uint32_t x = scan_inplace_1024(blk_cnt, nblk);
+  if (threadIdx.x == 0) {
+    *n_clusters = x;
+    c->status.n_clusters = x;
+    if ((uint64_t)x > max_clusters) set_error(c, TPX3_ERR_CAPACITY);
   }
 }
 

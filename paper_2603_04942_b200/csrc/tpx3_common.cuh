@@ -50,6 +50,47 @@ __device__ __forceinline__ uint32_t lanemask_lt() {
 __device__ __forceinline__ void atomic_min_u64(unsigned long long* p, unsigned long long v) { atomicMin(p, v); }
 __device__ __forceinline__ void atomic_max_u64(unsigned long long* p, unsigned long long v) { atomicMax(p, v); }
 
+// Exclusive prefix sum of v[0..n) in place by ONE block of 1024 threads (each thread owns a contiguous
+// run). Returns the total, the same value in every thread. Sums are taken modulo 2^32, so two's-complement
+// signed counts scan correctly too.
+__device__ __forceinline__ uint32_t scan_inplace_1024(uint32_t* v, uint32_t n) {
+  __shared__ uint32_t s_warp[33];
+  const uint32_t per = (n + 1023u) / 1024u;
+  uint32_t beg = threadIdx.x * per, end = beg + per;
+  if (beg > n) beg = n;
+  if (end > n) end = n;
+  uint32_t s = 0;
+  for (uint32_t i = beg; i < end; ++i) s += v[i];
+  const uint32_t lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+  uint32_t inc = s;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= (uint32_t)o) inc += t;
+  }
+  if (lane == 31u) s_warp[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    const uint32_t ws = s_warp[lane];
+    uint32_t x = ws;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, x, o);
+      if (lane >= (uint32_t)o) x += t;
+    }
+    s_warp[lane] = x - ws;
+    if (lane == 31u) s_warp[32] = x;
+  }
+  __syncthreads();
+  uint32_t run = s_warp[w] + inc - s;
+  for (uint32_t i = beg; i < end; ++i) {
+    const uint32_t t = v[i];
+    v[i] = run;
+    run += t;
+  }
+  return s_warp[32];
+}
+
 // Fill `n` 32-bit words (general_only: skipped when the fused path already succeeded).
 __global__ void __launch_bounds__(256) k_fill_u32(Ctrl* c, int general_only, uint32_t* p, uint64_t n, uint32_t v) {
   if (general_only && c->fused_state == 1) return;

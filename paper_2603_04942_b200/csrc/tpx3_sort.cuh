@@ -110,36 +110,7 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_hist(Ctrl* c, int pass, 
 // Exclusive scan of counts[kRadix * nblk] in place (single block of 1024 threads).
 __global__ void __launch_bounds__(1024) k_radix_scan(Ctrl* c, int pass, uint32_t* counts, uint32_t total) {
   if (c->fused_state == 1 || (uint32_t)pass >= c->npass) return;
-  __shared__ uint32_t warp_sums[32];
-  const uint32_t per = (total + 1023) / 1024;
-  uint32_t beg = threadIdx.x * per, end = beg + per;
-  if (beg > total) beg = total;
-  if (end > total) end = total;
-  uint32_t s = 0;
-  for (uint32_t i = beg; i < end; ++i) s += counts[i];
-  // block exclusive scan of s
-  uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5, v = s;
-  for (int o = 1; o < 32; o <<= 1) {
-    uint32_t t = __shfl_up_sync(0xffffffffu, v, o);
-    if (lane >= (uint32_t)o) v += t;
-  }
-  if (lane == 31) warp_sums[w] = v;
-  __syncthreads();
-  if (w == 0) {
-    uint32_t ws = warp_sums[lane], x = ws;
-    for (int o = 1; o < 32; o <<= 1) {
-      uint32_t t = __shfl_up_sync(0xffffffffu, x, o);
-      if (lane >= (uint32_t)o) x += t;
-    }
-    warp_sums[lane] = x - ws;
-  }
-  __syncthreads();
-  uint32_t run = warp_sums[w] + v - s;
-  for (uint32_t i = beg; i < end; ++i) {
-    uint32_t t = counts[i];
-    counts[i] = run;
-    run += t;
-  }
+  scan_inplace_1024(counts, total);
 }
 
 __global__ void __launch_bounds__(kSortThreads) k_radix_scatter(Ctrl* c, int pass, const uint64_t* __restrict__ toa,

@@ -62,42 +62,8 @@ __global__ void __launch_bounds__(kUnwrapThreads) k_unwrap_count(UnwrapArgs a) {
 }
 
 __global__ void __launch_bounds__(1024) k_unwrap_scan(UnwrapArgs a) {
-  __shared__ uint32_t warp_sums[32];
-  const uint32_t nblk = a.nblk;
-  const uint32_t per = (nblk + 1023) / 1024;
-  uint32_t beg = threadIdx.x * per, end = beg + per;
-  if (beg > nblk) beg = nblk;
-  if (end > nblk) end = nblk;
-  uint32_t s = 0;
-  for (uint32_t i = beg; i < end; ++i) s += a.blk[i];
-  const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  uint32_t v = s;
-  for (int o = 1; o < 32; o <<= 1) {
-    const uint32_t t = __shfl_up_sync(0xffffffffu, v, o);
-    if (lane >= (uint32_t)o) v += t;
-  }
-  if (lane == 31) warp_sums[w] = v;
-  __syncthreads();
-  uint32_t ws = 0, x = 0;
-  if (w == 0) {
-    ws = warp_sums[lane]; x = ws;
-    for (int o = 1; o < 32; o <<= 1) {
-      const uint32_t t = __shfl_up_sync(0xffffffffu, x, o);
-      if (lane >= (uint32_t)o) x += t;
-    }
-  }
-  __syncthreads();
-  if (w == 0) {
-    warp_sums[lane] = x - ws;
-    if (lane == 31) *a.wraps_out = a.wraps_in + (long long)(int)x;
-  }
-  __syncthreads();
-  uint32_t run = warp_sums[w] + v - s;
-  for (uint32_t i = beg; i < end; ++i) {
-    const uint32_t t = a.blk[i];
-    a.blk[i] = run;
-    run += t;
-  }
+  const uint32_t x = scan_inplace_1024(a.blk, a.nblk);
+  if (threadIdx.x == 0) *a.wraps_out = a.wraps_in + (long long)(int)x;
 }
 
 __global__ void __launch_bounds__(kUnwrapThreads) k_unwrap_apply(UnwrapArgs a) {
