@@ -133,7 +133,8 @@ int tpx3_cluster_centroid(tpx3_plan_t plan, void* workspace, void* cuda_stream, 
  * neighbour of greater (ToT, sorted position) inside the box |dX| <= wx, |dY| <= wy, |dToF| <= wt
  * of the same shot (all inclusive; tie: the later pixel wins, :150); its centroid
  * is Eq. 9 over that box (row i of A, A_ii = 1) for X, Y and ToF alike (:165). Uses the plan's
- * shot period and the general path's stable sort; the plan's toa_window_ticks is not used.
+ * shot period; the plan's toa_window_ticks is not used. Shot-contiguous streams run in the fused
+ * tile kernel (as tpx3_cluster_centroid), anything else in the general kernels; same results.
  * Outputs [dev]: perm uint32[n]; lmax uint32[n], lmax[k] = k if sorted position k is a hit and
  * 0xFFFFFFFF otherwise; one row of `out` per hit in ascending k (label = k, size = pixels in the
  * box, toa_peak = ToA of the local maximum, sums and centroids over the box); n_hits uint32[1].

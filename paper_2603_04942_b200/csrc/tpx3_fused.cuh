@@ -33,11 +33,17 @@
 //            atomicMin per event), ordinals of the labels by block scan (S3)
 //   reduce   members chained to their label (one atomicExch each); one thread per hit walks the
 //            chain: exact 64-bit sums, brightest pixel by (ToT, sorted index) (S4)
+//            (+ sum tot*tof for the time-of-flight centroid)
 //   centroid fp32(sum tot*x) / fp32(sum tot), IEEE RN (S5, Eq. 9), in k_fused_compact
 //
-// A tile that cannot be handled (a shot longer than L, a decreasing shot number, shot offset and
-// time of flight too wide for one 32-bit key) marks the call as failed; the general kernels, enqueued behind this one,
-// then redo the call.
+// Template MODE 1 is the paper-literal mode (tpx3_localmax_centroid, R21): same tiling, load, sort,
+// hash, staging and compaction, but in place of link / label / reduce an event is a hit when its box holds no
+// greater (ToT, sorted index), and the sums run over that box. Boxes of <= 81 cells are scanned cell by cell
+// through the hash, larger ones by walking the time window of the sorted tile.
+//
+// A tile that cannot be handled (a shot longer than L, a decreasing shot number, shot offset and time of
+// flight too wide for one 32-bit key) marks the call as failed; the general kernels, enqueued from the device
+// behind this one (k_fallback_dispatch), then redo the call.
 #pragma once
 #include "tpx3_common.cuh"
 #include "tpx3_localmax.cuh"
