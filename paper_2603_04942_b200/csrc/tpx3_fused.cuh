@@ -438,20 +438,24 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   if (unsorted) {
     uint16_t* buf0 = reinterpret_cast<uint16_t*>(smem + L::kRegX);
     uint16_t* buf1 = buf0 + T;
-    uint32_t* wcnt = reinterpret_cast<uint32_t*>(smem + L::kRegX + 4 * T);  // [WARPS][256]
-    static_assert(WARPS * 256 * 4 <= 4 * T, "warp digit counters");
+    // digit counters per warp, 16 bit (a count is <= T); one thread per digit value, so up to 9-bit digits
+    // with >= 512 threads: 18 key bits (14 of time of flight + 4 of shot offset on cfg 4) take 2 passes, not 3
+    constexpr uint32_t DB = THREADS >= 512 ? 9u : 8u;
+    constexpr uint32_t RMAX = 1u << DB;
+    uint16_t* wcnt = reinterpret_cast<uint16_t*>(smem + L::kRegX + 4 * T);  // [WARPS][RMAX]
+    static_assert(WARPS * RMAX * 2 <= 4 * T && T <= 65535, "warp digit counters");
     // sort key without the gap between the tof bits and the shot bits
     const uint32_t tofb = misc->max_tof ? 32u - (uint32_t)__clz(misc->max_tof) : 1u;
     const uint32_t key_bits = tofb + sbits;
-    const uint32_t npass = (key_bits + 7u) / 8u;
-    const uint32_t dbits = (key_bits + npass - 1u) / npass;         // <= 8
+    const uint32_t npass = (key_bits + DB - 1u) / DB;
+    const uint32_t dbits = (key_bits + npass - 1u) / npass;         // <= DB
     const uint32_t radix = 1u << dbits, dmask = radix - 1u;
     const uint32_t lt = lanemask_lt();
     for (uint32_t pass = 0; pass < npass; ++pass) {
       const uint16_t* src = (pass & 1u) ? buf1 : buf0;
       uint16_t* dst = (pass & 1u) ? buf0 : buf1;
       const uint32_t shift = pass * dbits;
-      for (uint32_t i = tid; i < WARPS * 256u; i += THREADS) wcnt[i] = 0;
+      for (uint32_t i = tid; i < WARPS * RMAX / 2u; i += THREADS) reinterpret_cast<uint32_t*>(wcnt)[i] = 0u;
       __syncthreads();
       uint32_t e_src[IPT], e_dig[IPT], e_rank[IPT];
 #pragma unroll
@@ -470,12 +474,12 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
           peers &= one ? bal : ~bal;
         }
         const uint32_t lr = __popc(peers & lt);
-        const uint32_t c0 = valid ? wcnt[warp * 256u + d] : 0u;
+        const uint32_t c0 = valid ? (uint32_t)wcnt[warp * RMAX + d] : 0u;
         __syncwarp();
-        if (valid && lr == 0) wcnt[warp * 256u + d] = c0 + __popc(peers);
+        if (valid && lr == 0) wcnt[warp * RMAX + d] = (uint16_t)(c0 + __popc(peers));
         __syncwarp();
         e_src[j] = s;
-        e_dig[j] = valid ? d : 256u;                                        // 256: "no event"
+        e_dig[j] = valid ? d : RMAX;                                        // RMAX: "no event"
         e_rank[j] = c0 + lr;
       }
       __syncthreads();
@@ -484,8 +488,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       if (tid < radix) {
 #pragma unroll 4
         for (int w = 0; w < WARPS; ++w) {
-          uint32_t c = wcnt[w * 256 + tid];
-          wcnt[w * 256 + tid] = tot_d;
+          const uint32_t c = wcnt[w * RMAX + tid];
+          wcnt[w * RMAX + tid] = (uint16_t)tot_d;
           tot_d += c;
         }
       }
@@ -495,19 +499,19 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
         if (lane >= (uint32_t)o) inc += t;
       }
-      if (lane == 31 && warp < 8) misc->warp_sums[warp] = inc;
+      if (lane == 31 && warp < RMAX / 32u) misc->warp_sums[warp] = inc;
       __syncthreads();
       if (tid < radix) {
         uint32_t wbase = 0;
         for (uint32_t w = 0; w < warp; ++w) wbase += misc->warp_sums[w];
         const uint32_t dbase = wbase + inc - tot_d;
 #pragma unroll 4
-        for (int w = 0; w < WARPS; ++w) wcnt[w * 256 + tid] += dbase;
+        for (int w = 0; w < WARPS; ++w) wcnt[w * RMAX + tid] = (uint16_t)(wcnt[w * RMAX + tid] + dbase);
       }
       __syncthreads();
 #pragma unroll
       for (int j = 0; j < IPT; ++j) {
-        if (e_dig[j] < 256u) dst[wcnt[warp * 256u + e_dig[j]] + e_rank[j]] = (uint16_t)e_src[j];
+        if (e_dig[j] < RMAX) dst[(uint32_t)wcnt[warp * RMAX + e_dig[j]] + e_rank[j]] = (uint16_t)e_src[j];
       }
       __syncthreads();
     }
