@@ -151,6 +151,8 @@ struct FusedArgs {
 };
 
 constexpr uint32_t kNone = 0xFFFFFFFFu;
+constexpr int kHalvePre = 2;    // pointer-halving rounds before the deferred unions
+constexpr int kHalvePost = 0;   // and before the root search
 constexpr uint32_t kGold = 0x9E3779B1u;
 constexpr uint32_t kTaskBase = 0xFFF8u;   // deferred-list entries k << 16 | (kTaskBase + direction) are scan tasks
 
@@ -714,6 +716,14 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   // ---- deferred links: union by compare-and-swap hooks ---------------------------------------------
   {
     const uint32_t nl = misc->n_list;
+    // the plain parent stores left chains as long as a blob is tall: halve them first, so that the finds of
+    // the unions (few threads, everybody else waits for them) are short. A halving store never touches a
+    // root and any ancestor is a valid parent, so it may race with the hooks.
+    for (int hr = 0; hr < kHalvePre; ++hr)
+      for (uint32_t k = tid; k < mm; k += THREADS) {
+        const uint32_t p1 = par[k], g = par[p1];
+        if (g != p1) par[k] = (uint16_t)g;
+      }
     if (nl > (uint32_t)L::kListCap) {
       // the list overflowed (very dense tile): redo the probes, uniting on the spot
       for (uint32_t k = tid; k < mm; k += THREADS) {
@@ -755,10 +765,11 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 #pragma unroll
     for (int q = 0; q < 8 * T / 16 / THREADS; ++q) f[q * THREADS + tid] = ones;   // minidx and head
   }
-  // two rounds of pointer halving (any ancestor is a valid parent, so the plain stores may race),
+  // kHalvePost more rounds of pointer halving (any ancestor is a valid parent, so the plain stores may race;
+  // measured: 2 rounds before the unions and none here is best),
   // then the roots
 #pragma unroll
-  for (int round = 0; round < 2; ++round) {
+  for (int round = 0; round < kHalvePost; ++round) {
 #pragma unroll
     for (int j = 0; j < IPT; ++j) {
       const uint32_t k = (uint32_t)j * THREADS + tid;
