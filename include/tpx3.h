@@ -66,10 +66,12 @@ typedef struct {
   int32_t device;              /* CUDA device ordinal                                          */
   uint32_t flags;              /* TPX3_FLAG_*                                                  */
   uint32_t max_shot_hits;      /* hint: most events one shot can hold; sizes the fused path's
-                                  tiles (0 = 4096). <= 512: 2048-event tiles, 4 CTAs per SM;
-                                  <= 1024: 4096-event tiles, 2 CTAs per SM; <= 4096: 8192-event
-                                  tiles; larger, or a shot that exceeds the hint: the general
-                                  path runs (same results, slower).                            */
+                                  tiles. <= 512: 2048-event tiles, 4 CTAs per SM; <= 1024:
+                                  4096-event tiles, 2 CTAs per SM; <= 4096: 8192-event tiles;
+                                  larger, or a shot that exceeds the hint: the general path
+                                  runs (same results, slower). 0 = no hint: 1024, then 2048,
+                                  then 4096 are tried on the device (a failed try stops within
+                                  its first wave of tiles), then the general path.             */
   uint32_t reserved;           /* must be 0                                                    */
 } tpx3_config_t;
 

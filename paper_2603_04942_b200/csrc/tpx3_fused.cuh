@@ -183,6 +183,7 @@ struct FusedMisc {
   unsigned int max_tof, max_sl;
   unsigned int n_roots;
   unsigned int n_list;         // deferred links pushed (may exceed the capacity: overflow)
+  unsigned int skip;           // the call already failed in another tile
   unsigned int warp_sums[33];
 };
 static_assert(sizeof(FusedMisc) <= 512, "FusedMisc must fit kMiscBytes");
@@ -235,6 +236,9 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   if (tid == 0) {
     misc->lo = kNone;
     misc->hi = kNone;
+    // another tile already gave up: this attempt is lost, do not spend time on it (the next attempt — a
+    // variant with longer shots, or the general kernels — is enqueued behind; k_fallback_dispatch)
+    misc->skip = atomicAdd(&a.ctrl->fused_fail, 0u);
     misc->fail = 0;
     misc->max_tof = 0;
     misc->max_sl = 0;
@@ -243,6 +247,15 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   }
   __syncthreads();
   const uint32_t b = blockIdx.x;
+  if (misc->skip != 0u) {
+    if (tid == 0) {
+      a.tiles[b] = 0ull;
+      __threadfence();
+      const uint32_t done = atomicAdd(&a.ctrl->tiles_done, 1u);
+      if (done + 1u == a.num_tiles) a.ctrl->fused_state = 2u;
+    }
+    return;
+  }
   const uint64_t base = (uint64_t)b * a.S;             // first event this tile looks at
   const uint64_t avail = a.n - base;                   // > 0 by construction
   const uint32_t cnt = avail < (uint64_t)T ? (uint32_t)avail : (uint32_t)T;  // events readable
@@ -1020,7 +1033,7 @@ struct FusedGeom {
 inline FusedGeom fused_geom(uint64_t P, uint32_t W, uint32_t max_shot_hits) {
   FusedGeom g{0, 0, 0};
   if (P == 0 || P > (1ull << 24) || W >= (1u << 24)) return g;   // tof + W must fit the 32-bit tile key
-  const uint32_t Lh = max_shot_hits ? max_shot_hits : 4096u;
+  const uint32_t Lh = max_shot_hits ? max_shot_hits : 1024u;      // no hint: first rung of the ladder (below)
   if (Lh <= 512u) { g.variant = 3; g.T = 2048; }
   else if (Lh <= 1024u) { g.variant = 1; g.T = 4096; }
   else if (Lh <= 4096u) { g.variant = 2; g.T = 8192; }
@@ -1042,16 +1055,25 @@ inline int launch_fused(const FusedArgs& a, cudaStream_t st) {
   return cudaGetLastError() == cudaSuccess ? TPX3_OK : TPX3_ERR_CUDA;
 }
 
-// Returns TPX3_OK (launched or not applicable; *launched says which) or an error.
-inline int enqueue_fused(const FusedGeom& g, uint64_t* launches, Ctrl* ctrl, unsigned long long* tiles,
-                         cudaStream_t st, const Params& prm, const uint16_t* x, const uint16_t* y,
-                         const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label,
-                         uint64_t max_clusters, const tpx3_clusters_t& out, uint32_t* n_clusters, void* stage,
-                         bool* launched, uint32_t mode = 0, uint32_t lm_wx = 0, uint32_t lm_wy = 0) {
-  *launched = false;
-  if (g.variant == 0 || prm.n == 0) return TPX3_OK;
-  // the 128-bit load phase needs 16-byte aligned inputs (PyTorch allocations are 256-byte aligned)
-  if ((((uintptr_t)x | (uintptr_t)y | (uintptr_t)toa | (uintptr_t)tot) & 15u) != 0) return TPX3_OK;
+// Without a hint the shot length is tried in rungs: 1024 (4096-event tiles), 2048 and 4096 (8192-event tiles).
+// A rung whose tiles meet a longer shot fails within its first wave (every later tile returns at once), and
+// k_fallback_dispatch launches the next rung from the device; after the last one the general kernels run.
+constexpr int kLadderMax = 2;   // rungs after the first
+struct FusedLadder {
+  int n;                        // rungs still to try after the one the host enqueued
+  uint32_t S[kLadderMax];       // their slice lengths (8192-event tiles)
+};
+
+inline FusedLadder fused_ladder(uint32_t max_shot_hits) {
+  FusedLadder l{0, {0, 0}};
+  if (max_shot_hits == 0) { l.n = 2; l.S[0] = 8192u - 2048u; l.S[1] = 8192u - 4096u; }
+  return l;
+}
+
+inline FusedArgs make_fused_args(uint32_t S, Ctrl* ctrl, unsigned long long* tiles, const Params& prm, const uint16_t* x,
+                                 const uint16_t* y, const uint64_t* toa, const uint16_t* tot, uint32_t* perm,
+                                 uint32_t* label, uint64_t max_clusters, const tpx3_clusters_t& out,
+                                 uint32_t* n_clusters, void* stage, uint32_t mode, uint32_t lm_wx, uint32_t lm_wy) {
   FusedArgs a;
   a.ctrl = ctrl;
   a.tiles = tiles;
@@ -1060,8 +1082,8 @@ inline int enqueue_fused(const FusedGeom& g, uint64_t* launches, Ctrl* ctrl, uns
   a.divP = make_div64(prm.P);
   a.divP32 = make_div32((uint32_t)prm.P);
   a.W = prm.W;
-  a.S = g.S;
-  a.num_tiles = (uint32_t)((prm.n + g.S - 1) / g.S);
+  a.S = S;
+  a.num_tiles = (uint32_t)((prm.n + S - 1) / S);
   a.sensor_w = prm.sensor_w;
   a.sensor_h = prm.sensor_h;
   a.flags = prm.flags;
@@ -1076,6 +1098,52 @@ inline int enqueue_fused(const FusedGeom& g, uint64_t* launches, Ctrl* ctrl, uns
   a.stage_c = reinterpret_cast<uint64_t*>(a.stage_b + prm.n);
   a.stage_d = a.stage_c + prm.n;
   a.mode = mode; a.lm_wx = lm_wx; a.lm_wy = lm_wy;
+  return a;
+}
+
+__host__ __device__ inline void compact_grid(uint32_t num_tiles, uint32_t* ctas, uint32_t* tiles_per_cta) {
+  uint32_t c = num_tiles < (uint32_t)(kNumSMs * 8) ? num_tiles : (uint32_t)(kNumSMs * 8);
+  if (c == 0) c = 1;
+  const uint32_t t = (num_tiles + c - 1) / c;
+  *tiles_per_cta = t ? t : 1u;
+  *ctas = t ? (num_tiles + t - 1) / t : 1u;
+}
+
+// Device side: the next rung (8192-event tiles), tail-launched by k_fallback_dispatch.
+__device__ inline void launch_fused_rung_device(FusedArgs a) {
+  uint32_t ctas, tpc;
+  compact_grid(a.num_tiles, &ctas, &tpc);
+  if (a.mode == 0u)
+    k_fused_shot_tiles<8192, 1024, 0><<<a.num_tiles, 1024, FusedSmem<8192>::kBytes, cudaStreamTailLaunch>>>(a);
+  else
+    k_fused_shot_tiles<8192, 1024, 1><<<a.num_tiles, 1024, FusedSmem<8192>::kBytes, cudaStreamTailLaunch>>>(a);
+  k_fused_compact<<<ctas, kCompactThreads, 0, cudaStreamTailLaunch>>>(a, tpc);
+}
+
+// Host side. Returns TPX3_OK (launched or not applicable; *launched says which) or an error. *args receives the
+// arguments of the enqueued rung (the later rungs differ in S and num_tiles only).
+inline int enqueue_fused(const FusedGeom& g, uint64_t* launches, Ctrl* ctrl, unsigned long long* tiles,
+                         cudaStream_t st, const Params& prm, const uint16_t* x, const uint16_t* y,
+                         const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label,
+                         uint64_t max_clusters, const tpx3_clusters_t& out, uint32_t* n_clusters, void* stage,
+                         bool* launched, FusedArgs* args, uint32_t mode = 0, uint32_t lm_wx = 0, uint32_t lm_wy = 0) {
+  *launched = false;
+  if (g.variant == 0 || prm.n == 0) return TPX3_OK;
+  // the 128-bit load phase needs 16-byte aligned inputs (PyTorch allocations are 256-byte aligned)
+  if ((((uintptr_t)x | (uintptr_t)y | (uintptr_t)toa | (uintptr_t)tot) & 15u) != 0) return TPX3_OK;
+  const FusedArgs a = make_fused_args(g.S, ctrl, tiles, prm, x, y, toa, tot, perm, label, max_clusters, out, n_clusters,
+                                      stage, mode, lm_wx, lm_wy);
+  *args = a;
+  // the 8192-event variants may be launched from the device later on: their attribute must be set by then
+  static bool ladder_configured = false;
+  if (!ladder_configured) {
+    if (cudaFuncSetAttribute(k_fused_shot_tiles<8192, 1024, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             FusedSmem<8192>::kBytes) != cudaSuccess ||
+        cudaFuncSetAttribute(k_fused_shot_tiles<8192, 1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             FusedSmem<8192>::kBytes) != cudaSuccess)
+      return TPX3_ERR_CUDA;
+    ladder_configured = true;
+  }
   int rc;
   if (mode == 0u)
     rc = g.variant == 3 ? launch_fused<2048, 256, 0>(a, st)
@@ -1085,9 +1153,8 @@ inline int enqueue_fused(const FusedGeom& g, uint64_t* launches, Ctrl* ctrl, uns
                         : g.variant == 1 ? launch_fused<4096, 512, 1>(a, st) : launch_fused<8192, 1024, 1>(a, st);
   if (rc != TPX3_OK) return rc;
   ++*launches;
-  uint32_t ctas = a.num_tiles < (uint32_t)(kNumSMs * 8) ? a.num_tiles : (uint32_t)(kNumSMs * 8);
-  const uint32_t tiles_per_cta = (a.num_tiles + ctas - 1) / ctas;
-  ctas = (a.num_tiles + tiles_per_cta - 1) / tiles_per_cta;
+  uint32_t ctas, tiles_per_cta;
+  compact_grid(a.num_tiles, &ctas, &tiles_per_cta);
   k_fused_compact<<<ctas, kCompactThreads, 0, st>>>(a, tiles_per_cta);
   if (cudaGetLastError() != cudaSuccess) return TPX3_ERR_CUDA;
   ++*launches;

@@ -215,23 +215,30 @@ __host__ __device__ inline uint32_t grid_for_hd(uint64_t n, int threads, int num
        (A).max_clusters, (A).out);                                                                                    \
   } while (0)
 
-// Device-side fallback: one tiny kernel behind the fused path. If the fused kernel could not serve
-// the call it enqueues the whole general path as tail launches (they run, in order, after this grid
-// and before anything the host enqueued later on the stream). A successful fused call thus pays for
-// one empty launch instead of the 36 early-exit launches of the general path.
-__global__ void k_fallback_dispatch(GenArgs a) {
-  if (a.w.ctrl->fused_state == 1u) return;
+// Device-side fallback: one tiny kernel behind the fused path. If the fused kernel served the call it returns
+// at once. Otherwise it enqueues, as tail launches (they run, in order, after this grid and before anything
+// the host enqueued later on the stream), either the next rung of the shot-length ladder (plans without a
+// hint: the same tile kernel with room for longer shots, then this dispatcher again) or, after the last rung,
+// the whole general path. A successful fused call thus pays for one empty launch instead of the 36 early-exit
+// launches of the general path. lm != 0: the paper-literal mode.
+__global__ void k_fallback_dispatch(GenArgs a, FusedArgs fa, FusedLadder ladder, int rung, int lm) {
+  Ctrl* c = a.w.ctrl;
+  if (c->fused_state == 1u) return;
+  if (rung < ladder.n) {
+    c->tiles_done = 0; c->fused_fail = 0; c->fused_state = 0;
+    fa.S = ladder.S[rung];
+    fa.num_tiles = (uint32_t)((fa.n + fa.S - 1) / fa.S);
+    launch_fused_rung_device(fa);
+    k_fallback_dispatch<<<1, 1, 0, cudaStreamTailLaunch>>>(a, fa, ladder, rung + 1, lm);
+    return;
+  }
 #define GP(stage, kernel, grid, block, ...) kernel<<<(grid), (block), 0, cudaStreamTailLaunch>>>(__VA_ARGS__)
-  TPX3_GENERAL_CLUSTER_SEQUENCE(a);
-  TPX3_GENERAL_CENTROID_SEQUENCE(a);
-#undef GP
-}
-
-// The same for the paper-literal mode.
-__global__ void k_fallback_dispatch_lm(GenArgs a) {
-  if (a.w.ctrl->fused_state == 1u) return;
-#define GP(stage, kernel, grid, block, ...) kernel<<<(grid), (block), 0, cudaStreamTailLaunch>>>(__VA_ARGS__)
-  TPX3_LOCALMAX_SEQUENCE(a);
+  if (lm) {
+    TPX3_LOCALMAX_SEQUENCE(a);
+  } else {
+    TPX3_GENERAL_CLUSTER_SEQUENCE(a);
+    TPX3_GENERAL_CENTROID_SEQUENCE(a);
+  }
 #undef GP
 }
 
@@ -426,12 +433,13 @@ int tpx3_cluster_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uin
   if (try_fused) {
     bool launched = false;
     StageTimer timer(p, st, TPX3_STAGE_FUSED);
+    FusedArgs fa;
     rc = enqueue_fused(p->fused, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, label, max_clusters,
-                       *out, n_clusters, (char*)workspace + p->off_keyA, &launched);
+                       *out, n_clusters, (char*)workspace + p->off_keyA, &launched, &fa);
     if (rc != TPX3_OK) return rc;
     if (launched) {
-      // the general path, only if the fused kernel gave up: decided and enqueued on the device
-      k_fallback_dispatch<<<1, 1, 0, st>>>(ga);
+      // the next rung or the general path, only if the fused kernel gave up: decided and enqueued on the device
+      k_fallback_dispatch<<<1, 1, 0, st>>>(ga, fa, fused_ladder(p->cfg.max_shot_hits), 0, 0);
       ++p->launches;
       return cuda_ok(cudaGetLastError());
     }
@@ -467,15 +475,14 @@ int tpx3_localmax_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, ui
     prm.n = n;
     prm.W = wt;
     bool launched = false;
-    {
-      StageTimer timer(p, st, TPX3_STAGE_FUSED);
-      int rc = enqueue_fused(p->fused, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, lmax, max_clusters,
-                             *out, n_hits, (char*)workspace + p->off_keyA, &launched, 1u, wx > 255u ? 255u : wx,
-                             wy > 255u ? 255u : wy);
-      if (rc != TPX3_OK) return rc;
-    }
+    StageTimer timer(p, st, TPX3_STAGE_FUSED);
+    FusedArgs fa;
+    int rc = enqueue_fused(p->fused, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, lmax, max_clusters,
+                           *out, n_hits, (char*)workspace + p->off_keyA, &launched, &fa, 1u, wx > 255u ? 255u : wx,
+                           wy > 255u ? 255u : wy);
+    if (rc != TPX3_OK) return rc;
     if (launched) {
-      k_fallback_dispatch_lm<<<1, 1, 0, st>>>(ga);
+      k_fallback_dispatch<<<1, 1, 0, st>>>(ga, fa, fused_ladder(p->cfg.max_shot_hits), 0, 1);
       ++p->launches;
       return cuda_ok(cudaGetLastError());
     }

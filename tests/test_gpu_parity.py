@@ -646,3 +646,19 @@ def test_localmax_capacity_and_args(tpx3):
     with pytest.raises(m.Tpx3Error):
         pl.localmax_centroid(*dev, 1, 1, W, m.Clusters(16, pl.device))  # n > max_hits
     pl.free()
+
+
+@pytest.mark.parametrize("per_shot,path", [(700, 1), (1500, 1), (3000, 1), (9000, 2)])
+def test_no_hint_ladder(tpx3, per_shot, path):
+    """max_shot_hits = 0: shot lengths 1024, 2048, 4096 are tried in turn on the device (a failed rung stops in
+    its first wave and the next one is launched from k_fallback_dispatch), then the general path."""
+    rng = np.random.default_rng(per_shot)
+    shots = 25
+    n = shots * per_shot
+    x = rng.integers(0, 256, n); y = rng.integers(0, 256, n)
+    toa = (np.repeat(np.arange(shots), per_shot) * P + np.sort(rng.integers(0, 60000, (shots, per_shot)), axis=1).ravel()
+           ).astype(np.uint64)
+    tot = rng.integers(1, 1024, n)
+    res, _ = check(tpx3, x, y, toa, tot, modes=("fused",), max_shot_hits=0, what="ladder %d" % per_shot)
+    assert res["status"]["path"] == path
+    check_localmax(tpx3, x, y, toa, tot, 1, 1, 200, what="ladder lm %d" % per_shot, hints=(0,))
