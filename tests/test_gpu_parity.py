@@ -662,3 +662,44 @@ def test_no_hint_ladder(tpx3, per_shot, path):
     res, _ = check(tpx3, x, y, toa, tot, modes=("fused",), max_shot_hits=0, what="ladder %d" % per_shot)
     assert res["status"]["path"] == path
     check_localmax(tpx3, x, y, toa, tot, 1, 1, 200, what="ladder lm %d" % per_shot, hints=(0,))
+
+
+def test_full_size_localmax_cfg1(tpx3):
+    """BASELINE.json configs[1] in full through the paper-literal mode (the bench configuration of
+    `bench.py --mode localmax`): sampled shot windows element by element, invariants on the whole output."""
+    import torch
+
+    m = tpx3
+    w = gen.generate(1)
+    n = w.n
+    wx, wy, wt = 2, 2, 320
+    pl = m.plan(m.Config(max_hits=n, toa_window_ticks=W, shot_period_ticks=P, max_shot_hits=gen.max_shot_hits(1)))
+    dev = [to_dev(a) for a in (w.x, w.y, w.toa, w.tot)]
+    cl = m.Clusters(max(n // 2, 1024), pl.device)
+    perm, lmax, nh = pl.localmax_centroid(*dev, wx, wy, wt, cl)
+    torch.cuda.synchronize()
+    st = pl.status()
+    assert st["error"] == 0 and st["path"] == 3, st
+    nhits = int(nh.cpu().numpy()[0])
+    perm, lmax = perm[:n].cpu().numpy(), lmax[:n].cpu().numpy()
+    c = cl.numpy(nhits)
+    pl.free()
+    k = np.arange(n, dtype=np.uint32)
+    assert np.all((lmax == k) | (lmax == 0xFFFFFFFF))
+    assert np.array_equal(np.flatnonzero(lmax == k).astype(np.uint32), c["c_label"])
+    assert np.array_equal(perm, k)                                    # cfg1 is delivered in ToA order
+    assert np.all(c["c_size"] >= 1) and np.all(c["c_size"] <= 25 * 4)  # a 5 x 5 box, a few repeated addresses
+    assert np.array_equal(c["c_toa_peak"], w.toa[c["c_label"]])
+    off = w.shot_offsets
+    for s0, s1 in _windows(w.shots, 300, 6):
+        a, b = int(off[s0]), int(off[s1])
+        s = w.slice_shots(s0, s1)
+        o = oracle.run_localmax(s.x, s.y, s.toa, s.tot, wx, wy, wt, P)
+        what = "shots [%d, %d)" % (s0, s1)
+        exp = np.where(o["lmax"] == 0xFFFFFFFF, np.uint32(0xFFFFFFFF), o["lmax"] + np.uint32(a))
+        np.testing.assert_array_equal(lmax[a:b], exp, err_msg=what + " lmax")
+        i0, i1 = np.searchsorted(c["c_label"], [a, b])
+        assert i1 - i0 == o["n_clusters"], what
+        np.testing.assert_array_equal(c["c_label"][i0:i1], o["c_label"] + np.uint32(a), err_msg=what)
+        for key in LM_KEYS[1:]:
+            np.testing.assert_array_equal(c[key][i0:i1], o[key], err_msg=what + " " + key)
