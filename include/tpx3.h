@@ -66,7 +66,7 @@ typedef struct {
   int32_t device;              /* CUDA device ordinal                                          */
   uint32_t flags;              /* TPX3_FLAG_*                                                  */
   uint32_t max_shot_hits;      /* hint: most events one shot can hold; sizes the fused path's
-                                  tiles. <= 512: 2048-event tiles, 4 CTAs per SM; <= 1024:
+                                  tiles. <= 512: 2048-event tiles, 4 CTAs per SM; <= 1536:
                                   4096-event tiles, 2 CTAs per SM; <= 4096: 8192-event tiles;
                                   larger, or a shot that exceeds the hint: the general path
                                   runs (same results, slower). 0 = no hint: 1024, then 2048,
