@@ -812,7 +812,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       const uint32_t l = minidx[root_r[j]];
       lab[k] = (uint16_t)l;
       a.label[out_base + k] = out_base + l;
-      if (l != k) nxt[k] = (uint16_t)atomicExch(&head[l], k);   // kNone truncates to 0xFFFF = end
+      nxt[k] = (uint16_t)atomicExch(&head[l], k);   // every member, the first pixel too; kNone truncates to 0xFFFF = end
     }
   }
   __syncthreads();
@@ -918,7 +918,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   for (uint32_t c = tid; c < n_roots; c += THREADS) {
     const uint32_t r = rootpos[c];
     unsigned long long sx = 0, sy = 0, sf = 0;
-    uint32_t st = 0, size = 0, best = 0, k = r;
+    uint32_t st = 0, size = 0, best = 0, k = head[r];   // the chain holds every member of the hit
     do {
       const uint2 rk = recS[k];
       const uint32_t w1 = rk.y;
@@ -929,9 +929,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       sy += (unsigned long long)(t * ((w1 >> 8) & 0xFFu));
       ++size;
       best = max(best, (t << 16) | k);   // (ToT, sorted index): the later pixel wins ties
-      if (k == r) k = head[r];
-      else { const uint32_t nk = nxt[k]; k = (nk == 0xFFFFu) ? kNone : nk; }
-    } while (k != kNone);
+      k = nxt[k];
+    } while (k != 0xFFFFu);
     const uint32_t keyp = recS[best & 0xFFFFu].x;
     const uint64_t o = (uint64_t)out_base + c;
     a.stage_a[o] = make_uint4(out_base + r, size, st, 0u);
