@@ -1002,15 +1002,40 @@ __global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, 
   __syncthreads();
   unsigned long long prefix = s_prefix;
   bool over = false;
-  for (uint32_t t = t0; t < t1; ++t) {
-    const unsigned long long w = a.tiles[t];
-    const uint32_t cnt = (uint32_t)(w & 0xFFFFFFFFull);
-    const uint64_t src = w >> 32;
-    for (uint32_t c = tid; c < cnt; c += kCompactThreads) {
-      const uint64_t o = prefix + c;
+  // the CTA's tiles in groups of 32: warp 0 turns the group's hit counts into offsets, then all threads walk the
+  // group's hits as ONE index range (a tile has about 300 hits: a loop per tile would leave most of the last
+  // iteration's lanes idle)
+  __shared__ uint32_t s_off[33];
+  __shared__ uint32_t s_src[32];
+  for (uint32_t g0 = t0; g0 < t1; g0 += 32u) {
+    const uint32_t ng = min(32u, t1 - g0);
+    __syncthreads();                      // the previous group's tables are no longer read
+    if (warp == 0) {
+      const unsigned long long w = lane < ng ? a.tiles[g0 + lane] : 0ull;
+      const uint32_t cnt = (uint32_t)(w & 0xFFFFFFFFull);
+      uint32_t inc = cnt;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= (uint32_t)o) inc += v;
+      }
+      s_off[lane] = inc - cnt;
+      s_src[lane] = (uint32_t)(w >> 32);
+      if (lane == 31) s_off[32] = inc;
+    }
+    __syncthreads();
+    const uint32_t total = s_off[32];
+    for (uint32_t i = tid; i < total; i += kCompactThreads) {
+      // tile of hit i: the last offset <= i (binary search over 32 offsets)
+      uint32_t q = 0;
+#pragma unroll
+      for (uint32_t step = 16; step; step >>= 1)
+        if (q + step < ng && s_off[q + step] <= i) q += step;
+      const uint64_t src = (uint64_t)s_src[q] + (i - s_off[q]);
+      const uint64_t o = prefix + i;
       if (o >= a.max_clusters) { over = true; continue; }
-      const uint4 va = a.stage_a[src + c], vb = a.stage_b[src + c];
-      const uint64_t toa_peak = a.stage_c[src + c];
+      const uint4 va = a.stage_a[src], vb = a.stage_b[src];
+      const uint64_t toa_peak = a.stage_c[src];
       const long long st = (long long)va.z;
       const long long sx = (long long)(((unsigned long long)vb.y << 32) | vb.x);
       const long long sy = (long long)(((unsigned long long)vb.w << 32) | vb.z);
@@ -1024,11 +1049,11 @@ __global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, 
       const float fst = __ll2float_rn(st);
       a.out.cx[o] = __fdiv_rn(__ll2float_rn(sx), fst);
       a.out.cy[o] = __fdiv_rn(__ll2float_rn(sy), fst);
-      const long long sf = (long long)a.stage_d[src + c];
+      const long long sf = (long long)a.stage_d[src];
       a.out.sum_tot_tof[o] = sf;
       a.out.ctof[o] = __fdiv_rn(__ll2float_rn(sf), fst);
     }
-    prefix += cnt;
+    prefix += total;
   }
   if (over) set_error(a.ctrl, TPX3_ERR_CAPACITY);
   if (t1 == a.num_tiles && tid == 0) {
