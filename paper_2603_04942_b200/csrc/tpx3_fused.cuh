@@ -598,6 +598,23 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       }
     }
   };
+  // The same, fast for the common cases: a cell that is empty or holds one or two events (below lim) is settled
+  // with the min/max match network; only a third event or an overflowed bucket takes the slot-by-slot scan
+  // (which then skips the first two).
+  auto scan_cell2 = [&](uint32_t c, uint32_t slk, uint32_t key, uint32_t lim, auto&& sink) {
+    const uint32_t h = ((c | (slk << 16)) * kGold) >> kHashShift;
+    const uint4 e = *reinterpret_cast<const uint4*>(tab + 4u * h);
+    const uint32_t want = c << 16;
+    const uint32_t d0 = (e.x ^ want) - 1u, d1 = (e.y ^ want) - 1u, d2 = (e.z ^ want) - 1u,
+                   d3 = ((e.w & ~0x8000u) ^ want) - 1u;
+    const uint32_t mn01 = min(d0, d1), mx01 = max(d0, d1), mn23 = min(d2, d3), mx23 = max(d2, d3);
+    const uint32_t lo2 = max(mn01, mn23), hi2 = min(mx01, mx23);
+    const uint32_t s1 = min(mn01, mn23), s2 = min(lo2, hi2), s3 = max(lo2, hi2);
+    if (s1 < lim && absdiff_u32(recS[s1].x, key) <= a.W) sink(s1);
+    if (s2 < lim && absdiff_u32(recS[s2].x, key) <= a.W) sink(s2);
+    if (s3 < lim || (e.w & 0x8000u))
+      scan_cell(c, slk, key, lim, [&](uint32_t j) { if (j != s1 && j != s2) sink(j); });
+  };
   // mode 1 with a small box: the neighbours are found through the hash, (2 wx + 1)(2 wy + 1) cells per event;
   // a large box is cheaper to serve by walking the time window of the sorted tile
   const bool lm_grid = MODE != 0 && (2u * a.lm_wx + 1u) * (2u * a.lm_wy + 1u) <= 81u;
@@ -608,22 +625,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     const uint32_t y0 = y > a.lm_wy ? y - a.lm_wy : 0u, y1 = min(y + a.lm_wy, a.sensor_h - 1u);
     for (uint32_t yy = y0; yy <= y1; ++yy)
       for (uint32_t xx = x0; xx <= x1; ++xx) {
-        // most cells are empty or hold one event: find it with the min/max network; a second one is
-        // looked at the same way; only a third event of the cell or an overflowed bucket takes the slot-by-slot
-        // scan (which then skips the first two)
-        const uint32_t c = (yy << 8) | xx;
-        const uint32_t h = ((c | (slk << 16)) * kGold) >> kHashShift;
-        const uint4 e = *reinterpret_cast<const uint4*>(tab + 4u * h);
-        const uint32_t want = c << 16;
-        const uint32_t d0 = (e.x ^ want) - 1u, d1 = (e.y ^ want) - 1u, d2 = (e.z ^ want) - 1u,
-                       d3 = ((e.w & ~0x8000u) ^ want) - 1u;
-        const uint32_t mn01 = min(d0, d1), mx01 = max(d0, d1), mn23 = min(d2, d3), mx23 = max(d2, d3);
-        const uint32_t lo2 = max(mn01, mn23), hi2 = min(mx01, mx23);
-        const uint32_t s1 = min(mn01, mn23), s2 = min(lo2, hi2), s3 = max(lo2, hi2);
-        if (s1 < (uint32_t)T && absdiff_u32(recS[s1].x, key) <= a.W) sink(s1);
-        if (s2 < (uint32_t)T && absdiff_u32(recS[s2].x, key) <= a.W) sink(s2);
-        if (s3 < (uint32_t)T || (e.w & 0x8000u))
-          scan_cell(c, slk, key, (uint32_t)T, [&](uint32_t j) { if (j != s1 && j != s2) sink(j); });
+        scan_cell2((yy << 8) | xx, slk, key, (uint32_t)T, sink);
       }
   };
 
@@ -779,8 +781,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
           const uint32_t q = j - kTaskBase;
           const uint2 r = recS[k];
           const uint32_t off = q == 0u ? 256u : (q == 1u ? 1u : (q == 2u ? 257u : (q == 3u ? 255u : 0u)));
-          scan_cell((r.y & 0xFFFFu) + off, r.x >> tb, r.x, q == 4u ? k : (uint32_t)T,
-                    [&](uint32_t jj) { uf_unite(par, k, jj); });
+          scan_cell2((r.y & 0xFFFFu) + off, r.x >> tb, r.x, q == 4u ? k : (uint32_t)T,
+                     [&](uint32_t jj) { uf_unite(par, k, jj); });
         }
       }
     }
