@@ -184,6 +184,8 @@ struct FusedMisc {
   unsigned int n_roots;
   unsigned int n_list;         // deferred links pushed (may exceed the capacity: overflow)
   unsigned int skip;           // the call already failed in another tile
+  unsigned int min_tof;        // smallest time of flight among the events the tile loaded
+  unsigned int n_klist;        // tight tiles: events whose S cell is empty (second pass of the link step)
   unsigned int warp_sums[33];
 };
 static_assert(sizeof(FusedMisc) <= 512, "FusedMisc must fit kMiscBytes");
@@ -241,6 +243,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     misc->skip = atomicAdd(&a.ctrl->fused_fail, 0u);
     misc->fail = 0;
     misc->max_tof = 0;
+    misc->min_tof = kNone;
+    misc->n_klist = 0;
     misc->max_sl = 0;
     misc->n_roots = 0;
     misc->n_list = 0;
@@ -333,7 +337,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   }
   // lo = first shot start in [0, S); hi = first shot start in [S, cnt) (or cnt == end of stream)
   {
-    uint32_t my_lo = kNone, my_hi = kNone, mt = 0, ml = 0;
+    uint32_t my_lo = kNone, my_hi = kNone, mt = 0, ml = 0, mn = kNone;
 #pragma unroll
     for (int j = IPT - 1; j >= 0; --j) {
       if (bnd & (1u << j)) {
@@ -342,7 +346,9 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       }
       mt = max(mt, tof[j]);
       ml = max(ml, sl[j]);
+      if (p0 + j < cnt) mn = min(mn, tof[j]);
     }
+    mn = __reduce_min_sync(0xffffffffu, mn);
     my_lo = __reduce_min_sync(0xffffffffu, my_lo);
     my_hi = __reduce_min_sync(0xffffffffu, my_hi);
     mt = __reduce_max_sync(0xffffffffu, mt);
@@ -352,6 +358,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       if (my_lo != kNone) atomicMin(&misc->lo, my_lo);
       if (my_hi != kNone) atomicMin(&misc->hi, my_hi);
       if (mt) atomicMax(&misc->max_tof, mt);
+      if (mn != kNone) atomicMin(&misc->min_tof, mn);
       if (ml) atomicMax(&misc->max_sl, ml);
       if (any_bad) misc->fail = 1;
     }
@@ -676,13 +683,13 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   __syncthreads();
 
   // ---- S2: probe the forward cells, prune implied links, first link = parent, others deferred ---
+  uint32_t list_cap = (uint32_t)L::kListCap;   // tight tiles lend the top of the list region to the second pass
   auto push_link = [&](uint32_t k, uint32_t j) {
     const uint32_t pos = atomicAdd(&misc->n_list, 1u);
-    if (pos < (uint32_t)L::kListCap) list[pos] = (k << 16) | j;
+    if (pos < list_cap) list[pos] = (k << 16) | j;
   };
-  for (uint32_t k0 = 0; k0 < mm; k0 += THREADS) {
-    const uint32_t k = k0 + tid;
-    if (k < mm) {
+  auto link_event = [&](const uint32_t k) {
+    {
       const uint2 r = recS[k];
       const uint32_t key = r.x, cell = r.y & 0xFFFFu, slk = key >> tb, hs = slk << 16;
       const uint32_t x = cell & 0xFFu, y = cell >> 8;
@@ -743,6 +750,57 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         push_link(k, kTaskBase + q);
       }
     }
+  };
+  // Tight tiles: every time of flight the tile loaded lies within W of every other one (electron VMI: arrival
+  // spread far below the link window), so two events of one shot always pass the time test and the pruning
+  // rule drops every other candidate of an event whose S cell is occupied. Such an event needs ONE probe. First
+  // pass: S only; the events whose S cell is empty (or whose bucket overflowed) are collected and take the
+  // full five-cell step densely packed in a second pass.
+  const bool tight = MODE == 0 && misc->max_tof - misc->min_tof <= a.W;
+  if (tight) {
+    uint16_t* kl_end = reinterpret_cast<uint16_t*>(smem + L::kMisc);   // grows downwards from the list's end
+    constexpr uint32_t kKlMax = (uint32_t)(4 * L::kListCap - 1024) / 2u;   // leaves 256 deferred-list entries
+    const uint32_t lt_mask = lanemask_lt();
+    for (uint32_t k0 = warp * 32u; k0 < mm; k0 += THREADS) {          // warp-uniform trip count (ballot inside)
+      const uint32_t k = k0 + lane;
+      bool second = false;
+      if (k < mm) {
+        const uint2 r = recS[k];
+        const uint32_t key = r.x, cell = r.y & 0xFFFFu;
+        second = true;
+        if ((cell >> 8) + 1u < a.sensor_h) {
+          const uint32_t c = cell + 256u;
+          const uint32_t h = ((c | ((key >> tb) << 16)) * kGold) >> kHashShift;
+          const uint4 e = *reinterpret_cast<const uint4*>(tab + 4u * h);
+          const uint32_t want = c << 16;
+          const uint32_t d0 = (e.x ^ want) - 1u, d1 = (e.y ^ want) - 1u, d2 = (e.z ^ want) - 1u,
+                         d3 = ((e.w & ~0x8000u) ^ want) - 1u;
+          const uint32_t s1 = min(min(d0, d1), min(d2, d3));
+          if (s1 < (uint32_t)T && !(e.w & 0x8000u) && absdiff_u32(recS[s1].x, key) <= a.W) {
+            par[k] = (uint16_t)s1;
+            second = false;
+          }
+        }
+      }
+      const uint32_t bal = __ballot_sync(0xffffffffu, second);
+      if (bal) {
+        uint32_t basepos = 0;
+        if (lane == 0) basepos = atomicAdd(&misc->n_klist, (uint32_t)__popc(bal));
+        basepos = __shfl_sync(0xffffffffu, basepos, 0);
+        const uint32_t idx = basepos + (uint32_t)__popc(bal & lt_mask);
+        if (second && idx < kKlMax) kl_end[-1 - (int)idx] = (uint16_t)k;
+      }
+    }
+    __syncthreads();
+    const uint32_t n2 = misc->n_klist;
+    if (n2 <= kKlMax) {
+      list_cap = ((uint32_t)(4 * L::kListCap) - 2u * n2) / 4u;   // what the collected events leave of the region
+      for (uint32_t i = tid; i < n2; i += THREADS) link_event(kl_end[-1 - (int)i]);
+    } else {                                                       // mostly isolated pixels: the plain single pass
+      for (uint32_t k = tid; k < mm; k += THREADS) link_event(k);
+    }
+  } else {
+    for (uint32_t k = tid; k < mm; k += THREADS) link_event(k);
   }
   __syncthreads();
   // ---- deferred links: union by compare-and-swap hooks ---------------------------------------------
@@ -756,7 +814,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         const uint32_t p1 = par[k], g = par[p1];
         if (g != p1) par[k] = (uint16_t)g;
       }
-    if (nl > (uint32_t)L::kListCap) {
+    if (nl > list_cap) {
       // the list overflowed (very dense tile): redo the probes, uniting on the spot
       for (uint32_t k = tid; k < mm; k += THREADS) {
         const uint2 r = recS[k];
