@@ -18,7 +18,9 @@
  *     caller (the Python binding passes PyTorch tensors); [host] is host memory. The library
  *     never frees or reallocates caller memory and never writes its inputs.
  *   - `workspace` is a [dev] scratch buffer of at least the `workspace_bytes` reported by
- *     tpx3_plan, 256-byte aligned. Its contents are undefined between calls.
+ *     tpx3_plan, 256-byte aligned. Its contents are undefined between calls and need no
+ *     initialisation (one word of the control block is a performance hint that is kept from
+ *     call to call when the same workspace is reused; it never changes a result).
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
  *     Device-pointer calls only ENQUEUE work on that stream and return; there is no hidden
  *     synchronisation. Outputs are valid once the stream has reached the end of the call.

@@ -22,8 +22,15 @@ struct Ctrl {
   uint32_t n_roots;              // scratch root counter
   uint32_t tiles_done;           // fused path: tiles finished
   uint32_t fused_fail;           // fused path: some tile could not be handled
-  uint32_t pad[2];
+  uint32_t tight_tiles;          // fused path: tiles of this call whose time clusters were all tight
+  uint32_t pad[1];
+  // Kept ACROSS calls on the same workspace (never reset; any garbage is a legal value: it only steers which of
+  // two exact code paths a tile takes). A stream keeps its character from chunk to chunk: when hardly any tile
+  // of a call had tight time clusters, the tiles of the next calls skip the check (and retry every 16th call).
+  uint32_t scan_hint;            // kScanSkip: the last call found the time-cluster check not worth its cost
+  uint32_t calls;                // fused calls served on this workspace
 };
+constexpr uint32_t kScanSkip = 0x5C1Fu;
 static_assert(sizeof(Ctrl) <= 256, "Ctrl must fit the 256-byte workspace header");
 
 // Parameters every kernel needs (passed by value).

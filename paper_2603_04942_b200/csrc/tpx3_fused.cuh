@@ -184,8 +184,9 @@ struct FusedMisc {
   unsigned int n_roots;
   unsigned int n_list;         // deferred links pushed (may exceed the capacity: overflow)
   unsigned int skip;           // the call already failed in another tile
+  unsigned int loose;          // some time cluster of the tile is wider than W ("within W" is not transitive)
   unsigned int min_tof;        // smallest time of flight among the events the tile loaded
-  unsigned int n_klist;        // tight tiles: events whose S cell is empty (second pass of the link step)
+  unsigned int n_klist;        // other tiles: events whose S cell is empty (second pass of the link step)
   unsigned int warp_sums[33];
 };
 static_assert(sizeof(FusedMisc) <= 512, "FusedMisc must fit kMiscBytes");
@@ -243,6 +244,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     misc->skip = atomicAdd(&a.ctrl->fused_fail, 0u);
     misc->fail = 0;
     misc->max_tof = 0;
+    misc->loose = 0;
     misc->min_tof = kNone;
     misc->n_klist = 0;
     misc->max_sl = 0;
@@ -392,7 +394,13 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 
   // ---- records as loaded -> region B, 128-bit loads of x / y / tot ------------------------------
   uint2* recB = reinterpret_cast<uint2*>(smem + L::kRegB);
+  // The time-cluster check (below) is skipped when all times of flight lie within W anyway, and when the last
+  // call on this workspace found hardly any tight tile (the hint; every 16th call looks again).
+  const bool cl_wide = misc->max_tof - misc->min_tof > a.W;
+  const bool cl_scan = MODE == 0 && cl_wide && (a.ctrl->scan_hint != kScanSkip || (a.ctrl->calls & 15u) == 0u);
   bool uns = false;
+  uint32_t cl_last_start = 0, cl_lead_last = 0;   // time-cluster check on the keys in registers
+  bool cl_have_lead = false, cl_loose = false;
   if (mm && p0 < hi && p0 + IPT > lo) {
     uint32_t key_r[IPT];
 #pragma unroll
@@ -403,6 +411,22 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 #pragma unroll
     for (int j = 1; j < IPT; ++j)
       if (p0 + j > lo && p0 + j < hi && key_r[j] < key_r[j - 1]) uns = true;
+    // time clusters (see "are the time clusters of the tile tight?" below): for a tile that is in order the
+    // keys are at hand here, in registers, in the blocked arrangement the check wants
+    if (cl_scan) {
+      uint32_t cur = 0;
+      bool have_cur = false;
+#pragma unroll
+      for (int j = 0; j < IPT; ++j) {
+        const uint32_t q = p0 + (uint32_t)j;
+        if (q >= lo && q < hi) {
+          const uint32_t key = key_r[j], prev = j ? key_r[j - 1] : keyp;
+          if (q == lo || key - prev > a.W) { cur = key; have_cur = true; cl_last_start = key; }
+          else if (have_cur) { if (key - cur > a.W) cl_loose = true; }
+          else { cl_lead_last = key; cl_have_lead = true; }
+        }
+      }
+    }
     uint4 vx, vy, vt;
     if (p0 + IPT <= cnt) {
       vx = ldg_nc_v4(a.x + base + p0);
@@ -453,7 +477,25 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 #pragma unroll
     for (int q = 0; q < 4; ++q) dst[q] = make_uint4(key_r[2 * q], w1[2 * q], key_r[2 * q + 1], w1[2 * q + 1]);
   }
+  uint32_t cl_carry = 0;
+  if (cl_scan) {
+    uint32_t cl_inc = cl_last_start;   // prefix maximum of the cluster starts: 0 = "none" is the identity
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, cl_inc, o);
+      if (lane >= (uint32_t)o) cl_inc = max(cl_inc, t);
+    }
+    if (lane == 31) misc->warp_sums[warp] = cl_inc;
+    cl_carry = __shfl_up_sync(0xffffffffu, cl_inc, 1);
+    if (lane == 0) cl_carry = 0;
+  }
   const bool unsorted = __syncthreads_or(uns ? 1 : 0) != 0;
+  if (cl_wide && !cl_scan && tid == 0) misc->loose = 1u;   // not checked: treated as not tight
+  if (!unsorted && cl_scan) {
+    for (uint32_t w = 0; w < warp; ++w) cl_carry = max(cl_carry, misc->warp_sums[w]);
+    if (cl_have_lead && cl_lead_last - cl_carry > a.W) cl_loose = true;   // position lo starts a cluster
+    if (cl_loose) misc->loose = 1u;
+  }
 
   // ---- S1: stable LSD radix sort of local indices by (shot offset, tof) (only if needed) --------
   uint2* recA = reinterpret_cast<uint2*>(smem + L::kRegA);
@@ -678,6 +720,44 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     }
     __syncthreads();
   } else {
+  // ---- are the time clusters of the tile tight? --------------------------------------------------------
+  // Cut the ascending keys into clusters wherever two neighbours are more than W apart (a new shot always is).
+  // If every cluster spans at most W, "within W" is an equivalence relation on the tile: two events that are
+  // both within W of a third are within W of each other. The link step below then needs one probe for most
+  // events. One pass over the sorted keys; the start of the cluster that runs into a warp's range is the largest
+  // cluster-start key of the warps before it (the keys ascend, so a prefix maximum).
+  // (Nothing to check when all times of flight of the tile lie within W: electron VMI. Tiles that arrived in
+  // order did this on the keys in registers while building their records; see there.)
+  if (unsorted && cl_scan) {
+    // thread t owns the sorted positions [8t, 8t + 8)
+    const uint32_t q0 = tid * (uint32_t)IPT;
+    uint32_t last_start = 0, lead_last = 0, cur = 0, prev = (q0 > 0u && q0 < mm) ? recS[q0 - 1u].x : 0u;
+    bool have_cur = false, have_lead = false, loose = false;
+#pragma unroll
+    for (int j = 0; j < IPT; ++j) {
+      const uint32_t k = q0 + (uint32_t)j;
+      if (k < mm) {
+        const uint32_t key = recS[k].x;
+        if (k == 0u || key - prev > a.W) { cur = key; have_cur = true; last_start = key; }
+        else if (have_cur) { if (key - cur > a.W) loose = true; }
+        else { lead_last = key; have_lead = true; }
+        prev = key;
+      }
+    }
+    uint32_t inc = last_start;   // 0 = "no start here" is the identity of max on keys
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= (uint32_t)o) inc = max(inc, t);
+    }
+    if (lane == 31) misc->warp_sums[warp] = inc;
+    uint32_t carry = __shfl_up_sync(0xffffffffu, inc, 1);
+    if (lane == 0) carry = 0;
+    __syncthreads();
+    for (uint32_t w = 0; w < warp; ++w) carry = max(carry, misc->warp_sums[w]);
+    if (have_lead && lead_last - carry > a.W) loose = true;   // position 0 starts a cluster, so a carry exists
+    if (loose) misc->loose = 1u;
+  }
   // ---- hash insert ----------------------------------------------------------------------------------
   hash_insert();
   __syncthreads();
@@ -751,12 +831,13 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       }
     }
   };
-  // Tight tiles: every time of flight the tile loaded lies within W of every other one (electron VMI: arrival
-  // spread far below the link window), so two events of one shot always pass the time test and the pruning
-  // rule drops every other candidate of an event whose S cell is occupied. Such an event needs ONE probe. First
-  // pass: S only; the events whose S cell is empty (or whose bucket overflowed) are collected and take the
-  // full five-cell step densely packed in a second pass.
-  const bool tight = MODE == 0 && misc->max_tof - misc->min_tof <= a.W;
+  // Tight tiles (all time clusters at most W wide: electron VMI, ion VMI with separated mass peaks): two events
+  // that pass the time test against a third pass it against each other, so the pruning rule drops every other
+  // candidate of an event whose S cell holds an event of its own time cluster. Such an event needs ONE probe.
+  // First pass: S only; the events whose S cell is empty, holds another cluster's event first, or overflowed are
+  // collected and take the full five-cell step densely packed in a second pass.
+  const bool tight = MODE == 0 && misc->loose == 0u;
+  if (tight && tid == 0) atomicAdd(&a.ctrl->tight_tiles, 1u);
   if (tight) {
     uint16_t* kl_end = reinterpret_cast<uint16_t*>(smem + L::kMisc);   // grows downwards from the list's end
     constexpr uint32_t kKlMax = (uint32_t)(4 * L::kListCap - 1024) / 2u;   // leaves 256 deferred-list entries
@@ -1121,6 +1202,10 @@ __global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, 
     a.ctrl->status.n_clusters = (uint32_t)prefix;
     a.ctrl->status.path = a.mode ? 3 : 1;
     a.ctrl->status.sort_passes = 0;
+    if (a.mode == 0u) {   // worth checking the time clusters next time? (fewer than 1 tile in 8 was tight: no)
+      a.ctrl->scan_hint = a.ctrl->tight_tiles * 8u < a.num_tiles ? kScanSkip : 0u;
+      a.ctrl->calls += 1u;
+    }
   }
 }
 
