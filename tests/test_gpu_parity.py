@@ -703,3 +703,31 @@ def test_full_size_localmax_cfg1(tpx3):
         np.testing.assert_array_equal(c["c_label"][i0:i1], o["c_label"] + np.uint32(a), err_msg=what)
         for key in LM_KEYS[1:]:
             np.testing.assert_array_equal(c[key][i0:i1], o[key], err_msg=what + " " + key)
+
+
+def test_time_cluster_hint_never_changes_results(tpx3):
+    """One plan (one workspace) serving calls of different character: the hint the fused kernel leaves in the
+    workspace (skip the time-cluster check after a call with hardly any tight tile) only selects between two
+    exact code paths, so every call must match the oracle whatever came before it."""
+    import torch
+
+    m = tpx3
+    loose = gen.generate(3, shots=300)      # noise hits chain the time clusters: no tight tiles
+    multi = gen.generate(2, shots=700)      # separated mass peaks: tight tiles with several clusters
+    narrow = gen.generate(1, shots=1500)    # all times of flight within W
+    nmax = max(w.n for w in (loose, multi, narrow))
+    pl = m.plan(m.Config(max_hits=nmax, toa_window_ticks=W, shot_period_ticks=P, max_shot_hits=gen.max_shot_hits(3)))
+    cl = m.Clusters(nmax, pl.device)
+    for name, w in [("loose", loose), ("loose again", loose), ("multi after loose", multi), ("multi again", multi),
+                    ("narrow", narrow), ("loose after narrow", loose), ("multi", multi)] + [("multi x%d" % i, multi) for i in range(16)]:
+        o = oracle.run(w.x, w.y, w.toa, w.tot, W, P)
+        dev = [to_dev(a) for a in (w.x, w.y, w.toa, w.tot)]
+        perm, label, nc = pl.cluster_centroid(*dev, cl)
+        torch.cuda.synchronize()
+        st = pl.status()
+        assert st["error"] == 0 and st["path"] == 1, name
+        ncl = int(nc.cpu().numpy()[0])
+        g = {"perm": perm[: w.n].cpu().numpy(), "label": label[: w.n].cpu().numpy(), "n_clusters": ncl}
+        g.update(cl.numpy(ncl))
+        assert_parity(g, o, name)
+    pl.free()
