@@ -768,7 +768,10 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     const uint32_t pos = atomicAdd(&misc->n_list, 1u);
     if (pos < list_cap) list[pos] = (k << 16) | j;
   };
-  auto link_event = [&](const uint32_t k) {
+  // tt: the tile is tight (see below). Then a candidate that passes the time test stands for every event of
+  // its cell and time cluster (they are connected among themselves: through their common S event, or by the
+  // later one's own-cell probe), and the cell needs no scan task.
+  auto link_event = [&](const uint32_t k, const bool tt) {
     {
       const uint2 r = recS[k];
       const uint32_t key = r.x, cell = r.y & 0xFFFFu, slk = key >> tb, hs = slk << 16;
@@ -790,8 +793,9 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         const bool any = valid && s1 < lim;
         jc = any ? s1 : k;
         kc = recS[jc].x;
-        if (valid && (s2 < lim || (e.w & 0x8000u))) slow |= bit;
-        return any && absdiff_u32(kc, key) <= a.W;
+        const bool pass = any && absdiff_u32(kc, key) <= a.W;
+        if (valid && (s2 < lim || (e.w & 0x8000u)) && !(tt && pass)) slow |= bit;
+        return pass;
       };
       uint32_t jS, kS, jE, kE, jSE, kSE, jSW, kSW, jO, kO;
       const bool pS = probe(256u, ys, (uint32_t)T, 1u, jS, kS);
@@ -876,12 +880,12 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     const uint32_t n2 = misc->n_klist;
     if (n2 <= kKlMax) {
       list_cap = ((uint32_t)(4 * L::kListCap) - 2u * n2) / 4u;   // what the collected events leave of the region
-      for (uint32_t i = tid; i < n2; i += THREADS) link_event(kl_end[-1 - (int)i]);
+      for (uint32_t i = tid; i < n2; i += THREADS) link_event(kl_end[-1 - (int)i], true);
     } else {                                                       // mostly isolated pixels: the plain single pass
-      for (uint32_t k = tid; k < mm; k += THREADS) link_event(k);
+      for (uint32_t k = tid; k < mm; k += THREADS) link_event(k, false);
     }
   } else {
-    for (uint32_t k = tid; k < mm; k += THREADS) link_event(k);
+    for (uint32_t k = tid; k < mm; k += THREADS) link_event(k, false);
   }
   __syncthreads();
   // ---- deferred links: union by compare-and-swap hooks ---------------------------------------------
