@@ -4,6 +4,7 @@ Plain, sequential CPU definitions of the paper's preprocessing steps (PAPER.md s
 paper's order with Python integers (no overflow games). They share no code with the CUDA path.
 
   unwrap_toa   section IV.A, PAPER.md:58-62   ToA counter unwrapping
+  StreamModel  SURVEY.md 8f NEXT #3, last clause: chunk cuts that are not shot-aligned (R24)
 """
 from __future__ import annotations
 
@@ -83,3 +84,64 @@ def preprocess(x, y, toa, tot, trig, cut: int, table, P_out: int, shot_base: int
         ts.append((shot_base + s) * P_out + tofc)
     return (np.array(xs, dtype=np.uint16), np.array(ys, dtype=np.uint16), np.array(ts, dtype=np.uint64),
             np.array(os_, dtype=np.uint16), np.array(idx, dtype=np.int64))
+
+
+STREAM_SAMPLE = 65536   # events at the end of a chunk that feed the running maximum (R24)
+
+
+class StreamModel:
+    """Chunked processing of an endless stream whose chunk cuts fall anywhere (SURVEY.md 8f NEXT #3:
+    "chunk cuts that are not shot-aligned"). The definition it must reproduce is the batch one: the hits of
+    the whole stream, because "each pixel [is] associated with the most recent laser trigger"
+    and no hit crosses a shot (reading R6) — so a chunk may be cut anywhere as long as every shot is
+    clustered in ONE piece. Reading R24, step by step for one push of a chunk (plain lists, stream order):
+
+      1. t_max = max(t_max, the ToA of the last STREAM_SAMPLE events of the chunk). The stream promises a
+         bounded disorder D: no later event has ToA < (largest ToA so far) - D (pixels report
+         out of order, dimmer ones first). Any lower bound of the largest ToA keeps step 2 safe.
+      2. s_cut = max(s_emitted, (t_max - D) div P): every shot below s_cut is complete. final: s_cut = inf.
+      3. working set = carried events ++ chunk, in that order (the carried ones came first in the stream):
+           shot <  s_emitted  -> late (its shot went out already): dropped and counted
+           shot <  s_cut      -> emitted now: one batch call on exactly these events, in stream order
+           otherwise          -> carried to the next push, in stream order
+      4. s_emitted = s_cut.
+    Returns per push the emitted events; the caller clusters them with the batch oracle. With no late event
+    the emitted sets, concatenated, are the stream re-cut at shot boundaries, so their hits in order are the
+    batch hits of the whole stream and `label_base` (events emitted before) makes the labels global."""
+
+    def __init__(self, P: int, D: int):
+        assert P > 0
+        self.P, self.D = int(P), int(D)
+        self.t_max = 0
+        self.s_emitted = 0
+        self.label_base = 0
+        self.carry = []          # (x, y, toa, tot) tuples in stream order
+        self.late_total = 0
+
+    def push(self, x, y, toa, tot, final: bool = False):
+        chunk = [(int(a), int(b), int(c), int(d)) for a, b, c, d in zip(x, y, toa, tot)]
+        for ev in chunk[-STREAM_SAMPLE:]:
+            self.t_max = max(self.t_max, ev[2])
+        if final:
+            s_cut = None
+        else:
+            s_cut = max(self.s_emitted, (self.t_max - self.D) // self.P if self.t_max >= self.D else 0)
+        emit, keep, late = [], [], 0
+        for ev in self.carry + chunk:
+            s = ev[2] // self.P
+            if s < self.s_emitted:
+                late += 1
+            elif s_cut is None or s < s_cut:
+                emit.append(ev)
+            else:
+                keep.append(ev)
+        self.carry = keep
+        if s_cut is not None:
+            self.s_emitted = s_cut
+        self.late_total += late
+        base = self.label_base
+        self.label_base += len(emit)
+        cols = list(zip(*emit)) if emit else [[], [], [], []]
+        return {"x": np.array(cols[0], dtype=np.uint16), "y": np.array(cols[1], dtype=np.uint16),
+                "toa": np.array(cols[2], dtype=np.uint64), "tot": np.array(cols[3], dtype=np.uint16),
+                "n_late": late, "n_carry": len(keep), "label_base": base}

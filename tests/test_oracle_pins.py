@@ -597,3 +597,105 @@ def test_preprocess_recovers_the_generated_stream():
     assert not np.any(is_dark[order][idx]) and len(idx) == w.n          # exactly the dark counts are cut
     back = np.argsort(order[idx], kind="stable")                        # original event order
     assert np.array_equal(ts[back], w.toa) and np.array_equal(xs[back], w.x) and np.array_equal(os_[back], w.tot)
+
+
+# ------------------------------------------------------------------ chunked stream, unaligned cuts (NEXT #3)
+def _stream_rows(model, chunks, W, P):
+    """Push the chunks (the last one with final=True); cluster every emitted set with the batch oracle and
+    concatenate the hit rows, labels made global with label_base."""
+    cols = {k: [] for k in ("c_label", "c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y",
+                            "c_sum_tot_tof", "c_toa_peak", "c_cx", "c_cy", "c_ctof")}
+    stats = []
+    for i, (x, y, toa, tot) in enumerate(chunks):
+        e = model.push(x, y, toa, tot, final=(i == len(chunks) - 1))
+        stats.append((len(e["x"]), e["n_carry"], e["n_late"]))
+        r = oracle.run(e["x"], e["y"], e["toa"], e["tot"], W, P)
+        for k in cols:
+            v = r[k]
+            cols[k].append(v + np.uint32(e["label_base"]) if k == "c_label" else v)
+    return {k: np.concatenate(v) for k, v in cols.items()}, stats
+
+
+def _cut(w, sizes):
+    out, i = [], 0
+    for s in sizes:
+        out.append((w.x[i:i + s], w.y[i:i + s], w.toa[i:i + s], w.tot[i:i + s]))
+        i += s
+    assert i == w.n
+    return out
+
+
+def _disorder(toa):
+    t = toa.astype(np.int64)
+    return int(np.max(np.maximum.accumulate(t) - t)) if len(t) else 0
+
+
+def test_stream_hand_example_cluster_across_the_cut():
+    """Two pixels of one hit on either side of a chunk cut, a second shot after them: the first push emits
+    nothing (shot 0 is not complete), the second emits shot 0 as ONE hit of two pixels, final emits shot 1."""
+    P, W = 1000, 5
+    m = pp.StreamModel(P, 0)
+    a = m.push([5], [5], [10], [3])
+    assert (len(a["x"]), a["n_carry"], a["n_late"]) == (0, 1, 0)
+    b = m.push([5, 9], [6, 9], [11, 1004], [4, 7])
+    assert b["toa"].tolist() == [10, 11] and b["n_carry"] == 1 and b["label_base"] == 0
+    r = oracle.run(b["x"], b["y"], b["toa"], b["tot"], W, P)
+    assert r["n_clusters"] == 1 and r["c_size"].tolist() == [2] and r["c_sum_tot_y"].tolist() == [3 * 5 + 4 * 6]
+    c = m.push([], [], [], [], final=True)
+    assert c["toa"].tolist() == [1004] and c["label_base"] == 2 and c["n_carry"] == 0
+
+
+def test_stream_late_event_is_counted_not_clustered():
+    P = 100
+    m = pp.StreamModel(P, 0)                     # the stream claims to be in order
+    a = m.push([1, 2], [1, 2], [10, 250], [5, 5])
+    assert a["toa"].tolist() == [10] and a["n_carry"] == 1
+    b = m.push([3], [3], [20], [5])              # shot 0 went out already
+    assert b["n_late"] == 1 and len(b["x"]) == 0 and m.late_total == 1
+    m2 = pp.StreamModel(P, 240)                  # with the true disorder bound nothing is late
+    a2 = m2.push([1, 2], [1, 2], [10, 250], [5, 5])
+    assert len(a2["x"]) == 0 and a2["n_carry"] == 2
+    b2 = m2.push([3], [3], [20], [5], final=True)
+    assert b2["toa"].tolist() == [10, 250, 20] and b2["n_late"] == 0
+
+
+@pytest.mark.parametrize("cfg,shots,sizes", [
+    (0, 12, "ones"), (0, 40, 997), (0, 40, "random"), (0, 40, "whole"), (4, 6, 4099), (4, 6, "random"),
+])
+def test_stream_model_equals_batch(cfg, shots, sizes):
+    """The definition: the hits of the chunked stream, in order, ARE the batch hits of the whole stream —
+    every column, labels included — wherever the cuts fall (inside shots, inside hits, chunks of one event,
+    one chunk for everything), for an in-order stream (D = 0) and a locally shuffled one (D = its bound)."""
+    w = gen.generate(cfg, shots=shots)
+    if cfg == 4:
+        assert _disorder(w.toa) > 0
+    rng = np.random.default_rng(5)
+    if sizes == "ones":
+        sz = [1] * w.n
+    elif sizes == "whole":
+        sz = [w.n]
+    elif sizes == "random":
+        sz = []
+        while sum(sz) < w.n:
+            sz.append(int(min(rng.integers(1, max(2, w.n // 9)), w.n - sum(sz))))
+    else:
+        sz = [sizes] * (w.n // sizes) + ([w.n % sizes] if w.n % sizes else [])
+    m = pp.StreamModel(P, _disorder(w.toa))
+    rows, stats = _stream_rows(m, _cut(w, sz), W, P)
+    ref = oracle.run(w.x, w.y, w.toa, w.tot, W, P)
+    assert m.late_total == 0 and sum(s[0] for s in stats) == w.n
+    for k, v in rows.items():
+        assert np.array_equal(v, ref[k]), k
+    if sizes not in ("whole",):
+        assert max(s[1] for s in stats) > 0          # something was carried: the cuts were not shot-aligned
+
+
+def test_stream_carry_is_bounded_by_the_open_shots():
+    """In-order stream: what is carried is never more than the events of the shot still open."""
+    w = gen.generate(0, shots=30)
+    m = pp.StreamModel(P, 0)
+    per_shot = np.bincount((w.toa // np.uint64(P)).astype(np.int64)).max()
+    for c in _cut(w, [500] * (w.n // 500) + [w.n % 500]):
+        e = m.push(*c)
+        assert e["n_carry"] <= per_shot
+        assert all(t // P >= m.s_emitted for t in (ev[2] for ev in m.carry))
