@@ -196,6 +196,46 @@ int tpx3_process_host(tpx3_plan_t plan, void* workspace, void* device_io, void* 
 /* Synchronise `cuda_stream` and copy the workspace's status word to *out [host]. */
 int tpx3_status(tpx3_plan_t plan, const void* workspace, void* cuda_stream, tpx3_status_t* out);
 
+/* Chunked stream with cuts that are not shot-aligned (last clause; DESIGN.md
+ * R24). An endless pixel stream arrives in chunks cut anywhere - inside a shot, inside a hit. Every
+ * pixel belongs to "the most recent laser trigger" and no hit crosses a shot, so the
+ * stream object holds back the events of shots that may still grow and clusters every shot in one
+ * piece: the hit rows of all pushes, in order, are exactly the rows one tpx3_cluster_centroid call
+ * on the whole stream would write (labels included: label = position in the (shot, ToA) order of
+ * the whole stream, modulo 2^32).
+ *   disorder_ticks  D: the stream promises that no event arrives with ToA < (largest ToA so far) - D
+ *                   (0 = in ToA order; pixels report out of order, dimmer ones first).
+ *   per push        t_max = max(t_max, ToA of the last 65536 events of the chunk); s_cut =
+ *                   max(s_emitted, (t_max - D) div P); of the carried events followed by the chunk,
+ *                   in stream order: shot < s_emitted: late (dropped, counted); shot < s_cut: emitted
+ *                   = clustered now; the rest carried. final != 0 emits everything and ends the
+ *                   stream.
+ * stream_buf [dev]: tpx3_stream_bytes(max_chunk, max_carry) bytes, caller-owned, holds the carried
+ * events, the emitted events of the current push and the stream state; max_chunk + max_carry <=
+ * the plan's max_hits; the plan's shot period must be > 0. tpx3_stream_open enqueues the reset of the
+ * state on cuda_stream. tpx3_stream_push: x, y, toa, tot [dev] of n <= max_chunk events; out,
+ * n_hits [dev] as tpx3_cluster_centroid; info [host] (may be NULL). The push SYNCHRONISES cuda_stream
+ * once (the number of emitted events sizes the clustering launch); the clustering itself is only
+ * enqueued. More than max_carry events to carry: TPX3_ERR_CAPACITY, and the stream is dead. Cluster
+ * capacity and input errors are reported as by tpx3_cluster_centroid (tpx3_status). */
+typedef struct tpx3_stream_s* tpx3_stream_t;
+typedef struct {
+  uint64_t n_emitted;     /* events clustered by this push                                  */
+  uint64_t n_carry;       /* events held back for the next push                             */
+  uint64_t n_late;        /* events of this push whose shot had gone out already (dropped)  */
+  uint64_t late_total;    /* the same, since tpx3_stream_open                               */
+  uint64_t label_base;    /* events emitted by earlier pushes (added to the label column)   */
+  uint64_t shots_emitted; /* every shot below this index is complete and written            */
+} tpx3_stream_info_t;
+size_t tpx3_stream_bytes(uint64_t max_chunk, uint64_t max_carry);
+int tpx3_stream_open(tpx3_plan_t plan, void* stream_buf, uint64_t max_chunk, uint64_t max_carry,
+                     uint64_t disorder_ticks, void* cuda_stream, tpx3_stream_t* out);
+int tpx3_stream_push(tpx3_stream_t stream, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x,
+                     const uint16_t* y, const uint64_t* toa, const uint16_t* tot, int final_push,
+                     uint64_t max_clusters, const tpx3_clusters_t* out, uint32_t* n_hits,
+                     tpx3_stream_info_t* info);
+int tpx3_stream_close(tpx3_stream_t stream);
+
 /* Number of kernels the library has launched through this plan (for launch accounting). */
 uint64_t tpx3_launch_count(tpx3_plan_t plan);
 

@@ -16,7 +16,7 @@ from dataclasses import dataclass
 from . import _build
 
 __all__ = [
-    "Tpx3Error", "Config", "Clusters", "Plan", "plan", "load_library", "exported_symbols",
+    "Tpx3Error", "Config", "Clusters", "Plan", "Stream", "plan", "load_library", "exported_symbols",
     "FLAG_VALIDATE_INPUT", "FLAG_FORCE_GENERAL", "strerror", "shard_shots",
 ]
 
@@ -29,6 +29,7 @@ OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_OUT_OF_RANGE, ERR_CUDA, ERR_UNIMPLEMENTED
 exported_symbols = (
     "tpx3_plan", "tpx3_cluster", "tpx3_centroid", "tpx3_cluster_centroid", "tpx3_localmax_centroid",
     "tpx3_unwrap_toa", "tpx3_timewalk_table", "tpx3_preprocess", "tpx3_host_io_bytes",
+    "tpx3_stream_bytes", "tpx3_stream_open", "tpx3_stream_push", "tpx3_stream_close",
     "tpx3_process_host", "tpx3_status", "tpx3_launch_count", "tpx3_profile_enable", "tpx3_profile_read",
     "tpx3_free", "tpx3_strerror",
 )
@@ -54,6 +55,11 @@ class _CClusters(ctypes.Structure):
     _fields_ = [(k, ctypes.c_void_p) for k in
                 ("label", "size", "shot", "sum_tot", "sum_tot_x", "sum_tot_y", "toa_peak", "cx", "cy", "sum_tot_tof",
                  "ctof")]
+
+
+class _CStreamInfo(ctypes.Structure):
+    _fields_ = [(k, ctypes.c_uint64) for k in ("n_emitted", "n_carry", "n_late", "late_total", "label_base",
+                                               "shots_emitted")]
 
 
 class _CStatus(ctypes.Structure):
@@ -95,6 +101,15 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.tpx3_preprocess.restype = ctypes.c_int
     lib.tpx3_preprocess.argtypes = [vp, vp, vp, u64, vp, vp, vp, vp, u64, vp, u64, vp, ctypes.c_uint32, u64,
                                     vp, vp, vp, vp, vp, vp]
+    lib.tpx3_stream_bytes.restype = ctypes.c_size_t
+    lib.tpx3_stream_bytes.argtypes = [u64, u64]
+    lib.tpx3_stream_open.restype = ctypes.c_int
+    lib.tpx3_stream_open.argtypes = [vp, vp, u64, u64, u64, vp, ctypes.POINTER(vp)]
+    lib.tpx3_stream_push.restype = ctypes.c_int
+    lib.tpx3_stream_push.argtypes = [vp, vp, vp, u64, vp, vp, vp, vp, ctypes.c_int, u64,
+                                     ctypes.POINTER(_CClusters), vp, ctypes.POINTER(_CStreamInfo)]
+    lib.tpx3_stream_close.restype = ctypes.c_int
+    lib.tpx3_stream_close.argtypes = [vp]
     lib.tpx3_host_io_bytes.restype = ctypes.c_size_t
     lib.tpx3_host_io_bytes.argtypes = [u64, u64]
     lib.tpx3_process_host.restype = ctypes.c_int
@@ -323,6 +338,10 @@ class Plan:
             raise Tpx3Error(rc, "tpx3_cluster_centroid")
         return perm, label, n_clusters
 
+    # -- chunked stream, cuts not shot-aligned -----------------------------
+    def stream_open(self, max_chunk: int, max_carry: int, disorder_ticks: int = 0, stream=None) -> "Stream":
+        return Stream(self, max_chunk, max_carry, disorder_ticks, stream)
+
     # -- end to end with host buffers ------------------------------------------------------------
     def process_host(self, x, y, toa, tot, clusters_host: Clusters, perm=None, label=None, stream=None) -> int:
         """x, y, toa, tot: host tensors (pinned for full copy speed). perm / label: host uint32
@@ -389,6 +408,54 @@ class Plan:
         _check_dev(tot, torch.uint16, n, "tot")
         if n > self.cfg.max_hits:
             raise Tpx3Error(ERR_INVALID_ARG, "n > max_hits")
+
+
+class Stream:
+    """tpx3_stream_open / _push / _close: argument marshalling only."""
+
+    def __init__(self, pl: "Plan", max_chunk: int, max_carry: int, disorder_ticks: int, stream=None):
+        import torch
+
+        self.plan = pl
+        self.buf = torch.empty(int(pl.lib.tpx3_stream_bytes(max_chunk, max_carry)), dtype=torch.uint8,
+                               device=pl.device)
+        h = ctypes.c_void_p()
+        rc = pl.lib.tpx3_stream_open(pl.handle, self.buf.data_ptr(), max_chunk, max_carry, disorder_ticks,
+                                     _stream_ptr(stream), ctypes.byref(h))
+        if rc != OK:
+            raise Tpx3Error(rc, "tpx3_stream_open")
+        self.handle = h
+
+    def push(self, x, y, toa, tot, clusters: "Clusters", final: bool = False, n_hits=None, stream=None):
+        """Returns (n_hits device tensor, info dict). Synchronises the stream once."""
+        import torch
+
+        pl = self.plan
+        n = int(x.numel())
+        pl._check_inputs(x, y, toa, tot, n)
+        n_hits = torch.empty(1, dtype=torch.uint32, device=pl.device) if n_hits is None else n_hits
+        c = clusters._c()
+        info = _CStreamInfo()
+        rc = pl.lib.tpx3_stream_push(self.handle, pl.workspace.data_ptr(), _stream_ptr(stream), n, x.data_ptr(),
+                                     y.data_ptr(), toa.data_ptr(), tot.data_ptr(), 1 if final else 0,
+                                     clusters.max_clusters, ctypes.byref(c), n_hits.data_ptr(), ctypes.byref(info))
+        d = {k: int(getattr(info, k)) for k, _ in _CStreamInfo._fields_}
+        if rc != OK:
+            e = Tpx3Error(rc, "tpx3_stream_push")
+            e.info = d
+            raise e
+        return n_hits, d
+
+    def close(self):
+        if self.handle:
+            self.plan.lib.tpx3_stream_close(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def plan(cfg: Config) -> Plan:

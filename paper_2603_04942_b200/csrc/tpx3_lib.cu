@@ -14,6 +14,7 @@
 #include "tpx3_localmax.cuh"
 #include "tpx3_preprocess.cuh"
 #include "tpx3_sort.cuh"
+#include "tpx3_stream.cuh"
 #include "tpx3_unwrap.cuh"
 
 using namespace tpx3;
@@ -545,6 +546,120 @@ int tpx3_preprocess(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t 
   TPX3_LAUNCH(p, k_pre_scan, 1, 1024, 0, st, a);
   if (a.nblk) TPX3_LAUNCH(p, k_pre_scatter, a.nblk, kPreThreads, 0, st, a);
   return cuda_ok(cudaGetLastError());
+}
+
+// ---- chunked stream (tpx3_stream.cuh) ------------------------------------------------------------
+struct tpx3_stream_s {
+  tpx3_plan_t plan;
+  uint64_t max_chunk, max_carry, disorder;
+  uint32_t n_carry;          // host mirror of the device counter
+  int bank;                  // which carry bank holds the carried events
+  bool failed;
+  tpx3::StreamCtrl* ctrl;
+  uint16_t *cx[2], *cy[2], *ctot[2];
+  uint64_t* ctoa[2];
+  uint16_t *wx, *wy, *wtot;
+  uint64_t* wtoa;
+  uint32_t *wperm, *wlabel, *blk_emit, *blk_keep;
+};
+
+namespace {
+struct StreamLayout {
+  size_t ctrl, cx[2], cy[2], ctot[2], ctoa[2], wx, wy, wtot, wtoa, wperm, wlabel, blk_emit, blk_keep, total;
+};
+StreamLayout stream_layout(uint64_t max_chunk, uint64_t max_carry) {
+  StreamLayout l;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes); return r; };
+  const uint64_t m = max_chunk + max_carry;
+  l.ctrl = take(sizeof(tpx3::StreamCtrl));
+  for (int b = 0; b < 2; ++b) {
+    l.cx[b] = take(2 * max_carry); l.cy[b] = take(2 * max_carry); l.ctot[b] = take(2 * max_carry);
+    l.ctoa[b] = take(8 * max_carry);
+  }
+  l.wx = take(2 * m); l.wy = take(2 * m); l.wtot = take(2 * m); l.wtoa = take(8 * m);
+  l.wperm = take(4 * m); l.wlabel = take(4 * m);
+  const size_t nblk = (size_t)((m + tpx3::kStreamTile - 1) / tpx3::kStreamTile) + 1;
+  l.blk_emit = take(4 * nblk); l.blk_keep = take(4 * nblk);
+  l.total = o;
+  return l;
+}
+}  // namespace
+
+size_t tpx3_stream_bytes(uint64_t max_chunk, uint64_t max_carry) { return stream_layout(max_chunk, max_carry).total; }
+
+int tpx3_stream_open(tpx3_plan_t p, void* stream_buf, uint64_t max_chunk, uint64_t max_carry, uint64_t disorder_ticks,
+                     void* cuda_stream, tpx3_stream_t* out) {
+  if (!p || !stream_buf || !out) return TPX3_ERR_INVALID_ARG;
+  if (p->cfg.shot_period_ticks == 0 || max_chunk == 0 || max_carry == 0) return TPX3_ERR_INVALID_ARG;
+  if (max_chunk + max_carry > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
+  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  tpx3_stream_s* s = new (std::nothrow) tpx3_stream_s();
+  if (!s) return TPX3_ERR_CUDA;
+  const StreamLayout l = stream_layout(max_chunk, max_carry);
+  char* b = (char*)stream_buf;
+  s->plan = p; s->max_chunk = max_chunk; s->max_carry = max_carry; s->disorder = disorder_ticks;
+  s->n_carry = 0; s->bank = 0; s->failed = false;
+  s->ctrl = (tpx3::StreamCtrl*)(b + l.ctrl);
+  for (int k = 0; k < 2; ++k) {
+    s->cx[k] = (uint16_t*)(b + l.cx[k]); s->cy[k] = (uint16_t*)(b + l.cy[k]); s->ctot[k] = (uint16_t*)(b + l.ctot[k]);
+    s->ctoa[k] = (uint64_t*)(b + l.ctoa[k]);
+  }
+  s->wx = (uint16_t*)(b + l.wx); s->wy = (uint16_t*)(b + l.wy); s->wtot = (uint16_t*)(b + l.wtot);
+  s->wtoa = (uint64_t*)(b + l.wtoa); s->wperm = (uint32_t*)(b + l.wperm); s->wlabel = (uint32_t*)(b + l.wlabel);
+  s->blk_emit = (uint32_t*)(b + l.blk_emit); s->blk_keep = (uint32_t*)(b + l.blk_keep);
+  TPX3_LAUNCH(p, tpx3::k_stream_open, 1, 256, 0, (cudaStream_t)cuda_stream, s->ctrl);
+  if (cudaGetLastError() != cudaSuccess) { delete s; return TPX3_ERR_CUDA; }
+  *out = s;
+  return TPX3_OK;
+}
+
+int tpx3_stream_push(tpx3_stream_t s, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x,
+                     const uint16_t* y, const uint64_t* toa, const uint16_t* tot, int final_push, uint64_t max_clusters,
+                     const tpx3_clusters_t* out, uint32_t* n_hits, tpx3_stream_info_t* info) {
+  if (!s || !workspace || !out || !n_hits) return TPX3_ERR_INVALID_ARG;
+  if (s->failed) return TPX3_ERR_CAPACITY;
+  if (n > s->max_chunk) return TPX3_ERR_INVALID_ARG;
+  if (n && (!x || !y || !toa || !tot)) return TPX3_ERR_INVALID_ARG;
+  tpx3_plan_t p = s->plan;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  tpx3::StreamArgs a;
+  a.c = s->ctrl; a.n = n; a.n_carry = s->n_carry; a.carry_cap = (uint32_t)s->max_carry;
+  a.x = x; a.y = y; a.tot = tot; a.toa = toa;
+  const int in = s->bank, ob = s->bank ^ 1;
+  a.cx = s->cx[in]; a.cy = s->cy[in]; a.ctot = s->ctot[in]; a.ctoa = s->ctoa[in];
+  a.nx = s->cx[ob]; a.ny = s->cy[ob]; a.ntot = s->ctot[ob]; a.ntoa = s->ctoa[ob];
+  a.wx = s->wx; a.wy = s->wy; a.wtot = s->wtot; a.wtoa = s->wtoa;
+  a.blk_emit = s->blk_emit; a.blk_keep = s->blk_keep;
+  a.nblk = (uint32_t)((n + s->n_carry + tpx3::kStreamTile - 1) / tpx3::kStreamTile);
+  a.P = p->cfg.shot_period_ticks; a.D = s->disorder; a.final_push = final_push ? 1 : 0;
+  TPX3_LAUNCH(p, tpx3::k_stream_cut, 1, 1024, 0, st, a);
+  if (a.nblk) TPX3_LAUNCH(p, tpx3::k_stream_mark, a.nblk, tpx3::kStreamThreads, 0, st, a);
+  TPX3_LAUNCH(p, tpx3::k_stream_scan, 1, 1024, 0, st, a);
+  if (a.nblk) TPX3_LAUNCH(p, tpx3::k_stream_scatter, a.nblk, tpx3::kStreamThreads, 0, st, a);
+  tpx3::StreamCtrl h;
+  if (cudaMemcpyAsync(&h, s->ctrl, sizeof(h), cudaMemcpyDeviceToHost, st) != cudaSuccess) return TPX3_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return TPX3_ERR_CUDA;   // the emit count sizes the clustering call
+  s->bank = ob;
+  s->n_carry = h.n_carry;
+  if (info) {
+    info->n_emitted = h.n_work; info->n_carry = h.n_carry; info->n_late = h.n_late; info->late_total = h.late_total;
+    info->label_base = h.label_base; info->shots_emitted = h.final_push ? h.s_emitted : h.s_cut;
+  }
+  if (h.overflow) { s->failed = true; return TPX3_ERR_CAPACITY; }
+  int rc = tpx3_cluster_centroid(p, workspace, cuda_stream, h.n_work, s->wx, s->wy, s->wtoa, s->wtot, s->wperm,
+                                 s->wlabel, max_clusters, out, n_hits);
+  if (rc != TPX3_OK) return rc;
+  if (h.n_work && max_clusters)
+    TPX3_LAUNCH(p, tpx3::k_stream_labels, 148, 256, 0, st, s->ctrl, n_hits, max_clusters, out->label);
+  return cuda_ok(cudaGetLastError());
+}
+
+int tpx3_stream_close(tpx3_stream_t s) {
+  if (!s) return TPX3_ERR_INVALID_ARG;
+  delete s;
+  return TPX3_OK;
 }
 
 size_t tpx3_host_io_bytes(uint64_t n, uint64_t max_clusters) {

@@ -1,0 +1,199 @@
+// Chunked stream with cuts that are not shot-aligned (last clause; R24).
+//
+// "Each pixel [is] associated with the most recent laser trigger" and no hit crosses a shot
+// (R6), so a chunk of an endless stream may be cut anywhere as long as every shot is clustered in ONE piece.
+// One push of a chunk:
+//   k_stream_cut      t_max = max(t_max, ToA of the last 65536 events of the chunk); with the stream's
+//                     disorder bound D (pixels report out of order) every shot below
+//                     s_cut = max(s_emitted, (t_max - D) div P) is complete
+//   k_stream_mark     working set = carried events ++ chunk (stream order); per block of 4096 the number of
+//                     events to emit (s_emitted <= shot < s_cut) and to carry (shot >= s_cut); the rest is late
+//   k_stream_scan     exclusive scans of both counts (one block), totals and the new stream state
+//   k_stream_scatter  order-preserving compaction into the emit arrays and the new carry arrays
+//   (host)            reads the two counts, then runs tpx3_cluster_centroid on the emit arrays
+//   k_stream_labels   label += events emitted by earlier pushes: rows continue the batch numbering
+// Shots are compared as times (t_lo = s_emitted * P <= ToA < t_cut = s_cut * P): no division per event.
+#pragma once
+#include "tpx3_centroid.cuh"
+#include "tpx3_common.cuh"
+
+namespace tpx3 {
+
+constexpr int kStreamThreads = 256;
+constexpr int kStreamItems = 16;
+constexpr int kStreamTile = kStreamThreads * kStreamItems;   // 4096 events per block
+constexpr uint32_t kStreamSample = 65536;                    // chunk tail that feeds the running maximum
+
+struct StreamCtrl {
+  uint64_t t_max;        // running maximum (a lower bound of the largest ToA seen)
+  uint64_t s_emitted;    // every shot below went out
+  uint64_t s_cut;        // this push
+  uint64_t t_lo, t_cut;  // s_emitted * P, s_cut * P
+  uint64_t label_base;   // events emitted by earlier pushes
+  uint64_t late_total;
+  uint32_t n_work, n_carry, n_late, overflow;
+  uint32_t final_push, pad;
+};
+
+struct StreamArgs {
+  StreamCtrl* c;
+  uint64_t n;            // chunk
+  uint32_t n_carry;      // carried in (host mirror of c->n_carry)
+  uint32_t carry_cap;
+  const uint16_t *x, *y, *tot;      // chunk
+  const uint64_t* toa;
+  const uint16_t *cx, *cy, *ctot;   // carried in
+  const uint64_t* ctoa;
+  uint16_t *nx, *ny, *ntot;         // carried out
+  uint64_t* ntoa;
+  uint16_t *wx, *wy, *wtot;         // emitted
+  uint64_t* wtoa;
+  uint32_t *blk_emit, *blk_keep;
+  uint32_t nblk;
+  uint64_t P, D;
+  int final_push;
+};
+
+__global__ void __launch_bounds__(256) k_stream_open(StreamCtrl* c) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) {
+    c->t_max = 0; c->s_emitted = 0; c->s_cut = 0; c->t_lo = 0; c->t_cut = 0; c->label_base = 0; c->late_total = 0;
+    c->n_work = 0; c->n_carry = 0; c->n_late = 0; c->overflow = 0; c->final_push = 0; c->pad = 0;
+  }
+}
+
+__global__ void __launch_bounds__(1024) k_stream_cut(StreamArgs a) {
+  __shared__ unsigned long long s_max[32];
+  const uint64_t m = a.n < kStreamSample ? a.n : kStreamSample;
+  const uint64_t beg = a.n - m;
+  unsigned long long v = 0;
+  for (uint64_t i = threadIdx.x; i < m; i += 1024) {
+    const unsigned long long t = a.toa[beg + i];
+    v = t > v ? t : v;
+  }
+  for (int o = 16; o; o >>= 1) {
+    const unsigned long long t = __shfl_xor_sync(0xffffffffu, v, o);
+    v = t > v ? t : v;
+  }
+  if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = v;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    StreamCtrl* c = a.c;
+    for (int w = 0; w < 32; ++w) v = s_max[w] > v ? s_max[w] : v;
+    const uint64_t t_max = c->t_max > v ? c->t_max : v;
+    uint64_t s_cut = t_max >= a.D ? (t_max - a.D) / a.P : 0ull;
+    if (s_cut < c->s_emitted) s_cut = c->s_emitted;
+    c->t_max = t_max;
+    c->s_cut = s_cut;
+    c->t_lo = c->s_emitted * a.P;
+    c->t_cut = s_cut * a.P;
+    c->label_base += c->n_work;     // what the previous push emitted
+    c->n_work = 0;
+    c->final_push = (uint32_t)a.final_push;
+  }
+}
+
+// 0 = late, 1 = emit, 2 = carry
+__device__ __forceinline__ uint32_t stream_class(uint64_t t, uint64_t t_lo, uint64_t t_cut, int final_push) {
+  if (t < t_lo) return 0u;
+  return (final_push || t < t_cut) ? 1u : 2u;
+}
+
+__device__ __forceinline__ uint64_t stream_toa(const StreamArgs& a, uint64_t v) {
+  return v < a.n_carry ? a.ctoa[v] : a.toa[v - a.n_carry];
+}
+
+__global__ void __launch_bounds__(kStreamThreads) k_stream_mark(StreamArgs a) {
+  __shared__ uint32_t s_cnt[2];
+  if (threadIdx.x < 2) s_cnt[threadIdx.x] = 0;
+  __syncthreads();
+  const uint64_t t_lo = a.c->t_lo, t_cut = a.c->t_cut, nv = a.n + a.n_carry;
+  const uint64_t base = (uint64_t)blockIdx.x * kStreamTile;
+  uint32_t e = 0, k = 0;
+#pragma unroll 4
+  for (int i = 0; i < kStreamItems; ++i) {
+    const uint64_t v = base + (uint64_t)i * kStreamThreads + threadIdx.x;
+    if (v < nv) {
+      const uint32_t cl = stream_class(stream_toa(a, v), t_lo, t_cut, a.final_push);
+      e += cl == 1u;
+      k += cl == 2u;
+    }
+  }
+  e = __reduce_add_sync(0xffffffffu, e);
+  k = __reduce_add_sync(0xffffffffu, k);
+  if ((threadIdx.x & 31) == 0) {
+    if (e) atomicAdd(&s_cnt[0], e);
+    if (k) atomicAdd(&s_cnt[1], k);
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    a.blk_emit[blockIdx.x] = s_cnt[0];
+    a.blk_keep[blockIdx.x] = s_cnt[1];
+  }
+}
+
+__global__ void __launch_bounds__(1024) k_stream_scan(StreamArgs a) {
+  const uint32_t e = scan_inplace_1024(a.blk_emit, a.nblk);
+  __syncthreads();
+  const uint32_t k = scan_inplace_1024(a.blk_keep, a.nblk);
+  if (threadIdx.x == 0) {
+    StreamCtrl* c = a.c;
+    const uint64_t nv = a.n + a.n_carry;
+    c->n_work = e;
+    c->n_carry = k > a.carry_cap ? a.carry_cap : k;
+    c->overflow = k > a.carry_cap ? 1u : 0u;       // sticky only for this push: the host turns it into an error
+    c->n_late = (uint32_t)(nv - e - k);
+    c->late_total += nv - e - k;
+    if (!a.final_push) c->s_emitted = c->s_cut;
+  }
+}
+
+__global__ void __launch_bounds__(kStreamThreads) k_stream_scatter(StreamArgs a) {
+  __shared__ uint32_t sm[33];
+  const uint64_t t_lo = a.c->t_lo, t_cut = a.c->t_cut, nv = a.n + a.n_carry;
+  // blocked arrangement: a thread owns 16 consecutive events, so ranks follow the stream order
+  const uint64_t base = (uint64_t)blockIdx.x * kStreamTile + (uint64_t)threadIdx.x * kStreamItems;
+  uint64_t t[kStreamItems];
+  uint32_t cls = 0, e = 0, k = 0;
+#pragma unroll
+  for (int i = 0; i < kStreamItems; ++i) {
+    const uint64_t v = base + i;
+    uint32_t cl = 0;
+    t[i] = 0;
+    if (v < nv) {
+      t[i] = stream_toa(a, v);
+      cl = stream_class(t[i], t_lo, t_cut, a.final_push);
+    }
+    cls |= cl << (2 * i);
+    e += cl == 1u;
+    k += cl == 2u;
+  }
+  uint32_t eo = block_exclusive_scan_256(e, sm, nullptr) + a.blk_emit[blockIdx.x];
+  uint32_t ko = block_exclusive_scan_256(k, sm, nullptr) + a.blk_keep[blockIdx.x];
+#pragma unroll
+  for (int i = 0; i < kStreamItems; ++i) {
+    const uint32_t cl = (cls >> (2 * i)) & 3u;
+    if (cl == 0u) continue;
+    const uint64_t v = base + i;
+    uint16_t ex, ey, et;
+    if (v < a.n_carry) { ex = a.cx[v]; ey = a.cy[v]; et = a.ctot[v]; }
+    else { const uint64_t j = v - a.n_carry; ex = a.x[j]; ey = a.y[j]; et = a.tot[j]; }
+    if (cl == 1u) {
+      a.wx[eo] = ex; a.wy[eo] = ey; a.wtot[eo] = et; a.wtoa[eo] = t[i];
+      ++eo;
+    } else {
+      if (ko < a.carry_cap) { a.nx[ko] = ex; a.ny[ko] = ey; a.ntot[ko] = et; a.ntoa[ko] = t[i]; }
+      ++ko;
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256) k_stream_labels(const StreamCtrl* c, const uint32_t* n_hits,
+                                                     uint64_t max_clusters, uint32_t* label) {
+  uint64_t nc = *n_hits;
+  if (nc > max_clusters) nc = max_clusters;
+  const uint32_t base = (uint32_t)c->label_base;
+  for (uint64_t h = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; h < nc; h += (uint64_t)gridDim.x * blockDim.x)
+    label[h] += base;
+}
+
+}  // namespace tpx3

@@ -731,3 +731,170 @@ def test_time_cluster_hint_never_changes_results(tpx3):
         g.update(cl.numpy(ncl))
         assert_parity(g, o, name)
     pl.free()
+
+
+# ------------------------------------------------------------------ chunked stream, cuts not shot-aligned (NEXT #3)
+from oracle import preprocess as opp  # noqa: E402
+
+_ROW_KEYS = ("c_label", "c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_sum_tot_tof",
+             "c_toa_peak", "c_cx", "c_cy", "c_ctof")
+
+
+def _disorder(toa):
+    t = np.asarray(toa).astype(np.int64)
+    return int(np.max(np.maximum.accumulate(t) - t)) if len(t) else 0
+
+
+def run_stream(m, w, sizes, D, max_carry, max_shot_hits=0, cap=None, final_empty=False):
+    """Push w in chunks of the given sizes through tpx3_stream_push; returns the concatenated hit rows,
+    the per-push info and the StreamModel's per-push (n_emitted, n_carry, n_late) for the same chunks."""
+    import torch
+
+    max_chunk = max(max(sizes), 1)
+    pl = m.plan(m.Config(toa_window_ticks=W, shot_period_ticks=P, max_hits=max_chunk + max_carry,
+                         max_shot_hits=max_shot_hits))
+    s = pl.stream_open(max_chunk, max_carry, D)
+    cl = m.Clusters(cap or (max_chunk + max_carry), pl.device)
+    dx, dy, dt, do = to_dev(w.x), to_dev(w.y), to_dev(w.toa), to_dev(w.tot)
+    model = opp.StreamModel(P, D)
+    rows = {k: [] for k in _ROW_KEYS}
+    infos, want = [], []
+    i = 0
+    pushes = [(sz, False) for sz in sizes]
+    if final_empty:
+        pushes.append((0, True))
+    else:
+        pushes[-1] = (pushes[-1][0], True)
+    for sz, fin in pushes:
+        nh, info = s.push(dx[i:i + sz], dy[i:i + sz], dt[i:i + sz], do[i:i + sz], cl, final=fin)
+        e = model.push(w.x[i:i + sz], w.y[i:i + sz], w.toa[i:i + sz], w.tot[i:i + sz], final=fin)
+        i += sz
+        torch.cuda.synchronize()
+        assert pl.status()["error"] == 0
+        k = int(nh.cpu().numpy()[0])
+        got = cl.numpy(k)
+        for key in _ROW_KEYS:
+            rows[key].append(got[key].copy())
+        infos.append(info)
+        want.append((len(e["x"]), e["n_carry"], e["n_late"], e["label_base"]))
+    s.close()
+    pl.free()
+    return {k: np.concatenate(v) for k, v in rows.items()}, infos, want
+
+
+def _sizes(n, chunk):
+    return [chunk] * (n // chunk) + ([n % chunk] if n % chunk else [])
+
+
+@pytest.mark.parametrize("cfg,shots,chunk", [(0, 1000, 997), (0, 300, 64), (1, 60, 100003), (1, 60, 1 << 20),
+                                             (2, 8, 250007), (3, 40, 30011), (4, 1200, 65536), (4, 1200, 300001),
+                                             (4, 1200, 1 << 22)])
+def test_stream_equals_batch(tpx3, cfg, shots, chunk):
+    """Chunks cut anywhere (inside shots and hits): the rows of all pushes, in order, are the oracle's rows for
+    the whole stream, every column bit for bit; per push the emitted / carried / late counts are the model's."""
+    w = gen.generate(cfg, shots=shots)
+    D = _disorder(w.toa)
+    assert (D > 0) == (cfg == 4)
+    per_shot = int(np.bincount((w.toa // np.uint64(P)).astype(np.int64) - int(w.toa.min() // P)).max())
+    rows, infos, want = run_stream(tpx3, w, _sizes(w.n, chunk), D, max_carry=4 * per_shot + 16)
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P, threads=0)
+    for k in _ROW_KEYS:
+        np.testing.assert_array_equal(rows[k], o[k], err_msg=k)
+    for info, (ne, nk, nl, lb) in zip(infos, want):
+        assert (info["n_emitted"], info["n_carry"], info["n_late"], info["label_base"]) == (ne, nk, nl, lb)
+    assert infos[-1]["late_total"] == 0 and infos[-1]["n_carry"] == 0
+    if chunk < w.n:
+        assert max(i["n_carry"] for i in infos) > 0       # the cuts were not shot-aligned
+
+
+def test_stream_random_chunks_and_empty_pushes(tpx3):
+    w = gen.generate(1, shots=40)
+    rng = np.random.default_rng(11)
+    sizes = []
+    while sum(sizes) < w.n:
+        sizes.append(int(min(rng.choice([0, 1, 17, 5000, 70000, 200000]), w.n - sum(sizes))))
+    rows, infos, want = run_stream(tpx3, w, sizes, 0, max_carry=200000, final_empty=True)
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P, threads=0)
+    for k in _ROW_KEYS:
+        np.testing.assert_array_equal(rows[k], o[k], err_msg=k)
+    assert [(i["n_emitted"], i["n_carry"], i["n_late"]) for i in infos] == [t[:3] for t in want]
+
+
+@pytest.mark.parametrize("cfg,shots,chunk,hint", [(1, None, 4000037, 1024), (4, 24000, (1 << 22) + 12345, 1536)])
+def test_stream_full_size(tpx3, cfg, shots, chunk, hint):
+    """configs[1] whole (3.6e7 hits) and a 1.7e7-hit stretch of configs[4], pushed in chunks of about 2^22
+    events cut anywhere: all rows against the oracle's for the whole stream."""
+    w = gen.generate(cfg, shots=shots) if shots else gen.generate(cfg)
+    D = _disorder(w.toa)
+    import torch
+
+    pl = tpx3.plan(tpx3.Config(toa_window_ticks=W, shot_period_ticks=P, max_hits=chunk + (1 << 18), max_shot_hits=hint))
+    s = pl.stream_open(chunk, 1 << 18, D)
+    cl = tpx3.Clusters(chunk + (1 << 18), pl.device)
+    dx, dy, dt, do = to_dev(w.x), to_dev(w.y), to_dev(w.toa), to_dev(w.tot)
+    rows = {k: [] for k in _ROW_KEYS}
+    sizes = _sizes(w.n, chunk)
+    i = emitted = 0
+    for j, sz in enumerate(sizes):
+        nh, info = s.push(dx[i:i + sz], dy[i:i + sz], dt[i:i + sz], do[i:i + sz], cl, final=(j == len(sizes) - 1))
+        i += sz
+        torch.cuda.synchronize()
+        st = pl.status()
+        assert st["error"] == 0 and st["path"] == 1 and info["n_late"] == 0 and info["label_base"] == emitted
+        emitted += info["n_emitted"]
+        got = cl.numpy(int(nh.cpu().numpy()[0]))
+        for k in _ROW_KEYS:
+            rows[k].append(got[k].copy())
+    assert emitted == w.n
+    s.close()
+    pl.free()
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P, threads=0)
+    for k in _ROW_KEYS:
+        np.testing.assert_array_equal(np.concatenate(rows[k]), o[k], err_msg=k)
+
+
+def test_stream_late_events_are_dropped_and_counted(tpx3):
+    """A stream that breaks its promise (D = 0, but the pixels of some shots arrive three shots later): those are
+    late. The rows are then the oracle's rows of what the model emitted (not the batch result), and the counts
+    match the model."""
+    import types
+
+    w0 = gen.generate(0, shots=400)
+    shot = (w0.toa // np.uint64(P)).astype(np.int64)
+    shot -= shot.min()
+    moved = (shot % 50 == 7) & (np.arange(w0.n) % 3 == 0)
+    key = np.where(moved, shot + 3, shot) * 4 + moved           # stable: behind the events of shot + 3
+    order = np.argsort(key, kind="stable")
+    w = types.SimpleNamespace(x=w0.x[order], y=w0.y[order], toa=w0.toa[order], tot=w0.tot[order], n=w0.n)
+    sizes = _sizes(w.n, 1013)
+    rows, infos, want = run_stream(tpx3, w, sizes, 0, max_carry=1 << 20)
+    assert infos[-1]["late_total"] > 0
+    assert [(i["n_emitted"], i["n_carry"], i["n_late"]) for i in infos] == [t[:3] for t in want]
+    model = opp.StreamModel(P, 0)
+    i, exp = 0, {k: [] for k in _ROW_KEYS}
+    for j, sz in enumerate(sizes):
+        e = model.push(w.x[i:i + sz], w.y[i:i + sz], w.toa[i:i + sz], w.tot[i:i + sz], final=(j == len(sizes) - 1))
+        i += sz
+        r = oracle.run(e["x"], e["y"], e["toa"], e["tot"], W, P, threads=0)
+        for k in _ROW_KEYS:
+            exp[k].append(r[k] + np.uint32(e["label_base"]) if k == "c_label" else r[k])
+    for k in _ROW_KEYS:
+        np.testing.assert_array_equal(rows[k], np.concatenate(exp[k]), err_msg=k)
+
+
+def test_stream_carry_overflow_is_an_error(tpx3):
+    w = gen.generate(1, shots=50)
+    with pytest.raises(tpx3.Tpx3Error) as ei:
+        run_stream(tpx3, w, _sizes(w.n, 4000), 0, max_carry=8)
+    assert ei.value.code == tpx3.ERR_CAPACITY
+
+
+def test_stream_rejects_bad_arguments(tpx3):
+    pl = tpx3.plan(tpx3.Config(toa_window_ticks=W, shot_period_ticks=P, max_hits=1000))
+    with pytest.raises(tpx3.Tpx3Error):
+        pl.stream_open(900, 200, 0)               # max_chunk + max_carry > max_hits
+    pl.free()
+    pl0 = tpx3.plan(tpx3.Config(toa_window_ticks=W, shot_period_ticks=0, max_hits=1000))
+    with pytest.raises(tpx3.Tpx3Error):
+        pl0.stream_open(500, 200, 0)              # no shot period: nothing is ever complete
+    pl0.free()
