@@ -416,6 +416,93 @@ def run_ours(args):
     return 0
 
 
+def run_stream(args):
+    """--mode stream: one step = the whole workload pushed through tpx3_stream_push in chunks of --chunk events
+    cut anywhere (SURVEY.md 8f NEXT #3, last clause). Single GPU; a secondary bench line (no cpu_baseline)."""
+    import numpy as np
+    import torch
+
+    import paper_2603_04942_b200 as m
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    m.load_library()
+    w = make_workload(args.workload, args.shots, 0)
+    n, chunk, carry = w.n, args.chunk, args.max_carry
+    t = w.toa.astype(np.int64)
+    D = int(np.max(np.maximum.accumulate(t) - t)) if n else 0
+    cfg = m.Config(max_hits=chunk + carry, toa_window_ticks=w.toa_window_ticks, shot_period_ticks=w.shot_period_ticks,
+                   max_shot_hits=(args.max_shot_hits if args.max_shot_hits is not None
+                                  else __import__("gen").max_shot_hits(w.cfg_id)))
+    pl = m.plan(cfg)
+    stream = torch.cuda.Stream(device=0)
+    dev = [torch.from_numpy(a).cuda() for a in (w.x, w.y, w.toa, w.tot)]
+    cl = m.Clusters(max((chunk + carry) // 2, 1024), pl.device)
+    nc = torch.zeros(1, dtype=torch.uint32, device=pl.device)
+    cuts = list(range(0, n, chunk)) + [n]
+    torch.cuda.synchronize()
+
+    def step(count=False):
+        s = pl.stream_open(chunk, carry, D, stream=stream)
+        hits = emitted = late = max_carry_seen = 0
+        for a, b in zip(cuts[:-1], cuts[1:]):
+            _, info = s.push(*(d[a:b] for d in dev), cl, final=(b == n), n_hits=nc, stream=stream)
+            emitted += info["n_emitted"]
+            late += info["n_late"]
+            max_carry_seen = max(max_carry_seen, info["n_carry"])
+            if count:
+                stream.synchronize()
+                hits += int(nc.cpu().numpy()[0])
+        s.close()
+        return hits, emitted, late, max_carry_seen
+
+    for _ in range(max(args.warmup, 1)):
+        ncl, emitted, late, carried = step(count=True)
+    assert emitted == n and late == 0, (emitted, n, late)
+    st = pl.status(stream)
+    if st["error"]:
+        raise RuntimeError("device status error %d" % st["error"])
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.3)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    l0 = pl.launch_count()
+    t_wall0 = time.time()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    launches = pl.launch_count() - l0
+    ms_step = ev0.elapsed_time(ev1) / max(args.steps, 1)
+    sampler.stop()
+    peak, peak_src = measured_peak()
+    # the stream layer reads ToA twice (sample + mark: 8 B, scatter: 8 B) and moves every event once (6 + 14 B)
+    bytes_step = STAGE_BYTES["fused"](n, ncl) + 36 * n
+    line = {
+        "metric": METRIC, "value": n / (ms_step * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int64", "data": "synthetic",
+        "config": {"workload": w.name, "mode": "chunked stream, cuts not shot-aligned (tpx3_stream_push)",
+                   "chunk_events": chunk, "pushes_per_step": len(cuts) - 1, "max_carry": carry,
+                   "largest_carry_seen": carried, "disorder_ticks": D, "pixel_hits_per_gpu": n,
+                   "particle_hits_per_gpu": ncl, "max_shot_hits": cfg.max_shot_hits,
+                   "path": {1: "fused", 2: "general"}.get(st["path"], st["path"])},
+        "particle_hits_per_s": ncl / (ms_step * 1e-3),
+        "gpu_launches": launches,
+        "roofline": {"bound": "hbm", "kernel": "whole push: stream split (3 kernels) + fused stage", "achieved":
+                     bytes_step / (ms_step * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                     "frac": bytes_step / (ms_step * 1e-3) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
+                     "algorithmic_bytes_per_step": bytes_step},
+        "clocks": sampler.summary(t_wall0, time.time()),
+    }
+    print(json.dumps(line), flush=True)
+    pl.free()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -427,7 +514,9 @@ def main():
     ap.add_argument("--force-general", action="store_true", help="never take the fused shot-tile path")
     ap.add_argument("--max-shot-hits", type=int, default=None,
                     help="tile-size hint for the plan (default: the workload recipe's bound on hits per shot)")
-    ap.add_argument("--mode", choices=("components", "localmax"), default="components",
+    ap.add_argument("--chunk", type=int, default=1 << 22, help="--mode stream: events per push")
+    ap.add_argument("--max-carry", type=int, default=1 << 20, help="--mode stream: carry capacity in events")
+    ap.add_argument("--mode", choices=("components", "localmax", "stream"), default="components",
                     help="components: the hot path (default). localmax: the paper-literal mode, SURVEY 8f NEXT #2")
     ap.add_argument("--window", type=int, nargs=3, default=(2, 2, 320), metavar=("WX", "WY", "WT"),
                     help="box half-widths of --mode localmax (pixels, pixels, ticks)")
@@ -436,7 +525,9 @@ def main():
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print("note: timing rules ask for >= 3 warm-up steps", file=sys.stderr)
-    return run_reference(args) if args.impl == "reference" else run_ours(args)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_stream(args) if args.mode == "stream" else run_ours(args)
 
 
 if __name__ == "__main__":

@@ -634,7 +634,7 @@ int tpx3_stream_push(tpx3_stream_t s, void* workspace, void* cuda_stream, uint64
   a.blk_emit = s->blk_emit; a.blk_keep = s->blk_keep;
   a.nblk = (uint32_t)((n + s->n_carry + tpx3::kStreamTile - 1) / tpx3::kStreamTile);
   a.P = p->cfg.shot_period_ticks; a.D = s->disorder; a.final_push = final_push ? 1 : 0;
-  TPX3_LAUNCH(p, tpx3::k_stream_cut, 1, 1024, 0, st, a);
+  if (n) TPX3_LAUNCH(p, tpx3::k_stream_cut, 64, 256, 0, st, a);
   if (a.nblk) TPX3_LAUNCH(p, tpx3::k_stream_mark, a.nblk, tpx3::kStreamThreads, 0, st, a);
   TPX3_LAUNCH(p, tpx3::k_stream_scan, 1, 1024, 0, st, a);
   if (a.nblk) TPX3_LAUNCH(p, tpx3::k_stream_scatter, a.nblk, tpx3::kStreamThreads, 0, st, a);

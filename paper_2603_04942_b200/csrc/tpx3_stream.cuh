@@ -3,9 +3,9 @@
 // "Each pixel [is] associated with the most recent laser trigger" and no hit crosses a shot
 // (R6), so a chunk of an endless stream may be cut anywhere as long as every shot is clustered in ONE piece.
 // One push of a chunk:
-//   k_stream_cut      t_max = max(t_max, ToA of the last 65536 events of the chunk); with the stream's
-//                     disorder bound D (pixels report out of order) every shot below
-//                     s_cut = max(s_emitted, (t_max - D) div P) is complete
+//   k_stream_cut      t_max = max(t_max, ToA of the last 65536 events of the chunk) (atomicMax per block); with
+//                     the stream's disorder bound D (pixels report out of order) every shot
+//                     below s_cut = max(s_emitted, (t_max - D) div P) is complete (stream_cut, per block)
 //   k_stream_mark     working set = carried events ++ chunk (stream order); per block of 4096 the number of
 //                     events to emit (s_emitted <= shot < s_cut) and to carry (shot >= s_cut); the rest is late
 //   k_stream_scan     exclusive scans of both counts (one block), totals and the new stream state
@@ -30,6 +30,7 @@ struct StreamCtrl {
   uint64_t s_cut;        // this push
   uint64_t t_lo, t_cut;  // s_emitted * P, s_cut * P
   uint64_t label_base;   // events emitted by earlier pushes
+  uint64_t label_next;   // ... including this one
   uint64_t late_total;
   uint32_t n_work, n_carry, n_late, overflow;
   uint32_t final_push, pad;
@@ -56,17 +57,17 @@ struct StreamArgs {
 
 __global__ void __launch_bounds__(256) k_stream_open(StreamCtrl* c) {
   if (threadIdx.x == 0 && blockIdx.x == 0) {
-    c->t_max = 0; c->s_emitted = 0; c->s_cut = 0; c->t_lo = 0; c->t_cut = 0; c->label_base = 0; c->late_total = 0;
+    c->t_max = 0; c->s_emitted = 0; c->s_cut = 0; c->t_lo = 0; c->t_cut = 0; c->label_base = 0; c->label_next = 0; c->late_total = 0;
     c->n_work = 0; c->n_carry = 0; c->n_late = 0; c->overflow = 0; c->final_push = 0; c->pad = 0;
   }
 }
 
-__global__ void __launch_bounds__(1024) k_stream_cut(StreamArgs a) {
-  __shared__ unsigned long long s_max[32];
+// Running maximum over the chunk's last kStreamSample events: 64 blocks, one atomicMax each.
+__global__ void __launch_bounds__(256) k_stream_cut(StreamArgs a) {
   const uint64_t m = a.n < kStreamSample ? a.n : kStreamSample;
   const uint64_t beg = a.n - m;
   unsigned long long v = 0;
-  for (uint64_t i = threadIdx.x; i < m; i += 1024) {
+  for (uint64_t i = (uint64_t)blockIdx.x * 256 + threadIdx.x; i < m; i += (uint64_t)gridDim.x * 256) {
     const unsigned long long t = a.toa[beg + i];
     v = t > v ? t : v;
   }
@@ -74,21 +75,19 @@ __global__ void __launch_bounds__(1024) k_stream_cut(StreamArgs a) {
     const unsigned long long t = __shfl_xor_sync(0xffffffffu, v, o);
     v = t > v ? t : v;
   }
-  if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = v;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    StreamCtrl* c = a.c;
-    for (int w = 0; w < 32; ++w) v = s_max[w] > v ? s_max[w] : v;
-    const uint64_t t_max = c->t_max > v ? c->t_max : v;
-    uint64_t s_cut = t_max >= a.D ? (t_max - a.D) / a.P : 0ull;
-    if (s_cut < c->s_emitted) s_cut = c->s_emitted;
-    c->t_max = t_max;
-    c->s_cut = s_cut;
-    c->t_lo = c->s_emitted * a.P;
-    c->t_cut = s_cut * a.P;
-    c->label_base += c->n_work;     // what the previous push emitted
-    c->n_work = 0;
-    c->final_push = (uint32_t)a.final_push;
+  if ((threadIdx.x & 31) == 0 && v) atomicMax(reinterpret_cast<unsigned long long*>(&a.c->t_max), v);
+}
+
+// Every block derives the cut of this push from the state (unchanged until k_stream_scan); block 0 records it.
+__device__ __forceinline__ void stream_cut(const StreamArgs& a, uint64_t& t_lo, uint64_t& t_cut) {
+  const StreamCtrl* c = a.c;
+  const uint64_t t_max = c->t_max, s_emitted = c->s_emitted;
+  uint64_t s_cut = t_max >= a.D ? (t_max - a.D) / a.P : 0ull;
+  if (s_cut < s_emitted) s_cut = s_emitted;
+  t_lo = s_emitted * a.P;
+  t_cut = s_cut * a.P;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    a.c->s_cut = s_cut; a.c->t_lo = t_lo; a.c->t_cut = t_cut; a.c->final_push = (uint32_t)a.final_push;
   }
 }
 
@@ -106,7 +105,9 @@ __global__ void __launch_bounds__(kStreamThreads) k_stream_mark(StreamArgs a) {
   __shared__ uint32_t s_cnt[2];
   if (threadIdx.x < 2) s_cnt[threadIdx.x] = 0;
   __syncthreads();
-  const uint64_t t_lo = a.c->t_lo, t_cut = a.c->t_cut, nv = a.n + a.n_carry;
+  uint64_t t_lo, t_cut;
+  stream_cut(a, t_lo, t_cut);
+  const uint64_t nv = a.n + a.n_carry;
   const uint64_t base = (uint64_t)blockIdx.x * kStreamTile;
   uint32_t e = 0, k = 0;
 #pragma unroll 4
@@ -138,6 +139,12 @@ __global__ void __launch_bounds__(1024) k_stream_scan(StreamArgs a) {
   if (threadIdx.x == 0) {
     StreamCtrl* c = a.c;
     const uint64_t nv = a.n + a.n_carry;
+    if (a.nblk == 0) {   // nothing to mark: record the (unchanged) cut here
+      uint64_t t_lo, t_cut;
+      stream_cut(a, t_lo, t_cut);
+    }
+    c->label_base = c->label_next;
+    c->label_next += e;
     c->n_work = e;
     c->n_carry = k > a.carry_cap ? a.carry_cap : k;
     c->overflow = k > a.carry_cap ? 1u : 0u;       // sticky only for this push: the host turns it into an error
@@ -148,41 +155,63 @@ __global__ void __launch_bounds__(1024) k_stream_scan(StreamArgs a) {
 }
 
 __global__ void __launch_bounds__(kStreamThreads) k_stream_scatter(StreamArgs a) {
+  __shared__ __align__(16) uint8_t s_cls[kStreamTile];
+  __shared__ uint16_t s_rank[kStreamTile];
   __shared__ uint32_t sm[33];
   const uint64_t t_lo = a.c->t_lo, t_cut = a.c->t_cut, nv = a.n + a.n_carry;
-  // blocked arrangement: a thread owns 16 consecutive events, so ranks follow the stream order
-  const uint64_t base = (uint64_t)blockIdx.x * kStreamTile + (uint64_t)threadIdx.x * kStreamItems;
+  const uint64_t base = (uint64_t)blockIdx.x * kStreamTile;
+  // striped (coalesced) pass: ToA and class of every event
   uint64_t t[kStreamItems];
-  uint32_t cls = 0, e = 0, k = 0;
 #pragma unroll
   for (int i = 0; i < kStreamItems; ++i) {
-    const uint64_t v = base + i;
+    const uint32_t loc = (uint32_t)i * kStreamThreads + threadIdx.x;
+    const uint64_t v = base + loc;
     uint32_t cl = 0;
     t[i] = 0;
     if (v < nv) {
       t[i] = stream_toa(a, v);
       cl = stream_class(t[i], t_lo, t_cut, a.final_push);
     }
-    cls |= cl << (2 * i);
+    s_cls[loc] = (uint8_t)cl;
+  }
+  __syncthreads();
+  // blocked pass over the classes: a thread owns 16 consecutive events, so ranks follow the stream order
+  const uint4 q = *reinterpret_cast<const uint4*>(&s_cls[threadIdx.x * kStreamItems]);
+  const uint32_t qw[4] = {q.x, q.y, q.z, q.w};
+  uint32_t e = 0, k = 0;
+#pragma unroll
+  for (int j = 0; j < kStreamItems; ++j) {
+    const uint32_t cl = (qw[j >> 2] >> (8 * (j & 3))) & 0xFFu;
     e += cl == 1u;
     k += cl == 2u;
   }
-  uint32_t eo = block_exclusive_scan_256(e, sm, nullptr) + a.blk_emit[blockIdx.x];
-  uint32_t ko = block_exclusive_scan_256(k, sm, nullptr) + a.blk_keep[blockIdx.x];
+  uint32_t eo = block_exclusive_scan_256(e, sm, nullptr);
+  uint32_t ko = block_exclusive_scan_256(k, sm, nullptr);
 #pragma unroll
+  for (int j = 0; j < kStreamItems; ++j) {
+    const uint32_t cl = (qw[j >> 2] >> (8 * (j & 3))) & 0xFFu;
+    if (cl == 1u) s_rank[threadIdx.x * kStreamItems + j] = (uint16_t)eo++;
+    else if (cl == 2u) s_rank[threadIdx.x * kStreamItems + j] = (uint16_t)ko++;
+  }
+  __syncthreads();
+  // striped pass again: neighbouring threads hold neighbouring ranks, so the copies are coalesced
+  const uint32_t e_base = a.blk_emit[blockIdx.x], k_base = a.blk_keep[blockIdx.x];
+#pragma unroll 4
   for (int i = 0; i < kStreamItems; ++i) {
-    const uint32_t cl = (cls >> (2 * i)) & 3u;
+    const uint32_t loc = (uint32_t)i * kStreamThreads + threadIdx.x;
+    const uint32_t cl = s_cls[loc];
     if (cl == 0u) continue;
-    const uint64_t v = base + i;
+    const uint64_t v = base + loc;
     uint16_t ex, ey, et;
     if (v < a.n_carry) { ex = a.cx[v]; ey = a.cy[v]; et = a.ctot[v]; }
     else { const uint64_t j = v - a.n_carry; ex = a.x[j]; ey = a.y[j]; et = a.tot[j]; }
+    const uint32_t r = s_rank[loc];
     if (cl == 1u) {
-      a.wx[eo] = ex; a.wy[eo] = ey; a.wtot[eo] = et; a.wtoa[eo] = t[i];
-      ++eo;
+      const uint32_t o = e_base + r;
+      a.wx[o] = ex; a.wy[o] = ey; a.wtot[o] = et; a.wtoa[o] = t[i];
     } else {
-      if (ko < a.carry_cap) { a.nx[ko] = ex; a.ny[ko] = ey; a.ntot[ko] = et; a.ntoa[ko] = t[i]; }
-      ++ko;
+      const uint32_t o = k_base + r;
+      if (o < a.carry_cap) { a.nx[o] = ex; a.ny[o] = ey; a.ntot[o] = et; a.ntoa[o] = t[i]; }
     }
   }
 }
