@@ -398,7 +398,7 @@ def run_ours(args):
         },
         "particle_hits_per_s": ncl_all / (ms_step * 1e-3),
         "e2e": {"value": n_all / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "ms_per_step": e2e_s * 1e3, "api": "tpx3_process_host (pinned host buffers; cluster table copied "
+                "ms_per_step": e2e_s * 1e3, "route": {0: "one piece", 1: "pipelined in 2^22-event chunks", 2: "pipelined attempt redone in one piece"}.get(pl.host_route()) if not lm else None, "api": "tpx3_process_host (pinned host buffers; cluster table copied "
                 "back, perm/label left on the device)" if not lm else "pinned H2D copies + tpx3_localmax_centroid + "
                 "D2H of the count and the hit table"},
         "gpu_launches": launches,

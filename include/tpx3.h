@@ -186,7 +186,13 @@ int tpx3_preprocess(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64
  * tpx3_cluster_centroid and copies perm, label (either may be NULL to skip), the first
  * min(n_clusters, max_clusters) entries of every non-NULL array of `out_host` and the count
  * back, then synchronises the stream. `device_io` is a [dev] staging buffer of at least
- * tpx3_host_io_bytes(n, max_clusters) bytes. Returns the device status error, if any. */
+ * tpx3_host_io_bytes(n, max_clusters) bytes. Returns the device status error, if any.
+ * Calls of n >= 2^23 events that ask for neither perm nor label (shot period > 0, no
+ * TPX3_FLAG_VALIDATE_INPUT) are pipelined: the input goes up in 2^22-event chunks on a copy stream
+ * of the library's own, each chunk is pushed through the stream calls below as it lands (disorder
+ * bound: half a shot period), and the hit rows of a push go back on a second copy stream under
+ * the next chunk's upload. Same rows as the one-piece route; a stream with late events or more
+ * than 2^20 carried events is redone in one piece (tpx3_host_route tells which). */
 size_t tpx3_host_io_bytes(uint64_t n, uint64_t max_clusters);
 int tpx3_process_host(tpx3_plan_t plan, void* workspace, void* device_io, void* cuda_stream,
                       uint64_t n, const uint16_t* x, const uint16_t* y, const uint64_t* toa,
@@ -235,6 +241,11 @@ int tpx3_stream_push(tpx3_stream_t stream, void* workspace, void* cuda_stream, u
                      uint64_t max_clusters, const tpx3_clusters_t* out, uint32_t* n_hits,
                      tpx3_stream_info_t* info);
 int tpx3_stream_close(tpx3_stream_t stream);
+
+/* Which route the last tpx3_process_host call of this plan took: 0 = one piece (copy in, one
+ * clustering call, copy out), 1 = pipelined (see tpx3_process_host), 2 = the pipelined attempt met
+ * late events or a carry overflow and the call was redone in one piece (same results). */
+int tpx3_host_route(tpx3_plan_t plan);
 
 /* Number of kernels the library has launched through this plan (for launch accounting). */
 uint64_t tpx3_launch_count(tpx3_plan_t plan);

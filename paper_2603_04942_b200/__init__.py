@@ -30,7 +30,7 @@ exported_symbols = (
     "tpx3_plan", "tpx3_cluster", "tpx3_centroid", "tpx3_cluster_centroid", "tpx3_localmax_centroid",
     "tpx3_unwrap_toa", "tpx3_timewalk_table", "tpx3_preprocess", "tpx3_host_io_bytes",
     "tpx3_stream_bytes", "tpx3_stream_open", "tpx3_stream_push", "tpx3_stream_close",
-    "tpx3_process_host", "tpx3_status", "tpx3_launch_count", "tpx3_profile_enable", "tpx3_profile_read",
+    "tpx3_process_host", "tpx3_host_route", "tpx3_status", "tpx3_launch_count", "tpx3_profile_enable", "tpx3_profile_read",
     "tpx3_free", "tpx3_strerror",
 )
 STAGES = ("fused", "sort", "link", "centroid")
@@ -115,6 +115,8 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.tpx3_process_host.restype = ctypes.c_int
     lib.tpx3_process_host.argtypes = [vp, vp, vp, vp, u64, vp, vp, vp, vp, vp, vp, u64,
                                       ctypes.POINTER(_CClusters), vp]
+    lib.tpx3_host_route.restype = ctypes.c_int
+    lib.tpx3_host_route.argtypes = [vp]
     lib.tpx3_status.restype = ctypes.c_int
     lib.tpx3_status.argtypes = [vp, vp, vp, ctypes.POINTER(_CStatus)]
     lib.tpx3_launch_count.restype = ctypes.c_uint64
@@ -370,6 +372,9 @@ class Plan:
             raise Tpx3Error(rc, "tpx3_status")
         return {"error": -int(s.error), "path": int(s.path), "n_clusters": int(s.n_clusters),
                 "sort_passes": int(s.sort_passes), "n": int(s.n)}
+
+    def host_route(self) -> int:
+        return int(self.lib.tpx3_host_route(self.handle))
 
     def launch_count(self) -> int:
         return int(self.lib.tpx3_launch_count(self.handle))

@@ -36,6 +36,7 @@ struct tpx3_plan_s {
   std::vector<Span> spans;
   std::vector<cudaEvent_t> free_events;
   uint64_t profiled_calls;
+  int host_route;           // last tpx3_process_host: 0 one piece, 1 pipelined, 2 pipelined attempt redone in one piece
 };
 
 namespace {
@@ -662,28 +663,172 @@ int tpx3_stream_close(tpx3_stream_t s) {
   return TPX3_OK;
 }
 
-size_t tpx3_host_io_bytes(uint64_t n, uint64_t max_clusters) {
-  size_t o = 0;
-  o = align_up(o + 2 * n);        // x
-  o = align_up(o + 2 * n);        // y
-  o = align_up(o + 8 * n);        // toa
-  o = align_up(o + 2 * n);        // tot
-  o = align_up(o + 4 * n);        // perm
-  o = align_up(o + 4 * n);        // label
-  o = align_up(o + 4 * max_clusters) * 1;  // label
-  o = align_up(o + 4 * max_clusters);      // size
-  o = align_up(o + 4 * max_clusters);      // shot
-  o = align_up(o + 8 * max_clusters);      // sum_tot
-  o = align_up(o + 8 * max_clusters);      // sum_tot_x
-  o = align_up(o + 8 * max_clusters);      // sum_tot_y
-  o = align_up(o + 8 * max_clusters);      // toa_peak
-  o = align_up(o + 4 * max_clusters);      // cx
-  o = align_up(o + 4 * max_clusters);      // cy
-  o = align_up(o + 8 * max_clusters);      // sum_tot_tof
-  o = align_up(o + 4 * max_clusters);      // ctof
-  o = align_up(o + 256);                   // n_clusters
-  return o;
+// ---- end to end with host buffers ------------------------------------------------------------------
+namespace {
+// Large calls are pipelined: the input goes up in chunks on a copy stream, every chunk is pushed through the
+// stream calls above as soon as it has landed (cut anywhere: open shots are carried), and the hit rows of
+// push j go back on a second copy stream while chunk j+1 is still on its way up.
+constexpr uint64_t kPipeChunk = 1ull << 22, kPipeCarry = 1ull << 20;
+inline bool pipe_sized(uint64_t n) { return n >= 2 * kPipeChunk; }
+
+struct HostIo {
+  uint16_t *x, *y, *tot;
+  uint64_t* toa;
+  uint32_t *perm, *label, *n;
+  tpx3_clusters_t d;          // the whole table (monolithic path)
+  tpx3_clusters_t bank[2];    // per-push tables (pipelined path)
+  uint32_t* bank_n[2];
+  void* stream_buf;
+  size_t total;
+};
+
+struct Carver {
+  char* b;
+  size_t o;
+  char* operator()(size_t bytes) { char* r = b + o; o = align_up(o + bytes); return r; }
+};
+
+tpx3_clusters_t carve_clusters(Carver& take, uint64_t cap) {
+  tpx3_clusters_t d;
+  d.label = (uint32_t*)take(4 * cap);
+  d.size = (uint32_t*)take(4 * cap);
+  d.shot = (uint32_t*)take(4 * cap);
+  d.sum_tot = (int64_t*)take(8 * cap);
+  d.sum_tot_x = (int64_t*)take(8 * cap);
+  d.sum_tot_y = (int64_t*)take(8 * cap);
+  d.toa_peak = (uint64_t*)take(8 * cap);
+  d.cx = (float*)take(4 * cap);
+  d.cy = (float*)take(4 * cap);
+  d.sum_tot_tof = (int64_t*)take(8 * cap);
+  d.ctof = (float*)take(4 * cap);
+  return d;
 }
+
+HostIo host_io_layout(char* b, uint64_t n, uint64_t max_clusters) {
+  HostIo io;
+  Carver take{b, 0};
+  io.x = (uint16_t*)take(2 * n);
+  io.y = (uint16_t*)take(2 * n);
+  io.toa = (uint64_t*)take(8 * n);
+  io.tot = (uint16_t*)take(2 * n);
+  io.perm = (uint32_t*)take(4 * n);
+  io.label = (uint32_t*)take(4 * n);
+  io.d = carve_clusters(take, max_clusters);
+  io.n = (uint32_t*)take(256);
+  io.stream_buf = nullptr;
+  if (pipe_sized(n)) {
+    for (int k = 0; k < 2; ++k) {
+      io.bank[k] = carve_clusters(take, kPipeChunk + kPipeCarry);
+      io.bank_n[k] = (uint32_t*)take(256);
+    }
+    io.stream_buf = take(tpx3_stream_bytes(kPipeChunk, kPipeCarry));
+  }
+  io.total = take.o;
+  return io;
+}
+
+// D2H of `cnt` rows of table `d` into the host table `h` at row `at` (columns the caller left NULL are skipped).
+cudaError_t copy_rows(const tpx3_clusters_t& h, uint64_t at, const tpx3_clusters_t& d, uint64_t cnt, cudaStream_t st) {
+  cudaError_t e = cudaSuccess;
+  if (!cnt) return e;
+#define TPX3_ROWS(field, bytes)                                                                            \
+  if (e == cudaSuccess && h.field)                                                                          \
+    e = cudaMemcpyAsync(h.field + at, d.field, (bytes) * cnt, cudaMemcpyDeviceToHost, st);
+  TPX3_ROWS(label, 4) TPX3_ROWS(size, 4) TPX3_ROWS(shot, 4) TPX3_ROWS(sum_tot, 8) TPX3_ROWS(sum_tot_x, 8)
+  TPX3_ROWS(sum_tot_y, 8) TPX3_ROWS(toa_peak, 8) TPX3_ROWS(cx, 4) TPX3_ROWS(cy, 4) TPX3_ROWS(sum_tot_tof, 8)
+  TPX3_ROWS(ctof, 4)
+#undef TPX3_ROWS
+  return e;
+}
+
+// Returns TPX3_OK with *fell_back = false when the pipelined run produced the result; *fell_back = true when
+// the stream did not keep its promise (late events, carry overflow): all inputs are on the device by then and
+// the caller runs the monolithic call on them.
+int process_host_pipelined(tpx3_plan_t p, void* workspace, const HostIo& io, cudaStream_t st, uint64_t n,
+                           const uint16_t* x, const uint16_t* y, const uint64_t* toa, const uint16_t* tot,
+                           uint64_t max_clusters, const tpx3_clusters_t* out_host, uint32_t* n_clusters_host,
+                           bool* fell_back) {
+  *fell_back = true;
+  const uint32_t nchunk = (uint32_t)((n + kPipeChunk - 1) / kPipeChunk);
+  cudaStream_t s_in = nullptr, s_out = nullptr;
+  std::vector<cudaEvent_t> ev(3 * (size_t)nchunk + 1, nullptr);   // [0] entry, then in / done / out per chunk
+  std::vector<uint32_t> nh(nchunk, 0);
+  tpx3_stream_t sh = nullptr;
+  int rc = TPX3_ERR_CUDA;
+  bool ok = cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking) == cudaSuccess;
+  for (size_t i = 0; ok && i < ev.size(); ++i) ok = cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming) == cudaSuccess;
+  auto e_in = [&](uint32_t j) { return ev[1 + 3 * (size_t)j]; };
+  auto e_done = [&](uint32_t j) { return ev[2 + 3 * (size_t)j]; };
+  auto e_out = [&](uint32_t j) { return ev[3 + 3 * (size_t)j]; };
+  uint64_t rows = 0, total = 0;
+  bool promise_kept = true;
+  if (ok) {
+    // the copies may not overtake earlier work of the caller's stream on the same buffers
+    ok = cudaEventRecord(ev[0], st) == cudaSuccess && cudaStreamWaitEvent(s_in, ev[0], 0) == cudaSuccess &&
+         cudaStreamWaitEvent(s_out, ev[0], 0) == cudaSuccess;
+    for (uint32_t j = 0; ok && j < nchunk; ++j) {
+      const uint64_t a = (uint64_t)j * kPipeChunk, m = (a + kPipeChunk <= n ? kPipeChunk : n - a);
+      ok = cudaMemcpyAsync(io.toa + a, toa + a, 8 * m, cudaMemcpyHostToDevice, s_in) == cudaSuccess &&
+           cudaMemcpyAsync(io.x + a, x + a, 2 * m, cudaMemcpyHostToDevice, s_in) == cudaSuccess &&
+           cudaMemcpyAsync(io.y + a, y + a, 2 * m, cudaMemcpyHostToDevice, s_in) == cudaSuccess &&
+           cudaMemcpyAsync(io.tot + a, tot + a, 2 * m, cudaMemcpyHostToDevice, s_in) == cudaSuccess &&
+           cudaEventRecord(e_in(j), s_in) == cudaSuccess;
+    }
+  }
+  if (ok) {
+    // D = half a shot period: right for any stream whose pixels arrive less than half a period late; a stream
+    // that is worse shows late events and is redone in one piece
+    rc = tpx3_stream_open(p, io.stream_buf, kPipeChunk, kPipeCarry, p->cfg.shot_period_ticks / 2, st, &sh);
+    ok = rc == TPX3_OK;
+  }
+  auto rows_back = [&](uint32_t j) {   // after the stream has been synchronised past push j's count
+    uint64_t cnt = nh[j];
+    total += cnt;
+    if (rows + cnt > max_clusters) cnt = max_clusters > rows ? max_clusters - rows : 0;
+    bool good = cudaStreamWaitEvent(s_out, e_done(j), 0) == cudaSuccess;
+    if (good && out_host) good = copy_rows(*out_host, rows, io.bank[j & 1], cnt, s_out) == cudaSuccess;
+    rows += cnt;
+    return good && cudaEventRecord(e_out(j), s_out) == cudaSuccess;
+  };
+  for (uint32_t j = 0; ok && promise_kept && j < nchunk; ++j) {
+    const uint64_t a = (uint64_t)j * kPipeChunk, m = (a + kPipeChunk <= n ? kPipeChunk : n - a);
+    ok = cudaStreamWaitEvent(st, e_in(j), 0) == cudaSuccess;
+    if (ok && j >= 2) ok = cudaStreamWaitEvent(st, e_out(j - 2), 0) == cudaSuccess;   // bank j & 1 is free again
+    if (!ok) break;
+    tpx3_stream_info_t info;
+    rc = tpx3_stream_push(sh, workspace, st, m, io.x + a, io.y + a, io.toa + a, io.tot + a, j + 1 == nchunk,
+                          kPipeChunk + kPipeCarry, &io.bank[j & 1], io.bank_n[j & 1], &info);
+    if (rc == TPX3_ERR_CAPACITY || (rc == TPX3_OK && info.late_total)) { promise_kept = false; rc = TPX3_OK; break; }
+    ok = rc == TPX3_OK;
+    if (!ok) break;
+    // the push synchronised the stream behind push j-1's clustering: its count is on the host now
+    if (j >= 1) ok = rows_back(j - 1);
+    ok = ok && cudaMemcpyAsync(&nh[j], io.bank_n[j & 1], 4, cudaMemcpyDeviceToHost, st) == cudaSuccess &&
+         cudaEventRecord(e_done(j), st) == cudaSuccess;
+  }
+  if (ok && promise_kept) {
+    ok = cudaStreamSynchronize(st) == cudaSuccess && rows_back(nchunk - 1) && cudaStreamSynchronize(s_out) == cudaSuccess;
+    if (ok) {
+      *n_clusters_host = (uint32_t)total;
+      *fell_back = false;
+      rc = total > max_clusters ? TPX3_ERR_CAPACITY : TPX3_OK;
+    }
+  }
+  // leave nothing in flight: the fallback (and the caller) reuse the buffers
+  if (s_in) cudaStreamSynchronize(s_in);
+  if (s_out) cudaStreamSynchronize(s_out);
+  cudaStreamSynchronize(st);
+  if (sh) tpx3_stream_close(sh);
+  for (auto e : ev) if (e) cudaEventDestroy(e);
+  if (s_in) cudaStreamDestroy(s_in);
+  if (s_out) cudaStreamDestroy(s_out);
+  if (!ok) return rc != TPX3_OK ? rc : TPX3_ERR_CUDA;
+  return rc;
+}
+}  // namespace
+
+size_t tpx3_host_io_bytes(uint64_t n, uint64_t max_clusters) { return host_io_layout(nullptr, n, max_clusters).total; }
 
 int tpx3_process_host(tpx3_plan_t p, void* workspace, void* device_io, void* cuda_stream, uint64_t n, const uint16_t* x,
                       const uint16_t* y, const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label,
@@ -693,66 +838,44 @@ int tpx3_process_host(tpx3_plan_t p, void* workspace, void* device_io, void* cud
   if (n && (!x || !y || !toa || !tot)) return TPX3_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
-  char* b = (char*)device_io;
-  size_t o = 0;
-  auto take = [&](size_t bytes) { char* r = b + o; o = align_up(o + bytes); return r; };
-  uint16_t* dx = (uint16_t*)take(2 * n);
-  uint16_t* dy = (uint16_t*)take(2 * n);
-  uint64_t* dtoa = (uint64_t*)take(8 * n);
-  uint16_t* dtot = (uint16_t*)take(2 * n);
-  uint32_t* dperm = (uint32_t*)take(4 * n);
-  uint32_t* dlabel = (uint32_t*)take(4 * n);
-  tpx3_clusters_t d;
-  d.label = (uint32_t*)take(4 * max_clusters);
-  d.size = (uint32_t*)take(4 * max_clusters);
-  d.shot = (uint32_t*)take(4 * max_clusters);
-  d.sum_tot = (int64_t*)take(8 * max_clusters);
-  d.sum_tot_x = (int64_t*)take(8 * max_clusters);
-  d.sum_tot_y = (int64_t*)take(8 * max_clusters);
-  d.toa_peak = (uint64_t*)take(8 * max_clusters);
-  d.cx = (float*)take(4 * max_clusters);
-  d.cy = (float*)take(4 * max_clusters);
-  d.sum_tot_tof = (int64_t*)take(8 * max_clusters);
-  d.ctof = (float*)take(4 * max_clusters);
-  uint32_t* dn = (uint32_t*)take(256);
+  const HostIo io = host_io_layout((char*)device_io, n, max_clusters);
   cudaError_t e = cudaSuccess;
-  if (n) {
-    e = cudaMemcpyAsync(dx, x, 2 * n, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(dy, y, 2 * n, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(dtoa, toa, 8 * n, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(dtot, tot, 2 * n, cudaMemcpyHostToDevice, st);
+  bool resident = false;
+  if (pipe_sized(n) && p->cfg.shot_period_ticks && !perm && !label && !(p->cfg.flags & TPX3_FLAG_VALIDATE_INPUT)) {
+    bool fell_back = true;
+    const int rc = process_host_pipelined(p, workspace, io, st, n, x, y, toa, tot, max_clusters, out_host,
+                                          n_clusters_host, &fell_back);
+    p->host_route = fell_back ? 2 : 1;
+    if (!fell_back || (rc != TPX3_OK && rc != TPX3_ERR_CAPACITY)) return rc;
+    resident = true;   // every chunk went up before the stream gave up
+  } else {
+    p->host_route = 0;
+  }
+  if (n && !resident) {
+    e = cudaMemcpyAsync(io.x, x, 2 * n, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(io.y, y, 2 * n, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(io.toa, toa, 8 * n, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(io.tot, tot, 2 * n, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return TPX3_ERR_CUDA;
   }
-  int rc = tpx3_cluster_centroid(p, workspace, cuda_stream, n, dx, dy, dtoa, dtot, dperm, dlabel, max_clusters, &d, dn);
+  int rc = tpx3_cluster_centroid(p, workspace, cuda_stream, n, io.x, io.y, io.toa, io.tot, io.perm, io.label,
+                                 max_clusters, &io.d, io.n);
   if (rc != TPX3_OK) return rc;
-  e = cudaMemcpyAsync(n_clusters_host, dn, 4, cudaMemcpyDeviceToHost, st);
-  if (e == cudaSuccess && perm && n) e = cudaMemcpyAsync(perm, dperm, 4 * n, cudaMemcpyDeviceToHost, st);
-  if (e == cudaSuccess && label && n) e = cudaMemcpyAsync(label, dlabel, 4 * n, cudaMemcpyDeviceToHost, st);
+  e = cudaMemcpyAsync(n_clusters_host, io.n, 4, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && perm && n) e = cudaMemcpyAsync(perm, io.perm, 4 * n, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && label && n) e = cudaMemcpyAsync(label, io.label, 4 * n, cudaMemcpyDeviceToHost, st);
   if (e != cudaSuccess) return TPX3_ERR_CUDA;
   if (cudaStreamSynchronize(st) != cudaSuccess) return TPX3_ERR_CUDA;  // the count decides the copy sizes
   uint64_t nc = *n_clusters_host;
   if (nc > max_clusters) nc = max_clusters;
-  if (out_host && nc) {
-    const tpx3_clusters_t& h = *out_host;
-    if (h.label) e = cudaMemcpyAsync(h.label, d.label, 4 * nc, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && h.size) e = cudaMemcpyAsync(h.size, d.size, 4 * nc, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && h.shot) e = cudaMemcpyAsync(h.shot, d.shot, 4 * nc, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && h.sum_tot) e = cudaMemcpyAsync(h.sum_tot, d.sum_tot, 8 * nc, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && h.sum_tot_x) e = cudaMemcpyAsync(h.sum_tot_x, d.sum_tot_x, 8 * nc, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && h.sum_tot_y) e = cudaMemcpyAsync(h.sum_tot_y, d.sum_tot_y, 8 * nc, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && h.toa_peak) e = cudaMemcpyAsync(h.toa_peak, d.toa_peak, 8 * nc, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && h.cx) e = cudaMemcpyAsync(h.cx, d.cx, 4 * nc, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && h.cy) e = cudaMemcpyAsync(h.cy, d.cy, 4 * nc, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && h.sum_tot_tof)
-      e = cudaMemcpyAsync(h.sum_tot_tof, d.sum_tot_tof, 8 * nc, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && h.ctof) e = cudaMemcpyAsync(h.ctof, d.ctof, 4 * nc, cudaMemcpyDeviceToHost, st);
-    if (e != cudaSuccess) return TPX3_ERR_CUDA;
-  }
+  if (out_host && copy_rows(*out_host, 0, io.d, nc, st) != cudaSuccess) return TPX3_ERR_CUDA;
   tpx3_status_t s;
   rc = tpx3_status(p, workspace, cuda_stream, &s);
   if (rc != TPX3_OK) return rc;
   return s.error ? -(int)s.error : TPX3_OK;
 }
+
+int tpx3_host_route(tpx3_plan_t p) { return p ? p->host_route : TPX3_ERR_INVALID_ARG; }
 
 int tpx3_status(tpx3_plan_t p, const void* workspace, void* cuda_stream, tpx3_status_t* out) {
   if (!p || !workspace || !out) return TPX3_ERR_INVALID_ARG;

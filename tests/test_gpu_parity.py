@@ -898,3 +898,60 @@ def test_stream_rejects_bad_arguments(tpx3):
     with pytest.raises(tpx3.Tpx3Error):
         pl0.stream_open(500, 200, 0)              # no shot period: nothing is ever complete
     pl0.free()
+
+
+@pytest.mark.parametrize("cfg,shots,hint,pipelined", [(1, 24000, 1024, True), (4, 13000, 1536, True), (1, 24000, 1024, False)])
+def test_process_host_pipelined(tpx3, cfg, shots, hint, pipelined):
+    """Calls of >= 2^23 events go up in 2^22-event chunks pushed through the stream calls while later chunks
+    are still being copied (tpx3_process_host): all rows against the oracle. The last case asks for perm and
+    label as well, which takes the one-piece route on the same input: same rows."""
+    import torch
+
+    w = gen.generate(cfg, shots=shots)
+    assert w.n >= 1 << 23
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P, threads=0)
+    pl = tpx3.plan(tpx3.Config(max_hits=w.n, max_shot_hits=hint))
+    hx, hy, htoa, htot = (torch.from_numpy(a).pin_memory() for a in (w.x, w.y, w.toa, w.tot))
+    cap = w.n // 2
+    cl = tpx3.Clusters(cap, "cpu", pin=True)
+    extra = () if pipelined else (torch.empty(w.n, dtype=torch.uint32).pin_memory(),
+                                  torch.empty(w.n, dtype=torch.uint32).pin_memory())
+    for _ in range(2):                      # the second call reuses the device buffers of the first
+        l0 = pl.launch_count()
+        ncl = pl.process_host(hx, hy, htoa, htot, cl, *extra)
+        launches = pl.launch_count() - l0
+        assert ncl == o["n_clusters"]
+        g = cl.numpy(ncl)
+        for k in _ROW_KEYS:
+            np.testing.assert_array_equal(g[k], o[k], err_msg=k)
+        assert pl.host_route() == (1 if pipelined else 0)
+        if pipelined:
+            assert launches > 12            # several pushes, not one call
+        else:
+            assert launches <= 8
+            np.testing.assert_array_equal(extra[0].numpy(), o["perm"])
+            np.testing.assert_array_equal(extra[1].numpy(), o["label"])
+    pl.free()
+
+
+def test_process_host_pipelined_falls_back_on_a_broken_promise(tpx3):
+    """Pixels that arrive four shots late, behind a chunk cut, break the half-period disorder bound the pipelined route assumes: it
+    notices (late events) and redoes the call in one piece; the rows are the oracle's all the same."""
+    import torch
+
+    w0 = gen.generate(1, shots=24000)
+    shot = (w0.toa // np.uint64(P)).astype(np.int64)
+    shot -= shot.min()
+    s_b = shot[1 << 22]                       # the shot the first chunk cut falls into
+    moved = (shot == s_b - 3) & (np.arange(w0.n) % 3 == 0)      # ... arrive in the second chunk, 4 shots late
+    order = np.argsort(np.where(moved, shot + 4, shot) * 4 + moved, kind="stable")
+    x, y, toa, tot = w0.x[order], w0.y[order], w0.toa[order], w0.tot[order]
+    o = oracle.run(x, y, toa, tot, W, P, threads=0)
+    pl = tpx3.plan(tpx3.Config(max_hits=w0.n))
+    cl = tpx3.Clusters(w0.n // 2, "cpu", pin=True)
+    ncl = pl.process_host(*(torch.from_numpy(a).pin_memory() for a in (x, y, toa, tot)), cl)
+    assert ncl == o["n_clusters"] and pl.host_route() == 2
+    g = cl.numpy(ncl)
+    for k in _ROW_KEYS:
+        np.testing.assert_array_equal(g[k], o[k], err_msg=k)
+    pl.free()
