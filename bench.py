@@ -503,6 +503,88 @@ def run_stream(args):
     return 0
 
 
+def run_aux(args):
+    """--mode unwrap | preprocess: the two preprocessing calls of SURVEY.md 8f NEXT #4 / #3 on the workload's
+    events (device-resident, device-timed), against the HBM roofline of their algorithmic bytes."""
+    import numpy as np
+    import torch
+
+    import paper_2603_04942_b200 as m
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    m.load_library()
+    w = make_workload(args.workload, args.shots, 0)
+    n, P = w.n, w.shot_period_ticks
+    pl = m.plan(m.Config(max_hits=max(n, 1), toa_window_ticks=w.toa_window_ticks, shot_period_ticks=P))
+    stream = torch.cuda.Stream(device=0)
+    if args.mode == "unwrap":
+        # the workload's ToA folded into a counter of 2^34 ticks (several wraps over the run), PAPER.md:58-62
+        modulus, jump = 1 << 34, 1 << 33
+        raw = torch.from_numpy((w.toa % np.uint64(modulus)).astype(np.uint64)).cuda()
+        out = torch.empty_like(raw)
+        wr = torch.empty(1, dtype=torch.int64, device="cuda")
+        step = lambda: pl.unwrap_toa(raw, modulus, jump, out=out, wraps_out=wr, stream=stream)  # noqa: E731
+        bytes_step = 16 * n
+        what = {"call": "tpx3_unwrap_toa", "modulus": modulus, "jump": jump}
+    else:
+        # irregular triggers, timewalk added to every pixel, every 10th event turned into a dark count past the cut
+        shot = (w.toa // np.uint64(P)).astype(np.int64)
+        s0 = int(shot.min())
+        nshot = int(shot.max()) - s0 + 1
+        trig = (np.arange(nshot, dtype=np.int64) + s0) * P + 1000 * (np.arange(nshot) % 7)
+        table = m.timewalk_table(2000.0, 2.0, 3.0, 1.2, 1024)
+        cut = 64000
+        toa = trig[shot - s0] + (w.toa.astype(np.int64) - shot * P) + table[np.minimum(w.tot, 1023)]
+        dark = np.arange(n) % 10 == 0
+        toa[dark] = trig[shot[dark] - s0] + cut + 1 + (np.arange(n)[dark] % 1000)
+        dev = [torch.from_numpy(a).cuda() for a in (w.x, w.y, toa.astype(np.uint64), w.tot)]
+        dtrig = torch.from_numpy(trig.astype(np.uint64)).cuda()
+        dtab = torch.from_numpy(table).cuda()
+        res = {}
+
+        def step():
+            res["out"] = pl.preprocess(*dev, dtrig, cut, dtab, shot_base=s0, stream=stream)
+
+        step()
+        torch.cuda.synchronize()
+        kept = int(res["out"][5].cpu().numpy()[0])
+        bytes_step = 14 * n + 18 * kept + 4 * kept
+        what = {"call": "tpx3_preprocess", "triggers": nshot, "cut_ticks": cut, "kept": kept, "dropped": n - kept}
+    for _ in range(max(args.warmup, 1)):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.3)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = pl.launch_count()
+    t_wall0 = time.time()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    launches = pl.launch_count() - l0
+    ms_step = ev0.elapsed_time(ev1) / max(args.steps, 1)
+    sampler.stop()
+    peak, peak_src = measured_peak()
+    what.update({"workload": w.name, "mode": args.mode, "pixel_hits_per_gpu": n})
+    line = {
+        "metric": METRIC, "value": n / (ms_step * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int64", "data": "synthetic", "config": what, "gpu_launches": launches,
+        "roofline": {"bound": "hbm", "kernel": what["call"] + " (3 kernels)", "achieved": bytes_step / (ms_step * 1e-3) / 1e9,
+                     "peak": peak, "unit": "GB/s", "frac": bytes_step / (ms_step * 1e-3) / 1e9 / peak, "traffic": None,
+                     "peak_source": peak_src, "algorithmic_bytes_per_step": bytes_step},
+        "clocks": sampler.summary(t_wall0, time.time()),
+    }
+    print(json.dumps(line), flush=True)
+    pl.free()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -516,7 +598,7 @@ def main():
                     help="tile-size hint for the plan (default: the workload recipe's bound on hits per shot)")
     ap.add_argument("--chunk", type=int, default=1 << 22, help="--mode stream: events per push")
     ap.add_argument("--max-carry", type=int, default=1 << 20, help="--mode stream: carry capacity in events")
-    ap.add_argument("--mode", choices=("components", "localmax", "stream"), default="components",
+    ap.add_argument("--mode", choices=("components", "localmax", "stream", "unwrap", "preprocess"), default="components",
                     help="components: the hot path (default). localmax: the paper-literal mode, SURVEY 8f NEXT #2")
     ap.add_argument("--window", type=int, nargs=3, default=(2, 2, 320), metavar=("WX", "WY", "WT"),
                     help="box half-widths of --mode localmax (pixels, pixels, ticks)")
@@ -527,6 +609,8 @@ def main():
         print("note: timing rules ask for >= 3 warm-up steps", file=sys.stderr)
     if args.impl == "reference":
         return run_reference(args)
+    if args.mode in ("unwrap", "preprocess"):
+        return run_aux(args)
     return run_stream(args) if args.mode == "stream" else run_ours(args)
 
 

@@ -540,7 +540,6 @@ int tpx3_preprocess(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t 
   a.P = p->cfg.shot_period_ticks; a.shot_base = shot_base; a.table = table; a.table_len = table_len;
   a.x_out = x_out; a.y_out = y_out; a.tot_out = tot_out; a.toa_out = toa_out; a.index_out = index_out;
   a.n_out = n_out;
-  a.tmp = w.keyA;       // 8 bytes per event
   a.blk = w.counts;     // the sort's digit counters: room for 2^28 / 4096 block counts
   a.nblk = (uint32_t)((n + kPreTile - 1) / kPreTile);
   if (a.nblk) TPX3_LAUNCH(p, k_pre_mark, a.nblk, kPreThreads, 0, st, a);

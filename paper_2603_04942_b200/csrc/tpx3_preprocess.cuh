@@ -6,17 +6,19 @@
 //           the table uses its last entry), clamped to [0, P - 1] (R23)
 //   rebase  ToA' = (shot_base + s) * P + ToF': downstream `shot = ToA' div P` is the trigger index (R6)
 // Kept events stay in stream order (an order-preserving stream compaction):
-//   k_pre_mark     ToA' or "dropped" per event (binary search in the trigger list, L2-resident), kept per block
+//   k_pre_mark     kept / dropped per event (trigger lookup: 64 triggers around the block's first event in
+//                  shared memory, binary search in the L2-resident list otherwise), kept per block; reads ToA only
 //   k_pre_scan     exclusive scan of the block counts (one block); total -> n_out
-//   k_pre_scatter  in-block ranks in stream order, coalesced copies of x, y, ToT, ToA' and the input index
+//   k_pre_scatter  ToA' again (striped, coalesced), in-block ranks in stream order through shared memory,
+//                  striped coalesced copies of x, y, ToT, ToA' and the input index
 #pragma once
 #include "tpx3_centroid.cuh"
 #include "tpx3_common.cuh"
 
 namespace tpx3 {
 
-constexpr int kPreThreads = 256;
-constexpr int kPreItems = 16;
+constexpr int kPreThreads = 512;
+constexpr int kPreItems = 8;
 constexpr int kPreTile = kPreThreads * kPreItems;   // 4096 events per block
 constexpr uint64_t kPreDropped = ~0ull;
 
@@ -33,27 +35,70 @@ struct PreArgs {
   uint64_t* toa_out;
   uint32_t* index_out;   // may be null
   uint32_t* n_out;
-  uint64_t* tmp;         // ToA' or kPreDropped per event
   uint32_t* blk;
   uint32_t nblk;
 };
 
-__device__ __forceinline__ uint64_t pre_event(const PreArgs& a, uint64_t k) {
-  const uint64_t t = a.toa[k];
-  uint64_t lo = 0, hi = a.n_trig;       // first trigger later than t
+constexpr int kPreWin = 64;   // triggers of the block's neighbourhood held in shared memory
+
+// The block's window of the trigger list: trig[h0 .. h0 + valid), h0 a few triggers before the most recent
+// trigger of the block's first event (the stream is close to time order, so nearly every event of the block
+// finds its trigger inside the window; the rest take the binary search in global memory).
+struct PreWindow {
+  uint64_t trig[kPreWin];
+  uint64_t h0;
+  uint32_t valid;
+};
+
+__device__ __forceinline__ uint64_t pre_search(const PreArgs& a, uint64_t t) {   // first trigger later than t
+  uint64_t lo = 0, hi = a.n_trig;
   while (lo < hi) {
     const uint64_t mid = (lo + hi) >> 1;
     if (a.trig[mid] <= t) lo = mid + 1; else hi = mid;
   }
-  if (lo == 0) return kPreDropped;
-  const uint64_t s = lo - 1;
+  return lo;
+}
+
+__device__ __forceinline__ void pre_window_fill(const PreArgs& a, uint64_t k_first, PreWindow* w) {
+  if (threadIdx.x == 0) {
+    uint64_t lo = k_first < a.n ? pre_search(a, a.toa[k_first]) : 0ull;
+    lo = lo > 9 ? lo - 9 : 0ull;
+    w->h0 = lo;
+    w->valid = (uint32_t)(a.n_trig - lo < (uint64_t)kPreWin ? a.n_trig - lo : (uint64_t)kPreWin);
+  }
+  __syncthreads();
+  if (threadIdx.x < kPreWin) w->trig[threadIdx.x] = threadIdx.x < w->valid ? a.trig[w->h0 + threadIdx.x] : ~0ull;
+  __syncthreads();
+}
+
+// Index of the most recent trigger (largest s with trig[s] <= t), or false if there is none. Exact for any
+// input: the window only answers when t lies strictly inside it.
+__device__ __forceinline__ bool pre_find(const PreArgs& a, const PreWindow* w, uint64_t t, uint64_t& s) {
+  const uint32_t valid = w->valid;
+  if (valid >= 2 && t >= w->trig[0] && t < w->trig[valid - 1]) {
+    uint32_t lo = 0;                      // largest j with trig[j] <= t, j in [0, valid - 1)
+#pragma unroll
+    for (uint32_t step = kPreWin / 2; step; step >>= 1)
+      if (lo + step < valid && w->trig[lo + step] <= t) lo += step;
+    s = w->h0 + lo;
+    return true;
+  }
+  const uint64_t lo = pre_search(a, t);
+  if (lo == 0) return false;
+  s = lo - 1;
+  return true;
+}
+
+// ToA' of event k, or kPreDropped (no trigger yet, or ToF beyond the cut).
+__device__ __forceinline__ uint64_t pre_event(const PreArgs& a, const PreWindow* w, uint64_t t, uint32_t tt,
+                                              bool with_tot) {
+  uint64_t s = 0;
+  if (!pre_find(a, w, t, s)) return kPreDropped;
   const uint64_t tof = t - a.trig[s];
   if (tof > a.cut) return kPreDropped;
+  if (!with_tot) return 0ull;            // the mark pass only needs kept / dropped
   long long corr = 0;
-  if (a.table_len) {
-    const uint32_t tt = a.tot[k];
-    corr = a.table[tt < a.table_len ? tt : a.table_len - 1u];
-  }
+  if (a.table_len) corr = a.table[tt < a.table_len ? tt : a.table_len - 1u];
   long long tc = (long long)tof - corr;   // tof <= cut < 2^63
   if (tc < 0) tc = 0;
   if ((uint64_t)tc > a.P - 1ull) tc = (long long)(a.P - 1ull);
@@ -61,21 +106,27 @@ __device__ __forceinline__ uint64_t pre_event(const PreArgs& a, uint64_t k) {
 }
 
 __global__ void __launch_bounds__(kPreThreads) k_pre_mark(PreArgs a) {
-  __shared__ uint32_t sm[33];
+  __shared__ uint32_t s_cnt;
+  __shared__ PreWindow s_win;
   const uint64_t base = (uint64_t)blockIdx.x * kPreTile;
+  if (threadIdx.x == 0) s_cnt = 0;
+  pre_window_fill(a, base, &s_win);
   uint32_t cnt = 0;
-#pragma unroll 2
+  uint64_t t[kPreItems];
+#pragma unroll
+  for (int i = 0; i < kPreItems; ++i) {      // all loads first: independent and coalesced
+    const uint64_t k = base + (uint64_t)i * kPreThreads + threadIdx.x;
+    t[i] = k < a.n ? a.toa[k] : 0ull;
+  }
+#pragma unroll
   for (int i = 0; i < kPreItems; ++i) {
     const uint64_t k = base + (uint64_t)i * kPreThreads + threadIdx.x;
-    if (k < a.n) {
-      const uint64_t v = pre_event(a, k);
-      a.tmp[k] = v;
-      cnt += v != kPreDropped;
-    }
+    if (k < a.n) cnt += pre_event(a, &s_win, t[i], 0u, false) != kPreDropped;
   }
-  uint32_t total;
-  block_exclusive_scan_256(cnt, sm, &total);
-  if (threadIdx.x == 0) a.blk[blockIdx.x] = total;
+  cnt = __reduce_add_sync(0xffffffffu, cnt);
+  if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(&s_cnt, cnt);
+  __syncthreads();
+  if (threadIdx.x == 0) a.blk[blockIdx.x] = s_cnt;
 }
 
 __global__ void __launch_bounds__(1024) k_pre_scan(PreArgs a) {
@@ -84,29 +135,52 @@ __global__ void __launch_bounds__(1024) k_pre_scan(PreArgs a) {
 }
 
 __global__ void __launch_bounds__(kPreThreads) k_pre_scatter(PreArgs a) {
+  __shared__ __align__(16) uint8_t s_keep[kPreTile];
+  __shared__ uint16_t s_rank[kPreTile];
   __shared__ uint32_t sm[33];
-  // blocked arrangement: a thread owns 16 consecutive events, so ranks follow the stream order
-  const uint64_t base = (uint64_t)blockIdx.x * kPreTile + (uint64_t)threadIdx.x * kPreItems;
+  __shared__ PreWindow s_win;
+  const uint64_t base = (uint64_t)blockIdx.x * kPreTile;
+  pre_window_fill(a, base, &s_win);
+  // striped (coalesced) pass: ToA' of every event
   uint64_t v[kPreItems];
-  uint32_t cnt = 0;
+  uint16_t tt[kPreItems];
 #pragma unroll
-  for (int i = 0; i < kPreItems; ++i) {
-    const uint64_t k = base + i;
-    v[i] = k < a.n ? a.tmp[k] : kPreDropped;
-    cnt += v[i] != kPreDropped;
+  for (int i = 0; i < kPreItems; ++i) {      // all loads first: independent and coalesced
+    const uint64_t k = base + (uint64_t)i * kPreThreads + threadIdx.x;
+    v[i] = k < a.n ? a.toa[k] : 0ull;
+    tt[i] = k < a.n ? a.tot[k] : (uint16_t)0;
   }
-  uint32_t off = block_exclusive_scan_256(cnt, sm, nullptr) + a.blk[blockIdx.x];
 #pragma unroll
   for (int i = 0; i < kPreItems; ++i) {
-    if (v[i] != kPreDropped) {
-      const uint64_t k = base + i;
-      a.x_out[off] = a.x[k];
-      a.y_out[off] = a.y[k];
-      a.tot_out[off] = a.tot[k];
-      a.toa_out[off] = v[i];
-      if (a.index_out) a.index_out[off] = (uint32_t)k;
-      ++off;
-    }
+    const uint32_t loc = (uint32_t)i * kPreThreads + threadIdx.x;
+    const uint64_t k = base + loc;
+    v[i] = k < a.n ? pre_event(a, &s_win, v[i], tt[i], true) : kPreDropped;
+    s_keep[loc] = v[i] != kPreDropped;
+  }
+  __syncthreads();
+  // blocked pass over the flags: a thread owns 8 consecutive events, so ranks follow the stream order
+  static_assert(kPreItems == 8, "one 8-byte load of flags per thread");
+  const uint2 q = *reinterpret_cast<const uint2*>(&s_keep[threadIdx.x * kPreItems]);
+  const uint32_t qw[2] = {q.x, q.y};
+  const uint32_t cnt = __popc(q.x) + __popc(q.y);
+  uint32_t off = block_exclusive_scan_256(cnt, sm, nullptr);
+#pragma unroll
+  for (int j = 0; j < kPreItems; ++j)
+    if ((qw[j >> 2] >> (8 * (j & 3))) & 1u) s_rank[threadIdx.x * kPreItems + j] = (uint16_t)off++;
+  __syncthreads();
+  // striped pass again: neighbouring threads hold neighbouring ranks, so the copies are coalesced
+  const uint32_t blk_off = a.blk[blockIdx.x];
+#pragma unroll
+  for (int i = 0; i < kPreItems; ++i) {
+    if (v[i] == kPreDropped) continue;
+    const uint32_t loc = (uint32_t)i * kPreThreads + threadIdx.x;
+    const uint64_t k = base + loc;
+    const uint32_t o = blk_off + s_rank[loc];
+    a.x_out[o] = a.x[k];
+    a.y_out[o] = a.y[k];
+    a.tot_out[o] = tt[i];
+    a.toa_out[o] = v[i];
+    if (a.index_out) a.index_out[o] = (uint32_t)k;
   }
 }
 

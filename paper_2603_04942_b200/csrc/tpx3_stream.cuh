@@ -19,8 +19,8 @@
 
 namespace tpx3 {
 
-constexpr int kStreamThreads = 256;
-constexpr int kStreamItems = 16;
+constexpr int kStreamThreads = 512;
+constexpr int kStreamItems = 8;
 constexpr int kStreamTile = kStreamThreads * kStreamItems;   // 4096 events per block
 constexpr uint32_t kStreamSample = 65536;                    // chunk tail that feeds the running maximum
 
@@ -175,9 +175,10 @@ __global__ void __launch_bounds__(kStreamThreads) k_stream_scatter(StreamArgs a)
     s_cls[loc] = (uint8_t)cl;
   }
   __syncthreads();
-  // blocked pass over the classes: a thread owns 16 consecutive events, so ranks follow the stream order
-  const uint4 q = *reinterpret_cast<const uint4*>(&s_cls[threadIdx.x * kStreamItems]);
-  const uint32_t qw[4] = {q.x, q.y, q.z, q.w};
+  // blocked pass over the classes: a thread owns 8 consecutive events, so ranks follow the stream order
+  static_assert(kStreamItems == 8, "one 8-byte load of classes per thread");
+  const uint2 q = *reinterpret_cast<const uint2*>(&s_cls[threadIdx.x * kStreamItems]);
+  const uint32_t qw[2] = {q.x, q.y};
   uint32_t e = 0, k = 0;
 #pragma unroll
   for (int j = 0; j < kStreamItems; ++j) {
@@ -196,7 +197,7 @@ __global__ void __launch_bounds__(kStreamThreads) k_stream_scatter(StreamArgs a)
   __syncthreads();
   // striped pass again: neighbouring threads hold neighbouring ranks, so the copies are coalesced
   const uint32_t e_base = a.blk_emit[blockIdx.x], k_base = a.blk_keep[blockIdx.x];
-#pragma unroll 4
+#pragma unroll
   for (int i = 0; i < kStreamItems; ++i) {
     const uint32_t loc = (uint32_t)i * kStreamThreads + threadIdx.x;
     const uint32_t cl = s_cls[loc];

@@ -12,15 +12,15 @@
 // ADJACENT difference raw[k] - raw[k-1] alone: a prefix sum, not a sequential dependence.
 //   k_unwrap_count   d_k summed per block of 4096 events
 //   k_unwrap_scan    exclusive scan of the block sums (one block); total -> wraps_out
-//   k_unwrap_apply   in-block scan, toa[i] = raw[i] + wraps_i * modulus
+//   k_unwrap_apply   in-block scan (ballots per 32-event row), toa[i] = raw[i] + wraps_i * modulus
 #pragma once
 #include "tpx3_centroid.cuh"
 #include "tpx3_common.cuh"
 
 namespace tpx3 {
 
-constexpr int kUnwrapThreads = 256;
-constexpr int kUnwrapItems = 16;
+constexpr int kUnwrapThreads = 512;
+constexpr int kUnwrapItems = 8;
 constexpr int kUnwrapTile = kUnwrapThreads * kUnwrapItems;   // 4096 events per block
 
 struct UnwrapArgs {
@@ -66,34 +66,47 @@ __global__ void __launch_bounds__(1024) k_unwrap_scan(UnwrapArgs a) {
   if (threadIdx.x == 0) *a.wraps_out = a.wraps_in + (long long)(int)x;
 }
 
+// A warp owns 256 consecutive events and walks them in 8 rows of 32 (coalesced 256-byte rows). Within a row
+// the running count is two ballots (+1 lanes, -1 lanes) and two popcounts; the row total carries to the next.
 __global__ void __launch_bounds__(kUnwrapThreads) k_unwrap_apply(UnwrapArgs a) {
-  __shared__ uint32_t sm[33];
-  // blocked arrangement: a thread owns 16 consecutive events, so the in-block order is the stream order
-  const uint64_t base = (uint64_t)blockIdx.x * kUnwrapTile + (uint64_t)threadIdx.x * kUnwrapItems;
+  __shared__ int s_warp[kUnwrapThreads / 32];
+  const uint32_t lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
+  const uint64_t base = (uint64_t)blockIdx.x * kUnwrapTile + (uint64_t)wid * (32 * kUnwrapItems);
+  const uint32_t le = 0xFFFFFFFFu >> (31u - lane);   // lanes <= this one
   uint64_t v[kUnwrapItems];
   int pre[kUnwrapItems];
-  int s = 0;
-  uint64_t p = 0;
-  bool havep = false;
-  if (base < a.n) {
-    if (base > 0) { p = a.raw[base - 1]; havep = true; }
-    else if (a.has_prev) { p = a.prev_raw; havep = true; }
-  }
+  int run = 0;
+  // all loads first (independent, coalesced); the predecessor of an event comes from the neighbouring lane
 #pragma unroll
   for (int i = 0; i < kUnwrapItems; ++i) {
-    const uint64_t k = base + i;
+    const uint64_t k = base + (uint64_t)i * 32 + lane;
     v[i] = k < a.n ? a.raw[k] : 0ull;
-    if (k < a.n && havep) s += unwrap_delta(p, v[i], a.jump);
-    pre[i] = s;
-    p = v[i];
-    havep = true;
   }
-  const uint32_t off = block_exclusive_scan_256((uint32_t)s, sm, nullptr) + a.blk[blockIdx.x];
+  uint64_t before = a.prev_raw;          // predecessor of the warp's first event
+  bool have_before = a.has_prev != 0;
+  if (base > 0 && base < a.n) { before = a.raw[base - 1]; have_before = true; }
 #pragma unroll
   for (int i = 0; i < kUnwrapItems; ++i) {
-    const uint64_t k = base + i;
+    const uint64_t k = base + (uint64_t)i * 32 + lane;
+    uint64_t p = __shfl_up_sync(0xffffffffu, v[i], 1);
+    bool havep = true;
+    if (lane == 0) { p = before; havep = have_before; }
+    before = __shfl_sync(0xffffffffu, v[i], 31);
+    have_before = true;
+    const int d = (k < a.n && havep) ? unwrap_delta(p, v[i], a.jump) : 0;
+    const uint32_t up = __ballot_sync(0xffffffffu, d > 0), dn = __ballot_sync(0xffffffffu, d < 0);
+    pre[i] = run + __popc(up & le) - __popc(dn & le);
+    run += __popc(up) - __popc(dn);
+  }
+  if (lane == 0) s_warp[wid] = run;
+  __syncthreads();
+  int off = (int)a.blk[blockIdx.x];
+  for (uint32_t w2 = 0; w2 < wid; ++w2) off += s_warp[w2];
+#pragma unroll
+  for (int i = 0; i < kUnwrapItems; ++i) {
+    const uint64_t k = base + (uint64_t)i * 32 + lane;
     if (k < a.n) {
-      const long long wraps = a.wraps_in + (long long)(int)(off + (uint32_t)pre[i]);
+      const long long wraps = a.wraps_in + (long long)(off + pre[i]);
       a.out[k] = v[i] + (uint64_t)wraps * a.modulus;   // two's complement: a negative count subtracts
     }
   }
