@@ -955,3 +955,25 @@ def test_process_host_pipelined_falls_back_on_a_broken_promise(tpx3):
     for k in _ROW_KEYS:
         np.testing.assert_array_equal(g[k], o[k], err_msg=k)
     pl.free()
+
+
+def test_process_host_pipelined_capacity(tpx3):
+    """A host table too small for the hits of a pipelined call: TPX3_ERR_CAPACITY, the rows that fit are the
+    first rows of the oracle's table, and the plan serves the next call as usual."""
+    import torch
+
+    w = gen.generate(1, shots=24000)
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P, threads=0)
+    pl = tpx3.plan(tpx3.Config(max_hits=w.n, max_shot_hits=1024))
+    host = [torch.from_numpy(a).pin_memory() for a in (w.x, w.y, w.toa, w.tot)]
+    small = tpx3.Clusters(400001, "cpu", pin=True)
+    with pytest.raises(tpx3.Tpx3Error) as ei:
+        pl.process_host(*host, small)
+    assert ei.value.code == tpx3.ERR_CAPACITY and pl.host_route() == 1
+    g = small.numpy(400001)
+    for k in _ROW_KEYS:
+        np.testing.assert_array_equal(g[k], o[k][:400001], err_msg=k)
+    cl = tpx3.Clusters(w.n // 2, "cpu", pin=True)
+    assert pl.process_host(*host, cl) == o["n_clusters"]
+    np.testing.assert_array_equal(cl.numpy(o["n_clusters"])["c_sum_tot_tof"], o["c_sum_tot_tof"])
+    pl.free()
