@@ -134,7 +134,7 @@ __global__ void __launch_bounds__(1024) k_pre_scan(PreArgs a) {
   if (threadIdx.x == 0) *a.n_out = x;
 }
 
-__global__ void __launch_bounds__(kPreThreads) k_pre_scatter(PreArgs a) {
+__global__ void __launch_bounds__(kPreThreads, 2) k_pre_scatter(PreArgs a) {
   __shared__ __align__(16) uint8_t s_keep[kPreTile];
   __shared__ uint16_t s_rank[kPreTile];
   __shared__ uint32_t sm[33];
@@ -170,14 +170,21 @@ __global__ void __launch_bounds__(kPreThreads) k_pre_scatter(PreArgs a) {
   __syncthreads();
   // striped pass again: neighbouring threads hold neighbouring ranks, so the copies are coalesced
   const uint32_t blk_off = a.blk[blockIdx.x];
+  // all loads before the first store (the compiler cannot prove that the outputs do not alias the inputs)
+  uint32_t exy[kPreItems];
+#pragma unroll
+  for (int i = 0; i < kPreItems; ++i) {
+    const uint64_t k = base + (uint32_t)i * kPreThreads + threadIdx.x;
+    exy[i] = v[i] != kPreDropped ? (uint32_t)a.x[k] | ((uint32_t)a.y[k] << 16) : 0u;
+  }
 #pragma unroll
   for (int i = 0; i < kPreItems; ++i) {
     if (v[i] == kPreDropped) continue;
     const uint32_t loc = (uint32_t)i * kPreThreads + threadIdx.x;
     const uint64_t k = base + loc;
     const uint32_t o = blk_off + s_rank[loc];
-    a.x_out[o] = a.x[k];
-    a.y_out[o] = a.y[k];
+    a.x_out[o] = (uint16_t)exy[i];
+    a.y_out[o] = (uint16_t)(exy[i] >> 16);
     a.tot_out[o] = tt[i];
     a.toa_out[o] = v[i];
     if (a.index_out) a.index_out[o] = (uint32_t)k;

@@ -154,7 +154,7 @@ __global__ void __launch_bounds__(1024) k_stream_scan(StreamArgs a) {
   }
 }
 
-__global__ void __launch_bounds__(kStreamThreads) k_stream_scatter(StreamArgs a) {
+__global__ void __launch_bounds__(kStreamThreads, 3) k_stream_scatter(StreamArgs a) {
   __shared__ __align__(16) uint8_t s_cls[kStreamTile];
   __shared__ uint16_t s_rank[kStreamTile];
   __shared__ uint32_t sm[33];

@@ -51,10 +51,21 @@ __global__ void __launch_bounds__(kUnwrapThreads) k_unwrap_count(UnwrapArgs a) {
   __shared__ uint32_t sm[33];
   const uint64_t base = (uint64_t)blockIdx.x * kUnwrapTile;
   int s = 0;
-#pragma unroll 4
+  uint64_t v[kUnwrapItems];
+#pragma unroll
+  for (int i = 0; i < kUnwrapItems; ++i) {      // all loads first
+    const uint64_t k = base + (uint64_t)i * kUnwrapThreads + threadIdx.x;
+    v[i] = k < a.n ? a.raw[k] : 0ull;
+  }
+#pragma unroll
   for (int i = 0; i < kUnwrapItems; ++i) {
     const uint64_t k = base + (uint64_t)i * kUnwrapThreads + threadIdx.x;
-    if (k < a.n) s += unwrap_delta_at(a, k);
+    // the predecessor is the neighbouring lane's value; lane 0 reads it (the previous warp's line, an L1 / L2 hit)
+    uint64_t p = __shfl_up_sync(0xffffffffu, v[i], 1);
+    if (k < a.n) {
+      if ((threadIdx.x & 31) == 0) s += unwrap_delta_at(a, k);
+      else s += unwrap_delta(p, v[i], a.jump);
+    }
   }
   uint32_t total;
   block_exclusive_scan_256((uint32_t)s, sm, &total);
@@ -68,7 +79,7 @@ __global__ void __launch_bounds__(1024) k_unwrap_scan(UnwrapArgs a) {
 
 // A warp owns 256 consecutive events and walks them in 8 rows of 32 (coalesced 256-byte rows). Within a row
 // the running count is two ballots (+1 lanes, -1 lanes) and two popcounts; the row total carries to the next.
-__global__ void __launch_bounds__(kUnwrapThreads) k_unwrap_apply(UnwrapArgs a) {
+__global__ void __launch_bounds__(kUnwrapThreads, 3) k_unwrap_apply(UnwrapArgs a) {
   __shared__ int s_warp[kUnwrapThreads / 32];
   const uint32_t lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
   const uint64_t base = (uint64_t)blockIdx.x * kUnwrapTile + (uint64_t)wid * (32 * kUnwrapItems);
