@@ -36,6 +36,7 @@ struct tpx3_plan_s {
   std::vector<Span> spans;
   std::vector<cudaEvent_t> free_events;
   uint64_t profiled_calls;
+  cudaStream_t copy_in, copy_out;   // copy streams of the pipelined tpx3_process_host (created on first use)
   int host_route;           // last tpx3_process_host: 0 one piece, 1 pipelined, 2 pipelined attempt redone in one piece
 };
 
@@ -342,6 +343,8 @@ int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace
   p->launches = 0;
   p->profiling = false;
   p->profiled_calls = 0;
+  p->copy_in = p->copy_out = nullptr;
+  p->host_route = 0;
   p->num_sms = kNumSMs;
   Params& prm = p->prm;
   prm.n = 0;
@@ -684,7 +687,11 @@ struct HostIo {
 struct Carver {
   char* b;
   size_t o;
-  char* operator()(size_t bytes) { char* r = b + o; o = align_up(o + bytes); return r; }
+  char* operator()(size_t bytes) {   // b == nullptr: sizes only
+    char* r = b ? b + o : nullptr;
+    o = align_up(o + bytes);
+    return r;
+  }
 };
 
 tpx3_clusters_t carve_clusters(Carver& take, uint64_t cap) {
@@ -749,13 +756,13 @@ int process_host_pipelined(tpx3_plan_t p, void* workspace, const HostIo& io, cud
                            bool* fell_back) {
   *fell_back = true;
   const uint32_t nchunk = (uint32_t)((n + kPipeChunk - 1) / kPipeChunk);
-  cudaStream_t s_in = nullptr, s_out = nullptr;
   std::vector<cudaEvent_t> ev(3 * (size_t)nchunk + 1, nullptr);   // [0] entry, then in / done / out per chunk
   std::vector<uint32_t> nh(nchunk, 0);
   tpx3_stream_t sh = nullptr;
   int rc = TPX3_ERR_CUDA;
-  bool ok = cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking) == cudaSuccess &&
-            cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking) == cudaSuccess;
+  bool ok = (p->copy_in || cudaStreamCreateWithFlags(&p->copy_in, cudaStreamNonBlocking) == cudaSuccess) &&
+            (p->copy_out || cudaStreamCreateWithFlags(&p->copy_out, cudaStreamNonBlocking) == cudaSuccess);
+  cudaStream_t s_in = p->copy_in, s_out = p->copy_out;
   for (size_t i = 0; ok && i < ev.size(); ++i) ok = cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming) == cudaSuccess;
   auto e_in = [&](uint32_t j) { return ev[1 + 3 * (size_t)j]; };
   auto e_done = [&](uint32_t j) { return ev[2 + 3 * (size_t)j]; };
@@ -820,8 +827,6 @@ int process_host_pipelined(tpx3_plan_t p, void* workspace, const HostIo& io, cud
   cudaStreamSynchronize(st);
   if (sh) tpx3_stream_close(sh);
   for (auto e : ev) if (e) cudaEventDestroy(e);
-  if (s_in) cudaStreamDestroy(s_in);
-  if (s_out) cudaStreamDestroy(s_out);
   if (!ok) return rc != TPX3_OK ? rc : TPX3_ERR_CUDA;
   return rc;
 }
@@ -918,6 +923,8 @@ int tpx3_free(tpx3_plan_t p) {
   if (!p) return TPX3_ERR_INVALID_ARG;
   for (auto& s : p->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
   for (auto e : p->free_events) cudaEventDestroy(e);
+  if (p->copy_in) cudaStreamDestroy(p->copy_in);
+  if (p->copy_out) cudaStreamDestroy(p->copy_out);
   delete p;
   return TPX3_OK;
 }
