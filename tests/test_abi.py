@@ -117,3 +117,21 @@ def test_timewalk_table_host_helper_matches_the_oracle():
                           (0.0, 1.0, 2.5, 1.0, 8), (123.456, 0.0, -7.25, 0.9, 300), (50.0, -2.0, 0.0, 1.0, 16)]:
         assert np.array_equal(m.timewalk_table(a, b, c, d, n), pp.timewalk_table(a, b, c, d, n)), (a, b, c, d)
     assert m.timewalk_table(1.0, 1.0, 1.0, 1.0, 0).shape == (0,)
+
+
+def test_stream_and_pipeline_buffer_sizes_host_only():
+    """Pure host arithmetic of the two size queries: the stream buffer holds two carry banks, the emit arrays
+    (14 bytes per event plus perm and label) and the block counters; the host-I/O buffer grows by the two
+    per-push tables and a stream buffer exactly when the call is large enough to be pipelined (2^23 events)."""
+    lib = m.load_library()
+    chunk, carry = 1 << 20, 1 << 16
+    b = lib.tpx3_stream_bytes(chunk, carry)
+    floor = 2 * 14 * carry + (14 + 8) * (chunk + carry)
+    assert floor <= b <= floor + (1 << 20)
+    assert lib.tpx3_stream_bytes(2 * chunk, carry) > b and lib.tpx3_stream_bytes(chunk, 2 * carry) > b
+    n_small, n_big, cap = (1 << 23) - 1, 1 << 23, 1 << 20
+    small, big = lib.tpx3_host_io_bytes(n_small, cap), lib.tpx3_host_io_bytes(n_big, cap)
+    per_push = (1 << 22) + (1 << 20)
+    extra = 2 * 64 * per_push + lib.tpx3_stream_bytes(1 << 22, 1 << 20)
+    assert extra <= big - small <= extra + (1 << 16)
+    assert m.load_library().tpx3_host_route(None) == m.ERR_INVALID_ARG
