@@ -59,12 +59,38 @@ __device__ __forceinline__ uint64_t pre_search(const PreArgs& a, uint64_t t) {  
   return lo;
 }
 
+// Every thread of the block must call this. The position of the block's first event in the trigger list is
+// found by the whole block in two rounds of loads (every stride-th trigger, then the stride that holds it)
+// instead of 17 dependent steps of one thread; a list too long for that (more than blockDim^2 triggers)
+// finishes the second round with a binary search.
 __device__ __forceinline__ void pre_window_fill(const PreArgs& a, uint64_t k_first, PreWindow* w) {
+  const uint64_t nt = a.n_trig;
+  uint64_t lo = 0;                                   // first trigger later than the block's first event
+  if (k_first < a.n && nt) {                         // block-uniform
+    const uint64_t t0 = a.toa[k_first];
+    const uint64_t stride = (nt + blockDim.x - 1) / blockDim.x;
+    const uint64_t p1 = (uint64_t)threadIdx.x * stride;
+    const int c1 = __syncthreads_count(p1 < nt && a.trig[p1] <= t0);      // trig ascending: a prefix of the threads
+    if (c1) {
+      const uint64_t seg = (uint64_t)(c1 - 1) * stride;
+      if (stride <= blockDim.x) {
+        const uint64_t p2 = seg + threadIdx.x;
+        const int c2 = __syncthreads_count(threadIdx.x < stride && p2 < nt && a.trig[p2] <= t0);
+        lo = seg + (uint64_t)c2;
+      } else {
+        uint64_t l = seg, h = seg + stride < nt ? seg + stride : nt;
+        while (l < h) {
+          const uint64_t mid = (l + h) >> 1;
+          if (a.trig[mid] <= t0) l = mid + 1; else h = mid;
+        }
+        lo = l;
+      }
+    }
+  }
   if (threadIdx.x == 0) {
-    uint64_t lo = k_first < a.n ? pre_search(a, a.toa[k_first]) : 0ull;
-    lo = lo > 9 ? lo - 9 : 0ull;
-    w->h0 = lo;
-    w->valid = (uint32_t)(a.n_trig - lo < (uint64_t)kPreWin ? a.n_trig - lo : (uint64_t)kPreWin);
+    const uint64_t h0 = lo > 9 ? lo - 9 : 0ull;
+    w->h0 = h0;
+    w->valid = (uint32_t)(nt - h0 < (uint64_t)kPreWin ? nt - h0 : (uint64_t)kPreWin);
   }
   __syncthreads();
   if (threadIdx.x < kPreWin) w->trig[threadIdx.x] = threadIdx.x < w->valid ? a.trig[w->h0 + threadIdx.x] : ~0ull;

@@ -977,3 +977,33 @@ def test_process_host_pipelined_capacity(tpx3):
     assert pl.process_host(*host, cl) == o["n_clusters"]
     np.testing.assert_array_equal(cl.numpy(o["n_clusters"])["c_sum_tot_tof"], o["c_sum_tot_tof"])
     pl.free()
+
+
+def test_preprocess_long_trigger_list(tpx3):
+    """More than 512^2 triggers (the block-wide window search finishes with a binary search), events scattered
+    over the whole list, some before the first trigger and some beyond the cut: against the oracle."""
+    import torch
+    from oracle import preprocess as pp
+
+    rng = np.random.default_rng(23)
+    nt, n = 300000, 30011
+    trig = np.cumsum(rng.integers(500, 900, nt)).astype(np.uint64) + np.uint64(1000)
+    toa = np.sort(rng.integers(0, int(trig[-1]) + 2000, n)).astype(np.uint64)
+    swap = rng.integers(0, n - 1, 500)                       # a little disorder
+    toa[swap], toa[swap + 1] = toa[swap + 1].copy(), toa[swap].copy()
+    x = rng.integers(0, 256, n).astype(np.uint16)
+    y = rng.integers(0, 256, n).astype(np.uint16)
+    tot = rng.integers(1, 1024, n).astype(np.uint16)
+    table = tpx3.timewalk_table(300.0, 1.0, 2.0, 1.1, 64)
+    pl = tpx3.plan(tpx3.Config(max_hits=n, shot_period_ticks=P))
+    xo, yo, to, oo, io, no = pl.preprocess(to_dev(x), to_dev(y), to_dev(toa), to_dev(tot), to_dev(trig), 400,
+                                           to_dev(table), 5)
+    torch.cuda.synchronize()
+    k = int(no.cpu().numpy()[0])
+    ex, ey, et, eo, ei = pp.preprocess(x, y, toa, tot, trig, 400, table, P, 5)
+    assert k == len(ei) and 0 < k < n
+    np.testing.assert_array_equal(to[:k].cpu().numpy(), et)
+    np.testing.assert_array_equal(io[:k].cpu().numpy().astype(np.int64), ei)
+    np.testing.assert_array_equal(xo[:k].cpu().numpy(), ex)
+    np.testing.assert_array_equal(oo[:k].cpu().numpy(), eo)
+    pl.free()
