@@ -5,9 +5,12 @@
 
 One "step" = one pass of the whole hot path (S0-S5: shot/key, stable sort, neighbour link, label
 compression, segmented reduction, centroid — tpx3_cluster_centroid) over the whole synthetic
-workload. Default workload: BASELINE.json configs[1] (electron VMI at 1 kHz, 100 000 shots x 30
-electrons, about 3.6e7 pixel hits, 0.5 GB of input: larger than the 126 MB L2, so no explicit L2
-flush is needed between steps). Metric: pixel hits/s clustered + centroided, device-timed.
+workload. Default workload: the largest streaming configuration of BASELINE.json, one shot-aligned
+2^28-hit chunk of configs[4] (ion VMI with time of flight, delivery order locally shuffled, so the
+in-tile sort runs; 3.76 GB of input: far larger than the 126 MB L2, so no explicit L2 flush is
+needed between steps) — the configuration north_star's roofline target is stated on. The same line
+carries the smaller chunk sizes of configs[4] (2^20 / 2^24 / 2^26 hits, `chunk_sweep`); the other
+configs are `--workload cfg0..cfg3`. Metric: pixel hits/s clustered + centroided, device-timed.
 
 Multi-GPU (torchrun, one rank per GPU): shots are independent units, so every rank processes its
 own contiguous range of `shots` shots (rank r: shots [r*S, (r+1)*S)) with no data-path
@@ -301,6 +304,45 @@ def run_ours(args):
     ms_step = ms_total / max(args.steps, 1)
     value = n_all / (ms_step * 1e-3)
 
+    # ---- the smaller chunk sizes of configs[4] (BASELINE.json: "Report hits/s and HBM GB/s per chunk size"):
+    #      shot-aligned prefixes of the same stream, same plan, device-timed after the headline region ------
+    sweep = None
+    if w.cfg_id == 4 and not lm and world == 1 and not args.no_sweep:
+        sweep = {}
+        peak_gbs, _ = measured_peak()
+        for cname, chunk in (("2^20", 1 << 20), ("2^24", 1 << 24), ("2^26", 1 << 26)):
+            if chunk >= n:
+                continue
+            s1 = int(np.searchsorted(w.shot_offsets, chunk, side="right")) - 1
+            mc = int(w.shot_offsets[s1])
+            if mc == 0:
+                continue
+            views = [d[:mc] for d in dev]
+
+            def cstep():
+                pl.cluster_centroid(*views, cl, perm=perm, label=label, n_clusters=nc, stream=stream)
+
+            for _ in range(3):
+                cstep()
+            torch.cuda.synchronize()
+            c_ncl = int(nc.cpu().numpy()[0])
+            reps = max(5, min(200, int((1 << 28) // mc)))
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                cstep()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            c_ms = e0.elapsed_time(e1) / reps
+            c_bytes = STAGE_BYTES["fused"](mc, c_ncl)
+            sweep[cname] = {"pixel_hits": mc, "particle_hits": c_ncl, "shots": s1, "ms_per_step": c_ms, "steps": reps,
+                            "pixel_hits_per_s": mc / (c_ms * 1e-3), "algorithmic_gbs": c_bytes / (c_ms * 1e-3) / 1e9,
+                            "frac_of_hbm_peak": c_bytes / (c_ms * 1e-3) / 1e9 / peak_gbs,
+                            "l2": "fits the 126 MB L2: launch-latency bound, DRAM not exercised" if 22 * mc < 126e6
+                                  else "larger than L2"}
+        step()   # leave the full-size result in the output buffers
+        torch.cuda.synchronize()
+
     # ---- end to end through the C ABI with HOST buffers (tpx3_process_host) --------------------
     clh = m.Clusters(max_clusters, "cpu", pin=True)
 
@@ -361,8 +403,10 @@ def run_ours(args):
     try:
         with open(traffic_file) as f:
             tr = json.load(f)
-        key = "%s:%s" % (w.name, dom)
-        if key in tr and tr[key].get("pixel_hits", n) == n:   # a capture is of one workload size
+        key = "%s:%s:%d" % (w.name, dom, n)                   # a capture is of one workload size
+        if key not in tr:
+            key = "%s:%s" % (w.name, dom)
+        if key in tr and tr[key].get("pixel_hits", n) == n:
             roofline["traffic"] = tr[key]["dram_bytes_per_launch"]
             roofline["traffic_source"] = tr[key].get("source")
             wi = tr[key].get("warp_instructions_per_launch")
@@ -409,6 +453,8 @@ def run_ours(args):
     }
     if cpu is not None:
         line["cpu_baseline"] = cpu
+    if sweep is not None:
+        line["chunk_sweep"] = sweep
     print(json.dumps(line), flush=True)
     pl.free()
     if world > 1:
@@ -591,7 +637,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
-    ap.add_argument("--workload", choices=sorted(WORKLOADS), default="cfg1")
+    ap.add_argument("--workload", choices=sorted(WORKLOADS), default="cfg4_256M")
     ap.add_argument("--shots", type=int, default=None, help="override the number of shots (testing only)")
     ap.add_argument("--force-general", action="store_true", help="never take the fused shot-tile path")
     ap.add_argument("--max-shot-hits", type=int, default=None,
@@ -603,6 +649,7 @@ def main():
     ap.add_argument("--window", type=int, nargs=3, default=(2, 2, 320), metavar=("WX", "WY", "WT"),
                     help="box half-widths of --mode localmax (pixels, pixels, ticks)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true", help="cfg4 workloads: skip the smaller chunk sizes")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":

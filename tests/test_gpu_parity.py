@@ -341,8 +341,13 @@ def _full_size_check(m, w, windows, hint):
     assert int(c["c_sum_tot"].sum()) == int(w.tot.astype(np.int64).sum())
     assert int(c["c_sum_tot_x"].sum()) == int((w.tot.astype(np.int64) * w.x.astype(np.int64)).sum())
     assert int(c["c_sum_tot_y"].sum()) == int((w.tot.astype(np.int64) * w.y.astype(np.int64)).sum())
-    assert np.array_equal(np.sort(perm.astype(np.int64)), np.arange(n, dtype=np.int64))  # a permutation
-    assert np.all(np.diff(w.toa[perm].astype(np.int64)) >= 0)                             # in ToA order
+    seen = np.zeros(n, dtype=bool)
+    seen[perm] = True
+    assert seen.all()                                                                     # a permutation
+    del seen
+    st_toa = w.toa[perm]
+    assert np.all(st_toa[1:] >= st_toa[:-1])                                              # in ToA order
+    del st_toa
     # sampled shot windows, element by element (shots are contiguous in the stream: a window of shots
     # is a window of input positions and of sorted positions)
     off = w.shot_offsets
@@ -385,6 +390,74 @@ def test_full_size_cfg3_quarter(tpx3):
     """A quarter of config 3 (12 500 shots, 2.6e7 hits, about 2 100 hits per shot: the 8192-event tiles)."""
     w = gen.generate(3, shots=12500)
     _full_size_check(tpx3, w, _windows(w.shots, 60, 5), gen.max_shot_hits(3))
+
+
+def test_full_size_cfg2(tpx3):
+    """BASELINE.json configs[2] in full (200 000 shots, 1.8e8 hits)."""
+    w = gen.generate(2)
+    ncl = _full_size_check(tpx3, w, _windows(w.shots, 120, 7), gen.max_shot_hits(2))
+    assert ncl > 8_500_000
+
+
+def test_full_size_cfg3(tpx3):
+    """BASELINE.json configs[3] in full (50 000 shots, 1.05e8 hits, noise pixels chaining the blobs)."""
+    w = gen.generate(3)
+    ncl = _full_size_check(tpx3, w, _windows(w.shots, 50, 7), gen.max_shot_hits(3))
+    assert ncl > 11_000_000
+
+
+@pytest.mark.parametrize("log2_chunk,count", [(26, 6), (28, 8)])
+def test_full_size_cfg4_chunk(tpx3, log2_chunk, count):
+    """One 2^26- and one 2^28-hit chunk of config 4 (locally shuffled: the in-tile sort runs) — 2^28 is the
+    configuration bench.py times by default and the largest a plan accepts: 32-bit positions, the 12.9 GB
+    staging table and about 10^5 tiles are at their limits. Sampled shot windows (first, last and spread over
+    the chunk) element by element against the oracle; the invariants on the whole output."""
+    chunk = 1 << log2_chunk
+    w = gen.generate(4, shots=chunk // 850 + 64, max_hits=chunk)
+    assert w.n > chunk - 2000
+    _full_size_check(tpx3, w, _windows(w.shots, 150, count), gen.max_shot_hits(4))
+
+
+def test_cfg4_rows_do_not_depend_on_the_chunk_size(tpx3):
+    """one stretch of config 4 (2^26 hits) cut at shot boundaries into chunks of 2^20, 2^24 and
+    2^26 hits gives the same hit rows (labels made global by the chunk's first position): every column, in
+    order, not only as a multiset."""
+    import torch
+
+    m = tpx3
+    n_max = 1 << 26
+    w = gen.generate(4, shots=n_max // 850 + 64, max_hits=n_max)
+    pl = m.plan(m.Config(max_hits=w.n, toa_window_ticks=W, shot_period_ticks=P, max_shot_hits=gen.max_shot_hits(4)))
+    dev = [to_dev(a) for a in (w.x, w.y, w.toa, w.tot)]
+    cl = m.Clusters(max(w.n // 2, 1024), pl.device)
+    perm = torch.empty(w.n, dtype=torch.uint32, device=pl.device)
+    label = torch.empty(w.n, dtype=torch.uint32, device=pl.device)
+    nc = torch.zeros(1, dtype=torch.uint32, device=pl.device)
+    off = w.shot_offsets
+    ref = None
+    for log2 in (26, 24, 20):
+        rows = {k: [] for k in LM_KEYS}
+        perm_all = np.empty(w.n, dtype=np.uint32)
+        for s0, s1 in w.chunks(1 << log2):
+            a, b = int(off[s0]), int(off[s1])
+            pl.cluster_centroid(*(d[a:b] for d in dev), cl, perm=perm, label=label, n_clusters=nc)
+            torch.cuda.synchronize()
+            k = int(nc.cpu().numpy()[0])
+            c = cl.numpy(k)
+            c["c_label"] = c["c_label"] + np.uint32(a)
+            for key in LM_KEYS:
+                rows[key].append(c[key])
+            perm_all[a:b] = perm[: b - a].cpu().numpy() + np.uint32(a)
+        assert pl.status()["error"] == 0
+        rows = {k: np.concatenate(v) for k, v in rows.items()}
+        if ref is None:
+            ref, ref_perm = rows, perm_all
+            assert len(ref["c_label"]) > 3_000_000
+        else:
+            for key in LM_KEYS:
+                np.testing.assert_array_equal(rows[key], ref[key], err_msg="chunks of 2^%d: %s" % (log2, key))
+            np.testing.assert_array_equal(perm_all, ref_perm, err_msg="chunks of 2^%d: perm" % log2)
+    pl.free()
 
 
 def test_small_tile_variant_with_in_tile_sort(tpx3):
