@@ -7,7 +7,7 @@
 
 namespace tpx3 {
 
-constexpr int kNumSMs = 148;               // B200
+constexpr int kNumSMs = 148;               // B200; sizes compile-time tables only (the plan reads the device's count)
 constexpr uint32_t kEmpty = 0xFFFFFFFFu;   // empty hash slot / "no hit"
 constexpr uint64_t kMaxHits = 1ull << 28;  // sorted index fits 28 bits
 
@@ -23,7 +23,7 @@ struct Ctrl {
   uint32_t tiles_done;           // fused path: tiles finished
   uint32_t fused_fail;           // fused path: some tile could not be handled
   uint32_t tight_tiles;          // fused path: tiles of this call whose time clusters were all tight
-  uint32_t pad[1];
+  uint32_t tiles_run;            // fused path: tiles of this call that owned events
   // Kept ACROSS calls on the same workspace (never reset; any garbage is a legal value: it only steers which of
   // two exact code paths a tile takes). A stream keeps its character from chunk to chunk: when hardly any tile
   // of a call had tight time clusters, the tiles of the next calls skip the check (and retry every 16th call).

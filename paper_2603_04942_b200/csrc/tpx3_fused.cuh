@@ -6,8 +6,11 @@
 // with a shot-contiguous stream the stable (shot, ToA) order only permutes events INSIDE a shot.
 // So the stream is cut into tiles of whole shots and each tile is finished in shared memory:
 //
-//   tile b owns the shots that START inside input slice [b*S, (b+1)*S); it reads up to T = S + L
-//   events (L = the largest shot the variant supports) to reach the end of its last shot. The
+//   the stream is cut into SEGMENTS of G events; CTA g walks segment g tile by tile. A tile starts at a
+//   shot start (the first tile of a segment finds the first shot start at or after g*G), reads a window
+//   of T events and owns the whole shots that lie inside the window and start before (g+1)*G; the next
+//   tile starts where this one ended, so nothing but the shot that straddles the window's end is read
+//   twice (round 1 cut fixed slices and read S + L events to own S: 58 % overlap on config 4). The
 //   global sorted position of an event is tile start + local rank: perm and label need no
 //   inter-tile communication. Only the ordinal of a hit in the ascending-label cluster table
 //   needs a prefix over tiles: tiles write their hits to a staging table at their own position
@@ -19,8 +22,11 @@
 //            fits 32 bits; shot offset sl = rel div P by a 32-bit multiply-high; tof = rel - sl*P.
 //            key = sl << tb | tof with 2^tb > max tof + W, so |key_i - key_j| <= W already implies
 //            "same shot" and ONE compare is the whole time test of Eq. 5.
-//   sort     skipped when the keys are already ascending; otherwise stable LSD radix sort of 16-bit
-//            local indices, digits ranked per warp with ballots (S1)
+//   sort     skipped when the keys are already ascending; otherwise the rank of every event in the
+//            stable (shot, ToA) order by counting: bitmap of the keys that occur -> dense key number
+//            (prefix popcount) -> count per dense key -> offsets; events of one key (a few) are ordered
+//            by input position. Keys too wide for the bitmap, or one key held by very many events: stable
+//            LSD radix sort of 16-bit local indices, digits ranked per warp with ballots (S1)
 //   hash     open table of 4-slot buckets (one 128-bit load reads a bucket), key (shot, cell),
 //            entry = cell << 16 | k+1; a bucket that overflows spills to the next one and marks
 //            itself, so the common probe is straight-line code
@@ -41,8 +47,8 @@
 // greater (ToT, sorted index), and the sums run over that box. Boxes of <= 81 cells are scanned cell by cell
 // through the hash, larger ones by walking the time window of the sorted tile.
 //
-// A tile that cannot be handled (a shot longer than L, a decreasing shot number, shot offset and time of
-// flight too wide for one 32-bit key) marks the call as failed; the general kernels, enqueued from the device
+// A tile that cannot be handled (a shot longer than the window, a decreasing shot number, shot offset and time
+// of flight too wide for one 32-bit key) marks the call as failed; the general kernels, enqueued from the device
 // behind this one (k_fallback_dispatch), then redo the call.
 #pragma once
 #include "tpx3_common.cuh"
@@ -128,8 +134,11 @@ struct FusedArgs {
   Div64 divP;
   Div32 divP32;
   uint32_t W;
-  uint32_t S;          // slice length (events); tile b owns shots starting in [b*S, (b+1)*S)
-  uint32_t num_tiles;
+  uint32_t G;          // segment length (events, multiple of 8); CTA g owns the shots starting in [g*G, (g+1)*G)
+  uint32_t nseg;       // segments = CTAs
+  uint32_t maxt;       // tile status words per segment
+  uint32_t num_tiles;  // nseg * maxt: status words (most of them stay 0)
+  uint32_t num_sms;
   uint32_t sensor_w, sensor_h;
   uint32_t flags;
   const uint16_t* x;
@@ -178,7 +187,8 @@ struct FusedSmem {
 };
 
 struct FusedMisc {
-  unsigned int lo, hi;         // owned range, relative to the tile base
+  unsigned int lo, hi;         // first shot start of the window; first one at or after the segment's end
+  unsigned int last;           // last shot start of the window
   unsigned int fail;
   unsigned int max_tof, max_sl;
   unsigned int n_roots;
@@ -236,9 +246,21 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   FusedMisc* misc = reinterpret_cast<FusedMisc*>(smem + L::kMisc);
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
 
+  // ---- the CTA walks its segment tile by tile ---------------------------------------------------------
+  const uint32_t seg = blockIdx.x;
+  const uint64_t seg_begin = (uint64_t)seg * a.G;
+  const uint64_t seg_end = seg_begin + a.G < a.n ? seg_begin + a.G : a.n;
+  const uint32_t P32 = (uint32_t)a.P;
+  uint64_t tile_at = seg_begin;     // where the next tile starts; a shot start except for the segment's first tile
+  bool at_start = seg == 0;         // tile_at is known to be a shot start
+  uint32_t tile_i = 0;              // status words written so far
+  bool seg_failed = false;
+  for (;;) {
+  __syncthreads();                  // the previous tile is done with the shared memory
   if (tid == 0) {
     misc->lo = kNone;
     misc->hi = kNone;
+    misc->last = 0;
     // another tile already gave up: this attempt is lost, do not spend time on it (the next attempt — a
     // variant with longer shots, or the general kernels — is enqueued behind; k_fallback_dispatch)
     misc->skip = atomicAdd(&a.ctrl->fused_fail, 0u);
@@ -252,21 +274,13 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     misc->n_list = 0;
   }
   __syncthreads();
-  const uint32_t b = blockIdx.x;
-  if (misc->skip != 0u) {
-    if (tid == 0) {
-      a.tiles[b] = 0ull;
-      __threadfence();
-      const uint32_t done = atomicAdd(&a.ctrl->tiles_done, 1u);
-      if (done + 1u == a.num_tiles) a.ctrl->fused_state = 2u;
-    }
-    return;
-  }
-  const uint64_t base = (uint64_t)b * a.S;             // first event this tile looks at
+  if (misc->skip != 0u || tile_i >= a.maxt) { seg_failed = tile_i >= a.maxt; break; }
+  const uint64_t base = tile_at & ~7ull;               // window start: aligned for the 128-bit loads
+  const uint32_t skp = (uint32_t)(tile_at - base);     // window positions below skp belong to the previous tile
   const uint64_t avail = a.n - base;                   // > 0 by construction
   const uint32_t cnt = avail < (uint64_t)T ? (uint32_t)avail : (uint32_t)T;  // events readable
-  const uint32_t p0 = tid * IPT;                       // this thread's 8 tile-relative positions
-  const uint32_t P32 = (uint32_t)a.P;
+  const uint32_t e_rel = seg_end - base > (uint64_t)T ? kNone : (uint32_t)(seg_end - base);   // segment end in the window
+  const uint32_t p0 = tid * IPT;                       // this thread's 8 window positions
 
   // ---- load ToA (2 events per 128-bit load) ----------------------------------------------------
   uint64_t toa_r[IPT];
@@ -282,12 +296,13 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 #pragma unroll
     for (int j = 0; j < IPT; ++j) toa_r[j] = (p0 + j < cnt) ? a.toa[base + p0 + j] : 0ull;
   }
-  // the event just before this warp's first one (lanes > 0 get it from the previous lane)
+  // the event just before this warp's first one (lanes > 0 get it from the previous lane); only the segment's
+  // first tile needs it: a later tile starts at a known shot start
   uint64_t t_prev = 0;
-  const bool has_prev = lane == 0 && p0 < cnt && base + p0 > 0;
+  const bool has_prev = lane == 0 && p0 < cnt && base + p0 > 0 && !(at_start && p0 <= skp);
   if (has_prev) t_prev = a.toa[base + p0 - 1];
   // reference time of the tile: start of the shot its first event belongs to
-  const uint64_t s_base = div64(a.toa[base], a.divP);
+  const uint64_t s_base = div64(a.toa[tile_at], a.divP);
   const uint64_t ref = s_base * a.P;
 
   // ---- shot offsets and times of flight; shot boundaries ----------------------------------------
@@ -296,7 +311,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 #pragma unroll
   for (int j = 0; j < IPT; ++j) {
     const uint64_t r64 = toa_r[j] - ref;
-    const bool in = p0 + j < cnt;
+    const bool in = p0 + j < cnt && p0 + j >= skp;
     const uint32_t rel = in ? (uint32_t)r64 : 0u;
     sl[j] = div32(rel, a.divP32);
     tof[j] = rel - sl[j] * P32;
@@ -325,40 +340,44 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   uint32_t bnd = 0;  // bit j: event p0+j starts a shot
   bool viol = false;
   {
-    if (p0 < cnt) {
-      if (start0) bnd |= 1u;
-      if (viol0 && p0 < a.S) viol = true;            // each position is checked by exactly one tile
+    if (p0 < cnt && p0 >= skp) {
+      if (start0 || (at_start && p0 == skp)) bnd |= 1u;
+      if (viol0 && !(at_start && p0 == skp)) viol = true;
     }
 #pragma unroll
     for (int j = 1; j < IPT; ++j) {
-      if (p0 + j < cnt) {
-        if (sl[j] != sl[j - 1]) bnd |= 1u << j;
-        if (sl[j] < sl[j - 1] && p0 + j < a.S) viol = true;
+      if (p0 + j < cnt && p0 + j >= skp) {
+        const bool first = at_start && p0 + j == skp;   // the known shot start of a chained tile
+        if (first || sl[j] != sl[j - 1]) bnd |= 1u << j;
+        if (!first && sl[j] < sl[j - 1]) viol = true;
       }
     }
   }
-  // lo = first shot start in [0, S); hi = first shot start in [S, cnt) (or cnt == end of stream)
+  // lo = first shot start of the window; last = the last one; hi = the first one at or after the segment's end
   {
-    uint32_t my_lo = kNone, my_hi = kNone, mt = 0, ml = 0, mn = kNone;
+    uint32_t my_lo = kNone, my_hi = kNone, my_last = 0, mt = 0, ml = 0, mn = kNone;
 #pragma unroll
     for (int j = IPT - 1; j >= 0; --j) {
       if (bnd & (1u << j)) {
-        if (p0 + j < a.S) my_lo = p0 + j;
-        else my_hi = p0 + j;
+        my_lo = p0 + j;
+        if (p0 + j >= e_rel) my_hi = p0 + j;
+        my_last = max(my_last, p0 + (uint32_t)j);
       }
       mt = max(mt, tof[j]);
       ml = max(ml, sl[j]);
-      if (p0 + j < cnt) mn = min(mn, tof[j]);
+      if (p0 + j < cnt && p0 + j >= skp) mn = min(mn, tof[j]);
     }
     mn = __reduce_min_sync(0xffffffffu, mn);
     my_lo = __reduce_min_sync(0xffffffffu, my_lo);
     my_hi = __reduce_min_sync(0xffffffffu, my_hi);
+    my_last = __reduce_max_sync(0xffffffffu, my_last);
     mt = __reduce_max_sync(0xffffffffu, mt);
     ml = __reduce_max_sync(0xffffffffu, ml);
     const uint32_t any_bad = __any_sync(0xffffffffu, bad || viol);
     if (lane == 0) {
       if (my_lo != kNone) atomicMin(&misc->lo, my_lo);
       if (my_hi != kNone) atomicMin(&misc->hi, my_hi);
+      if (my_last) atomicMax(&misc->last, my_last);
       if (mt) atomicMax(&misc->max_tof, mt);
       if (mn != kNone) atomicMin(&misc->min_tof, mn);
       if (ml) atomicMax(&misc->max_sl, ml);
@@ -376,13 +395,30 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     static_assert(2 * T / 16 <= THREADS, "counter clear");
   }
   __syncthreads();
-  uint32_t lo = misc->lo, hi = misc->hi;
+  // Owned range [lo, hi) of the window: whole shots that start before the segment's end and end inside the
+  // window. The end of the stream counts as a shot start.
+  uint32_t lo = misc->lo, hi;
   bool failed = misc->fail != 0;
-  if (hi == kNone) {
-    if (base + cnt >= a.n) hi = cnt;                      // the stream ends inside this tile's window
-    else if (lo != kNone) { hi = lo; failed = true; }     // last shot longer than the window
+  uint64_t next_at;               // where the next tile of this segment starts (>= seg_end: none)
+  {
+    const bool to_end = base + cnt >= a.n;
+    const uint32_t last = to_end ? cnt : misc->last;          // misc->last >= lo whenever lo exists
+    if (lo == kNone) {            // no shot starts in this window: nothing owned, look further on
+      lo = hi = 0;
+      next_at = base + cnt;
+    } else if (lo >= e_rel) {     // the first shot start belongs to the next segment
+      hi = lo;
+      next_at = seg_end;
+    } else {
+      hi = min(last, misc->hi);   // misc->hi: kNone when the segment's end is not in sight
+      next_at = base + hi;
+      if (hi == lo) {             // not even the first shot ends inside the window
+        if (lo > skp) next_at = base + lo;     // start again with the window at that shot's start
+        else failed = true;                    // a shot longer than the window
+      }
+    }
+    if (to_end && next_at >= base + cnt) next_at = a.n;
   }
-  if (lo == kNone) { lo = 0; hi = 0; }                    // no shot starts in this slice: nothing owned
   // key layout: 2^tb > max tof + W, so keys of different shots differ by more than W
   const uint32_t tspan = misc->max_tof + a.W;
   const uint32_t tb = tspan ? 32u - (uint32_t)__clz(tspan) : 0u;
@@ -497,20 +533,155 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     if (cl_loose) misc->loose = 1u;
   }
 
-  // ---- S1: stable LSD radix sort of local indices by (shot offset, tof) (only if needed) --------
+  // ---- S1: stable order of the owned events by (shot offset, tof) (only if needed) -------------------
   uint2* recA = reinterpret_cast<uint2*>(smem + L::kRegA);
   if (unsorted) {
     uint16_t* buf0 = reinterpret_cast<uint16_t*>(smem + L::kRegX);
     uint16_t* buf1 = buf0 + T;
+    // sort key without the gap between the tof bits and the shot bits
+    const uint32_t tofb = misc->max_tof ? 32u - (uint32_t)__clz(misc->max_tof) : 1u;
+    const uint32_t key_bits = tofb + sbits;
+    const uint16_t* fin;
+    // (a) Rank by counting. What has to be computed is the RANK of every event among the composite values
+    // (key, input position), which are all different, so nothing here needs to be stable. Detector streams hold
+    // few distinct keys per tile (time of flight is quantised and bunched: 5 mass peaks of about 100 ticks on
+    // config 4), so: bitmap of the keys that occur (region A, already zero) -> dense key number by a prefix
+    // popcount -> events per dense key (shared-memory atomics; the returned value is the event's arrival slot
+    // inside its key group) -> offsets by an exclusive scan -> the few events of one key are ordered by input
+    // position with a count of smaller positions. About 60 thread instructions per event; the two-pass LSD sort
+    // below (one ballot per digit bit) took 42 % of the kernel's instructions on config 4 (profiles/r02_*).
+    constexpr uint32_t kBitmapBits = 32u * (uint32_t)T;           // 4T bytes of region A
+    constexpr uint32_t kGroupMax = 64u;                            // larger key groups: LSD (keeps the step O(n))
+    uint32_t* bitmap = reinterpret_cast<uint32_t*>(smem + L::kRegA);             // [T] words
+    uint16_t* wpre = reinterpret_cast<uint16_t*>(smem + L::kRegA + 4 * T);       // [T] dense number of a word's first key
+    uint32_t* gcnt = reinterpret_cast<uint32_t*>(smem + L::kRegX + 4 * T);       // [T + 32] u16 pairs: events per dense key
+    uint16_t* gbase = reinterpret_cast<uint16_t*>(smem + L::kRegX + 4 * T);
+    bool counted = key_bits <= 31u && (1u << key_bits) <= kBitmapBits;
+    if (counted) {
+      const uint32_t nwords = ((1u << key_bits) + 31u) >> 5;
+      uint32_t sk_r[IPT];
+#pragma unroll
+      for (int j = 0; j < IPT; ++j) {
+        const uint32_t k = (uint32_t)j * THREADS + tid;
+        uint32_t sk = 0;
+        if (k < mm) {
+          const uint32_t key = recB[lo + k].x;
+          sk = ((key >> tb) << tofb) | (key & tmask);
+          atomicOr(&bitmap[sk >> 5], 1u << (sk & 31u));
+        }
+        sk_r[j] = sk;
+      }
+      __syncthreads();
+      {   // dense key numbers: exclusive prefix popcount over the bitmap words, 8 consecutive words per thread
+        uint32_t c[IPT], sum = 0;
+        const uint4 w0 = *reinterpret_cast<const uint4*>(bitmap + p0), w1 = *reinterpret_cast<const uint4*>(bitmap + p0 + 4);
+        const uint32_t ww[IPT] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+#pragma unroll
+        for (int j = 0; j < IPT; ++j) { c[j] = p0 + j < nwords ? (uint32_t)__popc(ww[j]) : 0u; sum += c[j]; }
+        uint32_t inc = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+          if (lane >= (uint32_t)o) inc += t;
+        }
+        if (lane == 31) misc->warp_sums[warp] = inc;
+        __syncthreads();
+        uint32_t run = inc - sum;
+        for (uint32_t w = 0; w < warp; ++w) run += misc->warp_sums[w];
+        uint32_t pk[4];
+#pragma unroll
+        for (int j = 0; j < IPT; j += 2) {
+          pk[j >> 1] = run | ((run + c[j]) << 16);
+          run += c[j] + c[j + 1];
+        }
+        *reinterpret_cast<uint4*>(wpre + p0) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+      }
+      __syncthreads();
+      uint32_t dk_r[IPT];   // dense key | arrival slot << 16
+#pragma unroll
+      for (int j = 0; j < IPT; ++j) {
+        const uint32_t k = (uint32_t)j * THREADS + tid;
+        dk_r[j] = 0;
+        if (k < mm) {
+          const uint32_t sk = sk_r[j], w = sk >> 5;
+          const uint32_t dk = (uint32_t)wpre[w] + (uint32_t)__popc(bitmap[w] & ((1u << (sk & 31u)) - 1u));
+          const uint32_t sh = (dk & 1u) * 16u;
+          const uint32_t r = (atomicAdd(&gcnt[dk >> 1], 1u << sh) >> sh) & 0xFFFFu;
+          dk_r[j] = dk | (r << 16);
+        }
+      }
+      __syncthreads();
+      bool big = false;
+      {   // offsets: exclusive scan of the counts, 8 consecutive dense keys per thread (there are at most mm <= T keys)
+        const uint4 q = *reinterpret_cast<const uint4*>(gbase + p0);
+        const uint32_t qw[4] = {q.x, q.y, q.z, q.w};
+        uint32_t c[IPT], sum = 0;
+#pragma unroll
+        for (int j = 0; j < IPT; ++j) {
+          c[j] = (qw[j >> 1] >> ((j & 1) * 16)) & 0xFFFFu;
+          sum += c[j];
+          big = big || c[j] > kGroupMax;
+        }
+        uint32_t inc = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+          if (lane >= (uint32_t)o) inc += t;
+        }
+        if (lane == 31) misc->warp_sums[warp] = inc;
+        big = __syncthreads_or(big ? 1 : 0) != 0;
+        uint32_t run = inc - sum;
+        for (uint32_t w = 0; w < warp; ++w) run += misc->warp_sums[w];
+        uint32_t pk[4];
+#pragma unroll
+        for (int j = 0; j < IPT; j += 2) {
+          pk[j >> 1] = run | ((run + c[j]) << 16);
+          run += c[j] + c[j + 1];
+        }
+        *reinterpret_cast<uint4*>(gbase + p0) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+        if (tid == THREADS - 1) gbase[T] = (uint16_t)run;     // = mm: end of the last group
+      }
+      __syncthreads();
+      if (!big) {
+        uint32_t b0_r[IPT];
+#pragma unroll
+        for (int j = 0; j < IPT; ++j) {
+          const uint32_t k = (uint32_t)j * THREADS + tid;
+          b0_r[j] = 0;
+          if (k < mm) {
+            const uint32_t dk = dk_r[j] & 0xFFFFu, r = dk_r[j] >> 16;
+            const uint32_t b0 = gbase[dk], m = (uint32_t)gbase[dk + 1u] - b0;
+            b0_r[j] = b0 | (m << 16);
+            if (m == 1u) buf1[b0] = (uint16_t)k;      // alone with its key: final position
+            else buf0[b0 + r] = (uint16_t)k;          // the group's members in arrival order
+          }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < IPT; ++j) {
+          const uint32_t k = (uint32_t)j * THREADS + tid;
+          const uint32_t b0 = b0_r[j] & 0xFFFFu, m = b0_r[j] >> 16;
+          if (k < mm && m > 1u) {
+            uint32_t c = 0;
+            for (uint32_t q = 0; q < m; ++q) c += (uint32_t)buf0[b0 + q] < k ? 1u : 0u;   // members at earlier input positions
+            buf1[b0 + c] = (uint16_t)k;
+          }
+        }
+        fin = buf1;
+      } else {
+        counted = false;      // one key held by very many events: the LSD sort below
+        for (uint32_t i = tid; i < (uint32_t)(2 * T + 64) / 4u; i += THREADS) gcnt[i] = 0u;   // its digit counters live here
+      }
+      __syncthreads();
+    }
+    if (!counted) {
+    // (b) Stable LSD radix sort of 16-bit local indices, digits ranked per warp with ballots.
     // digit counters per warp, 16 bit (a count is <= T); one thread per digit value, so up to 9-bit digits
-    // with >= 512 threads: 18 key bits (14 of time of flight + 4 of shot offset on cfg 4) take 2 passes, not 3
+    // with >= 512 threads
     constexpr uint32_t DB = THREADS >= 512 ? 9u : 8u;
     constexpr uint32_t RMAX = 1u << DB;
     uint16_t* wcnt = reinterpret_cast<uint16_t*>(smem + L::kRegX + 4 * T);  // [WARPS][RMAX]
     static_assert(WARPS * RMAX * 2 <= 4 * T && T <= 65535, "warp digit counters");
-    // sort key without the gap between the tof bits and the shot bits
-    const uint32_t tofb = misc->max_tof ? 32u - (uint32_t)__clz(misc->max_tof) : 1u;
-    const uint32_t key_bits = tofb + sbits;
     const uint32_t npass = (key_bits + DB - 1u) / DB;
     const uint32_t dbits = (key_bits + npass - 1u) / npass;         // <= DB
     const uint32_t radix = 1u << dbits, dmask = radix - 1u;
@@ -579,7 +750,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       }
       __syncthreads();
     }
-    const uint16_t* fin = (npass & 1u) ? buf1 : buf0;
+    fin = (npass & 1u) ? buf1 : buf0;
+    }
     // gather the records into sorted order (region A) and emit perm
     for (uint32_t k = tid; k < mm; k += THREADS) {
       const uint32_t s = fin[k];
@@ -1101,13 +1273,25 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     a.stage_d[o] = sf;
   }
 
-  // ---- completion: the last tile to finish publishes the outcome of the call --------------------
+  // ---- the tile's status word (tiles that own something only); on to the segment's next tile -------------
+  if (mm) {
+    if (tid == 0) a.tiles[(uint64_t)seg * a.maxt + tile_i] = ((unsigned long long)out_base << 32) | (unsigned long long)n_roots;
+    ++tile_i;
+  }
+  if (failed) { seg_failed = true; break; }
+  at_start = misc->lo != kNone;     // everything but "no shot start in sight" ends at a shot start
+  tile_at = next_at;
+  if (tile_at >= seg_end) break;
+  }   // tiles of the segment
+
+  // ---- completion: the last segment to finish publishes the outcome of the call -------------------
   if (tid == 0) {
-    a.tiles[b] = ((unsigned long long)out_base << 32) | (unsigned long long)n_roots;
-    if (failed) atomicExch(&a.ctrl->fused_fail, 1u);
+    for (uint32_t i = tile_i; i < a.maxt; ++i) a.tiles[(uint64_t)seg * a.maxt + i] = 0ull;
+    if (seg_failed) atomicExch(&a.ctrl->fused_fail, 1u);
+    if (tile_i) atomicAdd(&a.ctrl->tiles_run, tile_i);
     __threadfence();
     const uint32_t done = atomicAdd(&a.ctrl->tiles_done, 1u);
-    if (done + 1u == a.num_tiles) {
+    if (done + 1u == a.nseg) {
       __threadfence();
       const uint32_t any_fail = atomicAdd(&a.ctrl->fused_fail, 0u);
       // 2: the general kernels behind this one redo the call; 1: k_fused_compact finishes it
@@ -1207,63 +1391,89 @@ __global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, 
     a.ctrl->status.path = a.mode ? 3 : 1;
     a.ctrl->status.sort_passes = 0;
     if (a.mode == 0u) {   // worth checking the time clusters next time? (fewer than 1 tile in 8 was tight: no)
-      a.ctrl->scan_hint = a.ctrl->tight_tiles * 8u < a.num_tiles ? kScanSkip : 0u;
+      a.ctrl->scan_hint = a.ctrl->tight_tiles * 8u < a.ctrl->tiles_run ? kScanSkip : 0u;
       a.ctrl->calls += 1u;
     }
   }
 }
 
-// Which variant serves a plan: L = largest supported shot (events), T = tile capacity, S = T - L.
+// Which variant serves a plan. T = tile capacity = window length (events); a shot of up to T - 8 events fits.
 struct FusedGeom {
   int variant;      // 0 = fused path not available for this plan, 1 = T 4096 / 512 thr, 2 = T 8192 / 1024 thr,
                     // 3 = T 2048 / 256 thr (4 CTAs per SM: +2.5 % over variant 1 on cfg 1 at the same hint)
-  uint32_t T, S;
+  uint32_t T;
 };
 
 inline FusedGeom fused_geom(uint64_t P, uint32_t W, uint32_t max_shot_hits) {
-  FusedGeom g{0, 0, 0};
+  FusedGeom g{0, 0};
   if (P == 0 || P > (1ull << 24) || W >= (1u << 24)) return g;   // tof + W must fit the 32-bit tile key
   const uint32_t Lh = max_shot_hits ? max_shot_hits : 1024u;      // no hint: first rung of the ladder (below)
   if (Lh <= 512u) { g.variant = 3; g.T = 2048; }
-  else if (Lh <= 1536u) { g.variant = 1; g.T = 4096; }   // two tiles per SM beat one 8192-event tile even
-                                                           // when 60 % of a tile is overlap (cfg 2: +2.4 %)
+  else if (Lh <= 1536u) { g.variant = 1; g.T = 4096; }   // two tiles per SM beat one 8192-event tile
   else if (Lh <= 4096u) { g.variant = 2; g.T = 8192; }
   else return g;
-  g.S = (g.T - Lh) & ~7u;
   return g;
+}
+
+// Segment length and status words per segment for n events in tiles of T (host and device: the ladder's rungs
+// are sized on the device). Segments of 4 windows keep the re-read of a segment's first window at a few per
+// cent; short inputs get shorter segments so that every SM has work. Two consecutive tiles that own something
+// advance by at least T - 7 events together (what one leaves behind, at most a shot, the next one takes), hence
+// the bound on status words.
+struct FusedSegs {
+  uint32_t G, nseg, maxt;
+};
+
+__host__ __device__ inline FusedSegs fused_segs(uint64_t n, uint32_t T, uint32_t num_sms) {
+  FusedSegs s;
+  uint64_t G = 4ull * T;
+  const uint64_t want = (uint64_t)num_sms * 16ull;           // segments to aim for (load balance)
+  if (n / G < want) {
+    G = (n / want + 7ull) & ~7ull;
+    if (G < 2ull * T) G = 2ull * T;
+  }
+  s.G = (uint32_t)G;
+  s.nseg = (uint32_t)((n + G - 1) / G);
+  s.maxt = 2u * (uint32_t)(G / T + 2u) + 2u;
+  return s;
 }
 
 template <int T, int THREADS, int MODE>
 inline int launch_fused(const FusedArgs& a, cudaStream_t st) {
-  auto kern = k_fused_shot_tiles<T, THREADS, MODE>;
-  static bool configured = false;   // per process; the attribute is per function and device-wide
-  if (!configured) {
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, FusedSmem<T>::kBytes) != cudaSuccess)
-      return TPX3_ERR_CUDA;
-    configured = true;
-  }
-  kern<<<a.num_tiles, THREADS, FusedSmem<T>::kBytes, st>>>(a);
+  k_fused_shot_tiles<T, THREADS, MODE><<<a.nseg, THREADS, FusedSmem<T>::kBytes, st>>>(a);
   return cudaGetLastError() == cudaSuccess ? TPX3_OK : TPX3_ERR_CUDA;
 }
 
-// Without a hint the shot length is tried in rungs: 1024 (4096-event tiles), 2048 and 4096 (8192-event tiles).
-// A rung whose tiles meet a longer shot fails within its first wave (every later tile returns at once), and
-// k_fallback_dispatch launches the next rung from the device; after the last one the general kernels run.
-constexpr int kLadderMax = 2;   // rungs after the first
+// The opt-in to more than 48 KB of dynamic shared memory is per function AND per device: tpx3_plan calls this
+// after cudaSetDevice for its device (the 8192-event variants may also be launched from the device later on).
+inline int fused_configure_device() {
+#define TPX3_FUSED_ATTR(T, THREADS, MODE)                                                                          \
+  if (cudaFuncSetAttribute(k_fused_shot_tiles<T, THREADS, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,     \
+                           FusedSmem<T>::kBytes) != cudaSuccess)                                                  \
+    return TPX3_ERR_CUDA;
+  TPX3_FUSED_ATTR(2048, 256, 0) TPX3_FUSED_ATTR(2048, 256, 1) TPX3_FUSED_ATTR(4096, 512, 0)
+  TPX3_FUSED_ATTR(4096, 512, 1) TPX3_FUSED_ATTR(8192, 1024, 0) TPX3_FUSED_ATTR(8192, 1024, 1)
+#undef TPX3_FUSED_ATTR
+  return TPX3_OK;
+}
+
+// Without a hint the window length is tried in rungs: 4096 events, then 8192. A rung whose tiles meet a shot
+// that does not fit fails within its first wave (every later tile returns at once), and k_fallback_dispatch
+// launches the next rung from the device; after the last one the general kernels run.
+constexpr int kLadderMax = 1;   // rungs after the first
 struct FusedLadder {
-  int n;                        // rungs still to try after the one the host enqueued
-  uint32_t S[kLadderMax];       // their slice lengths (8192-event tiles)
+  int n;                        // rungs still to try after the one the host enqueued (8192-event tiles)
 };
 
 inline FusedLadder fused_ladder(uint32_t max_shot_hits) {
-  FusedLadder l{0, {0, 0}};
-  if (max_shot_hits == 0) { l.n = 2; l.S[0] = 8192u - 2048u; l.S[1] = 8192u - 4096u; }
+  FusedLadder l{0};
+  if (max_shot_hits == 0) l.n = 1;
   return l;
 }
 
-inline FusedArgs make_fused_args(uint32_t S, Ctrl* ctrl, unsigned long long* tiles, const Params& prm, const uint16_t* x,
-                                 const uint16_t* y, const uint64_t* toa, const uint16_t* tot, uint32_t* perm,
-                                 uint32_t* label, uint64_t max_clusters, const tpx3_clusters_t& out,
+inline FusedArgs make_fused_args(uint32_t T, uint32_t num_sms, Ctrl* ctrl, unsigned long long* tiles, const Params& prm,
+                                 const uint16_t* x, const uint16_t* y, const uint64_t* toa, const uint16_t* tot,
+                                 uint32_t* perm, uint32_t* label, uint64_t max_clusters, const tpx3_clusters_t& out,
                                  uint32_t* n_clusters, void* stage, uint32_t mode, uint32_t lm_wx, uint32_t lm_wy) {
   FusedArgs a;
   a.ctrl = ctrl;
@@ -1273,8 +1483,12 @@ inline FusedArgs make_fused_args(uint32_t S, Ctrl* ctrl, unsigned long long* til
   a.divP = make_div64(prm.P);
   a.divP32 = make_div32((uint32_t)prm.P);
   a.W = prm.W;
-  a.S = S;
-  a.num_tiles = (uint32_t)((prm.n + S - 1) / S);
+  const FusedSegs sg = fused_segs(prm.n, T, num_sms);
+  a.G = sg.G;
+  a.nseg = sg.nseg;
+  a.maxt = sg.maxt;
+  a.num_tiles = sg.nseg * sg.maxt;
+  a.num_sms = num_sms;
   a.sensor_w = prm.sensor_w;
   a.sensor_h = prm.sensor_h;
   a.flags = prm.flags;
@@ -1292,8 +1506,8 @@ inline FusedArgs make_fused_args(uint32_t S, Ctrl* ctrl, unsigned long long* til
   return a;
 }
 
-__host__ __device__ inline void compact_grid(uint32_t num_tiles, uint32_t* ctas, uint32_t* tiles_per_cta) {
-  uint32_t c = num_tiles < (uint32_t)(kNumSMs * 8) ? num_tiles : (uint32_t)(kNumSMs * 8);
+__host__ __device__ inline void compact_grid(uint32_t num_tiles, uint32_t num_sms, uint32_t* ctas, uint32_t* tiles_per_cta) {
+  uint32_t c = num_tiles < num_sms * 8u ? num_tiles : num_sms * 8u;
   if (c == 0) c = 1;
   const uint32_t t = (num_tiles + c - 1) / c;
   *tiles_per_cta = t ? t : 1u;
@@ -1303,17 +1517,17 @@ __host__ __device__ inline void compact_grid(uint32_t num_tiles, uint32_t* ctas,
 // Device side: the next rung (8192-event tiles), tail-launched by k_fallback_dispatch.
 __device__ inline void launch_fused_rung_device(FusedArgs a) {
   uint32_t ctas, tpc;
-  compact_grid(a.num_tiles, &ctas, &tpc);
+  compact_grid(a.num_tiles, a.num_sms, &ctas, &tpc);
   if (a.mode == 0u)
-    k_fused_shot_tiles<8192, 1024, 0><<<a.num_tiles, 1024, FusedSmem<8192>::kBytes, cudaStreamTailLaunch>>>(a);
+    k_fused_shot_tiles<8192, 1024, 0><<<a.nseg, 1024, FusedSmem<8192>::kBytes, cudaStreamTailLaunch>>>(a);
   else
-    k_fused_shot_tiles<8192, 1024, 1><<<a.num_tiles, 1024, FusedSmem<8192>::kBytes, cudaStreamTailLaunch>>>(a);
+    k_fused_shot_tiles<8192, 1024, 1><<<a.nseg, 1024, FusedSmem<8192>::kBytes, cudaStreamTailLaunch>>>(a);
   k_fused_compact<<<ctas, kCompactThreads, 0, cudaStreamTailLaunch>>>(a, tpc);
 }
 
 // Host side. Returns TPX3_OK (launched or not applicable; *launched says which) or an error. *args receives the
-// arguments of the enqueued rung (the later rungs differ in S and num_tiles only).
-inline int enqueue_fused(const FusedGeom& g, uint64_t* launches, Ctrl* ctrl, unsigned long long* tiles,
+// arguments of the enqueued rung (the later rungs differ in the segment geometry only).
+inline int enqueue_fused(const FusedGeom& g, uint32_t num_sms, uint64_t* launches, Ctrl* ctrl, unsigned long long* tiles,
                          cudaStream_t st, const Params& prm, const uint16_t* x, const uint16_t* y,
                          const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label,
                          uint64_t max_clusters, const tpx3_clusters_t& out, uint32_t* n_clusters, void* stage,
@@ -1322,19 +1536,9 @@ inline int enqueue_fused(const FusedGeom& g, uint64_t* launches, Ctrl* ctrl, uns
   if (g.variant == 0 || prm.n == 0) return TPX3_OK;
   // the 128-bit load phase needs 16-byte aligned inputs (PyTorch allocations are 256-byte aligned)
   if ((((uintptr_t)x | (uintptr_t)y | (uintptr_t)toa | (uintptr_t)tot) & 15u) != 0) return TPX3_OK;
-  const FusedArgs a = make_fused_args(g.S, ctrl, tiles, prm, x, y, toa, tot, perm, label, max_clusters, out, n_clusters,
-                                      stage, mode, lm_wx, lm_wy);
+  const FusedArgs a = make_fused_args(g.T, num_sms, ctrl, tiles, prm, x, y, toa, tot, perm, label, max_clusters, out,
+                                      n_clusters, stage, mode, lm_wx, lm_wy);
   *args = a;
-  // the 8192-event variants may be launched from the device later on: their attribute must be set by then
-  static bool ladder_configured = false;
-  if (!ladder_configured) {
-    if (cudaFuncSetAttribute(k_fused_shot_tiles<8192, 1024, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             FusedSmem<8192>::kBytes) != cudaSuccess ||
-        cudaFuncSetAttribute(k_fused_shot_tiles<8192, 1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             FusedSmem<8192>::kBytes) != cudaSuccess)
-      return TPX3_ERR_CUDA;
-    ladder_configured = true;
-  }
   int rc;
   if (mode == 0u)
     rc = g.variant == 3 ? launch_fused<2048, 256, 0>(a, st)
@@ -1345,7 +1549,7 @@ inline int enqueue_fused(const FusedGeom& g, uint64_t* launches, Ctrl* ctrl, uns
   if (rc != TPX3_OK) return rc;
   ++*launches;
   uint32_t ctas, tiles_per_cta;
-  compact_grid(a.num_tiles, &ctas, &tiles_per_cta);
+  compact_grid(a.num_tiles, num_sms, &ctas, &tiles_per_cta);
   k_fused_compact<<<ctas, kCompactThreads, 0, st>>>(a, tiles_per_cta);
   if (cudaGetLastError() != cudaSuccess) return TPX3_ERR_CUDA;
   ++*launches;

@@ -38,6 +38,7 @@ struct tpx3_plan_s {
   uint64_t profiled_calls;
   cudaStream_t copy_in, copy_out;   // copy streams of the pipelined tpx3_process_host (created on first use)
   int host_route;           // last tpx3_process_host: 0 one piece, 1 pipelined, 2 pipelined attempt redone in one piece
+  bool device_ready;        // use_device has run for this plan
 };
 
 namespace {
@@ -228,9 +229,9 @@ __global__ void k_fallback_dispatch(GenArgs a, FusedArgs fa, FusedLadder ladder,
   Ctrl* c = a.w.ctrl;
   if (c->fused_state == 1u) return;
   if (rung < ladder.n) {
-    c->tiles_done = 0; c->fused_fail = 0; c->fused_state = 0;
-    fa.S = ladder.S[rung];
-    fa.num_tiles = (uint32_t)((fa.n + fa.S - 1) / fa.S);
+    c->tiles_done = 0; c->fused_fail = 0; c->fused_state = 0; c->tight_tiles = 0; c->tiles_run = 0;
+    const FusedSegs sg = fused_segs(fa.n, 8192u, fa.num_sms);
+    fa.G = sg.G; fa.nseg = sg.nseg; fa.maxt = sg.maxt; fa.num_tiles = sg.nseg * sg.maxt;
     launch_fused_rung_device(fa);
     k_fallback_dispatch<<<1, 1, 0, cudaStreamTailLaunch>>>(a, fa, ladder, rung + 1, lm);
     return;
@@ -320,6 +321,24 @@ int enqueue_centroid(tpx3_plan_s* p, const GenArgs& a, cudaStream_t st) {
   return cuda_ok(cudaGetLastError());
 }
 
+// Every device call starts here: makes the plan's device current and, the first time for a plan, reads its SM
+// count and opts the fused kernels in to their dynamic shared memory. The opt-in is per function AND per device,
+// so it is tied to the plan (one plan = one device), not to the process; tpx3_plan itself stays host-only.
+// Concurrent first calls on one plan are the caller's to serialise (a plan is not thread-safe anyway: it counts
+// launches); the work is idempotent.
+int use_device(tpx3_plan_s* p) {
+  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  if (!p->device_ready) {
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->cfg.device) != cudaSuccess || sms <= 0)
+      return TPX3_ERR_CUDA;
+    if (fused_configure_device() != TPX3_OK) return TPX3_ERR_CUDA;
+    p->num_sms = sms;
+    p->device_ready = true;
+  }
+  return TPX3_OK;
+}
+
 bool clusters_ok(const tpx3_clusters_t* o) {
   return o && o->label && o->size && o->shot && o->sum_tot && o->sum_tot_x && o->sum_tot_y && o->toa_peak && o->cx &&
          o->cy && o->sum_tot_tof && o->ctof;
@@ -345,7 +364,8 @@ int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace
   p->profiled_calls = 0;
   p->copy_in = p->copy_out = nullptr;
   p->host_route = 0;
-  p->num_sms = kNumSMs;
+  p->num_sms = kNumSMs;      // until the first device call reads the device's count (use_device)
+  p->device_ready = false;
   Params& prm = p->prm;
   prm.n = 0;
   prm.P = cfg->shot_period_ticks;
@@ -374,7 +394,7 @@ int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace
   p->off_slot = p->off_keyA;                    // 4N <= 8N
   p->off_peak = p->off_keyB;                    // 8N
   p->off_blkcnt = p->off_idxA;                  // 4 * ceil(N/4096) <= 4N
-  p->off_tiles = o; o = align_up(o + 8 * (size_t)(N / 1024 + 1024));  // fused path tile status words (S >= 3072)
+  p->off_tiles = o; o = align_up(o + 8 * (size_t)(N / 256 + 65536));   // fused path tile status words (fused_segs: nseg * maxt)
   p->workspace_bytes = o;
   *workspace_bytes = o;
   *out_plan = p;
@@ -387,7 +407,7 @@ int tpx3_cluster(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, 
   if (n > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
   if (n && (!x || !y || !toa || !tot || !perm || !label)) return TPX3_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
   Ws w = carve(p, workspace);
   if (p->profiling) ++p->profiled_calls;
   TPX3_LAUNCH(p, k_ctrl_init, 1, 256, 0, st, w.ctrl, n, w.tiles, 0u, n_clusters);
@@ -405,7 +425,7 @@ int tpx3_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n,
   if (max_clusters && !clusters_ok(out)) return TPX3_ERR_INVALID_ARG;
   if (n && !out) return TPX3_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
   Ws w = carve(p, workspace);
   if (p->profiling) ++p->profiled_calls;
   TPX3_LAUNCH(p, k_ctrl_init, 1, 256, 0, st, w.ctrl, n, w.tiles, 0u, n_clusters);
@@ -423,13 +443,11 @@ int tpx3_cluster_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uin
   if (n && (!x || !y || !toa || !tot || !perm || !label || !out)) return TPX3_ERR_INVALID_ARG;
   if (max_clusters && !clusters_ok(out)) return TPX3_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
   Ws w = carve(p, workspace);
   if (p->profiling) ++p->profiled_calls;
   const bool try_fused = !(p->cfg.flags & TPX3_FLAG_FORCE_GENERAL) && p->fused.variant != 0 && n != 0;
-  const uint32_t num_tiles = try_fused ? (uint32_t)((n + p->fused.S - 1) / p->fused.S) : 0u;
-  TPX3_LAUNCH(p, k_ctrl_init, num_tiles > 256 * 64 ? 64 : (num_tiles + 255) / 256 + 1, 256, 0, st, w.ctrl, n, w.tiles,
-              num_tiles, n_clusters);
+  TPX3_LAUNCH(p, k_ctrl_init, 1, 256, 0, st, w.ctrl, n, w.tiles, 0u, n_clusters);
   if (n == 0) return cuda_ok(cudaGetLastError());
   Params prm = p->prm;
   prm.n = n;
@@ -439,7 +457,7 @@ int tpx3_cluster_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uin
     bool launched = false;
     StageTimer timer(p, st, TPX3_STAGE_FUSED);
     FusedArgs fa;
-    rc = enqueue_fused(p->fused, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, label, max_clusters,
+    rc = enqueue_fused(p->fused, (uint32_t)p->num_sms, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, label, max_clusters,
                        *out, n_clusters, (char*)workspace + p->off_keyA, &launched, &fa);
     if (rc != TPX3_OK) return rc;
     if (launched) {
@@ -463,13 +481,11 @@ int tpx3_localmax_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, ui
   if (n && (!x || !y || !toa || !tot || !perm || !lmax || !out)) return TPX3_ERR_INVALID_ARG;
   if (max_clusters && !clusters_ok(out)) return TPX3_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
   Ws w = carve(p, workspace);
   if (p->profiling) ++p->profiled_calls;
   const bool lm_fused = !(p->cfg.flags & TPX3_FLAG_FORCE_GENERAL) && p->fused.variant != 0 && wt < (1u << 24) && n != 0;
-  const uint32_t num_tiles = lm_fused ? (uint32_t)((n + p->fused.S - 1) / p->fused.S) : 0u;
-  TPX3_LAUNCH(p, k_ctrl_init, num_tiles > 256 * 64 ? 64 : (num_tiles + 255) / 256 + 1, 256, 0, st, w.ctrl, n, w.tiles,
-              num_tiles, n_hits);
+  TPX3_LAUNCH(p, k_ctrl_init, 1, 256, 0, st, w.ctrl, n, w.tiles, 0u, n_hits);
   if (n == 0) return cuda_ok(cudaGetLastError());
   GenArgs ga = make_gen_args(p, w, 0, n, x, y, toa, tot, perm, lmax, max_clusters, out, n_hits);
   ga.lm_wx = wx; ga.lm_wy = wy; ga.lm_wt = wt;
@@ -482,7 +498,7 @@ int tpx3_localmax_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, ui
     bool launched = false;
     StageTimer timer(p, st, TPX3_STAGE_FUSED);
     FusedArgs fa;
-    int rc = enqueue_fused(p->fused, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, lmax, max_clusters,
+    int rc = enqueue_fused(p->fused, (uint32_t)p->num_sms, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, lmax, max_clusters,
                            *out, n_hits, (char*)workspace + p->off_keyA, &launched, &fa, 1u, wx > 255u ? 255u : wx,
                            wy > 255u ? 255u : wy);
     if (rc != TPX3_OK) return rc;
@@ -502,7 +518,7 @@ int tpx3_unwrap_toa(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t 
   if (n > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
   if (n && (!raw || !toa_out)) return TPX3_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
   Ws w = carve(p, workspace);
   UnwrapArgs a;
   a.n = n; a.raw = raw; a.modulus = modulus; a.jump = jump; a.wraps_in = (long long)wraps_in;
@@ -536,7 +552,7 @@ int tpx3_preprocess(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t 
   if (n && (!x || !y || !toa || !tot || !x_out || !y_out || !toa_out || !tot_out)) return TPX3_ERR_INVALID_ARG;
   if ((n_trig && !trig) || (table_len && !table)) return TPX3_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
   Ws w = carve(p, workspace);
   PreArgs a;
   a.n = n; a.x = x; a.y = y; a.tot = tot; a.toa = toa; a.n_trig = n_trig; a.trig = trig; a.cut = cut;
@@ -596,7 +612,7 @@ int tpx3_stream_open(tpx3_plan_t p, void* stream_buf, uint64_t max_chunk, uint64
   if (!p || !stream_buf || !out) return TPX3_ERR_INVALID_ARG;
   if (p->cfg.shot_period_ticks == 0 || max_chunk == 0 || max_carry == 0) return TPX3_ERR_INVALID_ARG;
   if (max_chunk + max_carry > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
-  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
   tpx3_stream_s* s = new (std::nothrow) tpx3_stream_s();
   if (!s) return TPX3_ERR_CUDA;
   const StreamLayout l = stream_layout(max_chunk, max_carry);
@@ -626,7 +642,7 @@ int tpx3_stream_push(tpx3_stream_t s, void* workspace, void* cuda_stream, uint64
   if (n && (!x || !y || !toa || !tot)) return TPX3_ERR_INVALID_ARG;
   tpx3_plan_t p = s->plan;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
   tpx3::StreamArgs a;
   a.c = s->ctrl; a.n = n; a.n_carry = s->n_carry; a.carry_cap = (uint32_t)s->max_carry;
   a.x = x; a.y = y; a.tot = tot; a.toa = toa;
@@ -655,7 +671,7 @@ int tpx3_stream_push(tpx3_stream_t s, void* workspace, void* cuda_stream, uint64
                                  s->wlabel, max_clusters, out, n_hits);
   if (rc != TPX3_OK) return rc;
   if (h.n_work && max_clusters)
-    TPX3_LAUNCH(p, tpx3::k_stream_labels, 148, 256, 0, st, s->ctrl, n_hits, max_clusters, out->label);
+    TPX3_LAUNCH(p, tpx3::k_stream_labels, p->num_sms, 256, 0, st, s->ctrl, n_hits, max_clusters, out->label);
   return cuda_ok(cudaGetLastError());
 }
 
@@ -841,7 +857,7 @@ int tpx3_process_host(tpx3_plan_t p, void* workspace, void* device_io, void* cud
   if (n > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
   if (n && (!x || !y || !toa || !tot)) return TPX3_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
   const HostIo io = host_io_layout((char*)device_io, n, max_clusters);
   cudaError_t e = cudaSuccess;
   bool resident = false;
@@ -884,7 +900,7 @@ int tpx3_host_route(tpx3_plan_t p) { return p ? p->host_route : TPX3_ERR_INVALID
 int tpx3_status(tpx3_plan_t p, const void* workspace, void* cuda_stream, tpx3_status_t* out) {
   if (!p || !workspace || !out) return TPX3_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
   if (cudaMemcpyAsync(out, workspace, sizeof(tpx3_status_t), cudaMemcpyDeviceToHost, st) != cudaSuccess)
     return TPX3_ERR_CUDA;
   if (cudaStreamSynchronize(st) != cudaSuccess) return TPX3_ERR_CUDA;
@@ -895,14 +911,14 @@ uint64_t tpx3_launch_count(tpx3_plan_t p) { return p ? p->launches : 0; }
 
 int tpx3_profile_enable(tpx3_plan_t p, int enable) {
   if (!p) return TPX3_ERR_INVALID_ARG;
-  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
   p->profiling = enable != 0;
   return TPX3_OK;
 }
 
 int tpx3_profile_read(tpx3_plan_t p, tpx3_profile_t* out) {
   if (!p || !out) return TPX3_ERR_INVALID_ARG;
-  if (cudaSetDevice(p->cfg.device) != cudaSuccess) return TPX3_ERR_CUDA;
+  if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
   memset(out, 0, sizeof(*out));
   int rc = TPX3_OK;
   for (auto& s : p->spans) {

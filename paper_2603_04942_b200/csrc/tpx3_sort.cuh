@@ -44,7 +44,7 @@ __global__ void __launch_bounds__(256) k_ctrl_init(Ctrl* c, uint64_t n, unsigned
     c->status.error = 0; c->status.path = 0; c->status.n_clusters = 0; c->status.sort_passes = 0;
     c->status.n = n;
     c->toa_min = ~0ull; c->toa_max = 0ull; c->npass = 1; c->fused_state = 0; c->tile_ticket = 0; c->n_roots = 0;
-    c->tiles_done = 0; c->fused_fail = 0; c->tight_tiles = 0;
+    c->tiles_done = 0; c->fused_fail = 0; c->tight_tiles = 0; c->tiles_run = 0;
     if (n_clusters) *n_clusters = 0;
   }
   for (uint32_t t = i; t < num_tiles; t += gridDim.x * blockDim.x) tiles[t] = 0ull;
