@@ -251,9 +251,14 @@ def run_ours(args):
     lm = args.mode == "localmax"
     wx, wy, wt = args.window
 
+    split = args.mode == "split"
+
     def step():
         if lm:   # paper-literal mode: local ToT maxima + box centroid
             pl.localmax_centroid(*dev, wx, wy, wt, cl, perm=perm, lmax=label, n_hits=nc, stream=stream)
+        elif split:   # the two calls BASELINE.json north_star names: tpx3_cluster (S0-S3), then tpx3_centroid (S4-S5)
+            pl.cluster(*dev, perm=perm, label=label, n_clusters=nc, stream=stream)
+            pl.centroid(*dev, perm, label, cl, n_clusters=nc, stream=stream)
         else:
             pl.cluster_centroid(*dev, cl, perm=perm, label=label, n_clusters=nc, stream=stream)
 
@@ -360,20 +365,22 @@ def run_ours(args):
         stream.synchronize()
         return k
 
-    for _ in range(2):
-        e2e_step()
-    barrier()
-    e2e_steps = max(1, min(args.steps, 5))
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        ncl_e2e = e2e_step()
-    torch.cuda.synchronize()
-    e2e_s = (time.perf_counter() - t0) / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    assert ncl_e2e == ncl, (ncl_e2e, ncl)
+    e2e_s = None
+    if not args.no_e2e:
+        for _ in range(2):
+            e2e_step()
+        barrier()
+        e2e_steps = max(1, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            ncl_e2e = e2e_step()
+        torch.cuda.synchronize()
+        e2e_s = (time.perf_counter() - t0) / e2e_steps
+        if world > 1:
+            t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_s = float(t.item())
+        assert ncl_e2e == ncl, (ncl_e2e, ncl)
     if rank == 0:
         sampler.stop()
     if rank != 0:
@@ -383,7 +390,7 @@ def run_ours(args):
 
     # ---- roofline of the dominant stage (CUDA-event time per stage, recorded on `stream`) ------
     peak, peak_src = measured_peak()
-    stage_ms = {k: v / max(prof["calls"], 1) for k, v in prof["ms"].items()}
+    stage_ms = {k: v / max(args.steps, 1) for k, v in prof["ms"].items()}   # per step (a step may be two calls)
     dom = max(stage_ms, key=lambda k: stage_ms[k])
     dom_bytes = STAGE_BYTES[dom](n, ncl)
     dom_gbs = dom_bytes / (stage_ms[dom] * 1e-3) / 1e9 if stage_ms[dom] > 0 else 0.0
@@ -394,7 +401,7 @@ def run_ours(args):
                                    "centroid": "centroid stage"}[dom],
         "achieved": dom_gbs, "peak": peak, "unit": "GB/s", "frac": dom_gbs / peak, "traffic": None,
         "peak_source": peak_src, "algorithmic_bytes_per_launch": dom_bytes,
-        "stage_ms": stage_ms, "stage_launches": {k: v / max(prof["calls"], 1) for k, v in prof["launches"].items()},
+        "stage_ms": stage_ms, "stage_launches": {k: v / max(args.steps, 1) for k, v in prof["launches"].items()},
         "whole_path": {"algorithmic_bytes_per_step": whole_bytes,
                        "achieved": whole_bytes / (ms_step * 1e-3) / 1e9 * (n_all / max(n, 1)) / max(world, 1),
                        "frac": whole_bytes / (ms_step * 1e-3) / 1e9 / peak},
@@ -432,7 +439,7 @@ def run_ours(args):
         "dtype": "int64", "data": "synthetic",
         "config": {
             "workload": w.name, "mode": ("paper-literal local maxima, box (wx, wy, wt) = (%d, %d, %d)" % (wx, wy, wt))
-            if lm else "connected components (north_star)", "shots_per_gpu": w.shots, "pixel_hits_per_gpu": n, "particle_hits_per_gpu": ncl,
+            if lm else ("connected components, tpx3_cluster then tpx3_centroid (two calls)" if split else "connected components (north_star)"), "shots_per_gpu": w.shots, "pixel_hits_per_gpu": n, "particle_hits_per_gpu": ncl,
             "pixel_hits_total": n_all, "particle_hits_total": ncl_all, "toa_window_ticks": w.toa_window_ticks,
             "shot_period_ticks": w.shot_period_ticks, "path": {1: "fused", 2: "general", 3: "localmax"}.get(st["path"], st["path"]),
             "sort_passes": st["sort_passes"], "max_shot_hits": cfg.max_shot_hits, "parallelism": "shots sharded over %d gpu(s), no collective" % world,
@@ -441,7 +448,7 @@ def run_ours(args):
             "input_hash": {"toa": __import__("gen").array_hash(w.toa), "x": __import__("gen").array_hash(w.x)},
         },
         "particle_hits_per_s": ncl_all / (ms_step * 1e-3),
-        "e2e": {"value": n_all / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+        "e2e": None if e2e_s is None else {"value": n_all / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_s * 1e3, "route": {0: "one piece", 1: "pipelined in 2^22-event chunks", 2: "pipelined attempt redone in one piece"}.get(pl.host_route()) if not lm else None, "api": "tpx3_process_host (pinned host buffers; cluster table copied "
                 "back, perm/label left on the device)" if not lm else "pinned H2D copies + tpx3_localmax_centroid + "
                 "D2H of the count and the hit table"},
@@ -644,11 +651,12 @@ def main():
                     help="tile-size hint for the plan (default: the workload recipe's bound on hits per shot)")
     ap.add_argument("--chunk", type=int, default=1 << 22, help="--mode stream: events per push")
     ap.add_argument("--max-carry", type=int, default=1 << 20, help="--mode stream: carry capacity in events")
-    ap.add_argument("--mode", choices=("components", "localmax", "stream", "unwrap", "preprocess"), default="components",
+    ap.add_argument("--mode", choices=("components", "split", "localmax", "stream", "unwrap", "preprocess"), default="components",
                     help="components: the hot path (default). localmax: the paper-literal mode, SURVEY 8f NEXT #2")
     ap.add_argument("--window", type=int, nargs=3, default=(2, 2, 320), metavar=("WX", "WY", "WT"),
                     help="box half-widths of --mode localmax (pixels, pixels, ticks)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="development only: skip the end-to-end (host buffer) leg")
     ap.add_argument("--no-sweep", action="store_true", help="cfg4 workloads: skip the smaller chunk sizes")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     args = ap.parse_args()

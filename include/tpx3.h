@@ -68,12 +68,13 @@ typedef struct {
   int32_t device;              /* CUDA device ordinal                                          */
   uint32_t flags;              /* TPX3_FLAG_*                                                  */
   uint32_t max_shot_hits;      /* hint: most events one shot can hold; sizes the fused path's
-                                  tiles. <= 512: 2048-event tiles, 4 CTAs per SM; <= 1536:
-                                  4096-event tiles, 2 CTAs per SM; <= 4096: 8192-event tiles;
-                                  larger, or a shot that exceeds the hint: the general path
-                                  runs (same results, slower). 0 = no hint: 1024, then 2048,
-                                  then 4096 are tried on the device (a failed try stops within
-                                  its first wave of tiles), then the general path.             */
+                                  tile windows. <= 1536: 2048-event windows, 4 CTAs per SM;
+                                  <= 3584: 4096 events, 2 CTAs per SM; <= 8184: 8192 events;
+                                  larger, or a shot that does not fit the window: the general
+                                  path runs (same results, slower). 0 = no hint: windows of
+                                  2048, then 4096, then 8192 events are tried on the device (a
+                                  failed try stops within its first wave of tiles), then the
+                                  general path.                                                */
   uint32_t reserved;           /* must be 0                                                    */
 } tpx3_config_t;
 

@@ -157,7 +157,7 @@ class Config:
     max_hits: int = 1 << 20
     device: int = 0
     flags: int = 0
-    max_shot_hits: int = 0  # hint: most events in one shot (0 = 4096); sizes the fused path's tiles
+    max_shot_hits: int = 0  # hint: most events in one shot; picks the fused path's window (0 = no hint: 2048, 4096, 8192 are tried on the device, tpx3.h)
 
 
 _CLUSTER_FIELDS = (

@@ -154,7 +154,8 @@ struct FusedArgs {
   uint4* stage_b;      //                                            {sum tot*x (lo, hi), sum tot*y (lo, hi)}
   uint64_t* stage_c;   //                                            ToA of the brightest pixel
   uint64_t* stage_d;   //                                            sum tot*tof
-  uint32_t mode;       // 0: hit = connected component (north_star); 1: paper-literal mode, hit = local ToT
+  uint32_t mode;       // (2: as 0 but S0-S3 only; 3: S4-S5 on the caller's perm / label)
+                       // 0: hit = connected component (north_star); 1: paper-literal mode, hit = local ToT
                        //    maximum of the box (lm_wx, lm_wy, W) and sums over that box (tpx3_localmax.cuh)
   uint32_t lm_wx, lm_wy;
 };
@@ -232,10 +233,16 @@ __device__ __forceinline__ void uf_unite(uint16_t* par, uint32_t a, uint32_t b) 
 }
 
 // One tile per CTA. T = tile capacity (events), THREADS = T / 8.
-// MODE 0: hit = connected component (north_star). MODE 1: paper-literal mode (FusedArgs::mode).
+// MODE 0: hit = connected component (north_star), S0-S5. MODE 1: paper-literal mode. MODE 2: S0-S3 only
+// (tpx3_cluster). MODE 3: S4-S5 on the caller's (perm, label) (tpx3_centroid): the events are read THROUGH perm,
+// in the caller's order, and the tile takes label[] as it is. (FusedArgs::mode holds the same number.)
 template <int T, int THREADS, int MODE>
 __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))) k_fused_shot_tiles(FusedArgs a) {
   constexpr int IPT = T / THREADS;  // 8 events per thread
+  constexpr bool kLM = MODE == 1;            // paper-literal mode (tpx3_localmax_centroid)
+  constexpr bool kLabelsOnly = MODE == 2;    // S0-S3 only: perm, label, hit count (tpx3_cluster)
+  constexpr bool kGiven = MODE == 3;         // S4-S5 for a given (perm, label) (tpx3_centroid): no sort, no link
+  constexpr bool kCC = MODE == 0 || MODE == 2;   // hits are connected components found here
   static_assert(IPT == 8, "the 128-bit load phase assumes 8 events per thread");
   constexpr int WARPS = THREADS / 32;
   constexpr uint32_t NB = T;        // hash buckets of 4 slots (16 bytes each)
@@ -263,7 +270,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     misc->last = 0;
     // another tile already gave up: this attempt is lost, do not spend time on it (the next attempt — a
     // variant with longer shots, or the general kernels — is enqueued behind; k_fallback_dispatch)
-    misc->skip = atomicAdd(&a.ctrl->fused_fail, 0u);
+    misc->skip = tile_at == seg_begin ? atomicAdd(&a.ctrl->fused_fail, 0u) : 0u;
     misc->fail = 0;
     misc->max_tof = 0;
     misc->loose = 0;
@@ -284,7 +291,17 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 
   // ---- load ToA (2 events per 128-bit load) ----------------------------------------------------
   uint64_t toa_r[IPT];
-  if (p0 + IPT <= cnt) {
+  if (kGiven) {     // position p of the caller's order is input event perm[p]
+    if (p0 + IPT <= cnt) {
+      const uint4 i0 = ldg_nc_v4(a.perm + base + p0), i1 = ldg_nc_v4(a.perm + base + p0 + 4);
+      const uint32_t ix[IPT] = {i0.x, i0.y, i0.z, i0.w, i1.x, i1.y, i1.z, i1.w};
+#pragma unroll
+      for (int j = 0; j < IPT; ++j) toa_r[j] = a.toa[ix[j]];
+    } else {
+#pragma unroll
+      for (int j = 0; j < IPT; ++j) toa_r[j] = (p0 + j < cnt) ? a.toa[a.perm[base + p0 + j]] : 0ull;
+    }
+  } else if (p0 + IPT <= cnt) {
     const uint4* src = reinterpret_cast<const uint4*>(a.toa + base + p0);
 #pragma unroll
     for (int j = 0; j < IPT / 2; ++j) {
@@ -300,9 +317,9 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   // first tile needs it: a later tile starts at a known shot start
   uint64_t t_prev = 0;
   const bool has_prev = lane == 0 && p0 < cnt && base + p0 > 0 && !(at_start && p0 <= skp);
-  if (has_prev) t_prev = a.toa[base + p0 - 1];
+  if (has_prev) t_prev = kGiven ? a.toa[a.perm[base + p0 - 1]] : a.toa[base + p0 - 1];
   // reference time of the tile: start of the shot its first event belongs to
-  const uint64_t s_base = div64(a.toa[tile_at], a.divP);
+  const uint64_t s_base = div64(kGiven ? a.toa[a.perm[tile_at]] : a.toa[tile_at], a.divP);
   const uint64_t ref = s_base * a.P;
 
   // ---- shot offsets and times of flight; shot boundaries ----------------------------------------
@@ -433,7 +450,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   // The time-cluster check (below) is skipped when all times of flight lie within W anyway, and when the last
   // call on this workspace found hardly any tight tile (the hint; every 16th call looks again).
   const bool cl_wide = misc->max_tof - misc->min_tof > a.W;
-  const bool cl_scan = MODE == 0 && cl_wide && (a.ctrl->scan_hint != kScanSkip || (a.ctrl->calls & 15u) == 0u);
+  const bool cl_scan = kCC && cl_wide && (a.ctrl->scan_hint != kScanSkip || (a.ctrl->calls & 15u) == 0u);
   bool uns = false;
   uint32_t cl_last_start = 0, cl_lead_last = 0;   // time-cluster check on the keys in registers
   bool cl_have_lead = false, cl_loose = false;
@@ -464,7 +481,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       }
     }
     uint4 vx, vy, vt;
-    if (p0 + IPT <= cnt) {
+    if (!kGiven && p0 + IPT <= cnt) {
       vx = ldg_nc_v4(a.x + base + p0);
       vy = ldg_nc_v4(a.y + base + p0);
       vt = ldg_nc_v4(a.tot + base + p0);
@@ -473,9 +490,10 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 #pragma unroll
       for (int j = 0; j < IPT; ++j) {
         bool ok = p0 + j < cnt;
-        tx[j] = ok ? a.x[base + p0 + j] : (uint16_t)0;
-        ty[j] = ok ? a.y[base + p0 + j] : (uint16_t)0;
-        tt[j] = ok ? a.tot[base + p0 + j] : (uint16_t)1;
+        const uint64_t src = ok ? (kGiven ? (uint64_t)a.perm[base + p0 + j] : base + p0 + j) : 0ull;
+        tx[j] = ok ? a.x[src] : (uint16_t)0;
+        ty[j] = ok ? a.y[src] : (uint16_t)0;
+        tt[j] = ok ? a.tot[src] : (uint16_t)1;
       }
       vx = make_uint4(tx[0] | ((uint32_t)tx[1] << 16), tx[2] | ((uint32_t)tx[3] << 16),
                       tx[4] | ((uint32_t)tx[5] << 16), tx[6] | ((uint32_t)tx[7] << 16));
@@ -525,7 +543,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     cl_carry = __shfl_up_sync(0xffffffffu, cl_inc, 1);
     if (lane == 0) cl_carry = 0;
   }
-  const bool unsorted = __syncthreads_or(uns ? 1 : 0) != 0;
+  const bool unsorted = __syncthreads_or(!kGiven && uns ? 1 : 0) != 0;
   if (cl_wide && !cl_scan && tid == 0) misc->loose = 1u;   // not checked: treated as not tight
   if (!unsorted && cl_scan) {
     for (uint32_t w = 0; w < warp; ++w) cl_carry = max(cl_carry, misc->warp_sums[w]);
@@ -548,14 +566,21 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     // config 4), so: bitmap of the keys that occur (region A, already zero) -> dense key number by a prefix
     // popcount -> events per dense key (shared-memory atomics; the returned value is the event's arrival slot
     // inside its key group) -> offsets by an exclusive scan -> the few events of one key are ordered by input
-    // position with a count of smaller positions. About 60 thread instructions per event; the two-pass LSD sort
+    // position: by position block through the counts, inside a block with a count of smaller positions. About 60 thread instructions per event; the two-pass LSD sort
     // below (one ballot per digit bit) took 42 % of the kernel's instructions on config 4 (profiles/r02_*).
     constexpr uint32_t kBitmapBits = 32u * (uint32_t)T;           // 4T bytes of region A
-    constexpr uint32_t kGroupMax = 64u;                            // larger key groups: LSD (keeps the step O(n))
     uint32_t* bitmap = reinterpret_cast<uint32_t*>(smem + L::kRegA);             // [T] words
     uint16_t* wpre = reinterpret_cast<uint16_t*>(smem + L::kRegA + 4 * T);       // [T] dense number of a word's first key
-    uint32_t* gcnt = reinterpret_cast<uint32_t*>(smem + L::kRegX + 4 * T);       // [T + 32] u16 pairs: events per dense key
-    uint16_t* gbase = reinterpret_cast<uint16_t*>(smem + L::kRegX + 4 * T);
+    uint16_t* gbase = reinterpret_cast<uint16_t*>(smem + L::kRegA + 4 * T);      // [T + 1] offsets (over wpre, once dead)
+    // events per (dense key, block of THREADS input positions): eight 4-bit counts per word. A key group's
+    // members of different position blocks are ordered by the block; only the members of one block (rarely
+    // more than one) are left to the count of smaller positions.
+    uint32_t* gcnt = reinterpret_cast<uint32_t*>(smem + L::kRegX + 4 * T);       // [T] words
+    static_assert(IPT == 8, "eight position blocks = eight 4-bit counts per word");
+    auto nib_sum = [](uint32_t w) -> uint32_t {                                   // sum of the eight 4-bit fields
+      w = (w & 0x0F0F0F0Fu) + ((w >> 4) & 0x0F0F0F0Fu);
+      return (w * 0x01010101u) >> 24;
+    };
     bool counted = key_bits <= 31u && (1u << key_bits) <= kBitmapBits;
     if (counted) {
       const uint32_t nwords = ((1u << key_bits) + 31u) >> 5;
@@ -597,7 +622,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         *reinterpret_cast<uint4*>(wpre + p0) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
       }
       __syncthreads();
-      uint32_t dk_r[IPT];   // dense key | arrival slot << 16
+      uint32_t dk_r[IPT];   // dense key | arrival slot inside (key, position block) << 16
+      bool big = false;     // a 4-bit count overflowed: one key held by 16 events of one position block
 #pragma unroll
       for (int j = 0; j < IPT; ++j) {
         const uint32_t k = (uint32_t)j * THREADS + tid;
@@ -605,44 +631,38 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         if (k < mm) {
           const uint32_t sk = sk_r[j], w = sk >> 5;
           const uint32_t dk = (uint32_t)wpre[w] + (uint32_t)__popc(bitmap[w] & ((1u << (sk & 31u)) - 1u));
-          const uint32_t sh = (dk & 1u) * 16u;
-          const uint32_t r = (atomicAdd(&gcnt[dk >> 1], 1u << sh) >> sh) & 0xFFFFu;
+          const uint32_t r = (atomicAdd(&gcnt[dk], 1u << (4 * j)) >> (4 * j)) & 15u;
+          big = big || r == 15u;
           dk_r[j] = dk | (r << 16);
         }
       }
-      __syncthreads();
-      bool big = false;
-      {   // offsets: exclusive scan of the counts, 8 consecutive dense keys per thread (there are at most mm <= T keys)
-        const uint4 q = *reinterpret_cast<const uint4*>(gbase + p0);
-        const uint32_t qw[4] = {q.x, q.y, q.z, q.w};
-        uint32_t c[IPT], sum = 0;
-#pragma unroll
-        for (int j = 0; j < IPT; ++j) {
-          c[j] = (qw[j >> 1] >> ((j & 1) * 16)) & 0xFFFFu;
-          sum += c[j];
-          big = big || c[j] > kGroupMax;
-        }
-        uint32_t inc = sum;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-          if (lane >= (uint32_t)o) inc += t;
-        }
-        if (lane == 31) misc->warp_sums[warp] = inc;
-        big = __syncthreads_or(big ? 1 : 0) != 0;
-        uint32_t run = inc - sum;
-        for (uint32_t w = 0; w < warp; ++w) run += misc->warp_sums[w];
-        uint32_t pk[4];
-#pragma unroll
-        for (int j = 0; j < IPT; j += 2) {
-          pk[j >> 1] = run | ((run + c[j]) << 16);
-          run += c[j] + c[j + 1];
-        }
-        *reinterpret_cast<uint4*>(gbase + p0) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
-        if (tid == THREADS - 1) gbase[T] = (uint16_t)run;     // = mm: end of the last group
-      }
-      __syncthreads();
+      big = __syncthreads_or(big ? 1 : 0) != 0;
       if (!big) {
+        {   // offsets: exclusive scan of the group sizes, 8 consecutive dense keys per thread (at most mm <= T keys)
+          const uint4 q0 = *reinterpret_cast<const uint4*>(gcnt + p0), q1 = *reinterpret_cast<const uint4*>(gcnt + p0 + 4);
+          const uint32_t qw[IPT] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w};
+          uint32_t c[IPT], sum = 0;
+#pragma unroll
+          for (int j = 0; j < IPT; ++j) { c[j] = nib_sum(qw[j]); sum += c[j]; }
+          uint32_t inc = sum;
+#pragma unroll
+          for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= (uint32_t)o) inc += t;
+          }
+          if (lane == 31) misc->warp_sums[warp] = inc;
+          __syncthreads();
+          uint32_t run = inc - sum;
+          for (uint32_t w = 0; w < warp; ++w) run += misc->warp_sums[w];
+          uint32_t pk[4];
+#pragma unroll
+          for (int j = 0; j < IPT; j += 2) {
+            pk[j >> 1] = run | ((run + c[j]) << 16);
+            run += c[j] + c[j + 1];
+          }
+          *reinterpret_cast<uint4*>(gbase + p0) = make_uint4(pk[0], pk[1], pk[2], pk[3]);   // wpre is dead
+        }
+        __syncthreads();
         uint32_t b0_r[IPT];
 #pragma unroll
         for (int j = 0; j < IPT; ++j) {
@@ -650,10 +670,12 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
           b0_r[j] = 0;
           if (k < mm) {
             const uint32_t dk = dk_r[j] & 0xFFFFu, r = dk_r[j] >> 16;
-            const uint32_t b0 = gbase[dk], m = (uint32_t)gbase[dk + 1u] - b0;
+            const uint32_t w = gcnt[dk];
+            // the group's members of earlier position blocks come first
+            const uint32_t b0 = (uint32_t)gbase[dk] + nib_sum(w & ((1u << (4 * j)) - 1u)), m = (w >> (4 * j)) & 15u;
             b0_r[j] = b0 | (m << 16);
-            if (m == 1u) buf1[b0] = (uint16_t)k;      // alone with its key: final position
-            else buf0[b0 + r] = (uint16_t)k;          // the group's members in arrival order
+            if (m == 1u) buf1[b0] = (uint16_t)k;      // alone with its key in its position block: final position
+            else buf0[b0 + r] = (uint16_t)k;          // the sub-group's members in arrival order
           }
         }
         __syncthreads();
@@ -669,8 +691,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         }
         fin = buf1;
       } else {
-        counted = false;      // one key held by very many events: the LSD sort below
-        for (uint32_t i = tid; i < (uint32_t)(2 * T + 64) / 4u; i += THREADS) gcnt[i] = 0u;   // its digit counters live here
+        counted = false;      // the LSD sort below
       }
       __syncthreads();
     }
@@ -766,7 +787,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     for (int q = 0; q < 16 * T / 16 / THREADS; ++q) z[q * THREADS + tid] = zero;
     __syncthreads();
   } else {
-    for (uint32_t k = tid; k < mm; k += THREADS) a.perm[out_base + k] = out_base + k;
+    if (!kGiven)
+      for (uint32_t k = tid; k < mm; k += THREADS) a.perm[out_base + k] = out_base + k;
   }
   const uint2* recS = unsorted ? recA : recB + lo;
   unsigned char* hreg = smem + (unsorted ? L::kRegX : L::kRegA);   // 16T bytes: hash table, later the label / chain arrays
@@ -777,9 +799,9 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   uint32_t* head = reinterpret_cast<uint32_t*>(hreg + 4 * T);           // [T] member chain head per label
   // mode 1 keeps the hash table alive until the end: its marks go where mode 0 keeps the parents, and the
   // ordinal list may overwrite them (the ordinal step has read every mark before it writes the first ordinal)
-  uint16_t* lab = MODE ? reinterpret_cast<uint16_t*>(smem + L::kPar)
+  uint16_t* lab = kLM ? reinterpret_cast<uint16_t*>(smem + L::kPar)
                        : reinterpret_cast<uint16_t*>(hreg + 8 * T);     // [T] label per event
-  uint16_t* rootpos = MODE ? lab : reinterpret_cast<uint16_t*>(hreg + 10 * T);   // [T] ordinal -> label
+  uint16_t* rootpos = kLM ? lab : reinterpret_cast<uint16_t*>(hreg + 10 * T);   // [T] ordinal -> label
   uint16_t* nxt = reinterpret_cast<uint16_t*>(hreg + 12 * T);           // [T] next member of the same hit
 
   // Scans one neighbour cell completely (home bucket and, while marked, the following ones) and
@@ -838,7 +860,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   };
   // mode 1 with a small box: the neighbours are found through the hash, (2 wx + 1)(2 wy + 1) cells per event;
   // a large box is cheaper to serve by walking the time window of the sorted tile
-  const bool lm_grid = MODE != 0 && (2u * a.lm_wx + 1u) * (2u * a.lm_wy + 1u) <= 81u;
+  const bool lm_grid = kLM && (2u * a.lm_wx + 1u) * (2u * a.lm_wy + 1u) <= 81u;
   // calls sink(j) for every event j of the box of event (cell, slk, key), the event itself included
   auto scan_box = [&](uint32_t cell, uint32_t slk, uint32_t key, auto&& sink) {
     const uint32_t x = cell & 0xFFu, y = cell >> 8;
@@ -850,7 +872,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       }
   };
 
-  if (MODE != 0 && lm_grid) {
+  if (kLM && lm_grid) {
     // ---- paper-literal mode (Eq. 5-7, :122-150) through the hash: k is a hit if no event of its box —
     //      same shot, |dX| <= wx, |dY| <= wy, |dToF| <= W, all inclusive — has a greater (ToT, sorted index)
     hash_insert();
@@ -868,7 +890,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       lab[k] = is_max ? (uint16_t)k : (uint16_t)0xFFFFu;
     }
     __syncthreads();
-  } else if (MODE != 0) {
+  } else if (kLM) {
     // ---- paper-literal mode (Eq. 5-7, :122-150): k is a hit if no event of its box — same shot,
     //      |dX| <= wx, |dY| <= wy, |dToF| <= W, all inclusive — has a greater (ToT, sorted index). The keys
     //      ascend and keys of different shots differ by more than W, so the time neighbours of k are one
@@ -891,6 +913,30 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       a.label[out_base + k] = is_max ? out_base + k : kNone;
     }
     __syncthreads();
+  } else if (kGiven) {
+    // ---- mode 3 (tpx3_centroid): the caller's labels. A hit must lie inside the tile (labels of tpx3_cluster do:
+    //      no hit crosses a shot); one that does not sends the call to the general kernels --------------------
+    {
+      uint4* f = reinterpret_cast<uint4*>(hreg);
+      const uint4 ones = make_uint4(kNone, kNone, kNone, kNone);
+#pragma unroll
+      for (int q = 0; q < 8 * T / 16 / THREADS; ++q) f[q * THREADS + tid] = ones;   // (minidx and) head
+    }
+    __syncthreads();
+    bool outside = false;
+#pragma unroll
+    for (int j = 0; j < IPT; ++j) {
+      const uint32_t k = (uint32_t)j * THREADS + tid;
+      if (k < mm) {
+        const uint32_t l = a.label[out_base + k] - out_base;      // a label before the tile wraps to a huge value
+        if (l >= mm) { outside = true; lab[k] = (uint16_t)0xFFFFu; }
+        else {
+          lab[k] = (uint16_t)l;
+          nxt[k] = (uint16_t)atomicExch(&head[l], k);
+        }
+      }
+    }
+    if (__syncthreads_or(outside ? 1 : 0)) failed = true;
   } else {
   // ---- are the time clusters of the tile tight? --------------------------------------------------------
   // Cut the ascending keys into clusters wherever two neighbours are more than W apart (a new shot always is).
@@ -1012,7 +1058,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   // candidate of an event whose S cell holds an event of its own time cluster. Such an event needs ONE probe.
   // First pass: S only; the events whose S cell is empty, holds another cluster's event first, or overflowed are
   // collected and take the full five-cell step densely packed in a second pass.
-  const bool tight = MODE == 0 && misc->loose == 0u;
+  const bool tight = kCC && misc->loose == 0u;
   if (tight && tid == 0) atomicAdd(&a.ctrl->tight_tiles, 1u);
   if (tight) {
     uint16_t* kl_end = reinterpret_cast<uint16_t*>(smem + L::kMisc);   // grows downwards from the list's end
@@ -1146,7 +1192,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       const uint32_t l = minidx[root_r[j]];
       lab[k] = (uint16_t)l;
       a.label[out_base + k] = out_base + l;
-      nxt[k] = (uint16_t)atomicExch(&head[l], k);   // every member, the first pixel too; kNone truncates to 0xFFFF = end
+      if (!kLabelsOnly) nxt[k] = (uint16_t)atomicExch(&head[l], k);   // every member, the first pixel too; kNone truncates to 0xFFFF = end
     }
   }
   __syncthreads();
@@ -1185,14 +1231,14 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 #pragma unroll
     for (int j = 0; j < IPT; ++j)
       if (flags & (1u << j)) rootpos[ord++] = (uint16_t)(p0 + j);
-    n_roots = misc->n_roots;
+    n_roots = (kGiven && failed) ? 0u : misc->n_roots;
   }
   __syncthreads();   // rootpos complete
 
   // ---- S4: one thread per hit walks its chain: exact sums, brightest pixel. The hit goes to the
   //      staging table at the tile's own position out_base + c (a tile has no more hits than events);
   //      k_fused_compact moves it to its ordinal once every tile's count is known -------------------
-  if (MODE != 0 && lm_grid) {
+  if (kLM && lm_grid) {
     // paper-literal mode: the row sums of Eq. 9 over the box about every local maximum
     for (uint32_t c = tid; c < n_roots; c += THREADS) {
       const uint32_t r = rootpos[c];
@@ -1214,7 +1260,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       a.stage_c[o] = ref + (uint64_t)(rr.x >> tb) * a.P + (uint64_t)(rr.x & tmask);
       a.stage_d[o] = sf;
     }
-  } else if (MODE != 0) {
+  } else if (kLM) {
     // the same by walking the time window of the sorted tile (large boxes)
     for (uint32_t c = tid; c < n_roots; c += THREADS) {
       const uint32_t r = rootpos[c];
@@ -1248,7 +1294,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       a.stage_c[o] = ref + (uint64_t)(rr.x >> tb) * a.P + (uint64_t)(rr.x & tmask);
       a.stage_d[o] = sf;
     }
-  } else
+  } else if (!kLabelsOnly)
   for (uint32_t c = tid; c < n_roots; c += THREADS) {
     const uint32_t r = rootpos[c];
     unsigned long long sx = 0, sy = 0, sf = 0;
@@ -1354,7 +1400,7 @@ __global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, 
     }
     __syncthreads();
     const uint32_t total = s_off[32];
-    for (uint32_t i = tid; i < total; i += kCompactThreads) {
+    for (uint32_t i = tid; a.mode != 2u && i < total; i += kCompactThreads) {
       // tile of hit i: the last offset <= i (binary search over 32 offsets)
       uint32_t q = 0;
 #pragma unroll
@@ -1388,9 +1434,9 @@ __global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, 
   if (t1 == a.num_tiles && tid == 0) {
     *a.n_clusters = (uint32_t)prefix;
     a.ctrl->status.n_clusters = (uint32_t)prefix;
-    a.ctrl->status.path = a.mode ? 3 : 1;
+    a.ctrl->status.path = a.mode == 1u ? 3 : 1;
     a.ctrl->status.sort_passes = 0;
-    if (a.mode == 0u) {   // worth checking the time clusters next time? (fewer than 1 tile in 8 was tight: no)
+    if (a.mode == 0u || a.mode == 2u) {   // worth checking the time clusters next time? (fewer than 1 tile in 8 was tight: no)
       a.ctrl->scan_hint = a.ctrl->tight_tiles * 8u < a.ctrl->tiles_run ? kScanSkip : 0u;
       a.ctrl->calls += 1u;
     }
@@ -1408,26 +1454,31 @@ inline FusedGeom fused_geom(uint64_t P, uint32_t W, uint32_t max_shot_hits) {
   FusedGeom g{0, 0};
   if (P == 0 || P > (1ull << 24) || W >= (1u << 24)) return g;   // tof + W must fit the 32-bit tile key
   const uint32_t Lh = max_shot_hits ? max_shot_hits : 1024u;      // no hint: first rung of the ladder (below)
-  if (Lh <= 512u) { g.variant = 3; g.T = 2048; }
-  else if (Lh <= 1536u) { g.variant = 1; g.T = 4096; }   // two tiles per SM beat one 8192-event tile
-  else if (Lh <= 4096u) { g.variant = 2; g.T = 8192; }
+  // a window must hold the longest shot (T - 8 events when the tile starts at an odd position); the smaller
+  // window wins whenever it does (4 CTAs of 2048 events per SM against 2 of 4096: cfg2 +6.7 %, cfg4 +5 %,
+  // cfg1 equal; 8192 against 4096 on cfg3: equal)
+  if (Lh <= 1536u) { g.variant = 3; g.T = 2048; }
+  else if (Lh <= 3584u) { g.variant = 1; g.T = 4096; }
+  else if (Lh <= 8184u) { g.variant = 2; g.T = 8192; }
   else return g;
   return g;
 }
 
 // Segment length and status words per segment for n events in tiles of T (host and device: the ladder's rungs
-// are sized on the device). Segments of 4 windows keep the re-read of a segment's first window at a few per
+// are sized on the device). Segments of 8 windows keep the re-read of a segment's first window at a few per
 // cent; short inputs get shorter segments so that every SM has work. Two consecutive tiles that own something
 // advance by at least T - 7 events together (what one leaves behind, at most a shot, the next one takes), hence
-// the bound on status words.
+// the bound on status words. Measured and dropped: the stream's last wave in segments a quarter as long (cfg1
+// 4 % slower: every segment start re-reads half a shot).
 struct FusedSegs {
   uint32_t G, nseg, maxt;
 };
 
 __host__ __device__ inline FusedSegs fused_segs(uint64_t n, uint32_t T, uint32_t num_sms) {
   FusedSegs s;
-  uint64_t G = 4ull * T;
-  const uint64_t want = (uint64_t)num_sms * 16ull;           // segments to aim for (load balance)
+  uint64_t G = 8ull * T;
+  const uint64_t slots = (uint64_t)num_sms * (T <= 2048u ? 4u : (T <= 4096u ? 2u : 1u));   // resident CTAs
+  const uint64_t want = slots * 8ull;                        // segments to aim for (load balance)
   if (n / G < want) {
     G = (n / want + 7ull) & ~7ull;
     if (G < 2ull * T) G = 2ull * T;
@@ -1451,23 +1502,26 @@ inline int fused_configure_device() {
   if (cudaFuncSetAttribute(k_fused_shot_tiles<T, THREADS, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,     \
                            FusedSmem<T>::kBytes) != cudaSuccess)                                                  \
     return TPX3_ERR_CUDA;
-  TPX3_FUSED_ATTR(2048, 256, 0) TPX3_FUSED_ATTR(2048, 256, 1) TPX3_FUSED_ATTR(4096, 512, 0)
-  TPX3_FUSED_ATTR(4096, 512, 1) TPX3_FUSED_ATTR(8192, 1024, 0) TPX3_FUSED_ATTR(8192, 1024, 1)
+  TPX3_FUSED_ATTR(2048, 256, 0) TPX3_FUSED_ATTR(2048, 256, 1) TPX3_FUSED_ATTR(2048, 256, 2) TPX3_FUSED_ATTR(2048, 256, 3)
+  TPX3_FUSED_ATTR(4096, 512, 0) TPX3_FUSED_ATTR(4096, 512, 1) TPX3_FUSED_ATTR(4096, 512, 2) TPX3_FUSED_ATTR(4096, 512, 3)
+  TPX3_FUSED_ATTR(8192, 1024, 0) TPX3_FUSED_ATTR(8192, 1024, 1) TPX3_FUSED_ATTR(8192, 1024, 2)
+  TPX3_FUSED_ATTR(8192, 1024, 3)
 #undef TPX3_FUSED_ATTR
   return TPX3_OK;
 }
 
-// Without a hint the window length is tried in rungs: 4096 events, then 8192. A rung whose tiles meet a shot
-// that does not fit fails within its first wave (every later tile returns at once), and k_fallback_dispatch
-// launches the next rung from the device; after the last one the general kernels run.
-constexpr int kLadderMax = 1;   // rungs after the first
+// Without a hint the window length is tried in rungs: 2048 events, then 4096, then 8192. A rung whose tiles meet
+// a shot that does not fit fails within its first wave (every later segment returns at once), and
+// k_fallback_dispatch launches the next rung from the device; after the last one the general kernels run.
+constexpr int kLadderMax = 2;   // rungs after the first
 struct FusedLadder {
-  int n;                        // rungs still to try after the one the host enqueued (8192-event tiles)
+  int n;                        // rungs still to try after the one the host enqueued
+  uint32_t T[kLadderMax];       // their window lengths
 };
 
 inline FusedLadder fused_ladder(uint32_t max_shot_hits) {
-  FusedLadder l{0};
-  if (max_shot_hits == 0) l.n = 1;
+  FusedLadder l{0, {0, 0}};
+  if (max_shot_hits == 0) { l.n = 2; l.T[0] = 4096u; l.T[1] = 8192u; }
   return l;
 }
 
@@ -1514,14 +1568,24 @@ __host__ __device__ inline void compact_grid(uint32_t num_tiles, uint32_t num_sm
   *ctas = t ? (num_tiles + t - 1) / t : 1u;
 }
 
-// Device side: the next rung (8192-event tiles), tail-launched by k_fallback_dispatch.
-__device__ inline void launch_fused_rung_device(FusedArgs a) {
+// Device side: the next rung, tail-launched by k_fallback_dispatch.
+__device__ inline void launch_fused_rung_device(FusedArgs a, uint32_t T) {
   uint32_t ctas, tpc;
   compact_grid(a.num_tiles, a.num_sms, &ctas, &tpc);
-  if (a.mode == 0u)
-    k_fused_shot_tiles<8192, 1024, 0><<<a.nseg, 1024, FusedSmem<8192>::kBytes, cudaStreamTailLaunch>>>(a);
-  else
-    k_fused_shot_tiles<8192, 1024, 1><<<a.nseg, 1024, FusedSmem<8192>::kBytes, cudaStreamTailLaunch>>>(a);
+#define TPX3_RUNG(T_, THREADS_, MODE_) \
+  k_fused_shot_tiles<T_, THREADS_, MODE_><<<a.nseg, THREADS_, FusedSmem<T_>::kBytes, cudaStreamTailLaunch>>>(a)
+  if (T == 4096u) {
+    if (a.mode == 0u) TPX3_RUNG(4096, 512, 0);
+    else if (a.mode == 1u) TPX3_RUNG(4096, 512, 1);
+    else if (a.mode == 2u) TPX3_RUNG(4096, 512, 2);
+    else TPX3_RUNG(4096, 512, 3);
+  } else {
+    if (a.mode == 0u) TPX3_RUNG(8192, 1024, 0);
+    else if (a.mode == 1u) TPX3_RUNG(8192, 1024, 1);
+    else if (a.mode == 2u) TPX3_RUNG(8192, 1024, 2);
+    else TPX3_RUNG(8192, 1024, 3);
+  }
+#undef TPX3_RUNG
   k_fused_compact<<<ctas, kCompactThreads, 0, cudaStreamTailLaunch>>>(a, tpc);
 }
 
@@ -1536,16 +1600,19 @@ inline int enqueue_fused(const FusedGeom& g, uint32_t num_sms, uint64_t* launche
   if (g.variant == 0 || prm.n == 0) return TPX3_OK;
   // the 128-bit load phase needs 16-byte aligned inputs (PyTorch allocations are 256-byte aligned)
   if ((((uintptr_t)x | (uintptr_t)y | (uintptr_t)toa | (uintptr_t)tot) & 15u) != 0) return TPX3_OK;
+  if (mode == 3u && ((uintptr_t)perm & 15u) != 0) return TPX3_OK;
   const FusedArgs a = make_fused_args(g.T, num_sms, ctrl, tiles, prm, x, y, toa, tot, perm, label, max_clusters, out,
                                       n_clusters, stage, mode, lm_wx, lm_wy);
   *args = a;
   int rc;
-  if (mode == 0u)
-    rc = g.variant == 3 ? launch_fused<2048, 256, 0>(a, st)
-                        : g.variant == 1 ? launch_fused<4096, 512, 0>(a, st) : launch_fused<8192, 1024, 0>(a, st);
-  else
-    rc = g.variant == 3 ? launch_fused<2048, 256, 1>(a, st)
-                        : g.variant == 1 ? launch_fused<4096, 512, 1>(a, st) : launch_fused<8192, 1024, 1>(a, st);
+#define TPX3_PICK(MODE_)                                                \
+  (g.variant == 3 ? launch_fused<2048, 256, MODE_>(a, st)               \
+                  : g.variant == 1 ? launch_fused<4096, 512, MODE_>(a, st) : launch_fused<8192, 1024, MODE_>(a, st))
+  if (mode == 0u) rc = TPX3_PICK(0);
+  else if (mode == 1u) rc = TPX3_PICK(1);
+  else if (mode == 2u) rc = TPX3_PICK(2);
+  else rc = TPX3_PICK(3);
+#undef TPX3_PICK
   if (rc != TPX3_OK) return rc;
   ++*launches;
   uint32_t ctas, tiles_per_cta;

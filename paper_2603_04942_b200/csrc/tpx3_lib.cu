@@ -225,23 +225,23 @@ __host__ __device__ inline uint32_t grid_for_hd(uint64_t n, int threads, int num
 // hint: the same tile kernel with room for longer shots, then this dispatcher again) or, after the last rung,
 // the whole general path. A successful fused call thus pays for one empty launch instead of the 36 early-exit
 // launches of the general path. lm != 0: the paper-literal mode.
-__global__ void k_fallback_dispatch(GenArgs a, FusedArgs fa, FusedLadder ladder, int rung, int lm) {
+__global__ void k_fallback_dispatch(GenArgs a, FusedArgs fa, FusedLadder ladder, int rung, int what) {
   Ctrl* c = a.w.ctrl;
   if (c->fused_state == 1u) return;
   if (rung < ladder.n) {
     c->tiles_done = 0; c->fused_fail = 0; c->fused_state = 0; c->tight_tiles = 0; c->tiles_run = 0;
-    const FusedSegs sg = fused_segs(fa.n, 8192u, fa.num_sms);
+    const FusedSegs sg = fused_segs(fa.n, ladder.T[rung], fa.num_sms);
     fa.G = sg.G; fa.nseg = sg.nseg; fa.maxt = sg.maxt; fa.num_tiles = sg.nseg * sg.maxt;
-    launch_fused_rung_device(fa);
-    k_fallback_dispatch<<<1, 1, 0, cudaStreamTailLaunch>>>(a, fa, ladder, rung + 1, lm);
+    launch_fused_rung_device(fa, ladder.T[rung]);
+    k_fallback_dispatch<<<1, 1, 0, cudaStreamTailLaunch>>>(a, fa, ladder, rung + 1, what);
     return;
   }
 #define GP(stage, kernel, grid, block, ...) kernel<<<(grid), (block), 0, cudaStreamTailLaunch>>>(__VA_ARGS__)
-  if (lm) {
+  if (what == 1) {
     TPX3_LOCALMAX_SEQUENCE(a);
   } else {
-    TPX3_GENERAL_CLUSTER_SEQUENCE(a);
-    TPX3_GENERAL_CENTROID_SEQUENCE(a);
+    if (what != 3) TPX3_GENERAL_CLUSTER_SEQUENCE(a);
+    if (what != 2) TPX3_GENERAL_CENTROID_SEQUENCE(a);
   }
 #undef GP
 }
@@ -394,54 +394,20 @@ int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace
   p->off_slot = p->off_keyA;                    // 4N <= 8N
   p->off_peak = p->off_keyB;                    // 8N
   p->off_blkcnt = p->off_idxA;                  // 4 * ceil(N/4096) <= 4N
-  p->off_tiles = o; o = align_up(o + 8 * (size_t)(N / 256 + 65536));   // fused path tile status words (fused_segs: nseg * maxt)
+  p->off_tiles = o; o = align_up(o + 8 * (size_t)(N / 128 + 262144));   // fused path tile status words (fused_segs: nseg * maxt)
   p->workspace_bytes = o;
   *workspace_bytes = o;
   *out_plan = p;
   return TPX3_OK;
 }
 
-int tpx3_cluster(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x, const uint16_t* y,
-                 const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label, uint32_t* n_clusters) {
-  if (!p || !workspace || !n_clusters) return TPX3_ERR_INVALID_ARG;
-  if (n > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
-  if (n && (!x || !y || !toa || !tot || !perm || !label)) return TPX3_ERR_INVALID_ARG;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
-  Ws w = carve(p, workspace);
-  if (p->profiling) ++p->profiled_calls;
-  TPX3_LAUNCH(p, k_ctrl_init, 1, 256, 0, st, w.ctrl, n, w.tiles, 0u, n_clusters);
-  if (n == 0) return cuda_ok(cudaGetLastError());
-  GenArgs ga = make_gen_args(p, w, 0, n, x, y, toa, tot, perm, label, 0, nullptr, n_clusters);
-  return enqueue_general_cluster(p, ga, st);
-}
-
-int tpx3_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x, const uint16_t* y,
-                  const uint64_t* toa, const uint16_t* tot, const uint32_t* perm, const uint32_t* label,
-                  uint64_t max_clusters, const tpx3_clusters_t* out, uint32_t* n_clusters) {
-  if (!p || !workspace || !n_clusters) return TPX3_ERR_INVALID_ARG;
-  if (n > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
-  if (n && (!x || !y || !toa || !tot || !perm || !label)) return TPX3_ERR_INVALID_ARG;
-  if (max_clusters && !clusters_ok(out)) return TPX3_ERR_INVALID_ARG;
-  if (n && !out) return TPX3_ERR_INVALID_ARG;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
-  Ws w = carve(p, workspace);
-  if (p->profiling) ++p->profiled_calls;
-  TPX3_LAUNCH(p, k_ctrl_init, 1, 256, 0, st, w.ctrl, n, w.tiles, 0u, n_clusters);
-  if (n == 0) return cuda_ok(cudaGetLastError());
-  GenArgs ga = make_gen_args(p, w, 0, n, x, y, toa, tot, const_cast<uint32_t*>(perm), const_cast<uint32_t*>(label),
-                             max_clusters, out, n_clusters);
-  return enqueue_centroid(p, ga, st);
-}
-
-int tpx3_cluster_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x,
-                          const uint16_t* y, const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label,
-                          uint64_t max_clusters, const tpx3_clusters_t* out, uint32_t* n_clusters) {
-  if (!p || !workspace || !n_clusters) return TPX3_ERR_INVALID_ARG;
-  if (n > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
-  if (n && (!x || !y || !toa || !tot || !perm || !label || !out)) return TPX3_ERR_INVALID_ARG;
-  if (max_clusters && !clusters_ok(out)) return TPX3_ERR_INVALID_ARG;
+// S0-S3 / S4-S5 / S0-S5 share one body: the fused tile kernel in the mode that matches the call (0: everything,
+// 2: stop after the labels, 3: start from the caller's perm / label), with the general kernels enqueued from the
+// device when it gives up.
+static int run_fused_or_general(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x,
+                                const uint16_t* y, const uint64_t* toa, const uint16_t* tot, uint32_t* perm,
+                                uint32_t* label, uint64_t max_clusters, const tpx3_clusters_t* out, uint32_t* n_clusters,
+                                uint32_t mode) {
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
   Ws w = carve(p, workspace);
@@ -452,24 +418,58 @@ int tpx3_cluster_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uin
   Params prm = p->prm;
   prm.n = n;
   int rc = TPX3_OK;
-  GenArgs ga = make_gen_args(p, w, 1, n, x, y, toa, tot, perm, label, max_clusters, out, n_clusters);
+  tpx3_clusters_t none;
+  memset(&none, 0, sizeof(none));
+  GenArgs ga = make_gen_args(p, w, mode == 2u ? 0 : 1, n, x, y, toa, tot, perm, label, max_clusters, out, n_clusters);
   if (try_fused) {
     bool launched = false;
     StageTimer timer(p, st, TPX3_STAGE_FUSED);
     FusedArgs fa;
-    rc = enqueue_fused(p->fused, (uint32_t)p->num_sms, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, label, max_clusters,
-                       *out, n_clusters, (char*)workspace + p->off_keyA, &launched, &fa);
+    rc = enqueue_fused(p->fused, (uint32_t)p->num_sms, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, label,
+                       max_clusters, out ? *out : none, n_clusters, (char*)workspace + p->off_keyA, &launched, &fa, mode);
     if (rc != TPX3_OK) return rc;
     if (launched) {
       // the next rung or the general path, only if the fused kernel gave up: decided and enqueued on the device
-      k_fallback_dispatch<<<1, 1, 0, st>>>(ga, fa, fused_ladder(p->cfg.max_shot_hits), 0, 0);
+      k_fallback_dispatch<<<1, 1, 0, st>>>(ga, fa, fused_ladder(p->cfg.max_shot_hits), 0, (int)mode);
       ++p->launches;
       return cuda_ok(cudaGetLastError());
     }
   }
-  rc = enqueue_general_cluster(p, ga, st);
-  if (rc != TPX3_OK) return rc;
-  return enqueue_centroid(p, ga, st);
+  if (mode != 3u) {
+    rc = enqueue_general_cluster(p, ga, st);
+    if (rc != TPX3_OK) return rc;
+  }
+  return mode != 2u ? enqueue_centroid(p, ga, st) : TPX3_OK;
+}
+
+int tpx3_cluster(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x, const uint16_t* y,
+                 const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label, uint32_t* n_clusters) {
+  if (!p || !workspace || !n_clusters) return TPX3_ERR_INVALID_ARG;
+  if (n > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
+  if (n && (!x || !y || !toa || !tot || !perm || !label)) return TPX3_ERR_INVALID_ARG;
+  return run_fused_or_general(p, workspace, cuda_stream, n, x, y, toa, tot, perm, label, 0, nullptr, n_clusters, 2u);
+}
+
+int tpx3_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x, const uint16_t* y,
+                  const uint64_t* toa, const uint16_t* tot, const uint32_t* perm, const uint32_t* label,
+                  uint64_t max_clusters, const tpx3_clusters_t* out, uint32_t* n_clusters) {
+  if (!p || !workspace || !n_clusters) return TPX3_ERR_INVALID_ARG;
+  if (n > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
+  if (n && (!x || !y || !toa || !tot || !perm || !label)) return TPX3_ERR_INVALID_ARG;
+  if (max_clusters && !clusters_ok(out)) return TPX3_ERR_INVALID_ARG;
+  if (n && !out) return TPX3_ERR_INVALID_ARG;
+  return run_fused_or_general(p, workspace, cuda_stream, n, x, y, toa, tot, const_cast<uint32_t*>(perm),
+                              const_cast<uint32_t*>(label), max_clusters, out, n_clusters, 3u);
+}
+
+int tpx3_cluster_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x,
+                          const uint16_t* y, const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label,
+                          uint64_t max_clusters, const tpx3_clusters_t* out, uint32_t* n_clusters) {
+  if (!p || !workspace || !n_clusters) return TPX3_ERR_INVALID_ARG;
+  if (n > p->cfg.max_hits) return TPX3_ERR_INVALID_ARG;
+  if (n && (!x || !y || !toa || !tot || !perm || !label || !out)) return TPX3_ERR_INVALID_ARG;
+  if (max_clusters && !clusters_ok(out)) return TPX3_ERR_INVALID_ARG;
+  return run_fused_or_general(p, workspace, cuda_stream, n, x, y, toa, tot, perm, label, max_clusters, out, n_clusters, 0u);
 }
 
 int tpx3_localmax_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x,

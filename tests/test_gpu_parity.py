@@ -266,6 +266,70 @@ def test_centroid_accepts_oracle_labels(tpx3):
     assert_parity(g, o, "oracle labels")
 
 
+@pytest.mark.parametrize("cfg,shots,hint", [(1, 2000, 600), (4, 1200, 1500), (3, 300, 3360), (4, 1200, 0)])
+def test_split_calls_take_the_tile_kernel(tpx3, cfg, shots, hint):
+    """tpx3_cluster (S0-S3) and tpx3_centroid (S4-S5) run in the fused tile kernel too (labels only / labels
+    given): same outputs as the oracle, and the status word says which path served each call."""
+    import torch
+
+    w = gen.generate(cfg, shots=shots)
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P)
+    pl = tpx3.plan(tpx3.Config(max_hits=w.n, max_shot_hits=hint))
+    dev = [to_dev(a) for a in (w.x, w.y, w.toa, w.tot)]
+    perm, label, nc = pl.cluster(*dev)
+    torch.cuda.synchronize()
+    st = pl.status()
+    assert st["error"] == 0 and st["path"] == 1, st
+    assert int(nc.cpu().numpy()[0]) == o["n_clusters"]
+    np.testing.assert_array_equal(perm[: w.n].cpu().numpy(), o["perm"])
+    np.testing.assert_array_equal(label[: w.n].cpu().numpy(), o["label"])
+    cl = tpx3.Clusters(w.n, pl.device)
+    nc2 = pl.centroid(*dev, perm, label, cl)
+    torch.cuda.synchronize()
+    st = pl.status()
+    assert st["error"] == 0 and st["path"] == 1, st
+    ncl = int(nc2.cpu().numpy()[0])
+    g = {"perm": o["perm"], "label": o["label"], "n_clusters": ncl}
+    g.update(cl.numpy(ncl))
+    assert_parity(g, o, "split cfg%d" % cfg)
+    pl.free()
+
+
+def test_centroid_with_hits_that_cross_shots(tpx3):
+    """tpx3_centroid takes ANY valid (perm, label): here every event of the stream is declared one hit (label 0),
+    so the hit crosses every shot and every tile: the tile kernel gives up and the general kernels serve the
+    call. Expected row recomputed with numpy from the definition (Eq. 8-9)."""
+    import torch
+
+    w = gen.generate(1, shots=40)
+    n = w.n
+    perm = np.argsort(w.toa, kind="stable").astype(np.uint32)
+    label = np.zeros(n, dtype=np.uint32)
+    # and a second variant: two hits, the second one starting in the middle of a shot
+    cut = int(w.shot_offsets[17]) + 5
+    label2 = np.where(np.arange(n) < cut, 0, cut).astype(np.uint32)
+    for lab in (label, label2):
+        pl = tpx3.plan(tpx3.Config(max_hits=n, max_shot_hits=600))
+        cl = tpx3.Clusters(16, pl.device)
+        nc = pl.centroid(to_dev(w.x), to_dev(w.y), to_dev(w.toa), to_dev(w.tot), to_dev(perm), to_dev(lab), cl)
+        torch.cuda.synchronize()
+        assert pl.status()["error"] == 0
+        roots = np.flatnonzero(lab == np.arange(n))
+        assert int(nc.cpu().numpy()[0]) == len(roots)
+        g = cl.numpy(len(roots))
+        x, y, tot, toa = (a[perm].astype(np.int64) for a in (w.x, w.y, w.tot, w.toa))
+        for i, r in enumerate(roots):
+            m = lab == r
+            assert g["c_label"][i] == r and g["c_size"][i] == m.sum()
+            assert g["c_sum_tot"][i] == tot[m].sum()
+            assert g["c_sum_tot_x"][i] == (tot[m] * x[m]).sum()
+            assert g["c_sum_tot_y"][i] == (tot[m] * y[m]).sum()
+            best = np.flatnonzero(m)[np.lexsort((np.flatnonzero(m), tot[m]))[-1]]   # max (ToT, sorted position)
+            assert g["c_toa_peak"][i] == toa[best]
+            assert g["c_cx"][i] == np.float32(np.float32((tot[m] * x[m]).sum()) / np.float32(tot[m].sum()))
+        pl.free()
+
+
 # ------------------------------------------------------------------ error behaviour
 def test_capacity_error(tpx3):
     w = gen.generate(0, shots=50)
@@ -721,10 +785,10 @@ def test_localmax_capacity_and_args(tpx3):
     pl.free()
 
 
-@pytest.mark.parametrize("per_shot,path", [(700, 1), (1500, 1), (3000, 1), (9000, 2)])
+@pytest.mark.parametrize("per_shot,path", [(700, 1), (1500, 1), (3000, 1), (6000, 1), (9000, 2)])
 def test_no_hint_ladder(tpx3, per_shot, path):
-    """max_shot_hits = 0: shot lengths 1024, 2048, 4096 are tried in turn on the device (a failed rung stops in
-    its first wave and the next one is launched from k_fallback_dispatch), then the general path."""
+    """max_shot_hits = 0: windows of 2048, 4096 and 8192 events are tried in turn on the device (a failed rung
+    stops in its first wave and the next one is launched from k_fallback_dispatch), then the general path."""
     rng = np.random.default_rng(per_shot)
     shots = 25
     n = shots * per_shot
