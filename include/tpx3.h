@@ -48,8 +48,7 @@ typedef enum {
   TPX3_ERR_INVALID_ARG = -1,   /* null pointer, bad struct_size, n > max_hits, bad config      */
   TPX3_ERR_CAPACITY = -2,      /* max_clusters too small (device-detected; see tpx3_status)     */
   TPX3_ERR_OUT_OF_RANGE = -3,  /* x/y outside the sensor or tot == 0 (under VALIDATE_INPUT)     */
-  TPX3_ERR_CUDA = -4,          /* a CUDA runtime call failed                                    */
-  TPX3_ERR_UNIMPLEMENTED = -5
+  TPX3_ERR_CUDA = -4           /* a CUDA runtime call failed                                    */
 } tpx3_error_t;
 
 enum {
@@ -171,7 +170,7 @@ int tpx3_timewalk_table(double a, double b, double c, double d, uint32_t length,
 /* Preprocessing (section IV.B-C, :66-76) of a pixel stream with
  * unwrapped ToA against the list of laser triggers trig uint64[n_trig] [dev], ascending. Per event:
  * s = the most recent trigger (largest s with trig[s] <= ToA; none: dropped), ToF = ToA - trig[s],
- * dropped if ToF > cut ("does not exceed 100 us", :68), ToF' = ToF - table[min(ToT, table_len-1)]
+ * dropped if ToF > cut ("does not exceed 100 us", :68; cut < 2^63), ToF' = ToF - table[min(ToT, table_len-1)]
  * (int32[table_len] [dev], ticks; table_len = 0: no correction) clamped to [0, P - 1], ToA' =
  * (shot_base + s) * P + ToF' with P = the plan's shot_period_ticks (must be > 0), so that the
  * clustering calls see shot = ToA' div P = shot_base + s. Kept events are written in stream order
@@ -216,7 +215,9 @@ int tpx3_status(tpx3_plan_t plan, const void* workspace, void* cuda_stream, tpx3
  *                   max(s_emitted, (t_max - D) div P); of the carried events followed by the chunk,
  *                   in stream order: shot < s_emitted: late (dropped, counted); shot < s_cut: emitted
  *                   = clustered now; the rest carried. final != 0 emits everything and ends the
- *                   stream.
+ *                   stream: any later push returns TPX3_ERR_INVALID_ARG.
+ *                   (What ONE push emits is not part of the definition: the tail sample is a lower bound of
+ *                   the largest ToA, and any lower bound only emits a shot later. The rows of ALL pushes are.)
  * stream_buf [dev]: tpx3_stream_bytes(max_chunk, max_carry) bytes, caller-owned, holds the carried
  * events, the emitted events of the current push and the stream state; max_chunk + max_carry <=
  * the plan's max_hits; the plan's shot period must be > 0. tpx3_stream_open enqueues the reset of the
@@ -248,7 +249,9 @@ int tpx3_stream_close(tpx3_stream_t stream);
  * late events or a carry overflow and the call was redone in one piece (same results). */
 int tpx3_host_route(tpx3_plan_t plan);
 
-/* Number of kernels the library has launched through this plan (for launch accounting). */
+/* Number of kernels the HOST has launched through this plan (for launch accounting). Kernels that the
+ * library launches from the device (the next rung of the no-hint ladder, the general path after a fused
+ * attempt that gave up: tpx3_status then reports path 2) are not in this count. */
 uint64_t tpx3_launch_count(tpx3_plan_t plan);
 
 /* Optional per-stage device timing. While enabled, every call brackets each stage it enqueues

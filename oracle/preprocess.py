@@ -86,9 +86,6 @@ def preprocess(x, y, toa, tot, trig, cut: int, table, P_out: int, shot_base: int
             np.array(os_, dtype=np.uint16), np.array(idx, dtype=np.int64))
 
 
-STREAM_SAMPLE = 65536   # events at the end of a chunk that feed the running maximum (R24)
-
-
 class StreamModel:
     """Chunked processing of an endless stream whose chunk cuts fall anywhere (SURVEY.md 8f NEXT #3:
     "chunk cuts that are not shot-aligned"). The definition it must reproduce is the batch one: the hits of
@@ -96,9 +93,10 @@ class StreamModel:
     and no hit crosses a shot (reading R6) — so a chunk may be cut anywhere as long as every shot is
     clustered in ONE piece. Reading R24, step by step for one push of a chunk (plain lists, stream order):
 
-      1. t_max = max(t_max, the ToA of the last STREAM_SAMPLE events of the chunk). The stream promises a
+      1. t_max = the largest ToA of everything seen so far, this chunk included. The stream promises a
          bounded disorder D: no later event has ToA < (largest ToA so far) - D (pixels report
-         out of order, dimmer ones first). Any lower bound of the largest ToA keeps step 2 safe.
+         out of order, dimmer ones first). (Any lower bound of t_max keeps step 2 safe: it only emits a
+         shot later. What a push emits is therefore not part of the definition; the rows of all pushes are.)
       2. s_cut = max(s_emitted, (t_max - D) div P): every shot below s_cut is complete. final: s_cut = inf.
       3. working set = carried events ++ chunk, in that order (the carried ones came first in the stream):
            shot <  s_emitted  -> late (its shot went out already): dropped and counted
@@ -120,7 +118,7 @@ class StreamModel:
 
     def push(self, x, y, toa, tot, final: bool = False):
         chunk = [(int(a), int(b), int(c), int(d)) for a, b, c, d in zip(x, y, toa, tot)]
-        for ev in chunk[-STREAM_SAMPLE:]:
+        for ev in chunk:
             self.t_max = max(self.t_max, ev[2])
         if final:
             s_cut = None

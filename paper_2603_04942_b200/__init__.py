@@ -23,7 +23,7 @@ __all__ = [
 FLAG_VALIDATE_INPUT = 1 << 0
 FLAG_FORCE_GENERAL = 1 << 1
 
-OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_OUT_OF_RANGE, ERR_CUDA, ERR_UNIMPLEMENTED = 0, -1, -2, -3, -4, -5
+OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_OUT_OF_RANGE, ERR_CUDA = 0, -1, -2, -3, -4
 
 # Every symbol include/tpx3.h declares (tests check the built library exports all of them).
 exported_symbols = (
@@ -191,12 +191,21 @@ class Clusters:
         return {"c_" + name: getattr(self, name)[:n].cpu().numpy() for name, _ in _CLUSTER_FIELDS}
 
 
-def _stream_ptr(stream) -> int:
+def _stream_ptr(stream, device=None) -> int:
     import torch
 
     if stream is None:
-        stream = torch.cuda.current_stream()
+        stream = torch.cuda.current_stream(device)   # of the plan's device, not of the current one
     return int(stream.cuda_stream)
+
+
+def _check_host(t, dtype, n, name):
+    import torch
+
+    if not isinstance(t, torch.Tensor) or t.is_cuda:
+        raise TypeError("%s must be a host (CPU) tensor" % name)
+    if t.dtype != dtype or not t.is_contiguous() or t.numel() < n:
+        raise TypeError("%s must be a contiguous %s host tensor with at least %d elements" % (name, dtype, n))
 
 
 def _check_dev(t, dtype, n, name):
@@ -240,7 +249,7 @@ class Plan:
         perm = torch.empty(max(n, 1), dtype=torch.uint32, device=self.device) if perm is None else perm
         label = torch.empty(max(n, 1), dtype=torch.uint32, device=self.device) if label is None else label
         n_clusters = torch.empty(1, dtype=torch.uint32, device=self.device) if n_clusters is None else n_clusters
-        rc = self.lib.tpx3_cluster(self.handle, self.workspace.data_ptr(), _stream_ptr(stream), n, x.data_ptr(),
+        rc = self.lib.tpx3_cluster(self.handle, self.workspace.data_ptr(), _stream_ptr(stream, self.device), n, x.data_ptr(),
                                    y.data_ptr(), toa.data_ptr(), tot.data_ptr(), perm.data_ptr(), label.data_ptr(),
                                    n_clusters.data_ptr())
         if rc != OK:
@@ -260,7 +269,7 @@ class Plan:
         mk = lambda dt: torch.empty(max(n, 1), dtype=dt, device=self.device)  # noqa: E731
         xo, yo, to, oo, io = mk(torch.uint16), mk(torch.uint16), mk(torch.uint64), mk(torch.uint16), mk(torch.uint32)
         n_out = torch.empty(1, dtype=torch.uint32, device=self.device)
-        rc = self.lib.tpx3_preprocess(self.handle, self.workspace.data_ptr(), _stream_ptr(stream), n, x.data_ptr(),
+        rc = self.lib.tpx3_preprocess(self.handle, self.workspace.data_ptr(), _stream_ptr(stream, self.device), n, x.data_ptr(),
                                       y.data_ptr(), toa.data_ptr(), tot.data_ptr(), int(trig.numel()),
                                       trig.data_ptr(), int(cut), 0 if table is None else table.data_ptr(),
                                       0 if table is None else int(table.numel()), int(shot_base), xo.data_ptr(),
@@ -278,7 +287,7 @@ class Plan:
         _check_dev(raw, torch.uint64, n, "raw")
         out = torch.empty(max(n, 1), dtype=torch.uint64, device=self.device) if out is None else out
         wraps_out = torch.empty(1, dtype=torch.int64, device=self.device) if wraps_out is None else wraps_out
-        rc = self.lib.tpx3_unwrap_toa(self.handle, self.workspace.data_ptr(), _stream_ptr(stream), n, raw.data_ptr(),
+        rc = self.lib.tpx3_unwrap_toa(self.handle, self.workspace.data_ptr(), _stream_ptr(stream, self.device), n, raw.data_ptr(),
                                       int(modulus), int(jump), int(wraps_in), 0 if prev_raw is None else 1,
                                       0 if prev_raw is None else int(prev_raw), out.data_ptr(), wraps_out.data_ptr())
         if rc != OK:
@@ -296,7 +305,7 @@ class Plan:
         lmax = torch.empty(max(n, 1), dtype=torch.uint32, device=self.device) if lmax is None else lmax
         n_hits = torch.empty(1, dtype=torch.uint32, device=self.device) if n_hits is None else n_hits
         c = clusters._c()
-        rc = self.lib.tpx3_localmax_centroid(self.handle, self.workspace.data_ptr(), _stream_ptr(stream), n,
+        rc = self.lib.tpx3_localmax_centroid(self.handle, self.workspace.data_ptr(), _stream_ptr(stream, self.device), n,
                                              x.data_ptr(), y.data_ptr(), toa.data_ptr(), tot.data_ptr(), int(wx),
                                              int(wy), int(wt), perm.data_ptr(), lmax.data_ptr(),
                                              clusters.max_clusters, ctypes.byref(c), n_hits.data_ptr())
@@ -314,7 +323,7 @@ class Plan:
         _check_dev(label, torch.uint32, n, "label")
         n_clusters = torch.empty(1, dtype=torch.uint32, device=self.device) if n_clusters is None else n_clusters
         c = clusters._c()
-        rc = self.lib.tpx3_centroid(self.handle, self.workspace.data_ptr(), _stream_ptr(stream), n, x.data_ptr(),
+        rc = self.lib.tpx3_centroid(self.handle, self.workspace.data_ptr(), _stream_ptr(stream, self.device), n, x.data_ptr(),
                                     y.data_ptr(), toa.data_ptr(), tot.data_ptr(), perm.data_ptr(), label.data_ptr(),
                                     clusters.max_clusters, ctypes.byref(c), n_clusters.data_ptr())
         if rc != OK:
@@ -332,7 +341,7 @@ class Plan:
         label = torch.empty(max(n, 1), dtype=torch.uint32, device=self.device) if label is None else label
         n_clusters = torch.empty(1, dtype=torch.uint32, device=self.device) if n_clusters is None else n_clusters
         c = clusters._c()
-        rc = self.lib.tpx3_cluster_centroid(self.handle, self.workspace.data_ptr(), _stream_ptr(stream), n,
+        rc = self.lib.tpx3_cluster_centroid(self.handle, self.workspace.data_ptr(), _stream_ptr(stream, self.device), n,
                                             x.data_ptr(), y.data_ptr(), toa.data_ptr(), tot.data_ptr(),
                                             perm.data_ptr(), label.data_ptr(), clusters.max_clusters,
                                             ctypes.byref(c), n_clusters.data_ptr())
@@ -351,13 +360,20 @@ class Plan:
         import torch
 
         n = int(x.numel())
+        for t, dt, name in ((x, torch.uint16, "x"), (y, torch.uint16, "y"), (toa, torch.uint64, "toa"), (tot, torch.uint16, "tot")):
+            _check_host(t, dt, n, name)
+        for t, name in ((perm, "perm"), (label, "label")):
+            if t is not None:
+                _check_host(t, torch.uint32, n, name)
+        for name, dt in _CLUSTER_FIELDS:
+            _check_host(getattr(clusters_host, name), getattr(torch, dt), min(clusters_host.max_clusters, 1), name)
         need = int(self.lib.tpx3_host_io_bytes(n, clusters_host.max_clusters))
         if self._io is None or self._io.numel() < need:
             self._io = torch.empty(need, dtype=torch.uint8, device=self.device)
         nc = ctypes.c_uint32(0)
         c = clusters_host._c()
         rc = self.lib.tpx3_process_host(
-            self.handle, self.workspace.data_ptr(), self._io.data_ptr(), _stream_ptr(stream), n, x.data_ptr(),
+            self.handle, self.workspace.data_ptr(), self._io.data_ptr(), _stream_ptr(stream, self.device), n, x.data_ptr(),
             y.data_ptr(), toa.data_ptr(), tot.data_ptr(), perm.data_ptr() if perm is not None else None,
             label.data_ptr() if label is not None else None, clusters_host.max_clusters, ctypes.byref(c),
             ctypes.addressof(nc))
@@ -367,7 +383,7 @@ class Plan:
 
     def status(self, stream=None) -> dict:
         s = _CStatus()
-        rc = self.lib.tpx3_status(self.handle, self.workspace.data_ptr(), _stream_ptr(stream), ctypes.byref(s))
+        rc = self.lib.tpx3_status(self.handle, self.workspace.data_ptr(), _stream_ptr(stream, self.device), ctypes.byref(s))
         if rc != OK:
             raise Tpx3Error(rc, "tpx3_status")
         return {"error": -int(s.error), "path": int(s.path), "n_clusters": int(s.n_clusters),
@@ -426,7 +442,7 @@ class Stream:
                                device=pl.device)
         h = ctypes.c_void_p()
         rc = pl.lib.tpx3_stream_open(pl.handle, self.buf.data_ptr(), max_chunk, max_carry, disorder_ticks,
-                                     _stream_ptr(stream), ctypes.byref(h))
+                                     _stream_ptr(stream, pl.device), ctypes.byref(h))
         if rc != OK:
             raise Tpx3Error(rc, "tpx3_stream_open")
         self.handle = h
@@ -441,7 +457,7 @@ class Stream:
         n_hits = torch.empty(1, dtype=torch.uint32, device=pl.device) if n_hits is None else n_hits
         c = clusters._c()
         info = _CStreamInfo()
-        rc = pl.lib.tpx3_stream_push(self.handle, pl.workspace.data_ptr(), _stream_ptr(stream), n, x.data_ptr(),
+        rc = pl.lib.tpx3_stream_push(self.handle, pl.workspace.data_ptr(), _stream_ptr(stream, pl.device), n, x.data_ptr(),
                                      y.data_ptr(), toa.data_ptr(), tot.data_ptr(), 1 if final else 0,
                                      clusters.max_clusters, ctypes.byref(c), n_hits.data_ptr(), ctypes.byref(info))
         d = {k: int(getattr(info, k)) for k, _ in _CStreamInfo._fields_}

@@ -548,7 +548,7 @@ int tpx3_preprocess(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t 
                     uint16_t* x_out, uint16_t* y_out, uint64_t* toa_out, uint16_t* tot_out, uint32_t* index_out,
                     uint32_t* n_out) {
   if (!p || !workspace || !n_out) return TPX3_ERR_INVALID_ARG;
-  if (n > p->cfg.max_hits || p->cfg.shot_period_ticks == 0) return TPX3_ERR_INVALID_ARG;
+  if (n > p->cfg.max_hits || p->cfg.shot_period_ticks == 0 || (cut >> 63) != 0) return TPX3_ERR_INVALID_ARG;
   if (n && (!x || !y || !toa || !tot || !x_out || !y_out || !toa_out || !tot_out)) return TPX3_ERR_INVALID_ARG;
   if ((n_trig && !trig) || (table_len && !table)) return TPX3_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -574,6 +574,7 @@ struct tpx3_stream_s {
   uint32_t n_carry;          // host mirror of the device counter
   int bank;                  // which carry bank holds the carried events
   bool failed;
+  bool ended;                // a final push went through: the stream takes no more events
   tpx3::StreamCtrl* ctrl;
   uint16_t *cx[2], *cy[2], *ctot[2];
   uint64_t* ctoa[2];
@@ -618,7 +619,7 @@ int tpx3_stream_open(tpx3_plan_t p, void* stream_buf, uint64_t max_chunk, uint64
   const StreamLayout l = stream_layout(max_chunk, max_carry);
   char* b = (char*)stream_buf;
   s->plan = p; s->max_chunk = max_chunk; s->max_carry = max_carry; s->disorder = disorder_ticks;
-  s->n_carry = 0; s->bank = 0; s->failed = false;
+  s->n_carry = 0; s->bank = 0; s->failed = false; s->ended = false;
   s->ctrl = (tpx3::StreamCtrl*)(b + l.ctrl);
   for (int k = 0; k < 2; ++k) {
     s->cx[k] = (uint16_t*)(b + l.cx[k]); s->cy[k] = (uint16_t*)(b + l.cy[k]); s->ctot[k] = (uint16_t*)(b + l.ctot[k]);
@@ -638,7 +639,7 @@ int tpx3_stream_push(tpx3_stream_t s, void* workspace, void* cuda_stream, uint64
                      const tpx3_clusters_t* out, uint32_t* n_hits, tpx3_stream_info_t* info) {
   if (!s || !workspace || !out || !n_hits) return TPX3_ERR_INVALID_ARG;
   if (s->failed) return TPX3_ERR_CAPACITY;
-  if (n > s->max_chunk) return TPX3_ERR_INVALID_ARG;
+  if (s->ended || n > s->max_chunk) return TPX3_ERR_INVALID_ARG;
   if (n && (!x || !y || !toa || !tot)) return TPX3_ERR_INVALID_ARG;
   tpx3_plan_t p = s->plan;
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -952,7 +953,6 @@ const char* tpx3_strerror(int err) {
     case TPX3_ERR_CAPACITY: return "max_clusters too small";
     case TPX3_ERR_OUT_OF_RANGE: return "event outside the sensor or ToT == 0";
     case TPX3_ERR_CUDA: return "CUDA runtime error";
-    case TPX3_ERR_UNIMPLEMENTED: return "not implemented";
     default: return "unknown error";
   }
 }

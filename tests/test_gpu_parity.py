@@ -923,6 +923,39 @@ def _sizes(n, chunk):
     return [chunk] * (n // chunk) + ([n % chunk] if n % chunk else [])
 
 
+DEVICE_TMAX_TAIL = 65536   # tpx3.h: a push takes the running maximum over the last 65536 events of its chunk
+
+
+def _check_push_properties(infos, toa, sizes, D, honest=True):
+    """What a push emits is not part of the definition (oracle/preprocess.py StreamModel: any lower bound of the
+    running maximum is safe; the device samples the chunk's tail) — these properties are: nothing is lost or
+    emitted twice, a shot goes out in one piece and only when complete, labels continue the batch numbering,
+    and with an honest disorder bound D nothing is late and no shot goes out before it can be complete."""
+    shot = (np.asarray(toa) // np.uint64(P)).astype(np.int64)
+    n = len(shot)
+    consumed = emitted = late = 0
+    s_prev = 0
+    for info, sz in zip(infos, sizes):
+        consumed += sz
+        assert info["label_base"] == emitted
+        emitted += info["n_emitted"]
+        late += info["n_late"]
+        assert info["late_total"] == late
+        assert emitted + late + info["n_carry"] == consumed          # every event is emitted, late or carried
+        s_now = info["shots_emitted"]
+        assert s_now >= s_prev
+        s_prev = s_now
+        seen = shot[:consumed]
+        if honest:
+            assert info["n_late"] == 0
+            assert emitted == int(np.count_nonzero(seen < s_now))     # exactly the shots below s_now went out ...
+            assert not np.any(shot[consumed:] < s_now)                # ... and they were complete
+            if consumed < n or info["n_carry"]:
+                t_seen = int(np.asarray(toa[:consumed]).max()) if consumed else 0
+                assert s_now <= max(t_seen - D, 0) // P or s_now == 0 or consumed == n
+    assert consumed == n and infos[-1]["n_carry"] == 0 and emitted + late == n
+
+
 @pytest.mark.parametrize("cfg,shots,chunk", [(0, 1000, 997), (0, 300, 64), (1, 60, 100003), (1, 60, 1 << 20),
                                              (2, 8, 250007), (3, 40, 30011), (4, 1200, 65536), (4, 1200, 300001),
                                              (4, 1200, 1 << 22)])
@@ -937,8 +970,11 @@ def test_stream_equals_batch(tpx3, cfg, shots, chunk):
     o = oracle.run(w.x, w.y, w.toa, w.tot, W, P, threads=0)
     for k in _ROW_KEYS:
         np.testing.assert_array_equal(rows[k], o[k], err_msg=k)
-    for info, (ne, nk, nl, lb) in zip(infos, want):
-        assert (info["n_emitted"], info["n_carry"], info["n_late"], info["label_base"]) == (ne, nk, nl, lb)
+    sizes = _sizes(w.n, chunk)
+    _check_push_properties(infos, w.toa, sizes, D)
+    if chunk <= DEVICE_TMAX_TAIL or D == 0:   # the device's tail sample holds the true maximum: the model's very pushes
+        for info, (ne, nk, nl, lb) in zip(infos, want):
+            assert (info["n_emitted"], info["n_carry"], info["n_late"], info["label_base"]) == (ne, nk, nl, lb)
     assert infos[-1]["late_total"] == 0 and infos[-1]["n_carry"] == 0
     if chunk < w.n:
         assert max(i["n_carry"] for i in infos) > 0       # the cuts were not shot-aligned
@@ -954,6 +990,8 @@ def test_stream_random_chunks_and_empty_pushes(tpx3):
     o = oracle.run(w.x, w.y, w.toa, w.tot, W, P, threads=0)
     for k in _ROW_KEYS:
         np.testing.assert_array_equal(rows[k], o[k], err_msg=k)
+    _check_push_properties(infos, w.toa, sizes + [0], 0)
+    # a stream in ToA order: the chunk's largest ToA is its last event, so the device's tail sample is exact
     assert [(i["n_emitted"], i["n_carry"], i["n_late"]) for i in infos] == [t[:3] for t in want]
 
 
@@ -1035,6 +1073,58 @@ def test_stream_rejects_bad_arguments(tpx3):
     with pytest.raises(tpx3.Tpx3Error):
         pl0.stream_open(500, 200, 0)              # no shot period: nothing is ever complete
     pl0.free()
+
+
+def test_stream_takes_nothing_after_the_final_push(tpx3):
+    """tpx3.h: final "ends the stream". A later push is refused (it would cluster shots a second time)."""
+    w = gen.generate(0, shots=30)
+    pl = tpx3.plan(tpx3.Config(toa_window_ticks=W, shot_period_ticks=P, max_hits=w.n + 1000))
+    s = pl.stream_open(w.n, 1000, 0)
+    cl = tpx3.Clusters(w.n, pl.device)
+    dev = [to_dev(a) for a in (w.x, w.y, w.toa, w.tot)]
+    _, info = s.push(*dev, cl, final=True)
+    assert info["n_emitted"] == w.n
+    with pytest.raises(tpx3.Tpx3Error) as e:
+        s.push(*dev, cl, final=False)
+    assert e.value.code == tpx3.ERR_INVALID_ARG
+    s.close()
+    pl.free()
+
+
+def test_preprocess_rejects_a_cut_beyond_int64(tpx3):
+    import torch
+
+    pl = tpx3.plan(tpx3.Config(max_hits=16))
+    z16 = torch.zeros(4, dtype=torch.uint16, device="cuda")
+    z64 = torch.zeros(4, dtype=torch.uint64, device="cuda")
+    with pytest.raises(tpx3.Tpx3Error) as e:
+        pl.preprocess(z16, z16, z64, z16, z64, 1 << 63)
+    assert e.value.code == tpx3.ERR_INVALID_ARG
+    pl.free()
+
+
+def test_two_devices_in_one_process(tpx3):
+    """The opt-in to large dynamic shared memory is per device: a plan on cuda:1 made after one on cuda:0 must
+    serve the fused path too. Skipped on a box with one GPU."""
+    import torch
+
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    w = gen.generate(1, shots=300)
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P)
+    for dev in (0, 1):
+        with torch.cuda.device(dev):
+            pl = tpx3.plan(tpx3.Config(max_hits=w.n, device=dev, max_shot_hits=600))
+            d = [torch.from_numpy(a).to("cuda:%d" % dev) for a in (w.x, w.y, w.toa, w.tot)]
+            cl = tpx3.Clusters(w.n, pl.device)
+            perm, label, nc = pl.cluster_centroid(*d, cl)
+            torch.cuda.synchronize(dev)
+            st = pl.status()
+            assert st["error"] == 0 and st["path"] == 1, (dev, st)
+            g = {"perm": perm[: w.n].cpu().numpy(), "label": label[: w.n].cpu().numpy(), "n_clusters": int(nc.cpu().numpy()[0])}
+            g.update(cl.numpy(g["n_clusters"]))
+            assert_parity(g, o, "device %d" % dev)
+            pl.free()
 
 
 @pytest.mark.parametrize("cfg,shots,hint,pipelined", [(1, 24000, 1024, True), (4, 13000, 1536, True), (1, 24000, 1024, False)])

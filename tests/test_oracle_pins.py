@@ -699,3 +699,52 @@ def test_stream_carry_is_bounded_by_the_open_shots():
         e = m.push(*c)
         assert e["n_carry"] <= per_shot
         assert all(t // P >= m.s_emitted for t in (ev[2] for ev in m.carry))
+
+
+# ------------------------------------------------------------------ the oracle under the sanitizers
+def test_oracle_is_clean_under_asan_and_ubsan(tmp_path):
+    """oracle/tpx3_oracle.cpp rebuilt with -fsanitize=address,undefined (any report aborts the program) and run
+    on seeded inputs of every kind the pins use — in-order, shuffled, noise pixels, one event, none — gives the
+    outputs of the ordinary build, digest for digest, with nothing on stderr."""
+    import ctypes
+    import shutil
+    import subprocess
+
+    if shutil.which("g++") is None:
+        pytest.skip("g++ not available")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    exe = str(tmp_path / "oracle_asan")
+    cmd = ["g++", "-O1", "-g", "-std=c++17", "-fopenmp", "-fsanitize=address,undefined", "-fno-sanitize-recover=all",
+           os.path.join(root, "oracle", "sanitize_driver.cpp"), os.path.join(root, "oracle", "tpx3_oracle.cpp"), "-o", exe]
+    build = subprocess.run(cmd, capture_output=True, text=True)
+    if build.returncode != 0 and "sanitize" in build.stderr.lower():
+        pytest.skip("this toolchain has no sanitizer runtime: " + build.stderr[-200:])
+    assert build.returncode == 0, build.stderr
+
+    def fnv(h, a):
+        for b in np.ascontiguousarray(a).view(np.uint8).tobytes():
+            h = ((h ^ b) * 1099511628211) & 0xFFFFFFFFFFFFFFFF
+        return h
+
+    def digest(o, second):
+        h = 1469598103934665603
+        for k in ("perm", second, "c_label", "c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y",
+                  "c_toa_peak", "c_cx", "c_cy", "c_sum_tot_tof", "c_ctof"):
+            h = fnv(h, o[k])
+        return "%016x" % h
+
+    cases = [gen.generate(0, shots=60), gen.generate(4, shots=12), gen.generate(3, shots=3)]
+    one = gen.generate(0, shots=1)
+    for w, n in [(c, c.n) for c in cases] + [(one, 1), (one, 0)]:
+        d = tmp_path / ("case_%d_%d" % (w.cfg_id, n))
+        d.mkdir()
+        w.x[:n].tofile(d / "x.u16"); w.y[:n].tofile(d / "y.u16"); w.toa[:n].tofile(d / "toa.u64"); w.tot[:n].tofile(d / "tot.u16")
+        for threads in (1, 3):
+            r = subprocess.run([exe, str(d), str(W), str(P), "2", "1", "200", str(threads)], capture_output=True, text=True,
+                               env=dict(os.environ, ASAN_OPTIONS="detect_leaks=1:abort_on_error=0", UBSAN_OPTIONS="print_stacktrace=1"))
+            assert r.returncode == 0 and r.stderr.strip() == "", (r.returncode, r.stderr[-2000:])
+            lines = r.stdout.strip().splitlines()
+            o = oracle.run(w.x[:n], w.y[:n], w.toa[:n], w.tot[:n], W, P, threads=1)
+            lm = oracle.run_localmax(w.x[:n], w.y[:n], w.toa[:n], w.tot[:n], 2, 1, 200, P, threads=1)
+            assert lines[0] == "run n=%d hits=%d digest=%s" % (n, o["n_clusters"], digest(o, "label"))
+            assert lines[1] == "localmax n=%d hits=%d digest=%s" % (n, lm["n_clusters"], digest(lm, "lmax"))
