@@ -500,11 +500,12 @@ def run_stream(args):
         s = pl.stream_open(chunk, carry, D, stream=stream)
         hits = emitted = late = max_carry_seen = 0
         for a, b in zip(cuts[:-1], cuts[1:]):
-            _, info = s.push(*(d[a:b] for d in dev), cl, final=(b == n), n_hits=nc, stream=stream)
-            emitted += info["n_emitted"]
-            late += info["n_late"]
-            max_carry_seen = max(max_carry_seen, info["n_carry"])
+            # timed steps: nothing waits on the host (no per-push counts); the counting step reads them
+            _, info = s.push(*(d[a:b] for d in dev), cl, final=(b == n), n_hits=nc, stream=stream, want_info=count)
             if count:
+                emitted += info["n_emitted"]
+                late += info["n_late"]
+                max_carry_seen = max(max_carry_seen, info["n_carry"])
                 stream.synchronize()
                 hits += int(nc.cpu().numpy()[0])
         s.close()

@@ -447,8 +447,10 @@ class Stream:
             raise Tpx3Error(rc, "tpx3_stream_open")
         self.handle = h
 
-    def push(self, x, y, toa, tot, clusters: "Clusters", final: bool = False, n_hits=None, stream=None):
-        """Returns (n_hits device tensor, info dict). Synchronises the stream once."""
+    def push(self, x, y, toa, tot, clusters: "Clusters", final: bool = False, n_hits=None, stream=None,
+             want_info: bool = True):
+        """Returns (n_hits device tensor, info dict). With want_info the call synchronises the stream once to read
+        the per-push counts; without it nothing waits (info is None; a carry overflow shows in Plan.status())."""
         import torch
 
         pl = self.plan
@@ -459,8 +461,9 @@ class Stream:
         info = _CStreamInfo()
         rc = pl.lib.tpx3_stream_push(self.handle, pl.workspace.data_ptr(), _stream_ptr(stream, pl.device), n, x.data_ptr(),
                                      y.data_ptr(), toa.data_ptr(), tot.data_ptr(), 1 if final else 0,
-                                     clusters.max_clusters, ctypes.byref(c), n_hits.data_ptr(), ctypes.byref(info))
-        d = {k: int(getattr(info, k)) for k, _ in _CStreamInfo._fields_}
+                                     clusters.max_clusters, ctypes.byref(c), n_hits.data_ptr(),
+                                     ctypes.byref(info) if want_info else None)
+        d = {k: int(getattr(info, k)) for k, _ in _CStreamInfo._fields_} if want_info else None
         if rc != OK:
             e = Tpx3Error(rc, "tpx3_stream_push")
             e.info = d

@@ -130,10 +130,12 @@ __global__ void __launch_bounds__(256) k_accumulate(Ctrl* c, int general_only, u
 __global__ void __launch_bounds__(256) k_finalize(Ctrl* c, int general_only, Params p,
                                                 const uint64_t* __restrict__ toa, const uint32_t* __restrict__ perm,
                                                 const uint32_t* n_clusters, uint64_t max_clusters, tpx3_clusters_t out,
-                                                const unsigned long long* __restrict__ peak) {
+                                                const unsigned long long* __restrict__ peak,
+                                                const uint64_t* __restrict__ label_base) {
   if (general_only && c->fused_state == 1) return;
   uint64_t nc = *n_clusters;
   if (nc > max_clusters) nc = max_clusters;
+  const uint32_t lbase = label_base ? (uint32_t)*label_base : 0u;   // stream pushes: labels continue the batch numbering
   for (uint64_t s = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; s < nc; s += (uint64_t)gridDim.x * blockDim.x) {
     uint32_t kpeak = (uint32_t)(peak[s] & 0xFFFFFFFFull);
     out.toa_peak[s] = toa[perm[kpeak]];
@@ -144,6 +146,7 @@ __global__ void __launch_bounds__(256) k_finalize(Ctrl* c, int general_only, Par
     out.cx[s] = __fdiv_rn(__ll2float_rn(sx), fst);
     out.cy[s] = __fdiv_rn(__ll2float_rn(sy), fst);
     out.ctof[s] = __fdiv_rn(__ll2float_rn(out.sum_tot_tof[s]), fst);
+    if (lbase) out.label[s] += lbase;     // after the reads of out.label above
   }
 }
 

@@ -158,7 +158,44 @@ struct FusedArgs {
                        // 0: hit = connected component (north_star); 1: paper-literal mode, hit = local ToT
                        //    maximum of the box (lm_wx, lm_wy, W) and sums over that box (tpx3_localmax.cuh)
   uint32_t lm_wx, lm_wy;
+  const uint64_t* label_base;   // [dev] or null: added (low 32 bits) to the label column (stream pushes, R24)
+  const uint32_t* n_dev;        // [dev] or null: the event count is device state (a stream push): n, G, nseg, maxt and
+                                // num_tiles above are upper bounds then (they size the grids) and every kernel
+                                // derives the true ones from *n_dev; the staging table is laid out for the bound
 };
+
+// Segment length and status words per segment for n events in tiles of T (host and device: the ladder's rungs
+// are sized on the device). Segments of 8 windows keep the re-read of a segment's first window at a few per
+// cent; short inputs get shorter segments so that every SM has work. Two consecutive tiles that own something
+// advance by at least T - 7 events together (what one leaves behind, at most a shot, the next one takes), hence
+// the bound on status words. Measured and dropped: the stream's last wave in segments a quarter as long (cfg1
+// 4 % slower: every segment start re-reads half a shot).
+struct FusedSegs {
+  uint32_t G, nseg, maxt;
+};
+
+__host__ __device__ inline FusedSegs fused_segs(uint64_t n, uint32_t T, uint32_t num_sms) {
+  FusedSegs s;
+  uint64_t G = 8ull * T;
+  const uint64_t slots = (uint64_t)num_sms * (T <= 2048u ? 4u : (T <= 4096u ? 2u : 1u));   // resident CTAs
+  const uint64_t want = slots * 8ull;                        // segments to aim for (load balance)
+  if (n / G < want) {
+    G = (n / want + 7ull) & ~7ull;
+    if (G < 2ull * T) G = 2ull * T;
+  }
+  s.G = (uint32_t)G;
+  s.nseg = (uint32_t)((n + G - 1) / G);
+  s.maxt = 2u * (uint32_t)(G / T + 2u) + 2u;
+  return s;
+}
+
+__host__ __device__ inline void compact_grid(uint32_t num_tiles, uint32_t num_sms, uint32_t* ctas, uint32_t* tiles_per_cta) {
+  uint32_t c = num_tiles < num_sms * 8u ? num_tiles : num_sms * 8u;
+  if (c == 0) c = 1;
+  const uint32_t t = (num_tiles + c - 1) / c;
+  *tiles_per_cta = t ? t : 1u;
+  *ctas = t ? (num_tiles + t - 1) / t : 1u;
+}
 
 constexpr uint32_t kNone = 0xFFFFFFFFu;
 constexpr int kHalvePre = 2;    // pointer-halving rounds before the deferred unions
@@ -255,8 +292,16 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 
   // ---- the CTA walks its segment tile by tile ---------------------------------------------------------
   const uint32_t seg = blockIdx.x;
-  const uint64_t seg_begin = (uint64_t)seg * a.G;
-  const uint64_t seg_end = seg_begin + a.G < a.n ? seg_begin + a.G : a.n;
+  uint64_t n_ev = a.n;
+  uint32_t seg_G = a.G, seg_n = a.nseg, seg_maxt = a.maxt;
+  if (a.n_dev) {                     // a stream push: the count was decided on the device
+    n_ev = *a.n_dev;
+    const FusedSegs sg = fused_segs(n_ev, (uint32_t)T, a.num_sms);
+    seg_G = sg.G; seg_n = sg.nseg; seg_maxt = sg.maxt;
+    if (seg >= seg_n) return;        // the grid was sized for the largest count
+  }
+  const uint64_t seg_begin = (uint64_t)seg * seg_G;
+  const uint64_t seg_end = seg_begin + seg_G < n_ev ? seg_begin + seg_G : n_ev;
   const uint32_t P32 = (uint32_t)a.P;
   uint64_t tile_at = seg_begin;     // where the next tile starts; a shot start except for the segment's first tile
   bool at_start = seg == 0;         // tile_at is known to be a shot start
@@ -281,10 +326,10 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     misc->n_list = 0;
   }
   __syncthreads();
-  if (misc->skip != 0u || tile_i >= a.maxt) { seg_failed = tile_i >= a.maxt; break; }
+  if (misc->skip != 0u || tile_i >= seg_maxt) { seg_failed = tile_i >= seg_maxt; break; }
   const uint64_t base = tile_at & ~7ull;               // window start: aligned for the 128-bit loads
   const uint32_t skp = (uint32_t)(tile_at - base);     // window positions below skp belong to the previous tile
-  const uint64_t avail = a.n - base;                   // > 0 by construction
+  const uint64_t avail = n_ev - base;                  // > 0 by construction
   const uint32_t cnt = avail < (uint64_t)T ? (uint32_t)avail : (uint32_t)T;  // events readable
   const uint32_t e_rel = seg_end - base > (uint64_t)T ? kNone : (uint32_t)(seg_end - base);   // segment end in the window
   const uint32_t p0 = tid * IPT;                       // this thread's 8 window positions
@@ -418,7 +463,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   bool failed = misc->fail != 0;
   uint64_t next_at;               // where the next tile of this segment starts (>= seg_end: none)
   {
-    const bool to_end = base + cnt >= a.n;
+    const bool to_end = base + cnt >= n_ev;
     const uint32_t last = to_end ? cnt : misc->last;          // misc->last >= lo whenever lo exists
     if (lo == kNone) {            // no shot starts in this window: nothing owned, look further on
       lo = hi = 0;
@@ -434,7 +479,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         else failed = true;                    // a shot longer than the window
       }
     }
-    if (to_end && next_at >= base + cnt) next_at = a.n;
+    if (to_end && next_at >= base + cnt) next_at = n_ev;
   }
   // key layout: 2^tb > max tof + W, so keys of different shots differ by more than W
   const uint32_t tspan = misc->max_tof + a.W;
@@ -1321,7 +1366,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 
   // ---- the tile's status word (tiles that own something only); on to the segment's next tile -------------
   if (mm) {
-    if (tid == 0) a.tiles[(uint64_t)seg * a.maxt + tile_i] = ((unsigned long long)out_base << 32) | (unsigned long long)n_roots;
+    if (tid == 0) a.tiles[(uint64_t)seg * seg_maxt + tile_i] = ((unsigned long long)out_base << 32) | (unsigned long long)n_roots;
     ++tile_i;
   }
   if (failed) { seg_failed = true; break; }
@@ -1332,12 +1377,12 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 
   // ---- completion: the last segment to finish publishes the outcome of the call -------------------
   if (tid == 0) {
-    for (uint32_t i = tile_i; i < a.maxt; ++i) a.tiles[(uint64_t)seg * a.maxt + i] = 0ull;
+    for (uint32_t i = tile_i; i < seg_maxt; ++i) a.tiles[(uint64_t)seg * seg_maxt + i] = 0ull;
     if (seg_failed) atomicExch(&a.ctrl->fused_fail, 1u);
     if (tile_i) atomicAdd(&a.ctrl->tiles_run, tile_i);
     __threadfence();
     const uint32_t done = atomicAdd(&a.ctrl->tiles_done, 1u);
-    if (done + 1u == a.nseg) {
+    if (done + 1u == seg_n) {
       __threadfence();
       const uint32_t any_fail = atomicAdd(&a.ctrl->fused_fail, 0u);
       // 2: the general kernels behind this one redo the call; 1: k_fused_compact finishes it
@@ -1355,8 +1400,15 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 // fp32(sum tot*x) / fp32(sum tot), IEEE RN (Eq. 9).
 constexpr int kCompactThreads = 256;
 
-__global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, uint32_t tiles_per_cta) {
+__global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, uint32_t tiles_per_cta, uint32_t T) {
   if (a.ctrl->fused_state != 1u) return;   // the fused kernel gave up: the general path redoes the call
+  if (a.n_dev) {                           // a stream push: the true geometry from the device's count
+    const FusedSegs sg = fused_segs((uint64_t)*a.n_dev, T, a.num_sms);
+    a.num_tiles = sg.nseg * sg.maxt;
+    uint32_t ctas;
+    compact_grid(a.num_tiles, a.num_sms, &ctas, &tiles_per_cta);
+    if (blockIdx.x >= ctas) return;
+  }
   __shared__ unsigned long long s_part[kCompactThreads / 32];
   __shared__ unsigned long long s_prefix;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
@@ -1376,6 +1428,7 @@ __global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, 
   }
   __syncthreads();
   unsigned long long prefix = s_prefix;
+  const uint32_t label_base = a.label_base ? (uint32_t)*a.label_base : 0u;
   bool over = false;
   // the CTA's tiles in groups of 32: warp 0 turns the group's hit counts into offsets, then all threads walk the
   // group's hits as ONE index range (a tile has about 300 hits: a loop per tile would leave most of the last
@@ -1414,7 +1467,7 @@ __global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, 
       const long long st = (long long)va.z;
       const long long sx = (long long)(((unsigned long long)vb.y << 32) | vb.x);
       const long long sy = (long long)(((unsigned long long)vb.w << 32) | vb.z);
-      a.out.label[o] = va.x;
+      a.out.label[o] = va.x + label_base;
       a.out.size[o] = va.y;
       a.out.shot[o] = (uint32_t)div64(toa_peak, a.divP);
       a.out.sum_tot[o] = st;
@@ -1464,31 +1517,6 @@ inline FusedGeom fused_geom(uint64_t P, uint32_t W, uint32_t max_shot_hits) {
   return g;
 }
 
-// Segment length and status words per segment for n events in tiles of T (host and device: the ladder's rungs
-// are sized on the device). Segments of 8 windows keep the re-read of a segment's first window at a few per
-// cent; short inputs get shorter segments so that every SM has work. Two consecutive tiles that own something
-// advance by at least T - 7 events together (what one leaves behind, at most a shot, the next one takes), hence
-// the bound on status words. Measured and dropped: the stream's last wave in segments a quarter as long (cfg1
-// 4 % slower: every segment start re-reads half a shot).
-struct FusedSegs {
-  uint32_t G, nseg, maxt;
-};
-
-__host__ __device__ inline FusedSegs fused_segs(uint64_t n, uint32_t T, uint32_t num_sms) {
-  FusedSegs s;
-  uint64_t G = 8ull * T;
-  const uint64_t slots = (uint64_t)num_sms * (T <= 2048u ? 4u : (T <= 4096u ? 2u : 1u));   // resident CTAs
-  const uint64_t want = slots * 8ull;                        // segments to aim for (load balance)
-  if (n / G < want) {
-    G = (n / want + 7ull) & ~7ull;
-    if (G < 2ull * T) G = 2ull * T;
-  }
-  s.G = (uint32_t)G;
-  s.nseg = (uint32_t)((n + G - 1) / G);
-  s.maxt = 2u * (uint32_t)(G / T + 2u) + 2u;
-  return s;
-}
-
 template <int T, int THREADS, int MODE>
 inline int launch_fused(const FusedArgs& a, cudaStream_t st) {
   k_fused_shot_tiles<T, THREADS, MODE><<<a.nseg, THREADS, FusedSmem<T>::kBytes, st>>>(a);
@@ -1528,7 +1556,8 @@ inline FusedLadder fused_ladder(uint32_t max_shot_hits) {
 inline FusedArgs make_fused_args(uint32_t T, uint32_t num_sms, Ctrl* ctrl, unsigned long long* tiles, const Params& prm,
                                  const uint16_t* x, const uint16_t* y, const uint64_t* toa, const uint16_t* tot,
                                  uint32_t* perm, uint32_t* label, uint64_t max_clusters, const tpx3_clusters_t& out,
-                                 uint32_t* n_clusters, void* stage, uint32_t mode, uint32_t lm_wx, uint32_t lm_wy) {
+                                 uint32_t* n_clusters, void* stage, uint32_t mode, uint32_t lm_wx, uint32_t lm_wy,
+                                 const uint32_t* n_dev = nullptr) {
   FusedArgs a;
   a.ctrl = ctrl;
   a.tiles = tiles;
@@ -1557,15 +1586,19 @@ inline FusedArgs make_fused_args(uint32_t T, uint32_t num_sms, Ctrl* ctrl, unsig
   a.stage_c = reinterpret_cast<uint64_t*>(a.stage_b + prm.n);
   a.stage_d = a.stage_c + prm.n;
   a.mode = mode; a.lm_wx = lm_wx; a.lm_wy = lm_wy;
+  a.label_base = nullptr;
+  a.n_dev = n_dev;      // then prm.n is the largest count: it sizes the grids and lays out the staging table
   return a;
 }
 
-__host__ __device__ inline void compact_grid(uint32_t num_tiles, uint32_t num_sms, uint32_t* ctas, uint32_t* tiles_per_cta) {
-  uint32_t c = num_tiles < num_sms * 8u ? num_tiles : num_sms * 8u;
-  if (c == 0) c = 1;
-  const uint32_t t = (num_tiles + c - 1) / c;
-  *tiles_per_cta = t ? t : 1u;
-  *ctas = t ? (num_tiles + t - 1) / t : 1u;
+// The fields that depend on the event count (a stream push learns it on the device).
+__host__ __device__ inline void fused_set_n(FusedArgs& a, uint64_t n, uint32_t T) {
+  a.n = n;
+  const FusedSegs sg = fused_segs(n, T, a.num_sms);
+  a.G = sg.G; a.nseg = sg.nseg; a.maxt = sg.maxt; a.num_tiles = sg.nseg * sg.maxt;
+  a.stage_b = a.stage_a + n;
+  a.stage_c = reinterpret_cast<uint64_t*>(a.stage_b + n);
+  a.stage_d = a.stage_c + n;
 }
 
 // Device side: the next rung, tail-launched by k_fallback_dispatch.
@@ -1574,7 +1607,12 @@ __device__ inline void launch_fused_rung_device(FusedArgs a, uint32_t T) {
   compact_grid(a.num_tiles, a.num_sms, &ctas, &tpc);
 #define TPX3_RUNG(T_, THREADS_, MODE_) \
   k_fused_shot_tiles<T_, THREADS_, MODE_><<<a.nseg, THREADS_, FusedSmem<T_>::kBytes, cudaStreamTailLaunch>>>(a)
-  if (T == 4096u) {
+  if (T == 2048u) {
+    if (a.mode == 0u) TPX3_RUNG(2048, 256, 0);
+    else if (a.mode == 1u) TPX3_RUNG(2048, 256, 1);
+    else if (a.mode == 2u) TPX3_RUNG(2048, 256, 2);
+    else TPX3_RUNG(2048, 256, 3);
+  } else if (T == 4096u) {
     if (a.mode == 0u) TPX3_RUNG(4096, 512, 0);
     else if (a.mode == 1u) TPX3_RUNG(4096, 512, 1);
     else if (a.mode == 2u) TPX3_RUNG(4096, 512, 2);
@@ -1586,7 +1624,7 @@ __device__ inline void launch_fused_rung_device(FusedArgs a, uint32_t T) {
     else TPX3_RUNG(8192, 1024, 3);
   }
 #undef TPX3_RUNG
-  k_fused_compact<<<ctas, kCompactThreads, 0, cudaStreamTailLaunch>>>(a, tpc);
+  k_fused_compact<<<ctas, kCompactThreads, 0, cudaStreamTailLaunch>>>(a, tpc, T);
 }
 
 // Host side. Returns TPX3_OK (launched or not applicable; *launched says which) or an error. *args receives the
@@ -1595,14 +1633,21 @@ inline int enqueue_fused(const FusedGeom& g, uint32_t num_sms, uint64_t* launche
                          cudaStream_t st, const Params& prm, const uint16_t* x, const uint16_t* y,
                          const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label,
                          uint64_t max_clusters, const tpx3_clusters_t& out, uint32_t* n_clusters, void* stage,
-                         bool* launched, FusedArgs* args, uint32_t mode = 0, uint32_t lm_wx = 0, uint32_t lm_wy = 0) {
+                         bool* launched, FusedArgs* args, uint32_t mode = 0, uint32_t lm_wx = 0, uint32_t lm_wy = 0,
+                         const uint32_t* n_dev = nullptr, const uint64_t* label_base = nullptr) {
   *launched = false;
   if (g.variant == 0 || prm.n == 0) return TPX3_OK;
   // the 128-bit load phase needs 16-byte aligned inputs (PyTorch allocations are 256-byte aligned)
   if ((((uintptr_t)x | (uintptr_t)y | (uintptr_t)toa | (uintptr_t)tot) & 15u) != 0) return TPX3_OK;
   if (mode == 3u && ((uintptr_t)perm & 15u) != 0) return TPX3_OK;
-  const FusedArgs a = make_fused_args(g.T, num_sms, ctrl, tiles, prm, x, y, toa, tot, perm, label, max_clusters, out,
-                                      n_clusters, stage, mode, lm_wx, lm_wy);
+  FusedArgs a = make_fused_args(g.T, num_sms, ctrl, tiles, prm, x, y, toa, tot, perm, label, max_clusters, out,
+                                n_clusters, stage, mode, lm_wx, lm_wy, n_dev);
+  a.label_base = label_base;
+  if (n_dev) {   // grids that cover every count up to prm.n (fused_segs: a short input is cut into up to `want` segments)
+    const uint32_t want = num_sms * (g.T <= 2048u ? 4u : (g.T <= 4096u ? 2u : 1u)) * 8u + 1u;
+    if (a.nseg < want) a.nseg = want;
+    a.num_tiles = a.nseg * 22u;     // maxt <= 2 * (8 + 2) + 2
+  }
   *args = a;
   int rc;
 #define TPX3_PICK(MODE_)                                                \
@@ -1617,7 +1662,7 @@ inline int enqueue_fused(const FusedGeom& g, uint32_t num_sms, uint64_t* launche
   ++*launches;
   uint32_t ctas, tiles_per_cta;
   compact_grid(a.num_tiles, num_sms, &ctas, &tiles_per_cta);
-  k_fused_compact<<<ctas, kCompactThreads, 0, st>>>(a, tiles_per_cta);
+  k_fused_compact<<<ctas, kCompactThreads, 0, st>>>(a, tiles_per_cta, g.T);
   if (cudaGetLastError() != cudaSuccess) return TPX3_ERR_CUDA;
   ++*launches;
   *launched = true;

@@ -45,7 +45,7 @@ namespace {
 
 inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
-inline uint32_t table_size_for(uint64_t n) {  // power of two >= 2n, >= 1024
+__host__ __device__ inline uint32_t table_size_for(uint64_t n) {  // power of two >= 2n, >= 1024
   uint64_t s = 1024;
   while (s < 2 * n) s <<= 1;
   return (uint32_t)s;
@@ -134,7 +134,17 @@ struct GenArgs {
   tpx3_clusters_t out;
   uint32_t lm_wx, lm_wy;   // paper-literal mode: box half-widths
   uint64_t lm_wt;
+  const uint64_t* label_base;   // [dev] or null (stream pushes): added to the label column
 };
+
+// The fields that depend on the event count (a stream push learns it on the device).
+__host__ __device__ inline void gen_set_n(GenArgs& a, uint64_t n) {
+  a.prm.n = n;
+  a.g = sort_geom(n);
+  a.tsize = table_size_for(n);
+  a.cent_nblk = (uint32_t)((n + kCentTile - 1) / kCentTile);
+  if (a.cent_nblk == 0) a.cent_nblk = 1;
+}
 
 __host__ __device__ inline uint32_t grid_for_hd(uint64_t n, int threads, int num_sms, int per_sm = 8) {
   uint64_t b = (n + threads - 1) / threads;
@@ -195,7 +205,7 @@ __host__ __device__ inline uint32_t grid_for_hd(uint64_t n, int threads, int num
        (A).w.peak);                \
     GP(TPX3_STAGE_CENTROID, k_finalize,                                                                               \
        grid_for_hd((A).max_clusters < n_ ? (A).max_clusters : n_, 256, (A).sms), 256, (A).w.ctrl, (A).general_only,   \
-       (A).prm, (A).toa, (A).perm, (A).n_clusters, (A).max_clusters, (A).out, (A).w.peak);                            \
+       (A).prm, (A).toa, (A).perm, (A).n_clusters, (A).max_clusters, (A).out, (A).w.peak, (A).label_base);            \
   } while (0)
 
 // Paper-literal mode on the general kernels: the sort stage, then the window walks of tpx3_localmax.cuh. The
@@ -228,6 +238,12 @@ __host__ __device__ inline uint32_t grid_for_hd(uint64_t n, int threads, int num
 __global__ void k_fallback_dispatch(GenArgs a, FusedArgs fa, FusedLadder ladder, int rung, int what) {
   Ctrl* c = a.w.ctrl;
   if (c->fused_state == 1u) return;
+  if (fa.n_dev) {                       // a stream push: the count is device state
+    const uint64_t n = *fa.n_dev;
+    if (n == 0) return;
+    gen_set_n(a, n);
+    fa.n = n;
+  }
   if (rung < ladder.n) {
     c->tiles_done = 0; c->fused_fail = 0; c->fused_state = 0; c->tight_tiles = 0; c->tiles_run = 0;
     const FusedSegs sg = fused_segs(fa.n, ladder.T[rung], fa.num_sms);
@@ -253,11 +269,7 @@ GenArgs make_gen_args(tpx3_plan_s* p, const Ws& w, int general_only, uint64_t n,
   memset(&a, 0, sizeof(a));
   a.w = w;
   a.prm = p->prm;
-  a.prm.n = n;
-  a.g = sort_geom(n);
-  a.tsize = table_size_for(n);
-  a.cent_nblk = (uint32_t)((n + kCentTile - 1) / kCentTile);
-  if (a.cent_nblk == 0) a.cent_nblk = 1;
+  gen_set_n(a, n);
   a.sms = p->num_sms;
   a.general_only = general_only;
   a.x = x; a.y = y; a.tot = tot; a.toa = toa;
@@ -407,13 +419,17 @@ int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace
 static int run_fused_or_general(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x,
                                 const uint16_t* y, const uint64_t* toa, const uint16_t* tot, uint32_t* perm,
                                 uint32_t* label, uint64_t max_clusters, const tpx3_clusters_t* out, uint32_t* n_clusters,
-                                uint32_t mode) {
+                                uint32_t mode, const tpx3::StreamCtrl* sc = nullptr) {
+  // sc != null: a stream push. n is then the LARGEST count the push can emit; the true one (sc->n_work) is
+  // device state that every kernel reads for itself, so the host never waits for it.
+  const uint32_t* n_dev = sc ? &sc->n_work : nullptr;
+  const uint64_t* label_base = sc ? &sc->label_base : nullptr;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
   Ws w = carve(p, workspace);
   if (p->profiling) ++p->profiled_calls;
   const bool try_fused = !(p->cfg.flags & TPX3_FLAG_FORCE_GENERAL) && p->fused.variant != 0 && n != 0;
-  TPX3_LAUNCH(p, k_ctrl_init, 1, 256, 0, st, w.ctrl, n, w.tiles, 0u, n_clusters);
+  TPX3_LAUNCH(p, k_ctrl_init, 1, 256, 0, st, w.ctrl, n, w.tiles, 0u, n_clusters, n_dev, sc ? &sc->dead : nullptr);
   if (n == 0) return cuda_ok(cudaGetLastError());
   Params prm = p->prm;
   prm.n = n;
@@ -421,12 +437,22 @@ static int run_fused_or_general(tpx3_plan_t p, void* workspace, void* cuda_strea
   tpx3_clusters_t none;
   memset(&none, 0, sizeof(none));
   GenArgs ga = make_gen_args(p, w, mode == 2u ? 0 : 1, n, x, y, toa, tot, perm, label, max_clusters, out, n_clusters);
+  ga.label_base = label_base;
+  if (sc && !try_fused) {   // general kernels only: launched from the device, which knows the count
+    FusedArgs fa = make_fused_args(2048u, (uint32_t)p->num_sms, w.ctrl, w.tiles, prm, x, y, toa, tot, perm, label,
+                                   max_clusters, out ? *out : none, n_clusters, (char*)workspace + p->off_keyA, mode, 0u,
+                                   0u, n_dev);
+    k_fallback_dispatch<<<1, 1, 0, st>>>(ga, fa, FusedLadder{0, {0, 0}}, 0, (int)mode);
+    ++p->launches;
+    return cuda_ok(cudaGetLastError());
+  }
   if (try_fused) {
     bool launched = false;
     StageTimer timer(p, st, TPX3_STAGE_FUSED);
     FusedArgs fa;
     rc = enqueue_fused(p->fused, (uint32_t)p->num_sms, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm, label,
-                       max_clusters, out ? *out : none, n_clusters, (char*)workspace + p->off_keyA, &launched, &fa, mode);
+                       max_clusters, out ? *out : none, n_clusters, (char*)workspace + p->off_keyA, &launched, &fa, mode,
+                       0u, 0u, n_dev, label_base);
     if (rc != TPX3_OK) return rc;
     if (launched) {
       // the next rung or the general path, only if the fused kernel gave up: decided and enqueued on the device
@@ -571,7 +597,6 @@ int tpx3_preprocess(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t 
 struct tpx3_stream_s {
   tpx3_plan_t plan;
   uint64_t max_chunk, max_carry, disorder;
-  uint32_t n_carry;          // host mirror of the device counter
   int bank;                  // which carry bank holds the carried events
   bool failed;
   bool ended;                // a final push went through: the stream takes no more events
@@ -619,7 +644,7 @@ int tpx3_stream_open(tpx3_plan_t p, void* stream_buf, uint64_t max_chunk, uint64
   const StreamLayout l = stream_layout(max_chunk, max_carry);
   char* b = (char*)stream_buf;
   s->plan = p; s->max_chunk = max_chunk; s->max_carry = max_carry; s->disorder = disorder_ticks;
-  s->n_carry = 0; s->bank = 0; s->failed = false; s->ended = false;
+  s->bank = 0; s->failed = false; s->ended = false;
   s->ctrl = (tpx3::StreamCtrl*)(b + l.ctrl);
   for (int k = 0; k < 2; ++k) {
     s->cx[k] = (uint16_t*)(b + l.cx[k]); s->cy[k] = (uint16_t*)(b + l.cy[k]); s->ctot[k] = (uint16_t*)(b + l.ctot[k]);
@@ -641,39 +666,44 @@ int tpx3_stream_push(tpx3_stream_t s, void* workspace, void* cuda_stream, uint64
   if (s->failed) return TPX3_ERR_CAPACITY;
   if (s->ended || n > s->max_chunk) return TPX3_ERR_INVALID_ARG;
   if (n && (!x || !y || !toa || !tot)) return TPX3_ERR_INVALID_ARG;
+  if (max_clusters && !clusters_ok(out)) return TPX3_ERR_INVALID_ARG;
   tpx3_plan_t p = s->plan;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
   tpx3::StreamArgs a;
-  a.c = s->ctrl; a.n = n; a.n_carry = s->n_carry; a.carry_cap = (uint32_t)s->max_carry;
+  a.c = s->ctrl; a.n = n; a.carry_cap = (uint32_t)s->max_carry;
   a.x = x; a.y = y; a.tot = tot; a.toa = toa;
   const int in = s->bank, ob = s->bank ^ 1;
   a.cx = s->cx[in]; a.cy = s->cy[in]; a.ctot = s->ctot[in]; a.ctoa = s->ctoa[in];
   a.nx = s->cx[ob]; a.ny = s->cy[ob]; a.ntot = s->ctot[ob]; a.ntoa = s->ctoa[ob];
   a.wx = s->wx; a.wy = s->wy; a.wtot = s->wtot; a.wtoa = s->wtoa;
   a.blk_emit = s->blk_emit; a.blk_keep = s->blk_keep;
-  a.nblk = (uint32_t)((n + s->n_carry + tpx3::kStreamTile - 1) / tpx3::kStreamTile);
+  // the number of carried events is device state: the grids cover the largest it can be (blocks past the end
+  // of carried ++ chunk count nothing and return)
+  a.nblk = (uint32_t)((n + s->max_carry + tpx3::kStreamTile - 1) / tpx3::kStreamTile);
   a.P = p->cfg.shot_period_ticks; a.D = s->disorder; a.final_push = final_push ? 1 : 0;
-  if (n) TPX3_LAUNCH(p, tpx3::k_stream_cut, 64, 256, 0, st, a);
-  if (a.nblk) TPX3_LAUNCH(p, tpx3::k_stream_mark, a.nblk, tpx3::kStreamThreads, 0, st, a);
+  TPX3_LAUNCH(p, tpx3::k_stream_cut, n ? 64 : 1, 256, 0, st, a);
+  TPX3_LAUNCH(p, tpx3::k_stream_mark, a.nblk, tpx3::kStreamThreads, 0, st, a);
   TPX3_LAUNCH(p, tpx3::k_stream_scan, 1, 1024, 0, st, a);
-  if (a.nblk) TPX3_LAUNCH(p, tpx3::k_stream_scatter, a.nblk, tpx3::kStreamThreads, 0, st, a);
+  TPX3_LAUNCH(p, tpx3::k_stream_scatter, a.nblk, tpx3::kStreamThreads, 0, st, a);
+  s->bank = ob;
+  // clustering of the emit arrays: enqueued now with grids for the largest emit count; the kernels read the true
+  // count (and the label offset) from the stream state
+  {
+    const int rc = run_fused_or_general(p, workspace, cuda_stream, n + s->max_carry, s->wx, s->wy, s->wtoa, s->wtot,
+                                        s->wperm, s->wlabel, max_clusters, out, n_hits, 0u, s->ctrl);
+    if (rc != TPX3_OK) return rc;
+  }
+  if (cudaGetLastError() != cudaSuccess) return TPX3_ERR_CUDA;
+  if (final_push) s->ended = true;
+  if (!info) return TPX3_OK;            // fully asynchronous: a carry overflow shows in tpx3_status (TPX3_ERR_CAPACITY)
   tpx3::StreamCtrl h;
   if (cudaMemcpyAsync(&h, s->ctrl, sizeof(h), cudaMemcpyDeviceToHost, st) != cudaSuccess) return TPX3_ERR_CUDA;
-  if (cudaStreamSynchronize(st) != cudaSuccess) return TPX3_ERR_CUDA;   // the emit count sizes the clustering call
-  s->bank = ob;
-  s->n_carry = h.n_carry;
-  if (info) {
-    info->n_emitted = h.n_work; info->n_carry = h.n_carry; info->n_late = h.n_late; info->late_total = h.late_total;
-    info->label_base = h.label_base; info->shots_emitted = h.final_push ? h.s_emitted : h.s_cut;
-  }
-  if (h.overflow) { s->failed = true; return TPX3_ERR_CAPACITY; }
-  int rc = tpx3_cluster_centroid(p, workspace, cuda_stream, h.n_work, s->wx, s->wy, s->wtoa, s->wtot, s->wperm,
-                                 s->wlabel, max_clusters, out, n_hits);
-  if (rc != TPX3_OK) return rc;
-  if (h.n_work && max_clusters)
-    TPX3_LAUNCH(p, tpx3::k_stream_labels, p->num_sms, 256, 0, st, s->ctrl, n_hits, max_clusters, out->label);
-  return cuda_ok(cudaGetLastError());
+  if (cudaStreamSynchronize(st) != cudaSuccess) return TPX3_ERR_CUDA;
+  info->n_emitted = h.n_work; info->n_carry = h.n_carry; info->n_late = h.n_late; info->late_total = h.late_total;
+  info->label_base = h.label_base; info->shots_emitted = h.final_push ? h.s_emitted : h.s_cut;
+  if (h.dead) { s->failed = true; return TPX3_ERR_CAPACITY; }
+  return TPX3_OK;
 }
 
 int tpx3_stream_close(tpx3_stream_t s) {

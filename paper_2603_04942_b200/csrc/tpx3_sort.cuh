@@ -26,7 +26,7 @@ struct SortGeom {
   uint32_t tiles_per_blk;   // tiles each block walks sequentially
 };
 
-inline SortGeom sort_geom(uint64_t n) {
+__host__ __device__ inline SortGeom sort_geom(uint64_t n) {
   uint64_t tiles = (n + kSortTile - 1) / kSortTile;
   SortGeom g;
   g.nblk = (uint32_t)(tiles < (uint64_t)kSortMaxBlocks ? (tiles ? tiles : 1) : kSortMaxBlocks);
@@ -38,11 +38,13 @@ inline SortGeom sort_geom(uint64_t n) {
 // ---- min / max ToA ------------------------------------------------------------------------
 // Also clears the fused path's tile status words and the caller's hit counter.
 __global__ void __launch_bounds__(256) k_ctrl_init(Ctrl* c, uint64_t n, unsigned long long* tiles, uint32_t num_tiles,
-                                                 uint32_t* n_clusters) {
+                                                 uint32_t* n_clusters, const uint32_t* n_dev = nullptr,
+                                                 const uint32_t* dead = nullptr) {
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i == 0) {
     c->status.error = 0; c->status.path = 0; c->status.n_clusters = 0; c->status.sort_passes = 0;
-    c->status.n = n;
+    c->status.n = n_dev ? (uint64_t)*n_dev : n;                              // stream push: the device's count
+    if (dead && *dead) c->status.error = (uint32_t)(-TPX3_ERR_CAPACITY);   // ... and a carry overflow of the stream
     c->toa_min = ~0ull; c->toa_max = 0ull; c->npass = 1; c->fused_state = 0; c->tile_ticket = 0; c->n_roots = 0;
     c->tiles_done = 0; c->fused_fail = 0; c->tight_tiles = 0; c->tiles_run = 0;
     if (n_clusters) *n_clusters = 0;

@@ -10,8 +10,10 @@
 //                     events to emit (s_emitted <= shot < s_cut) and to carry (shot >= s_cut); the rest is late
 //   k_stream_scan     exclusive scans of both counts (one block), totals and the new stream state
 //   k_stream_scatter  order-preserving compaction into the emit arrays and the new carry arrays
-//   (host)            reads the two counts, then runs tpx3_cluster_centroid on the emit arrays
-//   k_stream_labels   label += events emitted by earlier pushes: rows continue the batch numbering
+//   k_stream_dispatch (tpx3_lib.cu, one thread) reads the emit count and launches the clustering of the emit arrays
+//                     from the device (tile kernel, compaction, fallback dispatcher): the host never waits for
+//                     the count. The compaction adds the events emitted by earlier pushes to the label column,
+//                     so the rows continue the batch numbering.
 // Shots are compared as times (t_lo = s_emitted * P <= ToA < t_cut = s_cut * P): no division per event.
 #pragma once
 #include "tpx3_centroid.cuh"
@@ -33,14 +35,14 @@ struct StreamCtrl {
   uint64_t label_next;   // ... including this one
   uint64_t late_total;
   uint32_t n_work, n_carry, n_late, overflow;
-  uint32_t final_push, pad;
+  uint32_t final_push, dead;   // dead: a push overflowed the carry; every later push reports TPX3_ERR_CAPACITY
+  uint32_t n_carry_in, pad;    // the carry this push started with (n_carry is overwritten by its scan)
 };
 
 struct StreamArgs {
   StreamCtrl* c;
   uint64_t n;            // chunk
-  uint32_t n_carry;      // carried in (host mirror of c->n_carry)
-  uint32_t carry_cap;
+  uint32_t carry_cap;    // (the number of carried events is device state: c->n_carry_in)
   const uint16_t *x, *y, *tot;      // chunk
   const uint64_t* toa;
   const uint16_t *cx, *cy, *ctot;   // carried in
@@ -58,12 +60,14 @@ struct StreamArgs {
 __global__ void __launch_bounds__(256) k_stream_open(StreamCtrl* c) {
   if (threadIdx.x == 0 && blockIdx.x == 0) {
     c->t_max = 0; c->s_emitted = 0; c->s_cut = 0; c->t_lo = 0; c->t_cut = 0; c->label_base = 0; c->label_next = 0; c->late_total = 0;
-    c->n_work = 0; c->n_carry = 0; c->n_late = 0; c->overflow = 0; c->final_push = 0; c->pad = 0;
+    c->n_work = 0; c->n_carry = 0; c->n_late = 0; c->overflow = 0; c->final_push = 0; c->dead = 0; c->n_carry_in = 0; c->pad = 0;
   }
 }
 
-// Running maximum over the chunk's last kStreamSample events: 64 blocks, one atomicMax each.
+// Running maximum over the chunk's last kStreamSample events: 64 blocks, one atomicMax each. Also the first
+// kernel of a push: records the carry the push starts with.
 __global__ void __launch_bounds__(256) k_stream_cut(StreamArgs a) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) a.c->n_carry_in = a.c->n_carry;
   const uint64_t m = a.n < kStreamSample ? a.n : kStreamSample;
   const uint64_t beg = a.n - m;
   unsigned long long v = 0;
@@ -97,8 +101,8 @@ __device__ __forceinline__ uint32_t stream_class(uint64_t t, uint64_t t_lo, uint
   return (final_push || t < t_cut) ? 1u : 2u;
 }
 
-__device__ __forceinline__ uint64_t stream_toa(const StreamArgs& a, uint64_t v) {
-  return v < a.n_carry ? a.ctoa[v] : a.toa[v - a.n_carry];
+__device__ __forceinline__ uint64_t stream_toa(const StreamArgs& a, uint32_t n_carry, uint64_t v) {
+  return v < n_carry ? a.ctoa[v] : a.toa[v - n_carry];
 }
 
 __global__ void __launch_bounds__(kStreamThreads) k_stream_mark(StreamArgs a) {
@@ -107,14 +111,15 @@ __global__ void __launch_bounds__(kStreamThreads) k_stream_mark(StreamArgs a) {
   __syncthreads();
   uint64_t t_lo, t_cut;
   stream_cut(a, t_lo, t_cut);
-  const uint64_t nv = a.n + a.n_carry;
-  const uint64_t base = (uint64_t)blockIdx.x * kStreamTile;
+  const uint32_t n_carry = a.c->n_carry_in;
+  const uint64_t nv = a.n + n_carry;
+  const uint64_t base = (uint64_t)blockIdx.x * kStreamTile;     // the grid covers n + carry_cap: blocks past nv count 0
   uint32_t e = 0, k = 0;
 #pragma unroll 4
   for (int i = 0; i < kStreamItems; ++i) {
     const uint64_t v = base + (uint64_t)i * kStreamThreads + threadIdx.x;
     if (v < nv) {
-      const uint32_t cl = stream_class(stream_toa(a, v), t_lo, t_cut, a.final_push);
+      const uint32_t cl = stream_class(stream_toa(a, n_carry, v), t_lo, t_cut, a.final_push);
       e += cl == 1u;
       k += cl == 2u;
     }
@@ -138,16 +143,17 @@ __global__ void __launch_bounds__(1024) k_stream_scan(StreamArgs a) {
   const uint32_t k = scan_inplace_1024(a.blk_keep, a.nblk);
   if (threadIdx.x == 0) {
     StreamCtrl* c = a.c;
-    const uint64_t nv = a.n + a.n_carry;
+    const uint64_t nv = a.n + c->n_carry_in;
     if (a.nblk == 0) {   // nothing to mark: record the (unchanged) cut here
       uint64_t t_lo, t_cut;
       stream_cut(a, t_lo, t_cut);
     }
     c->label_base = c->label_next;
     c->label_next += e;
-    c->n_work = e;
     c->n_carry = k > a.carry_cap ? a.carry_cap : k;
-    c->overflow = k > a.carry_cap ? 1u : 0u;       // sticky only for this push: the host turns it into an error
+    c->overflow = k > a.carry_cap ? 1u : 0u;
+    if (c->overflow) c->dead = 1u;                  // more events to carry than the buffer holds: the stream is dead
+    c->n_work = c->dead ? 0u : e;                   // (a dead stream clusters nothing; the status word says CAPACITY)
     c->n_late = (uint32_t)(nv - e - k);
     c->late_total += nv - e - k;
     if (!a.final_push) c->s_emitted = c->s_cut;
@@ -158,8 +164,10 @@ __global__ void __launch_bounds__(kStreamThreads, 3) k_stream_scatter(StreamArgs
   __shared__ __align__(16) uint8_t s_cls[kStreamTile];
   __shared__ uint16_t s_rank[kStreamTile];
   __shared__ uint32_t sm[33];
-  const uint64_t t_lo = a.c->t_lo, t_cut = a.c->t_cut, nv = a.n + a.n_carry;
+  const uint32_t n_carry = a.c->n_carry_in;
+  const uint64_t t_lo = a.c->t_lo, t_cut = a.c->t_cut, nv = a.n + n_carry;
   const uint64_t base = (uint64_t)blockIdx.x * kStreamTile;
+  if (base >= nv) return;
   // striped (coalesced) pass: ToA and class of every event
   uint64_t t[kStreamItems];
 #pragma unroll
@@ -169,7 +177,7 @@ __global__ void __launch_bounds__(kStreamThreads, 3) k_stream_scatter(StreamArgs
     uint32_t cl = 0;
     t[i] = 0;
     if (v < nv) {
-      t[i] = stream_toa(a, v);
+      t[i] = stream_toa(a, n_carry, v);
       cl = stream_class(t[i], t_lo, t_cut, a.final_push);
     }
     s_cls[loc] = (uint8_t)cl;
@@ -204,8 +212,8 @@ __global__ void __launch_bounds__(kStreamThreads, 3) k_stream_scatter(StreamArgs
     if (cl == 0u) continue;
     const uint64_t v = base + loc;
     uint16_t ex, ey, et;
-    if (v < a.n_carry) { ex = a.cx[v]; ey = a.cy[v]; et = a.ctot[v]; }
-    else { const uint64_t j = v - a.n_carry; ex = a.x[j]; ey = a.y[j]; et = a.tot[j]; }
+    if (v < n_carry) { ex = a.cx[v]; ey = a.cy[v]; et = a.ctot[v]; }
+    else { const uint64_t j = v - n_carry; ex = a.x[j]; ey = a.y[j]; et = a.tot[j]; }
     const uint32_t r = s_rank[loc];
     if (cl == 1u) {
       const uint32_t o = e_base + r;
@@ -215,15 +223,6 @@ __global__ void __launch_bounds__(kStreamThreads, 3) k_stream_scatter(StreamArgs
       if (o < a.carry_cap) { a.nx[o] = ex; a.ny[o] = ey; a.ntot[o] = et; a.ntoa[o] = t[i]; }
     }
   }
-}
-
-__global__ void __launch_bounds__(256) k_stream_labels(const StreamCtrl* c, const uint32_t* n_hits,
-                                                     uint64_t max_clusters, uint32_t* label) {
-  uint64_t nc = *n_hits;
-  if (nc > max_clusters) nc = max_clusters;
-  const uint32_t base = (uint32_t)c->label_base;
-  for (uint64_t h = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; h < nc; h += (uint64_t)gridDim.x * blockDim.x)
-    label[h] += base;
 }
 
 }  // namespace tpx3

@@ -948,6 +948,9 @@ def _check_push_properties(infos, toa, sizes, D, honest=True):
         seen = shot[:consumed]
         if honest:
             assert info["n_late"] == 0
+            if consumed == n and info["n_carry"] == 0:                # the final push emits what is left
+                assert emitted == n
+                continue
             assert emitted == int(np.count_nonzero(seen < s_now))     # exactly the shots below s_now went out ...
             assert not np.any(shot[consumed:] < s_now)                # ... and they were complete
             if consumed < n or info["n_carry"]:
@@ -1073,6 +1076,48 @@ def test_stream_rejects_bad_arguments(tpx3):
     with pytest.raises(tpx3.Tpx3Error):
         pl0.stream_open(500, 200, 0)              # no shot period: nothing is ever complete
     pl0.free()
+
+
+def test_stream_pushes_without_info_do_not_wait_and_give_the_same_rows(tpx3):
+    """info = NULL: the push only enqueues (the emit count sizes the clustering launch on the device). The rows of
+    all pushes — read back once, at the end, from one table per push — are the batch oracle's; a carry overflow is
+    reported by the status word."""
+    import torch
+
+    w = gen.generate(4, shots=900)
+    D = _disorder(w.toa)
+    chunk, carry = 100003, 8192
+    pl = tpx3.plan(tpx3.Config(toa_window_ticks=W, shot_period_ticks=P, max_hits=chunk + carry, max_shot_hits=1500))
+    s = pl.stream_open(chunk, carry, D)
+    dev = [to_dev(a) for a in (w.x, w.y, w.toa, w.tot)]
+    sizes = _sizes(w.n, chunk)
+    tabs = [tpx3.Clusters(chunk + carry, pl.device) for _ in sizes]
+    counts = [torch.zeros(1, dtype=torch.uint32, device=pl.device) for _ in sizes]
+    i = 0
+    for j, sz in enumerate(sizes):
+        _, info = s.push(*(d[i:i + sz] for d in dev), tabs[j], final=(j == len(sizes) - 1), n_hits=counts[j],
+                         want_info=False)
+        assert info is None
+        i += sz
+    torch.cuda.synchronize()
+    assert pl.status()["error"] == 0
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P, threads=0)
+    rows = {k: np.concatenate([t.numpy(int(c.cpu().numpy()[0]))[k] for t, c in zip(tabs, counts)]) for k in _ROW_KEYS}
+    for k in _ROW_KEYS:
+        np.testing.assert_array_equal(rows[k], o[k], err_msg=k)
+    s.close()
+    # overflow: a carry capacity below one shot
+    s = pl.stream_open(chunk, 64, D)
+    s.push(*(d[:chunk] for d in dev), tabs[0], n_hits=counts[0], want_info=False)
+    torch.cuda.synchronize()
+    assert pl.status()["error"] == tpx3.ERR_CAPACITY
+    s.push(*(d[chunk:2 * chunk] for d in dev), tabs[0], n_hits=counts[0], want_info=False)   # the stream stays dead
+    torch.cuda.synchronize()
+    assert pl.status()["error"] == tpx3.ERR_CAPACITY and int(counts[0].cpu().numpy()[0]) == 0
+    with pytest.raises(tpx3.Tpx3Error):
+        s.push(*(d[:chunk] for d in dev), tabs[0], n_hits=counts[0])       # with info: the call itself reports it
+    s.close()
+    pl.free()
 
 
 def test_stream_takes_nothing_after_the_final_push(tpx3):
