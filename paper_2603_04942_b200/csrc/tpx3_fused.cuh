@@ -308,25 +308,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   uint32_t tile_i = 0;              // status words written so far
   bool seg_failed = false;
   for (;;) {
-  __syncthreads();                  // the previous tile is done with the shared memory
-  if (tid == 0) {
-    misc->lo = kNone;
-    misc->hi = kNone;
-    misc->last = 0;
-    // another tile already gave up: this attempt is lost, do not spend time on it (the next attempt — a
-    // variant with longer shots, or the general kernels — is enqueued behind; k_fallback_dispatch)
-    misc->skip = tile_at == seg_begin ? atomicAdd(&a.ctrl->fused_fail, 0u) : 0u;
-    misc->fail = 0;
-    misc->max_tof = 0;
-    misc->loose = 0;
-    misc->min_tof = kNone;
-    misc->n_klist = 0;
-    misc->max_sl = 0;
-    misc->n_roots = 0;
-    misc->n_list = 0;
-  }
-  __syncthreads();
-  if (misc->skip != 0u || tile_i >= seg_maxt) { seg_failed = tile_i >= seg_maxt; break; }
+  // the next window's ToA is requested BEFORE the barrier that ends the previous tile: the loads touch no shared
+  // memory, so the DRAM round trip runs under the wait for the previous tile's slowest warp
   const uint64_t base = tile_at & ~7ull;               // window start: aligned for the 128-bit loads
   const uint32_t skp = (uint32_t)(tile_at - base);     // window positions below skp belong to the previous tile
   const uint64_t avail = n_ev - base;                  // > 0 by construction
@@ -363,8 +346,28 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   uint64_t t_prev = 0;
   const bool has_prev = lane == 0 && p0 < cnt && base + p0 > 0 && !(at_start && p0 <= skp);
   if (has_prev) t_prev = kGiven ? a.toa[a.perm[base + p0 - 1]] : a.toa[base + p0 - 1];
+  const uint64_t t_first = kGiven ? a.toa[a.perm[tile_at]] : a.toa[tile_at];
+  __syncthreads();                  // the previous tile is done with the shared memory
+  if (tid == 0) {
+    misc->lo = kNone;
+    misc->hi = kNone;
+    misc->last = 0;
+    // another tile already gave up: this attempt is lost, do not spend time on it (the next attempt — a
+    // variant with longer shots, or the general kernels — is enqueued behind; k_fallback_dispatch)
+    misc->skip = tile_at == seg_begin ? atomicAdd(&a.ctrl->fused_fail, 0u) : 0u;
+    misc->fail = 0;
+    misc->max_tof = 0;
+    misc->loose = 0;
+    misc->min_tof = kNone;
+    misc->n_klist = 0;
+    misc->max_sl = 0;
+    misc->n_roots = 0;
+    misc->n_list = 0;
+  }
+  __syncthreads();
+  if (misc->skip != 0u || tile_i >= seg_maxt) { seg_failed = tile_i >= seg_maxt; break; }
   // reference time of the tile: start of the shot its first event belongs to
-  const uint64_t s_base = div64(kGiven ? a.toa[a.perm[tile_at]] : a.toa[tile_at], a.divP);
+  const uint64_t s_base = div64(t_first, a.divP);
   const uint64_t ref = s_base * a.P;
 
   // ---- shot offsets and times of flight; shot boundaries ----------------------------------------
