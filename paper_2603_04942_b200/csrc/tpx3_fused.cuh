@@ -159,6 +159,7 @@ struct FusedArgs {
                        //    maximum of the box (lm_wx, lm_wy, W) and sums over that box (tpx3_localmax.cuh)
   uint32_t lm_wx, lm_wy;
   const uint64_t* label_base;   // [dev] or null: added (low 32 bits) to the label column (stream pushes, R24)
+  uint32_t labels_only;         // mode 5 only: stop after the labels (the general route of tpx3_cluster)
   const uint32_t* n_dev;        // [dev] or null: the event count is device state (a stream push): n, G, nseg, maxt and
                                 // num_tiles above are upper bounds then (they size the grids) and every kernel
                                 // derives the true ones from *n_dev; the staging table is laid out for the bound
@@ -279,7 +280,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   constexpr bool kLM = MODE == 1;            // paper-literal mode (tpx3_localmax_centroid)
   constexpr bool kLabelsOnly = MODE == 2;    // S0-S3 only: perm, label, hit count (tpx3_cluster)
   constexpr bool kGiven = MODE == 3;         // S4-S5 for a given (perm, label) (tpx3_centroid): no sort, no link
-  constexpr bool kCC = MODE == 0 || MODE == 2;   // hits are connected components found here
+  constexpr bool kPerm = MODE == 3 || MODE == 5;   // the events are read through a given perm, which is not written
+  constexpr bool kCC = MODE == 0 || MODE == 2 || MODE == 5;   // hits are connected components found here
   static_assert(IPT == 8, "the 128-bit load phase assumes 8 events per thread");
   constexpr int WARPS = THREADS / 32;
   constexpr uint32_t NB = T;        // hash buckets of 4 slots (16 bytes each)
@@ -319,7 +321,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 
   // ---- load ToA (2 events per 128-bit load) ----------------------------------------------------
   uint64_t toa_r[IPT];
-  if (kGiven) {     // position p of the caller's order is input event perm[p]
+  if (kPerm) {      // position p of the given order is input event perm[p]
     if (p0 + IPT <= cnt) {
       const uint4 i0 = ldg_nc_v4(a.perm + base + p0), i1 = ldg_nc_v4(a.perm + base + p0 + 4);
       const uint32_t ix[IPT] = {i0.x, i0.y, i0.z, i0.w, i1.x, i1.y, i1.z, i1.w};
@@ -345,8 +347,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   // first tile needs it: a later tile starts at a known shot start
   uint64_t t_prev = 0;
   const bool has_prev = lane == 0 && p0 < cnt && base + p0 > 0 && !(at_start && p0 <= skp);
-  if (has_prev) t_prev = kGiven ? a.toa[a.perm[base + p0 - 1]] : a.toa[base + p0 - 1];
-  const uint64_t t_first = kGiven ? a.toa[a.perm[tile_at]] : a.toa[tile_at];
+  if (has_prev) t_prev = kPerm ? a.toa[a.perm[base + p0 - 1]] : a.toa[base + p0 - 1];
+  const uint64_t t_first = kPerm ? a.toa[a.perm[tile_at]] : a.toa[tile_at];
   __syncthreads();                  // the previous tile is done with the shared memory
   if (tid == 0) {
     misc->lo = kNone;
@@ -529,7 +531,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       }
     }
     uint4 vx, vy, vt;
-    if (!kGiven && p0 + IPT <= cnt) {
+    if (!kPerm && p0 + IPT <= cnt) {
       vx = ldg_nc_v4(a.x + base + p0);
       vy = ldg_nc_v4(a.y + base + p0);
       vt = ldg_nc_v4(a.tot + base + p0);
@@ -538,7 +540,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 #pragma unroll
       for (int j = 0; j < IPT; ++j) {
         bool ok = p0 + j < cnt;
-        const uint64_t src = ok ? (kGiven ? (uint64_t)a.perm[base + p0 + j] : base + p0 + j) : 0ull;
+        const uint64_t src = ok ? (kPerm ? (uint64_t)a.perm[base + p0 + j] : base + p0 + j) : 0ull;
         tx[j] = ok ? a.x[src] : (uint16_t)0;
         ty[j] = ok ? a.y[src] : (uint16_t)0;
         tt[j] = ok ? a.tot[src] : (uint16_t)1;
@@ -591,7 +593,9 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     cl_carry = __shfl_up_sync(0xffffffffu, cl_inc, 1);
     if (lane == 0) cl_carry = 0;
   }
-  const bool unsorted = __syncthreads_or(!kGiven && uns ? 1 : 0) != 0;
+  const bool out_of_order = __syncthreads_or(!kGiven && uns ? 1 : 0) != 0;
+  const bool unsorted = !kPerm && out_of_order;    // a given perm is never re-sorted (mode 5: it IS the (shot, ToA) order)
+  if (MODE == 5 && out_of_order) failed = true;
   if (cl_wide && !cl_scan && tid == 0) misc->loose = 1u;   // not checked: treated as not tight
   if (!unsorted && cl_scan) {
     for (uint32_t w = 0; w < warp; ++w) cl_carry = max(cl_carry, misc->warp_sums[w]);
@@ -835,7 +839,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     for (int q = 0; q < 16 * T / 16 / THREADS; ++q) z[q * THREADS + tid] = zero;
     __syncthreads();
   } else {
-    if (!kGiven)
+    if (!kPerm)
       for (uint32_t k = tid; k < mm; k += THREADS) a.perm[out_base + k] = out_base + k;
   }
   const uint2* recS = unsorted ? recA : recB + lo;
@@ -1240,7 +1244,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       const uint32_t l = minidx[root_r[j]];
       lab[k] = (uint16_t)l;
       a.label[out_base + k] = out_base + l;
-      if (!kLabelsOnly) nxt[k] = (uint16_t)atomicExch(&head[l], k);   // every member, the first pixel too; kNone truncates to 0xFFFF = end
+      if (!kLabelsOnly && !(MODE == 5 && a.labels_only)) nxt[k] = (uint16_t)atomicExch(&head[l], k);   // every member, the first pixel too; kNone truncates to 0xFFFF = end
     }
   }
   __syncthreads();
@@ -1342,7 +1346,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       a.stage_c[o] = ref + (uint64_t)(rr.x >> tb) * a.P + (uint64_t)(rr.x & tmask);
       a.stage_d[o] = sf;
     }
-  } else if (!kLabelsOnly)
+  } else if (!kLabelsOnly && !(MODE == 5 && a.labels_only))
   for (uint32_t c = tid; c < n_roots; c += THREADS) {
     const uint32_t r = rootpos[c];
     unsigned long long sx = 0, sy = 0, sf = 0;
@@ -1456,7 +1460,7 @@ __global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, 
     }
     __syncthreads();
     const uint32_t total = s_off[32];
-    for (uint32_t i = tid; a.mode != 2u && i < total; i += kCompactThreads) {
+    for (uint32_t i = tid; a.mode != 2u && !a.labels_only && i < total; i += kCompactThreads) {
       // tile of hit i: the last offset <= i (binary search over 32 offsets)
       uint32_t q = 0;
 #pragma unroll
@@ -1490,9 +1494,11 @@ __global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, 
   if (t1 == a.num_tiles && tid == 0) {
     *a.n_clusters = (uint32_t)prefix;
     a.ctrl->status.n_clusters = (uint32_t)prefix;
-    a.ctrl->status.path = a.mode == 1u ? 3 : 1;
-    a.ctrl->status.sort_passes = 0;
-    if (a.mode == 0u || a.mode == 2u) {   // worth checking the time clusters next time? (fewer than 1 tile in 8 was tight: no)
+    if (a.mode != 5u) {     // mode 5 runs behind the general path's global sort: path 2 and its pass count stand
+      a.ctrl->status.path = a.mode == 1u ? 3 : 1;
+      a.ctrl->status.sort_passes = 0;
+    }
+    if (a.mode == 0u || a.mode == 2u || a.mode == 5u) {   // worth checking the time clusters next time? (fewer than 1 tile in 8 was tight: no)
       a.ctrl->scan_hint = a.ctrl->tight_tiles * 8u < a.ctrl->tiles_run ? kScanSkip : 0u;
       a.ctrl->calls += 1u;
     }
@@ -1536,7 +1542,7 @@ inline int fused_configure_device() {
   TPX3_FUSED_ATTR(2048, 256, 0) TPX3_FUSED_ATTR(2048, 256, 1) TPX3_FUSED_ATTR(2048, 256, 2) TPX3_FUSED_ATTR(2048, 256, 3)
   TPX3_FUSED_ATTR(4096, 512, 0) TPX3_FUSED_ATTR(4096, 512, 1) TPX3_FUSED_ATTR(4096, 512, 2) TPX3_FUSED_ATTR(4096, 512, 3)
   TPX3_FUSED_ATTR(8192, 1024, 0) TPX3_FUSED_ATTR(8192, 1024, 1) TPX3_FUSED_ATTR(8192, 1024, 2)
-  TPX3_FUSED_ATTR(8192, 1024, 3)
+  TPX3_FUSED_ATTR(8192, 1024, 3) TPX3_FUSED_ATTR(8192, 1024, 5)
 #undef TPX3_FUSED_ATTR
   return TPX3_OK;
 }
@@ -1590,6 +1596,7 @@ inline FusedArgs make_fused_args(uint32_t T, uint32_t num_sms, Ctrl* ctrl, unsig
   a.stage_d = a.stage_c + prm.n;
   a.mode = mode; a.lm_wx = lm_wx; a.lm_wy = lm_wy;
   a.label_base = nullptr;
+  a.labels_only = 0;
   a.n_dev = n_dev;      // then prm.n is the largest count: it sizes the grids and lays out the staging table
   return a;
 }
@@ -1624,7 +1631,8 @@ __device__ inline void launch_fused_rung_device(FusedArgs a, uint32_t T) {
     if (a.mode == 0u) TPX3_RUNG(8192, 1024, 0);
     else if (a.mode == 1u) TPX3_RUNG(8192, 1024, 1);
     else if (a.mode == 2u) TPX3_RUNG(8192, 1024, 2);
-    else TPX3_RUNG(8192, 1024, 3);
+    else if (a.mode == 3u) TPX3_RUNG(8192, 1024, 3);
+    else TPX3_RUNG(8192, 1024, 5);
   }
 #undef TPX3_RUNG
   k_fused_compact<<<ctas, kCompactThreads, 0, cudaStreamTailLaunch>>>(a, tpc, T);

@@ -135,6 +135,7 @@ struct GenArgs {
   uint32_t lm_wx, lm_wy;   // paper-literal mode: box half-widths
   uint64_t lm_wt;
   const uint64_t* label_base;   // [dev] or null (stream pushes): added to the label column
+  int sorted_tiles;             // the plan has a tile kernel: after the global sort, link through it first (mode 5)
 };
 
 // The fields that depend on the event count (a stream push learns it on the device).
@@ -235,6 +236,9 @@ __host__ __device__ inline uint32_t grid_for_hd(uint64_t n, int threads, int num
 // hint: the same tile kernel with room for longer shots, then this dispatcher again) or, after the last rung,
 // the whole general path. A successful fused call thus pays for one empty launch instead of the 36 early-exit
 // launches of the general path. lm != 0: the paper-literal mode.
+__global__ void k_general_sorted_tiles(GenArgs a, FusedArgs fa, int what);
+__global__ void k_general_slab(GenArgs a, int what);
+
 __global__ void k_fallback_dispatch(GenArgs a, FusedArgs fa, FusedLadder ladder, int rung, int what) {
   Ctrl* c = a.w.ctrl;
   if (c->fused_state == 1u) return;
@@ -255,11 +259,40 @@ __global__ void k_fallback_dispatch(GenArgs a, FusedArgs fa, FusedLadder ladder,
 #define GP(stage, kernel, grid, block, ...) kernel<<<(grid), (block), 0, cudaStreamTailLaunch>>>(__VA_ARGS__)
   if (what == 1) {
     TPX3_LOCALMAX_SEQUENCE(a);
+  } else if (what != 3 && a.sorted_tiles) {
+    // general route, first choice: the global sort, then the tile kernel on the sorted stream (read through perm)
+    TPX3_GENERAL_SORT_SEQUENCE(a);
+    k_general_sorted_tiles<<<1, 1, 0, cudaStreamTailLaunch>>>(a, fa, what);
   } else {
     if (what != 3) TPX3_GENERAL_CLUSTER_SEQUENCE(a);
     if (what != 2) TPX3_GENERAL_CENTROID_SEQUENCE(a);
   }
 #undef GP
+}
+
+// General route, last resort (one shot longer than a tile, P = 0 plans never get here): global sort again (the
+// tile attempt's staging table aliases the sort buffers), slab-hash linking, atomic sums.
+__global__ void k_general_slab(GenArgs a, int what) {
+  Ctrl* c = a.w.ctrl;
+  if (c->fused_state == 1u) return;
+#define GP(stage, kernel, grid, block, ...) kernel<<<(grid), (block), 0, cudaStreamTailLaunch>>>(__VA_ARGS__)
+  TPX3_GENERAL_CLUSTER_SEQUENCE(a);
+  if (what != 2) TPX3_GENERAL_CENTROID_SEQUENCE(a);
+#undef GP
+}
+
+// General route behind the global sort: perm now IS the (shot, ToA) order of ANY input (shots interleaved in the
+// stream, a globally shuffled file), so the tile kernel can finish the call reading the events through perm
+// (mode 5, 8192-event windows). Only a shot that does not fit a window sends the call on to k_general_slab.
+__global__ void k_general_sorted_tiles(GenArgs a, FusedArgs fa, int what) {
+  Ctrl* c = a.w.ctrl;
+  c->tiles_done = 0; c->fused_fail = 0; c->fused_state = 0; c->tight_tiles = 0; c->tiles_run = 0;
+  fa.mode = 5u;
+  fa.labels_only = what == 2 ? 1u : 0u;
+  const FusedSegs sg = fused_segs(fa.n, 8192u, fa.num_sms);
+  fa.G = sg.G; fa.nseg = sg.nseg; fa.maxt = sg.maxt; fa.num_tiles = sg.nseg * sg.maxt;
+  launch_fused_rung_device(fa, 8192u);
+  k_general_slab<<<1, 1, 0, cudaStreamTailLaunch>>>(a, what);
 }
 
 GenArgs make_gen_args(tpx3_plan_s* p, const Ws& w, int general_only, uint64_t n, const uint16_t* x, const uint16_t* y,
@@ -314,6 +347,13 @@ int enqueue_general_cluster(tpx3_plan_s* p, const GenArgs& a, cudaStream_t st) {
     ++p->launches;                                                 \
   } while (0)
   TPX3_GENERAL_CLUSTER_SEQUENCE(a);
+  hl.leave();
+  return cuda_ok(cudaGetLastError());
+}
+
+int enqueue_general_sort(tpx3_plan_s* p, const GenArgs& a, cudaStream_t st) {
+  HostLauncher hl{p, st, -1, false, 0};
+  TPX3_GENERAL_SORT_SEQUENCE(a);
   hl.leave();
   return cuda_ok(cudaGetLastError());
 }
@@ -438,6 +478,9 @@ static int run_fused_or_general(tpx3_plan_t p, void* workspace, void* cuda_strea
   memset(&none, 0, sizeof(none));
   GenArgs ga = make_gen_args(p, w, mode == 2u ? 0 : 1, n, x, y, toa, tot, perm, label, max_clusters, out, n_clusters);
   ga.label_base = label_base;
+  // the general route links through the tile kernel too, behind its global sort (mode 5), when the plan has one
+  ga.sorted_tiles = p->fused.variant != 0 && mode != 3u &&
+                    (((uintptr_t)x | (uintptr_t)y | (uintptr_t)toa | (uintptr_t)tot | (uintptr_t)perm) & 15u) == 0;
   if (sc && !try_fused) {   // general kernels only: launched from the device, which knows the count
     FusedArgs fa = make_fused_args(2048u, (uint32_t)p->num_sms, w.ctrl, w.tiles, prm, x, y, toa, tot, perm, label,
                                    max_clusters, out ? *out : none, n_clusters, (char*)workspace + p->off_keyA, mode, 0u,
@@ -460,6 +503,27 @@ static int run_fused_or_general(tpx3_plan_t p, void* workspace, void* cuda_strea
       ++p->launches;
       return cuda_ok(cudaGetLastError());
     }
+  }
+  if (ga.sorted_tiles) {
+    // global sort, then the tile kernel on the sorted stream (read through perm); the slab-hash kernels only if a
+    // shot does not fit a window (decided on the device: k_general_slab)
+    rc = enqueue_general_sort(p, ga, st);
+    if (rc != TPX3_OK) return rc;
+    {
+      StageTimer timer(p, st, TPX3_STAGE_FUSED);
+      FusedArgs fa = make_fused_args(8192u, (uint32_t)p->num_sms, w.ctrl, w.tiles, prm, x, y, toa, tot, perm, label,
+                                     max_clusters, out ? *out : none, n_clusters, (char*)workspace + p->off_keyA, 5u, 0u,
+                                     0u, nullptr);
+      fa.label_base = label_base;
+      fa.labels_only = mode == 2u ? 1u : 0u;
+      k_fused_shot_tiles<8192, 1024, 5><<<fa.nseg, 1024, FusedSmem<8192>::kBytes, st>>>(fa);
+      uint32_t ctas, tpc;
+      compact_grid(fa.num_tiles, (uint32_t)p->num_sms, &ctas, &tpc);
+      k_fused_compact<<<ctas, kCompactThreads, 0, st>>>(fa, tpc, 8192u);
+      k_general_slab<<<1, 1, 0, st>>>(ga, (int)mode);
+      p->launches += 3;
+    }
+    return cuda_ok(cudaGetLastError());
   }
   if (mode != 3u) {
     rc = enqueue_general_cluster(p, ga, st);
