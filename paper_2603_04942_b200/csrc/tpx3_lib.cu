@@ -172,7 +172,7 @@ __host__ __device__ inline uint32_t grid_for_hd(uint64_t n, int threads, int num
     /* passes needed for the largest span a ToA can have; the ones past the device-computed npass return at once */  \
     for (int pass_ = 0; pass_ < kMaxPasses; ++pass_) {                                                                \
       GP(TPX3_STAGE_SORT, k_radix_hist, (A).g.nblk, kSortThreads, (A).w.ctrl, pass_, (A).toa, b_, n_, (A).g);         \
-      GP(TPX3_STAGE_SORT, k_radix_scan, 1, 1024, (A).w.ctrl, pass_, (A).w.counts, (uint32_t)(kRadix * (A).g.nblk));   \
+      GP(TPX3_STAGE_SORT, k_radix_scan, kRadix / 8, 256, (A).w.ctrl, pass_, (A).w.counts, (A).g.nblk);                 \
       GP(TPX3_STAGE_SORT, k_radix_scatter, (A).g.nblk, kSortThreads, (A).w.ctrl, pass_, (A).toa, b_, (A).perm, n_,    \
          (A).g);                                                                                                      \
     }                                                                                                                 \
@@ -438,7 +438,7 @@ int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace
   p->off_tot = o; o = align_up(o + 2 * N);
   p->off_slab = o; o = align_up(o + 8 * N);
   p->off_table = o; o = align_up(o + 4 * (size_t)table_size_for(N));
-  p->off_counts = o; o = align_up(o + 4 * (size_t)kRadix * kSortMaxBlocks);
+  p->off_counts = o; o = align_up(o + 4 * (size_t)kRadix * (kSortMaxBlocks + 1));   // + the digit totals
   // the fused path's staging table (48 bytes per event) aliases keyA .. table
   if (o - p->off_keyA < 48 * (size_t)N) o = align_up(p->off_keyA + 48 * (size_t)N);
   // centroid buffers alias the sort buffers (the two steps never run concurrently and the

@@ -109,10 +109,29 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_hist(Ctrl* c, int pass, 
   b.counts[(size_t)threadIdx.x * g.nblk + blockIdx.x] = hist[threadIdx.x];
 }
 
-// Exclusive scan of counts[kRadix * nblk] in place (single block of 1024 threads).
-__global__ void __launch_bounds__(1024) k_radix_scan(Ctrl* c, int pass, uint32_t* counts, uint32_t total) {
+// Exclusive scan of counts[kRadix][nblk] in place, digit by digit: one warp per digit value (32 blocks of 8 warps)
+// scans that digit's nblk block counts and leaves the digit's total in counts[kRadix * nblk + d]; the scatter
+// kernel adds the exclusive prefix over the 256 totals itself. (One block scanning all 303 K counters took
+// 0.33 ms per pass on cfg1, as much as the histogram and half of the scatter.)
+__global__ void __launch_bounds__(256) k_radix_scan(Ctrl* c, int pass, uint32_t* counts, uint32_t nblk) {
   if (c->fused_state == 1 || (uint32_t)pass >= c->npass) return;
-  scan_inplace_1024(counts, total);
+  const uint32_t lane = threadIdx.x & 31u, d = blockIdx.x * 8u + (threadIdx.x >> 5);
+  if (d >= (uint32_t)kRadix) return;
+  uint32_t* row = counts + (size_t)d * nblk;
+  uint32_t run = 0;
+  for (uint32_t b0 = 0; b0 < nblk; b0 += 32u) {
+    const uint32_t b = b0 + lane;
+    const uint32_t v = b < nblk ? row[b] : 0u;
+    uint32_t inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= (uint32_t)o) inc += t;
+    }
+    if (b < nblk) row[b] = run + inc - v;
+    run += __shfl_sync(0xffffffffu, inc, 31);
+  }
+  if (lane == 0) counts[(size_t)kRadix * nblk + d] = run;
 }
 
 __global__ void __launch_bounds__(kSortThreads) k_radix_scatter(Ctrl* c, int pass, const uint64_t* __restrict__ toa,
@@ -127,7 +146,21 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_scatter(Ctrl* c, int pas
   uint32_t* __restrict__ didx = last ? perm : b.idx[pass & 1];
   const uint32_t* __restrict__ sidx = pass == 0 ? nullptr : b.idx[(pass - 1) & 1];
   const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5, lt = lanemask_lt();
-  running[threadIdx.x] = b.counts[(size_t)threadIdx.x * g.nblk + blockIdx.x];
+  {   // exclusive prefix over the 256 digit totals (thread d = digit d), plus this block's offset inside the digit
+    const uint32_t tot_d = b.counts[(size_t)kRadix * g.nblk + threadIdx.x];
+    uint32_t inc = tot_d;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= (uint32_t)o) inc += t;
+    }
+    __shared__ uint32_t wtot[kSortWarps];
+    if (lane == 31) wtot[w] = inc;
+    __syncthreads();
+    uint32_t base = inc - tot_d;
+    for (uint32_t ww = 0; ww < w; ++ww) base += wtot[ww];
+    running[threadIdx.x] = base + b.counts[(size_t)threadIdx.x * g.nblk + blockIdx.x];
+  }
   uint64_t t0 = (uint64_t)blockIdx.x * g.tiles_per_blk * kSortTile;
   for (uint32_t t = 0; t < g.tiles_per_blk; ++t, t0 += kSortTile) {
     if (t0 >= n) break;
@@ -142,7 +175,15 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_scatter(Ctrl* c, int pas
       bool valid = pos < n;
       key[i] = valid ? sort_load_key(pass, c, toa, b, pos) : 0;
       uint32_t d = valid ? ((uint32_t)(key[i] >> shift) & (kRadix - 1)) : (uint32_t)kRadix;
-      uint32_t peers = __match_any_sync(0xffffffffu, d);
+      // lanes holding the same digit: one ballot per digit bit (match.any is far dearer on sm_100)
+      uint32_t peers = __ballot_sync(0xffffffffu, valid);
+      if (!valid) peers = ~peers;
+#pragma unroll
+      for (int bit = 0; bit < kRadixBits; ++bit) {
+        const bool one = (d >> bit) & 1u;
+        const uint32_t bal = __ballot_sync(0xffffffffu, one);
+        peers &= one ? bal : ~bal;
+      }
       uint32_t lr = __popc(peers & lt);
       uint32_t base = valid ? warp_cnt[w][d] : 0;
       __syncwarp();
