@@ -222,8 +222,36 @@ struct FusedSmem {
   static constexpr int kListCap = 3 * T / 8;           // deferred links the list holds
   static constexpr int kMisc = kList + 4 * kListCap;   // 27.5 T
   static constexpr int kMiscBytes = 512;
+#ifdef TPX3_BULK_TOA   // experiment: the next window's ToA by cp.async.bulk + mbarrier into 8T more bytes
+  static constexpr int kBulk = kMisc + kMiscBytes;
+  static constexpr int kBytes = kBulk + (T <= 4096 ? 8 * T + 16 : 0);   // 8192-event windows: no room
+#else
   static constexpr int kBytes = kMisc + kMiscBytes;
+#endif
 };
+
+#ifdef TPX3_BULK_TOA
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(void* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, void* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity) {
+  asm volatile(
+      "{\n.reg .pred p;\nWAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+#endif
 
 struct FusedMisc {
   unsigned int lo, hi;         // first shot start of the window; first one at or after the segment's end
@@ -309,6 +337,25 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   bool at_start = seg == 0;         // tile_at is known to be a shot start
   uint32_t tile_i = 0;              // status words written so far
   bool seg_failed = false;
+#ifdef TPX3_BULK_TOA
+  uint64_t* toa_s = reinterpret_cast<uint64_t*>(smem + L::kBulk);
+  void* bulk_bar = smem + L::kBulk + 8 * T;
+  uint32_t bulk_phase = 0;
+  bool bulk_have = false;            // the window at tile_at has been requested into toa_s (block-uniform)
+  constexpr bool kBulkOn = !kPerm && T <= 4096;
+  if (kBulkOn) {
+    if (tid == 0) {
+      mbar_init(bulk_bar, 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    bulk_have = n_ev - (tile_at & ~7ull) >= (uint64_t)T;
+    if (bulk_have && tid == 0) {
+      mbar_expect_tx(bulk_bar, 8u * T);
+      bulk_g2s(toa_s, a.toa + (tile_at & ~7ull), 8u * T, bulk_bar);
+    }
+  }
+#endif
   for (;;) {
   // the next window's ToA is requested BEFORE the barrier that ends the previous tile: the loads touch no shared
   // memory, so the DRAM round trip runs under the wait for the previous tile's slowest warp
@@ -331,6 +378,18 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 #pragma unroll
       for (int j = 0; j < IPT; ++j) toa_r[j] = (p0 + j < cnt) ? a.toa[a.perm[base + p0 + j]] : 0ull;
     }
+#ifdef TPX3_BULK_TOA
+  } else if (bulk_have) {
+    mbar_wait(bulk_bar, bulk_phase);
+    bulk_phase ^= 1u;
+    const uint4* src = reinterpret_cast<const uint4*>(toa_s + p0);
+#pragma unroll
+    for (int j = 0; j < IPT / 2; ++j) {
+      uint4 v = src[j];
+      toa_r[2 * j] = ((uint64_t)v.y << 32) | v.x;
+      toa_r[2 * j + 1] = ((uint64_t)v.w << 32) | v.z;
+    }
+#endif
   } else if (p0 + IPT <= cnt) {
     const uint4* src = reinterpret_cast<const uint4*>(a.toa + base + p0);
 #pragma unroll
@@ -486,6 +545,16 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     }
     if (to_end && next_at >= base + cnt) next_at = n_ev;
   }
+#ifdef TPX3_BULK_TOA
+  if (kBulkOn) {  // every thread has its ToA in registers (two barriers ago): the buffer may take the next window
+    bulk_have = !failed && next_at < seg_end && n_ev - (next_at & ~7ull) >= (uint64_t)T;
+    if (bulk_have && tid == 0) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_expect_tx(bulk_bar, 8u * T);
+      bulk_g2s(toa_s, a.toa + (next_at & ~7ull), 8u * T, bulk_bar);
+    }
+  }
+#endif
   // key layout: 2^tb > max tof + W, so keys of different shots differ by more than W
   const uint32_t tspan = misc->max_tof + a.W;
   const uint32_t tb = tspan ? 32u - (uint32_t)__clz(tspan) : 0u;
