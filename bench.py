@@ -571,8 +571,10 @@ def run_aux(args):
     m.load_library()
     w = make_workload(args.workload, args.shots, 0)
     n, P = w.n, w.shot_period_ticks
-    pl = m.plan(m.Config(max_hits=max(n, 1), toa_window_ticks=w.toa_window_ticks, shot_period_ticks=P))
+    pl = m.plan(m.Config(max_hits=max(n, 1), toa_window_ticks=w.toa_window_ticks, shot_period_ticks=P,
+                         max_shot_hits=__import__("gen").max_shot_hits(w.cfg_id)))
     stream = torch.cuda.Stream(device=0)
+    two_calls = None
     if args.mode == "unwrap":
         # the workload's ToA folded into a counter of 2^34 ticks (several wraps over the run)
         modulus, jump = 1 << 34, 1 << 33
@@ -606,6 +608,43 @@ def run_aux(args):
         kept = int(res["out"][5].cpu().numpy()[0])
         bytes_step = 14 * n + 18 * kept + 4 * kept
         what = {"call": "tpx3_preprocess", "triggers": nshot, "cut_ticks": cut, "kept": kept, "dropped": n - kept}
+        if args.mode == "prefused":
+            # SURVEY 8f NEXT #3 as worded: the preprocessing inside the clustering call, against the two calls back to back
+            cl = m.Clusters(max(n // 2, 1024), pl.device)
+            perm = torch.empty(max(n, 1), dtype=torch.uint32, device=pl.device)
+            label = torch.empty(max(n, 1), dtype=torch.uint32, device=pl.device)
+            nc = torch.zeros(1, dtype=torch.uint32, device=pl.device)
+            nk = torch.zeros(1, dtype=torch.uint32, device=pl.device)
+
+            def two():
+                xo, yo, to, oo, io, no = pl.preprocess(*dev, dtrig, cut, dtab, shot_base=s0, stream=stream)
+                pl.cluster_centroid(xo[:kept], yo[:kept], to[:kept], oo[:kept], cl, perm=perm, label=label, n_clusters=nc,
+                                    stream=stream)
+
+            def step():
+                pl.preprocess_cluster_centroid(*dev, dtrig, cut, dtab, s0, cl, perm=perm, label=label, n_clusters=nc,
+                                               n_kept=nk, stream=stream)
+
+            for _ in range(max(args.warmup, 1)):
+                two()
+            torch.cuda.synchronize()
+            ncl_two = int(nc.cpu().numpy()[0])
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(args.steps):
+                two()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            two_calls = e0.elapsed_time(e1) / max(args.steps, 1)
+            step()
+            torch.cuda.synchronize()
+            st = pl.status(stream)
+            if st["error"] or int(nc.cpu().numpy()[0]) != ncl_two or int(nk.cpu().numpy()[0]) != kept:
+                raise RuntimeError("fused preprocessing call disagrees with the two calls: %r" % (st,))
+            ncl = ncl_two
+            bytes_step = 8 * n + 14 * n + 8 * kept + 64 * ncl     # pre-pass ToA + the tile kernel's single touch
+            what = {"call": "tpx3_preprocess_cluster_centroid", "triggers": nshot, "cut_ticks": cut, "kept": kept,
+                    "dropped": n - kept, "particle_hits": ncl}
     for _ in range(max(args.warmup, 1)):
         step()
     torch.cuda.synchronize()
@@ -625,11 +664,13 @@ def run_aux(args):
     sampler.stop()
     peak, peak_src = measured_peak()
     what.update({"workload": w.name, "mode": args.mode, "pixel_hits_per_gpu": n})
+    if two_calls is not None:
+        what.update({"two_calls_ms_per_step": two_calls, "speedup_over_two_calls": two_calls / ms_step})
     line = {
         "metric": METRIC, "value": n / (ms_step * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "int64", "data": "synthetic", "config": what, "gpu_launches": launches,
-        "roofline": {"bound": "hbm", "kernel": what["call"] + " (3 kernels)", "achieved": bytes_step / (ms_step * 1e-3) / 1e9,
+        "roofline": {"bound": "hbm", "kernel": what["call"] + (" (3 kernels)" if two_calls is None else " (pre-pass + tile kernel)"), "achieved": bytes_step / (ms_step * 1e-3) / 1e9,
                      "peak": peak, "unit": "GB/s", "frac": bytes_step / (ms_step * 1e-3) / 1e9 / peak, "traffic": None,
                      "peak_source": peak_src, "algorithmic_bytes_per_step": bytes_step},
         "clocks": sampler.summary(t_wall0, time.time()),
@@ -652,7 +693,7 @@ def main():
                     help="tile-size hint for the plan (default: the workload recipe's bound on hits per shot)")
     ap.add_argument("--chunk", type=int, default=1 << 22, help="--mode stream: events per push")
     ap.add_argument("--max-carry", type=int, default=1 << 20, help="--mode stream: carry capacity in events")
-    ap.add_argument("--mode", choices=("components", "split", "localmax", "stream", "unwrap", "preprocess"), default="components",
+    ap.add_argument("--mode", choices=("components", "split", "localmax", "stream", "unwrap", "preprocess", "prefused"), default="components",
                     help="components: the hot path (default). localmax: the paper-literal mode, SURVEY 8f NEXT #2")
     ap.add_argument("--window", type=int, nargs=3, default=(2, 2, 320), metavar=("WX", "WY", "WT"),
                     help="box half-widths of --mode localmax (pixels, pixels, ticks)")
@@ -665,7 +706,7 @@ def main():
         print("note: timing rules ask for >= 3 warm-up steps", file=sys.stderr)
     if args.impl == "reference":
         return run_reference(args)
-    if args.mode in ("unwrap", "preprocess"):
+    if args.mode in ("unwrap", "preprocess", "prefused"):
         return run_aux(args)
     return run_stream(args) if args.mode == "stream" else run_ours(args)
 

@@ -48,7 +48,10 @@ typedef enum {
   TPX3_ERR_INVALID_ARG = -1,   /* null pointer, bad struct_size, n > max_hits, bad config      */
   TPX3_ERR_CAPACITY = -2,      /* max_clusters too small (device-detected; see tpx3_status)     */
   TPX3_ERR_OUT_OF_RANGE = -3,  /* x/y outside the sensor or tot == 0 (under VALIDATE_INPUT)     */
-  TPX3_ERR_CUDA = -4           /* a CUDA runtime call failed                                    */
+  TPX3_ERR_CUDA = -4,          /* a CUDA runtime call failed                                    */
+  TPX3_ERR_NOT_CONTIGUOUS = -5 /* tpx3_preprocess_cluster_centroid only (device-detected): the stream
+                                  is not shot-contiguous or a shot does not fit the plan's window;
+                                  use tpx3_preprocess followed by tpx3_cluster_centroid            */
 } tpx3_error_t;
 
 enum {
@@ -181,6 +184,26 @@ int tpx3_preprocess(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64
                     const uint64_t* trig, uint64_t cut, const int32_t* table, uint32_t table_len,
                     uint64_t shot_base, uint16_t* x_out, uint16_t* y_out, uint64_t* toa_out,
                     uint16_t* tot_out, uint32_t* index_out, uint32_t* n_out);
+
+/* Preprocessing FUSED into the clustering call (SURVEY.md 8f NEXT #3 as worded: "fused into the key-build
+ * pass"): same arguments and per-event rules as tpx3_preprocess (trigger assignment, ToF cut, timewalk table,
+ * rebase), same hits as tpx3_preprocess followed by tpx3_cluster_centroid on its output, but the
+ * intermediate stream is never written: a pre-pass counts the surviving events per segment (reads ToA and the
+ * trigger list), and the tile kernel applies the preprocessing in its load phase, before it builds its keys.
+ * Outputs [dev]: n_kept uint32[1] = events that survive; perm uint32[n] (first n_kept entries written): perm[k]
+ * = INPUT position (into x, y, toa, tot) of the surviving event at sorted position k (the two-call route gives
+ * index_out[perm[k]]); label uint32[n] (first n_kept entries), indexed by sorted position among the surviving
+ * events; `out` / n_clusters as tpx3_cluster_centroid, with toa_peak and shot in the REBASED time
+ * ((shot_base + s) * P + ToF'). Serves shot-contiguous raw streams (the trigger index never decreases along the
+ * stream) whose shots fit the plan's window (max_shot_hits, counted on the raw stream, must be given); anything
+ * else is detected on the device and reported as TPX3_ERR_NOT_CONTIGUOUS by tpx3_status — nothing valid has been
+ * written then. The plan's shot period must be > 0 and <= 2^24. Enqueue only. */
+int tpx3_preprocess_cluster_centroid(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64_t n,
+                                     const uint16_t* x, const uint16_t* y, const uint64_t* toa,
+                                     const uint16_t* tot, uint64_t n_trig, const uint64_t* trig, uint64_t cut,
+                                     const int32_t* table, uint32_t table_len, uint64_t shot_base,
+                                     uint32_t* perm, uint32_t* label, uint64_t max_clusters,
+                                     const tpx3_clusters_t* out, uint32_t* n_clusters, uint32_t* n_kept);
 
 /* End-to-end variant with HOST buffers: copies x, y, toa, tot [host] to the device, runs
  * tpx3_cluster_centroid and copies perm, label (either may be NULL to skip), the first

@@ -23,12 +23,12 @@ __all__ = [
 FLAG_VALIDATE_INPUT = 1 << 0
 FLAG_FORCE_GENERAL = 1 << 1
 
-OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_OUT_OF_RANGE, ERR_CUDA = 0, -1, -2, -3, -4
+OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_OUT_OF_RANGE, ERR_CUDA, ERR_NOT_CONTIGUOUS = 0, -1, -2, -3, -4, -5
 
 # Every symbol include/tpx3.h declares (tests check the built library exports all of them).
 exported_symbols = (
     "tpx3_plan", "tpx3_cluster", "tpx3_centroid", "tpx3_cluster_centroid", "tpx3_localmax_centroid",
-    "tpx3_unwrap_toa", "tpx3_timewalk_table", "tpx3_preprocess", "tpx3_host_io_bytes",
+    "tpx3_unwrap_toa", "tpx3_timewalk_table", "tpx3_preprocess", "tpx3_preprocess_cluster_centroid", "tpx3_host_io_bytes",
     "tpx3_stream_bytes", "tpx3_stream_open", "tpx3_stream_push", "tpx3_stream_close",
     "tpx3_process_host", "tpx3_host_route", "tpx3_status", "tpx3_launch_count", "tpx3_profile_enable", "tpx3_profile_read",
     "tpx3_free", "tpx3_strerror",
@@ -98,6 +98,9 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.tpx3_unwrap_toa.argtypes = [vp, vp, vp, u64, vp, u64, u64, ctypes.c_int64, ctypes.c_int, u64, vp, vp]
     lib.tpx3_timewalk_table.restype = ctypes.c_int
     lib.tpx3_timewalk_table.argtypes = [ctypes.c_double] * 4 + [ctypes.c_uint32, vp]
+    lib.tpx3_preprocess_cluster_centroid.restype = ctypes.c_int
+    lib.tpx3_preprocess_cluster_centroid.argtypes = [vp, vp, vp, u64, vp, vp, vp, vp, u64, vp, u64, vp, ctypes.c_uint32,
+                                                     u64, vp, vp, u64, ctypes.POINTER(_CClusters), u32p, u32p]
     lib.tpx3_preprocess.restype = ctypes.c_int
     lib.tpx3_preprocess.argtypes = [vp, vp, vp, u64, vp, vp, vp, vp, u64, vp, u64, vp, ctypes.c_uint32, u64,
                                     vp, vp, vp, vp, vp, vp]
@@ -277,6 +280,35 @@ class Plan:
         if rc != OK:
             raise Tpx3Error(rc, "tpx3_preprocess")
         return xo, yo, to, oo, io, n_out
+
+    # -- preprocessing fused into the clustering call (tpx3.h) ---------------------------------------
+    def preprocess_cluster_centroid(self, x, y, toa, tot, trig, cut: int, table, shot_base: int, clusters: "Clusters",
+                                    perm=None, label=None, n_clusters=None, n_kept=None, stream=None):
+        """Returns (perm, label, n_clusters, n_kept): perm[k] = input position of the surviving event at sorted
+        position k; label over the surviving events. A stream the tile kernel cannot take shows as
+        ERR_NOT_CONTIGUOUS in status()."""
+        import torch
+
+        n = int(x.numel())
+        self._check_inputs(x, y, toa, tot, n)
+        _check_dev(trig, torch.uint64, 0, "trig")
+        if table is not None:
+            _check_dev(table, torch.int32, 0, "table")
+        mk = lambda k: torch.empty(k, dtype=torch.uint32, device=self.device)  # noqa: E731
+        perm = mk(max(n, 1)) if perm is None else perm
+        label = mk(max(n, 1)) if label is None else label
+        n_clusters = mk(1) if n_clusters is None else n_clusters
+        n_kept = mk(1) if n_kept is None else n_kept
+        c = clusters._c()
+        rc = self.lib.tpx3_preprocess_cluster_centroid(
+            self.handle, self.workspace.data_ptr(), _stream_ptr(stream, self.device), n, x.data_ptr(), y.data_ptr(),
+            toa.data_ptr(), tot.data_ptr(), int(trig.numel()), trig.data_ptr(), int(cut),
+            0 if table is None else table.data_ptr(), 0 if table is None else int(table.numel()), int(shot_base),
+            perm.data_ptr(), label.data_ptr(), clusters.max_clusters, ctypes.byref(c), n_clusters.data_ptr(),
+            n_kept.data_ptr())
+        if rc != OK:
+            raise Tpx3Error(rc, "tpx3_preprocess_cluster_centroid")
+        return perm, label, n_clusters, n_kept
 
     # -- ToA counter unwrapping (PAPER.md IV.A) ----------------------------------------------------
     def unwrap_toa(self, raw, modulus: int, jump: int, wraps_in: int = 0, prev_raw=None, out=None, wraps_out=None,

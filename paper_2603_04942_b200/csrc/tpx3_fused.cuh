@@ -53,6 +53,7 @@
 #pragma once
 #include "tpx3_common.cuh"
 #include "tpx3_localmax.cuh"
+#include "tpx3_preprocess.cuh"
 
 namespace tpx3 {
 
@@ -159,6 +160,8 @@ struct FusedArgs {
                        //    maximum of the box (lm_wx, lm_wy, W) and sums over that box (tpx3_localmax.cuh)
   uint32_t lm_wx, lm_wy;
   const uint64_t* label_base;   // [dev] or null: added (low 32 bits) to the label column (stream pushes, R24)
+  PreArgs pre;                  // mode 4 only: trigger list, cut, timewalk table (tpx3_preprocess.cuh)
+  const uint32_t* seg_kept;     // mode 4 only: events that survive the preprocessing in front of every segment
   uint32_t labels_only;         // mode 5 only: stop after the labels (the general route of tpx3_cluster)
   const uint32_t* n_dev;        // [dev] or null: the event count is device state (a stream push): n, G, nseg, maxt and
                                 // num_tiles above are upper bounds then (they size the grids) and every kernel
@@ -263,8 +266,11 @@ struct FusedMisc {
   unsigned int skip;           // the call already failed in another tile
   unsigned int loose;          // some time cluster of the tile is wider than W ("within W" is not transitive)
   unsigned int min_tof;        // smallest time of flight among the events the tile loaded
+  unsigned int s_next;               // mode 4: shot offset of the event the next tile starts at
+  unsigned int kept_own, kept_pre;   // mode 4: events of the owned range / in front of it that survive the preprocessing
   unsigned int n_klist;        // other tiles: events whose S cell is empty (second pass of the link step)
   unsigned int warp_sums[33];
+  unsigned int warp_cnt[33], warp_max[33];   // mode 4: surviving events / largest surviving key per warp (compaction)
 };
 static_assert(sizeof(FusedMisc) <= 512, "FusedMisc must fit kMiscBytes");
 
@@ -309,7 +315,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   constexpr bool kLabelsOnly = MODE == 2;    // S0-S3 only: perm, label, hit count (tpx3_cluster)
   constexpr bool kGiven = MODE == 3;         // S4-S5 for a given (perm, label) (tpx3_centroid): no sort, no link
   constexpr bool kPerm = MODE == 3 || MODE == 5;   // the events are read through a given perm, which is not written
-  constexpr bool kCC = MODE == 0 || MODE == 2 || MODE == 5;   // hits are connected components found here
+  constexpr bool kPre = MODE == 4;           // S0-S5 on a RAW stream: trigger assignment, ToF cut, timewalk, rebase in the load phase
+  constexpr bool kCC = MODE == 0 || MODE == 2 || MODE == 4 || MODE == 5;   // hits are connected components found here
   static_assert(IPT == 8, "the 128-bit load phase assumes 8 events per thread");
   constexpr int WARPS = THREADS / 32;
   constexpr uint32_t NB = T;        // hash buckets of 4 slots (16 bytes each)
@@ -334,6 +341,9 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   const uint64_t seg_end = seg_begin + seg_G < n_ev ? seg_begin + seg_G : n_ev;
   const uint32_t P32 = (uint32_t)a.P;
   uint64_t tile_at = seg_begin;     // where the next tile starts; a shot start except for the segment's first tile
+  uint32_t kept_run = kPre ? a.seg_kept[seg] : 0u;   // mode 4: surviving events in front of tile_at
+  uint64_t pre_next_s = 0;          // mode 4: trigger index of the event at tile_at, when the previous tile saw it
+  bool pre_have_s = false;
   bool at_start = seg == 0;         // tile_at is known to be a shot start
   uint32_t tile_i = 0;              // status words written so far
   bool seg_failed = false;
@@ -408,6 +418,19 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   const bool has_prev = lane == 0 && p0 < cnt && base + p0 > 0 && !(at_start && p0 <= skp);
   if (has_prev) t_prev = kPerm ? a.toa[a.perm[base + p0 - 1]] : a.toa[base + p0 - 1];
   const uint64_t t_first = kPerm ? a.toa[a.perm[tile_at]] : a.toa[tile_at];
+  // mode 4 needs the ToT for the timewalk correction before the keys can be laid out: requested here as well
+  uint4 vt_early = make_uint4(0u, 0u, 0u, 0u);
+  uint32_t tot_prev = 0;
+  if (kPre) {
+    if (p0 + IPT <= cnt) vt_early = ldg_nc_v4(a.tot + base + p0);
+    else {
+      uint32_t tt[IPT];
+#pragma unroll
+      for (int j = 0; j < IPT; ++j) tt[j] = p0 + j < cnt ? (uint32_t)a.tot[base + p0 + j] : 1u;
+      vt_early = make_uint4(tt[0] | (tt[1] << 16), tt[2] | (tt[3] << 16), tt[4] | (tt[5] << 16), tt[6] | (tt[7] << 16));
+    }
+    if (has_prev) tot_prev = a.tot[base + p0 - 1];
+  }
   __syncthreads();                  // the previous tile is done with the shared memory
   if (tid == 0) {
     misc->lo = kNone;
@@ -421,6 +444,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     misc->loose = 0;
     misc->min_tof = kNone;
     misc->n_klist = 0;
+    misc->kept_own = 0;
+    misc->kept_pre = 0;
     misc->max_sl = 0;
     misc->n_roots = 0;
     misc->n_list = 0;
@@ -428,12 +453,102 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   __syncthreads();
   if (misc->skip != 0u || tile_i >= seg_maxt) { seg_failed = tile_i >= seg_maxt; break; }
   // reference time of the tile: start of the shot its first event belongs to
-  const uint64_t s_base = div64(t_first, a.divP);
-  const uint64_t ref = s_base * a.P;
-
+  uint64_t ref;
+  uint64_t s_ref = 0;               // mode 4: trigger index of the tile's first event
   // ---- shot offsets and times of flight; shot boundaries ----------------------------------------
   uint32_t sl[IPT], tof[IPT];
+  uint32_t keepm = 0xFFu;           // mode 4: bit j = event p0 + j survives the preprocessing
+  bool keepp = true;                // ... and so does the event in front of this thread's first one
+  uint32_t slp, tofp;
+  bool start0, viol0;
   bool bad = false;
+  if constexpr (kPre) {
+    // Preprocessing in the load phase (R23; the arithmetic of tpx3_preprocess.cuh): shot =
+    // index of the most recent trigger, ToF = ToA - trigger, dropped beyond the cut, ToF' = ToF - table[ToT] clamped
+    // to [0, P - 1]. No division: the shot offset is a difference of trigger indices. Every event keeps the shot
+    // of its trigger period, dropped or not, so shot boundaries are found on the raw stream.
+    PreWindow* win = reinterpret_cast<PreWindow*>(smem + L::kList);     // the list region is free until the link step
+    if (pre_have_s) {     // the previous tile knew the trigger of this tile's first event: no search for the window
+      if (tid == 0) {
+        const uint64_t h0 = pre_next_s > 8ull ? pre_next_s - 8ull : 0ull;
+        win->h0 = h0;
+        win->valid = (uint32_t)(a.pre.n_trig - h0 < (uint64_t)kPreWin ? a.pre.n_trig - h0 : (uint64_t)kPreWin);
+      }
+      __syncthreads();
+      if (tid < kPreWin) win->trig[tid] = tid < win->valid ? a.pre.trig[win->h0 + tid] : ~0ull;
+      __syncthreads();
+    } else {
+      pre_window_fill(a.pre, tile_at, win);
+    }
+    {
+      uint64_t s0;
+      s_ref = pre_find(a.pre, win, t_first, s0) ? s0 : 0ull;
+    }
+    ref = (a.pre.shot_base + s_ref) * a.P;
+    // a thread's 8 events are neighbours in the stream, so nearly always in the trigger period of the one before:
+    // the last period found is kept ([c_lo, c_hi) = trigger c_s up to the next one) and tried first
+    uint64_t c_s = 0, c_lo = 1, c_hi = 0;            // empty interval
+    auto trig_at = [&](uint64_t s1) -> uint64_t {
+      const uint64_t o = s1 - win->h0;
+      return o < (uint64_t)win->valid ? win->trig[o] : a.pre.trig[s1];
+    };
+    auto pre_one = [&](uint64_t t, uint32_t tt, uint64_t& s_out, uint32_t& tof_out) -> bool {   // true: kept
+      uint64_t s1 = c_s;
+      if (!(t >= c_lo && t < c_hi)) {
+        const bool has = pre_find(a.pre, win, t, s1);
+        if (!has) { s_out = 0ull; tof_out = 0; return false; }   // no trigger yet: counted to shot 0, dropped
+        c_s = s1;
+        c_lo = trig_at(s1);
+        c_hi = s1 + 1ull < a.pre.n_trig ? trig_at(s1 + 1ull) : ~0ull;
+      }
+      s_out = s1;
+      tof_out = 0;
+      const uint64_t tf = t - c_lo;
+      if (tf > a.pre.cut) return false;
+      long long corr = 0;
+      if (a.pre.table_len) corr = a.pre.table[tt < a.pre.table_len ? tt : a.pre.table_len - 1u];
+      long long tc = (long long)tf - corr;
+      if (tc < 0) tc = 0;
+      if ((uint64_t)tc > a.P - 1ull) tc = (long long)(a.P - 1ull);
+      tof_out = (uint32_t)tc;                        // P <= 2^24
+      return true;
+    };
+    keepm = 0;
+    const uint32_t tw[4] = {vt_early.x, vt_early.y, vt_early.z, vt_early.w};
+#pragma unroll
+    for (int j = 0; j < IPT; ++j) {
+      const bool in = p0 + j < cnt && p0 + j >= skp;
+      sl[j] = 0; tof[j] = 0;
+      if (in) {
+        uint64_t s1;
+        const bool keep = pre_one(toa_r[j], (tw[j >> 1] >> ((j & 1) * 16)) & 0xFFFFu, s1, tof[j]);
+        const uint64_t d = s1 - s_ref;
+        if (d >> 31) bad = true;                     // an earlier shot behind a later one, or out of range
+        sl[j] = (uint32_t)d;
+        if (keep) keepm |= 1u << j;
+      }
+    }
+    slp = __shfl_up_sync(0xffffffffu, sl[IPT - 1], 1);
+    tofp = __shfl_up_sync(0xffffffffu, tof[IPT - 1], 1);
+    keepp = __shfl_up_sync(0xffffffffu, (keepm >> (IPT - 1)) & 1u, 1) != 0u;
+    start0 = sl[0] != slp; viol0 = sl[0] < slp;
+    if (lane == 0) {
+      if (!has_prev) { start0 = p0 < cnt; viol0 = false; slp = 0; tofp = 0; keepp = false; }
+      else {
+        uint64_t s1;
+        keepp = pre_one(t_prev, tot_prev, s1, tofp);
+        if (s1 < s_ref) { start0 = true; viol0 = false; slp = 0; keepp = false; }       // previous shot
+        else {
+          const uint64_t d = s1 - s_ref;
+          slp = (d >> 31) ? kNone : (uint32_t)d;
+          start0 = sl[0] != slp;
+          viol0 = sl[0] < slp;
+        }
+      }
+    }
+  } else {
+  const uint64_t s_base = div64(t_first, a.divP);
+  ref = s_base * a.P;
 #pragma unroll
   for (int j = 0; j < IPT; ++j) {
     const uint64_t r64 = toa_r[j] - ref;
@@ -448,9 +563,9 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       tof[j] = (uint32_t)(r64 - q * a.P);
     }
   }
-  uint32_t slp = __shfl_up_sync(0xffffffffu, sl[IPT - 1], 1);
-  uint32_t tofp = __shfl_up_sync(0xffffffffu, tof[IPT - 1], 1);
-  bool start0 = sl[0] != slp, viol0 = sl[0] < slp;
+  slp = __shfl_up_sync(0xffffffffu, sl[IPT - 1], 1);
+  tofp = __shfl_up_sync(0xffffffffu, tof[IPT - 1], 1);
+  start0 = sl[0] != slp; viol0 = sl[0] < slp;
   if (lane == 0) {
     if (!has_prev) { start0 = p0 < cnt; viol0 = false; slp = 0; tofp = 0; }          // position 0 of the stream
     else if (t_prev < ref) { start0 = true; viol0 = false; slp = 0; tofp = 0; }        // previous shot
@@ -463,6 +578,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       viol0 = sl[0] < slp;
     }
   }
+  }   // not mode 4
   uint32_t bnd = 0;  // bit j: event p0+j starts a shot
   bool viol = false;
   {
@@ -491,7 +607,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       }
       mt = max(mt, tof[j]);
       ml = max(ml, sl[j]);
-      if (p0 + j < cnt && p0 + j >= skp) mn = min(mn, tof[j]);
+      if (p0 + j < cnt && p0 + j >= skp && ((keepm >> j) & 1u)) mn = min(mn, tof[j]);
     }
     mn = __reduce_min_sync(0xffffffffu, mn);
     my_lo = __reduce_min_sync(0xffffffffu, my_lo);
@@ -559,10 +675,32 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   const uint32_t tspan = misc->max_tof + a.W;
   const uint32_t tb = tspan ? 32u - (uint32_t)__clz(tspan) : 0u;
   const uint32_t sbits = misc->max_sl ? 32u - (uint32_t)__clz(misc->max_sl) : 0u;
-  if (tb + sbits > 32u) failed = true;
-  const uint32_t mm = failed ? 0u : hi - lo;   // owned events; a failed tile owns nothing
+  if (tb + sbits > (kPre ? 31u : 32u)) failed = true;      // mode 4 keeps the key 0xFFFFFFFF for dropped events
+  const uint32_t mm_raw = failed ? 0u : hi - lo;   // owned events of the window; a failed tile owns nothing
+  uint32_t mm = mm_raw;                            // owned events that are clustered (mode 4: those that survive)
   const uint32_t tmask = tb >= 32u ? 0xFFFFFFFFu : ((1u << tb) - 1u);
-  const uint32_t out_base = (uint32_t)(base + lo);  // global sorted position of local rank 0 (n <= 2^28)
+  const uint32_t raw_base = (uint32_t)(base + lo);  // input position of the window's first owned event (n <= 2^28)
+  uint32_t out_base = raw_base;                     // global sorted position of local rank 0
+  if constexpr (kPre) {
+    // surviving events of the owned range and of what this window skips in front of it (counted into kept_run)
+    const uint32_t pre_end = misc->lo == kNone ? cnt : lo;
+    uint32_t c_own = 0, c_pre = 0;
+#pragma unroll
+    for (int j = 0; j < IPT; ++j) {
+      const uint32_t q = p0 + (uint32_t)j, kb = (keepm >> j) & 1u;
+      c_own += (q >= lo && q < lo + mm_raw) ? kb : 0u;
+      c_pre += (q >= skp && q < pre_end) ? kb : 0u;
+    }
+    c_own = __reduce_add_sync(0xffffffffu, c_own);
+    c_pre = __reduce_add_sync(0xffffffffu, c_pre);
+    if (lane == 0) {
+      if (c_own) atomicAdd(&misc->kept_own, c_own);
+      if (c_pre) atomicAdd(&misc->kept_pre, c_pre);
+    }
+    // the trigger of the event the next tile starts at (read at the end of this tile)
+    const uint64_t nrel = next_at - base;
+    if (nrel >= p0 && nrel < p0 + IPT && nrel < cnt && nrel >= skp) misc->s_next = sl[nrel - p0];
+  }
 
   // ---- records as loaded -> region B, 128-bit loads of x / y / tot ------------------------------
   uint2* recB = reinterpret_cast<uint2*>(smem + L::kRegB);
@@ -573,11 +711,26 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   bool uns = false;
   uint32_t cl_last_start = 0, cl_lead_last = 0;   // time-cluster check on the keys in registers
   bool cl_have_lead = false, cl_loose = false;
-  if (mm && p0 < hi && p0 + IPT > lo) {
+  uint32_t kp_cnt = 0, kp_max = 0, kp_first = kNone;   // mode 4: surviving owned events of this thread, their largest / first key
+  bool kp_viol = false;                                 // ... and whether they descend somewhere
+  if (mm_raw && p0 < hi && p0 + IPT > lo) {
     uint32_t key_r[IPT];
 #pragma unroll
-    for (int j = 0; j < IPT; ++j) key_r[j] = (tb >= 32u ? 0u : (sl[j] << tb)) | tof[j];
-    const uint32_t keyp = (tb >= 32u ? 0u : (slp << tb)) | tofp;
+    for (int j = 0; j < IPT; ++j)
+      key_r[j] = ((keepm >> j) & 1u) ? ((tb >= 32u ? 0u : (sl[j] << tb)) | tof[j]) : 0xFFFFFFFFu;   // dropped: behind all others
+    const uint32_t keyp = keepp ? ((tb >= 32u ? 0u : (slp << tb)) | tofp) : 0xFFFFFFFFu;
+    if constexpr (kPre) {   // for the compaction below: this thread's surviving owned events
+#pragma unroll
+      for (int j = 0; j < IPT; ++j) {
+        const uint32_t q = p0 + (uint32_t)j;
+        if (q >= lo && q < hi && ((keepm >> j) & 1u)) {
+          if (kp_cnt && key_r[j] < kp_max) kp_viol = true;
+          if (!kp_cnt) kp_first = key_r[j];
+          kp_max = max(kp_max, key_r[j]);
+          ++kp_cnt;
+        }
+      }
+    }
     // already in (shot, ToA) order? (configs 0-3 arrive sorted; config 4 does not)
     if (p0 > lo && key_r[0] < keyp) uns = true;
 #pragma unroll
@@ -603,7 +756,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     if (!kPerm && p0 + IPT <= cnt) {
       vx = ldg_nc_v4(a.x + base + p0);
       vy = ldg_nc_v4(a.y + base + p0);
-      vt = ldg_nc_v4(a.tot + base + p0);
+      vt = kPre ? vt_early : ldg_nc_v4(a.tot + base + p0);
     } else {
       uint16_t tx[IPT], ty[IPT], tt[IPT];
 #pragma unroll
@@ -662,9 +815,27 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     cl_carry = __shfl_up_sync(0xffffffffu, cl_inc, 1);
     if (lane == 0) cl_carry = 0;
   }
+  uint32_t kp_excl = 0, kp_pmax = 0;
+  if constexpr (kPre) {   // warp scans: surviving events in front of this thread (sum) and their largest key (max)
+    uint32_t ic = kp_cnt, im = kp_max;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t tc = __shfl_up_sync(0xffffffffu, ic, o), tm = __shfl_up_sync(0xffffffffu, im, o);
+      if (lane >= (uint32_t)o) { ic += tc; im = max(im, tm); }
+    }
+    if (lane == 31) { misc->warp_cnt[warp] = ic; misc->warp_max[warp] = im; }
+    kp_excl = ic - kp_cnt;
+    kp_pmax = __shfl_up_sync(0xffffffffu, im, 1);
+    if (lane == 0) kp_pmax = 0;
+  }
   const bool out_of_order = __syncthreads_or(!kGiven && uns ? 1 : 0) != 0;
   const bool unsorted = !kPerm && out_of_order;    // a given perm is never re-sorted (mode 5: it IS the (shot, ToA) order)
   if (MODE == 5 && out_of_order) failed = true;
+  if constexpr (kPre) {     // (a tile whose keys ascend has its dropped events, key 0xFFFFFFFF, at the end: first mm records)
+    mm = failed ? 0u : misc->kept_own;
+    out_base = kept_run + misc->kept_pre;
+    kept_run = out_base + mm;
+  }
   if (cl_wide && !cl_scan && tid == 0) misc->loose = 1u;   // not checked: treated as not tight
   if (!unsorted && cl_scan) {
     for (uint32_t w = 0; w < warp; ++w) cl_carry = max(cl_carry, misc->warp_sums[w]);
@@ -681,6 +852,25 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     const uint32_t tofb = misc->max_tof ? 32u - (uint32_t)__clz(misc->max_tof) : 1u;
     const uint32_t key_bits = tofb + sbits;
     const uint16_t* fin;
+    // (0) Mode 4: a tile is usually out of order only because dropped events (key 0xFFFFFFFF) sit between the
+    // surviving ones. If the surviving keys ascend, their ranks are a prefix count: no sort.
+    bool compacted = false;
+    if constexpr (kPre) {
+      for (uint32_t w = 0; w < warp; ++w) { kp_excl += misc->warp_cnt[w]; kp_pmax = max(kp_pmax, misc->warp_max[w]); }
+      const bool desc = kp_viol || (kp_cnt && kp_first < kp_pmax);
+      compacted = __syncthreads_or(desc ? 1 : 0) == 0;
+      if (compacted) {
+        uint32_t r = kp_excl;
+#pragma unroll
+        for (int j = 0; j < IPT; ++j) {
+          const uint32_t q = p0 + (uint32_t)j;
+          if (q >= lo && q < hi && ((keepm >> j) & 1u)) buf1[r++] = (uint16_t)(q - lo);
+        }
+        fin = buf1;
+        __syncthreads();
+      }
+    }
+    if (!compacted) {
     // (a) Rank by counting. What has to be computed is the RANK of every event among the composite values
     // (key, input position), which are all different, so nothing here needs to be stable. Detector streams hold
     // few distinct keys per tile (time of flight is quantised and bunched: 5 mass peaks of about 100 ticks on
@@ -698,10 +888,6 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     // more than one) are left to the count of smaller positions.
     uint32_t* gcnt = reinterpret_cast<uint32_t*>(smem + L::kRegX + 4 * T);       // [T] words
     static_assert(IPT == 8, "eight position blocks = eight 4-bit counts per word");
-    auto nib_sum = [](uint32_t w) -> uint32_t {                                   // sum of the eight 4-bit fields
-      w = (w & 0x0F0F0F0Fu) + ((w >> 4) & 0x0F0F0F0Fu);
-      return (w * 0x01010101u) >> 24;
-    };
     bool counted = key_bits <= 31u && (1u << key_bits) <= kBitmapBits;
     if (counted) {
       const uint32_t nwords = ((1u << key_bits) + 31u) >> 5;
@@ -709,11 +895,13 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 #pragma unroll
       for (int j = 0; j < IPT; ++j) {
         const uint32_t k = (uint32_t)j * THREADS + tid;
-        uint32_t sk = 0;
-        if (k < mm) {
+        uint32_t sk = kNone;                  // kNone: no event here (mode 4: or one the preprocessing dropped)
+        if (k < mm_raw) {
           const uint32_t key = recB[lo + k].x;
-          sk = ((key >> tb) << tofb) | (key & tmask);
-          atomicOr(&bitmap[sk >> 5], 1u << (sk & 31u));
+          if (!kPre || key != 0xFFFFFFFFu) {
+            sk = ((key >> tb) << tofb) | (key & tmask);
+            atomicOr(&bitmap[sk >> 5], 1u << (sk & 31u));
+          }
         }
         sk_r[j] = sk;
       }
@@ -744,27 +932,48 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       }
       __syncthreads();
       uint32_t dk_r[IPT];   // dense key | arrival slot inside (key, position block) << 16
-      bool big = false;     // a 4-bit count overflowed: one key held by 16 events of one position block
-#pragma unroll
-      for (int j = 0; j < IPT; ++j) {
-        const uint32_t k = (uint32_t)j * THREADS + tid;
-        dk_r[j] = 0;
-        if (k < mm) {
-          const uint32_t sk = sk_r[j], w = sk >> 5;
-          const uint32_t dk = (uint32_t)wpre[w] + (uint32_t)__popc(bitmap[w] & ((1u << (sk & 31u)) - 1u));
-          const uint32_t r = (atomicAdd(&gcnt[dk], 1u << (4 * j)) >> (4 * j)) & 15u;
-          big = big || r == 15u;
-          dk_r[j] = dk | (r << 16);
+      // Counter fields: first eight 4-bit counts per key (position blocks of THREADS events). If one of them
+      // overflows — 16 events of one key inside one position block: electron VMI, where a shot's few hundred
+      // events share 95 ticks — the step is redone with four 8-bit counts (blocks of 2 * THREADS events); the
+      // members of one field are then ordered by the count of smaller positions, whatever their number.
+      auto fsum = [](uint32_t w, uint32_t cb) -> uint32_t {            // sum of the fields of a counter word
+        if (cb == 4u) {
+          w = (w & 0x0F0F0F0Fu) + ((w >> 4) & 0x0F0F0F0Fu);
+          return (w * 0x01010101u) >> 24;
         }
+        return (w & 0xFFu) + ((w >> 8) & 0xFFu) + ((w >> 16) & 0xFFu) + (w >> 24);
+      };
+      bool big = false;
+      uint32_t cb = 4u;
+      for (;;) {
+        const uint32_t fmask = (1u << cb) - 1u;
+        big = false;
+#pragma unroll
+        for (int j = 0; j < IPT; ++j) {
+          dk_r[j] = kNone;
+          if (sk_r[j] != kNone) {
+            const uint32_t sk = sk_r[j], w = sk >> 5;
+            const uint32_t dk = (uint32_t)wpre[w] + (uint32_t)__popc(bitmap[w] & ((1u << (sk & 31u)) - 1u));
+            const uint32_t sh = cb == 4u ? 4u * (uint32_t)j : 8u * ((uint32_t)j >> 1);
+            const uint32_t r = (atomicAdd(&gcnt[dk], 1u << sh) >> sh) & fmask;
+            big = big || r == fmask;
+            dk_r[j] = dk | (r << 16);
+          }
+        }
+        big = __syncthreads_or(big ? 1 : 0) != 0;
+        if (!big || cb == 8u) break;
+        for (uint32_t i = tid; i < (uint32_t)T; i += THREADS) gcnt[i] = 0u;     // again, with wider fields
+        cb = 8u;
+        __syncthreads();
       }
-      big = __syncthreads_or(big ? 1 : 0) != 0;
       if (!big) {
+        const uint32_t fmask = (1u << cb) - 1u;
         {   // offsets: exclusive scan of the group sizes, 8 consecutive dense keys per thread (at most mm <= T keys)
           const uint4 q0 = *reinterpret_cast<const uint4*>(gcnt + p0), q1 = *reinterpret_cast<const uint4*>(gcnt + p0 + 4);
           const uint32_t qw[IPT] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w};
           uint32_t c[IPT], sum = 0;
 #pragma unroll
-          for (int j = 0; j < IPT; ++j) { c[j] = nib_sum(qw[j]); sum += c[j]; }
+          for (int j = 0; j < IPT; ++j) { c[j] = fsum(qw[j], cb); sum += c[j]; }
           uint32_t inc = sum;
 #pragma unroll
           for (int o = 1; o < 32; o <<= 1) {
@@ -789,11 +998,12 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         for (int j = 0; j < IPT; ++j) {
           const uint32_t k = (uint32_t)j * THREADS + tid;
           b0_r[j] = 0;
-          if (k < mm) {
+          if (dk_r[j] != kNone) {
             const uint32_t dk = dk_r[j] & 0xFFFFu, r = dk_r[j] >> 16;
             const uint32_t w = gcnt[dk];
+            const uint32_t sh = cb == 4u ? 4u * (uint32_t)j : 8u * ((uint32_t)j >> 1);
             // the group's members of earlier position blocks come first
-            const uint32_t b0 = (uint32_t)gbase[dk] + nib_sum(w & ((1u << (4 * j)) - 1u)), m = (w >> (4 * j)) & 15u;
+            const uint32_t b0 = (uint32_t)gbase[dk] + fsum(w & ((1u << sh) - 1u), cb), m = (w >> sh) & fmask;
             b0_r[j] = b0 | (m << 16);
             if (m == 1u) buf1[b0] = (uint16_t)k;      // alone with its key in its position block: final position
             else buf0[b0 + r] = (uint16_t)k;          // the sub-group's members in arrival order
@@ -804,7 +1014,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         for (int j = 0; j < IPT; ++j) {
           const uint32_t k = (uint32_t)j * THREADS + tid;
           const uint32_t b0 = b0_r[j] & 0xFFFFu, m = b0_r[j] >> 16;
-          if (k < mm && m > 1u) {
+          if (m > 1u) {
             uint32_t c = 0;
             for (uint32_t q = 0; q < m; ++q) c += (uint32_t)buf0[b0 + q] < k ? 1u : 0u;   // members at earlier input positions
             buf1[b0 + c] = (uint16_t)k;
@@ -812,7 +1022,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         }
         fin = buf1;
       } else {
-        counted = false;      // the LSD sort below
+        counted = false;      // 256 events of one key in one position block: the LSD sort below
       }
       __syncthreads();
     }
@@ -838,9 +1048,11 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 #pragma unroll
       for (int j = 0; j < IPT; ++j) {
         const uint32_t k = warp * (32u * IPT) + (uint32_t)j * 32u + lane;   // warps own ascending slices
-        const bool valid = k < mm;
+        // first pass: the owned events as loaded (mode 4: but for the dropped ones); later passes: the mm survivors
+        bool valid = pass == 0 ? k < mm_raw : k < mm;
         const uint32_t s = valid ? (pass == 0 ? k : (uint32_t)src[k]) : 0u;
         const uint32_t key = valid ? recB[lo + s].x : 0u;
+        if (kPre && key == 0xFFFFFFFFu) valid = false;
         const uint32_t sk = ((key >> tb) << tofb) | (key & tmask);
         const uint32_t d = (sk >> shift) & dmask;
         // lanes holding the same digit (ballot per digit bit; match.any is 20x dearer on sm_100)
@@ -894,11 +1106,12 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     }
     fin = (npass & 1u) ? buf1 : buf0;
     }
+    }   // not compacted
     // gather the records into sorted order (region A) and emit perm
     for (uint32_t k = tid; k < mm; k += THREADS) {
       const uint32_t s = fin[k];
       recA[k] = recB[lo + s];
-      a.perm[out_base + k] = out_base + s;
+      a.perm[out_base + k] = raw_base + s;
     }
     __syncthreads();
     // the hash table now takes X + B: clear it
@@ -909,7 +1122,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     __syncthreads();
   } else {
     if (!kPerm)
-      for (uint32_t k = tid; k < mm; k += THREADS) a.perm[out_base + k] = out_base + k;
+      for (uint32_t k = tid; k < mm; k += THREADS) a.perm[out_base + k] = raw_base + k;
   }
   const uint2* recS = unsorted ? recA : recB + lo;
   unsigned char* hreg = smem + (unsorted ? L::kRegX : L::kRegA);   // 16T bytes: hash table, later the label / chain arrays
@@ -1447,6 +1660,10 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   }
   if (failed) { seg_failed = true; break; }
   at_start = misc->lo != kNone;     // everything but "no shot start in sight" ends at a shot start
+  if constexpr (kPre) {
+    pre_have_s = next_at < base + cnt && next_at - base >= skp;
+    pre_next_s = s_ref + misc->s_next;
+  }
   tile_at = next_at;
   if (tile_at >= seg_end) break;
   }   // tiles of the segment
@@ -1612,6 +1829,7 @@ inline int fused_configure_device() {
   TPX3_FUSED_ATTR(4096, 512, 0) TPX3_FUSED_ATTR(4096, 512, 1) TPX3_FUSED_ATTR(4096, 512, 2) TPX3_FUSED_ATTR(4096, 512, 3)
   TPX3_FUSED_ATTR(8192, 1024, 0) TPX3_FUSED_ATTR(8192, 1024, 1) TPX3_FUSED_ATTR(8192, 1024, 2)
   TPX3_FUSED_ATTR(8192, 1024, 3) TPX3_FUSED_ATTR(8192, 1024, 5)
+  TPX3_FUSED_ATTR(2048, 256, 4) TPX3_FUSED_ATTR(4096, 512, 4) TPX3_FUSED_ATTR(8192, 1024, 4)
 #undef TPX3_FUSED_ATTR
   return TPX3_OK;
 }
@@ -1665,6 +1883,8 @@ inline FusedArgs make_fused_args(uint32_t T, uint32_t num_sms, Ctrl* ctrl, unsig
   a.stage_d = a.stage_c + prm.n;
   a.mode = mode; a.lm_wx = lm_wx; a.lm_wy = lm_wy;
   a.label_base = nullptr;
+  memset(&a.pre, 0, sizeof(a.pre));
+  a.seg_kept = nullptr;
   a.labels_only = 0;
   a.n_dev = n_dev;      // then prm.n is the largest count: it sizes the grids and lays out the staging table
   return a;
@@ -1714,7 +1934,8 @@ inline int enqueue_fused(const FusedGeom& g, uint32_t num_sms, uint64_t* launche
                          const uint64_t* toa, const uint16_t* tot, uint32_t* perm, uint32_t* label,
                          uint64_t max_clusters, const tpx3_clusters_t& out, uint32_t* n_clusters, void* stage,
                          bool* launched, FusedArgs* args, uint32_t mode = 0, uint32_t lm_wx = 0, uint32_t lm_wy = 0,
-                         const uint32_t* n_dev = nullptr, const uint64_t* label_base = nullptr) {
+                         const uint32_t* n_dev = nullptr, const uint64_t* label_base = nullptr,
+                         const PreArgs* pre = nullptr, const uint32_t* seg_kept = nullptr) {
   *launched = false;
   if (g.variant == 0 || prm.n == 0) return TPX3_OK;
   // the 128-bit load phase needs 16-byte aligned inputs (PyTorch allocations are 256-byte aligned)
@@ -1723,6 +1944,7 @@ inline int enqueue_fused(const FusedGeom& g, uint32_t num_sms, uint64_t* launche
   FusedArgs a = make_fused_args(g.T, num_sms, ctrl, tiles, prm, x, y, toa, tot, perm, label, max_clusters, out,
                                 n_clusters, stage, mode, lm_wx, lm_wy, n_dev);
   a.label_base = label_base;
+  if (pre) { a.pre = *pre; a.seg_kept = seg_kept; }
   if (n_dev) {   // grids that cover every count up to prm.n (fused_segs: a short input is cut into up to `want` segments)
     const uint32_t want = num_sms * (g.T <= 2048u ? 4u : (g.T <= 4096u ? 2u : 1u)) * 8u + 1u;
     if (a.nseg < want) a.nseg = want;
@@ -1736,6 +1958,7 @@ inline int enqueue_fused(const FusedGeom& g, uint32_t num_sms, uint64_t* launche
   if (mode == 0u) rc = TPX3_PICK(0);
   else if (mode == 1u) rc = TPX3_PICK(1);
   else if (mode == 2u) rc = TPX3_PICK(2);
+  else if (mode == 4u) rc = TPX3_PICK(4);
   else rc = TPX3_PICK(3);
 #undef TPX3_PICK
   if (rc != TPX3_OK) return rc;

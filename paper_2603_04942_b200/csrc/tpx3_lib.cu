@@ -27,7 +27,7 @@ struct tpx3_plan_s {
   int num_sms;
   // workspace offsets (bytes from the workspace base), sized for cfg.max_hits
   size_t off_keyA, off_keyB, off_idxA, off_idxB, off_xy, off_tot, off_slab, off_table, off_counts;
-  size_t off_slot, off_peak, off_blkcnt, off_tiles;
+  size_t off_slot, off_peak, off_blkcnt, off_tiles, off_segk;
   uint32_t table_mask_max;
   FusedGeom fused;          // which fused variant serves this plan (variant 0: none)
   // optional per-stage timing (tpx3_profile_*)
@@ -93,6 +93,7 @@ struct Ws {
   uint16_t* tot;
   unsigned long long* peak;
   unsigned long long* tiles;
+  uint32_t* segk;
 };
 
 inline Ws carve(const tpx3_plan_s* p, void* workspace) {
@@ -112,6 +113,7 @@ inline Ws carve(const tpx3_plan_s* p, void* workspace) {
   w.peak = (unsigned long long*)(b + p->off_peak);
   w.blkcnt = (uint32_t*)(b + p->off_blkcnt);
   w.tiles = (unsigned long long*)(b + p->off_tiles);
+  w.segk = (uint32_t*)(b + p->off_segk);
   return w;
 }
 
@@ -254,6 +256,10 @@ __global__ void k_fallback_dispatch(GenArgs a, FusedArgs fa, FusedLadder ladder,
     fa.G = sg.G; fa.nseg = sg.nseg; fa.maxt = sg.maxt; fa.num_tiles = sg.nseg * sg.maxt;
     launch_fused_rung_device(fa, ladder.T[rung]);
     k_fallback_dispatch<<<1, 1, 0, cudaStreamTailLaunch>>>(a, fa, ladder, rung + 1, what);
+    return;
+  }
+  if (what == 4) {                      // the fused preprocessing call has no second route: the status word says so
+    set_error(c, TPX3_ERR_NOT_CONTIGUOUS);
     return;
   }
 #define GP(stage, kernel, grid, block, ...) kernel<<<(grid), (block), 0, cudaStreamTailLaunch>>>(__VA_ARGS__)
@@ -447,6 +453,9 @@ int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace
   p->off_peak = p->off_keyB;                    // 8N
   p->off_blkcnt = p->off_idxA;                  // 4 * ceil(N/4096) <= 4N
   p->off_tiles = o; o = align_up(o + 8 * (size_t)(N / 128 + 262144));   // fused path tile status words (fused_segs: nseg * maxt)
+  // fused preprocessing call: surviving events in front of every segment (read while the staging table is written,
+  // so it may not alias the sort buffers)
+  p->off_segk = o; o = align_up(o + 4 * (size_t)(N / 4096 + 16384));
   p->workspace_bytes = o;
   *workspace_bytes = o;
   *out_plan = p;
@@ -560,6 +569,51 @@ int tpx3_cluster_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uin
   if (n && (!x || !y || !toa || !tot || !perm || !label || !out)) return TPX3_ERR_INVALID_ARG;
   if (max_clusters && !clusters_ok(out)) return TPX3_ERR_INVALID_ARG;
   return run_fused_or_general(p, workspace, cuda_stream, n, x, y, toa, tot, perm, label, max_clusters, out, n_clusters, 0u);
+}
+
+int tpx3_preprocess_cluster_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x,
+                                     const uint16_t* y, const uint64_t* toa, const uint16_t* tot, uint64_t n_trig,
+                                     const uint64_t* trig, uint64_t cut, const int32_t* table, uint32_t table_len,
+                                     uint64_t shot_base, uint32_t* perm, uint32_t* label, uint64_t max_clusters,
+                                     const tpx3_clusters_t* out, uint32_t* n_clusters, uint32_t* n_kept) {
+  if (!p || !workspace || !n_clusters || !n_kept) return TPX3_ERR_INVALID_ARG;
+  if (n > p->cfg.max_hits || (cut >> 63) != 0) return TPX3_ERR_INVALID_ARG;
+  if (p->fused.variant == 0 || p->cfg.max_shot_hits == 0) return TPX3_ERR_INVALID_ARG;   // needs a tile kernel and its window
+  if (n && (!x || !y || !toa || !tot || !perm || !label || !out)) return TPX3_ERR_INVALID_ARG;
+  if ((n_trig && !trig) || (table_len && !table)) return TPX3_ERR_INVALID_ARG;
+  if (max_clusters && !clusters_ok(out)) return TPX3_ERR_INVALID_ARG;
+  if ((((uintptr_t)x | (uintptr_t)y | (uintptr_t)toa | (uintptr_t)tot) & 15u) != 0) return TPX3_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (use_device(p) != TPX3_OK) return TPX3_ERR_CUDA;
+  Ws w = carve(p, workspace);
+  if (p->profiling) ++p->profiled_calls;
+  TPX3_LAUNCH(p, k_ctrl_init, 1, 256, 0, st, w.ctrl, n, w.tiles, 0u, n_clusters);
+  if (n == 0) {
+    if (cudaMemsetAsync(n_kept, 0, sizeof(uint32_t), st) != cudaSuccess) return TPX3_ERR_CUDA;
+    return cuda_ok(cudaGetLastError());
+  }
+  PreArgs pa;
+  memset(&pa, 0, sizeof(pa));
+  pa.n = n; pa.x = x; pa.y = y; pa.tot = tot; pa.toa = toa; pa.n_trig = n_trig; pa.trig = trig; pa.cut = cut;
+  pa.P = p->cfg.shot_period_ticks; pa.shot_base = shot_base; pa.table = table; pa.table_len = table_len;
+  Params prm = p->prm;
+  prm.n = n;
+  StageTimer timer(p, st, TPX3_STAGE_FUSED);
+  // pre-pass: surviving events in front of every segment of the tile kernel's grid (same segment length)
+  const FusedSegs sg = fused_segs(n, p->fused.T, (uint32_t)p->num_sms);
+  TPX3_LAUNCH(p, k_pre_seg_count, sg.nseg, kPreThreads, 0, st, pa, sg.G, w.segk);
+  TPX3_LAUNCH(p, k_pre_seg_scan, 1, 1024, 0, st, w.segk, sg.nseg, n_kept);
+  GenArgs ga = make_gen_args(p, w, 1, n, x, y, toa, tot, perm, label, max_clusters, out, n_clusters);
+  bool launched = false;
+  FusedArgs fa;
+  int rc = enqueue_fused(p->fused, (uint32_t)p->num_sms, &p->launches, w.ctrl, w.tiles, st, prm, x, y, toa, tot, perm,
+                         label, max_clusters, *out, n_clusters, (char*)workspace + p->off_keyA, &launched, &fa, 4u, 0u, 0u,
+                         nullptr, nullptr, &pa, w.segk);
+  if (rc != TPX3_OK) return rc;
+  if (!launched) return TPX3_ERR_INVALID_ARG;
+  k_fallback_dispatch<<<1, 1, 0, st>>>(ga, fa, FusedLadder{0, {0, 0}}, 0, 4);
+  ++p->launches;
+  return cuda_ok(cudaGetLastError());
 }
 
 int tpx3_localmax_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t n, const uint16_t* x,
@@ -1047,6 +1101,7 @@ const char* tpx3_strerror(int err) {
     case TPX3_ERR_CAPACITY: return "max_clusters too small";
     case TPX3_ERR_OUT_OF_RANGE: return "event outside the sensor or ToT == 0";
     case TPX3_ERR_CUDA: return "CUDA runtime error";
+    case TPX3_ERR_NOT_CONTIGUOUS: return "stream not shot-contiguous or a shot longer than the window (fused preprocessing call)";
     default: return "unknown error";
   }
 }

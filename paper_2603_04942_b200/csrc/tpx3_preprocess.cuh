@@ -155,6 +155,43 @@ __global__ void __launch_bounds__(kPreThreads) k_pre_mark(PreArgs a) {
   if (threadIdx.x == 0) a.blk[blockIdx.x] = s_cnt;
 }
 
+// Fused route (tpx3_preprocess_cluster_centroid): the tile kernel drops events in its load phase, so all it needs
+// from a pre-pass is the number of SURVIVING events in front of every segment of G events (its sorted positions
+// count only those). Block g counts segment g, 4096 events at a time; reads ToA only, like k_pre_mark.
+__global__ void __launch_bounds__(kPreThreads) k_pre_seg_count(PreArgs a, uint32_t G, uint32_t* seg_kept) {
+  __shared__ uint32_t s_cnt;
+  __shared__ PreWindow s_win;
+  const uint64_t seg_begin = (uint64_t)blockIdx.x * G;
+  const uint64_t seg_end = seg_begin + G < a.n ? seg_begin + G : a.n;
+  if (threadIdx.x == 0) s_cnt = 0;
+  uint32_t cnt = 0;
+  for (uint64_t base = seg_begin; base < seg_end; base += kPreTile) {     // block-uniform trip count
+    pre_window_fill(a, base, &s_win);
+    uint64_t t[kPreItems];
+#pragma unroll
+    for (int i = 0; i < kPreItems; ++i) {
+      const uint64_t k = base + (uint64_t)i * kPreThreads + threadIdx.x;
+      t[i] = k < seg_end ? a.toa[k] : 0ull;
+    }
+#pragma unroll
+    for (int i = 0; i < kPreItems; ++i) {
+      const uint64_t k = base + (uint64_t)i * kPreThreads + threadIdx.x;
+      if (k < seg_end) cnt += pre_event(a, &s_win, t[i], 0u, false) != kPreDropped;
+    }
+    __syncthreads();                                                       // the window is refilled next round
+  }
+  cnt = __reduce_add_sync(0xffffffffu, cnt);
+  if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(&s_cnt, cnt);
+  __syncthreads();
+  if (threadIdx.x == 0) seg_kept[blockIdx.x] = s_cnt;
+}
+
+// Exclusive scan over the segments (one block); the total is the number of surviving events.
+__global__ void __launch_bounds__(1024) k_pre_seg_scan(uint32_t* seg_kept, uint32_t nseg, uint32_t* n_kept) {
+  const uint32_t x = scan_inplace_1024(seg_kept, nseg);
+  if (threadIdx.x == 0) *n_kept = x;
+}
+
 __global__ void __launch_bounds__(1024) k_pre_scan(PreArgs a) {
   const uint32_t x = scan_inplace_1024(a.blk, a.nblk);
   if (threadIdx.x == 0) *a.n_out = x;

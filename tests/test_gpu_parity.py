@@ -1136,6 +1136,145 @@ def test_stream_takes_nothing_after_the_final_push(tpx3):
     pl.free()
 
 
+def _raw_stream(cfg, shots, seed, dark_every=10, shuffle=False):
+    """A config stream moved onto irregular trigger times with timewalk added and dark counts beyond the cut,
+    in raw-time order (or as delivered by config 4: locally shuffled). Returns the raw arrays and the call's
+    parameters; the original stream comes back from oracle.preprocess (tests/test_oracle_pins.py pins that)."""
+    from oracle import preprocess as pp
+
+    w = gen.generate(cfg, shots=shots)
+    rng = np.random.default_rng(seed)
+    trig = np.cumsum(rng.integers(P - 2000, P + 2000, w.shots)).astype(np.int64) + 12345
+    table = pp.timewalk_table(800.0, 4.0, 0.0, 1.0, 1024)
+    shot = (w.toa // np.uint64(P)).astype(np.int64)
+    shot -= shot.min()
+    tof = (w.toa % np.uint64(P)).astype(np.int64)
+    raw = trig[shot] + tof + table[np.minimum(w.tot, 1023)]
+    cut = int(tof.max() + table.max())
+    nd = w.n // dark_every if dark_every else 0
+    dshot = rng.integers(0, w.shots, nd)
+    draw = trig[dshot] + rng.integers(cut + 1, P - 3000, nd)
+    allx = np.concatenate([w.x, rng.integers(0, 256, nd).astype(np.uint16)])
+    ally = np.concatenate([w.y, rng.integers(0, 256, nd).astype(np.uint16)])
+    alltot = np.concatenate([w.tot, rng.integers(1, 30, nd).astype(np.uint16)])
+    allraw = np.concatenate([raw, draw]).astype(np.uint64)
+    if shuffle:   # keep config 4's delivery order inside a shot; dark counts go behind their shot's events
+        order = np.argsort(np.concatenate([shot, dshot]), kind="stable")
+    else:
+        order = np.argsort(allraw, kind="stable")
+    per_shot = int(np.bincount(np.concatenate([shot, dshot])).max())
+    return allx[order], ally[order], allraw[order], alltot[order], trig.astype(np.uint64), cut, table, per_shot
+
+
+@pytest.mark.parametrize("cfg,shots,dark,shuffle", [(2, 300, 10, False), (1, 1500, 0, False), (4, 300, 7, True),
+                                                    (0, 900, 3, False), (3, 60, 10, False)])
+def test_preprocess_fused_into_the_clustering_call(tpx3, cfg, shots, dark, shuffle):
+    """tpx3_preprocess_cluster_centroid (SURVEY 8f NEXT #3 as worded): the oracle's preprocessing followed by the
+    oracle's clustering, element by element — perm (as input positions), labels, every hit column — and the
+    two-call device route gives the same."""
+    import torch
+    from oracle import preprocess as pp
+
+    x, y, raw, tot, trig, cut, table, per_shot = _raw_stream(cfg, shots, 100 + cfg, dark, shuffle)
+    n = len(x)
+    ex, ey, et, eo, ei = pp.preprocess(x, y, raw, tot, trig, cut, table, P, 5)
+    o = oracle.run(ex, ey, et, eo, W, P)
+    pl = tpx3.plan(tpx3.Config(max_hits=n, toa_window_ticks=W, shot_period_ticks=P, max_shot_hits=per_shot))
+    dev = [to_dev(a) for a in (x, y, raw, tot)]
+    dtrig, dtab = to_dev(trig), to_dev(np.asarray(table, dtype=np.int32))
+    cl = tpx3.Clusters(n, pl.device)
+    perm, label, nc, nk = pl.preprocess_cluster_centroid(*dev, dtrig, cut, dtab, 5, cl)
+    torch.cuda.synchronize()
+    st = pl.status()
+    assert st["error"] == 0 and st["path"] == 1, st
+    k = int(nk.cpu().numpy()[0])
+    assert k == len(ei)
+    ncl = int(nc.cpu().numpy()[0])
+    g = {"perm": perm[:k].cpu().numpy(), "label": label[:k].cpu().numpy(), "n_clusters": ncl}
+    g.update(cl.numpy(ncl))
+    want = dict(o)
+    want["perm"] = ei[o["perm"]].astype(np.uint32)          # input positions
+    assert_parity(g, want, "fused preprocessing cfg%d" % cfg)
+    # the two calls on the device: same hits
+    xo, yo, to, oo, io, no = pl.preprocess(*dev, dtrig, cut, dtab, 5)
+    torch.cuda.synchronize()
+    k2 = int(no.cpu().numpy()[0])
+    assert k2 == k
+    cl2 = tpx3.Clusters(n, pl.device)
+    perm2, label2, nc2 = pl.cluster_centroid(xo[:k].contiguous(), yo[:k].contiguous(), to[:k].contiguous(),
+                                             oo[:k].contiguous(), cl2)
+    torch.cuda.synchronize()
+    assert int(nc2.cpu().numpy()[0]) == ncl
+    np.testing.assert_array_equal(io[:k].cpu().numpy()[perm2[:k].cpu().numpy()], g["perm"])
+    np.testing.assert_array_equal(label2[:k].cpu().numpy(), g["label"])
+    g2 = cl2.numpy(ncl)
+    for key in LM_KEYS:
+        np.testing.assert_array_equal(g2[key], g[key], err_msg=key)
+    pl.free()
+
+
+def test_preprocess_fused_edge_cases(tpx3):
+    import torch
+    from oracle import preprocess as pp
+
+    def run(x, y, toa, tot, trig, cut, table, shot_base, hint=64):
+        x = np.asarray(x, dtype=np.uint16); y = np.asarray(y, dtype=np.uint16)
+        toa = np.asarray(toa, dtype=np.uint64); tot = np.asarray(tot, dtype=np.uint16)
+        trig = np.asarray(trig, dtype=np.uint64)
+        n = len(x)
+        pl = tpx3.plan(tpx3.Config(max_hits=max(n, 1), toa_window_ticks=W, shot_period_ticks=P, max_shot_hits=hint))
+        dv = lambda a, dt: to_dev(a) if len(a) else torch.empty(0, dtype=dt, device="cuda")  # noqa: E731
+        tb = None if table is None else to_dev(np.asarray(table, dtype=np.int32))
+        cl = tpx3.Clusters(max(n, 1), pl.device)
+        perm, label, nc, nk = pl.preprocess_cluster_centroid(dv(x, torch.uint16), dv(y, torch.uint16), dv(toa, torch.uint64),
+                                                             dv(tot, torch.uint16), dv(trig, torch.uint64), cut, tb,
+                                                             shot_base, cl)
+        torch.cuda.synchronize()
+        st = pl.status()
+        k, ncl = int(nk.cpu().numpy()[0]), int(nc.cpu().numpy()[0])
+        g = {"perm": perm[:k].cpu().numpy(), "label": label[:k].cpu().numpy(), "n_clusters": ncl}
+        g.update(cl.numpy(ncl))
+        pl.free()
+        return st, k, g
+
+    def want(x, y, toa, tot, trig, cut, table, shot_base):
+        ex, ey, et, eo, ei = pp.preprocess(np.asarray(x, np.uint16), np.asarray(y, np.uint16), np.asarray(toa, np.uint64),
+                                           np.asarray(tot, np.uint16), np.asarray(trig, np.uint64), cut,
+                                           [] if table is None else table, P, shot_base)
+        o = dict(oracle.run(ex, ey, et, eo, W, P))
+        o["perm"] = ei[o["perm"]].astype(np.uint32)
+        return len(ei), o
+
+    # the hand example of the oracle pins, with the triggers a shot period apart so that it is shot-contiguous:
+    # cut edge, clamp at 0, ToT beyond the table, an event before the first trigger
+    base = [1000, 1000 + P, 1000 + 2 * P]
+    toa = [900, 1000, 1300, 1301, base[1] + 4, base[1] + 150, base[1] + 999, base[2] + 100, base[2] + 3]
+    args = (list(range(9)), [2 * v for v in range(9)], toa, [1, 1, 2, 2, 3, 3, 9, 1, 1], base, 300, [9, 5, 2, 0], 7)
+    st, k, g = run(*args)
+    kk, o = want(*args)
+    assert st["error"] == 0 and k == kk
+    assert_parity(g, o, "hand example")
+    # nothing in; no triggers (everything dropped); no table
+    st, k, g = run([], [], [], [], [5], 10, [1], 0)
+    assert st["error"] == 0 and k == 0 and g["n_clusters"] == 0
+    st, k, g = run([1, 2], [3, 4], [100, 200], [5, 6], [], 10, [1], 0)
+    assert st["error"] == 0 and k == 0 and g["n_clusters"] == 0
+    args = ([1, 2], [3, 4], [100, 200], [5, 6], [50], 1000, None, 3)
+    st, k, g = run(*args)
+    kk, o = want(*args)
+    assert st["error"] == 0 and k == kk == 2
+    assert_parity(g, o, "no table")
+    # a stream that is not shot-contiguous (shots interleaved) and one whose shots exceed the window: reported
+    x, y, raw, tot, trig, cut, table, per_shot = _raw_stream(1, 200, 3, 10, False)
+    rng = np.random.default_rng(0)
+    p = rng.permutation(len(x))
+    st, _, _ = run(x[p], y[p], raw[p], tot[p], trig, cut, table, 0, hint=per_shot)
+    assert st["error"] == tpx3.ERR_NOT_CONTIGUOUS
+    x, y, raw, tot, trig, cut, table, per_shot = _raw_stream(3, 20, 4, 10, False)
+    st, _, _ = run(x, y, raw, tot, trig, cut, table, 0, hint=512)      # 2100-event shots, 2048-event windows
+    assert st["error"] == tpx3.ERR_NOT_CONTIGUOUS
+
+
 def test_preprocess_rejects_a_cut_beyond_int64(tpx3):
     import torch
 
