@@ -51,6 +51,8 @@
 // of flight too wide for one 32-bit key) marks the call as failed; the general kernels, enqueued from the device
 // behind this one (k_fallback_dispatch), then redo the call.
 #pragma once
+#include <type_traits>
+
 #include "tpx3_common.cuh"
 #include "tpx3_localmax.cuh"
 #include "tpx3_preprocess.cuh"
@@ -931,23 +933,22 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         *reinterpret_cast<uint4*>(wpre + p0) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
       }
       __syncthreads();
-      uint32_t dk_r[IPT];   // dense key | arrival slot inside (key, position block) << 16
       // Counter fields: first eight 4-bit counts per key (position blocks of THREADS events). If one of them
       // overflows — 16 events of one key inside one position block: electron VMI, where a shot's few hundred
       // events share 95 ticks — the step is redone with four 8-bit counts (blocks of 2 * THREADS events); the
       // members of one field are then ordered by the count of smaller positions, whatever their number.
-      auto fsum = [](uint32_t w, uint32_t cb) -> uint32_t {            // sum of the fields of a counter word
-        if (cb == 4u) {
-          w = (w & 0x0F0F0F0Fu) + ((w >> 4) & 0x0F0F0F0Fu);
-          return (w * 0x01010101u) >> 24;
-        }
-        return (w & 0xFFu) + ((w >> 8) & 0xFFu) + ((w >> 16) & 0xFFu) + (w >> 24);
-      };
-      bool big = false;
-      uint32_t cb = 4u;
-      for (;;) {
-        const uint32_t fmask = (1u << cb) - 1u;
-        big = false;
+      // (Two instantiations of one generic lambda: the field width is a compile-time constant in both.)
+      auto rank_by_fields = [&](auto cb_tag) -> bool {              // false: a field overflowed, nothing usable written
+        constexpr uint32_t cb = decltype(cb_tag)::value, fmask = (1u << cb) - 1u;
+        auto fsum = [](uint32_t w) -> uint32_t {                    // sum of the fields of a counter word
+          if (cb == 4u) {
+            w = (w & 0x0F0F0F0Fu) + ((w >> 4) & 0x0F0F0F0Fu);
+            return (w * 0x01010101u) >> 24;
+          }
+          return (w & 0xFFu) + ((w >> 8) & 0xFFu) + ((w >> 16) & 0xFFu) + (w >> 24);
+        };
+        uint32_t dk_r[IPT];   // dense key | arrival slot inside (key, position block) << 16
+        bool big = false;
 #pragma unroll
         for (int j = 0; j < IPT; ++j) {
           dk_r[j] = kNone;
@@ -960,20 +961,13 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
             dk_r[j] = dk | (r << 16);
           }
         }
-        big = __syncthreads_or(big ? 1 : 0) != 0;
-        if (!big || cb == 8u) break;
-        for (uint32_t i = tid; i < (uint32_t)T; i += THREADS) gcnt[i] = 0u;     // again, with wider fields
-        cb = 8u;
-        __syncthreads();
-      }
-      if (!big) {
-        const uint32_t fmask = (1u << cb) - 1u;
+        if (__syncthreads_or(big ? 1 : 0)) return false;
         {   // offsets: exclusive scan of the group sizes, 8 consecutive dense keys per thread (at most mm <= T keys)
           const uint4 q0 = *reinterpret_cast<const uint4*>(gcnt + p0), q1 = *reinterpret_cast<const uint4*>(gcnt + p0 + 4);
           const uint32_t qw[IPT] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w};
           uint32_t c[IPT], sum = 0;
 #pragma unroll
-          for (int j = 0; j < IPT; ++j) { c[j] = fsum(qw[j], cb); sum += c[j]; }
+          for (int j = 0; j < IPT; ++j) { c[j] = fsum(qw[j]); sum += c[j]; }
           uint32_t inc = sum;
 #pragma unroll
           for (int o = 1; o < 32; o <<= 1) {
@@ -1003,7 +997,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
             const uint32_t w = gcnt[dk];
             const uint32_t sh = cb == 4u ? 4u * (uint32_t)j : 8u * ((uint32_t)j >> 1);
             // the group's members of earlier position blocks come first
-            const uint32_t b0 = (uint32_t)gbase[dk] + fsum(w & ((1u << sh) - 1u), cb), m = (w >> sh) & fmask;
+            const uint32_t b0 = (uint32_t)gbase[dk] + fsum(w & ((1u << sh) - 1u)), m = (w >> sh) & fmask;
             b0_r[j] = b0 | (m << 16);
             if (m == 1u) buf1[b0] = (uint16_t)k;      // alone with its key in its position block: final position
             else buf0[b0 + r] = (uint16_t)k;          // the sub-group's members in arrival order
@@ -1020,10 +1014,16 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
             buf1[b0 + c] = (uint16_t)k;
           }
         }
-        fin = buf1;
-      } else {
-        counted = false;      // 256 events of one key in one position block: the LSD sort below
+        return true;
+      };
+      bool ranked = rank_by_fields(std::integral_constant<uint32_t, 4u>{});
+      if (!ranked) {
+        for (uint32_t i = tid; i < (uint32_t)T; i += THREADS) gcnt[i] = 0u;     // again, with wider fields
+        __syncthreads();
+        ranked = rank_by_fields(std::integral_constant<uint32_t, 8u>{});
       }
+      if (ranked) fin = buf1;
+      else counted = false;      // 256 events of one key in one position block: the LSD sort below
       __syncthreads();
     }
     if (!counted) {

@@ -539,6 +539,38 @@ def test_small_tile_variant_with_in_tile_sort(tpx3):
     assert np.any(res["perm"] != np.arange(w.n))
 
 
+@pytest.mark.parametrize("hint", [600, 2000, 4000])
+def test_in_tile_order_with_many_events_per_key(tpx3, hint):
+    """Electron VMI delivered out of order inside each shot: a shot's 360 events share 95 ticks, so up to 20 events
+    of one (shot, ToF) key fall into one position block and the rank by counting needs its 8-bit counter fields."""
+    w = gen.generate(1, shots=800)
+    rng = np.random.default_rng(5)
+    p = np.arange(w.n)
+    off = w.shot_offsets
+    for s in range(w.shots):
+        a, b = int(off[s]), int(off[s + 1])
+        p[a:b] = a + rng.permutation(b - a)
+    res, _ = check(tpx3, w.x[p], w.y[p], w.toa[p], w.tot[p], modes=("fused", "split"), max_shot_hits=hint,
+                   what="cfg1 shuffled, hint %d" % hint)
+    assert res["status"]["path"] == 1
+    assert np.any(res["perm"] != np.arange(w.n))
+
+
+def test_in_tile_order_falls_back_to_the_radix_sort(tpx3):
+    """Hundreds of events with ONE key inside one position block overflow even the 8-bit counter fields: the stable
+    LSD radix sort of the tile takes over. Two time values per shot, the later one delivered first."""
+    rng = np.random.default_rng(8)
+    shots, per = 12, 1400
+    n = shots * per
+    x = rng.integers(0, 256, n); y = rng.integers(0, 256, n)
+    tof = np.tile(np.concatenate([np.full(per // 2, 900), np.full(per - per // 2, 100)]), shots)
+    toa = (np.repeat(np.arange(shots), per) * P + tof).astype(np.uint64)
+    tot = rng.integers(1, 1024, n)
+    for hint in (1500, 3000):
+        res, _ = check(tpx3, x, y, toa, tot, modes=("fused",), max_shot_hits=hint, what="two keys per shot, hint %d" % hint)
+        assert res["status"]["path"] == 1
+
+
 # ------------------------------------------------------------------ paper-literal mode (NEXT #2)
 LM_KEYS = ("c_label", "c_size", "c_shot", "c_sum_tot", "c_sum_tot_x", "c_sum_tot_y", "c_toa_peak", "c_sum_tot_tof",
            "c_cx", "c_cy", "c_ctof")
