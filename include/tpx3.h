@@ -112,7 +112,8 @@ typedef struct {
 int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace_bytes);
 
 /* S0-S3. x, y, tot: uint16[n]; toa: uint64[n] (all [dev], SoA, 14 B/event).
- * Outputs [dev]: perm uint32[n], label uint32[n], n_clusters uint32[1]. n may be 0. */
+ * Outputs [dev]: perm uint32[n], label uint32[n], n_clusters uint32[1]. n may be 0. Runs where
+ * tpx3_cluster_centroid runs (same kernel, stopped after the labels; same decision on the device). */
 int tpx3_cluster(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64_t n,
                  const uint16_t* x, const uint16_t* y, const uint64_t* toa, const uint16_t* tot,
                  uint32_t* perm, uint32_t* label, uint32_t* n_clusters);
@@ -120,7 +121,10 @@ int tpx3_cluster(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64_t 
 /* S4-S5 for ANY (perm, label) satisfying the post-conditions of tpx3_cluster (perm a
  * permutation; label[k] <= k; label[label[k]] == label[k]). Writes min(n_clusters,
  * max_clusters) entries of `out` and the true count to n_clusters [dev]; if the count exceeds
- * max_clusters the status word records TPX3_ERR_CAPACITY. */
+ * max_clusters the status word records TPX3_ERR_CAPACITY. (perm, label) whose hits each lie inside
+ * one shot of a shot-contiguous order - what tpx3_cluster writes - are served by the tile kernel
+ * (events read through perm, in the given order: "sorted position" in the tie rule means position in
+ * perm); anything else by the general sums. Same results. */
 int tpx3_centroid(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64_t n,
                   const uint16_t* x, const uint16_t* y, const uint64_t* toa, const uint16_t* tot,
                   const uint32_t* perm, const uint32_t* label, uint64_t max_clusters,
@@ -129,8 +133,10 @@ int tpx3_centroid(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64_t
 /* S0-S5 in one call (same results as tpx3_cluster followed by tpx3_centroid). When the input
  * is shot-contiguous (shot = ToA div P never decreases along the stream, as in a TimePix3
  * readout where disorder is confined to one readout window) and every shot fits one
- * shared-memory tile, the whole path runs as ONE fused kernel; otherwise the general kernels
- * run. The decision is taken on the device; tpx3_status reports which path ran. */
+ * shared-memory tile, the whole path runs as ONE fused kernel; otherwise the general route
+ * runs: a global radix sort by ToA, then the same tile kernel on the sorted stream, and only
+ * for a shot longer than a tile (or a plan without a shot period) the slab-hash linking and
+ * atomic sums. The decision is taken on the device; tpx3_status reports path 1 or 2. */
 int tpx3_cluster_centroid(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64_t n,
                           const uint16_t* x, const uint16_t* y, const uint64_t* toa,
                           const uint16_t* tot, uint32_t* perm, uint32_t* label,
