@@ -365,7 +365,7 @@ def run_ours(args):
         stream.synchronize()
         return k
 
-    e2e_s = None
+    e2e_s = e2e_full_s = route_e2e = None
     if not args.no_e2e:
         for _ in range(2):
             e2e_step()
@@ -381,6 +381,19 @@ def run_ours(args):
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             e2e_s = float(t.item())
         assert ncl_e2e == ncl, (ncl_e2e, ncl)
+        route_e2e = pl.host_route()
+        # the same call asking for perm and label as well (8 B/hit more on the way back; runs in one piece)
+        e2e_full_s = None
+        if not lm and world == 1:
+            hperm = torch.empty(max(n, 1), dtype=torch.uint32).pin_memory()
+            hlabel = torch.empty(max(n, 1), dtype=torch.uint32).pin_memory()
+            pl.process_host(*host, clh, hperm, hlabel, stream=stream)
+            t0 = time.perf_counter()
+            for _ in range(2):
+                pl.process_host(*host, clh, hperm, hlabel, stream=stream)
+            torch.cuda.synchronize()
+            e2e_full_s = (time.perf_counter() - t0) / 2
+            del hperm, hlabel
     if rank == 0:
         sampler.stop()
     if rank != 0:
@@ -449,7 +462,9 @@ def run_ours(args):
         },
         "particle_hits_per_s": ncl_all / (ms_step * 1e-3),
         "e2e": None if e2e_s is None else {"value": n_all / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "ms_per_step": e2e_s * 1e3, "route": {0: "one piece", 1: "pipelined in 2^22-event chunks", 2: "pipelined attempt redone in one piece"}.get(pl.host_route()) if not lm else None, "api": "tpx3_process_host (pinned host buffers; cluster table copied "
+                "ms_per_step": e2e_s * 1e3, "route": {0: "one piece", 1: "pipelined in 2^22-event chunks", 2: "pipelined attempt redone in one piece"}.get(route_e2e) if not lm else None,
+                "with_perm_label": None if e2e_full_s is None else {"value": n_all / e2e_full_s, "ms_per_step": e2e_full_s * 1e3,
+                                                                   "d2h_bytes_per_step": d2h + 8 * n, "route": "one piece"}, "api": "tpx3_process_host (pinned host buffers; cluster table copied "
                 "back, perm/label left on the device)" if not lm else "pinned H2D copies + tpx3_localmax_centroid + "
                 "D2H of the count and the hit table"},
         "gpu_launches": launches,

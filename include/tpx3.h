@@ -200,10 +200,11 @@ int tpx3_preprocess(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64
  * = INPUT position (into x, y, toa, tot) of the surviving event at sorted position k (the two-call route gives
  * index_out[perm[k]]); label uint32[n] (first n_kept entries), indexed by sorted position among the surviving
  * events; `out` / n_clusters as tpx3_cluster_centroid, with toa_peak and shot in the REBASED time
- * ((shot_base + s) * P + ToF'). Serves shot-contiguous raw streams (the trigger index never decreases along the
- * stream) whose shots fit the plan's window (max_shot_hits, counted on the raw stream, must be given); anything
- * else is detected on the device and reported as TPX3_ERR_NOT_CONTIGUOUS by tpx3_status — nothing valid has been
- * written then. The plan's shot period must be > 0 and <= 2^24. Enqueue only. */
+ * ((shot_base + s) * P + ToF'). Serves shot-contiguous raw streams (the trigger index never decreases along
+ * the stream; an event before the first trigger counts to trigger 0 for this purpose) whose shots fit the
+ * plan's window (max_shot_hits, counted on the raw stream, must be given); anything else is detected on the
+ * device and reported as TPX3_ERR_NOT_CONTIGUOUS by tpx3_status - nothing valid has been written then. The
+ * plan's shot period must be > 0 and <= 2^24. Enqueue only. */
 int tpx3_preprocess_cluster_centroid(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64_t n,
                                      const uint16_t* x, const uint16_t* y, const uint64_t* toa,
                                      const uint16_t* tot, uint64_t n_trig, const uint64_t* trig, uint64_t cut,
