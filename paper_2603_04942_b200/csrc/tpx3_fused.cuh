@@ -334,18 +334,18 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 
   // ---- the CTA walks its segment tile by tile ---------------------------------------------------------
   const uint32_t seg = blockIdx.x;
-  uint64_t n_ev = a.n;
+  uint32_t n_ev = (uint32_t)a.n;     // positions fit 32 bits: a plan takes at most 2^28 events
   uint32_t seg_G = a.G, seg_n = a.nseg, seg_maxt = a.maxt;
   if (a.n_dev) {                     // a stream push: the count was decided on the device
     n_ev = *a.n_dev;
-    const FusedSegs sg = fused_segs(n_ev, (uint32_t)T, a.num_sms);
+    const FusedSegs sg = fused_segs((uint64_t)n_ev, (uint32_t)T, a.num_sms);
     seg_G = sg.G; seg_n = sg.nseg; seg_maxt = sg.maxt;
     if (seg >= seg_n) return;        // the grid was sized for the largest count
   }
-  const uint64_t seg_begin = (uint64_t)seg * seg_G;
-  const uint64_t seg_end = seg_begin + seg_G < n_ev ? seg_begin + seg_G : n_ev;
+  const uint32_t seg_begin = seg * seg_G;
+  const uint32_t seg_end = seg_begin + seg_G < n_ev ? seg_begin + seg_G : n_ev;
   const uint32_t P32 = (uint32_t)a.P;
-  uint64_t tile_at = seg_begin;     // where the next tile starts; a shot start except for the segment's first tile
+  uint32_t tile_at = seg_begin;     // where the next tile starts; a shot start except for the segment's first tile
   uint32_t kept_run = kPre ? a.seg_kept[seg] : 0u;   // mode 4: surviving events in front of tile_at
   uint64_t pre_next_s = 0;          // mode 4: trigger index of the event at tile_at, when the previous tile saw it
   bool pre_have_s = false;
@@ -364,21 +364,21 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    bulk_have = n_ev - (tile_at & ~7ull) >= (uint64_t)T;
+    bulk_have = n_ev - (tile_at & ~7u) >= (uint32_t)T;
     if (bulk_have && tid == 0) {
       mbar_expect_tx(bulk_bar, 8u * T);
-      bulk_g2s(toa_s, a.toa + (tile_at & ~7ull), 8u * T, bulk_bar);
+      bulk_g2s(toa_s, a.toa + (tile_at & ~7u), 8u * T, bulk_bar);
     }
   }
 #endif
   for (;;) {
   // the next window's ToA is requested BEFORE the barrier that ends the previous tile: the loads touch no shared
   // memory, so the DRAM round trip runs under the wait for the previous tile's slowest warp
-  const uint64_t base = tile_at & ~7ull;               // window start: aligned for the 128-bit loads
-  const uint32_t skp = (uint32_t)(tile_at - base);     // window positions below skp belong to the previous tile
-  const uint64_t avail = n_ev - base;                  // > 0 by construction
-  const uint32_t cnt = avail < (uint64_t)T ? (uint32_t)avail : (uint32_t)T;  // events readable
-  const uint32_t e_rel = seg_end - base > (uint64_t)T ? kNone : (uint32_t)(seg_end - base);   // segment end in the window
+  const uint32_t base = tile_at & ~7u;                 // window start: aligned for the 128-bit loads
+  const uint32_t skp = tile_at - base;                 // window positions below skp belong to the previous tile
+  const uint32_t avail = n_ev - base;                  // > 0 by construction
+  const uint32_t cnt = avail < (uint32_t)T ? avail : (uint32_t)T;  // events readable
+  const uint32_t e_rel = seg_end - base > (uint32_t)T ? kNone : seg_end - base;   // segment end in the window
   const uint32_t p0 = tid * IPT;                       // this thread's 8 window positions
 
   // ---- load ToA (2 events per 128-bit load) ----------------------------------------------------
@@ -646,7 +646,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   // window. The end of the stream counts as a shot start.
   uint32_t lo = misc->lo, hi;
   bool failed = misc->fail != 0;
-  uint64_t next_at;               // where the next tile of this segment starts (>= seg_end: none)
+  uint32_t next_at;               // where the next tile of this segment starts (>= seg_end: none)
   {
     const bool to_end = base + cnt >= n_ev;
     const uint32_t last = to_end ? cnt : misc->last;          // misc->last >= lo whenever lo exists
@@ -668,11 +668,11 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   }
 #ifdef TPX3_BULK_TOA
   if (kBulkOn) {  // every thread has its ToA in registers (two barriers ago): the buffer may take the next window
-    bulk_have = !failed && next_at < seg_end && n_ev - (next_at & ~7ull) >= (uint64_t)T;
+    bulk_have = !failed && next_at < seg_end && n_ev - (next_at & ~7u) >= (uint32_t)T;
     if (bulk_have && tid == 0) {
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       mbar_expect_tx(bulk_bar, 8u * T);
-      bulk_g2s(toa_s, a.toa + (next_at & ~7ull), 8u * T, bulk_bar);
+      bulk_g2s(toa_s, a.toa + (next_at & ~7u), 8u * T, bulk_bar);
     }
   }
 #endif
@@ -684,7 +684,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   const uint32_t mm_raw = failed ? 0u : hi - lo;   // owned events of the window; a failed tile owns nothing
   uint32_t mm = mm_raw;                            // owned events that are clustered (mode 4: those that survive)
   const uint32_t tmask = tb >= 32u ? 0xFFFFFFFFu : ((1u << tb) - 1u);
-  const uint32_t raw_base = (uint32_t)(base + lo);  // input position of the window's first owned event (n <= 2^28)
+  const uint32_t raw_base = base + lo;              // input position of the window's first owned event (n <= 2^28)
   uint32_t out_base = raw_base;                     // global sorted position of local rank 0
   if constexpr (kPre) {
     // surviving events of the owned range and of what this window skips in front of it (counted into kept_run)
@@ -703,7 +703,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
       if (c_pre) atomicAdd(&misc->kept_pre, c_pre);
     }
     // the trigger of the event the next tile starts at (read at the end of this tile)
-    const uint64_t nrel = next_at - base;
+    const uint32_t nrel = next_at - base;
     if (nrel >= p0 && nrel < p0 + IPT && nrel < cnt && nrel >= skp) misc->s_next = sl[nrel - p0];
   }
 
