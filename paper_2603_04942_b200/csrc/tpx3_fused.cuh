@@ -1110,11 +1110,41 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     fin = (npass & 1u) ? buf1 : buf0;
     }
     }   // not compacted
-    // gather the records into sorted order (region A) and emit perm
-    for (uint32_t k = tid; k < mm; k += THREADS) {
-      const uint32_t s = fin[k];
-      recA[k] = recB[lo + s];
-      a.perm[out_base + k] = raw_base + s;
+    // gather the records into sorted order (region A) and emit perm. The sorted keys pass through the registers of
+    // consecutive lanes here, so the time-cluster check ("are the time clusters of the tile tight?", below) rides
+    // along: per block of 32 sorted positions the largest cluster-start key and the key of the last event in front
+    // of the block's first start go to the (still free) list region, and are stitched together after the barrier.
+    // (Reading the keys again afterwards, 8 consecutive records per thread, was a 16-way bank conflict: 7 % of the
+    // kernel's shared-memory wavefronts on config 4.)
+    uint32_t* cl_blk = reinterpret_cast<uint32_t*>(smem + L::kList);      // [T / 32][2]
+    bool cl_loose2 = false;
+    for (uint32_t k0 = warp * 32u; k0 < mm; k0 += THREADS) {               // warp-uniform trip count
+      const uint32_t k = k0 + lane;
+      const bool valid = k < mm;
+      uint2 rec = make_uint2(0xFFFFFFFFu, 0u);
+      if (valid) {
+        const uint32_t s = fin[k];
+        rec = recB[lo + s];
+        recA[k] = rec;
+        a.perm[out_base + k] = raw_base + s;
+      }
+      if (cl_scan) {
+        const uint32_t key = rec.x;
+        uint32_t prev = __shfl_up_sync(0xffffffffu, key, 1);
+        if (lane == 0) prev = k0 ? recB[lo + fin[k0 - 1u]].x : 0u;
+        const bool st = valid && (k == 0u || key - prev > a.W);
+        uint32_t ps = st ? key : 0u;                                       // prefix maximum of the start keys (0: none)
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const uint32_t t = __shfl_up_sync(0xffffffffu, ps, o);
+          if (lane >= (uint32_t)o) ps = max(ps, t);
+        }
+        // a start at key 0 looks like "none": its followers are then checked against the carry, which is 0 too
+        const bool lead = valid && ps == 0u;
+        if (valid && ps != 0u && key - ps > a.W) cl_loose2 = true;
+        const uint32_t lead_last = __reduce_max_sync(0xffffffffu, lead ? key + 1u : 0u);   // + 1: 0 = no lead event
+        if (lane == 31) { cl_blk[2u * (k0 >> 5)] = ps; cl_blk[2u * (k0 >> 5) + 1u] = lead_last; }
+      }
     }
     __syncthreads();
     // the hash table now takes X + B: clear it
@@ -1122,6 +1152,15 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
     for (int q = 0; q < 16 * T / 16 / THREADS; ++q) z[q * THREADS + tid] = zero;
+    if (cl_scan) {
+      const uint32_t nb = (mm + 31u) >> 5;
+      if (tid < nb && cl_blk[2u * tid + 1u]) {          // block tid begins inside a cluster that started before it
+        uint32_t carry = 0;
+        for (uint32_t b2 = 0; b2 < tid; ++b2) carry = max(carry, cl_blk[2u * b2]);
+        if (cl_blk[2u * tid + 1u] - 1u - carry > a.W) cl_loose2 = true;
+      }
+      if (cl_loose2) misc->loose = 1u;
+    }
     __syncthreads();
   } else {
     if (!kPerm)
@@ -1283,36 +1322,6 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   // cluster-start key of the warps before it (the keys ascend, so a prefix maximum).
   // (Nothing to check when all times of flight of the tile lie within W: electron VMI. Tiles that arrived in
   // order did this on the keys in registers while building their records; see there.)
-  if (unsorted && cl_scan) {
-    // thread t owns the sorted positions [8t, 8t + 8)
-    const uint32_t q0 = tid * (uint32_t)IPT;
-    uint32_t last_start = 0, lead_last = 0, cur = 0, prev = (q0 > 0u && q0 < mm) ? recS[q0 - 1u].x : 0u;
-    bool have_cur = false, have_lead = false, loose = false;
-#pragma unroll
-    for (int j = 0; j < IPT; ++j) {
-      const uint32_t k = q0 + (uint32_t)j;
-      if (k < mm) {
-        const uint32_t key = recS[k].x;
-        if (k == 0u || key - prev > a.W) { cur = key; have_cur = true; last_start = key; }
-        else if (have_cur) { if (key - cur > a.W) loose = true; }
-        else { lead_last = key; have_lead = true; }
-        prev = key;
-      }
-    }
-    uint32_t inc = last_start;   // 0 = "no start here" is the identity of max on keys
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= (uint32_t)o) inc = max(inc, t);
-    }
-    if (lane == 31) misc->warp_sums[warp] = inc;
-    uint32_t carry = __shfl_up_sync(0xffffffffu, inc, 1);
-    if (lane == 0) carry = 0;
-    __syncthreads();
-    for (uint32_t w = 0; w < warp; ++w) carry = max(carry, misc->warp_sums[w]);
-    if (have_lead && lead_last - carry > a.W) loose = true;   // position 0 starts a cluster, so a carry exists
-    if (loose) misc->loose = 1u;
-  }
   // ---- hash insert ----------------------------------------------------------------------------------
   hash_insert();
   __syncthreads();
