@@ -1977,6 +1977,7 @@ inline int enqueue_fused(const FusedGeom& g, uint32_t num_sms, uint64_t* launche
   ++*launches;
   uint32_t ctas, tiles_per_cta;
   compact_grid(a.num_tiles, num_sms, &ctas, &tiles_per_cta);
+  if (n_dev) ctas = num_sms * 8u;   // the kernel sizes itself from the device's count: the most compact_grid ever asks for
   k_fused_compact<<<ctas, kCompactThreads, 0, st>>>(a, tiles_per_cta, g.T);
   if (cudaGetLastError() != cudaSuccess) return TPX3_ERR_CUDA;
   ++*launches;
