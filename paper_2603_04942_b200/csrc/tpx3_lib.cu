@@ -494,6 +494,7 @@ static int run_fused_or_general(tpx3_plan_t p, void* workspace, void* cuda_strea
     FusedArgs fa = make_fused_args(2048u, (uint32_t)p->num_sms, w.ctrl, w.tiles, prm, x, y, toa, tot, perm, label,
                                    max_clusters, out ? *out : none, n_clusters, (char*)workspace + p->off_keyA, mode, 0u,
                                    0u, n_dev);
+    fa.label_base = label_base;
     k_fallback_dispatch<<<1, 1, 0, st>>>(ga, fa, FusedLadder{0, {0, 0}}, 0, (int)mode);
     ++p->launches;
     return cuda_ok(cudaGetLastError());

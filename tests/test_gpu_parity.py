@@ -914,14 +914,14 @@ def _disorder(toa):
     return int(np.max(np.maximum.accumulate(t) - t)) if len(t) else 0
 
 
-def run_stream(m, w, sizes, D, max_carry, max_shot_hits=0, cap=None, final_empty=False):
+def run_stream(m, w, sizes, D, max_carry, max_shot_hits=0, cap=None, final_empty=False, flags=0):
     """Push w in chunks of the given sizes through tpx3_stream_push; returns the concatenated hit rows,
     the per-push info and the StreamModel's per-push (n_emitted, n_carry, n_late) for the same chunks."""
     import torch
 
     max_chunk = max(max(sizes), 1)
     pl = m.plan(m.Config(toa_window_ticks=W, shot_period_ticks=P, max_hits=max_chunk + max_carry,
-                         max_shot_hits=max_shot_hits))
+                         max_shot_hits=max_shot_hits, flags=flags))
     s = pl.stream_open(max_chunk, max_carry, D)
     cl = m.Clusters(cap or (max_chunk + max_carry), pl.device)
     dx, dy, dt, do = to_dev(w.x), to_dev(w.y), to_dev(w.toa), to_dev(w.tot)
@@ -1013,6 +1013,58 @@ def test_stream_equals_batch(tpx3, cfg, shots, chunk):
     assert infos[-1]["late_total"] == 0 and infos[-1]["n_carry"] == 0
     if chunk < w.n:
         assert max(i["n_carry"] for i in infos) > 0       # the cuts were not shot-aligned
+
+
+@pytest.mark.parametrize("cfg,shots,chunk,hint", [(1, 60, 7001, 600), (4, 200, 50021, 1500), (3, 12, 9973, 512)])
+def test_stream_on_the_general_route(tpx3, cfg, shots, chunk, hint):
+    """Stream pushes whose clustering takes the general route, sized and enqueued from the device (the emit count is
+    device state): forced by the plan's flag (global sort, then the tile kernel through perm), and - last case,
+    2100-event shots against 2048-event windows - after the tile kernel gave up."""
+    w = gen.generate(cfg, shots=shots)
+    D = _disorder(w.toa)
+    per_shot = int(np.bincount((w.toa // np.uint64(P)).astype(np.int64) - int(w.toa.min() // P)).max())
+    sizes = _sizes(w.n, chunk)
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P, threads=0)
+    for flags in ((tpx3.FLAG_FORCE_GENERAL, 0) if cfg != 3 else (0,)):
+        rows, infos, _ = run_stream(tpx3, w, sizes, D, max_carry=4 * per_shot + 16, max_shot_hits=hint, flags=flags)
+        for k in _ROW_KEYS:
+            np.testing.assert_array_equal(rows[k], o[k], err_msg="%s flags %d" % (k, flags))
+        _check_push_properties(infos, w.toa, sizes, D)
+
+
+def test_shot_period_beyond_the_tile_key(tpx3):
+    """P > 2^24 ticks: the time of flight does not fit the tile kernel's 32-bit key, the plan has no tile kernel and
+    every call runs the slab-hash kernels: batch call, split calls, and stream pushes (device-sized, labels offset)."""
+    import torch
+
+    P2 = (1 << 25) + 12345
+    w = gen.generate(0, shots=400)
+    shot = (w.toa // np.uint64(P)).astype(np.uint64)
+    toa = shot * np.uint64(P2) + (w.toa % np.uint64(P)) * np.uint64(37)          # ToF spread over 2.3e6 ticks
+    Wr = 320 * 37
+    o = oracle.run(w.x, w.y, toa, w.tot, Wr, P2, threads=0)
+    res, _ = check(tpx3, w.x, w.y, toa, w.tot, W=Wr, P=P2, modes=("split", "fused"), what="P > 2^24")
+    assert res["status"]["path"] == 2
+    chunk, carry = 5003, 2048
+    pl = tpx3.plan(tpx3.Config(toa_window_ticks=Wr, shot_period_ticks=P2, max_hits=chunk + carry))
+    s = pl.stream_open(chunk, carry, 0)
+    cl = tpx3.Clusters(chunk + carry, pl.device)
+    dev = [to_dev(a) for a in (w.x, w.y, toa, w.tot)]
+    rows = {k: [] for k in _ROW_KEYS}
+    sizes = _sizes(w.n, chunk)
+    i = 0
+    for j, sz in enumerate(sizes):
+        nh, info = s.push(*(d[i:i + sz] for d in dev), cl, final=(j == len(sizes) - 1))
+        i += sz
+        torch.cuda.synchronize()
+        assert pl.status()["error"] == 0
+        got = cl.numpy(int(nh.cpu().numpy()[0]))
+        for k in _ROW_KEYS:
+            rows[k].append(got[k].copy())
+    s.close()
+    pl.free()
+    for k in _ROW_KEYS:
+        np.testing.assert_array_equal(np.concatenate(rows[k]), o[k], err_msg=k)
 
 
 def test_stream_random_chunks_and_empty_pushes(tpx3):
