@@ -49,9 +49,11 @@ typedef enum {
   TPX3_ERR_CAPACITY = -2,      /* max_clusters too small (device-detected; see tpx3_status)     */
   TPX3_ERR_OUT_OF_RANGE = -3,  /* x/y outside the sensor or tot == 0 (under VALIDATE_INPUT)     */
   TPX3_ERR_CUDA = -4,          /* a CUDA runtime call failed                                    */
-  TPX3_ERR_NOT_CONTIGUOUS = -5 /* tpx3_preprocess_cluster_centroid only (device-detected): the stream
+  TPX3_ERR_NOT_CONTIGUOUS = -5,/* tpx3_preprocess_cluster_centroid only (device-detected): the stream
                                   is not shot-contiguous or a shot does not fit the plan's window;
                                   use tpx3_preprocess followed by tpx3_cluster_centroid            */
+  TPX3_ERR_TOO_LARGE = -6      /* tpx3_unwrap_toa_static only: n beyond TPX3_STATIC_UNWRAP_MAX, the
+                                  size its fixed scratch array serves; use tpx3_unwrap_toa          */
 } tpx3_error_t;
 
 enum {
@@ -170,6 +172,23 @@ int tpx3_localmax_centroid(tpx3_plan_t plan, void* workspace, void* cuda_stream,
 int tpx3_unwrap_toa(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64_t n, const uint64_t* raw,
                     uint64_t modulus, uint64_t jump, int64_t wraps_in, int has_prev, uint64_t prev_raw,
                     uint64_t* toa_out, int64_t* wraps_out);
+
+/* The same unwrapping for callers that cannot allocate device memory (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): no plan, no workspace. The scratch the three
+ * kernels share (one 32-bit count per 4096 events) lives in a file-scope `static __device__` array of the
+ * library, 64 KB, which every GPU that loads the library holds until the process exits; it serves
+ * n <= TPX3_STATIC_UNWRAP_MAX events, a larger n returns TPX3_ERR_TOO_LARGE before anything is enqueued.
+ * The call allocates nothing (no cudaMalloc / cudaFree, no allocating library routine): the array's device
+ * address is looked up once per device (cudaGetSymbolAddress, with that device current) and kept.
+ * `device` is the CUDA device ordinal of raw / toa_out / wraps_out and of cuda_stream. Arguments, results
+ * and rounding are those of tpx3_unwrap_toa. ALL calls on a device share the one array: it keeps the last
+ * call's contents (nothing in it has to start at zero: every call overwrites the counts it reads), and
+ * two calls that overlap on the GPU (different streams, no ordering between them) race on it - keep them
+ * on one stream or order them with events. Enqueue only. */
+#define TPX3_STATIC_UNWRAP_MAX (1ull << 26)
+int tpx3_unwrap_toa_static(int device, void* cuda_stream, uint64_t n, const uint64_t* raw, uint64_t modulus,
+                           uint64_t jump, int64_t wraps_in, int has_prev, uint64_t prev_raw, uint64_t* toa_out,
+                           int64_t* wraps_out);
 
 /* Timewalk calibration product (Eq. 1): table_host[ToT] = a / (ToT + b)^d + c for
  * ToT = 0 .. length-1, evaluated in fp64 and rounded to the nearest integer tick (half away from

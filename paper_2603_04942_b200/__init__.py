@@ -17,18 +17,19 @@ from . import _build
 
 __all__ = [
     "Tpx3Error", "Config", "Clusters", "Plan", "Stream", "plan", "load_library", "exported_symbols",
-    "FLAG_VALIDATE_INPUT", "FLAG_FORCE_GENERAL", "strerror", "shard_shots",
+    "FLAG_VALIDATE_INPUT", "FLAG_FORCE_GENERAL", "strerror", "shard_shots", "unwrap_toa_static",
 ]
 
 FLAG_VALIDATE_INPUT = 1 << 0
 FLAG_FORCE_GENERAL = 1 << 1
 
-OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_OUT_OF_RANGE, ERR_CUDA, ERR_NOT_CONTIGUOUS = 0, -1, -2, -3, -4, -5
+OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_OUT_OF_RANGE, ERR_CUDA, ERR_NOT_CONTIGUOUS, ERR_TOO_LARGE = 0, -1, -2, -3, -4, -5, -6
+STATIC_UNWRAP_MAX = 1 << 26   # tpx3.h: TPX3_STATIC_UNWRAP_MAX
 
 # Every symbol include/tpx3.h declares (tests check the built library exports all of them).
 exported_symbols = (
     "tpx3_plan", "tpx3_cluster", "tpx3_centroid", "tpx3_cluster_centroid", "tpx3_localmax_centroid",
-    "tpx3_unwrap_toa", "tpx3_timewalk_table", "tpx3_preprocess", "tpx3_preprocess_cluster_centroid", "tpx3_host_io_bytes",
+    "tpx3_unwrap_toa", "tpx3_unwrap_toa_static", "tpx3_timewalk_table", "tpx3_preprocess", "tpx3_preprocess_cluster_centroid", "tpx3_host_io_bytes",
     "tpx3_stream_bytes", "tpx3_stream_open", "tpx3_stream_push", "tpx3_stream_close",
     "tpx3_process_host", "tpx3_host_route", "tpx3_status", "tpx3_launch_count", "tpx3_profile_enable", "tpx3_profile_read",
     "tpx3_free", "tpx3_strerror",
@@ -96,6 +97,8 @@ def load_library(build: bool = True) -> ctypes.CDLL:
                                            ctypes.c_uint32, vp, vp, u64, ctypes.POINTER(_CClusters), u32p]
     lib.tpx3_unwrap_toa.restype = ctypes.c_int
     lib.tpx3_unwrap_toa.argtypes = [vp, vp, vp, u64, vp, u64, u64, ctypes.c_int64, ctypes.c_int, u64, vp, vp]
+    lib.tpx3_unwrap_toa_static.restype = ctypes.c_int
+    lib.tpx3_unwrap_toa_static.argtypes = [ctypes.c_int, vp, u64, vp, u64, u64, ctypes.c_int64, ctypes.c_int, u64, vp, vp]
     lib.tpx3_timewalk_table.restype = ctypes.c_int
     lib.tpx3_timewalk_table.argtypes = [ctypes.c_double] * 4 + [ctypes.c_uint32, vp]
     lib.tpx3_preprocess_cluster_centroid.restype = ctypes.c_int
@@ -145,6 +148,27 @@ def timewalk_table(a: float, b: float, c: float, d: float, length: int):
     if rc != OK:
         raise Tpx3Error(rc, "tpx3_timewalk_table")
     return out
+
+
+def unwrap_toa_static(raw, modulus: int, jump: int, out, wraps_out, wraps_in: int = 0, prev_raw=None, stream=None):
+    """tpx3_unwrap_toa_static: ToA unwrapping without a plan or workspace and without any device allocation (the
+    scratch is a fixed array inside the library; n <= STATIC_UNWRAP_MAX). The caller passes every tensor, outputs
+    included; calls that overlap on the GPU race on the shared scratch. Argument marshalling only."""
+    import torch
+
+    n = int(raw.numel())
+    _check_dev(raw, torch.uint64, n, "raw")
+    _check_dev(out, torch.uint64, n, "out")
+    _check_dev(wraps_out, torch.int64, 1, "wraps_out")
+    dev = raw.device
+    rc = load_library().tpx3_unwrap_toa_static(dev.index if dev.index is not None else torch.cuda.current_device(),
+                                               _stream_ptr(stream, dev), n, raw.data_ptr(), int(modulus), int(jump),
+                                               int(wraps_in), 0 if prev_raw is None else 1,
+                                               0 if prev_raw is None else int(prev_raw), out.data_ptr(),
+                                               wraps_out.data_ptr())
+    if rc != OK:
+        raise Tpx3Error(rc, "tpx3_unwrap_toa_static")
+    return out, wraps_out
 
 
 def strerror(code: int) -> str:

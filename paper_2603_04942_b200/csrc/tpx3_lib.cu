@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -676,6 +677,48 @@ int tpx3_unwrap_toa(tpx3_plan_t p, void* workspace, void* cuda_stream, uint64_t 
   return cuda_ok(cudaGetLastError());
 }
 
+// ---- tpx3_unwrap_toa without any allocation: scratch in a file-scope device array (tpx3.h) ---------------------
+// One 32-bit block count per kUnwrapTile events, for n <= TPX3_STATIC_UNWRAP_MAX. In host code the NAME of the
+// array is a host-side stand-in, not a device address: the kernels get the address cudaGetSymbolAddress returns,
+// looked up once per device with that device current.
+namespace {
+constexpr uint32_t kStaticUnwrapBlocks = (uint32_t)(TPX3_STATIC_UNWRAP_MAX / kUnwrapTile);   // 16384 counts = 64 KB
+static __device__ __align__(256) uint32_t g_static_unwrap_blk[kStaticUnwrapBlocks];
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mutex;
+uint32_t* g_static_unwrap_ptr[kStaticMaxDevices];   // device address of the array on device d (null: not looked up yet)
+}  // namespace
+
+int tpx3_unwrap_toa_static(int device, void* cuda_stream, uint64_t n, const uint64_t* raw, uint64_t modulus,
+                           uint64_t jump, int64_t wraps_in, int has_prev, uint64_t prev_raw, uint64_t* toa_out,
+                           int64_t* wraps_out) {
+  if (device < 0 || device >= kStaticMaxDevices || !wraps_out || modulus == 0) return TPX3_ERR_INVALID_ARG;
+  if (n > TPX3_STATIC_UNWRAP_MAX) return TPX3_ERR_TOO_LARGE;
+  if (n && (!raw || !toa_out)) return TPX3_ERR_INVALID_ARG;
+  if (cudaSetDevice(device) != cudaSuccess) return TPX3_ERR_CUDA;
+  uint32_t* blk = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_unwrap_ptr[device]) {
+      void* ptr = nullptr;
+      if (cudaGetSymbolAddress(&ptr, g_static_unwrap_blk) != cudaSuccess || !ptr) return TPX3_ERR_CUDA;
+      g_static_unwrap_ptr[device] = (uint32_t*)ptr;
+    }
+    blk = g_static_unwrap_ptr[device];
+  }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  UnwrapArgs a;
+  a.n = n; a.raw = raw; a.modulus = modulus; a.jump = jump; a.wraps_in = (long long)wraps_in;
+  a.has_prev = has_prev; a.prev_raw = prev_raw; a.out = toa_out; a.wraps_out = (long long*)wraps_out;
+  a.blk = blk;
+  a.nblk = (uint32_t)((n + kUnwrapTile - 1) / kUnwrapTile);     // <= kStaticUnwrapBlocks
+  // every count the scan and the apply kernel read is written by the count kernel of THIS call: nothing to clear
+  if (a.nblk) k_unwrap_count<<<a.nblk, kUnwrapThreads, 0, st>>>(a);
+  k_unwrap_scan<<<1, 1024, 0, st>>>(a);
+  if (a.nblk) k_unwrap_apply<<<a.nblk, kUnwrapThreads, 0, st>>>(a);
+  return cuda_ok(cudaGetLastError());
+}
+
 int tpx3_timewalk_table(double a, double b, double c, double d, uint32_t length, int32_t* table_host) {
   if (!table_host && length) return TPX3_ERR_INVALID_ARG;
   for (uint32_t tot = 0; tot < length; ++tot) {
@@ -1102,6 +1145,7 @@ const char* tpx3_strerror(int err) {
     case TPX3_ERR_CAPACITY: return "max_clusters too small";
     case TPX3_ERR_OUT_OF_RANGE: return "event outside the sensor or ToT == 0";
     case TPX3_ERR_CUDA: return "CUDA runtime error";
+    case TPX3_ERR_TOO_LARGE: return "n beyond the fixed scratch of the no-allocation entry point (TPX3_STATIC_UNWRAP_MAX)";
     case TPX3_ERR_NOT_CONTIGUOUS: return "stream not shot-contiguous or a shot longer than the window (fused preprocessing call)";
     default: return "unknown error";
   }
