@@ -351,6 +351,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   bool pre_have_s = false;
   bool at_start = seg == 0;         // tile_at is known to be a shot start
   uint32_t tile_i = 0;              // status words written so far
+  uint32_t seg_hits_run = 0;        // hits of the segment's tiles so far
   bool seg_failed = false;
 #ifdef TPX3_BULK_TOA
   uint64_t* toa_s = reinterpret_cast<uint64_t*>(smem + L::kBulk);
@@ -1669,6 +1670,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   if (mm) {
     if (tid == 0) a.tiles[(uint64_t)seg * seg_maxt + tile_i] = ((unsigned long long)out_base << 32) | (unsigned long long)n_roots;
     ++tile_i;
+    seg_hits_run += n_roots;
   }
   if (failed) { seg_failed = true; break; }
   at_start = misc->lo != kNone;     // everything but "no shot start in sight" ends at a shot start
@@ -1683,6 +1685,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   // ---- completion: the last segment to finish publishes the outcome of the call -------------------
   if (tid == 0) {
     for (uint32_t i = tile_i; i < seg_maxt; ++i) a.tiles[(uint64_t)seg * seg_maxt + i] = 0ull;
+    // the segment's hit total, behind the status words: k_fused_compact sums these, not every tile word, for its prefix
+    reinterpret_cast<uint32_t*>(a.tiles + a.num_tiles)[seg] = seg_hits_run;
     if (seg_failed) atomicExch(&a.ctrl->fused_fail, 1u);
     if (tile_i) atomicAdd(&a.ctrl->tiles_run, tile_i);
     __threadfence();
@@ -1698,8 +1702,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
 
 // ---- S5 + ordering: staging table -> cluster table -----------------------------------------------
 // Runs behind k_fused_shot_tiles (same stream), so every tile's hit count is final: no tile waits
-// for another one. CTA i takes a contiguous range of tiles, sums the counts of all tiles before
-// its range (the tile words are a few hundred KB and L2-resident) and copies its tiles' hits to
+// for another one. CTA i takes a contiguous range of tiles, sums the hits in front of its range
+// (per-segment totals, L2-resident) and copies its tiles' hits to
 // their ordinals, ascending label order. Also computes what needs no tile state: shot = ToA of
 // the brightest pixel div P (the pixel belongs to the hit's shot, R6) and the centroid
 // fp32(sum tot*x) / fp32(sum tot), IEEE RN (Eq. 9).
@@ -1707,9 +1711,12 @@ constexpr int kCompactThreads = 256;
 
 __global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, uint32_t tiles_per_cta, uint32_t T) {
   if (a.ctrl->fused_state != 1u) return;   // the fused kernel gave up: the general path redoes the call
+  const uint32_t* seg_hits = reinterpret_cast<const uint32_t*>(a.tiles + a.num_tiles);   // per-segment hit totals
+  uint32_t maxt = a.maxt;
   if (a.n_dev) {                           // a stream push: the true geometry from the device's count
     const FusedSegs sg = fused_segs((uint64_t)*a.n_dev, T, a.num_sms);
     a.num_tiles = sg.nseg * sg.maxt;
+    maxt = sg.maxt;
     uint32_t ctas;
     compact_grid(a.num_tiles, a.num_sms, &ctas, &tiles_per_cta);
     if (blockIdx.x >= ctas) return;
@@ -1721,7 +1728,11 @@ __global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, 
   const uint32_t t1 = min(t0 + tiles_per_cta, a.num_tiles);
   if (t0 >= a.num_tiles) return;
   unsigned long long sum = 0;
-  for (uint32_t t = tid; t < t0; t += kCompactThreads) sum += a.tiles[t] & 0xFFFFFFFFull;
+  // hits in front of the CTA's range: whole segments by their totals, the rest tile by tile (summing all tile words
+  // here was 1.7 GB of L2 reads over the grid on the 2^28-hit chunk: as much as the rows the kernel moves)
+  const uint32_t seg0 = t0 / maxt;
+  for (uint32_t g = tid; g < seg0; g += kCompactThreads) sum += seg_hits[g];
+  for (uint32_t t = seg0 * maxt + tid; t < t0; t += kCompactThreads) sum += a.tiles[t] & 0xFFFFFFFFull;
 #pragma unroll
   for (int o = 16; o; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
   if (lane == 0) s_part[warp] = sum;
