@@ -349,7 +349,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- end to end through the C ABI with HOST buffers (tpx3_process_host) --------------------
-    clh = m.Clusters(max_clusters, "cpu", pin=True)
+    clh = m.Clusters(ncl + 4096, "cpu", pin=True)   # host table for the hits the workload has (count known from the warm-up)
 
     def e2e_step():
         if not lm:
