@@ -29,6 +29,7 @@ struct Ctrl {
   // of a call had tight time clusters, the tiles of the next calls skip the check (and retry every 16th call).
   uint32_t scan_hint;            // kScanSkip: the last call found the time-cluster check not worth its cost
   uint32_t calls;                // fused calls served on this workspace
+  uint32_t sort_packed;          // general sort of this call: key and index travel in one 64-bit word (tpx3_sort.cuh)
 };
 constexpr uint32_t kScanSkip = 0x5C1Fu;
 static_assert(sizeof(Ctrl) <= 256, "Ctrl must fit the 256-byte workspace header");

@@ -178,6 +178,8 @@ __host__ __device__ inline uint32_t grid_for_hd(uint64_t n, int threads, int num
       GP(TPX3_STAGE_SORT, k_radix_scan, kRadix / 8, 256, (A).w.ctrl, pass_, (A).w.counts, (A).g.nblk);                 \
       GP(TPX3_STAGE_SORT, k_radix_scatter, (A).g.nblk, kSortThreads, (A).w.ctrl, pass_, (A).toa, b_, (A).perm, n_,    \
          (A).g);                                                                                                      \
+      GP(TPX3_STAGE_SORT, k_radix_scatter_packed, (A).g.nblk, kSortThreads, (A).w.ctrl, pass_, (A).toa, b_,           \
+         (A).perm, n_, (A).g);                                                                                        \
     }                                                                                                                 \
   } while (0)
 

@@ -5,6 +5,11 @@
 // the ones past `npass` return immediately.
 //
 // Per pass: digit histogram per block -> exclusive scan (digit-major) -> stable scatter.
+// Packed mode (key span <= 36 bits, the usual case: 2^36 ticks = 107 s of data): key and input position travel
+// as ONE 64-bit word (ToA - min) << 28 | position (a plan takes at most 2^28 events), 8 instead of 12 bytes per
+// key and pass, and the scatter (k_radix_scatter_packed) orders a tile of 4096 keys in shared memory first, so
+// that consecutive threads write consecutive addresses of a digit's run. The last pass writes the plain key and
+// perm, so everything behind the sort sees the same buffers in both modes.
 // Stability inside a tile comes from warp-ordered ranking with __match_any_sync (each warp owns
 // a contiguous slice of the tile; items are visited in ascending position).
 #pragma once
@@ -16,7 +21,7 @@ constexpr int kSortThreads = 256;
 constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kSortItems = 8;                               // per thread per tile
 constexpr int kSortTile = kSortThreads * kSortItems;        // 2048
-constexpr int kSortMaxBlocks = kNumSMs * 8;                 // 1184
+constexpr int kSortMaxBlocks = kNumSMs * 8;                 // 1184 (one wave of 740 for the packed scatter, 5 blocks per SM: 3 % slower)
 constexpr int kRadixBits = 8;
 constexpr int kRadix = 1 << kRadixBits;
 constexpr int kMaxPasses = 8;
@@ -74,6 +79,7 @@ __global__ void k_sort_setup(Ctrl* c) {
   int bits = span ? 64 - __clzll((long long)span) : 1;
   uint32_t np = (uint32_t)((bits + kRadixBits - 1) / kRadixBits);
   c->npass = np ? np : 1;
+  c->sort_packed = bits <= 36 ? 1u : 0u;
   c->status.sort_passes = c->npass;
   c->status.path = 2;
 }
@@ -97,13 +103,22 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_hist(Ctrl* c, int pass, 
   __shared__ uint32_t hist[kRadix];
   hist[threadIdx.x] = 0;
   __syncthreads();
-  const int shift = pass * kRadixBits;
+  // (packed mode: from pass 1 on the source holds (ToA - min) << 28 | position)
+  const int shift = pass * kRadixBits + (c->sort_packed && pass > 0 ? 28 : 0);
   uint64_t t0 = (uint64_t)blockIdx.x * g.tiles_per_blk * kSortTile;
   uint64_t t1 = t0 + (uint64_t)g.tiles_per_blk * kSortTile;
   if (t1 > n) t1 = n;
   for (uint64_t i = t0 + threadIdx.x; i < t1; i += kSortThreads) {
     uint64_t k = sort_load_key(pass, c, toa, b, i);
-    atomicAdd(&hist[(uint32_t)(k >> shift) & (kRadix - 1)], 1u);
+    const uint32_t d = (uint32_t)(k >> shift) & (kRadix - 1);
+    // the high digits of a time-ordered stream are the same across a warp: one add instead of 32 serialised ones
+    const uint32_t act = __activemask();
+    const uint32_t d0 = __shfl_sync(act, d, __ffs(act) - 1);
+    if (__all_sync(act, d == d0)) {
+      if ((threadIdx.x & 31) == (uint32_t)(__ffs(act) - 1)) atomicAdd(&hist[d], (uint32_t)__popc(act));
+    } else {
+      atomicAdd(&hist[d], 1u);
+    }
   }
   __syncthreads();
   b.counts[(size_t)threadIdx.x * g.nblk + blockIdx.x] = hist[threadIdx.x];
@@ -137,7 +152,7 @@ __global__ void __launch_bounds__(256) k_radix_scan(Ctrl* c, int pass, uint32_t*
 __global__ void __launch_bounds__(kSortThreads) k_radix_scatter(Ctrl* c, int pass, const uint64_t* __restrict__ toa,
                                                               SortBufs b, uint32_t* __restrict__ perm, uint64_t n,
                                                               SortGeom g) {
-  if (c->fused_state == 1 || (uint32_t)pass >= c->npass) return;
+  if (c->fused_state == 1 || (uint32_t)pass >= c->npass || c->sort_packed) return;
   __shared__ uint32_t running[kRadix];
   __shared__ uint32_t warp_cnt[kSortWarps][kRadix];
   const int shift = pass * kRadixBits;
@@ -214,6 +229,119 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_scatter(Ctrl* c, int pas
       }
     }
     __syncthreads();
+  }
+}
+
+// ---- packed mode: one pass of the scatter ---------------------------------------------------------------------
+// A block walks the same key range as in k_radix_hist (so the scanned counts are its offsets), 4096 keys at a
+// time: ranks inside the tile by warp ballots (warp w owns the tile's w-th slice of 512 keys, visited in ascending
+// position: stable), the tile ordered by digit in shared memory, then written out run by run, coalesced.
+constexpr int kPackItems = 16;
+constexpr int kPackTile = kSortThreads * kPackItems;   // 4096
+static_assert(kPackTile % kSortTile == 0, "a block's key range is a multiple of the histogram's tile");
+
+__global__ void __launch_bounds__(kSortThreads) k_radix_scatter_packed(Ctrl* c, int pass, const uint64_t* __restrict__ toa,
+                                                                     SortBufs b, uint32_t* __restrict__ perm, uint64_t n,
+                                                                     SortGeom g) {
+  if (c->fused_state == 1 || (uint32_t)pass >= c->npass || !c->sort_packed) return;
+  __shared__ uint64_t stage[kPackTile];                 // 32 KB: the tile in digit order
+  __shared__ uint32_t running[kRadix];                  // global offset of the block's next key per digit
+  __shared__ uint32_t warp_cnt[kSortWarps][kRadix];     // per warp and digit: count, then tile-local offset
+  __shared__ uint32_t dig_base[kRadix + 1];             // tile-local start of a digit's run
+  __shared__ uint32_t wtot[kSortWarps];
+  const int shift = pass * kRadixBits + 28;             // digit of the PACKED word
+  const bool last = (uint32_t)pass + 1 == c->npass;
+  const uint64_t tmin = c->toa_min;
+  const uint64_t* __restrict__ skey = pass == 0 ? nullptr : b.key[(pass - 1) & 1];
+  uint64_t* __restrict__ dkey = b.key[pass & 1];
+  const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5, lt = lanemask_lt();
+  auto block_scan256 = [&](uint32_t v) -> uint32_t {    // exclusive prefix over the 256 threads' values
+    uint32_t inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= (uint32_t)o) inc += t;
+    }
+    __syncthreads();                                    // wtot of the previous use has been read
+    if (lane == 31) wtot[w] = inc;
+    __syncthreads();
+    uint32_t base = inc - v;
+    for (uint32_t ww = 0; ww < w; ++ww) base += wtot[ww];
+    return base;
+  };
+  {   // exclusive prefix over the 256 digit totals (thread d = digit d), plus this block's offset inside the digit
+    const uint32_t tot_d = b.counts[(size_t)kRadix * g.nblk + threadIdx.x];
+    running[threadIdx.x] = block_scan256(tot_d) + b.counts[(size_t)threadIdx.x * g.nblk + blockIdx.x];
+  }
+  const uint64_t r0 = (uint64_t)blockIdx.x * g.tiles_per_blk * kSortTile;
+  uint64_t r1 = r0 + (uint64_t)g.tiles_per_blk * kSortTile;
+  if (r1 > n) r1 = n;
+  for (uint64_t t0 = r0; t0 < r1; t0 += kPackTile) {
+    const uint32_t cnt = r1 - t0 < (uint64_t)kPackTile ? (uint32_t)(r1 - t0) : (uint32_t)kPackTile;
+    for (int i = threadIdx.x; i < kSortWarps * kRadix; i += kSortThreads) (&warp_cnt[0][0])[i] = 0;
+    __syncthreads();
+    uint64_t key[kPackItems];
+    uint16_t rank[kPackItems];
+    const uint32_t wbase = w * (32u * kPackItems) + lane;
+#pragma unroll
+    for (int i = 0; i < kPackItems; ++i) {              // all loads first: independent, 256 coalesced bytes per warp
+      const uint32_t q = wbase + (uint32_t)i * 32u;
+      key[i] = 0;
+      if (q < cnt) key[i] = pass == 0 ? (((toa[t0 + q] - tmin) << 28) | (t0 + q)) : skey[t0 + q];
+    }
+#pragma unroll
+    for (int i = 0; i < kPackItems; ++i) {
+      const uint32_t q = wbase + (uint32_t)i * 32u;
+      const bool valid = q < cnt;
+      const uint32_t d = valid ? ((uint32_t)(key[i] >> shift) & (kRadix - 1)) : 0u;
+      uint32_t peers = __ballot_sync(0xffffffffu, valid);
+      if (!valid) peers = 0u;
+#pragma unroll
+      for (int bit = 0; bit < kRadixBits; ++bit) {
+        const bool one = (d >> bit) & 1u;
+        const uint32_t bal = __ballot_sync(0xffffffffu, one);
+        peers &= one ? bal : ~bal;
+      }
+      const uint32_t lr = __popc(peers & lt);
+      const uint32_t base = valid ? warp_cnt[w][d] : 0u;
+      __syncwarp();
+      if (valid && lr == 0) warp_cnt[w][d] = base + __popc(peers);
+      __syncwarp();
+      rank[i] = (uint16_t)(base + lr);
+    }
+    __syncthreads();
+    uint32_t tot_d = 0;
+    {  // thread d: exclusive prefix over the warps; then over the digits
+#pragma unroll
+      for (int ww = 0; ww < kSortWarps; ++ww) {
+        const uint32_t cw = warp_cnt[ww][threadIdx.x];
+        warp_cnt[ww][threadIdx.x] = tot_d;
+        tot_d += cw;
+      }
+      const uint32_t db = block_scan256(tot_d);
+      dig_base[threadIdx.x] = db;
+      if (threadIdx.x == kRadix - 1) dig_base[kRadix] = db + tot_d;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < kPackItems; ++i) {
+      const uint32_t q = wbase + (uint32_t)i * 32u;
+      if (q < cnt) {
+        const uint32_t d = (uint32_t)(key[i] >> shift) & (kRadix - 1);
+        stage[dig_base[d] + warp_cnt[w][d] + rank[i]] = key[i];
+      }
+    }
+    __syncthreads();
+    for (uint32_t q = threadIdx.x; q < cnt; q += kSortThreads) {   // consecutive q of one digit -> consecutive addresses
+      const uint64_t k = stage[q];
+      const uint32_t d = (uint32_t)(k >> shift) & (kRadix - 1);
+      const uint32_t dst = running[d] + (q - dig_base[d]);
+      if (last) { dkey[dst] = k >> 28; perm[dst] = (uint32_t)k & 0x0FFFFFFFu; }
+      else dkey[dst] = k;
+    }
+    __syncthreads();
+    running[threadIdx.x] += tot_d;
+    // (the next round's first barrier orders this update before its use)
   }
 }
 
