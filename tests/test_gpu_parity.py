@@ -690,6 +690,18 @@ def test_unwrap_toa(tpx3):
     alt = np.where(np.arange(50000) % 2 == 0, 5, 1000).astype(np.uint64)
     run(alt, 1024, 600)
     run(rng.integers(0, 1024, 70000), 1024, 300)
+    # 1.3e7 events (3 000 blocks: the block-sum scan runs several rounds per thread): generated truth over 5.4 counter
+    # periods (the sequential oracle is a Python loop; the true times are what it must give back)
+    n = (1 << 23) + (1 << 22) + 54321
+    mod2 = 1 << 30
+    t = np.sort(rng.integers(0, 5 * mod2 + mod2 // 3, n).astype(np.int64)) + rng.integers(0, 3000, n) + mod2 - 7000
+    w0 = int(t[0] // mod2)
+    pl = m.plan(m.Config(max_hits=n))
+    out, w = pl.unwrap_toa(to_dev((t % mod2).astype(np.uint64)), mod2, mod2 // 2, wraps_in=w0)
+    torch.cuda.synchronize()
+    assert np.array_equal(out[:n].cpu().numpy().astype(np.int64), t)
+    assert int(w.cpu().numpy()[0]) == int(t[-1] // mod2) and int(w.cpu().numpy()[0]) >= 5
+    pl.free()
 
 
 # ------------------------------------------------------------------ preprocessing (NEXT #3)
