@@ -414,6 +414,7 @@ def run_ours(args):
                                    "centroid": "centroid stage"}[dom],
         "achieved": dom_gbs, "peak": peak, "unit": "GB/s", "frac": dom_gbs / peak, "traffic": None,
         "peak_source": peak_src, "algorithmic_bytes_per_launch": dom_bytes,
+        "frac_of_nominal_8TBs": dom_gbs / 8000.0,    # BASELINE.json north_star quotes the nominal peak too
         "stage_ms": stage_ms, "stage_launches": {k: v / max(args.steps, 1) for k, v in prof["launches"].items()},
         "whole_path": {"algorithmic_bytes_per_step": whole_bytes,
                        "achieved": whole_bytes / (ms_step * 1e-3) / 1e9 * (n_all / max(n, 1)) / max(world, 1),
@@ -429,6 +430,9 @@ def run_ours(args):
         if key in tr and tr[key].get("pixel_hits", n) == n:
             roofline["traffic"] = tr[key]["dram_bytes_per_launch"]
             roofline["traffic_source"] = tr[key].get("source")
+            if stage_ms[dom] > 0:
+                # achieved DRAM GB/s = ncu bytes (committed capture) / device time of this run's stage
+                roofline["dram_gbs_from_traffic"] = tr[key]["dram_bytes_per_launch"] / (stage_ms[dom] * 1e-3) / 1e9
             wi = tr[key].get("warp_instructions_per_launch")
             if wi and stage_ms[dom] > 0:
                 # what actually bounds the kernel: warp instructions issued per second against
