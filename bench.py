@@ -576,6 +576,95 @@ def run_stream(args):
     return 0
 
 
+def run_sweep1g(args):
+    """--mode sweep1g: BASELINE.json configs[4] to the letter: 10^9 pixel hits of the streaming config (whole shots, four
+    parts of up to 2^28 hits generated one after the other and kept resident: 14 GB), processed in shot-aligned chunks of
+    2^20, 2^24, 2^26 and 2^28 hits, one tpx3_cluster_centroid call per chunk; per chunk size the time of ONE pass over all
+    10^9 hits, device-timed. Single GPU; a secondary bench line (the default line times one 2^28 chunk)."""
+    import torch
+
+    import gen
+    import paper_2603_04942_b200 as m
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    m.load_library()
+    big = 1 << 28
+    target = 10 ** 9
+    parts, total, shot_begin = [], 0, 0
+    while total < target:
+        w = gen.generate(4, shots=int(big / 850) + 64, shot_begin=shot_begin, max_hits=min(big, target - total + 2000))
+        shot_begin += w.shots
+        total += w.n
+        parts.append(([torch.from_numpy(a).cuda() for a in (w.x, w.y, w.toa, w.tot)], w.shot_offsets.copy(),
+                      {sz: w.chunks(sz) for sz in (1 << 20, 1 << 24, 1 << 26, big)}, w.n))
+        del w
+    pl = m.plan(m.Config(max_hits=big, toa_window_ticks=gen.TOA_WINDOW_TICKS, shot_period_ticks=gen.SHOT_PERIOD_TICKS,
+                         max_shot_hits=gen.max_shot_hits(4)))
+    stream = torch.cuda.Stream(device=0)
+    cl = m.Clusters(big // 8, pl.device)
+    perm = torch.empty(big, dtype=torch.uint32, device=pl.device)
+    label = torch.empty(big, dtype=torch.uint32, device=pl.device)
+    nc = torch.zeros(1, dtype=torch.uint32, device=pl.device)
+
+    def one_pass(size, count=False):
+        hits = calls = 0
+        for dev, off, chunks, _ in parts:
+            for s0, s1 in chunks[size]:
+                a, b = int(off[s0]), int(off[s1])
+                pl.cluster_centroid(*(d[a:b] for d in dev), cl, perm=perm, label=label, n_clusters=nc, stream=stream)
+                calls += 1
+                if count:
+                    stream.synchronize()
+                    st = pl.status(stream)
+                    if st["error"] or st["path"] != 1:
+                        raise RuntimeError("chunk [%d, %d): %r" % (a, b, st))
+                    hits += st["n_clusters"]
+        return hits, calls
+
+    peak, peak_src = measured_peak()
+    sampler = ClockSampler(0)
+    sampler.start()
+    t_wall0 = time.time()
+    sweep, ncl = {}, None
+    for name, size in (("2^28", big), ("2^26", 1 << 26), ("2^24", 1 << 24), ("2^20", 1 << 20)):
+        hits, calls = one_pass(size, count=True)             # warm-up pass; also counts the hits and checks every call
+        if ncl is None:
+            ncl = hits
+        assert hits == ncl, (name, hits, ncl)                 # the rows do not depend on the chunk size
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = max(args.steps, 1) if size >= (1 << 24) else 1
+        e0.record(stream)
+        for _ in range(reps):
+            one_pass(size)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / reps
+        nbytes = STAGE_BYTES["fused"](total, ncl)
+        sweep[name] = {"calls_per_pass": calls, "ms_per_pass": ms, "pixel_hits_per_s": total / (ms * 1e-3),
+                       "particle_hits_per_s": ncl / (ms * 1e-3), "algorithmic_gbs": nbytes / (ms * 1e-3) / 1e9,
+                       "frac_of_hbm_peak": nbytes / (ms * 1e-3) / 1e9 / peak}
+    sampler.stop()
+    head = sweep["2^28"]
+    line = {
+        "metric": METRIC, "value": head["pixel_hits_per_s"], "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": 1, "ms_per_step": head["ms_per_pass"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int64", "data": "synthetic",
+        "config": {"workload": "cfg4_streaming, 10^9 pixel hits in %d resident parts" % len(parts), "mode": "sweep1g",
+                   "pixel_hits_total": total, "particle_hits_total": ncl, "max_shot_hits": gen.max_shot_hits(4),
+                   "what": "one step = one pass over all hits, one tpx3_cluster_centroid call per shot-aligned chunk"},
+        "chunk_sweep": sweep,
+        "roofline": {"bound": "hbm", "kernel": "fused stage, whole pass in 2^28-hit chunks", "achieved": head["algorithmic_gbs"],
+                     "peak": peak, "unit": "GB/s", "frac": head["frac_of_hbm_peak"], "traffic": None, "peak_source": peak_src},
+        "clocks": sampler.summary(t_wall0, time.time()),
+    }
+    print(json.dumps(line), flush=True)
+    pl.free()
+    return 0
+
+
 def run_aux(args):
     """--mode unwrap | preprocess: the two preprocessing calls of SURVEY.md 8f NEXT #4 / #3 on the workload's
     events (device-resident, device-timed), against the HBM roofline of their algorithmic bytes."""
@@ -712,7 +801,7 @@ def main():
                     help="tile-size hint for the plan (default: the workload recipe's bound on hits per shot)")
     ap.add_argument("--chunk", type=int, default=1 << 22, help="--mode stream: events per push")
     ap.add_argument("--max-carry", type=int, default=1 << 20, help="--mode stream: carry capacity in events")
-    ap.add_argument("--mode", choices=("components", "split", "localmax", "stream", "unwrap", "preprocess", "prefused"), default="components",
+    ap.add_argument("--mode", choices=("components", "split", "localmax", "stream", "unwrap", "preprocess", "prefused", "sweep1g"), default="components",
                     help="components: the hot path (default). localmax: the paper-literal mode, SURVEY 8f NEXT #2")
     ap.add_argument("--window", type=int, nargs=3, default=(2, 2, 320), metavar=("WX", "WY", "WT"),
                     help="box half-widths of --mode localmax (pixels, pixels, ticks)")
@@ -725,6 +814,8 @@ def main():
         print("note: timing rules ask for >= 3 warm-up steps", file=sys.stderr)
     if args.impl == "reference":
         return run_reference(args)
+    if args.mode == "sweep1g":
+        return run_sweep1g(args)
     if args.mode in ("unwrap", "preprocess", "prefused"):
         return run_aux(args)
     return run_stream(args) if args.mode == "stream" else run_ours(args)

@@ -24,6 +24,11 @@
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
  *     Device-pointer calls only ENQUEUE work on that stream and return; there is no hidden
  *     synchronisation. Outputs are valid once the stream has reached the end of the call.
+ *   - Alignment: every array at the natural alignment of its element type. The fast path reads with 128-bit loads;
+ *     x, y, toa, tot that start at the same element offset from a 16-byte boundary - a chunk of a resident
+ *     stream cut at any event, arrays offset alike - are served by it all the same (the library reads up to 7
+ *     elements in front of the pointers inside the same 16-byte block and ignores them); arrays that are not
+ *     offset alike take the general route (same results, slower).
  *   - `perm[k]`  = original (input) index of the event at sorted position k.
  *     `label[k]` = sorted position of the first event of k's hit; indexed by SORTED position.
  *     Clusters are listed in ascending `label` order (exactly one valid output exists).

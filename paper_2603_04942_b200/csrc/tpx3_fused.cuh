@@ -164,6 +164,11 @@ struct FusedArgs {
   const uint64_t* label_base;   // [dev] or null: added (low 32 bits) to the label column (stream pushes, R24)
   PreArgs pre;                  // mode 4 only: trigger list, cut, timewalk table (tpx3_preprocess.cuh)
   const uint32_t* seg_kept;     // mode 4 only: events that survive the preprocessing in front of every segment
+  uint32_t head;                // Inputs that are not 16-byte aligned (a chunk of a resident stream that starts at any event):
+                                // the position-indexed arrays are passed moved DOWN by `head` elements to the alignment
+                                // boundary, n counts those elements too, and the kernel starts at position `head`.
+                                // Position p of the kernel is element p - head of the caller's arrays; the values it
+                                // writes (perm, label) are in the caller's numbering.
   uint32_t labels_only;         // mode 5 only: stop after the labels (the general route of tpx3_cluster)
   const uint32_t* n_dev;        // [dev] or null: the event count is device state (a stream push): n, G, nseg, maxt and
                                 // num_tiles above are upper bounds then (they size the grids) and every kernel
@@ -345,7 +350,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   const uint32_t seg_begin = seg * seg_G;
   const uint32_t seg_end = seg_begin + seg_G < n_ev ? seg_begin + seg_G : n_ev;
   const uint32_t P32 = (uint32_t)a.P;
-  uint32_t tile_at = seg_begin;     // where the next tile starts; a shot start except for the segment's first tile
+  const uint32_t seg_first = seg == 0 ? a.head : seg_begin;   // (the elements below `head` are not the caller's)
+  uint32_t tile_at = seg_first;     // where the next tile starts; a shot start except for the segment's first tile
   uint32_t kept_run = kPre ? a.seg_kept[seg] : 0u;   // mode 4: surviving events in front of tile_at
   uint64_t pre_next_s = 0;          // mode 4: trigger index of the event at tile_at, when the previous tile saw it
   bool pre_have_s = false;
@@ -444,7 +450,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     misc->last = 0;
     // another tile already gave up: this attempt is lost, do not spend time on it (the next attempt — a
     // variant with longer shots, or the general kernels — is enqueued behind; k_fallback_dispatch)
-    misc->skip = tile_at == seg_begin ? atomicAdd(&a.ctrl->fused_fail, 0u) : 0u;
+    misc->skip = tile_at == seg_first ? atomicAdd(&a.ctrl->fused_fail, 0u) : 0u;
     misc->fail = 0;
     misc->max_tof = 0;
     misc->loose = 0;
@@ -842,6 +848,8 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     out_base = kept_run + misc->kept_pre;
     kept_run = out_base + mm;
   }
+  // what the tile writes as VALUES is in the caller's numbering (FusedArgs::head)
+  const uint32_t out_val = out_base - a.head, raw_val = raw_base - a.head;
   if (cl_wide && !cl_scan && tid == 0) misc->loose = 1u;   // not checked: treated as not tight
   if (!unsorted && cl_scan) {
     for (uint32_t w = 0; w < warp; ++w) cl_carry = max(cl_carry, misc->warp_sums[w]);
@@ -1127,7 +1135,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         const uint32_t s = fin[k];
         rec = recB[lo + s];
         recA[k] = rec;
-        a.perm[out_base + k] = raw_base + s;
+        a.perm[out_base + k] = raw_val + s;
       }
       if (cl_scan) {
         const uint32_t key = rec.x;
@@ -1165,7 +1173,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     __syncthreads();
   } else {
     if (!kPerm)
-      for (uint32_t k = tid; k < mm; k += THREADS) a.perm[out_base + k] = raw_base + k;
+      for (uint32_t k = tid; k < mm; k += THREADS) a.perm[out_base + k] = raw_val + k;
   }
   const uint2* recS = unsorted ? recA : recB + lo;
   unsigned char* hreg = smem + (unsorted ? L::kRegX : L::kRegA);   // 16T bytes: hash table, later the label / chain arrays
@@ -1263,7 +1271,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         if (tj > ti || (tj == ti && j > k)) is_max = false;      // equal ToT: the later pixel wins (:150)
       });
       // the marks overwrite the bucket counters (dead since the insert barrier), not the table
-      a.label[out_base + k] = is_max ? out_base + k : kNone;
+      a.label[out_base + k] = is_max ? out_val + k : kNone;
       lab[k] = is_max ? (uint16_t)k : (uint16_t)0xFFFFu;
     }
     __syncthreads();
@@ -1287,7 +1295,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         if ((q.y >> 16) >= ti && lm_near(r.y, q.y, a.lm_wx, a.lm_wy)) is_max = false;   // later: wins ties (:150)
       }
       lab[k] = is_max ? (uint16_t)k : (uint16_t)0xFFFFu;
-      a.label[out_base + k] = is_max ? out_base + k : kNone;
+      a.label[out_base + k] = is_max ? out_val + k : kNone;
     }
     __syncthreads();
   } else if (kGiven) {
@@ -1305,7 +1313,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     for (int j = 0; j < IPT; ++j) {
       const uint32_t k = (uint32_t)j * THREADS + tid;
       if (k < mm) {
-        const uint32_t l = a.label[out_base + k] - out_base;      // a label before the tile wraps to a huge value
+        const uint32_t l = a.label[out_base + k] - out_val;       // a label before the tile wraps to a huge value
         if (l >= mm) { outside = true; lab[k] = (uint16_t)0xFFFFu; }
         else {
           lab[k] = (uint16_t)l;
@@ -1538,7 +1546,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     if (k < mm) {
       const uint32_t l = minidx[root_r[j]];
       lab[k] = (uint16_t)l;
-      a.label[out_base + k] = out_base + l;
+      a.label[out_base + k] = out_val + l;
       if (!kLabelsOnly && !(MODE == 5 && a.labels_only)) nxt[k] = (uint16_t)atomicExch(&head[l], k);   // every member, the first pixel too; kNone truncates to 0xFFFF = end
     }
   }
@@ -1602,7 +1610,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         sf += (unsigned long long)t * (unsigned long long)(q.x & tmask);
       });
       const uint64_t o = (uint64_t)out_base + c;
-      a.stage_a[o] = make_uint4(out_base + r, size, st, 0u);
+      a.stage_a[o] = make_uint4(out_val + r, size, st, 0u);
       a.stage_b[o] = make_uint4((uint32_t)sx, (uint32_t)(sx >> 32), (uint32_t)sy, (uint32_t)(sy >> 32));
       a.stage_c[o] = ref + (uint64_t)(rr.x >> tb) * a.P + (uint64_t)(rr.x & tmask);
       a.stage_d[o] = sf;
@@ -1636,7 +1644,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
         add(q);
       }
       const uint64_t o = (uint64_t)out_base + c;
-      a.stage_a[o] = make_uint4(out_base + r, size, st, 0u);
+      a.stage_a[o] = make_uint4(out_val + r, size, st, 0u);
       a.stage_b[o] = make_uint4((uint32_t)sx, (uint32_t)(sx >> 32), (uint32_t)sy, (uint32_t)(sy >> 32));
       a.stage_c[o] = ref + (uint64_t)(rr.x >> tb) * a.P + (uint64_t)(rr.x & tmask);
       a.stage_d[o] = sf;
@@ -1660,7 +1668,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
     } while (k != 0xFFFFu);
     const uint32_t keyp = recS[best & 0xFFFFu].x;
     const uint64_t o = (uint64_t)out_base + c;
-    a.stage_a[o] = make_uint4(out_base + r, size, st, 0u);
+    a.stage_a[o] = make_uint4(out_val + r, size, st, 0u);
     a.stage_b[o] = make_uint4((uint32_t)sx, (uint32_t)(sx >> 32), (uint32_t)sy, (uint32_t)(sy >> 32));
     a.stage_c[o] = ref + (uint64_t)(keyp >> tb) * a.P + (uint64_t)(keyp & tmask);
     a.stage_d[o] = sf;
@@ -1906,6 +1914,7 @@ inline FusedArgs make_fused_args(uint32_t T, uint32_t num_sms, Ctrl* ctrl, unsig
   a.stage_d = a.stage_c + prm.n;
   a.mode = mode; a.lm_wx = lm_wx; a.lm_wy = lm_wy;
   a.label_base = nullptr;
+  a.head = 0;
   memset(&a.pre, 0, sizeof(a.pre));
   a.seg_kept = nullptr;
   a.labels_only = 0;
@@ -1950,6 +1959,41 @@ __device__ inline void launch_fused_rung_device(FusedArgs a, uint32_t T) {
   k_fused_compact<<<ctas, kCompactThreads, 0, cudaStreamTailLaunch>>>(a, tpc, T);
 }
 
+// How far the position-indexed arrays of a call sit behind a 16-byte boundary, in elements (FusedArgs::head); -1: they
+// are not aligned alike (or not to their element size): no tile kernel. Modes 0, 1, 2, 4 read x, y, tot (2 bytes) and toa
+// (8 bytes) by position with 128-bit loads; modes 3 and 5 read perm (4 bytes) that way and gather the events.
+__host__ __device__ inline int fused_head_of(uint32_t mode, const void* x, const void* y, const void* toa, const void* tot,
+                                             const void* perm) {
+  if (mode == 3u || mode == 5u) return ((uintptr_t)perm & 3u) ? -1 : (int)(((uintptr_t)perm >> 2) & 3u);
+  if ((((uintptr_t)x | (uintptr_t)y | (uintptr_t)tot) & 1u) || ((uintptr_t)toa & 7u)) return -1;
+  const uint32_t e = (uint32_t)(((uintptr_t)x >> 1) & 7u);
+  if ((((uintptr_t)y >> 1) & 7u) != e || (((uintptr_t)tot >> 1) & 7u) != e || (((uintptr_t)toa >> 3) & 1u) != (e & 1u)) return -1;
+  return (int)e;
+}
+
+// Moves the position-indexed arrays down to the boundary and lets the positions start at `e` (head 0 before the call).
+__host__ __device__ inline void fused_apply_head(FusedArgs& a, uint32_t e, uint32_t T) {
+  if (a.mode != 3u && a.mode != 5u) { a.x -= e; a.y -= e; a.toa -= e; a.tot -= e; }
+  a.perm -= e;
+  a.label -= e;
+  a.head = e;
+  fused_set_n(a, a.n + e, T);
+}
+
+// The general route's tile kernel (mode 5) from the arguments of a first attempt in mode 0 / 2 on the same call: back
+// to the caller's pointers, then the head that perm's alignment asks for; 8192-event windows.
+__host__ __device__ inline void fused_rebase_mode5(FusedArgs& a, uint32_t labels_only) {
+  const uint32_t e0 = a.head;
+  if (a.mode != 3u && a.mode != 5u) { a.x += e0; a.y += e0; a.toa += e0; a.tot += e0; }
+  a.perm += e0;
+  a.label += e0;
+  a.n -= e0;
+  a.head = 0;
+  a.mode = 5u;
+  a.labels_only = labels_only;
+  fused_apply_head(a, (uint32_t)(((uintptr_t)a.perm >> 2) & 3u), 8192u);
+}
+
 // Host side. Returns TPX3_OK (launched or not applicable; *launched says which) or an error. *args receives the
 // arguments of the enqueued rung (the later rungs differ in the segment geometry only).
 inline int enqueue_fused(const FusedGeom& g, uint32_t num_sms, uint64_t* launches, Ctrl* ctrl, unsigned long long* tiles,
@@ -1961,11 +2005,14 @@ inline int enqueue_fused(const FusedGeom& g, uint32_t num_sms, uint64_t* launche
                          const PreArgs* pre = nullptr, const uint32_t* seg_kept = nullptr) {
   *launched = false;
   if (g.variant == 0 || prm.n == 0) return TPX3_OK;
-  // the 128-bit load phase needs 16-byte aligned inputs (PyTorch allocations are 256-byte aligned)
-  if ((((uintptr_t)x | (uintptr_t)y | (uintptr_t)toa | (uintptr_t)tot) & 15u) != 0) return TPX3_OK;
-  if (mode == 3u && ((uintptr_t)perm & 15u) != 0) return TPX3_OK;
+  // the 128-bit load phase needs its arrays on a 16-byte boundary: a chunk of a resident stream that starts at any event
+  // is served by moving all of them down to the boundary alike (FusedArgs::head); arrays that are not aligned alike,
+  // and the calls whose count lives on the device or that preprocess (library-owned, resp. checked by the caller): not
+  const int e = fused_head_of(mode, x, y, toa, tot, perm);
+  if (e < 0 || (e > 0 && (n_dev != nullptr || mode == 4u))) return TPX3_OK;
   FusedArgs a = make_fused_args(g.T, num_sms, ctrl, tiles, prm, x, y, toa, tot, perm, label, max_clusters, out,
                                 n_clusters, stage, mode, lm_wx, lm_wy, n_dev);
+  if (e > 0) fused_apply_head(a, (uint32_t)e, g.T);
   a.label_base = label_base;
   if (pre) { a.pre = *pre; a.seg_kept = seg_kept; }
   if (n_dev) {   // grids that cover every count up to prm.n (fused_segs: a short input is cut into up to `want` segments)

@@ -296,10 +296,7 @@ __global__ void k_general_slab(GenArgs a, int what) {
 __global__ void k_general_sorted_tiles(GenArgs a, FusedArgs fa, int what) {
   Ctrl* c = a.w.ctrl;
   c->tiles_done = 0; c->fused_fail = 0; c->fused_state = 0; c->tight_tiles = 0; c->tiles_run = 0;
-  fa.mode = 5u;
-  fa.labels_only = what == 2 ? 1u : 0u;
-  const FusedSegs sg = fused_segs(fa.n, 8192u, fa.num_sms);
-  fa.G = sg.G; fa.nseg = sg.nseg; fa.maxt = sg.maxt; fa.num_tiles = sg.nseg * sg.maxt;
+  fused_rebase_mode5(fa, what == 2 ? 1u : 0u);
   launch_fused_rung_device(fa, 8192u);
   k_general_slab<<<1, 1, 0, cudaStreamTailLaunch>>>(a, what);
 }
@@ -449,7 +446,7 @@ int tpx3_plan(const tpx3_config_t* cfg, tpx3_plan_t* out_plan, size_t* workspace
   p->off_table = o; o = align_up(o + 4 * (size_t)table_size_for(N));
   p->off_counts = o; o = align_up(o + 4 * (size_t)kRadix * (kSortMaxBlocks + 1));   // + the digit totals
   // the fused path's staging table (48 bytes per event) aliases keyA .. table
-  if (o - p->off_keyA < 48 * (size_t)N) o = align_up(p->off_keyA + 48 * (size_t)N);
+  if (o - p->off_keyA < 48 * (size_t)(N + 8)) o = align_up(p->off_keyA + 48 * (size_t)(N + 8));   // + 8: FusedArgs::head
   // centroid buffers alias the sort buffers (the two steps never run concurrently and the
   // centroid step takes perm/label from the caller, not from the workspace)
   p->off_slot = p->off_keyA;                    // 4N <= 8N
@@ -491,8 +488,7 @@ static int run_fused_or_general(tpx3_plan_t p, void* workspace, void* cuda_strea
   GenArgs ga = make_gen_args(p, w, mode == 2u ? 0 : 1, n, x, y, toa, tot, perm, label, max_clusters, out, n_clusters);
   ga.label_base = label_base;
   // the general route links through the tile kernel too, behind its global sort (mode 5), when the plan has one
-  ga.sorted_tiles = p->fused.variant != 0 && mode != 3u &&
-                    (((uintptr_t)x | (uintptr_t)y | (uintptr_t)toa | (uintptr_t)tot | (uintptr_t)perm) & 15u) == 0;
+  ga.sorted_tiles = p->fused.variant != 0 && mode != 3u && ((uintptr_t)perm & 3u) == 0;
   if (sc && !try_fused) {   // general kernels only: launched from the device, which knows the count
     FusedArgs fa = make_fused_args(2048u, (uint32_t)p->num_sms, w.ctrl, w.tiles, prm, x, y, toa, tot, perm, label,
                                    max_clusters, out ? *out : none, n_clusters, (char*)workspace + p->off_keyA, mode, 0u,
@@ -528,7 +524,7 @@ static int run_fused_or_general(tpx3_plan_t p, void* workspace, void* cuda_strea
                                      max_clusters, out ? *out : none, n_clusters, (char*)workspace + p->off_keyA, 5u, 0u,
                                      0u, nullptr);
       fa.label_base = label_base;
-      fa.labels_only = mode == 2u ? 1u : 0u;
+      fused_rebase_mode5(fa, mode == 2u ? 1u : 0u);
       k_fused_shot_tiles<8192, 1024, 5><<<fa.nseg, 1024, FusedSmem<8192>::kBytes, st>>>(fa);
       uint32_t ctas, tpc;
       compact_grid(fa.num_tiles, (uint32_t)p->num_sms, &ctas, &tpc);

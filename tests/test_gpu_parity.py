@@ -295,6 +295,63 @@ def test_split_calls_take_the_tile_kernel(tpx3, cfg, shots, hint):
     pl.free()
 
 
+@pytest.mark.parametrize("off,poff", [(1, 0), (2, 3), (3, 1), (5, 2), (7, 7), (8, 5), (12347, 1)])
+def test_chunks_of_a_resident_stream_at_any_offset(tpx3, off, poff):
+    """Inputs (and outputs) that are views into larger device arrays at any element offset - a chunk of a resident
+    stream cut at a shot boundary - are not 16-byte aligned; the tile kernel still serves them (the arrays are moved down
+    to the boundary alike, FusedArgs::head): every route, outputs in the caller's numbering."""
+    import torch
+
+    w = gen.generate(4, shots=60)
+    n = w.n
+    o = oracle.run(w.x, w.y, w.toa, w.tot, W, P)
+    pad = lambda a: to_dev(np.concatenate([np.full(off, 7, a.dtype), a, np.full(9, 7, a.dtype)]))[off:off + n]  # noqa: E731
+    dev = [pad(a) for a in (w.x, w.y, w.toa, w.tot)]
+    assert dev[0].data_ptr() % 16 == (2 * off) % 16
+    for flags, want_path in ((0, 1), (tpx3.FLAG_FORCE_GENERAL, 2)):
+        pl = tpx3.plan(tpx3.Config(max_hits=n, max_shot_hits=1500, flags=flags))
+        mk = lambda: torch.full((n + poff + 8,), 0xDEAD, dtype=torch.uint32, device="cuda")  # noqa: E731
+        pbuf, lbuf = mk(), mk()
+        perm, label = pbuf[poff:poff + n], lbuf[poff:poff + n]
+        cl = tpx3.Clusters(n, pl.device)
+        _, _, nc = pl.cluster_centroid(*dev, cl, perm=perm, label=label)
+        torch.cuda.synchronize()
+        st = pl.status()
+        assert st["error"] == 0 and st["path"] == want_path, st
+        ncl = int(nc.cpu().numpy()[0])
+        g = {"perm": perm.cpu().numpy(), "label": label.cpu().numpy(), "n_clusters": ncl}
+        g.update(cl.numpy(ncl))
+        assert_parity(g, o, "offset %d flags %d" % (off, flags))
+        assert int(pbuf[poff + n].cpu()) == 0xDEAD and (poff == 0 or int(pbuf[poff - 1].cpu()) == 0xDEAD)   # nothing beside the view
+        assert int(lbuf[poff + n].cpu()) == 0xDEAD and (poff == 0 or int(lbuf[poff - 1].cpu()) == 0xDEAD)
+        # the two calls: labels only, then the sums on those (perm is read by position there)
+        pbuf2, lbuf2 = mk(), mk()
+        perm2, label2 = pbuf2[poff:poff + n], lbuf2[poff:poff + n]
+        pl.cluster(*dev, perm=perm2, label=label2)
+        cl2 = tpx3.Clusters(n, pl.device)
+        nc2 = pl.centroid(*dev, perm2, label2, cl2)
+        torch.cuda.synchronize()
+        st = pl.status()
+        assert st["error"] == 0 and (flags or st["path"] == 1), st
+        g2 = {"perm": perm2.cpu().numpy(), "label": label2.cpu().numpy(), "n_clusters": int(nc2.cpu().numpy()[0])}
+        g2.update(cl2.numpy(g2["n_clusters"]))
+        assert_parity(g2, o, "split, offset %d flags %d" % (off, flags))
+        pl.free()
+    # arrays that are NOT aligned alike (x one element further than the others): still the right answer, general route
+    if off == 1:
+        pl = tpx3.plan(tpx3.Config(max_hits=n, max_shot_hits=1500))
+        xs = to_dev(np.concatenate([np.zeros(2, np.uint16), w.x]))[2:]
+        cl = tpx3.Clusters(n, pl.device)
+        perm, label, nc = pl.cluster_centroid(xs, dev[1], dev[2], dev[3], cl)
+        torch.cuda.synchronize()
+        st = pl.status()
+        assert st["error"] == 0 and st["path"] == 2, st
+        g = {"perm": perm[:n].cpu().numpy(), "label": label[:n].cpu().numpy(), "n_clusters": int(nc.cpu().numpy()[0])}
+        g.update(cl.numpy(g["n_clusters"]))
+        assert_parity(g, o, "unlike alignment")
+        pl.free()
+
+
 def test_centroid_with_hits_that_cross_shots(tpx3):
     """tpx3_centroid takes ANY valid (perm, label): here every event of the stream is declared one hit (label 0),
     so the hit crosses every shot and every tile: the tile kernel gives up and the general kernels serve the
