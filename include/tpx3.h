@@ -228,7 +228,8 @@ int tpx3_preprocess(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64
  * the stream; an event before the first trigger counts to trigger 0 for this purpose) whose shots fit the
  * plan's window (max_shot_hits, counted on the raw stream, must be given); anything else is detected on the
  * device and reported as TPX3_ERR_NOT_CONTIGUOUS by tpx3_status - nothing valid has been written then. The
- * plan's shot period must be > 0 and <= 2^24. Enqueue only. */
+ * plan's shot period must be > 0 and <= 2^24; x, y, toa, tot must be 16-byte aligned (TPX3_ERR_INVALID_ARG otherwise: this
+ * call has no general route to fall back to). Enqueue only. */
 int tpx3_preprocess_cluster_centroid(tpx3_plan_t plan, void* workspace, void* cuda_stream, uint64_t n,
                                      const uint16_t* x, const uint16_t* y, const uint64_t* toa,
                                      const uint16_t* tot, uint64_t n_trig, const uint64_t* trig, uint64_t cut,

@@ -337,6 +337,25 @@ def test_chunks_of_a_resident_stream_at_any_offset(tpx3, off, poff):
         g2.update(cl2.numpy(g2["n_clusters"]))
         assert_parity(g2, o, "split, offset %d flags %d" % (off, flags))
         pl.free()
+    # the paper-literal mode on the same views
+    if off in (3, 12347):
+        olm = oracle.run_localmax(w.x, w.y, w.toa, w.tot, 2, 1, 200, P)
+        for flags in (0, tpx3.FLAG_FORCE_GENERAL):
+            pl = tpx3.plan(tpx3.Config(max_hits=n, max_shot_hits=1500, flags=flags))
+            pbuf, lbuf = torch.zeros(n + poff + 8, dtype=torch.uint32, device="cuda"), torch.zeros(n + poff + 8, dtype=torch.uint32, device="cuda")
+            cl = tpx3.Clusters(n, pl.device)
+            _, _, nh = pl.localmax_centroid(*dev, 2, 1, 200, cl, perm=pbuf[poff:poff + n], lmax=lbuf[poff:poff + n])
+            torch.cuda.synchronize()
+            st = pl.status()
+            assert st["error"] == 0 and st["path"] == 3, st
+            k = int(nh.cpu().numpy()[0])
+            assert k == olm["n_clusters"]
+            np.testing.assert_array_equal(pbuf[poff:poff + n].cpu().numpy(), olm["perm"])
+            np.testing.assert_array_equal(lbuf[poff:poff + n].cpu().numpy(), olm["lmax"])
+            got = cl.numpy(k)
+            for key in LM_KEYS:
+                np.testing.assert_array_equal(got[key], olm[key], err_msg="localmax offset %d flags %d %s" % (off, flags, key))
+            pl.free()
     # arrays that are NOT aligned alike (x one element further than the others): still the right answer, general route
     if off == 1:
         pl = tpx3.plan(tpx3.Config(max_hits=n, max_shot_hits=1500))
