@@ -321,10 +321,10 @@ __device__ __forceinline__ void uf_unite(uint16_t* par, uint32_t a, uint32_t b) 
 template <int T, int THREADS, int MODE>
 __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))) k_fused_shot_tiles(FusedArgs a) {
   constexpr int IPT = T / THREADS;  // 8 events per thread
-  constexpr bool kLM = MODE == 1;            // paper-literal mode (tpx3_localmax_centroid)
+  constexpr bool kLM = MODE == 1 || MODE == 6;   // paper-literal mode (tpx3_localmax_centroid); 6: behind the general sort
   constexpr bool kLabelsOnly = MODE == 2;    // S0-S3 only: perm, label, hit count (tpx3_cluster)
   constexpr bool kGiven = MODE == 3;         // S4-S5 for a given (perm, label) (tpx3_centroid): no sort, no link
-  constexpr bool kPerm = MODE == 3 || MODE == 5;   // the events are read through a given perm, which is not written
+  constexpr bool kPerm = MODE == 3 || MODE == 5 || MODE == 6;   // the events are read through a given perm, which is not written
   constexpr bool kPre = MODE == 4;           // S0-S5 on a RAW stream: trigger assignment, ToF cut, timewalk, rebase in the load phase
   constexpr bool kCC = MODE == 0 || MODE == 2 || MODE == 4 || MODE == 5;   // hits are connected components found here
   static_assert(IPT == 8, "the 128-bit load phase assumes 8 events per thread");
@@ -842,7 +842,7 @@ __global__ void __launch_bounds__(THREADS, (T <= 2048 ? 4 : (T <= 4096 ? 2 : 1))
   }
   const bool out_of_order = __syncthreads_or(!kGiven && uns ? 1 : 0) != 0;
   const bool unsorted = !kPerm && out_of_order;    // a given perm is never re-sorted (mode 5: it IS the (shot, ToA) order)
-  if (MODE == 5 && out_of_order) failed = true;
+  if ((MODE == 5 || MODE == 6) && out_of_order) failed = true;
   if constexpr (kPre) {     // (a tile whose keys ascend has its dropped events, key 0xFFFFFFFF, at the end: first mm records)
     mm = failed ? 0u : misc->kept_own;
     out_base = kept_run + misc->kept_pre;
@@ -1811,7 +1811,8 @@ __global__ void __launch_bounds__(kCompactThreads) k_fused_compact(FusedArgs a, 
   if (t1 == a.num_tiles && tid == 0) {
     *a.n_clusters = (uint32_t)prefix;
     a.ctrl->status.n_clusters = (uint32_t)prefix;
-    if (a.mode != 5u) {     // mode 5 runs behind the general path's global sort: path 2 and its pass count stand
+    if (a.mode == 6u) a.ctrl->status.path = 3;
+    if (a.mode != 5u && a.mode != 6u) {     // modes 5 and 6 run behind the general path's global sort: its pass count stands (mode 5: path 2 too)
       a.ctrl->status.path = a.mode == 1u ? 3 : 1;
       a.ctrl->status.sort_passes = 0;
     }
@@ -1859,7 +1860,7 @@ inline int fused_configure_device() {
   TPX3_FUSED_ATTR(2048, 256, 0) TPX3_FUSED_ATTR(2048, 256, 1) TPX3_FUSED_ATTR(2048, 256, 2) TPX3_FUSED_ATTR(2048, 256, 3)
   TPX3_FUSED_ATTR(4096, 512, 0) TPX3_FUSED_ATTR(4096, 512, 1) TPX3_FUSED_ATTR(4096, 512, 2) TPX3_FUSED_ATTR(4096, 512, 3)
   TPX3_FUSED_ATTR(8192, 1024, 0) TPX3_FUSED_ATTR(8192, 1024, 1) TPX3_FUSED_ATTR(8192, 1024, 2)
-  TPX3_FUSED_ATTR(8192, 1024, 3) TPX3_FUSED_ATTR(8192, 1024, 5)
+  TPX3_FUSED_ATTR(8192, 1024, 3) TPX3_FUSED_ATTR(8192, 1024, 5) TPX3_FUSED_ATTR(8192, 1024, 6)
   TPX3_FUSED_ATTR(2048, 256, 4) TPX3_FUSED_ATTR(4096, 512, 4) TPX3_FUSED_ATTR(8192, 1024, 4)
 #undef TPX3_FUSED_ATTR
   return TPX3_OK;
@@ -1953,6 +1954,7 @@ __device__ inline void launch_fused_rung_device(FusedArgs a, uint32_t T) {
     else if (a.mode == 1u) TPX3_RUNG(8192, 1024, 1);
     else if (a.mode == 2u) TPX3_RUNG(8192, 1024, 2);
     else if (a.mode == 3u) TPX3_RUNG(8192, 1024, 3);
+    else if (a.mode == 6u) TPX3_RUNG(8192, 1024, 6);
     else TPX3_RUNG(8192, 1024, 5);
   }
 #undef TPX3_RUNG
@@ -1964,7 +1966,7 @@ __device__ inline void launch_fused_rung_device(FusedArgs a, uint32_t T) {
 // (8 bytes) by position with 128-bit loads; modes 3 and 5 read perm (4 bytes) that way and gather the events.
 __host__ __device__ inline int fused_head_of(uint32_t mode, const void* x, const void* y, const void* toa, const void* tot,
                                              const void* perm) {
-  if (mode == 3u || mode == 5u) return ((uintptr_t)perm & 3u) ? -1 : (int)(((uintptr_t)perm >> 2) & 3u);
+  if (mode == 3u || mode == 5u || mode == 6u) return ((uintptr_t)perm & 3u) ? -1 : (int)(((uintptr_t)perm >> 2) & 3u);
   if ((((uintptr_t)x | (uintptr_t)y | (uintptr_t)tot) & 1u) || ((uintptr_t)toa & 7u)) return -1;
   const uint32_t e = (uint32_t)(((uintptr_t)x >> 1) & 7u);
   if ((((uintptr_t)y >> 1) & 7u) != e || (((uintptr_t)tot >> 1) & 7u) != e || (((uintptr_t)toa >> 3) & 1u) != (e & 1u)) return -1;
@@ -1973,7 +1975,7 @@ __host__ __device__ inline int fused_head_of(uint32_t mode, const void* x, const
 
 // Moves the position-indexed arrays down to the boundary and lets the positions start at `e` (head 0 before the call).
 __host__ __device__ inline void fused_apply_head(FusedArgs& a, uint32_t e, uint32_t T) {
-  if (a.mode != 3u && a.mode != 5u) { a.x -= e; a.y -= e; a.toa -= e; a.tot -= e; }
+  if (a.mode != 3u && a.mode != 5u && a.mode != 6u) { a.x -= e; a.y -= e; a.toa -= e; a.tot -= e; }
   a.perm -= e;
   a.label -= e;
   a.head = e;
@@ -1982,14 +1984,14 @@ __host__ __device__ inline void fused_apply_head(FusedArgs& a, uint32_t e, uint3
 
 // The general route's tile kernel (mode 5) from the arguments of a first attempt in mode 0 / 2 on the same call: back
 // to the caller's pointers, then the head that perm's alignment asks for; 8192-event windows.
-__host__ __device__ inline void fused_rebase_mode5(FusedArgs& a, uint32_t labels_only) {
+__host__ __device__ inline void fused_rebase_mode5(FusedArgs& a, uint32_t labels_only, uint32_t new_mode = 5u) {
   const uint32_t e0 = a.head;
-  if (a.mode != 3u && a.mode != 5u) { a.x += e0; a.y += e0; a.toa += e0; a.tot += e0; }
+  if (a.mode != 3u && a.mode != 5u && a.mode != 6u) { a.x += e0; a.y += e0; a.toa += e0; a.tot += e0; }
   a.perm += e0;
   a.label += e0;
   a.n -= e0;
   a.head = 0;
-  a.mode = 5u;
+  a.mode = new_mode;     // 5: connected components, 6: the paper-literal mode
   a.labels_only = labels_only;
   fused_apply_head(a, (uint32_t)(((uintptr_t)a.perm >> 2) & 3u), 8192u);
 }

@@ -266,7 +266,7 @@ __global__ void k_fallback_dispatch(GenArgs a, FusedArgs fa, FusedLadder ladder,
     return;
   }
 #define GP(stage, kernel, grid, block, ...) kernel<<<(grid), (block), 0, cudaStreamTailLaunch>>>(__VA_ARGS__)
-  if (what == 1) {
+  if (what == 1 && !a.sorted_tiles) {
     TPX3_LOCALMAX_SEQUENCE(a);
   } else if (what != 3 && a.sorted_tiles) {
     // general route, first choice: the global sort, then the tile kernel on the sorted stream (read through perm)
@@ -285,8 +285,12 @@ __global__ void k_general_slab(GenArgs a, int what) {
   Ctrl* c = a.w.ctrl;
   if (c->fused_state == 1u) return;
 #define GP(stage, kernel, grid, block, ...) kernel<<<(grid), (block), 0, cudaStreamTailLaunch>>>(__VA_ARGS__)
-  TPX3_GENERAL_CLUSTER_SEQUENCE(a);
-  if (what != 2) TPX3_GENERAL_CENTROID_SEQUENCE(a);
+  if (what == 1) {
+    TPX3_LOCALMAX_SEQUENCE(a);
+  } else {
+    TPX3_GENERAL_CLUSTER_SEQUENCE(a);
+    if (what != 2) TPX3_GENERAL_CENTROID_SEQUENCE(a);
+  }
 #undef GP
 }
 
@@ -296,7 +300,7 @@ __global__ void k_general_slab(GenArgs a, int what) {
 __global__ void k_general_sorted_tiles(GenArgs a, FusedArgs fa, int what) {
   Ctrl* c = a.w.ctrl;
   c->tiles_done = 0; c->fused_fail = 0; c->fused_state = 0; c->tight_tiles = 0; c->tiles_run = 0;
-  fused_rebase_mode5(fa, what == 2 ? 1u : 0u);
+  fused_rebase_mode5(fa, what == 2 ? 1u : 0u, what == 1 ? 6u : 5u);
   launch_fused_rung_device(fa, 8192u);
   k_general_slab<<<1, 1, 0, cudaStreamTailLaunch>>>(a, what);
 }
@@ -633,6 +637,8 @@ int tpx3_localmax_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, ui
   if (n == 0) return cuda_ok(cudaGetLastError());
   GenArgs ga = make_gen_args(p, w, 0, n, x, y, toa, tot, perm, lmax, max_clusters, out, n_hits);
   ga.lm_wx = wx; ga.lm_wy = wy; ga.lm_wt = wt;
+  // the general route runs the tile kernel too, behind its global sort (mode 6), when the plan has one
+  ga.sorted_tiles = p->fused.variant != 0 && wt < (1u << 24) && ((uintptr_t)perm & 3u) == 0;
   // shot-contiguous streams: the fused tile kernel in its paper-literal mode (the time window takes the place
   // of the link window in the tile key); anything else: the general kernels, enqueued from the device
   if (lm_fused) {
@@ -651,6 +657,25 @@ int tpx3_localmax_centroid(tpx3_plan_t p, void* workspace, void* cuda_stream, ui
       ++p->launches;
       return cuda_ok(cudaGetLastError());
     }
+  }
+  if (ga.sorted_tiles) {
+    int rc = enqueue_general_sort(p, ga, st);
+    if (rc != TPX3_OK) return rc;
+    StageTimer timer(p, st, TPX3_STAGE_FUSED);
+    Params prm = p->prm;
+    prm.n = n;
+    prm.W = wt;
+    FusedArgs fa = make_fused_args(8192u, (uint32_t)p->num_sms, w.ctrl, w.tiles, prm, x, y, toa, tot, perm, lmax, max_clusters,
+                                   *out, n_hits, (char*)workspace + p->off_keyA, 6u, wx > 255u ? 255u : wx,
+                                   wy > 255u ? 255u : wy, nullptr);
+    fused_rebase_mode5(fa, 0u, 6u);
+    k_fused_shot_tiles<8192, 1024, 6><<<fa.nseg, 1024, FusedSmem<8192>::kBytes, st>>>(fa);
+    uint32_t ctas, tpc;
+    compact_grid(fa.num_tiles, (uint32_t)p->num_sms, &ctas, &tpc);
+    k_fused_compact<<<ctas, kCompactThreads, 0, st>>>(fa, tpc, 8192u);
+    k_general_slab<<<1, 1, 0, st>>>(ga, 1);     // the window-walk kernels, only if a shot did not fit a window
+    p->launches += 3;
+    return cuda_ok(cudaGetLastError());
   }
   return enqueue_localmax(p, ga, st);
 }
