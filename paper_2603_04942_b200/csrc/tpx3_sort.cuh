@@ -240,7 +240,7 @@ constexpr int kPackItems = 16;
 constexpr int kPackTile = kSortThreads * kPackItems;   // 4096
 static_assert(kPackTile % kSortTile == 0, "a block's key range is a multiple of the histogram's tile");
 
-__global__ void __launch_bounds__(kSortThreads) k_radix_scatter_packed(Ctrl* c, int pass, const uint64_t* __restrict__ toa,
+__global__ void __launch_bounds__(kSortThreads, 4) k_radix_scatter_packed(Ctrl* c, int pass, const uint64_t* __restrict__ toa,
                                                                      SortBufs b, uint32_t* __restrict__ perm, uint64_t n,
                                                                      SortGeom g) {
   if (c->fused_state == 1 || (uint32_t)pass >= c->npass || !c->sort_packed) return;
