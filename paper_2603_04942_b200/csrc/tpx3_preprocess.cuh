@@ -197,7 +197,7 @@ __global__ void __launch_bounds__(1024) k_pre_scan(PreArgs a) {
   if (threadIdx.x == 0) *a.n_out = x;
 }
 
-__global__ void __launch_bounds__(kPreThreads, 2) k_pre_scatter(PreArgs a) {
+__global__ void __launch_bounds__(kPreThreads, 3) k_pre_scatter(PreArgs a) {
   __shared__ __align__(16) uint8_t s_keep[kPreTile];
   __shared__ uint16_t s_rank[kPreTile];
   __shared__ uint32_t sm[33];
